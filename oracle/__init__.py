@@ -1,0 +1,166 @@
+"""fp64 CPU oracle for the SL1M hot path -- TEST INFRASTRUCTURE, not the product.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline / `--impl reference` legs
+may import this package.  It shares nothing with `paper_1310_2078_b200/` (the CUDA path) and
+never imports it.  The arithmetic lives in `sl1m_oracle.c` (plain C, `double complex`, literal
+transcription of PAPER.md eqs (9), (16), (17), (18) and the FISTA listing); this file only
+compiles it with gcc and marshals numpy arrays through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sl1m_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile sl1m_oracle.c -> liboracle.so (gcc -O2 -fopenmp, no fast-math)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-fno-fast-math", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Problem(ctypes.Structure):
+    _fields_ = [
+        ("n_vis", ctypes.c_int64), ("uvw", ctypes.c_void_p),
+        ("ant_p", ctypes.c_void_p), ("ant_q", ctypes.c_void_p),
+        ("n_pix", ctypes.c_int64), ("l", ctypes.c_void_p), ("m", ctypes.c_void_p),
+        ("sigma", ctypes.c_void_p), ("n_ant", ctypes.c_int32), ("gains", ctypes.c_void_p),
+        ("gauss_model", ctypes.c_int32),
+    ]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        P = ctypes.POINTER(_Problem)
+        vp, i64, i32, f64 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_entry.argtypes = [P, i64, i64, vp]
+        lib.oracle_forward.argtypes = [P, vp, i64, vp, vp]
+        lib.oracle_adjoint.argtypes = [P, vp, i64, vp, vp]
+        lib.oracle_max_eig.argtypes = [P, i32]
+        lib.oracle_max_eig.restype = f64
+        lib.oracle_threshold.argtypes = [f64, f64]
+        lib.oracle_threshold.restype = f64
+        lib.oracle_fista.argtypes = [P, vp, f64, f64, i32, vp, vp, vp, vp]
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def threshold(x: float, d: float) -> float:
+    """eq (18)."""
+    return float(_load().oracle_threshold(float(x), float(d)))
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+class Oracle:
+    """One measurement problem (uvw, antenna pairs, pixel list, sigma, gains, Gaussian model)."""
+
+    def __init__(self, uvw, l, m, sigma=None, ant_p=None, ant_q=None, gains=None, gauss_model=1):
+        self.uvw = np.ascontiguousarray(uvw, dtype=np.float64).reshape(-1, 3)
+        self.l = np.ascontiguousarray(l, dtype=np.float64).ravel()
+        self.m = np.ascontiguousarray(m, dtype=np.float64).ravel()
+        self.n_vis, self.n_pix = self.uvw.shape[0], self.l.shape[0]
+        assert self.m.shape[0] == self.n_pix
+        self.sigma = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64).ravel()
+        self.gains = None
+        self.ant_p = self.ant_q = None
+        self.n_ant = 0
+        if gains is not None:
+            g = np.asarray(gains)
+            assert g.ndim == 2 and g.shape[1] == self.n_pix and np.iscomplexobj(g)
+            self.n_ant = g.shape[0]
+            # exact widening of the caller's complex64 table; layout [n_ant][n_pix][2]
+            self.gains = np.ascontiguousarray(g.astype(np.complex128)).view(np.float64)
+            self.ant_p = np.ascontiguousarray(ant_p, dtype=np.int32)
+            self.ant_q = np.ascontiguousarray(ant_q, dtype=np.int32)
+            assert self.ant_p.shape[0] == self.n_vis and self.ant_q.shape[0] == self.n_vis
+        self.gauss_model = int(gauss_model)
+        self._c = _Problem(self.n_vis, _ptr(self.uvw), _ptr(self.ant_p), _ptr(self.ant_q),
+                           self.n_pix, _ptr(self.l), _ptr(self.m), _ptr(self.sigma),
+                           self.n_ant, _ptr(self.gains), self.gauss_model)
+
+    @classmethod
+    def from_workload(cls, wl):
+        return cls(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, wl.gains, wl.gauss_model)
+
+    # O1
+    def entry(self, j: int, k: int) -> complex:
+        out = np.zeros(2)
+        _load().oracle_entry(ctypes.byref(self._c), int(j), int(k), _ptr(out))
+        return complex(out[0], out[1])
+
+    def dense(self) -> np.ndarray:
+        """The full matrix M (tiny problems only)."""
+        M = np.empty((self.n_vis, self.n_pix), dtype=np.complex128)
+        for j in range(self.n_vis):
+            for k in range(self.n_pix):
+                M[j, k] = self.entry(j, k)
+        return M
+
+    # O2
+    def forward(self, x, rows=None) -> np.ndarray:
+        x = np.ascontiguousarray(x, dtype=np.float64).ravel()
+        assert x.shape[0] == self.n_pix
+        if rows is not None:
+            rows = np.ascontiguousarray(rows, dtype=np.int64)
+            n = rows.shape[0]
+        else:
+            n = self.n_vis
+        v = np.zeros((n, 2))
+        _load().oracle_forward(ctypes.byref(self._c), _ptr(x), n, _ptr(rows), _ptr(v))
+        return v[:, 0] + 1j * v[:, 1]
+
+    # O3
+    def adjoint(self, r, cols=None) -> np.ndarray:
+        r = np.ascontiguousarray(np.asarray(r, dtype=np.complex128)).view(np.float64)
+        assert r.shape[0] == 2 * self.n_vis
+        if cols is not None:
+            cols = np.ascontiguousarray(cols, dtype=np.int64)
+            n = cols.shape[0]
+        else:
+            n = self.n_pix
+        g = np.zeros(n)
+        _load().oracle_adjoint(ctypes.byref(self._c), _ptr(r), n, _ptr(cols), _ptr(g))
+        return g
+
+    # O4
+    def max_eig(self, n_pow: int = 30) -> float:
+        return float(_load().oracle_max_eig(ctypes.byref(self._c), int(n_pow)))
+
+    # O5
+    def fista(self, V, lam: float, L: float, n_iter: int, x0=None, want_trace: bool = False):
+        V = np.ascontiguousarray(np.asarray(V, dtype=np.complex128)).view(np.float64)
+        assert V.shape[0] == 2 * self.n_vis
+        x0a = None if x0 is None else np.ascontiguousarray(x0, dtype=np.float64)
+        x = np.zeros(self.n_pix)
+        trace = np.zeros((max(n_iter, 1), 3)) if want_trace else None
+        info = np.zeros(3)
+        _load().oracle_fista(ctypes.byref(self._c), _ptr(V), float(lam), float(L), int(n_iter),
+                             _ptr(x0a), _ptr(x), _ptr(trace), _ptr(info))
+        out = dict(x=x, l2_term=float(info[0]), l1_term=float(info[1]), nnz=int(info[2]))
+        if want_trace:
+            out["trace"] = trace[:n_iter]
+        return out

@@ -1,0 +1,208 @@
+/*
+ * sl1m_oracle.c -- fp64 CPU ORACLE for the SL1M hot path (arXiv:1310.2078, S. J. Hardy 2013).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may call it.  It shares no code, header,
+ * table or pre/post-processing with the CUDA path (paper_1310_2078_b200/csrc); it takes the same
+ * raw inputs (uvw, antenna pairs, l, m, sigma, gains, V, lambda, L, K) and nothing else.
+ *
+ * Everything is a literal transcription of the paper's formulas in `double` /
+ * `double complex` with libm's csqrt-free primitives (sqrt, cexp); the only parallelism is an
+ * OpenMP `parallel for` over independent outputs.  No blocking, fusion, reordering, range
+ * reduction or real-arithmetic rewriting is done here, so it can be checked against the paper
+ * by eye.  Citations are PAPER.md:<line> plus the section / equation.
+ *
+ *   O1 matrix entry      eq (9)  PAPER.md:117-120 (section 2.1)   delta pixels
+ *                        eq (16) PAPER.md:160-163 (section 2.2)   Gaussian pixels, paraxial
+ *                        eq (17) PAPER.md:171-174 (section 2.3)   Gaussian pixels, wide field
+ *                        gains   PAPER.md:111 + abstract PAPER.md:13: A^(j)_k realised as
+ *                                g_p(k) conj(g_q(k)) for baseline j = (p,q)  (reading R4)
+ *   O2 forward  V = M I          eq (8)
+ *   O3 adjoint  Re M^H r         PAPER.md:192, 199 ("back projects the residual")  (reading R3)
+ *   O4 L = lambda_max            PAPER.md:190, 211; power iteration               (reading R10/R11)
+ *   O5 FISTA + T^d               listing PAPER.md:188-192, eq (18) PAPER.md:194-197 (readings R8, R9)
+ *
+ * Readings of garbled / ambiguous passages (full list with pins in DESIGN.md):
+ *   R5  eqs (16),(17) as printed carry a leftover 1/sigma_k^2 from eq (15); carrying out the
+ *       integral cancels it ("normalised so that the integral under the gaussian is one",
+ *       PAPER.md:137).  Prefactor used: G/(n_k D), D = 1 - i w_j sigma_k^2.
+ *   R6  residual phase in eqs (12),(17) is n - 1 + (l^2+m^2)/2 (printed with a minus), the only
+ *       sign consistent with eq (13)'s right-hand side and with the sigma->0 limit = eq (9).
+ *   R7  first exponential of eq (16) is exp(-2 pi i (l u + m v)/D) as printed in eq (17);
+ *       last exponential of eq (17) has u^2 + v^2 as in eq (16).
+ *   R8  FISTA momentum per Beck & Teboulle 2009a (the cited source):
+ *       t_{k+1} = (1 + sqrt(1 + 4 t_k^2))/2,  y_{k+1} = I_k + ((t_k - 1)/t_{k+1})(I_k - I_{k-1}).
+ *   R15 sigma_k == 0 always uses eq (9), whatever the plan's Gaussian model.
+ *
+ * Parity pins: tests/test_oracle_*.py (closed forms, limits, brute-force quadrature of eq (15)
+ * and of eq (4), adjoint identity, T^d hand values, t-sequence, DFT-lattice one-step FISTA, KKT,
+ * sparse recovery, L bounds).  Nothing here is "parity unpinned".
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_PI 3.14159265358979323846264338327950288
+
+typedef struct {
+    int64_t n_vis;
+    const double *uvw;     /* [n_vis][3] wavelengths */
+    const int32_t *ant_p;  /* [n_vis] or NULL iff gains NULL */
+    const int32_t *ant_q;
+    int64_t n_pix;
+    const double *l;       /* [n_pix] */
+    const double *m;       /* [n_pix] */
+    const double *sigma;   /* [n_pix] or NULL (all delta) */
+    int32_t n_ant;
+    const double *gains;   /* [n_ant][n_pix][2] (re,im) or NULL (unit) */
+    int32_t gauss_model;   /* 0 = eq (16) paraxial, 1 = eq (17) wide field */
+} oracle_problem;
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* O1: one matrix entry M_jk. */
+static double complex entry(const oracle_problem *P, int64_t j, int64_t k) {
+    const double u = P->uvw[3 * j + 0], v = P->uvw[3 * j + 1], w = P->uvw[3 * j + 2];
+    const double l = P->l[k], m = P->m[k];
+    const double n = sqrt(1.0 - l * l - m * m);
+    double complex G = 1.0;
+    if (P->gains) {
+        const int64_t p = P->ant_p[j], q = P->ant_q[j];
+        const double *gp = P->gains + 2 * (p * P->n_pix + k);
+        const double *gq = P->gains + 2 * (q * P->n_pix + k);
+        G = (gp[0] + I * gp[1]) * conj(gq[0] + I * gq[1]);
+    }
+    const double s = P->sigma ? P->sigma[k] : 0.0;
+    if (s == 0.0) {
+        /* eq (9) */
+        return G / n * cexp(-2.0 * ORACLE_PI * I * (u * l + v * m + w * (n - 1.0)));
+    }
+    /* eq (16) with readings R5, R7 */
+    const double complex D = 1.0 - I * w * s * s;
+    const double r2 = l * l + m * m;
+    double complex M = G / n * (1.0 / D)
+                       * cexp(-2.0 * ORACLE_PI * I * (l * u + m * v) / D)
+                       * cexp(I * ORACLE_PI * w * r2 / D)
+                       * cexp(-ORACLE_PI * s * s * (u * u + v * v) / D);
+    if (P->gauss_model == 1) {
+        /* eq (17) with reading R6: extra residual (non-paraxial) phase at the pixel centre */
+        M *= cexp(-2.0 * ORACLE_PI * I * w * (n - 1.0 + r2 / 2.0));
+    }
+    return M;
+}
+
+void oracle_entry(const oracle_problem *P, int64_t j, int64_t k, double *out2) {
+    double complex M = entry(P, j, k);
+    out2[0] = creal(M);
+    out2[1] = cimag(M);
+}
+
+/* O2: v_j = sum_k M_jk x_k for the listed rows (rows == NULL: j = 0..n_rows-1). */
+void oracle_forward(const oracle_problem *P, const double *x, int64_t n_rows, const int64_t *rows,
+                    double *v /* [n_rows][2] */) {
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t i = 0; i < n_rows; ++i) {
+        const int64_t j = rows ? rows[i] : i;
+        double complex acc = 0.0;
+        for (int64_t k = 0; k < P->n_pix; ++k) {
+            /* a term with x_k == 0 adds exactly 0; skipping it only saves time on sparse skies */
+            if (x[k] != 0.0) acc += entry(P, j, k) * x[k];
+        }
+        v[2 * i + 0] = creal(acc);
+        v[2 * i + 1] = cimag(acc);
+    }
+}
+
+/* O3: g_k = Re sum_j conj(M_jk) r_j for the listed pixels (cols == NULL: k = 0..n_cols-1). */
+void oracle_adjoint(const oracle_problem *P, const double *r /* [n_vis][2] */, int64_t n_cols,
+                    const int64_t *cols, double *g /* [n_cols] */) {
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t i = 0; i < n_cols; ++i) {
+        const int64_t k = cols ? cols[i] : i;
+        double complex acc = 0.0;
+        for (int64_t j = 0; j < P->n_vis; ++j) {
+            acc += conj(entry(P, j, k)) * (r[2 * j] + I * r[2 * j + 1]);
+        }
+        g[i] = creal(acc);
+    }
+}
+
+/* O4: power iteration on x -> Re A^H A x from the all-ones/sqrt(N) start; returns ||g|| of the
+ * last round (an estimate of lambda_max from below).  No RNG, so oracle and GPU agree. */
+double oracle_max_eig(const oracle_problem *P, int32_t n_pow) {
+    const int64_t np = P->n_pix, nv = P->n_vis;
+    double *x = (double *)malloc(sizeof(double) * np);
+    double *g = (double *)malloc(sizeof(double) * np);
+    double *v = (double *)malloc(sizeof(double) * 2 * nv);
+    for (int64_t k = 0; k < np; ++k) x[k] = 1.0 / sqrt((double)np);
+    double L = 0.0;
+    for (int32_t it = 0; it < n_pow; ++it) {
+        oracle_forward(P, x, nv, NULL, v);
+        oracle_adjoint(P, v, np, NULL, g);
+        double s = 0.0;
+        for (int64_t k = 0; k < np; ++k) s += g[k] * g[k];
+        L = sqrt(s);
+        if (L == 0.0) break;
+        for (int64_t k = 0; k < np; ++k) x[k] = g[k] / L;
+    }
+    free(x); free(g); free(v);
+    return L;
+}
+
+/* eq (18): T^d(x) = x - d if x > d, 0 if x <= d. */
+double oracle_threshold(double x, double d) { return (x > d) ? x - d : 0.0; }
+
+/* O5: FISTA as listed at PAPER.md:188-192 (readings R8, R9: step 1/L, threshold lambda/L).
+ * trace (nullable) gets, per iteration k, {||A y_k - V||^2, sum_i I_k[i], nnz(I_k)}.
+ * info3 gets {||A I_K - V||^2, sum I_K, nnz(I_K)}. */
+void oracle_fista(const oracle_problem *P, const double *V /* [n_vis][2] */, double lambda, double L,
+                  int32_t n_iter, const double *x0 /* nullable */, double *x_out /* [n_pix] */,
+                  double *trace /* [n_iter][3] or NULL */, double *info3 /* nullable */) {
+    const int64_t np = P->n_pix, nv = P->n_vis;
+    double *Ik = (double *)calloc(np, sizeof(double));
+    double *Iprev = (double *)calloc(np, sizeof(double));
+    double *y = (double *)calloc(np, sizeof(double));
+    double *g = (double *)malloc(sizeof(double) * np);
+    double *r = (double *)malloc(sizeof(double) * 2 * nv);
+    if (x0) { memcpy(Ik, x0, sizeof(double) * np); memcpy(y, x0, sizeof(double) * np); }
+    double t = 1.0;
+    const double d = lambda / L;
+    for (int32_t it = 0; it < n_iter; ++it) {
+        oracle_forward(P, y, nv, NULL, r);
+        double l2 = 0.0;
+        for (int64_t i = 0; i < 2 * nv; ++i) { r[i] -= V[i]; l2 += r[i] * r[i]; }
+        oracle_adjoint(P, r, np, NULL, g);
+        memcpy(Iprev, Ik, sizeof(double) * np);
+        double l1 = 0.0, nnz = 0.0;
+        for (int64_t k = 0; k < np; ++k) {
+            Ik[k] = oracle_threshold(y[k] - g[k] / L, d);
+            l1 += Ik[k];
+            nnz += (Ik[k] != 0.0);
+        }
+        const double t_next = (1.0 + sqrt(1.0 + 4.0 * t * t)) / 2.0;
+        const double beta = (t - 1.0) / t_next;
+        for (int64_t k = 0; k < np; ++k) y[k] = Ik[k] + beta * (Ik[k] - Iprev[k]);
+        t = t_next;
+        if (trace) { trace[3 * it] = l2; trace[3 * it + 1] = l1; trace[3 * it + 2] = nnz; }
+    }
+    memcpy(x_out, Ik, sizeof(double) * np);
+    if (info3) {
+        oracle_forward(P, Ik, nv, NULL, r);
+        double l2 = 0.0, l1 = 0.0, nnz = 0.0;
+        for (int64_t i = 0; i < 2 * nv; ++i) { const double e = r[i] - V[i]; l2 += e * e; }
+        for (int64_t k = 0; k < np; ++k) { l1 += Ik[k]; nnz += (Ik[k] != 0.0); }
+        info3[0] = l2; info3[1] = l1; info3[2] = nnz;
+    }
+    free(Ik); free(Iprev); free(y); free(g); free(r);
+}

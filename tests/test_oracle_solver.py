@@ -1,0 +1,184 @@
+"""Pins for the oracle's solver pieces O4 (power iteration) and O5 (FISTA + T^d): hand values,
+the textbook t-sequence, numpy eigenvalues, the DFT-lattice one-step case, KKT conditions, an
+independent NNLS solve, the Beck-Teboulle bound, and sparse recovery.  CPU only."""
+import math
+import os
+
+import numpy as np
+import scipy.optimize
+
+import oracle
+from workloads import make_workload
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rows(name):
+    out = []
+    with open(os.path.join(GOLD, name)) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                out.append([float(t) for t in line.split()])
+    return out
+
+
+def test_threshold_hand_values():
+    """eq (18), incl. the x = d tie and negatives (reading R12)."""
+    for x, d, want in _rows("threshold_hand_values.txt"):
+        assert oracle.threshold(x, d) == want
+
+
+def test_momentum_follows_the_textbook_t_sequence():
+    """Reading R8.  One pixel at the phase centre, N_v visibilities all equal to c: A = ones,
+    Re A^H A = N_v.  With L = 2 N_v and lambda = 0 the gradient step is I_k = (y_k + c)/2, so
+    the iterates follow from the momentum coefficients alone; those come from the golden
+    t-sequence (Beck & Teboulle 2009a), not from the oracle."""
+    gold = _rows("fista_t_sequence.txt")
+    beta = [row[2] for row in gold]
+    nv, c = 7, 3.0
+    uvw = np.random.default_rng(2).uniform(-100, 100, (nv, 3))
+    o = oracle.Oracle(uvw, [0.0], [0.0])
+    V = np.full(nv, c, dtype=complex)
+    I_prev, y = 0.0, 0.0
+    for k in range(1, 5):
+        I = (y + c) / 2
+        got = o.fista(V, lam=0.0, L=2.0 * nv, n_iter=k)["x"][0]
+        assert abs(got - I) < 2e-6 * c, (k, got, I)      # golden betas carry 6 digits
+        y = I + beta[k - 1] * (I - I_prev)
+        I_prev = I
+    # t_2 is the golden ratio: exact check of the "/2" (the listing prints "/t_{k+1}")
+    t2 = (1 + math.sqrt(5)) / 2
+    assert abs(gold[1][1] - t2) < 1e-6
+
+
+def _tiny(rng, n_vis=60, n_pix=40, wmax=50.0):
+    uvw = rng.uniform(-1, 1, (n_vis, 3)) * np.array([400.0, 400.0, wmax])
+    l = rng.uniform(-0.02, 0.02, n_pix)
+    m = rng.uniform(-0.02, 0.02, n_pix)
+    return oracle.Oracle(uvw, l, m)
+
+
+def test_max_eig_against_numpy_eigvalsh_and_bounds():
+    """Readings R10/R11: power iteration on x -> Re A^H A x converges FROM BELOW to
+    lambda_max(Re M^H M) (numpy.linalg.eigvalsh); bounds max_k sum_j|M_jk|^2 <= L <= ||M||_F^2;
+    a single-pixel plan gives L = sum_j |M_j0|^2 = N_v/n^2."""
+    rng = np.random.default_rng(21)
+    o = _tiny(rng)
+    M = o.dense()
+    H = (M.conj().T @ M).real
+    lam_max = np.linalg.eigvalsh(H)[-1]
+    L30 = o.max_eig(30)
+    L400 = o.max_eig(400)
+    assert L30 <= lam_max * (1 + 1e-12) and L400 <= lam_max * (1 + 1e-12)
+    assert abs(L400 - lam_max) < 1e-6 * lam_max
+    assert L30 > 0.9 * lam_max
+    col = (np.abs(M) ** 2).sum(0)
+    assert col.max() <= L400 * (1 + 1e-9) and L400 <= (np.abs(M) ** 2).sum() * (1 + 1e-12)
+    # the complex lambda_max(M^H M) is larger: the distinction in R10 is not cosmetic
+    assert np.linalg.eigvalsh(M.conj().T @ M)[-1] >= lam_max * (1 - 1e-12)
+    l0, m0 = 0.3, -0.2
+    o1 = oracle.Oracle(o.uvw, [l0], [m0])
+    assert abs(o1.max_eig(3) - o.n_vis / (1 - l0 * l0 - m0 * m0)) < 1e-9
+
+
+def test_fista_one_step_on_the_dft_lattice():
+    """Reading R13: N x N grid, w = 0, full DFT lattice, gains g = sqrt(n) on both antennas
+    (cancelling 1/n)  =>  Re A^H A = N^2 Id, L = N^2, and FISTA lands on the exact minimiser
+    T^{lambda/L}(Re A^H V / L) in ONE iteration and stays there.  Expected value via numpy FFT."""
+    N, delta = 8, 2e-3
+    k = np.arange(N * N)
+    l = (k % N - N // 2) * delta
+    m = (k // N - N // 2) * delta
+    a = np.arange(N)
+    uu, vv = np.meshgrid(a, a, indexing="xy")
+    uvw = np.stack([uu.ravel() / (N * delta), vv.ravel() / (N * delta), np.zeros(N * N)], 1)
+    g = np.sqrt(np.sqrt(1 - l * l - m * m))
+    gains = np.stack([g, g]).astype(np.complex64)
+    p = np.zeros(N * N, np.int32)
+    q = np.ones(N * N, np.int32)
+    o = oracle.Oracle(uvw, l, m, ant_p=p, ant_q=q, gains=gains)
+    assert abs(o.max_eig(5) - N * N) < 1e-4            # complex64 gains: n is cancelled to ~1e-7
+    rng = np.random.default_rng(8)
+    V = rng.standard_normal(N * N) + 1j * rng.standard_normal(N * N)
+    lam = 3.0
+    R = np.zeros((N, N), dtype=complex)
+    R[vv.ravel(), uu.ravel()] = V * ((-1.0) ** (uu.ravel() + vv.ravel()))
+    dirty = (np.fft.ifft2(R) * N * N).real.ravel()     # = Re A^H V up to the 1e-7 gain rounding
+    want = np.where(dirty / N**2 > lam / N**2, dirty / N**2 - lam / N**2, 0.0)
+    for K in (1, 2, 5):
+        got = o.fista(V, lam=lam, L=float(N * N), n_iter=K)["x"]
+        assert np.max(np.abs(got - want)) < 5e-6
+    assert np.count_nonzero(want) > 5 and np.count_nonzero(want == 0) > 5
+
+
+def test_fista_converges_to_kkt_point_and_matches_nnls():
+    """Reading R9: the listing (step 1/L, threshold lambda/L) minimises
+    F(I) = 1/2 ||V - A I||^2 + lambda sum I  s.t. I >= 0.
+    (i) KKT with g = Re A^H (A I - V): I_k > 0 => g_k = -lambda; I_k = 0 => g_k >= -lambda.
+    (ii) the same minimiser from scipy.optimize.nnls on the Cholesky-reduced problem
+         (independent library routine).  (iii) Beck-Teboulle bound F(I_k) - F* <= 2 L |I*|^2/(k+1)^2."""
+    rng = np.random.default_rng(31)
+    o = _tiny(rng, n_vis=80, n_pix=30)
+    x_true = np.zeros(o.n_pix)
+    x_true[[3, 11, 17, 25]] = [1.0, 0.4, 2.5, 0.7]
+    V = o.forward(x_true) + 0.01 * (rng.standard_normal(o.n_vis) + 1j * rng.standard_normal(o.n_vis))
+    M = o.dense()
+    H = (M.conj().T @ M).real
+    L = np.linalg.eigvalsh(H)[-1] * 1.0001
+    lam = 0.5
+    res = o.fista(V, lam=lam, L=L, n_iter=4000)
+    I = res["x"]
+    assert np.all(I >= 0)
+    grad = o.adjoint(o.forward(I) - V)
+    on = I > 0
+    assert np.max(np.abs(grad[on] + lam)) < 1e-6 * lam
+    assert np.min(grad[~on] + lam) > -1e-6 * lam
+    # (ii) NNLS: 1/2 x^T H x - b^T x, b = Re A^H V - lambda  ==  1/2 ||R x - R^-T b||^2 + const
+    b = (M.conj().T @ V).real - lam
+    Rch = np.linalg.cholesky(H).T
+    x_nnls, _ = scipy.optimize.nnls(Rch, np.linalg.solve(Rch.T, b), maxiter=2000)
+    assert np.max(np.abs(I - x_nnls)) < 1e-6
+
+    # (iii)
+    def F(x):
+        return 0.5 * np.sum(np.abs(M @ x - V) ** 2) + lam * np.sum(x)
+    Fstar = F(x_nnls)
+    for k in (1, 5, 20, 100):
+        Ik = o.fista(V, lam=lam, L=L, n_iter=k)["x"]
+        assert F(Ik) - Fstar <= 2 * L * np.sum(x_nnls ** 2) / (k + 1) ** 2 + 1e-9
+    # info terms (Table 1's separate L2 and L1 columns)
+    assert abs(res["l2_term"] - np.sum(np.abs(M @ I - V) ** 2)) < 1e-9
+    assert abs(res["l1_term"] - I.sum()) < 1e-12 and res["nnz"] == np.count_nonzero(I)
+
+
+def test_fista_trace_and_warm_start():
+    rng = np.random.default_rng(33)
+    o = _tiny(rng, n_vis=40, n_pix=20)
+    V = o.forward(rng.uniform(0, 1, o.n_pix))
+    L = o.max_eig(100) * 1.05
+    a = o.fista(V, lam=0.1, L=L, n_iter=6, want_trace=True)
+    # trace[0] is ||A y_1 - V||^2 with y_1 = 0
+    assert abs(a["trace"][0, 0] - np.sum(np.abs(V) ** 2)) < 1e-9
+    assert abs(a["trace"][-1, 1] - a["x"].sum()) < 1e-12
+    # warm start from x0 with K = 0 returns x0; from the converged point stays there
+    conv = o.fista(V, lam=0.1, L=L, n_iter=3000)["x"]
+    again = o.fista(V, lam=0.1, L=L, n_iter=3, x0=conv)["x"]
+    assert np.max(np.abs(again - conv)) < 1e-8
+
+
+def test_config1_noiseless_recovers_the_sparse_sky():
+    """north_star: "recovering a known sparse positive sky on a tiny noiseless problem".
+    Config 1 geometry (shrunk to 16x16 pixels so the CPU suite stays fast), noiseless,
+    small lambda: support recovered exactly, fluxes to the O(lambda) shrinkage bias."""
+    wl = make_workload(1, n_side=16, n_src=6)
+    o = oracle.Oracle.from_workload(wl)
+    V = o.forward(wl.x_true)
+    L = o.max_eig(60) * 1.05
+    lam = 1e-3 * np.max(np.abs(o.adjoint(V)))
+    I = o.fista(V, lam=lam, L=L, n_iter=3000)["x"]
+    assert np.all(I >= 0)
+    sup_true = set(np.flatnonzero(wl.x_true))
+    big = set(np.flatnonzero(I > 0.02))
+    assert big == sup_true
+    assert np.max(np.abs(I - wl.x_true)) < 0.02
