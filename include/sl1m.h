@@ -1,0 +1,149 @@
+/*
+ * sl1m.h -- C ABI of the B200-native SL1M hot path (arXiv:1310.2078, S. J. Hardy 2013).
+ *
+ * The library evaluates, on one sm_100a GPU, the direct (ungridded, matrix-free) measurement
+ * operator of the paper and the FISTA solver built on it.  Citations are PAPER.md:<line>.
+ *
+ *   M_jk   eq (9)  PAPER.md:117-120   delta pixels (sigma_k == 0)
+ *          eq (16) PAPER.md:160-163   Gaussian pixels, paraxial   (SL1M_GAUSS_PARAXIAL)
+ *          eq (17) PAPER.md:171-174   Gaussian pixels, wide field (SL1M_GAUSS_WIDEFIELD)
+ *          times G_jk = g_p(k) conj(g_q(k)) for baseline j = (p_j, q_j)
+ *   forward  v = M x          eq (8)  PAPER.md:113-115          sl1m_forward
+ *   adjoint  g = Re M^H r     PAPER.md:192, 199                 sl1m_adjoint
+ *   L = lambda_max(Re M^H M)  PAPER.md:190, 211                 sl1m_max_eig
+ *   FISTA + T^d               PAPER.md:188-197 (eq 18)          sl1m_solve
+ *
+ * Conventions
+ *  - Every call returns an sl1m_status (0 = OK).  Nothing throws or aborts across the ABI.
+ *    Arguments are validated before any device work.  sl1m_last_error() returns a thread-local
+ *    message for the most recent non-OK status.
+ *  - "HOST" pointers are ordinary CPU memory, "DEV" pointers are CUDA device memory of the
+ *    current device (e.g. torch.Tensor.data_ptr()).  `stream` is a cudaStream_t passed as
+ *    void* (NULL = the legacy default stream).
+ *  - The plan COPIES every plan-time input; the caller may free them on return.  Vectors passed
+ *    to forward/adjoint/solve stay caller-owned; outputs are overwritten, never accumulated.
+ *  - forward/adjoint are asynchronous on `stream`.  solve and max_eig enqueue all their work on
+ *    `stream` without any host round-trip per iteration and synchronise once at the end, only
+ *    when a host result (info / L) was asked for.  The *_host variants copy in and out of HOST
+ *    buffers on `stream` and synchronise before returning.
+ *  - A plan owns its workspaces: do not use one plan from two streams at once.
+ *  - Images are real fp32 [n_pix] in the CALLER's pixel order; visibilities are complex fp32,
+ *    interleaved (re, im), [n_vis][2], in the caller's order.
+ *  - There is no CPU fallback: without a usable CUDA device every call fails with SL1M_ERR_CUDA.
+ */
+#ifndef SL1M_H_
+#define SL1M_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sl1m_plan sl1m_plan; /* opaque; owns all device copies and workspaces */
+
+typedef enum {
+    SL1M_OK = 0,
+    SL1M_ERR_NULL = 1,   /* a required pointer is NULL */
+    SL1M_ERR_SIZE = 2,   /* n_vis < 1, n_pix < 1, n_ant < 1 with gains, sizes beyond 2^31-1 tiles */
+    SL1M_ERR_DOMAIN = 3, /* l^2 + m^2 >= 1, sigma < 0, NaN/Inf in uvw, l, m, sigma */
+    SL1M_ERR_INDEX = 4,  /* antenna index outside [0, n_ant) */
+    SL1M_ERR_ALLOC = 5,  /* host or device allocation failed */
+    SL1M_ERR_CUDA = 6,   /* CUDA runtime error (no device, launch failure, ...) */
+    SL1M_ERR_PARAM = 7   /* lambda < 0, L <= 0 with n_pow <= 0, n_iter < 0, unknown model/flag */
+} sl1m_status;
+
+typedef enum {
+    SL1M_GAUSS_PARAXIAL = 0, /* eq (16) */
+    SL1M_GAUSS_WIDEFIELD = 1 /* eq (17) */
+} sl1m_gauss_model;
+
+/* flags for sl1m_plan_create */
+#define SL1M_GAINS_ON_DEVICE 1u /* `gains` is a DEV pointer (default: HOST) */
+
+/*
+ * sl1m_plan_create -- build the operator for one set of visibilities and pixels.
+ *   uvw      HOST [n_vis][3] fp64, baseline coordinates in wavelengths.
+ *   ant_p/q  HOST [n_vis] int32 antenna (gain-row) indices; may be NULL iff gains == NULL.
+ *   l, m     HOST [n_pix] fp64 direction cosines of the pixel centres, any order, need not lie
+ *            on a grid.
+ *   sigma    HOST [n_pix] fp64, the paper's sigma_k of eq (11) (NOT a standard
+ *            deviation: std = sigma/sqrt(2 pi)); NULL or 0 => delta pixel, which always uses
+ *            eq (9).  sigma_k > 0 uses eq (16) or eq (17) according to `gauss_model`.
+ *   gains    [n_ant][n_pix][2] fp32 (re, im), HOST (or DEV with SL1M_GAINS_ON_DEVICE);
+ *            NULL => unit gains.  Time-varying beams: give each (antenna, time) its own row.
+ * Plan-time work (fp64 on the host): n_k, 1/n_k, n_k - 1 in the cancellation-free form
+ * -r^2/(1+n), a Morton sort of the pixels into compact tiles of 256 with fp64 tile centres,
+ * and the fp32 offsets from those centres that the kernels consume.
+ */
+int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uvw, const int32_t *ant_p,
+                     const int32_t *ant_q, int64_t n_pix, const double *l, const double *m,
+                     const double *sigma, int32_t n_ant, const float *gains, int gauss_model,
+                     uint32_t flags);
+
+/* v = M x.  x DEV [n_pix] fp32 (real), vis DEV [n_vis][2] fp32.  Asynchronous on stream. */
+int sl1m_forward(sl1m_plan *plan, const float *x_dev, float *vis_dev, void *stream);
+
+/* g = Re M^H r.  r DEV [n_vis][2] fp32, img DEV [n_pix] fp32.  Asynchronous on stream. */
+int sl1m_adjoint(sl1m_plan *plan, const float *r_dev, float *img_dev, void *stream);
+
+/* Same applies with HOST buffers: H2D copy, apply, D2H copy, stream synchronise. */
+int sl1m_forward_host(sl1m_plan *plan, const float *x_host, float *vis_host, void *stream);
+int sl1m_adjoint_host(sl1m_plan *plan, const float *r_host, float *img_host, void *stream);
+
+/*
+ * sl1m_max_eig -- L = lambda_max(Re M^H M) by n_pow rounds of power iteration from the
+ * deterministic start x = 1/sqrt(n_pix): g = M^H(M x), L = ||g||_2, x = g/L.  Approaches
+ * lambda_max FROM BELOW; callers normally multiply by a safety factor (e.g. 1.05) before
+ * passing it to sl1m_solve.  Writes *L_out_host (HOST) after one stream synchronise.
+ */
+int sl1m_max_eig(sl1m_plan *plan, int n_pow, float *L_out_host, void *stream);
+
+typedef struct {
+    int32_t n_iter_done;
+    float L_used;
+    double l2_term; /* ||M I_K - V||^2        (Table 1's "L2 term") */
+    double l1_term; /* sum_k I_K[k]           (Table 1's "L1 term")                    */
+    int64_t nnz;    /* number of non-zero pixels in I_K                                */
+} sl1m_solve_info;
+
+/*
+ * sl1m_solve -- n_iter FISTA iterations exactly as listed at PAPER.md:188-192:
+ *   y_1 = I_0 = x0 (0 if NULL), t_1 = 1;
+ *   I_k = T^{lambda/L}( y_k - (1/L) Re M^H (M y_k - V) ),          T^d of eq (18);
+ *   t_{k+1} = (1 + sqrt(1 + 4 t_k^2))/2,  y_{k+1} = I_k + ((t_k - 1)/t_{k+1}) (I_k - I_{k-1}).
+ * Its fixed point minimises 1/2 ||V - M I||^2 + lambda sum I, I >= 0 (eq (10) with
+ * lambda_paper = 2 lambda).
+ *   vis_dev   DEV [n_vis][2] measured visibilities V.
+ *   L         step constant; L <= 0 => computed by n_pow rounds of sl1m_max_eig (no safety
+ *             factor applied).
+ *   x0_dev    DEV [n_pix] or NULL.        x_out_dev  DEV [n_pix], receives I_K.
+ *   trace_dev DEV [n_iter][3] fp64 or NULL: per iteration {||M y_k - V||^2, sum I_k, nnz I_k},
+ *             written on the device, never read by the host.
+ *   info_host HOST or NULL; when non-NULL one extra forward evaluates ||M I_K - V||^2 and the
+ *             call synchronises `stream` once before returning.
+ */
+int sl1m_solve(sl1m_plan *plan, const float *vis_dev, float lambda, float L, int n_pow, int n_iter,
+               const float *x0_dev, float *x_out_dev, double *trace_dev,
+               sl1m_solve_info *info_host, void *stream);
+
+/* sl1m_solve with HOST vis / x0 / x_out (trace not available); always synchronises. */
+int sl1m_solve_host(sl1m_plan *plan, const float *vis_host, float lambda, float L, int n_pow,
+                    int n_iter, const float *x0_host, float *x_out_host,
+                    sl1m_solve_info *info_host, void *stream);
+
+/* Number of kernels this plan has launched since creation (for bench.py's gpu_launches). */
+int64_t sl1m_launch_count(const sl1m_plan *plan);
+
+/* Sizes the plan was created with (0 for a NULL plan). */
+int64_t sl1m_plan_n_vis(const sl1m_plan *plan);
+int64_t sl1m_plan_n_pix(const sl1m_plan *plan);
+
+void sl1m_destroy(sl1m_plan *plan);     /* NULL-safe */
+const char *sl1m_status_string(int st); /* static strings */
+const char *sl1m_last_error(void);      /* thread-local detail of the last non-OK status */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SL1M_H_ */

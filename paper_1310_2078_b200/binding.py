@@ -1,0 +1,256 @@
+"""ctypes binding of include/sl1m.h -- same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+import os
+import re
+from typing import Optional
+
+import numpy as np
+
+from .build import LIB, build_library
+
+GAUSS_PARAXIAL = 0   # eq (16)
+GAUSS_WIDEFIELD = 1  # eq (17)
+GAINS_ON_DEVICE = 1
+
+_HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "sl1m.h")
+
+
+class Sl1mError(RuntimeError):
+    def __init__(self, status: int, name: str, detail: str):
+        super().__init__(f"{name} ({status}): {detail}")
+        self.status, self.name, self.detail = status, name, detail
+
+
+class _SolveInfo(ctypes.Structure):
+    _fields_ = [("n_iter_done", ctypes.c_int32), ("L_used", ctypes.c_float),
+                ("l2_term", ctypes.c_double), ("l1_term", ctypes.c_double), ("nnz", ctypes.c_int64)]
+
+
+@dataclasses.dataclass
+class SolveInfo:
+    n_iter_done: int
+    L_used: float
+    l2_term: float
+    l1_term: float
+    nnz: int
+
+
+def library_path() -> str:
+    return LIB
+
+
+def exported_symbols() -> list:
+    """Every function name include/sl1m.h declares."""
+    txt = open(_HEADER).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(sl1m_[a-z0-9_]+)\s*\(", txt)))
+
+
+_lib = None
+
+
+def load_library():
+    """Load libsl1m.so (building it if the sources are newer).  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = build_library() if not os.path.exists(LIB) or os.environ.get("SL1M_REBUILD") else LIB
+    lib = ctypes.CDLL(path)
+    vp, i64, i32, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
+    lib.sl1m_plan_create.argtypes = [ctypes.POINTER(vp), i64, vp, vp, vp, i64, vp, vp, vp, i32, vp,
+                                     ctypes.c_int, ctypes.c_uint32]
+    lib.sl1m_forward.argtypes = [vp, vp, vp, vp]
+    lib.sl1m_adjoint.argtypes = [vp, vp, vp, vp]
+    lib.sl1m_forward_host.argtypes = [vp, vp, vp, vp]
+    lib.sl1m_adjoint_host.argtypes = [vp, vp, vp, vp]
+    lib.sl1m_max_eig.argtypes = [vp, ctypes.c_int, ctypes.POINTER(f32), vp]
+    lib.sl1m_solve.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, vp, vp, vp,
+                               ctypes.POINTER(_SolveInfo), vp]
+    lib.sl1m_solve_host.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, vp, vp,
+                                    ctypes.POINTER(_SolveInfo), vp]
+    lib.sl1m_launch_count.argtypes = [vp]
+    lib.sl1m_launch_count.restype = i64
+    lib.sl1m_plan_n_vis.argtypes = [vp]
+    lib.sl1m_plan_n_vis.restype = i64
+    lib.sl1m_plan_n_pix.argtypes = [vp]
+    lib.sl1m_plan_n_pix.restype = i64
+    lib.sl1m_destroy.argtypes = [vp]
+    lib.sl1m_destroy.restype = None
+    lib.sl1m_status_string.argtypes = [ctypes.c_int]
+    lib.sl1m_status_string.restype = ctypes.c_char_p
+    lib.sl1m_last_error.argtypes = []
+    lib.sl1m_last_error.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(st: int):
+    if st != 0:
+        lib = load_library()
+        raise Sl1mError(st, lib.sl1m_status_string(st).decode(), lib.sl1m_last_error().decode())
+
+
+def _np_ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _dev_ptr(t, dtype, numel: int, name: str):
+    import torch
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()
+            and t.numel() == numel):
+        raise ValueError(f"{name}: need a contiguous CUDA tensor of {dtype} with {numel} elements")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class Plan:
+    """sl1m_plan_create / sl1m_destroy.  Inputs are host arrays (numpy); see include/sl1m.h."""
+
+    def __init__(self, uvw, l, m, sigma=None, ant_p=None, ant_q=None, gains=None,
+                 gauss_model: int = GAUSS_WIDEFIELD):
+        import torch
+        self._h = None
+        lib = load_library()
+        uvw = np.ascontiguousarray(uvw, dtype=np.float64).reshape(-1, 3)
+        l = np.ascontiguousarray(l, dtype=np.float64).ravel()
+        m = np.ascontiguousarray(m, dtype=np.float64).ravel()
+        if m.shape != l.shape:
+            raise ValueError("l and m differ in length")
+        sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64).ravel()
+        if sg is not None and sg.shape != l.shape:
+            raise ValueError("sigma and l differ in length")
+        n_ant, g, flags = 0, None, 0
+        ap = aq = None
+        gptr = None
+        if gains is not None:
+            ap = np.ascontiguousarray(ant_p, dtype=np.int32).ravel()
+            aq = np.ascontiguousarray(ant_q, dtype=np.int32).ravel()
+            if ap.shape[0] != uvw.shape[0] or aq.shape[0] != uvw.shape[0]:
+                raise ValueError("ant_p/ant_q and uvw differ in length")
+            if isinstance(gains, torch.Tensor):
+                if not (gains.is_cuda and gains.dtype == torch.complex64 and gains.is_contiguous()):
+                    raise ValueError("device gains must be a contiguous CUDA complex64 tensor")
+                g = gains
+                n_ant = int(g.shape[0])
+                gptr = ctypes.c_void_p(g.data_ptr())
+                flags |= GAINS_ON_DEVICE
+            else:
+                g = np.ascontiguousarray(gains, dtype=np.complex64)
+                n_ant = int(g.shape[0])
+                gptr = _np_ptr(g)
+            if g.ndim != 2 or g.shape[1] != l.shape[0]:
+                raise ValueError("gains must be [n_ant][n_pix]")
+        h = ctypes.c_void_p()
+        _check(lib.sl1m_plan_create(ctypes.byref(h), uvw.shape[0], _np_ptr(uvw), _np_ptr(ap), _np_ptr(aq),
+                                    l.shape[0], _np_ptr(l), _np_ptr(m), _np_ptr(sg), n_ant, gptr,
+                                    int(gauss_model), flags))
+        self._h = h
+        self.n_vis, self.n_pix = int(uvw.shape[0]), int(l.shape[0])
+
+    @classmethod
+    def from_workload(cls, wl, gains_device=None):
+        g = wl.gains if gains_device is None else gains_device
+        return cls(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model)
+
+    def close(self):
+        if self._h is not None:
+            load_library().sl1m_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- device-pointer calls (torch tensors) ----
+    def forward(self, x, out=None, stream=None):
+        """sl1m_forward: x float32 [n_pix] -> complex64 [n_vis]."""
+        import torch
+        if out is None:
+            out = torch.empty(self.n_vis, dtype=torch.complex64, device=x.device)
+        _check(load_library().sl1m_forward(self._h, _dev_ptr(x, torch.float32, self.n_pix, "x"),
+                                           _dev_ptr(out, torch.complex64, self.n_vis, "out"),
+                                           _stream_ptr(stream)))
+        return out
+
+    def adjoint(self, r, out=None, stream=None):
+        """sl1m_adjoint: r complex64 [n_vis] -> float32 [n_pix]."""
+        import torch
+        if out is None:
+            out = torch.empty(self.n_pix, dtype=torch.float32, device=r.device)
+        _check(load_library().sl1m_adjoint(self._h, _dev_ptr(r, torch.complex64, self.n_vis, "r"),
+                                           _dev_ptr(out, torch.float32, self.n_pix, "out"),
+                                           _stream_ptr(stream)))
+        return out
+
+    def max_eig(self, n_pow: int = 30, stream=None) -> float:
+        L = ctypes.c_float(0.0)
+        _check(load_library().sl1m_max_eig(self._h, int(n_pow), ctypes.byref(L), _stream_ptr(stream)))
+        return float(L.value)
+
+    def solve(self, vis, lam: float, L: float = 0.0, n_pow: int = 30, n_iter: int = 100, x0=None,
+              out=None, trace=None, want_info: bool = True, stream=None):
+        """sl1m_solve.  Returns (x, SolveInfo or None)."""
+        import torch
+        if out is None:
+            out = torch.empty(self.n_pix, dtype=torch.float32, device=vis.device)
+        info = _SolveInfo()
+        _check(load_library().sl1m_solve(
+            self._h, _dev_ptr(vis, torch.complex64, self.n_vis, "vis"), float(lam), float(L), int(n_pow),
+            int(n_iter), _dev_ptr(x0, torch.float32, self.n_pix, "x0"),
+            _dev_ptr(out, torch.float32, self.n_pix, "out"),
+            _dev_ptr(trace, torch.float64, 3 * max(int(n_iter), 0), "trace") if trace is not None else None,
+            ctypes.byref(info) if want_info else None, _stream_ptr(stream)))
+        res = SolveInfo(info.n_iter_done, info.L_used, info.l2_term, info.l1_term, info.nnz) if want_info else None
+        return out, res
+
+    # ---- host-buffer calls (numpy / pinned torch CPU tensors) ----
+    @staticmethod
+    def _host_ptr(a, dtype, numel, name):
+        import torch
+        if a is None:
+            return None
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or not a.is_contiguous() or a.numel() != numel:
+                raise ValueError(f"{name}: need a contiguous CPU tensor with {numel} elements")
+            return ctypes.c_void_p(a.data_ptr())
+        if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous and a.size == numel):
+            raise ValueError(f"{name}: need a contiguous {dtype} array with {numel} elements")
+        return _np_ptr(a)
+
+    def forward_host(self, x_host, out_host, stream=None):
+        _check(load_library().sl1m_forward_host(self._h, self._host_ptr(x_host, np.float32, self.n_pix, "x"),
+                                                self._host_ptr(out_host, np.complex64, self.n_vis, "out"),
+                                                _stream_ptr(stream)))
+        return out_host
+
+    def adjoint_host(self, r_host, out_host, stream=None):
+        _check(load_library().sl1m_adjoint_host(self._h, self._host_ptr(r_host, np.complex64, self.n_vis, "r"),
+                                                self._host_ptr(out_host, np.float32, self.n_pix, "out"),
+                                                _stream_ptr(stream)))
+        return out_host
+
+    def solve_host(self, vis_host, lam, L, n_iter, out_host, n_pow=30, x0_host=None, want_info=True, stream=None):
+        info = _SolveInfo()
+        _check(load_library().sl1m_solve_host(
+            self._h, self._host_ptr(vis_host, np.complex64, self.n_vis, "vis"), float(lam), float(L), int(n_pow),
+            int(n_iter), self._host_ptr(x0_host, np.float32, self.n_pix, "x0"),
+            self._host_ptr(out_host, np.float32, self.n_pix, "out"),
+            ctypes.byref(info) if want_info else None, _stream_ptr(stream)))
+        res = SolveInfo(info.n_iter_done, info.L_used, info.l2_term, info.l1_term, info.nnz) if want_info else None
+        return out_host, res
+
+    @property
+    def launch_count(self) -> int:
+        return int(load_library().sl1m_launch_count(self._h))

@@ -1,0 +1,591 @@
+// sl1m.cu -- host side of the C ABI declared in include/sl1m.h: argument validation, the fp64
+// plan-time precompute (step a0 of SURVEY.md 8(a)), launch configuration and the solver loop.
+// All arithmetic of the method on the hot path runs in the kernels of sl1m_kernels.cuh /
+// sl1m_epilogue.cuh; there is no CPU fallback.
+#include "../../include/sl1m.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "sl1m_epilogue.cuh"
+#include "sl1m_kernels.cuh"
+
+using namespace sl1m;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int fail(int st, const std::string &msg) {
+    g_last_error = msg;
+    return st;
+}
+
+#define CUDA_TRY(expr)                                                                      \
+    do {                                                                                    \
+        cudaError_t e_ = (expr);                                                            \
+        if (e_ != cudaSuccess)                                                              \
+            return fail(e_ == cudaErrorMemoryAllocation ? SL1M_ERR_ALLOC : SL1M_ERR_CUDA,   \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                \
+    } while (0)
+
+constexpr int SM_COUNT_B200 = 148;
+
+}  // namespace
+
+struct sl1m_plan {
+    int64_t n_vis = 0, n_pix = 0;
+    int n_pix_pad = 0, n_tiles = 0, n_ant = 0;
+    bool gauss = false, gains = false;
+    // device arrays
+    double *u64 = nullptr, *v64 = nullptr, *w64 = nullptr;
+    int *ant_p = nullptr, *ant_q = nullptr;
+    float4 *pix4 = nullptr;
+    float2 *pixg = nullptr;
+    double4 *cen = nullptr;
+    float *amp = nullptr;
+    int *perm = nullptr;
+    float2 *gF = nullptr, *gA = nullptr;
+    // launch configuration
+    int fwd_rv = 8, fwd_vtiles = 0, fwd_split = 1, fwd_per_split = 0;
+    int adj_rp = 8, adj_pgroups = 0, adj_split = 1, adj_per_split = 0;
+    // workspaces
+    float2 *ws_v = nullptr;      // [fwd_split][n_vis]
+    float *ws_p = nullptr;       // [adj_split][n_pix_pad]
+    float2 *resid = nullptr;     // [n_vis]   residual / forward result
+    float *I_sorted = nullptr, *y_sorted = nullptr, *g_sorted = nullptr;   // [n_pix_pad]
+    double *part_a = nullptr, *part_b = nullptr, *part_c = nullptr;        // block partials
+    int n_part = 0;
+    double *scalars = nullptr;   // [4] device scalars (norm2, l2, l1, nnz)
+    // host-buffer variants
+    float *h_x = nullptr, *h_vis = nullptr, *h_img = nullptr;   // device staging for *_host calls
+    int64_t launches = 0;
+    int device = 0;
+};
+
+namespace {
+
+void free_plan(sl1m_plan *p) {
+    if (!p) return;
+    void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
+                    p->perm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
+                    p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img};
+    for (void *q : ptrs)
+        if (q) cudaFree(q);
+    delete p;
+}
+
+inline uint32_t spread16(uint32_t x) {  // interleave 16 bits with zeros
+    x &= 0xffffu;
+    x = (x | (x << 8)) & 0x00ff00ffu;
+    x = (x | (x << 4)) & 0x0f0f0f0fu;
+    x = (x | (x << 2)) & 0x33333333u;
+    x = (x | (x << 1)) & 0x55555555u;
+    return x;
+}
+
+template <typename T>
+int upload(T **dst, const T *src, size_t n) {
+    CUDA_TRY(cudaMalloc((void **)dst, std::max<size_t>(n, 1) * sizeof(T)));
+    if (n) CUDA_TRY(cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice));
+    return SL1M_OK;
+}
+
+ApplyParams make_params(const sl1m_plan *p) {
+    ApplyParams P;
+    memset(&P, 0, sizeof(P));
+    P.n_vis = (int)p->n_vis;
+    P.u64 = p->u64;
+    P.v64 = p->v64;
+    P.w64 = p->w64;
+    P.ant_p = p->ant_p;
+    P.ant_q = p->ant_q;
+    P.n_pix_pad = p->n_pix_pad;
+    P.n_tiles = p->n_tiles;
+    P.pix4 = p->pix4;
+    P.pixg = p->pixg;
+    P.cen = p->cen;
+    P.n_ant = p->n_ant;
+    P.gF = p->gF;
+    P.gA = p->gA;
+    P.ws_v = p->ws_v;
+    P.ws_p = p->ws_p;
+    return P;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// plan creation
+// ------------------------------------------------------------------------------------------
+extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uvw, const int32_t *ant_p,
+                                const int32_t *ant_q, int64_t n_pix, const double *l, const double *m,
+                                const double *sigma, int32_t n_ant, const float *gains, int gauss_model,
+                                uint32_t flags) {
+    if (!out) return fail(SL1M_ERR_NULL, "out is NULL");
+    *out = nullptr;
+    if (!uvw || !l || !m) return fail(SL1M_ERR_NULL, "uvw, l or m is NULL");
+    if (gains && (!ant_p || !ant_q)) return fail(SL1M_ERR_NULL, "gains given without ant_p/ant_q");
+    if (n_vis < 1 || n_pix < 1) return fail(SL1M_ERR_SIZE, "n_vis and n_pix must be >= 1");
+    if (n_vis > (int64_t)1 << 30 || n_pix > (int64_t)1 << 30) return fail(SL1M_ERR_SIZE, "size beyond 2^30");
+    if (gains && n_ant < 1) return fail(SL1M_ERR_SIZE, "n_ant must be >= 1 with gains");
+    if (gauss_model != SL1M_GAUSS_PARAXIAL && gauss_model != SL1M_GAUSS_WIDEFIELD)
+        return fail(SL1M_ERR_PARAM, "unknown gauss_model");
+    if (flags & ~SL1M_GAINS_ON_DEVICE) return fail(SL1M_ERR_PARAM, "unknown flag");
+    for (int64_t j = 0; j < 3 * n_vis; ++j)
+        if (!std::isfinite(uvw[j])) return fail(SL1M_ERR_DOMAIN, "non-finite uvw");
+    bool any_gauss = false;
+    for (int64_t k = 0; k < n_pix; ++k) {
+        if (!std::isfinite(l[k]) || !std::isfinite(m[k])) return fail(SL1M_ERR_DOMAIN, "non-finite l/m");
+        if (l[k] * l[k] + m[k] * m[k] >= 1.0) return fail(SL1M_ERR_DOMAIN, "l^2 + m^2 >= 1");
+        if (sigma) {
+            if (!std::isfinite(sigma[k]) || sigma[k] < 0.0) return fail(SL1M_ERR_DOMAIN, "sigma < 0 or non-finite");
+            any_gauss |= sigma[k] > 0.0;
+        }
+    }
+    if (gains)
+        for (int64_t j = 0; j < n_vis; ++j)
+            if (ant_p[j] < 0 || ant_p[j] >= n_ant || ant_q[j] < 0 || ant_q[j] >= n_ant)
+                return fail(SL1M_ERR_INDEX, "antenna index outside [0, n_ant)");
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(SL1M_ERR_CUDA, "no CUDA device: the SL1M library has no CPU fallback");
+    }
+
+    sl1m_plan *p = new (std::nothrow) sl1m_plan();
+    if (!p) return fail(SL1M_ERR_ALLOC, "host allocation failed");
+    struct Guard {
+        sl1m_plan *p;
+        ~Guard() { if (p) free_plan(p); }
+    } guard{p};
+    CUDA_TRY(cudaGetDevice(&p->device));
+    p->n_vis = n_vis;
+    p->n_pix = n_pix;
+    p->n_ant = gains ? n_ant : 0;
+    p->gauss = any_gauss;
+    p->gains = gains != nullptr;
+    p->n_pix_pad = (int)(((n_pix + PIX_PAD - 1) / PIX_PAD) * PIX_PAD);
+    p->n_tiles = p->n_pix_pad / TP;
+
+    try {
+        // ---- Morton sort of the pixel list: consecutive runs are spatially compact ----
+        double lmin = l[0], lmax = l[0], mmin = m[0], mmax = m[0];
+        for (int64_t k = 1; k < n_pix; ++k) {
+            lmin = std::min(lmin, l[k]); lmax = std::max(lmax, l[k]);
+            mmin = std::min(mmin, m[k]); mmax = std::max(mmax, m[k]);
+        }
+        const double ext = std::max(std::max(lmax - lmin, mmax - mmin), 1e-300);
+        std::vector<std::pair<uint32_t, int>> keys((size_t)n_pix);
+        for (int64_t k = 0; k < n_pix; ++k) {
+            const uint32_t ix = (uint32_t)std::min(65535.0, (l[k] - lmin) / ext * 65535.0);
+            const uint32_t iy = (uint32_t)std::min(65535.0, (m[k] - mmin) / ext * 65535.0);
+            keys[(size_t)k] = {spread16(ix) | (spread16(iy) << 1), (int)k};
+        }
+        std::stable_sort(keys.begin(), keys.end(),
+                         [](const std::pair<uint32_t, int> &a, const std::pair<uint32_t, int> &b) {
+                             return a.first < b.first;
+                         });
+
+        // ---- per-tile fp64 centres, per-pixel fp32 offsets (step a0) ----
+        const size_t npad = (size_t)p->n_pix_pad;
+        std::vector<float4> pix4(npad, make_float4(0.f, 0.f, 0.f, 0.f));
+        std::vector<float2> pixg(any_gauss ? npad : 0, make_float2(0.f, 0.f));
+        std::vector<double4> cen((size_t)p->n_tiles, make_double4(0.0, 0.0, 0.0, 0.0));
+        std::vector<float> amp(npad, 0.f);
+        std::vector<int> perm(npad, -1);
+        const double PI = 3.14159265358979323846, LOG2E = 1.4426950408889634074;
+        for (int t = 0; t < p->n_tiles; ++t) {
+            const int64_t k0 = (int64_t)t * TP, k1 = std::min<int64_t>(k0 + TP, n_pix);
+            if (k0 >= n_pix) break;
+            double a0 = 1e300, a1 = -1e300, b0 = 1e300, b1 = -1e300;
+            for (int64_t s = k0; s < k1; ++s) {
+                const int k = keys[(size_t)s].second;
+                a0 = std::min(a0, l[k]); a1 = std::max(a1, l[k]);
+                b0 = std::min(b0, m[k]); b1 = std::max(b1, m[k]);
+            }
+            const double lc = 0.5 * (a0 + a1), mc = 0.5 * (b0 + b1);
+            const double rc2 = lc * lc + mc * mc;
+            const double nc = -rc2 / (1.0 + std::sqrt(1.0 - rc2));   // n - 1 at the centre
+            cen[(size_t)t] = make_double4(lc, mc, nc, 0.0);
+            for (int64_t s = k0; s < k1; ++s) {
+                const int k = keys[(size_t)s].second;
+                const double r2 = l[k] * l[k] + m[k] * m[k];
+                const double n = std::sqrt(1.0 - r2);
+                const double sg = sigma ? sigma[k] : 0.0;
+                // eq (9)/(17): n' = n - 1 (cancellation-free); eq (16): n' = -r^2/2; sigma == 0 => eq (9)
+                const double npr = (sg > 0.0 && gauss_model == SL1M_GAUSS_PARAXIAL) ? -0.5 * r2
+                                                                                     : -r2 / (1.0 + n);
+                pix4[(size_t)s] = make_float4((float)(l[k] - lc), (float)(m[k] - mc), (float)(npr - nc), 0.f);
+                amp[(size_t)s] = (float)(1.0 / n);
+                perm[(size_t)s] = k;
+                if (any_gauss) pixg[(size_t)s] = make_float2((float)(sg * sg), (float)(-PI * LOG2E * sg * sg));
+            }
+        }
+
+        // ---- visibilities: SoA fp64 ----
+        std::vector<double> su((size_t)n_vis), sv((size_t)n_vis), sw((size_t)n_vis);
+        for (int64_t j = 0; j < n_vis; ++j) {
+            su[(size_t)j] = uvw[3 * j];
+            sv[(size_t)j] = uvw[3 * j + 1];
+            sw[(size_t)j] = uvw[3 * j + 2];
+        }
+
+        int st;
+        if ((st = upload(&p->u64, su.data(), su.size()))) return st;
+        if ((st = upload(&p->v64, sv.data(), sv.size()))) return st;
+        if ((st = upload(&p->w64, sw.data(), sw.size()))) return st;
+        if ((st = upload(&p->pix4, pix4.data(), npad))) return st;
+        if (any_gauss && (st = upload(&p->pixg, pixg.data(), npad))) return st;
+        if ((st = upload(&p->cen, cen.data(), cen.size()))) return st;
+        if ((st = upload(&p->amp, amp.data(), npad))) return st;
+        if ((st = upload(&p->perm, perm.data(), npad))) return st;
+        if (gains) {
+            if ((st = upload(&p->ant_p, ant_p, (size_t)n_vis))) return st;
+            if ((st = upload(&p->ant_q, ant_q, (size_t)n_vis))) return st;
+        }
+    } catch (const std::bad_alloc &) {
+        return fail(SL1M_ERR_ALLOC, "host allocation failed");
+    }
+
+    // ---- gains: re-layout on the device ----
+    if (gains) {
+        const size_t raw_n = (size_t)n_ant * (size_t)n_pix;
+        float2 *raw = nullptr;
+        if (flags & SL1M_GAINS_ON_DEVICE) {
+            raw = (float2 *)gains;
+        } else {
+            CUDA_TRY(cudaMalloc((void **)&raw, raw_n * sizeof(float2)));
+            cudaError_t e = cudaMemcpy(raw, gains, raw_n * sizeof(float2), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { cudaFree(raw); return fail(SL1M_ERR_CUDA, cudaGetErrorString(e)); }
+        }
+        const size_t lay_n = (size_t)p->n_pix_pad * (size_t)n_ant;
+        cudaError_t e1 = cudaMalloc((void **)&p->gF, lay_n * sizeof(float2));
+        cudaError_t e2 = (e1 == cudaSuccess) ? cudaMalloc((void **)&p->gA, lay_n * sizeof(float2)) : e1;
+        if (e2 == cudaSuccess) {
+            dim3 grid((p->n_pix_pad + ET - 1) / ET, n_ant);
+            gains_layout_kernel<<<grid, ET>>>(raw, n_ant, (int)n_pix, p->n_pix_pad, p->perm, p->gF, p->gA);
+            e2 = cudaDeviceSynchronize();
+            p->launches++;
+        }
+        if (!(flags & SL1M_GAINS_ON_DEVICE)) cudaFree(raw);
+        if (e2 != cudaSuccess)
+            return fail(e2 == cudaErrorMemoryAllocation ? SL1M_ERR_ALLOC : SL1M_ERR_CUDA, cudaGetErrorString(e2));
+    }
+
+    // ---- launch configuration: enough CTAs for 148 SMs x 4 resident CTAs x several waves ----
+    const int target = SM_COUNT_B200 * 4 * 8;
+    {
+        int rv = 8;
+        while (rv > 1 && (int64_t)((n_vis + NT * rv - 1) / (NT * rv)) * p->n_tiles < 2 * SM_COUNT_B200) rv >>= 1;
+        p->fwd_rv = rv;
+        p->fwd_vtiles = (int)((n_vis + NT * rv - 1) / (NT * rv));
+        int split = std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
+        p->fwd_per_split = (p->n_tiles + split - 1) / split;
+        p->fwd_split = (p->n_tiles + p->fwd_per_split - 1) / p->fwd_per_split;
+    }
+    {
+        const int n_chunks = (int)((n_vis + VC - 1) / VC);
+        int rp = 8;
+        while (rp > 1 && (int64_t)(p->n_pix_pad / (NT * rp)) * n_chunks < 2 * SM_COUNT_B200) rp >>= 1;
+        if (rp == 4) rp = 2;   // instantiated: 8, 2, 1
+        p->adj_rp = rp;
+        p->adj_pgroups = p->n_pix_pad / (NT * rp);
+        int split = std::min(n_chunks, std::max(1, (target + p->adj_pgroups - 1) / p->adj_pgroups));
+        p->adj_per_split = (n_chunks + split - 1) / split;
+        p->adj_split = (n_chunks + p->adj_per_split - 1) / p->adj_per_split;
+    }
+
+    // ---- workspaces ----
+    const size_t npad = (size_t)p->n_pix_pad;
+    CUDA_TRY(cudaMalloc((void **)&p->ws_v, (size_t)p->fwd_split * (size_t)n_vis * sizeof(float2)));
+    CUDA_TRY(cudaMalloc((void **)&p->ws_p, (size_t)p->adj_split * npad * sizeof(float)));
+    CUDA_TRY(cudaMalloc((void **)&p->resid, (size_t)n_vis * sizeof(float2)));
+    CUDA_TRY(cudaMalloc((void **)&p->I_sorted, npad * sizeof(float)));
+    CUDA_TRY(cudaMalloc((void **)&p->y_sorted, npad * sizeof(float)));
+    CUDA_TRY(cudaMalloc((void **)&p->g_sorted, npad * sizeof(float)));
+    p->n_part = (int)std::max<size_t>((npad + ET - 1) / ET, ((size_t)n_vis + ET - 1) / ET);
+    CUDA_TRY(cudaMalloc((void **)&p->part_a, (size_t)p->n_part * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&p->part_b, (size_t)p->n_part * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&p->part_c, (size_t)p->n_part * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&p->scalars, 4 * sizeof(double)));
+    CUDA_TRY(cudaMemset(p->scalars, 0, 4 * sizeof(double)));
+    CUDA_TRY(cudaDeviceSynchronize());
+
+    guard.p = nullptr;
+    *out = p;
+    return SL1M_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// launches
+// ------------------------------------------------------------------------------------------
+namespace {
+
+inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
+
+template <int PK, int GK>
+void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
+    switch (p->fwd_rv) {
+        case 8: fwd_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        case 4: fwd_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        case 2: fwd_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        default: fwd_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
+    }
+}
+
+template <int PK, int GK>
+void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
+    switch (p->adj_rp) {
+        case 8: adj_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        case 2: adj_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        default: adj_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
+    }
+}
+
+// forward main kernel: pix4.w must already hold a*x in sorted order; fills ws_v.
+void launch_fwd(sl1m_plan *p, cudaStream_t s) {
+    ApplyParams P = make_params(p);
+    P.per_split = p->fwd_per_split;
+    dim3 grid(p->fwd_vtiles, p->fwd_split);
+    if (p->gauss) {
+        if (p->gains) launch_fwd_rv<1, 1>(p, P, grid, s); else launch_fwd_rv<1, 0>(p, P, grid, s);
+    } else {
+        if (p->gains) launch_fwd_rv<0, 1>(p, P, grid, s); else launch_fwd_rv<0, 0>(p, P, grid, s);
+    }
+    p->launches++;
+}
+
+// adjoint main kernel on residual r (device, [n_vis]); fills ws_p.
+void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
+    ApplyParams P = make_params(p);
+    P.per_split = p->adj_per_split;
+    P.r = r;
+    dim3 grid(p->adj_pgroups, p->adj_split);
+    if (p->gauss) {
+        if (p->gains) launch_adj_rp<1, 1>(p, P, grid, s); else launch_adj_rp<1, 0>(p, P, grid, s);
+    } else {
+        if (p->gains) launch_adj_rp<0, 1>(p, P, grid, s); else launch_adj_rp<0, 0>(p, P, grid, s);
+    }
+    p->launches++;
+}
+
+int check_launch(const char *what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(SL1M_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    return SL1M_OK;
+}
+
+}  // namespace
+
+extern "C" int sl1m_forward(sl1m_plan *p, const float *x_dev, float *vis_dev, void *stream) {
+    if (!p || !x_dev || !vis_dev) return fail(SL1M_ERR_NULL, "sl1m_forward: NULL argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    pack_caller_kernel<<<egrid(p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->perm, x_dev, p->n_pix_pad);
+    launch_fwd(p, s);
+    fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis, nullptr,
+                                                     (float2 *)vis_dev, nullptr);
+    p->launches += 2;
+    return check_launch("sl1m_forward");
+}
+
+extern "C" int sl1m_adjoint(sl1m_plan *p, const float *r_dev, float *img_dev, void *stream) {
+    if (!p || !r_dev || !img_dev) return fail(SL1M_ERR_NULL, "sl1m_adjoint: NULL argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    launch_adj(p, (const float2 *)r_dev, s);
+    adj_reduce_kernel<<<egrid(p->n_pix_pad), ET, 0, s>>>(p->ws_p, p->adj_split, p->n_pix_pad, p->amp, p->perm,
+                                                         img_dev, nullptr, nullptr);
+    p->launches += 1;
+    return check_launch("sl1m_adjoint");
+}
+
+namespace {
+int ensure_host_staging(sl1m_plan *p) {
+    if (!p->h_x) CUDA_TRY(cudaMalloc((void **)&p->h_x, (size_t)p->n_pix * sizeof(float)));
+    if (!p->h_img) CUDA_TRY(cudaMalloc((void **)&p->h_img, (size_t)p->n_pix * sizeof(float)));
+    if (!p->h_vis) CUDA_TRY(cudaMalloc((void **)&p->h_vis, (size_t)p->n_vis * sizeof(float2)));
+    return SL1M_OK;
+}
+}  // namespace
+
+extern "C" int sl1m_forward_host(sl1m_plan *p, const float *x_host, float *vis_host, void *stream) {
+    if (!p || !x_host || !vis_host) return fail(SL1M_ERR_NULL, "sl1m_forward_host: NULL argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    int st = ensure_host_staging(p);
+    if (st) return st;
+    CUDA_TRY(cudaMemcpyAsync(p->h_x, x_host, (size_t)p->n_pix * sizeof(float), cudaMemcpyHostToDevice, s));
+    if ((st = sl1m_forward(p, p->h_x, p->h_vis, stream))) return st;
+    CUDA_TRY(cudaMemcpyAsync(vis_host, p->h_vis, (size_t)p->n_vis * sizeof(float2), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    return SL1M_OK;
+}
+
+extern "C" int sl1m_adjoint_host(sl1m_plan *p, const float *r_host, float *img_host, void *stream) {
+    if (!p || !r_host || !img_host) return fail(SL1M_ERR_NULL, "sl1m_adjoint_host: NULL argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    int st = ensure_host_staging(p);
+    if (st) return st;
+    CUDA_TRY(cudaMemcpyAsync(p->h_vis, r_host, (size_t)p->n_vis * sizeof(float2), cudaMemcpyHostToDevice, s));
+    if ((st = sl1m_adjoint(p, p->h_vis, p->h_img, stream))) return st;
+    CUDA_TRY(cudaMemcpyAsync(img_host, p->h_img, (size_t)p->n_pix * sizeof(float), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    return SL1M_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// a7: power iteration, entirely on the device; one synchronise at the end
+// ------------------------------------------------------------------------------------------
+extern "C" int sl1m_max_eig(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
+    if (!p || !L_out_host) return fail(SL1M_ERR_NULL, "sl1m_max_eig: NULL argument");
+    if (n_pow < 1) return fail(SL1M_ERR_PARAM, "n_pow must be >= 1");
+    cudaStream_t s = (cudaStream_t)stream;
+    const int npad = p->n_pix_pad;
+    // x0 = 1/sqrt(n_pix) on real pixels
+    fill_kernel<<<egrid(npad), ET, 0, s>>>(p->g_sorted, (float)(1.0 / std::sqrt((double)p->n_pix)), p->perm, npad);
+    pack_sorted_kernel<<<egrid(npad), ET, 0, s>>>(p->pix4, p->amp, p->g_sorted, npad);
+    p->launches += 2;
+    for (int it = 0; it < n_pow; ++it) {
+        launch_fwd(p, s);
+        fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis, nullptr, p->resid,
+                                                         nullptr);
+        launch_adj(p, p->resid, s);
+        adj_reduce_kernel<<<egrid(npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->perm, nullptr,
+                                                     p->g_sorted, p->part_a);
+        sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, nullptr, nullptr, egrid(npad), 0, 0, p->scalars, nullptr,
+                                             nullptr);
+        normalize_pack_kernel<<<egrid(npad), ET, 0, s>>>(p->g_sorted, p->scalars, p->amp, p->pix4, npad);
+        p->launches += 4;
+    }
+    int st = check_launch("sl1m_max_eig");
+    if (st) return st;
+    double norm2 = 0.0;
+    CUDA_TRY(cudaMemcpyAsync(&norm2, p->scalars, sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    *L_out_host = (float)std::sqrt(norm2);
+    return SL1M_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// a3-a6: FISTA, listing PAPER.md:188-192; no host round-trip per iteration
+// ------------------------------------------------------------------------------------------
+extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int n_iter,
+                          const float *x0_dev, float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host,
+                          void *stream) {
+    if (!p || !vis_dev || !x_out_dev) return fail(SL1M_ERR_NULL, "sl1m_solve: NULL argument");
+    if (!(lambda >= 0.f) || n_iter < 0) return fail(SL1M_ERR_PARAM, "lambda < 0 or n_iter < 0");
+    if (!(L > 0.f) && n_pow < 1) return fail(SL1M_ERR_PARAM, "L <= 0 needs n_pow >= 1");
+    cudaStream_t s = (cudaStream_t)stream;
+    const int npad = p->n_pix_pad;
+    int st;
+    if (!(L > 0.f)) {
+        if ((st = sl1m_max_eig(p, n_pow, &L, stream))) return st;
+        if (!(L > 0.f)) return fail(SL1M_ERR_PARAM, "power iteration returned L <= 0 (zero operator)");
+    }
+    const float inv_L = (float)(1.0 / (double)L);
+    const float thr = (float)((double)lambda / (double)L);
+
+    // y_1 = I_0 = x0 (or 0), in sorted order; a*y_1 packed into the pixel tiles
+    if (x0_dev) {
+        gather_kernel<<<egrid(npad), ET, 0, s>>>(x0_dev, p->perm, p->I_sorted, npad);
+        p->launches++;
+    } else {
+        CUDA_TRY(cudaMemsetAsync(p->I_sorted, 0, (size_t)npad * sizeof(float), s));
+    }
+    CUDA_TRY(cudaMemcpyAsync(p->y_sorted, p->I_sorted, (size_t)npad * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    pack_sorted_kernel<<<egrid(npad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, npad);
+    p->launches++;
+
+    double t = 1.0;
+    for (int k = 0; k < n_iter; ++k) {
+        const double t_next = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
+        const float beta = (float)((t - 1.0) / t_next);
+        t = t_next;
+        launch_fwd(p, s);
+        fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis,
+                                                         (const float2 *)vis_dev, p->resid,
+                                                         trace_dev ? p->part_a : nullptr);
+        launch_adj(p, p->resid, s);
+        fista_update_kernel<<<egrid(npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->pix4, p->I_sorted,
+                                                       p->y_sorted, inv_L, thr, beta,
+                                                       trace_dev ? p->part_b : nullptr,
+                                                       trace_dev ? p->part_c : nullptr);
+        p->launches += 2;
+        if (trace_dev) {
+            sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis), egrid(npad),
+                                                 egrid(npad), trace_dev + 3 * (size_t)k, trace_dev + 3 * (size_t)k + 1,
+                                                 trace_dev + 3 * (size_t)k + 2);
+            p->launches++;
+        }
+    }
+    scatter_kernel<<<egrid(npad), ET, 0, s>>>(p->I_sorted, p->perm, x_out_dev, npad);
+    p->launches++;
+    if ((st = check_launch("sl1m_solve"))) return st;
+
+    if (info_host) {
+        // one extra forward for ||M I_K - V||^2 (Table 1's L2 term)
+        pack_sorted_kernel<<<egrid(npad), ET, 0, s>>>(p->pix4, p->amp, p->I_sorted, npad);
+        launch_fwd(p, s);
+        fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis,
+                                                         (const float2 *)vis_dev, p->resid, p->part_a);
+        l1_nnz_kernel<<<egrid(npad), ET, 0, s>>>(p->I_sorted, npad, p->part_b, p->part_c);
+        sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis), egrid(npad),
+                                             egrid(npad), p->scalars + 1, p->scalars + 2, p->scalars + 3);
+        p->launches += 4;
+        if ((st = check_launch("sl1m_solve(info)"))) return st;
+        double h[4];
+        CUDA_TRY(cudaMemcpyAsync(h, p->scalars, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(cudaStreamSynchronize(s));
+        info_host->n_iter_done = n_iter;
+        info_host->L_used = L;
+        info_host->l2_term = h[1];
+        info_host->l1_term = h[2];
+        info_host->nnz = (int64_t)(h[3] + 0.5);
+    }
+    return SL1M_OK;
+}
+
+extern "C" int sl1m_solve_host(sl1m_plan *p, const float *vis_host, float lambda, float L, int n_pow, int n_iter,
+                               const float *x0_host, float *x_out_host, sl1m_solve_info *info_host,
+                               void *stream) {
+    if (!p || !vis_host || !x_out_host) return fail(SL1M_ERR_NULL, "sl1m_solve_host: NULL argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    int st = ensure_host_staging(p);
+    if (st) return st;
+    CUDA_TRY(cudaMemcpyAsync(p->h_vis, vis_host, (size_t)p->n_vis * sizeof(float2), cudaMemcpyHostToDevice, s));
+    if (x0_host)
+        CUDA_TRY(cudaMemcpyAsync(p->h_x, x0_host, (size_t)p->n_pix * sizeof(float), cudaMemcpyHostToDevice, s));
+    if ((st = sl1m_solve(p, p->h_vis, lambda, L, n_pow, n_iter, x0_host ? p->h_x : nullptr, p->h_img, nullptr,
+                         info_host, stream)))
+        return st;
+    CUDA_TRY(cudaMemcpyAsync(x_out_host, p->h_img, (size_t)p->n_pix * sizeof(float), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    return SL1M_OK;
+}
+
+extern "C" int64_t sl1m_launch_count(const sl1m_plan *p) { return p ? p->launches : 0; }
+extern "C" int64_t sl1m_plan_n_vis(const sl1m_plan *p) { return p ? p->n_vis : 0; }
+extern "C" int64_t sl1m_plan_n_pix(const sl1m_plan *p) { return p ? p->n_pix : 0; }
+
+extern "C" void sl1m_destroy(sl1m_plan *p) { free_plan(p); }
+
+extern "C" const char *sl1m_status_string(int st) {
+    switch (st) {
+        case SL1M_OK: return "SL1M_OK";
+        case SL1M_ERR_NULL: return "SL1M_ERR_NULL";
+        case SL1M_ERR_SIZE: return "SL1M_ERR_SIZE";
+        case SL1M_ERR_DOMAIN: return "SL1M_ERR_DOMAIN";
+        case SL1M_ERR_INDEX: return "SL1M_ERR_INDEX";
+        case SL1M_ERR_ALLOC: return "SL1M_ERR_ALLOC";
+        case SL1M_ERR_CUDA: return "SL1M_ERR_CUDA";
+        case SL1M_ERR_PARAM: return "SL1M_ERR_PARAM";
+        default: return "SL1M_ERR_UNKNOWN";
+    }
+}
+
+extern "C" const char *sl1m_last_error(void) { return g_last_error.c_str(); }

@@ -1,0 +1,202 @@
+// sl1m_epilogue.cuh -- the O(N) kernels around the two applies: packing a*x into the pixel tiles,
+// fixed-order reduction of the split partials, the fused FISTA update (steps a3-a6 of
+// SURVEY.md 8(a); listing PAPER.md:188-192, eq (18)) and power-iteration helpers.
+// Every reduction runs in a fixed order (no float atomics), so results are bit-stable run to run.
+#pragma once
+#include "sl1m_kernels.cuh"
+
+namespace sl1m {
+
+constexpr int ET = 256;  // threads per CTA in the epilogue kernels
+
+// Block-wide sum in fp64 (warp shuffles, then one warp over the per-warp partials).
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double s_part[ET / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();  // protect s_part across successive calls
+    if (lane == 0) s_part[warp] = v;
+    __syncthreads();
+    double t = (threadIdx.x < ET / 32) ? s_part[threadIdx.x] : 0.0;
+    if (warp == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    }
+    return t;  // valid in thread 0
+}
+
+// pix4[k].w = a_k * x[perm[k]]   (caller order -> sorted, padded pixels get 0)
+__global__ void __launch_bounds__(ET) pack_caller_kernel(float4 *pix4, const float *amp, const int *perm,
+                                                         const float *x, int n_pix_pad) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    if (k >= n_pix_pad) return;
+    const int src = perm[k];
+    pix4[k].w = (src >= 0) ? amp[k] * x[src] : 0.f;
+}
+
+// sorted[k] = caller[perm[k]] (0 on padding)
+__global__ void __launch_bounds__(ET) gather_kernel(const float *caller, const int *perm, float *sorted,
+                                                    int n_pix_pad) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    if (k >= n_pix_pad) return;
+    const int src = perm[k];
+    sorted[k] = (src >= 0) ? caller[src] : 0.f;
+}
+
+// caller[perm[k]] = sorted[k]
+__global__ void __launch_bounds__(ET) scatter_kernel(const float *sorted, const int *perm, float *caller,
+                                                     int n_pix_pad) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    if (k >= n_pix_pad) return;
+    const int dst = perm[k];
+    if (dst >= 0) caller[dst] = sorted[k];
+}
+
+// pix4[k].w = a_k * xs[k]  (sorted order in)
+__global__ void __launch_bounds__(ET) pack_sorted_kernel(float4 *pix4, const float *amp, const float *xs,
+                                                         int n_pix_pad) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    if (k < n_pix_pad) pix4[k].w = amp[k] * xs[k];
+}
+
+__global__ void __launch_bounds__(ET) fill_kernel(float *p, float v, const int *perm, int n_pix_pad) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    if (k < n_pix_pad) p[k] = (perm[k] >= 0) ? v : 0.f;
+}
+
+// Forward epilogue (a3): out[j] = sum_s ws[s][j] - V[j]; part[block] = sum |out|^2 (fp64).
+__global__ void __launch_bounds__(ET) fwd_reduce_kernel(const float2 *ws, int n_split, int n_vis,
+                                                        const float2 *V, float2 *out, double *part) {
+    const int j = blockIdx.x * ET + threadIdx.x;
+    double sq = 0.0;
+    if (j < n_vis) {
+        float re = 0.f, im = 0.f;
+        for (int s = 0; s < n_split; ++s) {
+            const float2 a = ws[(size_t)s * n_vis + j];
+            re += a.x;
+            im += a.y;
+        }
+        if (V) {
+            const float2 v = V[j];
+            re -= v.x;
+            im -= v.y;
+        }
+        out[j] = make_float2(re, im);
+        sq = (double)re * re + (double)im * im;
+    }
+    if (part) {
+        const double t = block_sum(sq);
+        if (threadIdx.x == 0) part[blockIdx.x] = t;
+    }
+}
+
+// Adjoint epilogue: g_k = a_k sum_s ws[s][k]; scattered to the caller's order and/or kept sorted.
+__global__ void __launch_bounds__(ET) adj_reduce_kernel(const float *ws, int n_split, int n_pix_pad,
+                                                        const float *amp, const int *perm, float *img_caller,
+                                                        float *g_sorted, double *part) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    double sq = 0.0;
+    if (k < n_pix_pad) {
+        float g = 0.f;
+        for (int s = 0; s < n_split; ++s) g += ws[(size_t)s * n_pix_pad + k];
+        g *= amp[k];
+        const int dst = perm[k];
+        if (img_caller && dst >= 0) img_caller[dst] = g;
+        if (g_sorted) g_sorted[k] = g;
+        sq = (double)g * g;
+    }
+    if (part) {
+        const double t = block_sum(sq);
+        if (threadIdx.x == 0) part[blockIdx.x] = t;
+    }
+}
+
+// Fused FISTA update (a4 + a5 + a6):  g = a sum_s ws;  z = y - g/L;  I = T^{thr}(z) (eq 18);
+// y' = I + beta (I - I_old);  writes I, y', a*y' into the pixel tiles, and block partials of
+// sum I and nnz I.
+__global__ void __launch_bounds__(ET) fista_update_kernel(const float *ws, int n_split, int n_pix_pad,
+                                                          const float *amp, float4 *pix4, float *I_sorted,
+                                                          float *y_sorted, float inv_L, float thr, float beta,
+                                                          double *part_l1, double *part_nnz) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    double l1 = 0.0, nz = 0.0;
+    if (k < n_pix_pad) {
+        float g = 0.f;
+        for (int s = 0; s < n_split; ++s) g += ws[(size_t)s * n_pix_pad + k];
+        const float a = amp[k];
+        g *= a;
+        const float y = y_sorted[k];
+        const float z = fmaf(-inv_L, g, y);
+        const float I_new = (z > thr) ? z - thr : 0.f;
+        const float I_old = I_sorted[k];
+        const float y_new = fmaf(beta, I_new - I_old, I_new);
+        I_sorted[k] = I_new;
+        y_sorted[k] = y_new;
+        pix4[k].w = a * y_new;
+        l1 = I_new;
+        nz = (I_new != 0.f) ? 1.0 : 0.0;
+    }
+    if (part_l1) {
+        const double t1 = block_sum(l1);
+        const double t2 = block_sum(nz);
+        if (threadIdx.x == 0) {
+            part_l1[blockIdx.x] = t1;
+            part_nnz[blockIdx.x] = t2;
+        }
+    }
+}
+
+// out[i] = sum of n partials of array i, i < n_arrays (single CTA, fixed order).
+__global__ void __launch_bounds__(ET) sum_partials_kernel(const double *p0, const double *p1, const double *p2,
+                                                          int n0, int n1, int n2, double *out0, double *out1,
+                                                          double *out2) {
+    const double *ps[3] = {p0, p1, p2};
+    const int ns[3] = {n0, n1, n2};
+    double *outs[3] = {out0, out1, out2};
+    for (int a = 0; a < 3; ++a) {
+        if (!ps[a] || !outs[a]) continue;
+        double v = 0.0;
+        for (int i = threadIdx.x; i < ns[a]; i += ET) v += ps[a][i];
+        const double t = block_sum(v);
+        if (threadIdx.x == 0) *outs[a] = t;
+    }
+}
+
+// Power iteration (a7): x = g / ||g||, packed straight into the pixel tiles; norm2 on device.
+__global__ void __launch_bounds__(ET) normalize_pack_kernel(const float *g_sorted, const double *norm2,
+                                                            const float *amp, float4 *pix4, int n_pix_pad) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    if (k >= n_pix_pad) return;
+    const double nrm = sqrt(*norm2);
+    const float x = (nrm > 0.0) ? (float)((double)g_sorted[k] / nrm) : 0.f;
+    pix4[k].w = amp[k] * x;
+}
+
+// Gain table re-layout: raw [n_ant][n_pix] (caller order) -> gF [n_pix_pad][n_ant], gA [n_ant][n_pix_pad].
+__global__ void __launch_bounds__(ET) gains_layout_kernel(const float2 *raw, int n_ant, int n_pix,
+                                                          int n_pix_pad, const int *perm, float2 *gF,
+                                                          float2 *gA) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    const int a = blockIdx.y;
+    if (k >= n_pix_pad) return;
+    const int src = perm[k];
+    const float2 g = (src >= 0) ? raw[(size_t)a * n_pix + src] : make_float2(0.f, 0.f);
+    gF[(size_t)k * n_ant + a] = g;
+    gA[(size_t)a * n_pix_pad + k] = g;
+}
+
+// Block partials of sum I and nnz I over a sorted image (for the final info struct).
+__global__ void __launch_bounds__(ET) l1_nnz_kernel(const float *I_sorted, int n_pix_pad, double *part_l1,
+                                                    double *part_nnz) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    const float v = (k < n_pix_pad) ? I_sorted[k] : 0.f;
+    const double t1 = block_sum((double)v);
+    const double t2 = block_sum(v != 0.f ? 1.0 : 0.0);
+    if (threadIdx.x == 0) {
+        part_l1[blockIdx.x] = t1;
+        part_nnz[blockIdx.x] = t2;
+    }
+}
+
+}  // namespace sl1m

@@ -1,0 +1,381 @@
+// sl1m_kernels.cuh -- sm_100a device code of the SL1M hot path (arXiv:1310.2078).
+//
+// The matrix M (eq 9 / 16 / 17) is never stored:
+// every (visibility j, pixel k) entry is generated on the fly.  Design:
+//
+//  * Pixels are Morton-sorted at plan time into compact tiles of TP = 256 with an fp64 centre
+//    (l_c, m_c, n'_c).  The phase of a term is split as
+//        2 pi (u l + v m + w n')  =  x0(j, tile)  +  u' dl_k + v' dm_k + w' dn'_k
+//    where x0 = 2 pi frac(u l_c + v m_c + w n'_c) is evaluated ONCE per (visibility, tile) in fp64
+//    and range-reduced there, and the small offsets (dl, dm, dn') and u' = 2 pi u ... are fp32.
+//    The per-term cost is 3 FFMA + FMUL.RZ + MUFU.SIN + MUFU.COS + 2 FFMA, and the fp32 phase
+//    error scales with the tile extent instead of the field extent.
+//  * forward: a thread owns RV visibilities in registers, the CTA streams pixel tiles through
+//    shared memory with 1-D TMA bulk copies (cp.async.bulk + mbarrier, double buffered); every
+//    lane reads the same pixel (broadcast LDS.128).
+//  * adjoint: a thread owns RP pixels in registers (a warp's pixels share one tile centre), the
+//    CTA stages chunks of visibilities (u', v', w', r, x0 per centre) in shared memory.
+//  * Outputs are split across CTAs (pixel splits / visibility splits) into a workspace and
+//    reduced in a fixed order by small epilogue kernels: no float atomics, bit-stable results.
+//
+// Gaussian pixels use the real-arithmetic form of eqs (16)/(17) derived in DESIGN.md and pinned by
+// tests/test_oracle_entry.py::test_real_form_identity_used_by_the_cuda_kernels:
+//    q = w s^2, den = 1 + q^2, A = -pi s^2 ((u - w l)^2 + (v - w m)^2)/den  (<= 0, no overflow)
+//    M = a/den (1 + i q) exp(A) exp(-i (X - q A)),   X = the delta-pixel phase with n' = n - 1
+//    (eq 17) or n' = -r^2/2 (eq 16).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sl1m {
+
+constexpr int TP = 256;        // pixels per tile (one fp64 centre per tile)
+constexpr int NT = 128;        // threads per CTA in the apply kernels
+constexpr int VC = 128;        // visibilities per staged chunk in the adjoint
+constexpr int PIX_PAD = 1024;  // pixel arrays are padded to a multiple of this
+constexpr double TWO_PI = 6.283185307179586476925286766559;
+
+struct ApplyParams {
+    // visibilities (caller order)
+    int n_vis;
+    const double *u64, *v64, *w64;  // [n_vis]
+    const int *ant_p, *ant_q;       // [n_vis] (gains only)
+    // pixels (sorted order, padded)
+    int n_pix_pad;
+    int n_tiles;                    // n_pix_pad / TP
+    const float4 *pix4;             // [n_pix_pad] (dl, dm, dn', a*x)   .w rewritten per forward
+    const float2 *pixg;             // [n_pix_pad] (sigma^2, -pi log2(e) sigma^2)  (Gaussian only)
+    const double4 *cen;             // [n_tiles]   (l_c, m_c, n'_c, 0)
+    // gains
+    int n_ant;
+    const float2 *gF;               // [n_pix_pad][n_ant]  forward layout
+    const float2 *gA;               // [n_ant][n_pix_pad]  adjoint layout
+    // split bookkeeping
+    int per_split;                  // forward: pixel tiles per split; adjoint: vis chunks per split
+    // I/O
+    const float2 *r;                // adjoint input [n_vis] (re, im)
+    float2 *ws_v;                   // forward partials [n_split][n_vis]
+    float *ws_p;                    // adjoint partials [n_split][n_pix_pad]
+};
+
+// ------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + 1-D TMA bulk copy (cp.async.bulk -> SASS UBLKCP)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t ok = 0;
+    const uint32_t a = smem_u32(bar);
+    while (!ok) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(a), "r"(parity)
+            : "memory");
+    }
+}
+__device__ __forceinline__ void tma_bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes,
+                                             uint64_t *bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// x0 = 2 pi * frac(u l_c + v m_c + w n'_c), fp64, reduced to [-pi, pi] before rounding to fp32.
+__device__ __forceinline__ float centre_phase(double u, double v, double w, const double4 &c) {
+    double t = fma(u, c.x, fma(v, c.y, w * c.z));
+    t -= rint(t);
+    return static_cast<float>(t * TWO_PI);
+}
+
+// One generated term.  X is the delta-pixel phase (radians).  Returns the complex entry WITHOUT
+// the per-pixel amplitude a_k (forward folds a_k x_k into `wt`; adjoint applies a_k at the end).
+//   delta:    e = (cos X, -sin X)
+//   Gaussian: e = (1/den) 2^E2 (1 + i q)(cos X' - i sin X'),  X' = X - q A,  A = E2 ln 2
+template <int PK>
+__device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, float sig2,
+                                          float nsp, float &ere, float &eim) {
+    if (PK == 0) {
+        float s, c;
+        __sincosf(X, &s, &c);
+        ere = c;
+        eim = -s;
+    } else {
+        const float q = w * sig2;
+        const float den = fmaf(q, q, 1.0f);
+        const float rden = rcp_approx(den);
+        const float s2 = fmaf(dv, dv, du * du);
+        const float E2 = (s2 * rden) * nsp;                 // log2 of the Gaussian amplitude (<= 0)
+        const float amp = ex2_approx(E2) * rden;
+        const float Xp = fmaf(-0.69314718056f * q, E2, X);  // X - q A
+        float s, c;
+        __sincosf(Xp, &s, &c);
+        ere = amp * fmaf(q, s, c);                          // Re (1+iq)(c - is) = c + q s
+        eim = amp * fmaf(q, c, -s);                         // Im               = q c - s
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// forward:  ws_v[split][j] = sum_{k in split} M_jk x_k        (a1)
+// grid = (vis tiles of NT*RV, pixel splits); block = NT
+// ------------------------------------------------------------------------------------------
+template <int RV, int PK, int GK>
+__global__ void __launch_bounds__(NT) fwd_kernel(const ApplyParams P) {
+    __shared__ __align__(128) float4 s_pix[2][TP];
+    __shared__ __align__(128) float2 s_pixg[PK ? 2 : 1][PK ? TP : 1];
+    __shared__ __align__(8) uint64_t s_bar[2];
+
+    const int tid = threadIdx.x;
+    const int t0 = blockIdx.y * P.per_split;
+    const int t1 = min(t0 + P.per_split, P.n_tiles);
+    const int jbase = blockIdx.x * (NT * RV);
+
+    double ud[RV], vd[RV], wd[RV];
+    float uf[RV], vf[RV], wf[RV], wl[RV], re[RV], im[RV];
+    int ap[RV], aq[RV];
+#pragma unroll
+    for (int r = 0; r < RV; ++r) {
+        const int j = min(jbase + r * NT + tid, P.n_vis - 1);
+        ud[r] = P.u64[j];
+        vd[r] = P.v64[j];
+        wd[r] = P.w64[j];
+        uf[r] = static_cast<float>(TWO_PI * ud[r]);
+        vf[r] = static_cast<float>(TWO_PI * vd[r]);
+        wf[r] = static_cast<float>(TWO_PI * wd[r]);
+        wl[r] = static_cast<float>(wd[r]);
+        re[r] = 0.f;
+        im[r] = 0.f;
+        if (GK) {
+            ap[r] = P.ant_p[j];
+            aq[r] = P.ant_q[j];
+        }
+    }
+
+    constexpr uint32_t kBytes = TP * sizeof(float4) + (PK ? TP * sizeof(float2) : 0);
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int t, int st) {
+        mbar_expect_tx(&s_bar[st], kBytes);
+        tma_bulk_g2s(&s_pix[st][0], P.pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
+        if (PK) tma_bulk_g2s(&s_pixg[st][0], P.pixg + (size_t)t * TP, TP * sizeof(float2), &s_bar[st]);
+    };
+    if (tid == 0) {
+        if (t0 < t1) issue(t0, 0);
+        if (t0 + 1 < t1) issue(t0 + 1, 1);
+    }
+
+    for (int t = t0; t < t1; ++t) {
+        const int st = (t - t0) & 1;
+        const uint32_t parity = ((t - t0) >> 1) & 1;
+        const double4 c = P.cen[t];
+        float x0[RV], uc[RV], vc[RV];
+#pragma unroll
+        for (int r = 0; r < RV; ++r) {
+            x0[r] = centre_phase(ud[r], vd[r], wd[r], c);
+            if (PK) {
+                uc[r] = static_cast<float>(ud[r] - wd[r] * c.x);
+                vc[r] = static_cast<float>(vd[r] - wd[r] * c.y);
+            }
+        }
+        mbar_wait(&s_bar[st], parity);
+        const float2 *gbase = GK ? P.gF + (size_t)t * TP * P.n_ant : nullptr;
+#pragma unroll 2
+        for (int p = 0; p < TP; ++p) {
+            const float4 px = s_pix[st][p];
+            float sig2 = 0.f, nsp = 0.f;
+            if (PK) {
+                const float2 pg = s_pixg[st][p];
+                sig2 = pg.x;
+                nsp = pg.y;
+            }
+#pragma unroll
+            for (int r = 0; r < RV; ++r) {
+                const float X = fmaf(uf[r], px.x, fmaf(vf[r], px.y, fmaf(wf[r], px.z, x0[r])));
+                float du = 0.f, dv = 0.f;
+                if (PK) {
+                    du = fmaf(-wl[r], px.x, uc[r]);
+                    dv = fmaf(-wl[r], px.y, vc[r]);
+                }
+                float ere, eim;
+                gen_entry<PK>(X, du, dv, wl[r], sig2, nsp, ere, eim);
+                if (GK) {
+                    const float2 gp = __ldg(gbase + (size_t)p * P.n_ant + ap[r]);
+                    const float2 gq = __ldg(gbase + (size_t)p * P.n_ant + aq[r]);
+                    const float Gr = fmaf(gp.y, gq.y, gp.x * gq.x);   // G = gp conj(gq)
+                    const float Gi = fmaf(gp.y, gq.x, -gp.x * gq.y);
+                    const float tr = fmaf(-Gi, eim, Gr * ere);
+                    const float ti = fmaf(Gi, ere, Gr * eim);
+                    re[r] = fmaf(px.w, tr, re[r]);
+                    im[r] = fmaf(px.w, ti, im[r]);
+                } else {
+                    re[r] = fmaf(px.w, ere, re[r]);
+                    im[r] = fmaf(px.w, eim, im[r]);
+                }
+            }
+        }
+        __syncthreads();  // every thread is done with stage st
+        if (tid == 0 && t + 2 < t1) issue(t + 2, st);
+    }
+
+    float2 *out = P.ws_v + (size_t)blockIdx.y * P.n_vis;
+#pragma unroll
+    for (int r = 0; r < RV; ++r) {
+        const int j = jbase + r * NT + tid;
+        if (j < P.n_vis) out[j] = make_float2(re[r], im[r]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// adjoint:  ws_p[split][k] = Re sum_{j in split} conj(M_jk / a_k) r_j      (a2)
+// grid = (pixel groups of NT*RP, visibility splits); block = NT.
+// Warp w owns the 32*RP consecutive sorted pixels starting at base + w*32*RP; with RP = 8 that
+// is exactly one tile (one centre per warp), with RP <= 2 the whole CTA sits inside one tile.
+// ------------------------------------------------------------------------------------------
+template <int RP, int PK, int GK>
+__global__ void __launch_bounds__(NT) adj_kernel(const ApplyParams P) {
+    constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
+    __shared__ __align__(16) float4 s_vis[2][VC];        // (u', v', w', w)
+    __shared__ __align__(8) float2 s_r[2][VC];           // residual (re, im)
+    __shared__ float s_x0[2][VC][NCEN];
+    __shared__ __align__(8) float2 s_uc[PK ? 2 : 1][PK ? VC : 1][PK ? NCEN : 1];
+    __shared__ __align__(8) int2 s_ant[GK ? 2 : 1][GK ? VC : 1];
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int base = blockIdx.x * (NT * RP);
+    const int kfirst = base + warp * (32 * RP);
+    const int tile0 = base / TP;
+    const int mycen = (kfirst / TP) - tile0;
+
+    float dl[RP], dm[RP], dn[RP], acc[RP], sig2[RP], nsp[RP];
+#pragma unroll
+    for (int i = 0; i < RP; ++i) {
+        const int k = kfirst + i * 32 + lane;
+        const float4 px = P.pix4[k];
+        dl[i] = px.x;
+        dm[i] = px.y;
+        dn[i] = px.z;
+        acc[i] = 0.f;
+        if (PK) {
+            const float2 pg = P.pixg[k];
+            sig2[i] = pg.x;
+            nsp[i] = pg.y;
+        }
+    }
+    double4 cen[NCEN];
+#pragma unroll
+    for (int c = 0; c < NCEN; ++c) cen[c] = P.cen[tile0 + c];
+
+    const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const int c0 = blockIdx.y * P.per_split;
+    const int c1 = min(c0 + P.per_split, n_chunks);
+
+    auto stage = [&](int chunk, int buf) {
+        const int j = chunk * VC + tid;   // NT == VC
+        double u = 0.0, v = 0.0, w = 0.0;
+        float2 rr = make_float2(0.f, 0.f);
+        int2 a = make_int2(0, 0);
+        if (j < P.n_vis) {
+            u = P.u64[j];
+            v = P.v64[j];
+            w = P.w64[j];
+            rr = P.r[j];
+            if (GK) a = make_int2(P.ant_p[j], P.ant_q[j]);
+        }
+        s_vis[buf][tid] = make_float4(static_cast<float>(TWO_PI * u), static_cast<float>(TWO_PI * v),
+                                      static_cast<float>(TWO_PI * w), static_cast<float>(w));
+        s_r[buf][tid] = rr;
+        if (GK) s_ant[buf][tid] = a;
+#pragma unroll
+        for (int c = 0; c < NCEN; ++c) {
+            s_x0[buf][tid][c] = centre_phase(u, v, w, cen[c]);
+            if (PK)
+                s_uc[buf][tid][c] = make_float2(static_cast<float>(u - w * cen[c].x),
+                                                static_cast<float>(v - w * cen[c].y));
+        }
+    };
+
+    if (c0 < c1) stage(c0, 0);
+    __syncthreads();
+    for (int ch = c0; ch < c1; ++ch) {
+        const int buf = (ch - c0) & 1;
+        if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
+#pragma unroll 2
+        for (int t = 0; t < VC; ++t) {
+            const float4 vv = s_vis[buf][t];
+            const float2 rr = s_r[buf][t];
+            const float x0 = s_x0[buf][t][mycen];
+            float ucx = 0.f, ucy = 0.f;
+            if (PK) {
+                const float2 uc = s_uc[buf][t][mycen];
+                ucx = uc.x;
+                ucy = uc.y;
+            }
+            const float2 *gpr = nullptr, *gqr = nullptr;
+            if (GK) {
+                const int2 a = s_ant[buf][t];
+                gpr = P.gA + (size_t)a.x * P.n_pix_pad + kfirst + lane;
+                gqr = P.gA + (size_t)a.y * P.n_pix_pad + kfirst + lane;
+            }
+#pragma unroll
+            for (int i = 0; i < RP; ++i) {
+                const float X = fmaf(vv.x, dl[i], fmaf(vv.y, dm[i], fmaf(vv.z, dn[i], x0)));
+                float du = 0.f, dv = 0.f;
+                if (PK) {
+                    du = fmaf(-vv.w, dl[i], ucx);
+                    dv = fmaf(-vv.w, dm[i], ucy);
+                }
+                float ere, eim;
+                gen_entry<PK>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim);
+                // z = conj(e) r = (ere - i eim)(r_re + i r_im)
+                if (GK) {
+                    const float zre = fmaf(eim, rr.y, ere * rr.x);
+                    const float zim = fmaf(-eim, rr.x, ere * rr.y);
+                    const float2 gp = __ldg(gpr + i * 32);
+                    const float2 gq = __ldg(gqr + i * 32);
+                    const float Gr = fmaf(gp.y, gq.y, gp.x * gq.x);
+                    const float Gi = fmaf(gp.y, gq.x, -gp.x * gq.y);
+                    acc[i] += fmaf(Gi, zim, Gr * zre);      // Re(conj(G) z)
+                } else {
+                    acc[i] = fmaf(ere, rr.x, fmaf(eim, rr.y, acc[i]));
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    float *out = P.ws_p + (size_t)blockIdx.y * P.n_pix_pad;
+#pragma unroll
+    for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
+}
+
+}  // namespace sl1m

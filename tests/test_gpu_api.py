@@ -1,0 +1,200 @@
+"""GPU tests of the C-ABI behaviour: edge cases, error paths, determinism, host-buffer calls,
+device-resident gains, warm start, fp32 adjoint identity."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+
+
+def rel_l2(got, want):
+    return float(np.linalg.norm(np.asarray(got) - np.asarray(want)) / max(np.linalg.norm(want), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def sl():
+    import torch
+    import paper_1310_2078_b200 as s
+    assert torch.cuda.is_available()
+    s.load_library()
+    return s
+
+
+def _dev(a, dtype):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).to(dtype).cuda()
+
+
+@pytest.mark.parametrize("n_vis,n_pix", [(1, 1), (1, 300), (130, 1), (127, 255), (129, 257), (1000, 1025), (2049, 4097)])
+def test_ragged_and_degenerate_sizes(sl, n_vis, n_pix):
+    """Single visibility / single pixel, sizes straddling the 128-visibility chunk, the 256-pixel
+    tile and the 1024-pixel padding; irregular (non-grid) pixel positions with full w."""
+    import torch
+    rng = np.random.default_rng(n_vis * 7 + n_pix)
+    uvw = rng.uniform(-1, 1, (n_vis, 3)) * np.array([1200.0, 1200.0, 900.0])
+    l = rng.uniform(-0.2, 0.2, n_pix)
+    m = rng.uniform(-0.2, 0.2, n_pix)
+    o = oracle.Oracle(uvw, l, m)
+    plan = sl.Plan(uvw, l, m)
+    x = rng.uniform(0, 1, n_pix)
+    r = (rng.standard_normal(n_vis) + 1j * rng.standard_normal(n_vis)).astype(np.complex64)
+    got_v = plan.forward(_dev(x, torch.float32)).cpu().numpy()
+    got_g = plan.adjoint(_dev(r, torch.complex64)).cpu().numpy()
+    assert rel_l2(got_v, o.forward(x.astype(np.float32))) <= 2e-4
+    assert rel_l2(got_g, o.adjoint(r)) <= 2e-4
+    plan.close()
+
+
+def test_mixed_delta_and_gaussian_pixels_with_gains(sl):
+    """sigma_k == 0 entries inside a Gaussian plan use eq (9) under both models (reading R15)."""
+    import torch
+    rng = np.random.default_rng(77)
+    n_vis, n_pix, n_ant = 700, 900, 9
+    uvw = rng.uniform(-1, 1, (n_vis, 3)) * np.array([800.0, 800.0, 600.0])
+    l = rng.uniform(-0.1, 0.1, n_pix)
+    m = rng.uniform(-0.1, 0.1, n_pix)
+    sigma = rng.uniform(2e-4, 3e-3, n_pix)
+    sigma[::3] = 0.0
+    p = rng.integers(0, n_ant, n_vis)
+    q = rng.integers(0, n_ant, n_vis)
+    g = (rng.standard_normal((n_ant, n_pix)) + 1j * rng.standard_normal((n_ant, n_pix))).astype(np.complex64)
+    x = rng.uniform(0, 1, n_pix).astype(np.float32)
+    r = (rng.standard_normal(n_vis) + 1j * rng.standard_normal(n_vis)).astype(np.complex64)
+    for model in (0, 1):
+        o = oracle.Oracle(uvw, l, m, sigma, p, q, g, gauss_model=model)
+        plan = sl.Plan(uvw, l, m, sigma, p, q, g, gauss_model=model)
+        assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x)) <= 2e-4
+        assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r)) <= 2e-4
+        plan.close()
+
+
+def test_large_defocus_gaussian(sl):
+    """q = w sigma^2 of order one: the (1 + iq)/(1 + q^2) multiplier and the q A phase term matter."""
+    import torch
+    rng = np.random.default_rng(78)
+    n_vis, n_pix = 400, 500
+    uvw = rng.uniform(-1, 1, (n_vis, 3)) * np.array([60.0, 60.0, 20000.0])
+    l = rng.uniform(-0.01, 0.01, n_pix)
+    m = rng.uniform(-0.01, 0.01, n_pix)
+    sigma = rng.uniform(2e-3, 8e-3, n_pix)
+    o = oracle.Oracle(uvw, l, m, sigma, gauss_model=1)
+    plan = sl.Plan(uvw, l, m, sigma, gauss_model=1)
+    x = rng.uniform(0, 1, n_pix).astype(np.float32)
+    r = (rng.standard_normal(n_vis) + 1j * rng.standard_normal(n_vis)).astype(np.complex64)
+    assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x)) <= 2e-4
+    assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r)) <= 2e-4
+    plan.close()
+
+
+def test_bitwise_determinism_and_host_variants(sl):
+    import torch
+    wl = make_workload(2, n_side=64, n_steps=3, n_src=30)
+    plan = sl.Plan.from_workload(wl)
+    rng = np.random.default_rng(5)
+    x = rng.uniform(0, 1, wl.n_pix).astype(np.float32)
+    r = (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis)).astype(np.complex64)
+    xd, rd = _dev(x, torch.float32), _dev(r, torch.complex64)
+    v1 = plan.forward(xd).cpu().numpy()
+    v2 = plan.forward(xd).cpu().numpy()
+    g1 = plan.adjoint(rd).cpu().numpy()
+    g2 = plan.adjoint(rd).cpu().numpy()
+    assert np.array_equal(v1, v2) and np.array_equal(g1, g2)
+    vh = np.empty(wl.n_vis, np.complex64)
+    gh = np.empty(wl.n_pix, np.float32)
+    plan.forward_host(x, vh)
+    plan.adjoint_host(r, gh)
+    assert np.array_equal(vh, v1) and np.array_equal(gh, g1)
+    # pinned torch CPU tensors work as host buffers too
+    xp = torch.from_numpy(x).pin_memory()
+    vp = torch.empty(wl.n_vis, dtype=torch.complex64).pin_memory()
+    plan.forward_host(xp, vp)
+    assert np.array_equal(vp.numpy(), v1)
+    # solve: device and host variants agree bit for bit; a second run repeats exactly
+    V = (v1 + 0.05 * r).astype(np.complex64)
+    L = plan.max_eig(10) * 1.05
+    a, ia = plan.solve(_dev(V, torch.complex64), 5.0, L=L, n_iter=8)
+    b, ib = plan.solve(_dev(V, torch.complex64), 5.0, L=L, n_iter=8)
+    out = np.empty(wl.n_pix, np.float32)
+    _, ih = plan.solve_host(V, 5.0, L, 8, out)
+    assert np.array_equal(a.cpu().numpy(), b.cpu().numpy()) and np.array_equal(out, a.cpu().numpy())
+    assert ia.l2_term == ib.l2_term == ih.l2_term and ia.nnz == ih.nnz
+    assert plan.launch_count > 0
+    plan.close()
+
+
+def test_adjoint_identity_fp32(sl):
+    """Re <A x, y> = <x, A^H y> on the GPU path, to fp32 accumulation accuracy."""
+    import torch
+    wl = make_workload(4, n_side=48, n_ant=12, n_steps=3, n_src=20)
+    plan = sl.Plan.from_workload(wl)
+    rng = np.random.default_rng(9)
+    x = rng.standard_normal(wl.n_pix).astype(np.float32)
+    y = (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis)).astype(np.complex64)
+    Ax = plan.forward(_dev(x, torch.float32)).cpu().numpy().astype(np.complex128)
+    Ahy = plan.adjoint(_dev(y, torch.complex64)).cpu().numpy().astype(np.float64)
+    lhs = np.real(np.vdot(Ax, y.astype(np.complex128)))
+    rhs = float(np.dot(x.astype(np.float64), Ahy))
+    scale = np.linalg.norm(Ax) * np.linalg.norm(y)
+    assert abs(lhs - rhs) <= 1e-5 * scale
+    plan.close()
+
+
+def test_device_resident_gains_and_warm_start(sl):
+    import torch
+    wl = make_workload(4, n_side=32, n_ant=8, n_steps=2, n_src=15)
+    g_dev = torch.from_numpy(wl.gains).cuda()
+    p_host = sl.Plan.from_workload(wl)
+    p_dev = sl.Plan.from_workload(wl, gains_device=g_dev)
+    x = _dev(np.random.default_rng(1).uniform(0, 1, wl.n_pix), torch.float32)
+    assert torch.equal(p_host.forward(x), p_dev.forward(x))
+    # K = 0 returns x0; warm start continues from it
+    V = p_host.forward(_dev(wl.x_true, torch.float32))
+    L = p_host.max_eig(10) * 1.05
+    x0 = x.clone()
+    out0, _ = p_host.solve(V, 0.1, L=L, n_iter=0, x0=x0)
+    assert torch.equal(out0, x0)
+    o = oracle.Oracle.from_workload(wl)
+    ref = o.fista(V.cpu().numpy(), 0.1, L, 5, x0=x0.cpu().numpy().astype(np.float64))
+    out5, _ = p_host.solve(V, 0.1, L=L, n_iter=5, x0=x0)
+    assert rel_l2(out5.cpu().numpy(), ref["x"]) <= 1e-3
+    # L <= 0: the library runs its own power iteration (n_pow rounds, no safety factor)
+    outL, info = p_host.solve(V, 0.1, L=0.0, n_pow=10, n_iter=2)
+    assert abs(info.L_used - L / 1.05) <= 1e-5 * L
+    p_host.close()
+    p_dev.close()
+
+
+def test_error_paths(sl):
+    import torch
+    uvw = np.zeros((4, 3))
+    l = np.array([0.0, 0.1])
+    m = np.array([0.0, 0.1])
+    E = sl.Sl1mError
+    with pytest.raises(E, match="SL1M_ERR_DOMAIN"):
+        sl.Plan(uvw, [0.8], [0.7])
+    with pytest.raises(E, match="SL1M_ERR_DOMAIN"):
+        sl.Plan(uvw, l, m, sigma=[-1.0, 0.0])
+    with pytest.raises(E, match="SL1M_ERR_DOMAIN"):
+        sl.Plan(np.full((4, 3), np.nan), l, m)
+    with pytest.raises(E, match="SL1M_ERR_SIZE"):
+        sl.Plan(np.zeros((0, 3)), l, m)
+    with pytest.raises(E, match="SL1M_ERR_INDEX"):
+        sl.Plan(uvw, l, m, ant_p=[0, 1, 2, 0], ant_q=[1, 0, 0, 1], gains=np.ones((2, 2), np.complex64))
+    with pytest.raises(E, match="SL1M_ERR_PARAM"):
+        sl.Plan(uvw, l, m, gauss_model=7)
+    plan = sl.Plan(uvw, l, m)
+    V = torch.zeros(4, dtype=torch.complex64, device="cuda")
+    with pytest.raises(E, match="SL1M_ERR_PARAM"):
+        plan.solve(V, -1.0, L=1.0, n_iter=1)
+    with pytest.raises(E, match="SL1M_ERR_PARAM"):
+        plan.solve(V, 1.0, L=0.0, n_pow=0, n_iter=1)
+    with pytest.raises(E, match="SL1M_ERR_PARAM"):
+        plan.solve(V, 1.0, L=1.0, n_iter=-1)
+    with pytest.raises(ValueError):
+        plan.forward(torch.zeros(3, device="cuda"))
+    lib = sl.load_library()
+    assert lib.sl1m_forward(None, None, None, None) == 1           # SL1M_ERR_NULL
+    lib.sl1m_destroy(None)                                          # NULL-safe
+    plan.close()

@@ -1,0 +1,272 @@
+"""GPU parity: the CUDA path (through the C ABI / ctypes binding) against the fp64 oracle,
+element by element on the same seeded inputs.  Tolerances are north_star's: relative L2
+<= 2e-4 per forward/adjoint apply, <= 1e-3 for the image after a fixed iteration count."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import fista_lambda, make_workload
+
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = 2e-4
+TOL_IMAGE = 1e-3
+
+
+def rel_l2(got, want):
+    got = np.asarray(got)
+    want = np.asarray(want)
+    return float(np.linalg.norm(got - want) / max(np.linalg.norm(want), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def sl():
+    import torch
+    import paper_1310_2078_b200 as s
+    assert torch.cuda.is_available()
+    s.load_library()
+    return s
+
+
+def _dev(a, dtype):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).to(dtype).cuda()
+
+
+def _measured(o, wl):
+    """V = A x_true (+ blobs through a separate truth list, eq 17) + noise, rounded to complex64."""
+    V = o.forward(wl.x_true)
+    if wl.truth_extra is not None:
+        te = wl.truth_extra
+        ot = oracle.Oracle(wl.uvw, te["l"], te["m"], te["sigma"], gauss_model=1)
+        V = V + ot.forward(te["flux"])
+    return (V + wl.noise).astype(np.complex64)
+
+
+def _check_applies(sl, wl, rows=None, cols=None, seed=0):
+    """Forward on the sparse truth and on a dense U(0,1) image; adjoint on CN(0,1) and on a
+    residual-like vector.  rows/cols: sampled outputs for sizes the oracle cannot do in full."""
+    import torch
+    o = oracle.Oracle.from_workload(wl)
+    plan = sl.Plan.from_workload(wl)
+    rng = np.random.default_rng(1000 + seed)
+    out = {}
+    x_dense = rng.uniform(0, 1, wl.n_pix)
+    for name, x in (("truth", wl.x_true), ("dense", x_dense)):
+        if rows is not None and name == "dense":
+            want = o.forward(x, rows=rows)
+        elif rows is not None:
+            want = o.forward(x)[rows]
+        else:
+            want = o.forward(x)
+        got = plan.forward(_dev(x, torch.float32)).cpu().numpy()
+        if rows is not None:
+            got = got[rows]
+        out["fwd_" + name] = rel_l2(got, want)
+    r_noise = rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis)
+    r_resid = o.forward(wl.x_true) * 0.1 + 0.3 * r_noise
+    for name, r in (("noise", r_noise), ("resid", r_resid)):
+        r32 = r.astype(np.complex64)
+        want = o.adjoint(r32, cols=cols)
+        got = plan.adjoint(_dev(r32, torch.complex64)).cpu().numpy()
+        if cols is not None:
+            got = got[cols]
+        out["adj_" + name] = rel_l2(got, want)
+    plan.close()
+    for k, v in out.items():
+        assert v <= TOL_APPLY, (wl.name, k, v, out)
+    return out
+
+
+# ----------------------------------------------------------------------------- config 1
+def test_config1_applies_full(sl):
+    res = _check_applies(sl, make_workload(1))
+    print("config1", res)
+
+
+def test_config1_solver_200_iterations(sl):
+    import torch
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = fista_lambda(wl)
+    ref = o.fista(V, lam, L, wl.n_iter, want_trace=True)
+    plan = sl.Plan.from_workload(wl)
+    trace = torch.zeros(wl.n_iter * 3, dtype=torch.float64, device="cuda")
+    x, info = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=wl.n_iter, trace=trace)
+    x = x.cpu().numpy()
+    err = rel_l2(x, ref["x"])
+    assert err <= TOL_IMAGE, err
+    assert np.all(x >= 0)
+    assert info.n_iter_done == wl.n_iter and abs(info.L_used - L) <= 1e-6 * L
+    assert abs(info.l2_term - ref["l2_term"]) <= 2e-3 * ref["l2_term"]
+    assert abs(info.l1_term - ref["l1_term"]) <= 2e-3 * ref["l1_term"]
+    tr = trace.cpu().numpy().reshape(-1, 3)
+    assert np.max(np.abs(tr[:, 0] - ref["trace"][:, 0]) / ref["trace"][:, 0]) < 2e-3
+    assert np.max(np.abs(tr[:, 1] - ref["trace"][:, 1])) <= 2e-3 * ref["trace"][:, 1].max()
+    # Gradient-step parity can flip a pixel sitting within rounding of the threshold: nnz may differ slightly.
+    assert abs(info.nnz - ref["nnz"]) <= max(3, 0.05 * ref["nnz"])
+    plan.close()
+
+
+def test_config1_max_eig_matches_oracle(sl):
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    plan = sl.Plan.from_workload(wl)
+    for n_pow in (1, 5, 30):
+        L_ref = o.max_eig(n_pow)
+        L = plan.max_eig(n_pow)
+        assert abs(L - L_ref) <= 1e-4 * L_ref, (n_pow, L, L_ref)
+    plan.close()
+
+
+# ----------------------------------------------------------------------------- config 2
+def test_config2_applies_full(sl):
+    """Full 256^2 x 20,160 problem, every output compared (1.3e9 terms per oracle apply)."""
+    res = _check_applies(sl, make_workload(2))
+    print("config2", res)
+
+
+def test_config2_solver_reduced(sl):
+    """K = 50 iterations on config 2's geometry shrunk to what the oracle iterates in ~a minute
+    (64^2 pixels, 4 hour-angle steps); several pixel tiles, ragged visibility tail."""
+    import torch
+    wl = make_workload(2, n_side=64, n_steps=4, n_src=40)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = fista_lambda(wl)
+    ref = o.fista(V, lam, L, 50)
+    plan = sl.Plan.from_workload(wl)
+    x, info = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=50)
+    err = rel_l2(x.cpu().numpy(), ref["x"])
+    assert err <= TOL_IMAGE, err
+    plan.close()
+
+
+# ----------------------------------------------------------------------------- config 3
+@pytest.mark.parametrize("model", [1, 0])
+def test_config3_gaussian_applies_reduced_full_output(sl, model):
+    wl = make_workload(3, n_side=64, n_steps=3, n_src=30, n_blob=5, gauss_model=model)
+    res = _check_applies(sl, wl, seed=3 + model)
+    print("config3-reduced", model, res)
+
+
+def test_config3_gaussian_applies_full_size_sampled(sl):
+    """Full config 3 (86,016 Gaussian pixels x 20,160 vis) in the launch configuration bench.py
+    would use; 384 sampled rows / pixels each a full-length sum."""
+    wl = make_workload(3)
+    rng = np.random.default_rng(33)
+    rows = np.sort(rng.choice(wl.n_vis, 384, replace=False))
+    cols = np.sort(rng.choice(wl.n_pix, 384, replace=False))
+    res = _check_applies(sl, wl, rows=rows, cols=cols, seed=33)
+    print("config3-full-sampled", res)
+
+
+def test_config3_solver_reduced(sl):
+    import torch
+    wl = make_workload(3, n_side=32, n_steps=3, n_src=20, n_blob=4)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = fista_lambda(wl)
+    ref = o.fista(V, lam, L, 25)
+    plan = sl.Plan.from_workload(wl)
+    x, _ = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=25)
+    err = rel_l2(x.cpu().numpy(), ref["x"])
+    assert err <= TOL_IMAGE, err
+    plan.close()
+
+
+# ----------------------------------------------------------------------------- config 4
+def test_config4_gains_applies_reduced_full_output(sl):
+    wl = make_workload(4, n_side=64, n_ant=24, n_steps=3, n_src=50)
+    res = _check_applies(sl, wl, seed=4)
+    print("config4-reduced", res)
+
+
+def test_config4_gains_full_size_sampled(sl):
+    """Full config 4: 512^2 jittered pixels, 65,024 vis, 128 x 262,144 complex gain table."""
+    wl = make_workload(4)
+    rng = np.random.default_rng(44)
+    rows = np.sort(rng.choice(wl.n_vis, 256, replace=False))
+    cols = np.sort(rng.choice(wl.n_pix, 256, replace=False))
+    res = _check_applies(sl, wl, rows=rows, cols=cols, seed=44)
+    print("config4-full-sampled", res)
+
+
+def test_config4_solver_reduced(sl):
+    import torch
+    wl = make_workload(4, n_side=32, n_ant=16, n_steps=3, n_src=20)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = 0.01 * float(np.max(np.abs(o.adjoint(V))))        # noiseless config: lambda from the dirty image
+    ref = o.fista(V, lam, L, 25)
+    plan = sl.Plan.from_workload(wl)
+    x, _ = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=25)
+    err = rel_l2(x.cpu().numpy(), ref["x"])
+    assert err <= TOL_IMAGE, err
+    plan.close()
+
+
+# ----------------------------------------------------------------------------- config 5
+def test_config5_full_size_sampled_applies_and_first_iteration(sl):
+    """Paper-scale 1024^2 x 406,400 in bench.py's launch configuration.  The oracle cannot do a
+    full apply (4.3e11 terms), so: forward on the sparse truth for 512 sampled rows, forward on a
+    dense image for 64 sampled rows, adjoint for 384 sampled pixels, and ONE solver iteration
+    (I_1 = T^{lambda/L}(Re A^H V / L), from y_1 = 0) on the sampled pixels."""
+    import torch
+    wl = make_workload(5)
+    o = oracle.Oracle.from_workload(wl)
+    plan = sl.Plan.from_workload(wl)
+    rng = np.random.default_rng(55)
+    rows = np.sort(rng.choice(wl.n_vis, 512, replace=False))
+    rows_d = rows[::8]
+    cols = np.sort(rng.choice(wl.n_pix, 384, replace=False))
+    # forward, sparse truth
+    got = plan.forward(_dev(wl.x_true, torch.float32)).cpu().numpy()
+    want = o.forward(wl.x_true, rows=rows)
+    e1 = rel_l2(got[rows], want)
+    # forward, dense image
+    xd = rng.uniform(0, 1, wl.n_pix)
+    gotd = plan.forward(_dev(xd, torch.float32)).cpu().numpy()
+    wantd = o.forward(xd, rows=rows_d)
+    e2 = rel_l2(gotd[rows_d], wantd)
+    # adjoint on measured-like data
+    V = (o.forward(wl.x_true) + wl.noise).astype(np.complex64)
+    g = plan.adjoint(_dev(V, torch.complex64)).cpu().numpy()
+    g_want = o.adjoint(V, cols=cols)
+    e3 = rel_l2(g[cols], g_want)
+    print("config5 sampled", dict(fwd_truth=e1, fwd_dense=e2, adj=e3))
+    assert max(e1, e2, e3) <= TOL_APPLY, (e1, e2, e3)
+    # one FISTA iteration on the sampled pixels
+    L = 1.0e6       # any L > 0 defines the first iterate; this is the order of lambda_max here
+    lam = fista_lambda(wl)
+    x1, info = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=1, want_info=False)
+    x1 = x1.cpu().numpy()
+    z = g_want / L
+    want1 = np.where(z > lam / L, z - lam / L, 0.0)
+    assert np.all(x1 >= 0)
+    assert np.linalg.norm(x1[cols] - want1) <= TOL_IMAGE * max(np.linalg.norm(want1), np.linalg.norm(z) * 1e-2)
+    plan.close()
+
+
+def test_config5_solver_reduced(sl):
+    """Config 5's geometry (30 deg field, full w) at 96^2 pixels x 5 time steps: 9,216 pixels
+    (9 tiles, ragged) x 40,640 visibilities; K = 10 iterations against the oracle."""
+    import torch
+    wl = make_workload(5, n_side=96, n_steps=5, n_src=60)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(20) * 1.05
+    lam = fista_lambda(wl)
+    ref = o.fista(V, lam, L, 10)
+    plan = sl.Plan.from_workload(wl)
+    x, _ = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=10)
+    err = rel_l2(x.cpu().numpy(), ref["x"])
+    assert err <= TOL_IMAGE, err
+    plan.close()
