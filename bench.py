@@ -35,7 +35,6 @@ METRIC = "pixel_x_visibility_terms_per_s (A and A^H inside one FISTA iteration)"
 UNIT = "terms/s"
 MUFU_PER_SM_PER_CLK = 16      # 4 SFU lanes per SM sub-partition x 4 (B200_PROFILING / B300_MICROARCH)
 SM_COUNT = 148
-MUFU_PER_TERM = {False: 2, True: 4}   # delta: sin+cos; Gaussian: + rcp + ex2  (SASS-counted)
 
 
 def _peaks():
@@ -275,24 +274,51 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     value = world * terms_per_step * args.steps / (t_max * 1e-3)
     e2e_value = world * terms_per_step / (e2e_mean * 1e-3)
     f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
-    mufu = MUFU_PER_TERM[wl.sigma is not None]
-    peak = SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / mufu
+    desc = plan.describe()
     fwd_ms, adj_ms = statistics.median(t_fwd), statistics.median(t_adj)
-    dom = "sl1m::adj_kernel" if adj_ms >= fwd_ms else "sl1m::fwd_kernel"
-    dom_ms = max(adj_ms, fwd_ms)
-    achieved = n_terms / (dom_ms * 1e-3)
+
+    def bound(poly, r, clock_hz):
+        """Issue-rate bound (terms/s) of one apply kernel for ITS instruction mix (SASS-counted,
+        DESIGN.md section 6): a fraction f = poly/r of the terms takes the FMA-pipe polynomial
+        sincos (0 MUFU, 20 issue slots), the rest the MUFU path (mufu_per_term MUFU, 8 issue
+        slots; Gaussian 24).  peak = min(MUFU-pipe bound, issue-slot bound)."""
+        f = poly / r if r else 0.0
+        mufu = desc["mufu_per_term_mufu_path"] * (1.0 - f)
+        slots = (8.0 if not desc["gaussian"] else 24.0) * (1.0 - f) + 20.0 * f + (1.0 / r if r else 0.0)
+        if desc["gains"]:
+            slots += 10.0
+        b_mufu = SM_COUNT * MUFU_PER_SM_PER_CLK * clock_hz / mufu
+        b_issue = SM_COUNT * 128.0 * clock_hz / slots
+        return min(b_mufu, b_issue), b_mufu, b_issue
+
+    pk_f, pk_f_mufu, pk_f_issue = bound(desc["fwd_poly_of_rv"], desc["fwd_rv"], f_max)
+    pk_a, pk_a_mufu, pk_a_issue = bound(desc["adj_poly_of_rp"], desc["adj_rp"], f_max)
+    mufu_only = SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / desc["mufu_per_term_mufu_path"]
+    ach_f, ach_a = n_terms / (fwd_ms * 1e-3), n_terms / (adj_ms * 1e-3)
+    dom_is_adj = adj_ms >= fwd_ms
+    dom = "sl1m::adj_kernel" if dom_is_adj else "sl1m::fwd_kernel"
+    achieved, peak = (ach_a, pk_a) if dom_is_adj else (ach_f, pk_f)
     roof = {
         "bound": "alu", "kernel": dom, "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "Tterm/s",
         "frac": achieved / peak, "traffic": None,
-        "peak_basis": f"MUFU issue: {SM_COUNT} SMs x {MUFU_PER_SM_PER_CLK}/clk x {f_max/1e6:.0f} MHz "
-                      f"(sm_max_mhz, {peaks_src}) / {mufu} MUFU per term",
-        "fwd": {"ms": fwd_ms, "Tterm_per_s": n_terms / fwd_ms / 1e9, "frac": n_terms / (fwd_ms * 1e-3) / peak},
-        "adj": {"ms": adj_ms, "Tterm_per_s": n_terms / adj_ms / 1e9, "frac": n_terms / (adj_ms * 1e-3) / peak},
+        "peak_basis": f"min(MUFU pipe, issue slots) for the kernel's SASS instruction mix at "
+                      f"{f_max/1e6:.0f} MHz (sm_max_mhz, {peaks_src}): {SM_COUNT} SMs x {MUFU_PER_SM_PER_CLK} MUFU/clk, "
+                      f"{SM_COUNT} SMs x 128 thread-instr/clk; fwd {desc['fwd_poly_of_rv']}/{desc['fwd_rv']} and adj "
+                      f"{desc['adj_poly_of_rp']}/{desc['adj_rp']} of the terms use FMA-pipe polynomial sincos",
+        "mufu_only_bound_Tterm_per_s": mufu_only / 1e12,
+        "frac_vs_mufu_only_bound": achieved / mufu_only,
+        "fwd": {"ms": fwd_ms, "Tterm_per_s": ach_f / 1e12, "peak": pk_f / 1e12, "frac": ach_f / pk_f,
+                "mufu_bound": pk_f_mufu / 1e12, "issue_bound": pk_f_issue / 1e12},
+        "adj": {"ms": adj_ms, "Tterm_per_s": ach_a / 1e12, "peak": pk_a / 1e12, "frac": ach_a / pk_a,
+                "mufu_bound": pk_a_mufu / 1e12, "issue_bound": pk_a_issue / 1e12},
+        "plan": desc,
         "note": "per-apply time = C-ABI call (main kernel + O(N) epilogues, < 0.1 % of it); "
                 "algorithmic HBM traffic ~30 MB per apply: not an HBM-bound path",
     }
     if clocks.get("sm_mhz"):
-        roof["frac_at_sampled_clock"] = achieved / (SM_COUNT * MUFU_PER_SM_PER_CLK * clocks["sm_mhz"] * 1e6 / mufu)
+        pk_c = bound(desc["adj_poly_of_rp"] if dom_is_adj else desc["fwd_poly_of_rv"],
+                     desc["adj_rp"] if dom_is_adj else desc["fwd_rv"], clocks["sm_mhz"] * 1e6)[0]
+        roof["frac_at_sampled_clock"] = achieved / pk_c
 
     cpu = None
     if not args.no_cpu_baseline:

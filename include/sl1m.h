@@ -132,6 +132,21 @@ int sl1m_solve_host(sl1m_plan *plan, const float *vis_host, float lambda, float 
                     int n_iter, const float *x0_host, float *x_out_host,
                     sl1m_solve_info *info_host, void *stream);
 
+/* Launch configuration and instruction mix of a plan (what bench.py's roofline arithmetic uses). */
+typedef struct {
+    int32_t n_pix_padded, n_tiles;       /* sorted pixel list padded to 1,024; tiles of 256        */
+    int32_t gaussian, gains;             /* 1 if any sigma_k > 0 / if a gain table was given       */
+    int32_t fwd_rv;                      /* visibilities per thread in the forward kernel          */
+    int32_t fwd_vis_tiles, fwd_pixel_splits, fwd_tiles_per_split;
+    int32_t fwd_poly_of_rv;              /* of those rv, how many use FMA-pipe polynomial sincos   */
+    int32_t adj_rp;                      /* pixels per thread in the adjoint kernel                */
+    int32_t adj_pixel_groups, adj_vis_splits, adj_chunks_per_split;
+    int32_t adj_poly_of_rp;
+    int32_t mufu_per_term_mufu_path;     /* 2 (delta) or 4 (Gaussian)                              */
+    int32_t reserved[5];
+} sl1m_plan_info;
+int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
+
 /* Number of kernels this plan has launched since creation (for bench.py's gpu_launches). */
 int64_t sl1m_launch_count(const sl1m_plan *plan);
 

@@ -24,6 +24,13 @@ class Sl1mError(RuntimeError):
         self.status, self.name, self.detail = status, name, detail
 
 
+class _PlanInfo(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in (
+        "n_pix_padded", "n_tiles", "gaussian", "gains", "fwd_rv", "fwd_vis_tiles", "fwd_pixel_splits",
+        "fwd_tiles_per_split", "fwd_poly_of_rv", "adj_rp", "adj_pixel_groups", "adj_vis_splits",
+        "adj_chunks_per_split", "adj_poly_of_rp", "mufu_per_term_mufu_path")] + [("reserved", ctypes.c_int32 * 5)]
+
+
 class _SolveInfo(ctypes.Structure):
     _fields_ = [("n_iter_done", ctypes.c_int32), ("L_used", ctypes.c_float),
                 ("l2_term", ctypes.c_double), ("l1_term", ctypes.c_double), ("nnz", ctypes.c_int64)]
@@ -57,7 +64,7 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    path = build_library() if not os.path.exists(LIB) or os.environ.get("SL1M_REBUILD") else LIB
+    path = os.environ.get("SL1M_LIBRARY") or (build_library() if not os.path.exists(LIB) or os.environ.get("SL1M_REBUILD") else LIB)
     lib = ctypes.CDLL(path)
     vp, i64, i32, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
     lib.sl1m_plan_create.argtypes = [ctypes.POINTER(vp), i64, vp, vp, vp, i64, vp, vp, vp, i32, vp,
@@ -71,6 +78,7 @@ def load_library():
                                ctypes.POINTER(_SolveInfo), vp]
     lib.sl1m_solve_host.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, vp, vp,
                                     ctypes.POINTER(_SolveInfo), vp]
+    lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
     lib.sl1m_launch_count.argtypes = [vp]
     lib.sl1m_launch_count.restype = i64
     lib.sl1m_plan_n_vis.argtypes = [vp]
@@ -250,6 +258,12 @@ class Plan:
             ctypes.byref(info) if want_info else None, _stream_ptr(stream)))
         res = SolveInfo(info.n_iter_done, info.L_used, info.l2_term, info.l1_term, info.nnz) if want_info else None
         return out_host, res
+
+    def describe(self) -> dict:
+        """sl1m_plan_describe: launch configuration and instruction mix."""
+        info = _PlanInfo()
+        _check(load_library().sl1m_plan_describe(self._h, ctypes.byref(info)))
+        return {n: int(getattr(info, n)) for n, _ in _PlanInfo._fields_ if n != "reserved"}
 
     @property
     def launch_count(self) -> int:

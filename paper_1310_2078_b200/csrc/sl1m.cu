@@ -284,6 +284,9 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     {
         int rv = 8;
         while (rv > 1 && (int64_t)((n_vis + NT * rv - 1) / (NT * rv)) * p->n_tiles < 2 * SM_COUNT_B200) rv >>= 1;
+#ifdef SL1M_FORCE_R
+        rv = SL1M_FORCE_R;
+#endif
         p->fwd_rv = rv;
         p->fwd_vtiles = (int)((n_vis + NT * rv - 1) / (NT * rv));
         int split = std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
@@ -294,7 +297,9 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         const int n_chunks = (int)((n_vis + VC - 1) / VC);
         int rp = 8;
         while (rp > 1 && (int64_t)(p->n_pix_pad / (NT * rp)) * n_chunks < 2 * SM_COUNT_B200) rp >>= 1;
-        if (rp == 4) rp = 2;   // instantiated: 8, 2, 1
+#ifdef SL1M_FORCE_R
+        rp = SL1M_FORCE_R;
+#endif
         p->adj_rp = rp;
         p->adj_pgroups = p->n_pix_pad / (NT * rp);
         int split = std::min(n_chunks, std::max(1, (target + p->adj_pgroups - 1) / p->adj_pgroups));
@@ -344,6 +349,7 @@ template <int PK, int GK>
 void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
     switch (p->adj_rp) {
         case 8: adj_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        case 4: adj_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
         case 2: adj_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
         default: adj_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
     }
@@ -565,6 +571,28 @@ extern "C" int sl1m_solve_host(sl1m_plan *p, const float *vis_host, float lambda
         return st;
     CUDA_TRY(cudaMemcpyAsync(x_out_host, p->h_img, (size_t)p->n_pix * sizeof(float), cudaMemcpyDeviceToHost, s));
     CUDA_TRY(cudaStreamSynchronize(s));
+    return SL1M_OK;
+}
+
+extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
+    if (!p || !o) return fail(SL1M_ERR_NULL, "sl1m_plan_describe: NULL argument");
+    memset(o, 0, sizeof(*o));
+    o->n_pix_padded = p->n_pix_pad;
+    o->n_tiles = p->n_tiles;
+    o->gaussian = p->gauss;
+    o->gains = p->gains;
+    o->fwd_rv = p->fwd_rv;
+    o->fwd_vis_tiles = p->fwd_vtiles;
+    o->fwd_pixel_splits = p->fwd_split;
+    o->fwd_tiles_per_split = p->fwd_per_split;
+    o->adj_rp = p->adj_rp;
+    o->adj_pixel_groups = p->adj_pgroups;
+    o->adj_vis_splits = p->adj_split;
+    o->adj_chunks_per_split = p->adj_per_split;
+    const int pk = p->gauss ? 1 : 0;
+    o->fwd_poly_of_rv = pk ? 0 : (p->fwd_rv == 8 ? SL1M_FWD_NPOLY8 : (p->fwd_rv == 4 ? SL1M_FWD_NPOLY8 / 2 : 0));
+    o->adj_poly_of_rp = pk ? 0 : (p->adj_rp == 8 ? SL1M_ADJ_NPOLY8 : (p->adj_rp == 4 ? SL1M_ADJ_NPOLY8 / 2 : 0));
+    o->mufu_per_term_mufu_path = pk ? 4 : 2;
     return SL1M_OK;
 }
 

@@ -114,16 +114,41 @@ __device__ __forceinline__ float centre_phase(double u, double v, double w, cons
     return static_cast<float>(t * TWO_PI);
 }
 
+// sin/cos on the FMA pipe (no MUFU): X = k pi + r, r in [-pi/2, pi/2]; sin r by an odd degree-9 and cos r
+// by an even degree-8 near-minimax polynomial (Chebyshev-node fits on z = r^2 over [0, (1.02 pi/2)^2];
+// max abs error 1.2e-7 / 2.9e-7 in fp32, i.e. at least as accurate as MUFU.SIN/COS).  Returns
+// sin r, cos r and the sign bit (-1)^k as a mask to be XOR-ed into whatever multiplies them.
+// Used for a fixed fraction of the terms so that the FMA pipe, which the MUFU-bound loop leaves
+// two-thirds idle, carries part of the transcendental load.
+__device__ __forceinline__ void sincos_poly(float X, float &s, float &c, uint32_t &sign) {
+    const float kf = fmaf(X, 0.318309886183790672f, 12582912.0f);  // 1.5*2^23: k in the low mantissa bits
+    const float kr = kf - 12582912.0f;
+    const float r = fmaf(kr, -3.14159265358979324f, X);
+    const float z = r * r;
+    float ps = fmaf(z, 2.629978780532838e-06f, -0.00019821235036943108f);
+    ps = fmaf(z, ps, 0.008333230391144753f);
+    ps = fmaf(z, ps, -0.1666666567325592f);
+    s = fmaf(r * z, ps, r);
+    float pc = fmaf(z, 2.3423957827617414e-05f, -0.0013866969384253025f);
+    pc = fmaf(z, pc, 0.04166554659605026f);
+    pc = fmaf(z, pc, -0.49999991059303284f);
+    c = fmaf(z, pc, 1.0f);
+    sign = __float_as_uint(kf) << 31;
+}
+__device__ __forceinline__ float fxor(float a, uint32_t m) { return __uint_as_float(__float_as_uint(a) ^ m); }
+
 // One generated term.  X is the delta-pixel phase (radians).  Returns the complex entry WITHOUT
 // the per-pixel amplitude a_k (forward folds a_k x_k into `wt`; adjoint applies a_k at the end).
 //   delta:    e = (cos X, -sin X)
 //   Gaussian: e = (1/den) 2^E2 (1 + i q)(cos X' - i sin X'),  X' = X - q A,  A = E2 ln 2
-template <int PK>
+// POLY (delta pixels only): sin/cos from sincos_poly; the caller applies `sign` to its multiplier.
+template <int PK, bool POLY>
 __device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, float sig2,
-                                          float nsp, float &ere, float &eim) {
+                                          float nsp, float &ere, float &eim, uint32_t &sign) {
+    sign = 0u;
     if (PK == 0) {
         float s, c;
-        __sincosf(X, &s, &c);
+        if (POLY) sincos_poly(X, s, c, sign); else __sincosf(X, &s, &c);
         ere = c;
         eim = -s;
     } else {
@@ -141,12 +166,32 @@ __device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, 
     }
 }
 
+// Tuning constants of the delta-pixel / unit-gain kernels (measured on B200):
+//   *_NPOLY8   how many of a thread's 8 register-tile entries take the polynomial sincos path
+//   *_MIN_CTAS resident CTAs per SM the kernel is compiled for (register budget 65536/(128*n))
+#ifndef SL1M_FWD_NPOLY8
+#define SL1M_FWD_NPOLY8 1
+#endif
+#ifndef SL1M_ADJ_NPOLY8
+#define SL1M_ADJ_NPOLY8 2
+#endif
+#ifndef SL1M_FWD_MIN_CTAS
+#define SL1M_FWD_MIN_CTAS 5
+#endif
+#ifndef SL1M_ADJ_MIN_CTAS
+#define SL1M_ADJ_MIN_CTAS 6
+#endif
+template <int R, int PK, int NPOLY8>
+struct PolySplit {
+    static constexpr int N = (PK != 0) ? 0 : (R == 8 ? NPOLY8 : (R == 4 ? NPOLY8 / 2 : 0));
+};
+
 // ------------------------------------------------------------------------------------------
 // forward:  ws_v[split][j] = sum_{k in split} M_jk x_k        (a1)
 // grid = (vis tiles of NT*RV, pixel splits); block = NT
 // ------------------------------------------------------------------------------------------
 template <int RV, int PK, int GK>
-__global__ void __launch_bounds__(NT) fwd_kernel(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : 1) fwd_kernel(const ApplyParams P) {
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(128) float2 s_pixg[PK ? 2 : 1][PK ? TP : 1];
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -156,19 +201,19 @@ __global__ void __launch_bounds__(NT) fwd_kernel(const ApplyParams P) {
     const int t1 = min(t0 + P.per_split, P.n_tiles);
     const int jbase = blockIdx.x * (NT * RV);
 
-    double ud[RV], vd[RV], wd[RV];
+    // fp64 uvw are re-read from global (L1/L2-resident) once per pixel tile instead of living in
+    // 6 registers per visibility: the register budget buys occupancy (6 CTAs per SM).
     float uf[RV], vf[RV], wf[RV], wl[RV], re[RV], im[RV];
     int ap[RV], aq[RV];
+    const int jlast = P.n_vis - 1;
 #pragma unroll
     for (int r = 0; r < RV; ++r) {
-        const int j = min(jbase + r * NT + tid, P.n_vis - 1);
-        ud[r] = P.u64[j];
-        vd[r] = P.v64[j];
-        wd[r] = P.w64[j];
-        uf[r] = static_cast<float>(TWO_PI * ud[r]);
-        vf[r] = static_cast<float>(TWO_PI * vd[r]);
-        wf[r] = static_cast<float>(TWO_PI * wd[r]);
-        wl[r] = static_cast<float>(wd[r]);
+        const int j = min(jbase + r * NT + tid, jlast);
+        const double wd = __ldg(P.w64 + j);
+        uf[r] = static_cast<float>(TWO_PI * __ldg(P.u64 + j));
+        vf[r] = static_cast<float>(TWO_PI * __ldg(P.v64 + j));
+        wf[r] = static_cast<float>(TWO_PI * wd);
+        wl[r] = static_cast<float>(wd);
         re[r] = 0.f;
         im[r] = 0.f;
         if (GK) {
@@ -201,10 +246,12 @@ __global__ void __launch_bounds__(NT) fwd_kernel(const ApplyParams P) {
         float x0[RV], uc[RV], vc[RV];
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
-            x0[r] = centre_phase(ud[r], vd[r], wd[r], c);
+            const int j = min(jbase + r * NT + tid, jlast);
+            const double ud = __ldg(P.u64 + j), vd = __ldg(P.v64 + j), wd = __ldg(P.w64 + j);
+            x0[r] = centre_phase(ud, vd, wd, c);
             if (PK) {
-                uc[r] = static_cast<float>(ud[r] - wd[r] * c.x);
-                vc[r] = static_cast<float>(vd[r] - wd[r] * c.y);
+                uc[r] = static_cast<float>(ud - wd * c.x);
+                vc[r] = static_cast<float>(vd - wd * c.y);
             }
         }
         mbar_wait(&s_bar[st], parity);
@@ -227,7 +274,10 @@ __global__ void __launch_bounds__(NT) fwd_kernel(const ApplyParams P) {
                     dv = fmaf(-wl[r], px.y, vc[r]);
                 }
                 float ere, eim;
-                gen_entry<PK>(X, du, dv, wl[r], sig2, nsp, ere, eim);
+                uint32_t sgn;
+                if (r < PolySplit<RV, PK, SL1M_FWD_NPOLY8>::N) gen_entry<PK, true>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
+                else gen_entry<PK, false>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
+                const float wt = (r < PolySplit<RV, PK, SL1M_FWD_NPOLY8>::N) ? fxor(px.w, sgn) : px.w;
                 if (GK) {
                     const float2 gp = __ldg(gbase + (size_t)p * P.n_ant + ap[r]);
                     const float2 gq = __ldg(gbase + (size_t)p * P.n_ant + aq[r]);
@@ -235,11 +285,11 @@ __global__ void __launch_bounds__(NT) fwd_kernel(const ApplyParams P) {
                     const float Gi = fmaf(gp.y, gq.x, -gp.x * gq.y);
                     const float tr = fmaf(-Gi, eim, Gr * ere);
                     const float ti = fmaf(Gi, ere, Gr * eim);
-                    re[r] = fmaf(px.w, tr, re[r]);
-                    im[r] = fmaf(px.w, ti, im[r]);
+                    re[r] = fmaf(wt, tr, re[r]);
+                    im[r] = fmaf(wt, ti, im[r]);
                 } else {
-                    re[r] = fmaf(px.w, ere, re[r]);
-                    im[r] = fmaf(px.w, eim, im[r]);
+                    re[r] = fmaf(wt, ere, re[r]);
+                    im[r] = fmaf(wt, eim, im[r]);
                 }
             }
         }
@@ -262,7 +312,7 @@ __global__ void __launch_bounds__(NT) fwd_kernel(const ApplyParams P) {
 // is exactly one tile (one centre per warp), with RP <= 2 the whole CTA sits inside one tile.
 // ------------------------------------------------------------------------------------------
 template <int RP, int PK, int GK>
-__global__ void __launch_bounds__(NT) adj_kernel(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS : 1) adj_kernel(const ApplyParams P) {
     constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
     __shared__ __align__(16) float4 s_vis[2][VC];        // (u', v', w', w)
     __shared__ __align__(8) float2 s_r[2][VC];           // residual (re, im)
@@ -291,9 +341,6 @@ __global__ void __launch_bounds__(NT) adj_kernel(const ApplyParams P) {
             nsp[i] = pg.y;
         }
     }
-    double4 cen[NCEN];
-#pragma unroll
-    for (int c = 0; c < NCEN; ++c) cen[c] = P.cen[tile0 + c];
 
     const int n_chunks = (P.n_vis + VC - 1) / VC;
     const int c0 = blockIdx.y * P.per_split;
@@ -317,10 +364,11 @@ __global__ void __launch_bounds__(NT) adj_kernel(const ApplyParams P) {
         if (GK) s_ant[buf][tid] = a;
 #pragma unroll
         for (int c = 0; c < NCEN; ++c) {
-            s_x0[buf][tid][c] = centre_phase(u, v, w, cen[c]);
+            const double4 cen = P.cen[tile0 + c];   // L1-resident; not worth 24 registers
+            s_x0[buf][tid][c] = centre_phase(u, v, w, cen);
             if (PK)
-                s_uc[buf][tid][c] = make_float2(static_cast<float>(u - w * cen[c].x),
-                                                static_cast<float>(v - w * cen[c].y));
+                s_uc[buf][tid][c] = make_float2(static_cast<float>(u - w * cen.x),
+                                                static_cast<float>(v - w * cen.y));
         }
     };
 
@@ -355,7 +403,14 @@ __global__ void __launch_bounds__(NT) adj_kernel(const ApplyParams P) {
                     dv = fmaf(-vv.w, dm[i], ucy);
                 }
                 float ere, eim;
-                gen_entry<PK>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim);
+                uint32_t sgn;
+                if (i < PolySplit<RP, PK, SL1M_ADJ_NPOLY8>::N) {
+                    gen_entry<PK, true>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim, sgn);
+                    ere = fxor(ere, sgn);
+                    eim = fxor(eim, sgn);
+                } else {
+                    gen_entry<PK, false>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim, sgn);
+                }
                 // z = conj(e) r = (ere - i eim)(r_re + i r_im)
                 if (GK) {
                     const float zre = fmaf(eim, rr.y, ere * rr.x);
