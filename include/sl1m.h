@@ -135,7 +135,8 @@ int sl1m_solve_host(sl1m_plan *plan, const float *vis_host, float lambda, float 
 /* Launch configuration and instruction mix of a plan (what bench.py's roofline arithmetic uses). */
 typedef struct {
     int32_t n_pix_padded, n_tiles;       /* sorted pixel list padded to 1,024; tiles of 256        */
-    int32_t gaussian, gains;             /* 1 if any sigma_k > 0 / if a gain table was given       */
+    int32_t gaussian, gains;             /* gaussian: 1 if any sigma_k > 0.  gains: 0 none, 1 per-term
+                                          * loads, 2 baseline-grouped (one gain product per 8 samples) */
     int32_t fwd_rv;                      /* visibilities per thread in the forward kernel          */
     int32_t fwd_vis_tiles, fwd_pixel_splits, fwd_tiles_per_split;
     int32_t fwd_poly_of_rv;              /* of those rv, how many use FMA-pipe polynomial sincos   */

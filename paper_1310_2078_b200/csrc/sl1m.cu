@@ -40,6 +40,9 @@ constexpr int SM_COUNT_B200 = 148;
 
 struct sl1m_plan {
     int64_t n_vis = 0, n_pix = 0;
+    int n_vis_int = 0;           // internal (possibly baseline-grouped, padded) visibility count
+    int gk = 0;                  // 0 unit gains, 1 per-term gains, 2 baseline-grouped gains
+    int *vperm = nullptr;        // internal position -> caller index (-1 = padding); NULL = identity
     int n_pix_pad = 0, n_tiles = 0, n_ant = 0;
     bool gauss = false, gains = false;
     // device arrays
@@ -73,7 +76,7 @@ namespace {
 void free_plan(sl1m_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
-                    p->perm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
+                    p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img};
     for (void *q : ptrs)
         if (q) cudaFree(q);
@@ -99,7 +102,7 @@ int upload(T **dst, const T *src, size_t n) {
 ApplyParams make_params(const sl1m_plan *p) {
     ApplyParams P;
     memset(&P, 0, sizeof(P));
-    P.n_vis = (int)p->n_vis;
+    P.n_vis = p->n_vis_int;
     P.u64 = p->u64;
     P.v64 = p->v64;
     P.w64 = p->w64;
@@ -229,12 +232,61 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
             }
         }
 
-        // ---- visibilities: SoA fp64 ----
-        std::vector<double> su((size_t)n_vis), sv((size_t)n_vis), sw((size_t)n_vis);
-        for (int64_t j = 0; j < n_vis; ++j) {
-            su[(size_t)j] = uvw[3 * j];
-            sv[(size_t)j] = uvw[3 * j + 1];
-            sw[(size_t)j] = uvw[3 * j + 2];
+        // ---- visibilities: SoA fp64 in the INTERNAL order ----
+        // With gains, visibilities are grouped by baseline (p, q) into groups of 8 samples (padded):
+        // the gain product g_p conj(g_q) of a group is then loaded once per pixel instead of once
+        // per term.  Sample r of group g sits at (g / 128) * 1024 + r * 128 + g % 128, which is the
+        // forward kernel's thread layout.  Used when padding costs < 25 %; else per-term gains.
+        std::vector<int> vperm;
+        std::vector<int> ip, iq;
+        p->n_vis_int = (int)n_vis;
+        p->gk = gains ? 1 : 0;
+        if (gains) {
+            std::vector<int> order((size_t)n_vis);
+            for (int64_t j = 0; j < n_vis; ++j) order[(size_t)j] = (int)j;
+            std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+                return ant_p[a] != ant_p[b] ? ant_p[a] < ant_p[b] : ant_q[a] < ant_q[b];
+            });
+            int64_t n_groups = 0;
+            for (int64_t s0 = 0; s0 < n_vis;) {
+                int64_t s1 = s0;
+                while (s1 < n_vis && ant_p[order[(size_t)s1]] == ant_p[order[(size_t)s0]] &&
+                       ant_q[order[(size_t)s1]] == ant_q[order[(size_t)s0]]) ++s1;
+                n_groups += (s1 - s0 + 7) / 8;
+                s0 = s1;
+            }
+            const int64_t n_groups_pad = ((n_groups + NT - 1) / NT) * NT;
+            if ((double)n_vis >= 0.75 * (double)(n_groups * 8) && n_groups_pad * 8 < ((int64_t)1 << 30)) {
+                p->gk = 2;
+                p->n_vis_int = (int)(n_groups_pad * 8);
+                vperm.assign((size_t)p->n_vis_int, -1);
+                ip.assign((size_t)p->n_vis_int, 0);
+                iq.assign((size_t)p->n_vis_int, 0);
+                int64_t g = 0;
+                for (int64_t s0 = 0; s0 < n_vis;) {
+                    int64_t s1 = s0;
+                    while (s1 < n_vis && ant_p[order[(size_t)s1]] == ant_p[order[(size_t)s0]] &&
+                           ant_q[order[(size_t)s1]] == ant_q[order[(size_t)s0]]) ++s1;
+                    for (int64_t b = s0; b < s1; b += 8, ++g) {
+                        for (int r = 0; r < 8; ++r) {
+                            const size_t pos = (size_t)((g / NT) * (NT * 8) + r * NT + g % NT);
+                            ip[pos] = ant_p[order[(size_t)s0]];
+                            iq[pos] = ant_q[order[(size_t)s0]];
+                            if (b + r < s1) vperm[pos] = order[(size_t)(b + r)];
+                        }
+                    }
+                    s0 = s1;
+                }
+            }
+        }
+        const size_t nvi = (size_t)p->n_vis_int;
+        std::vector<double> su(nvi, 0.0), sv(nvi, 0.0), sw(nvi, 0.0);
+        for (size_t js = 0; js < nvi; ++js) {
+            const int64_t j = vperm.empty() ? (int64_t)js : vperm[js];
+            if (j < 0) continue;
+            su[js] = uvw[3 * j];
+            sv[js] = uvw[3 * j + 1];
+            sw[js] = uvw[3 * j + 2];
         }
 
         int st;
@@ -247,8 +299,9 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         if ((st = upload(&p->amp, amp.data(), npad))) return st;
         if ((st = upload(&p->perm, perm.data(), npad))) return st;
         if (gains) {
-            if ((st = upload(&p->ant_p, ant_p, (size_t)n_vis))) return st;
-            if ((st = upload(&p->ant_q, ant_q, (size_t)n_vis))) return st;
+            if ((st = upload(&p->ant_p, vperm.empty() ? ant_p : ip.data(), nvi))) return st;
+            if ((st = upload(&p->ant_q, vperm.empty() ? ant_q : iq.data(), nvi))) return st;
+            if (!vperm.empty() && (st = upload(&p->vperm, vperm.data(), nvi))) return st;
         }
     } catch (const std::bad_alloc &) {
         return fail(SL1M_ERR_ALLOC, "host allocation failed");
@@ -282,19 +335,21 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     // ---- launch configuration: enough CTAs for 148 SMs x 4 resident CTAs x several waves ----
     const int target = SM_COUNT_B200 * 4 * 8;
     {
+        const int64_t nvi = p->n_vis_int;
         int rv = 8;
-        while (rv > 1 && (int64_t)((n_vis + NT * rv - 1) / (NT * rv)) * p->n_tiles < 2 * SM_COUNT_B200) rv >>= 1;
+        while (rv > 1 && p->gk != 2 && (int64_t)((nvi + NT * rv - 1) / (NT * rv)) * p->n_tiles < 2 * SM_COUNT_B200)
+            rv >>= 1;
 #ifdef SL1M_FORCE_R
         rv = SL1M_FORCE_R;
 #endif
         p->fwd_rv = rv;
-        p->fwd_vtiles = (int)((n_vis + NT * rv - 1) / (NT * rv));
+        p->fwd_vtiles = (int)((nvi + NT * rv - 1) / (NT * rv));
         int split = std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
         p->fwd_per_split = (p->n_tiles + split - 1) / split;
         p->fwd_split = (p->n_tiles + p->fwd_per_split - 1) / p->fwd_per_split;
     }
     {
-        const int n_chunks = (int)((n_vis + VC - 1) / VC);
+        const int n_chunks = (p->n_vis_int + VC - 1) / VC;
         int rp = 8;
         while (rp > 1 && (int64_t)(p->n_pix_pad / (NT * rp)) * n_chunks < 2 * SM_COUNT_B200) rp >>= 1;
 #ifdef SL1M_FORCE_R
@@ -309,13 +364,13 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
 
     // ---- workspaces ----
     const size_t npad = (size_t)p->n_pix_pad;
-    CUDA_TRY(cudaMalloc((void **)&p->ws_v, (size_t)p->fwd_split * (size_t)n_vis * sizeof(float2)));
+    CUDA_TRY(cudaMalloc((void **)&p->ws_v, (size_t)p->fwd_split * (size_t)p->n_vis_int * sizeof(float2)));
     CUDA_TRY(cudaMalloc((void **)&p->ws_p, (size_t)p->adj_split * npad * sizeof(float)));
-    CUDA_TRY(cudaMalloc((void **)&p->resid, (size_t)n_vis * sizeof(float2)));
+    CUDA_TRY(cudaMalloc((void **)&p->resid, (size_t)p->n_vis_int * sizeof(float2)));
     CUDA_TRY(cudaMalloc((void **)&p->I_sorted, npad * sizeof(float)));
     CUDA_TRY(cudaMalloc((void **)&p->y_sorted, npad * sizeof(float)));
     CUDA_TRY(cudaMalloc((void **)&p->g_sorted, npad * sizeof(float)));
-    p->n_part = (int)std::max<size_t>((npad + ET - 1) / ET, ((size_t)n_vis + ET - 1) / ET);
+    p->n_part = (int)std::max<size_t>((npad + ET - 1) / ET, ((size_t)p->n_vis_int + ET - 1) / ET);
     CUDA_TRY(cudaMalloc((void **)&p->part_a, (size_t)p->n_part * sizeof(double)));
     CUDA_TRY(cudaMalloc((void **)&p->part_b, (size_t)p->n_part * sizeof(double)));
     CUDA_TRY(cudaMalloc((void **)&p->part_c, (size_t)p->n_part * sizeof(double)));
@@ -337,11 +392,15 @@ inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
 
 template <int PK, int GK>
 void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
-    switch (p->fwd_rv) {
-        case 8: fwd_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P); break;
-        case 4: fwd_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
-        case 2: fwd_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
-        default: fwd_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
+    if constexpr (GK == 2) {
+        fwd_kernel<8, PK, 2><<<grid, NT, 0, s>>>(P);
+    } else {
+        switch (p->fwd_rv) {
+            case 8: fwd_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P); break;
+            case 4: fwd_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
+            case 2: fwd_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
+            default: fwd_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        }
     }
 }
 
@@ -360,24 +419,32 @@ void launch_fwd(sl1m_plan *p, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->fwd_per_split;
     dim3 grid(p->fwd_vtiles, p->fwd_split);
-    if (p->gauss) {
-        if (p->gains) launch_fwd_rv<1, 1>(p, P, grid, s); else launch_fwd_rv<1, 0>(p, P, grid, s);
-    } else {
-        if (p->gains) launch_fwd_rv<0, 1>(p, P, grid, s); else launch_fwd_rv<0, 0>(p, P, grid, s);
+    const int key = (p->gauss ? 3 : 0) + p->gk;
+    switch (key) {
+        case 0: launch_fwd_rv<0, 0>(p, P, grid, s); break;
+        case 1: launch_fwd_rv<0, 1>(p, P, grid, s); break;
+        case 2: launch_fwd_rv<0, 2>(p, P, grid, s); break;
+        case 3: launch_fwd_rv<1, 0>(p, P, grid, s); break;
+        case 4: launch_fwd_rv<1, 1>(p, P, grid, s); break;
+        default: launch_fwd_rv<1, 2>(p, P, grid, s); break;
     }
     p->launches++;
 }
 
-// adjoint main kernel on residual r (device, [n_vis]); fills ws_p.
+// adjoint main kernel on residual r (device, INTERNAL order [n_vis_int]); fills ws_p.
 void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->adj_per_split;
     P.r = r;
     dim3 grid(p->adj_pgroups, p->adj_split);
-    if (p->gauss) {
-        if (p->gains) launch_adj_rp<1, 1>(p, P, grid, s); else launch_adj_rp<1, 0>(p, P, grid, s);
-    } else {
-        if (p->gains) launch_adj_rp<0, 1>(p, P, grid, s); else launch_adj_rp<0, 0>(p, P, grid, s);
+    const int key = (p->gauss ? 3 : 0) + p->gk;
+    switch (key) {
+        case 0: launch_adj_rp<0, 0>(p, P, grid, s); break;
+        case 1: launch_adj_rp<0, 1>(p, P, grid, s); break;
+        case 2: launch_adj_rp<0, 2>(p, P, grid, s); break;
+        case 3: launch_adj_rp<1, 0>(p, P, grid, s); break;
+        case 4: launch_adj_rp<1, 1>(p, P, grid, s); break;
+        default: launch_adj_rp<1, 2>(p, P, grid, s); break;
     }
     p->launches++;
 }
@@ -395,8 +462,8 @@ extern "C" int sl1m_forward(sl1m_plan *p, const float *x_dev, float *vis_dev, vo
     cudaStream_t s = (cudaStream_t)stream;
     pack_caller_kernel<<<egrid(p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->perm, x_dev, p->n_pix_pad);
     launch_fwd(p, s);
-    fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis, nullptr,
-                                                     (float2 *)vis_dev, nullptr);
+    fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
+                                                         (float2 *)vis_dev, 0, nullptr);
     p->launches += 2;
     return check_launch("sl1m_forward");
 }
@@ -404,7 +471,13 @@ extern "C" int sl1m_forward(sl1m_plan *p, const float *x_dev, float *vis_dev, vo
 extern "C" int sl1m_adjoint(sl1m_plan *p, const float *r_dev, float *img_dev, void *stream) {
     if (!p || !r_dev || !img_dev) return fail(SL1M_ERR_NULL, "sl1m_adjoint: NULL argument");
     cudaStream_t s = (cudaStream_t)stream;
-    launch_adj(p, (const float2 *)r_dev, s);
+    const float2 *r_int = (const float2 *)r_dev;
+    if (p->vperm) {
+        vis_gather_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>((const float2 *)r_dev, p->vperm, p->resid, p->n_vis_int);
+        p->launches++;
+        r_int = p->resid;
+    }
+    launch_adj(p, r_int, s);
     adj_reduce_kernel<<<egrid(p->n_pix_pad), ET, 0, s>>>(p->ws_p, p->adj_split, p->n_pix_pad, p->amp, p->perm,
                                                          img_dev, nullptr, nullptr);
     p->launches += 1;
@@ -458,8 +531,8 @@ extern "C" int sl1m_max_eig(sl1m_plan *p, int n_pow, float *L_out_host, void *st
     p->launches += 2;
     for (int it = 0; it < n_pow; ++it) {
         launch_fwd(p, s);
-        fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis, nullptr, p->resid,
-                                                         nullptr);
+        fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
+                                                             p->resid, 1, nullptr);
         launch_adj(p, p->resid, s);
         adj_reduce_kernel<<<egrid(npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->perm, nullptr,
                                                      p->g_sorted, p->part_a);
@@ -513,9 +586,9 @@ extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, floa
         const float beta = (float)((t - 1.0) / t_next);
         t = t_next;
         launch_fwd(p, s);
-        fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis,
-                                                         (const float2 *)vis_dev, p->resid,
-                                                         trace_dev ? p->part_a : nullptr);
+        fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
+                                                             (const float2 *)vis_dev, p->resid, 1,
+                                                             trace_dev ? p->part_a : nullptr);
         launch_adj(p, p->resid, s);
         fista_update_kernel<<<egrid(npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->pix4, p->I_sorted,
                                                        p->y_sorted, inv_L, thr, beta,
@@ -523,7 +596,7 @@ extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, floa
                                                        trace_dev ? p->part_c : nullptr);
         p->launches += 2;
         if (trace_dev) {
-            sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis), egrid(npad),
+            sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
                                                  egrid(npad), trace_dev + 3 * (size_t)k, trace_dev + 3 * (size_t)k + 1,
                                                  trace_dev + 3 * (size_t)k + 2);
             p->launches++;
@@ -537,10 +610,10 @@ extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, floa
         // one extra forward for ||M I_K - V||^2 (Table 1's L2 term)
         pack_sorted_kernel<<<egrid(npad), ET, 0, s>>>(p->pix4, p->amp, p->I_sorted, npad);
         launch_fwd(p, s);
-        fwd_reduce_kernel<<<egrid(p->n_vis), ET, 0, s>>>(p->ws_v, p->fwd_split, (int)p->n_vis,
-                                                         (const float2 *)vis_dev, p->resid, p->part_a);
+        fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
+                                                             (const float2 *)vis_dev, p->resid, 1, p->part_a);
         l1_nnz_kernel<<<egrid(npad), ET, 0, s>>>(p->I_sorted, npad, p->part_b, p->part_c);
-        sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis), egrid(npad),
+        sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
                                              egrid(npad), p->scalars + 1, p->scalars + 2, p->scalars + 3);
         p->launches += 4;
         if ((st = check_launch("sl1m_solve(info)"))) return st;
@@ -580,7 +653,7 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->n_pix_padded = p->n_pix_pad;
     o->n_tiles = p->n_tiles;
     o->gaussian = p->gauss;
-    o->gains = p->gains;
+    o->gains = p->gk;
     o->fwd_rv = p->fwd_rv;
     o->fwd_vis_tiles = p->fwd_vtiles;
     o->fwd_pixel_splits = p->fwd_split;

@@ -65,30 +65,47 @@ __global__ void __launch_bounds__(ET) fill_kernel(float *p, float v, const int *
     if (k < n_pix_pad) p[k] = (perm[k] >= 0) ? v : 0.f;
 }
 
-// Forward epilogue (a3): out[j] = sum_s ws[s][j] - V[j]; part[block] = sum |out|^2 (fp64).
-__global__ void __launch_bounds__(ET) fwd_reduce_kernel(const float2 *ws, int n_split, int n_vis,
-                                                        const float2 *V, float2 *out, double *part) {
-    const int j = blockIdx.x * ET + threadIdx.x;
+// Forward epilogue (a3): value[js] = sum_s ws[s][js] - V[caller(js)] over INTERNAL positions js;
+// written to out[js] (internal order, solver residual) or out[caller(js)] (caller order, API
+// output).  vperm maps internal -> caller (-1 = padding, value forced to 0); NULL = identity.
+// part[block] = sum |value|^2 (fp64).
+__global__ void __launch_bounds__(ET) fwd_reduce_kernel(const float2 *ws, int n_split, int n_int,
+                                                        const int *vperm, const float2 *V, float2 *out,
+                                                        int out_internal, double *part) {
+    const int js = blockIdx.x * ET + threadIdx.x;
     double sq = 0.0;
-    if (j < n_vis) {
+    if (js < n_int) {
+        const int jc = vperm ? vperm[js] : js;
         float re = 0.f, im = 0.f;
-        for (int s = 0; s < n_split; ++s) {
-            const float2 a = ws[(size_t)s * n_vis + j];
-            re += a.x;
-            im += a.y;
+        if (jc >= 0) {
+            for (int s = 0; s < n_split; ++s) {
+                const float2 a = ws[(size_t)s * n_int + js];
+                re += a.x;
+                im += a.y;
+            }
+            if (V) {
+                const float2 v = V[jc];
+                re -= v.x;
+                im -= v.y;
+            }
         }
-        if (V) {
-            const float2 v = V[j];
-            re -= v.x;
-            im -= v.y;
-        }
-        out[j] = make_float2(re, im);
+        if (out_internal) out[js] = make_float2(re, im);
+        else if (jc >= 0) out[jc] = make_float2(re, im);
         sq = (double)re * re + (double)im * im;
     }
     if (part) {
         const double t = block_sum(sq);
         if (threadIdx.x == 0) part[blockIdx.x] = t;
     }
+}
+
+// internal[js] = caller[vperm[js]] (0 on padding): brings an API residual into the internal order.
+__global__ void __launch_bounds__(ET) vis_gather_kernel(const float2 *caller, const int *vperm, float2 *internal,
+                                                        int n_int) {
+    const int js = blockIdx.x * ET + threadIdx.x;
+    if (js >= n_int) return;
+    const int jc = vperm[js];
+    internal[js] = (jc >= 0) ? caller[jc] : make_float2(0.f, 0.f);
 }
 
 // Adjoint epilogue: g_k = a_k sum_s ws[s][k]; scattered to the caller's order and/or kept sorted.

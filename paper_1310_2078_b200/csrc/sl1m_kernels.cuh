@@ -181,9 +181,9 @@ __device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, 
 #ifndef SL1M_ADJ_MIN_CTAS
 #define SL1M_ADJ_MIN_CTAS 6
 #endif
-template <int R, int PK, int NPOLY8>
+template <int R, int PK, int GK, int NPOLY8>
 struct PolySplit {
-    static constexpr int N = (PK != 0) ? 0 : (R == 8 ? NPOLY8 : (R == 4 ? NPOLY8 / 2 : 0));
+    static constexpr int N = (PK != 0 || GK != 0) ? 0 : (R == 8 ? NPOLY8 : (R == 4 ? NPOLY8 / 2 : 0));
 };
 
 // ------------------------------------------------------------------------------------------
@@ -191,7 +191,7 @@ struct PolySplit {
 // grid = (vis tiles of NT*RV, pixel splits); block = NT
 // ------------------------------------------------------------------------------------------
 template <int RV, int PK, int GK>
-__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : 1) fwd_kernel(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : (GK == 2 ? 4 : 1)) fwd_kernel(const ApplyParams P) {
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(128) float2 s_pixg[PK ? 2 : 1][PK ? TP : 1];
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -221,6 +221,9 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
             aq[r] = P.ant_q[j];
         }
     }
+    // GK == 2 ("baseline-grouped" plan): the plan laid the visibilities out so that a thread's RV
+    // entries are samples of ONE baseline (p, q): the gain product G is loaded once per pixel.
+    static_assert(GK != 2 || RV == 8, "grouped gains need RV == 8");
 
     constexpr uint32_t kBytes = TP * sizeof(float4) + (PK ? TP * sizeof(float2) : 0);
     if (tid == 0) {
@@ -256,9 +259,28 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
         }
         mbar_wait(&s_bar[st], parity);
         const float2 *gbase = GK ? P.gF + (size_t)t * TP * P.n_ant : nullptr;
+        // grouped gains: register prefetch two pixels ahead (rows are cold in L1 on first touch)
+        float2 gp0, gq0, gp1, gq1;
+        if (GK == 2) {
+            gp0 = __ldg(gbase + ap[0]);
+            gq0 = __ldg(gbase + aq[0]);
+            gp1 = __ldg(gbase + P.n_ant + ap[0]);
+            gq1 = __ldg(gbase + P.n_ant + aq[0]);
+        }
 #pragma unroll 2
         for (int p = 0; p < TP; ++p) {
             const float4 px = s_pix[st][p];
+            float Gwr = 0.f, Gwi = 0.f;
+            if (GK == 2) {
+                const float2 gp = gp0, gq = gq0;
+                gp0 = gp1;
+                gq0 = gq1;
+                const int pn = min(p + 2, TP - 1);
+                gp1 = __ldg(gbase + (size_t)pn * P.n_ant + ap[0]);
+                gq1 = __ldg(gbase + (size_t)pn * P.n_ant + aq[0]);
+                Gwr = px.w * fmaf(gp.y, gq.y, gp.x * gq.x);    // a x G,  G = gp conj(gq)
+                Gwi = px.w * fmaf(gp.y, gq.x, -gp.x * gq.y);
+            }
             float sig2 = 0.f, nsp = 0.f;
             if (PK) {
                 const float2 pg = s_pixg[st][p];
@@ -275,10 +297,13 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 }
                 float ere, eim;
                 uint32_t sgn;
-                if (r < PolySplit<RV, PK, SL1M_FWD_NPOLY8>::N) gen_entry<PK, true>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
+                if (r < PolySplit<RV, PK, GK, SL1M_FWD_NPOLY8>::N) gen_entry<PK, true>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
                 else gen_entry<PK, false>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
-                const float wt = (r < PolySplit<RV, PK, SL1M_FWD_NPOLY8>::N) ? fxor(px.w, sgn) : px.w;
-                if (GK) {
+                const float wt = (r < PolySplit<RV, PK, GK, SL1M_FWD_NPOLY8>::N) ? fxor(px.w, sgn) : px.w;
+                if (GK == 2) {
+                    re[r] = fmaf(Gwr, ere, fmaf(-Gwi, eim, re[r]));
+                    im[r] = fmaf(Gwi, ere, fmaf(Gwr, eim, im[r]));
+                } else if (GK == 1) {
                     const float2 gp = __ldg(gbase + (size_t)p * P.n_ant + ap[r]);
                     const float2 gq = __ldg(gbase + (size_t)p * P.n_ant + aq[r]);
                     const float Gr = fmaf(gp.y, gq.y, gp.x * gq.x);   // G = gp conj(gq)
@@ -312,13 +337,13 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
 // is exactly one tile (one centre per warp), with RP <= 2 the whole CTA sits inside one tile.
 // ------------------------------------------------------------------------------------------
 template <int RP, int PK, int GK>
-__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS : 1) adj_kernel(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS : (GK == 2 ? 4 : 1)) adj_kernel(const ApplyParams P) {
     constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
     __shared__ __align__(16) float4 s_vis[2][VC];        // (u', v', w', w)
     __shared__ __align__(8) float2 s_r[2][VC];           // residual (re, im)
     __shared__ float s_x0[2][VC][NCEN];
     __shared__ __align__(8) float2 s_uc[PK ? 2 : 1][PK ? VC : 1][PK ? NCEN : 1];
-    __shared__ __align__(8) int2 s_ant[GK ? 2 : 1][GK ? VC : 1];
+    __shared__ __align__(8) int2 s_ant[GK ? 2 : 1][GK ? VC : 1];   // GK == 2 uses the first VC/8 only
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int base = blockIdx.x * (NT * RP);
@@ -346,8 +371,17 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     const int c0 = blockIdx.y * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
 
+    // GK == 2: a chunk is 16 baseline groups x 8 samples.  The plan stores sample r of group g at
+    // internal position (g / 128) * 1024 + r * 128 + g % 128 (the forward's thread layout); here
+    // it is staged group-major (slot = group * 8 + sample) so 8 consecutive slots share (p, q).
     auto stage = [&](int chunk, int buf) {
-        const int j = chunk * VC + tid;   // NT == VC
+        int j = chunk * VC + tid;   // NT == VC
+        int slot = tid;
+        if (GK == 2) {
+            const int g = chunk * (VC / 8) + (tid & 15), r = tid >> 4;
+            j = (g >> 7) * (NT * 8) + r * NT + (g & 127);
+            slot = (tid & 15) * 8 + r;
+        }
         double u = 0.0, v = 0.0, w = 0.0;
         float2 rr = make_float2(0.f, 0.f);
         int2 a = make_int2(0, 0);
@@ -358,17 +392,18 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
             rr = P.r[j];
             if (GK) a = make_int2(P.ant_p[j], P.ant_q[j]);
         }
-        s_vis[buf][tid] = make_float4(static_cast<float>(TWO_PI * u), static_cast<float>(TWO_PI * v),
-                                      static_cast<float>(TWO_PI * w), static_cast<float>(w));
-        s_r[buf][tid] = rr;
-        if (GK) s_ant[buf][tid] = a;
+        s_vis[buf][slot] = make_float4(static_cast<float>(TWO_PI * u), static_cast<float>(TWO_PI * v),
+                                       static_cast<float>(TWO_PI * w), static_cast<float>(w));
+        s_r[buf][slot] = rr;
+        if (GK == 1) s_ant[buf][slot] = a;
+        if (GK == 2 && tid < 16) s_ant[buf][tid] = a;   // sample 0 carries the group's (p, q)
 #pragma unroll
         for (int c = 0; c < NCEN; ++c) {
             const double4 cen = P.cen[tile0 + c];   // L1-resident; not worth 24 registers
-            s_x0[buf][tid][c] = centre_phase(u, v, w, cen);
+            s_x0[buf][slot][c] = centre_phase(u, v, w, cen);
             if (PK)
-                s_uc[buf][tid][c] = make_float2(static_cast<float>(u - w * cen.x),
-                                                static_cast<float>(v - w * cen.y));
+                s_uc[buf][slot][c] = make_float2(static_cast<float>(u - w * cen.x),
+                                                 static_cast<float>(v - w * cen.y));
         }
     };
 
@@ -377,8 +412,34 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     for (int ch = c0; ch < c1; ++ch) {
         const int buf = (ch - c0) & 1;
         if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
+        // grouped gains: G_i = gp_i conj(gq_i) per pixel is loaded once per group of 8 samples; the
+        // 8 samples accumulate Z_i = sum conj(e) r first, then acc_i += Re(conj(G_i) Z_i).
+        float Gr[GK == 2 ? RP : 1], Gi[GK == 2 ? RP : 1], Zr[GK == 2 ? RP : 1], Zi[GK == 2 ? RP : 1];
+        float2 gpn[GK == 2 ? RP : 1], gqn[GK == 2 ? RP : 1];
+        if (GK == 2) {
+            const int2 a = s_ant[buf][0];
+#pragma unroll
+            for (int i = 0; i < RP; ++i) {
+                gpn[i] = __ldg(P.gA + (size_t)a.x * P.n_pix_pad + kfirst + lane + i * 32);
+                gqn[i] = __ldg(P.gA + (size_t)a.y * P.n_pix_pad + kfirst + lane + i * 32);
+            }
+        }
+        constexpr int GSZ = (GK == 2) ? 8 : VC;   // slots that share one gain product
+        for (int tb = 0; tb < VC; tb += GSZ) {
+            if (GK == 2) {
+                const int2 a = s_ant[buf][min((tb >> 3) + 1, VC / 8 - 1)];
+#pragma unroll
+                for (int i = 0; i < RP; ++i) {
+                    Gr[i] = fmaf(gpn[i].y, gqn[i].y, gpn[i].x * gqn[i].x);
+                    Gi[i] = fmaf(gpn[i].y, gqn[i].x, -gpn[i].x * gqn[i].y);
+                    Zr[i] = 0.f;
+                    Zi[i] = 0.f;
+                    gpn[i] = __ldg(P.gA + (size_t)a.x * P.n_pix_pad + kfirst + lane + i * 32);
+                    gqn[i] = __ldg(P.gA + (size_t)a.y * P.n_pix_pad + kfirst + lane + i * 32);
+                }
+            }
 #pragma unroll 2
-        for (int t = 0; t < VC; ++t) {
+          for (int t = tb; t < tb + GSZ; ++t) {
             const float4 vv = s_vis[buf][t];
             const float2 rr = s_r[buf][t];
             const float x0 = s_x0[buf][t][mycen];
@@ -389,7 +450,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 ucy = uc.y;
             }
             const float2 *gpr = nullptr, *gqr = nullptr;
-            if (GK) {
+            if (GK == 1) {
                 const int2 a = s_ant[buf][t];
                 gpr = P.gA + (size_t)a.x * P.n_pix_pad + kfirst + lane;
                 gqr = P.gA + (size_t)a.y * P.n_pix_pad + kfirst + lane;
@@ -404,7 +465,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 }
                 float ere, eim;
                 uint32_t sgn;
-                if (i < PolySplit<RP, PK, SL1M_ADJ_NPOLY8>::N) {
+                if (i < PolySplit<RP, PK, GK, SL1M_ADJ_NPOLY8>::N) {
                     gen_entry<PK, true>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim, sgn);
                     ere = fxor(ere, sgn);
                     eim = fxor(eim, sgn);
@@ -412,7 +473,10 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                     gen_entry<PK, false>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim, sgn);
                 }
                 // z = conj(e) r = (ere - i eim)(r_re + i r_im)
-                if (GK) {
+                if (GK == 2) {
+                    Zr[i] = fmaf(ere, rr.x, fmaf(eim, rr.y, Zr[i]));
+                    Zi[i] = fmaf(ere, rr.y, fmaf(-eim, rr.x, Zi[i]));
+                } else if (GK == 1) {
                     const float zre = fmaf(eim, rr.y, ere * rr.x);
                     const float zim = fmaf(-eim, rr.x, ere * rr.y);
                     const float2 gp = __ldg(gpr + i * 32);
@@ -423,6 +487,11 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 } else {
                     acc[i] = fmaf(ere, rr.x, fmaf(eim, rr.y, acc[i]));
                 }
+            }
+          }
+            if (GK == 2) {
+#pragma unroll
+                for (int i = 0; i < RP; ++i) acc[i] = fmaf(Gr[i], Zr[i], fmaf(Gi[i], Zi[i], acc[i]));
             }
         }
         __syncthreads();

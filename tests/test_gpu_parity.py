@@ -188,6 +188,19 @@ def test_config4_gains_applies_reduced_full_output(sl):
     print("config4-reduced", res)
 
 
+@pytest.mark.parametrize("n_steps,expect_gk", [(8, 2), (7, 2), (16, 2), (3, 1)])
+def test_config4_gains_grouped_and_generic_paths(sl, n_steps, expect_gk):
+    """Baseline-grouped gain kernels (8 samples of one baseline share one gain product; 7 -> one
+    padded slot per group, 16 -> two groups per baseline) and the per-term fallback (3 samples
+    would waste 5/8 of each group)."""
+    wl = make_workload(4, n_side=64, n_ant=20, n_steps=n_steps, n_src=50)
+    plan = sl.Plan.from_workload(wl)
+    assert plan.describe()["gains"] == expect_gk
+    plan.close()
+    res = _check_applies(sl, wl, seed=40 + n_steps)
+    print("config4-grouped", n_steps, res)
+
+
 def test_config4_gains_full_size_sampled(sl):
     """Full config 4: 512^2 jittered pixels, 65,024 vis, 128 x 262,144 complex gain table."""
     wl = make_workload(4)
