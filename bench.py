@@ -33,8 +33,11 @@ from workloads import fista_lambda, make_workload  # noqa: E402
 
 METRIC = "pixel_x_visibility_terms_per_s (A and A^H inside one FISTA iteration)"
 UNIT = "terms/s"
-MUFU_PER_SM_PER_CLK = 16      # 4 SFU lanes per SM sub-partition x 4 (B200_PROFILING / B300_MICROARCH)
+MUFU_PER_SM_PER_CLK = 16      # 4 SFU lanes per SM sub-partition x 4 (measured 15.7, profiles/r1_microbench.md)
 SM_COUNT = 148
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
+# `ncu --set full` captures summarised under profiles/ (config, kernel) -> bytes
+NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 28.6e6, (5, "adj"): 30.3e6}
 
 
 def _peaks():
@@ -277,47 +280,67 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     desc = plan.describe()
     fwd_ms, adj_ms = statistics.median(t_fwd), statistics.median(t_adj)
 
-    def bound(poly, r, clock_hz):
-        """Issue-rate bound (terms/s) of one apply kernel for ITS instruction mix (SASS-counted,
-        DESIGN.md section 6): a fraction f = poly/r of the terms takes the FMA-pipe polynomial
-        sincos (0 MUFU, 20 issue slots), the rest the MUFU path (mufu_per_term MUFU, 8 issue
-        slots; Gaussian 24).  peak = min(MUFU-pipe bound, issue-slot bound)."""
-        f = poly / r if r else 0.0
+    def bound(per16, packed, clock_hz):
+        """Issue-rate bound (terms/s) of one apply kernel for ITS OWN instruction mix (SASS-counted,
+        DESIGN.md section 6).  A fraction f = per16/16 of the terms takes the FMA-pipe polynomial
+        sincos (0 MUFU), the rest the MUFU path.  Three per-SM limits, each in terms/clk:
+          MUFU pipe   16 results/clk            / (mufu_per_term * (1 - f))
+          FMA pipe    128 fp32 lanes/clk        / lane-ops per term (an FFMA2 is 2 lane-ops)
+          issue       4 warp-instr = 128 thread-instr/clk / issue slots per term
+        peak = the smallest of the three."""
+        f = per16 / 16.0
+        gauss, gains = bool(desc["gaussian"]), bool(desc["gains"])
         mufu = desc["mufu_per_term_mufu_path"] * (1.0 - f)
-        slots = (8.0 if not desc["gaussian"] else 24.0) * (1.0 - f) + 20.0 * f + (1.0 / r if r else 0.0)
-        if desc["gains"]:
-            slots += 10.0
+        lane_mufu_path = 20.0 if gauss else 6.0      # delta: 3 phase + FMUL.RZ + 2 accumulate
+        lane_poly_path = 18.0                        # 3 phase + 3 reduce + 1 + 5 sin + 4 cos + 2 accumulate
+        lanes = lane_mufu_path * (1.0 - f) + lane_poly_path * f + (10.0 if gains else 0.0)
+        if packed:   # FFMA2 halves the issue slots of everything but FMUL.RZ and MUFU
+            slots = 5.5 * (1.0 - f) + 11.0 * f + 0.25
+        else:
+            slots = (24.0 if gauss else 8.0) * (1.0 - f) + 20.0 * f + 0.125 + (10.0 if gains else 0.0)
         b_mufu = SM_COUNT * MUFU_PER_SM_PER_CLK * clock_hz / mufu
+        b_fma = SM_COUNT * 128.0 * clock_hz / lanes
         b_issue = SM_COUNT * 128.0 * clock_hz / slots
-        return min(b_mufu, b_issue), b_mufu, b_issue
+        return min(b_mufu, b_fma, b_issue), b_mufu, b_fma, b_issue
 
-    pk_f, pk_f_mufu, pk_f_issue = bound(desc["fwd_poly_of_rv"], desc["fwd_rv"], f_max)
-    pk_a, pk_a_mufu, pk_a_issue = bound(desc["adj_poly_of_rp"], desc["adj_rp"], f_max)
+    pk_f, pk_f_mufu, pk_f_fma, pk_f_issue = bound(desc["fwd_poly_per16"], desc["fwd_packed_pairs"], f_max)
+    pk_a, pk_a_mufu, pk_a_fma, pk_a_issue = bound(desc["adj_poly_per16"], desc["adj_packed_pairs"], f_max)
     mufu_only = SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / desc["mufu_per_term_mufu_path"]
+    # best any MUFU/FMA split of this instruction set could do (delta pixels): 16(1-f) = 6(1-f) + 18 f
+    f_bal = 10.0 / 28.0
+    balanced = (SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / (2.0 * (1.0 - f_bal))
+                if not (desc["gaussian"] or desc["gains"]) else None)
     ach_f, ach_a = n_terms / (fwd_ms * 1e-3), n_terms / (adj_ms * 1e-3)
     dom_is_adj = adj_ms >= fwd_ms
     dom = "sl1m::adj_kernel" if dom_is_adj else "sl1m::fwd_kernel"
+    if (desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"]):
+        dom += "_x2"
     achieved, peak = (ach_a, pk_a) if dom_is_adj else (ach_f, pk_f)
+    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "adj" if dom_is_adj else "fwd"))
     roof = {
         "bound": "alu", "kernel": dom, "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "Tterm/s",
-        "frac": achieved / peak, "traffic": None,
-        "peak_basis": f"min(MUFU pipe, issue slots) for the kernel's SASS instruction mix at "
+        "frac": achieved / peak, "traffic": traffic,
+        "peak_basis": f"min(MUFU pipe, FMA pipe, issue slots) for the kernel's own SASS instruction mix at "
                       f"{f_max/1e6:.0f} MHz (sm_max_mhz, {peaks_src}): {SM_COUNT} SMs x {MUFU_PER_SM_PER_CLK} MUFU/clk, "
-                      f"{SM_COUNT} SMs x 128 thread-instr/clk; fwd {desc['fwd_poly_of_rv']}/{desc['fwd_rv']} and adj "
-                      f"{desc['adj_poly_of_rp']}/{desc['adj_rp']} of the terms use FMA-pipe polynomial sincos",
+                      f"x 128 fp32 lanes/clk, x 128 thread-instr/clk; fwd {desc['fwd_poly_per16']}/16 and adj "
+                      f"{desc['adj_poly_per16']}/16 of the terms use FMA-pipe polynomial sincos",
+        "traffic_basis": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full "
+                         "(profiles/, same kernel and workload); algorithmic bytes ~30 MB per apply",
         "mufu_only_bound_Tterm_per_s": mufu_only / 1e12,
         "frac_vs_mufu_only_bound": achieved / mufu_only,
+        "best_split_bound_Tterm_per_s": None if balanced is None else balanced / 1e12,
+        "frac_vs_best_split_bound": None if balanced is None else achieved / balanced,
         "fwd": {"ms": fwd_ms, "Tterm_per_s": ach_f / 1e12, "peak": pk_f / 1e12, "frac": ach_f / pk_f,
-                "mufu_bound": pk_f_mufu / 1e12, "issue_bound": pk_f_issue / 1e12},
+                "mufu_bound": pk_f_mufu / 1e12, "fma_bound": pk_f_fma / 1e12, "issue_bound": pk_f_issue / 1e12},
         "adj": {"ms": adj_ms, "Tterm_per_s": ach_a / 1e12, "peak": pk_a / 1e12, "frac": ach_a / pk_a,
-                "mufu_bound": pk_a_mufu / 1e12, "issue_bound": pk_a_issue / 1e12},
+                "mufu_bound": pk_a_mufu / 1e12, "fma_bound": pk_a_fma / 1e12, "issue_bound": pk_a_issue / 1e12},
         "plan": desc,
         "note": "per-apply time = C-ABI call (main kernel + O(N) epilogues, < 0.1 % of it); "
-                "algorithmic HBM traffic ~30 MB per apply: not an HBM-bound path",
+                "not an HBM-bound path: the matrix is generated, never read",
     }
     if clocks.get("sm_mhz"):
-        pk_c = bound(desc["adj_poly_of_rp"] if dom_is_adj else desc["fwd_poly_of_rv"],
-                     desc["adj_rp"] if dom_is_adj else desc["fwd_rv"], clocks["sm_mhz"] * 1e6)[0]
+        pk_c = bound(desc["adj_poly_per16"] if dom_is_adj else desc["fwd_poly_per16"],
+                     desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"], clocks["sm_mhz"] * 1e6)[0]
         roof["frac_at_sampled_clock"] = achieved / pk_c
 
     cpu = None

@@ -139,12 +139,14 @@ typedef struct {
                                           * loads, 2 baseline-grouped (one gain product per 8 samples) */
     int32_t fwd_rv;                      /* visibilities per thread in the forward kernel          */
     int32_t fwd_vis_tiles, fwd_pixel_splits, fwd_tiles_per_split;
-    int32_t fwd_poly_of_rv;              /* of those rv, how many use FMA-pipe polynomial sincos   */
+    int32_t fwd_poly_per16;              /* of every 16 terms, how many use FMA-pipe polynomial sincos */
     int32_t adj_rp;                      /* pixels per thread in the adjoint kernel                */
     int32_t adj_pixel_groups, adj_vis_splits, adj_chunks_per_split;
-    int32_t adj_poly_of_rp;
+    int32_t adj_poly_per16;
     int32_t mufu_per_term_mufu_path;     /* 2 (delta) or 4 (Gaussian)                              */
-    int32_t reserved[5];
+    int32_t fwd_packed_pairs;            /* 1 = the packed fp32x2 (FFMA2) forward kernel is in use  */
+    int32_t adj_packed_pairs;
+    int32_t reserved[3];
 } sl1m_plan_info;
 int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
 

@@ -27,8 +27,9 @@ class Sl1mError(RuntimeError):
 class _PlanInfo(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in (
         "n_pix_padded", "n_tiles", "gaussian", "gains", "fwd_rv", "fwd_vis_tiles", "fwd_pixel_splits",
-        "fwd_tiles_per_split", "fwd_poly_of_rv", "adj_rp", "adj_pixel_groups", "adj_vis_splits",
-        "adj_chunks_per_split", "adj_poly_of_rp", "mufu_per_term_mufu_path")] + [("reserved", ctypes.c_int32 * 5)]
+        "fwd_tiles_per_split", "fwd_poly_per16", "adj_rp", "adj_pixel_groups", "adj_vis_splits",
+        "adj_chunks_per_split", "adj_poly_per16", "mufu_per_term_mufu_path", "fwd_packed_pairs",
+        "adj_packed_pairs")] + [("reserved", ctypes.c_int32 * 3)]
 
 
 class _SolveInfo(ctypes.Structure):

@@ -396,7 +396,10 @@ void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
         fwd_kernel<8, PK, 2><<<grid, NT, 0, s>>>(P);
     } else {
         switch (p->fwd_rv) {
-            case 8: fwd_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P); break;
+            case 8:
+                if constexpr (PK == 0 && GK == 0) fwd_kernel_x2<SL1M_FWD_NPQ><<<grid, NT, 0, s>>>(P);
+                else fwd_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P);
+                break;
             case 4: fwd_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
             case 2: fwd_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
             default: fwd_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
@@ -407,7 +410,10 @@ void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
 template <int PK, int GK>
 void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
     switch (p->adj_rp) {
-        case 8: adj_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        case 8:
+            if constexpr (PK == 0 && GK == 0) adj_kernel_x2<SL1M_ADJ_NPQ><<<grid, NT, 0, s>>>(P);
+            else adj_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P);
+            break;
         case 4: adj_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
         case 2: adj_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
         default: adj_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
@@ -663,9 +669,12 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->adj_vis_splits = p->adj_split;
     o->adj_chunks_per_split = p->adj_per_split;
     const int pk = p->gauss ? 1 : 0;
-    o->fwd_poly_of_rv = pk ? 0 : (p->fwd_rv == 8 ? SL1M_FWD_NPOLY8 : (p->fwd_rv == 4 ? SL1M_FWD_NPOLY8 / 2 : 0));
-    o->adj_poly_of_rp = pk ? 0 : (p->adj_rp == 8 ? SL1M_ADJ_NPOLY8 : (p->adj_rp == 4 ? SL1M_ADJ_NPOLY8 / 2 : 0));
+    const bool plain = !pk && p->gk == 0;          // delta pixels, unit gains
+    o->fwd_poly_per16 = !plain ? 0 : (p->fwd_rv == 8 ? SL1M_FWD_NPQ : (p->fwd_rv == 4 ? (SL1M_FWD_NPOLY8 / 2) * 4 : 0));
+    o->adj_poly_per16 = !plain ? 0 : (p->adj_rp == 8 ? SL1M_ADJ_NPQ : (p->adj_rp == 4 ? (SL1M_ADJ_NPOLY8 / 2) * 4 : 0));
     o->mufu_per_term_mufu_path = pk ? 4 : 2;
+    o->fwd_packed_pairs = plain && p->fwd_rv == 8;
+    o->adj_packed_pairs = plain && p->adj_rp == 8;
     return SL1M_OK;
 }
 

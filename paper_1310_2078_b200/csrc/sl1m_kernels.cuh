@@ -26,6 +26,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace sl1m {
 
@@ -137,6 +138,69 @@ __device__ __forceinline__ void sincos_poly(float X, float &s, float &c, uint32_
 }
 __device__ __forceinline__ float fxor(float a, uint32_t m) { return __uint_as_float(__float_as_uint(a) ^ m); }
 
+// ------------------------------------------------------------------------------------------
+// Packed fp32 pairs (sm_100a FFMA2/FMUL2/FADD2): one issue slot carries two FMAs.  The MUFU-bound
+// loop is limited by issue slots as soon as part of the sincos load moves to the FMA pipe, so the
+// delta-pixel kernels keep a thread's 8 register-tile entries as 4 pairs.
+// ------------------------------------------------------------------------------------------
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+    f32x2 d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ f32x2 bc2(float x) { return pk2(x, x); }
+__device__ __forceinline__ void up2(f32x2 d, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// sincos_poly on a pair: same reduction and polynomials, 13 packed instructions for two terms.
+// sg_lo / sg_hi: the integer k of each lane in the low mantissa bits (bit 0 = parity = sign flip).
+__device__ __forceinline__ void sincos_poly2(f32x2 X, f32x2 &s, f32x2 &c, uint32_t &k_lo, uint32_t &k_hi) {
+    const f32x2 kf = fma2(X, bc2(0.318309886183790672f), bc2(12582912.0f));
+    const f32x2 kr = add2(kf, bc2(-12582912.0f));
+    const f32x2 r = fma2(kr, bc2(-3.14159265358979324f), X);
+    const f32x2 z = mul2(r, r);
+    f32x2 ps = fma2(z, bc2(2.629978780532838e-06f), bc2(-0.00019821235036943108f));
+    ps = fma2(z, ps, bc2(0.008333230391144753f));
+    ps = fma2(z, ps, bc2(-0.1666666567325592f));
+    s = fma2(mul2(r, z), ps, r);
+    f32x2 pc = fma2(z, bc2(2.3423957827617414e-05f), bc2(-0.0013866969384253025f));
+    pc = fma2(z, pc, bc2(0.04166554659605026f));
+    pc = fma2(z, pc, bc2(-0.49999991059303284f));
+    c = fma2(z, pc, bc2(1.0f));
+    float a, b;
+    up2(kf, a, b);
+    k_lo = __float_as_uint(a);
+    k_hi = __float_as_uint(b);
+}
+// x with its sign flipped when k is odd: x_bits + (k << 31) (an LEA on the ALU pipe).
+#ifndef SL1M_SIGN_MODE
+#define SL1M_SIGN_MODE 1
+#endif
+__device__ __forceinline__ float flip_if_odd(float x, uint32_t k) {
+#if SL1M_SIGN_MODE == 0
+    return __uint_as_float(__float_as_uint(x) + (k << 31));     // IMAD (FMA pipe)
+#else
+    return __uint_as_float(__float_as_uint(x) ^ (k << 31));     // SHL + LOP3 (ALU pipe)
+#endif
+}
+
 // One generated term.  X is the delta-pixel phase (radians).  Returns the complex entry WITHOUT
 // the per-pixel amplitude a_k (forward folds a_k x_k into `wt`; adjoint applies a_k at the end).
 //   delta:    e = (cos X, -sin X)
@@ -174,6 +238,13 @@ __device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, 
 #endif
 #ifndef SL1M_ADJ_NPOLY8
 #define SL1M_ADJ_NPOLY8 2
+#endif
+//   *_NPQ      packed kernels: how many of every 16 register pairs take the polynomial path
+#ifndef SL1M_FWD_NPQ
+#define SL1M_FWD_NPQ 4
+#endif
+#ifndef SL1M_ADJ_NPQ
+#define SL1M_ADJ_NPQ 4
 #endif
 #ifndef SL1M_FWD_MIN_CTAS
 #define SL1M_FWD_MIN_CTAS 5
@@ -327,6 +398,114 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     for (int r = 0; r < RV; ++r) {
         const int j = jbase + r * NT + tid;
         if (j < P.n_vis) out[j] = make_float2(re[r], im[r]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// forward, delta pixels / unit gains, packed-pair variant (the configs 1, 2, 5 path at RV = 8).
+// A thread's 8 visibilities are 4 register pairs; per pixel and pair: 3 FFMA2 (phase) + either
+// {2 FMUL.RZ, 4 MUFU} or the 13-instruction packed polynomial + 2 FFMA2 (accumulate).  NP16 of
+// every 16 terms (2 consecutive pixels x 8 visibilities) take the polynomial path; NP16 is even
+// (whole pairs).  im is accumulated with the opposite sign and negated in the epilogue.
+// ------------------------------------------------------------------------------------------
+template <int NPQ>
+__global__ void __launch_bounds__(NT, SL1M_FWD_MIN_CTAS) fwd_kernel_x2(const ApplyParams P) {
+    constexpr int RV = 8, NPAIR = 4;
+    // NPQ of the 16 pairs of 4 consecutive pixels take the polynomial path: pixel q gets (NPQ + 3 - q) / 4
+    __shared__ __align__(128) float4 s_pix[2][TP];
+    __shared__ __align__(8) uint64_t s_bar[2];
+
+    const int tid = threadIdx.x;
+    const int t0 = blockIdx.y * P.per_split;
+    const int t1 = min(t0 + P.per_split, P.n_tiles);
+    const int jbase = blockIdx.x * (NT * RV);
+    const int jlast = P.n_vis - 1;
+
+    f32x2 U[NPAIR], V[NPAIR], W[NPAIR], RE[NPAIR], IM[NPAIR];
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
+        U[i] = pk2(static_cast<float>(TWO_PI * __ldg(P.u64 + ja)), static_cast<float>(TWO_PI * __ldg(P.u64 + jb)));
+        V[i] = pk2(static_cast<float>(TWO_PI * __ldg(P.v64 + ja)), static_cast<float>(TWO_PI * __ldg(P.v64 + jb)));
+        W[i] = pk2(static_cast<float>(TWO_PI * __ldg(P.w64 + ja)), static_cast<float>(TWO_PI * __ldg(P.w64 + jb)));
+        RE[i] = pk2(0.f, 0.f);
+        IM[i] = pk2(0.f, 0.f);
+    }
+
+    constexpr uint32_t kBytes = TP * sizeof(float4);
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int t, int st) {
+        mbar_expect_tx(&s_bar[st], kBytes);
+        tma_bulk_g2s(&s_pix[st][0], P.pix4 + (size_t)t * TP, kBytes, &s_bar[st]);
+    };
+    if (tid == 0) {
+        if (t0 < t1) issue(t0, 0);
+        if (t0 + 1 < t1) issue(t0 + 1, 1);
+    }
+
+    // one pixel against the 4 pairs; the first NPOLY pairs use the FMA-pipe polynomial
+    auto pixel = [&](const float4 px, const f32x2 (&X0)[NPAIR], auto npoly_tag) {
+        constexpr int NPOLY = decltype(npoly_tag)::value;
+        const f32x2 pxx = bc2(px.x), pxy = bc2(px.y), pxz = bc2(px.z);
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i) {
+            const f32x2 X = fma2(U[i], pxx, fma2(V[i], pxy, fma2(W[i], pxz, X0[i])));
+            if (i < NPOLY) {
+                f32x2 s, c;
+                uint32_t ka, kb;
+                sincos_poly2(X, s, c, ka, kb);
+                const f32x2 wt = pk2(flip_if_odd(px.w, ka), flip_if_odd(px.w, kb));
+                RE[i] = fma2(wt, c, RE[i]);
+                IM[i] = fma2(wt, s, IM[i]);
+            } else {
+                float xa, xb, sa, ca, sb, cb;
+                up2(X, xa, xb);
+                __sincosf(xa, &sa, &ca);
+                __sincosf(xb, &sb, &cb);
+                const f32x2 wt = bc2(px.w);
+                RE[i] = fma2(wt, pk2(ca, cb), RE[i]);
+                IM[i] = fma2(wt, pk2(sa, sb), IM[i]);
+            }
+        }
+    };
+
+    for (int t = t0; t < t1; ++t) {
+        const int st = (t - t0) & 1;
+        const uint32_t parity = ((t - t0) >> 1) & 1;
+        const double4 c = P.cen[t];
+        f32x2 X0[NPAIR];
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i) {
+            const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
+            X0[i] = pk2(centre_phase(__ldg(P.u64 + ja), __ldg(P.v64 + ja), __ldg(P.w64 + ja), c),
+                        centre_phase(__ldg(P.u64 + jb), __ldg(P.v64 + jb), __ldg(P.w64 + jb), c));
+        }
+        mbar_wait(&s_bar[st], parity);
+#pragma unroll 1
+        for (int p = 0; p < TP; p += 4) {
+            pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{});
+            pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{});
+            pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{});
+            pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{});
+        }
+        __syncthreads();  // every thread is done with stage st
+        if (tid == 0 && t + 2 < t1) issue(t + 2, st);
+    }
+
+    float2 *out = P.ws_v + (size_t)blockIdx.y * P.n_vis;
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        float ra, rb, ia, ib;
+        up2(RE[i], ra, rb);
+        up2(IM[i], ia, ib);
+        const int ja = jbase + (2 * i) * NT + tid, jb = jbase + (2 * i + 1) * NT + tid;
+        if (ja < P.n_vis) out[ja] = make_float2(ra, -ia);
+        if (jb < P.n_vis) out[jb] = make_float2(rb, -ib);
     }
 }
 
@@ -500,6 +679,106 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     float *out = P.ws_p + (size_t)blockIdx.y * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
+}
+
+// ------------------------------------------------------------------------------------------
+// adjoint, delta pixels / unit gains, packed-pair variant (RP = 8).  A thread's 8 pixels are 4
+// register pairs (dl, dm, dn', acc); the CTA (1,024 sorted pixels = 4 tiles, one per warp) stages
+// chunks of 128 visibilities as (u', v', w', x0[centre]) per centre plus (r_re, -r_im), so one
+// LDS.128 + one LDS.64 feed 8 terms.  NPQ of every 16 pairs (4 consecutive visibilities x 4
+// pairs) take the polynomial path.
+// ------------------------------------------------------------------------------------------
+template <int NPQ>
+__global__ void __launch_bounds__(NT, SL1M_ADJ_MIN_CTAS) adj_kernel_x2(const ApplyParams P) {
+    constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
+    __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre)
+    __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, -r_im)
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int base = blockIdx.x * (NT * RP);
+    const int kfirst = base + warp * (32 * RP);
+    const int tile0 = base / TP;
+    const int mycen = (kfirst / TP) - tile0;
+
+    f32x2 DL[NPAIR], DM[NPAIR], DN[NPAIR], ACC[NPAIR];
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        const float4 pa = P.pix4[kfirst + (2 * i) * 32 + lane], pb = P.pix4[kfirst + (2 * i + 1) * 32 + lane];
+        DL[i] = pk2(pa.x, pb.x);
+        DM[i] = pk2(pa.y, pb.y);
+        DN[i] = pk2(pa.z, pb.z);
+        ACC[i] = pk2(0.f, 0.f);
+    }
+
+    const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const int c0 = blockIdx.y * P.per_split;
+    const int c1 = min(c0 + P.per_split, n_chunks);
+
+    auto stage = [&](int chunk, int buf) {
+        const int j = chunk * VC + tid;   // NT == VC
+        double u = 0.0, v = 0.0, w = 0.0;
+        float2 rr = make_float2(0.f, 0.f);
+        if (j < P.n_vis) {
+            u = P.u64[j];
+            v = P.v64[j];
+            w = P.w64[j];
+            rr = P.r[j];
+        }
+        const float uf = static_cast<float>(TWO_PI * u), vf = static_cast<float>(TWO_PI * v),
+                    wf = static_cast<float>(TWO_PI * w);
+        s_r[buf][tid] = make_float2(rr.x, -rr.y);
+#pragma unroll
+        for (int c = 0; c < NCEN; ++c)
+            s_vc[buf][c][tid] = make_float4(uf, vf, wf, centre_phase(u, v, w, P.cen[tile0 + c]));
+    };
+
+    auto visibility = [&](const float4 vv, const float2 rr, auto npoly_tag) {
+        constexpr int NPOLY = decltype(npoly_tag)::value;
+        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z), x0 = bc2(vv.w);
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i) {
+            const f32x2 X = fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, x0)));
+            if (i < NPOLY) {
+                f32x2 s, c;
+                uint32_t ka, kb;
+                sincos_poly2(X, s, c, ka, kb);
+                const f32x2 rre = pk2(flip_if_odd(rr.x, ka), flip_if_odd(rr.x, kb));
+                const f32x2 rim = pk2(flip_if_odd(rr.y, ka), flip_if_odd(rr.y, kb));
+                ACC[i] = fma2(c, rre, fma2(s, rim, ACC[i]));
+            } else {
+                float xa, xb, sa, ca, sb, cb;
+                up2(X, xa, xb);
+                __sincosf(xa, &sa, &ca);
+                __sincosf(xb, &sb, &cb);
+                // Re conj(e) r = c r_re - s r_im
+                ACC[i] = fma2(pk2(ca, cb), bc2(rr.x), fma2(pk2(sa, sb), bc2(rr.y), ACC[i]));
+            }
+        }
+    };
+
+    if (c0 < c1) stage(c0, 0);
+    __syncthreads();
+    for (int ch = c0; ch < c1; ++ch) {
+        const int buf = (ch - c0) & 1;
+        if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
+#pragma unroll 1
+        for (int t = 0; t < VC; t += 4) {
+            visibility(s_vc[buf][mycen][t], s_r[buf][t], std::integral_constant<int, (NPQ + 3) / 4>{});
+            visibility(s_vc[buf][mycen][t + 1], s_r[buf][t + 1], std::integral_constant<int, (NPQ + 2) / 4>{});
+            visibility(s_vc[buf][mycen][t + 2], s_r[buf][t + 2], std::integral_constant<int, (NPQ + 1) / 4>{});
+            visibility(s_vc[buf][mycen][t + 3], s_r[buf][t + 3], std::integral_constant<int, NPQ / 4>{});
+        }
+        __syncthreads();
+    }
+
+    float *out = P.ws_p + (size_t)blockIdx.y * P.n_pix_pad;
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        float a, b;
+        up2(ACC[i], a, b);
+        out[kfirst + (2 * i) * 32 + lane] = a;
+        out[kfirst + (2 * i + 1) * 32 + lane] = b;
+    }
 }
 
 }  // namespace sl1m
