@@ -246,6 +246,12 @@ __device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, 
 #ifndef SL1M_ADJ_NPQ
 #define SL1M_ADJ_NPQ 4
 #endif
+#ifndef SL1M_FWD_X2_MIN_CTAS
+#define SL1M_FWD_X2_MIN_CTAS 4
+#endif
+#ifndef SL1M_ADJ_X2_MIN_CTAS
+#define SL1M_ADJ_X2_MIN_CTAS 5
+#endif
 #ifndef SL1M_FWD_MIN_CTAS
 #define SL1M_FWD_MIN_CTAS 5
 #endif
@@ -409,7 +415,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
 // (whole pairs).  im is accumulated with the opposite sign and negated in the epilogue.
 // ------------------------------------------------------------------------------------------
 template <int NPQ>
-__global__ void __launch_bounds__(NT, SL1M_FWD_MIN_CTAS) fwd_kernel_x2(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const ApplyParams P) {
     constexpr int RV = 8, NPAIR = 4;
     // NPQ of the 16 pairs of 4 consecutive pixels take the polynomial path: pixel q gets (NPQ + 3 - q) / 4
     __shared__ __align__(128) float4 s_pix[2][TP];
@@ -689,7 +695,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
 // pairs) take the polynomial path.
 // ------------------------------------------------------------------------------------------
 template <int NPQ>
-__global__ void __launch_bounds__(NT, SL1M_ADJ_MIN_CTAS) adj_kernel_x2(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const ApplyParams P) {
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
     __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre)
     __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, -r_im)
