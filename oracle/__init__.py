@@ -58,6 +58,8 @@ def _load():
         lib.oracle_threshold.argtypes = [f64, f64]
         lib.oracle_threshold.restype = f64
         lib.oracle_fista.argtypes = [P, vp, f64, f64, i32, vp, vp, vp, vp]
+        lib.oracle_fista_tol.argtypes = [P, vp, f64, f64, i32, f64, i32, vp, vp, vp, vp]
+        lib.oracle_fista_tol.restype = i32
         _lib = lib
     return _lib
 
@@ -164,3 +166,22 @@ class Oracle:
         if want_trace:
             out["trace"] = trace[:n_iter]
         return out
+
+    # O5 + the termination rule of PAPER.md:194 / :239 (reading R21)
+    def fista_tol(self, V, lam: float, L: float, max_iter: int, tol: float, check_every: int = 1, x0=None):
+        V = np.ascontiguousarray(np.asarray(V, dtype=np.complex128)).view(np.float64)
+        assert V.shape[0] == 2 * self.n_vis
+        x0a = None if x0 is None else np.ascontiguousarray(x0, dtype=np.float64)
+        x = np.zeros(self.n_pix)
+        trace = np.zeros((max(max_iter, 1), 3))
+        info = np.zeros(3)
+        n_done = _load().oracle_fista_tol(ctypes.byref(self._c), _ptr(V), float(lam), float(L), int(max_iter),
+                                          float(tol), int(check_every), _ptr(x0a), _ptr(x), _ptr(trace),
+                                          _ptr(info))
+        return dict(x=x, n_iter_done=int(n_done), trace=trace[:n_done], l2_term=float(info[0]),
+                    l1_term=float(info[1]), nnz=int(info[2]))
+
+    # PAPER.md:327 "use the dirty image as the initial condition": the back-projected data,
+    # scaled and clipped to the positive orthant the solver lives in (reading R22).
+    def dirty_image(self, V, scale: float):
+        return np.maximum(0.0, float(scale) * self.adjoint(V))

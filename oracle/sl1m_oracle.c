@@ -166,9 +166,19 @@ double oracle_threshold(double x, double d) { return (x > d) ? x - d : 0.0; }
 /* O5: FISTA as listed at PAPER.md:188-192 (readings R8, R9: step 1/L, threshold lambda/L).
  * trace (nullable) gets, per iteration k, {||A y_k - V||^2, sum_i I_k[i], nnz(I_k)}.
  * info3 gets {||A I_K - V||^2, sum I_K, nnz(I_K)}. */
-void oracle_fista(const oracle_problem *P, const double *V /* [n_vis][2] */, double lambda, double L,
-                  int32_t n_iter, const double *x0 /* nullable */, double *x_out /* [n_pix] */,
-                  double *trace /* [n_iter][3] or NULL */, double *info3 /* nullable */) {
+/* O5 with the termination rule of PAPER.md:194 ("terminated when an iteration leads to a
+ * sufficiently small change in the total error E, given by equation (10)"; section 4.1.1,
+ * "until the total error changes no more than 1 part in 10^6 or until 7000
+ * iterations were reached").  Reading R21: E is formed from what the iteration
+ * already has -- E_k = ||M y_k - V||^2 + 2 lambda sum I_k, i.e. eq (10) with lambda_paper =
+ * 2 lambda (reading R9) and the residual of y_k (MFISTA's extra evaluation of M is what the
+ * paper avoids).  The rule is looked at only when k is a multiple of check_every
+ * (k >= 2): stop after iteration k iff |E_k - E_{k-1}| <= tol * |E_k|.  tol < 0 never stops.
+ * Returns the number of iterations done. */
+int32_t oracle_fista_tol(const oracle_problem *P, const double *V /* [n_vis][2] */, double lambda, double L,
+                         int32_t n_iter /* cap */, double tol, int32_t check_every,
+                         const double *x0 /* nullable */, double *x_out /* [n_pix] */,
+                         double *trace /* [n_iter][3] or NULL */, double *info3 /* nullable */) {
     const int64_t np = P->n_pix, nv = P->n_vis;
     double *Ik = (double *)calloc(np, sizeof(double));
     double *Iprev = (double *)calloc(np, sizeof(double));
@@ -178,6 +188,8 @@ void oracle_fista(const oracle_problem *P, const double *V /* [n_vis][2] */, dou
     if (x0) { memcpy(Ik, x0, sizeof(double) * np); memcpy(y, x0, sizeof(double) * np); }
     double t = 1.0;
     const double d = lambda / L;
+    double E_prev = 0.0;
+    int32_t n_done = 0;
     for (int32_t it = 0; it < n_iter; ++it) {
         oracle_forward(P, y, nv, NULL, r);
         double l2 = 0.0;
@@ -195,6 +207,11 @@ void oracle_fista(const oracle_problem *P, const double *V /* [n_vis][2] */, dou
         for (int64_t k = 0; k < np; ++k) y[k] = Ik[k] + beta * (Ik[k] - Iprev[k]);
         t = t_next;
         if (trace) { trace[3 * it] = l2; trace[3 * it + 1] = l1; trace[3 * it + 2] = nnz; }
+        n_done = it + 1;
+        const double E = l2 + 2.0 * lambda * l1;                       /* eq (10), reading R21 */
+        const int look = tol >= 0.0 && n_done >= 2 && check_every >= 1 && (n_done % check_every) == 0;
+        if (look && fabs(E - E_prev) <= tol * fabs(E)) break;
+        E_prev = E;
     }
     memcpy(x_out, Ik, sizeof(double) * np);
     if (info3) {
@@ -205,4 +222,12 @@ void oracle_fista(const oracle_problem *P, const double *V /* [n_vis][2] */, dou
         info3[0] = l2; info3[1] = l1; info3[2] = nnz;
     }
     free(Ik); free(Iprev); free(y); free(g); free(r);
+    return n_done;
+}
+
+/* O5, fixed iteration count (north_star): the listing of PAPER.md:188-192 run n_iter times. */
+void oracle_fista(const oracle_problem *P, const double *V /* [n_vis][2] */, double lambda, double L,
+                  int32_t n_iter, const double *x0 /* nullable */, double *x_out /* [n_pix] */,
+                  double *trace /* [n_iter][3] or NULL */, double *info3 /* nullable */) {
+    (void)oracle_fista_tol(P, V, lambda, L, n_iter, -1.0, 1, x0, x_out, trace, info3);
 }

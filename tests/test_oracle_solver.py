@@ -182,3 +182,90 @@ def test_config1_noiseless_recovers_the_sparse_sky():
     big = set(np.flatnonzero(I > 0.02))
     assert big == sup_true
     assert np.max(np.abs(I - wl.x_true)) < 0.02
+
+
+def _dft_lattice(N=8, delta=2e-3):
+    k = np.arange(N * N)
+    l = (k % N - N // 2) * delta
+    m = (k // N - N // 2) * delta
+    a = np.arange(N)
+    uu, vv = np.meshgrid(a, a, indexing="xy")
+    uvw = np.stack([uu.ravel() / (N * delta), vv.ravel() / (N * delta), np.zeros(N * N)], 1)
+    g = np.sqrt(np.sqrt(1 - l * l - m * m))
+    gains = np.stack([g, g]).astype(np.complex64)
+    return oracle.Oracle(uvw, l, m, ant_p=np.zeros(N * N, np.int32), ant_q=np.ones(N * N, np.int32), gains=gains)
+
+
+def test_tolerance_stop_rule():
+    """Reading R21: stop when the total error E of eq (10) changes by no more
+    than `tol` relative, looked at every `check_every` iterations.
+    (i)  DFT lattice: FISTA sits on the exact minimiser from I_1 on (closed form, reading R13).
+         E_k carries the residual of y_k and y_1 = 0, y_2 = I_1, y_3 = I_2 = I_1: so E_1 != E_2 = E_3
+         and the rule must fire at the first looked-at k >= 3, for any tol > 0.
+    (ii) the stopping index is the first looked-at k whose |E_k - E_{k-1}| <= tol |E_k|, with E
+         formed independently here from the fixed-K run's trace and the dense matrix.
+    (iii) stopping only truncates: the result equals the fixed-K run at K = n_iter_done, tol < 0
+         never stops, and a smaller tol never stops earlier."""
+    o = _dft_lattice()
+    rng = np.random.default_rng(8)
+    V = rng.standard_normal(64) + 1j * rng.standard_normal(64)
+    for every, want in ((1, 3), (2, 4), (3, 3), (4, 4)):
+        r = o.fista_tol(V, lam=3.0, L=64.0, max_iter=50, tol=1e-4, check_every=every)
+        assert r["n_iter_done"] == want
+    # (ii), (iii) on a generic tiny problem
+    rng = np.random.default_rng(35)
+    o = _tiny(rng, n_vis=80, n_pix=30)
+    x_true = np.zeros(o.n_pix)
+    x_true[[3, 11, 17, 25]] = [1.0, 0.4, 2.5, 0.7]
+    V = o.forward(x_true) + 0.01 * (rng.standard_normal(o.n_vis) + 1j * rng.standard_normal(o.n_vis))
+    M = o.dense()
+    L = np.linalg.eigvalsh((M.conj().T @ M).real)[-1] * 1.05
+    lam, K = 0.5, 400
+    full = o.fista(V, lam=lam, L=L, n_iter=K, want_trace=True)
+    E = full["trace"][:, 0] + 2.0 * lam * full["trace"][:, 1]
+    # trace[:, 0] really is ||M y_k - V||^2: rebuild y_2 from the first two iterates by hand
+    I1 = o.fista(V, lam=lam, L=L, n_iter=1)["x"]
+    I2 = o.fista(V, lam=lam, L=L, n_iter=2)["x"]
+    t2 = (1 + math.sqrt(5)) / 2
+    t3 = (1 + math.sqrt(1 + 4 * t2 * t2)) / 2
+    y2 = I1                                   # beta_1 = (t_1 - 1)/t_2 = 0
+    y3 = I2 + (t2 - 1) / t3 * (I2 - I1)
+    assert abs(full["trace"][1, 0] - np.sum(np.abs(M @ y2 - V) ** 2)) < 1e-9
+    assert abs(full["trace"][2, 0] - np.sum(np.abs(M @ y3 - V) ** 2)) < 1e-9
+    last = 0
+    for tol in (1e-2, 1e-4, 1e-6, 1e-8):
+        for every in (1, 5):
+            ks = [k for k in range(2, K + 1) if k % every == 0 and abs(E[k - 1] - E[k - 2]) <= tol * abs(E[k - 1])]
+            want = ks[0] if ks else K
+            r = o.fista_tol(V, lam=lam, L=L, max_iter=K, tol=tol, check_every=every)
+            assert r["n_iter_done"] == want
+            same = o.fista(V, lam=lam, L=L, n_iter=want)
+            assert np.array_equal(r["x"], same["x"]) and r["l2_term"] == same["l2_term"]
+        assert want >= last
+        last = want
+    assert 2 < last < K                       # the sweep really exercised early stops
+    assert o.fista_tol(V, lam=lam, L=L, max_iter=37, tol=-1.0)["n_iter_done"] == 37
+
+
+def test_dirty_image_start():
+    """Reading R22: the dirty image max(0, s Re A^H V) as I_0.  On the DFT lattice
+    Re A^H V / N^2 is numpy's inverse FFT; and FISTA's first iterate from zero is
+    T^{lambda/L}(dirty/L), so starting from the dirty image must not change the fixed point."""
+    N = 8
+    o = _dft_lattice(N)
+    rng = np.random.default_rng(9)
+    V = rng.standard_normal(N * N) + 1j * rng.standard_normal(N * N)
+    a = np.arange(N)
+    uu, vv = np.meshgrid(a, a, indexing="xy")
+    R = np.zeros((N, N), dtype=complex)
+    R[vv.ravel(), uu.ravel()] = V * ((-1.0) ** (uu.ravel() + vv.ravel()))
+    want = np.maximum(0.0, np.fft.ifft2(R).real.ravel())
+    got = o.dirty_image(V, 1.0 / N**2)
+    assert np.max(np.abs(got - want)) < 5e-6 and np.count_nonzero(got) > 5
+    rng = np.random.default_rng(36)
+    o = _tiny(rng, n_vis=80, n_pix=30)
+    V = o.forward(rng.uniform(0, 1, o.n_pix))
+    L = o.max_eig(200) * 1.05
+    cold = o.fista(V, lam=0.2, L=L, n_iter=3000)["x"]
+    warm = o.fista(V, lam=0.2, L=L, n_iter=3000, x0=o.dirty_image(V, 1.0 / o.n_vis))["x"]
+    assert np.max(np.abs(cold - warm)) < 1e-7
