@@ -127,6 +127,32 @@ int sl1m_solve(sl1m_plan *plan, const float *vis_dev, float lambda, float L, int
                const float *x0_dev, float *x_out_dev, double *trace_dev,
                sl1m_solve_info *info_host, void *stream);
 
+/*
+ * sl1m_solve_tol -- sl1m_solve with the paper's termination rule ("terminated when
+ * an iteration leads to a sufficiently small change in the total error E, given by equation
+ * (10)"; section 4.1.1: "until the total error changes no more than 1 part in 10^6
+ * or until 7000 iterations were reached").  E is formed on the device from what the iteration
+ * already has: E_k = ||M y_k - V||^2 + 2 lambda sum I_k (eq (10) with lambda_paper = 2 lambda; the
+ * residual is that of y_k, because evaluating M I_k as well is what the paper declines to pay
+ * for).  After every `check_every`-th iteration k >= 2 the host reads the two
+ * newest trace rows (48 bytes) and stops iff |E_k - E_{k-1}| <= tol |E_k|; no other host
+ * round-trip happens inside the loop.  max_iter caps the count (the paper's 7000).
+ *   tol >= 0, check_every >= 1, info_host REQUIRED (n_iter_done is how the caller learns k).
+ *   trace_dev DEV [max_iter][3] fp64 or NULL (then a plan-owned buffer is used).
+ */
+int sl1m_solve_tol(sl1m_plan *plan, const float *vis_dev, float lambda, float L, int n_pow,
+                   int max_iter, double tol, int check_every, const float *x0_dev,
+                   float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host, void *stream);
+
+/*
+ * sl1m_dirty_image -- img = max(0, scale * Re M^H V): "use the dirty image as the initial
+ * condition", clipped to the positive orthant the solver lives in.  scale is the
+ * caller's normalisation (1/n_vis gives unit point-source response for delta pixels near the
+ * phase centre).  vis DEV [n_vis][2], img DEV [n_pix]; asynchronous on stream.  Pass the result
+ * as x0_dev to sl1m_solve / sl1m_solve_tol.
+ */
+int sl1m_dirty_image(sl1m_plan *plan, const float *vis_dev, float scale, float *img_dev, void *stream);
+
 /* sl1m_solve with HOST vis / x0 / x_out (trace not available); always synchronises. */
 int sl1m_solve_host(sl1m_plan *plan, const float *vis_host, float lambda, float L, int n_pow,
                     int n_iter, const float *x0_host, float *x_out_host,

@@ -79,6 +79,9 @@ def load_library():
                                ctypes.POINTER(_SolveInfo), vp]
     lib.sl1m_solve_host.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, vp, vp,
                                     ctypes.POINTER(_SolveInfo), vp]
+    lib.sl1m_solve_tol.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int,
+                                   vp, vp, vp, ctypes.POINTER(_SolveInfo), vp]
+    lib.sl1m_dirty_image.argtypes = [vp, vp, f32, vp, vp]
     lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
     lib.sl1m_launch_count.argtypes = [vp]
     lib.sl1m_launch_count.restype = i64
@@ -223,6 +226,33 @@ class Plan:
             ctypes.byref(info) if want_info else None, _stream_ptr(stream)))
         res = SolveInfo(info.n_iter_done, info.L_used, info.l2_term, info.l1_term, info.nnz) if want_info else None
         return out, res
+
+    def solve_tol(self, vis, lam: float, L: float, max_iter: int, tol: float, check_every: int = 1,
+                  n_pow: int = 30, x0=None, out=None, trace=None, stream=None):
+        """sl1m_solve_tol: FISTA until the total error changes by <= tol (relative) or max_iter.
+        Returns (x, SolveInfo); SolveInfo.n_iter_done is the iteration it stopped at."""
+        import torch
+        if out is None:
+            out = torch.empty(self.n_pix, dtype=torch.float32, device=vis.device)
+        info = _SolveInfo()
+        _check(load_library().sl1m_solve_tol(
+            self._h, _dev_ptr(vis, torch.complex64, self.n_vis, "vis"), float(lam), float(L), int(n_pow),
+            int(max_iter), float(tol), int(check_every), _dev_ptr(x0, torch.float32, self.n_pix, "x0"),
+            _dev_ptr(out, torch.float32, self.n_pix, "out"),
+            _dev_ptr(trace, torch.float64, 3 * max(int(max_iter), 0), "trace") if trace is not None else None,
+            ctypes.byref(info), _stream_ptr(stream)))
+        return out, SolveInfo(info.n_iter_done, info.L_used, info.l2_term, info.l1_term, info.nnz)
+
+    def dirty_image(self, vis, scale: float = None, out=None, stream=None):
+        """sl1m_dirty_image: max(0, scale * Re M^H vis); scale defaults to 1/n_vis."""
+        import torch
+        if out is None:
+            out = torch.empty(self.n_pix, dtype=torch.float32, device=vis.device)
+        _check(load_library().sl1m_dirty_image(
+            self._h, _dev_ptr(vis, torch.complex64, self.n_vis, "vis"),
+            float(1.0 / self.n_vis if scale is None else scale),
+            _dev_ptr(out, torch.float32, self.n_pix, "out"), _stream_ptr(stream)))
+        return out
 
     # ---- host-buffer calls (numpy / pinned torch CPU tensors) ----
     @staticmethod

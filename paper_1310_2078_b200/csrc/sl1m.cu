@@ -67,6 +67,8 @@ struct sl1m_plan {
     double *scalars = nullptr;   // [4] device scalars (norm2, l2, l1, nnz)
     // host-buffer variants
     float *h_x = nullptr, *h_vis = nullptr, *h_img = nullptr;   // device staging for *_host calls
+    double *trace_buf = nullptr;  // plan-owned trace for sl1m_solve_tol when the caller passes none
+    int trace_cap = 0;
     int64_t launches = 0;
     int device = 0;
 };
@@ -77,7 +79,8 @@ void free_plan(sl1m_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
-                    p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img};
+                    p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
+                    p->trace_buf};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -559,15 +562,27 @@ extern "C" int sl1m_max_eig(sl1m_plan *p, int n_pow, float *L_out_host, void *st
 // ------------------------------------------------------------------------------------------
 // a3-a6: FISTA, listing PAPER.md:188-192; no host round-trip per iteration
 // ------------------------------------------------------------------------------------------
-extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int n_iter,
-                          const float *x0_dev, float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host,
-                          void *stream) {
+namespace {
+// Shared body of sl1m_solve (tol < 0: fixed iteration count) and sl1m_solve_tol.
+int solve_impl(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int n_iter, double tol,
+               int check_every, const float *x0_dev, float *x_out_dev, double *trace_dev,
+               sl1m_solve_info *info_host, void *stream) {
     if (!p || !vis_dev || !x_out_dev) return fail(SL1M_ERR_NULL, "sl1m_solve: NULL argument");
     if (!(lambda >= 0.f) || n_iter < 0) return fail(SL1M_ERR_PARAM, "lambda < 0 or n_iter < 0");
     if (!(L > 0.f) && n_pow < 1) return fail(SL1M_ERR_PARAM, "L <= 0 needs n_pow >= 1");
     cudaStream_t s = (cudaStream_t)stream;
     const int npad = p->n_pix_pad;
     int st;
+    if (tol >= 0.0 && !trace_dev) {   // the stopping rule reads the trace: use the plan's own buffer
+        if (p->trace_cap < n_iter) {
+            if (p->trace_buf) cudaFree(p->trace_buf);
+            p->trace_buf = nullptr;
+            p->trace_cap = 0;
+            CUDA_TRY(cudaMalloc((void **)&p->trace_buf, (size_t)std::max(n_iter, 1) * 3 * sizeof(double)));
+            p->trace_cap = n_iter;
+        }
+        trace_dev = p->trace_buf;
+    }
     if (!(L > 0.f)) {
         if ((st = sl1m_max_eig(p, n_pow, &L, stream))) return st;
         if (!(L > 0.f)) return fail(SL1M_ERR_PARAM, "power iteration returned L <= 0 (zero operator)");
@@ -587,6 +602,7 @@ extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, floa
     p->launches++;
 
     double t = 1.0;
+    int n_done = 0;
     for (int k = 0; k < n_iter; ++k) {
         const double t_next = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
         const float beta = (float)((t - 1.0) / t_next);
@@ -607,6 +623,17 @@ extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, floa
                                                  trace_dev + 3 * (size_t)k + 2);
             p->launches++;
         }
+        n_done = k + 1;
+        // termination rule (reading R21), looked at every check_every
+        // iterations: the only host round-trip of the loop, 48 bytes.
+        if (tol >= 0.0 && n_done >= 2 && check_every >= 1 && n_done % check_every == 0) {
+            double h[6];
+            CUDA_TRY(cudaMemcpyAsync(h, trace_dev + 3 * (size_t)(n_done - 2), sizeof(h), cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(cudaStreamSynchronize(s));
+            const double E_before = h[0] + 2.0 * (double)lambda * h[1];
+            const double E_now = h[3] + 2.0 * (double)lambda * h[4];
+            if (std::fabs(E_now - E_before) <= tol * std::fabs(E_now)) break;
+        }
     }
     scatter_kernel<<<egrid(npad), ET, 0, s>>>(p->I_sorted, p->perm, x_out_dev, npad);
     p->launches++;
@@ -626,13 +653,39 @@ extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, floa
         double h[4];
         CUDA_TRY(cudaMemcpyAsync(h, p->scalars, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
         CUDA_TRY(cudaStreamSynchronize(s));
-        info_host->n_iter_done = n_iter;
+        info_host->n_iter_done = n_done;
         info_host->L_used = L;
         info_host->l2_term = h[1];
         info_host->l1_term = h[2];
         info_host->nnz = (int64_t)(h[3] + 0.5);
     }
     return SL1M_OK;
+}
+}  // namespace
+
+extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int n_iter,
+                          const float *x0_dev, float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host,
+                          void *stream) {
+    return solve_impl(p, vis_dev, lambda, L, n_pow, n_iter, -1.0, 1, x0_dev, x_out_dev, trace_dev, info_host, stream);
+}
+
+extern "C" int sl1m_solve_tol(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int max_iter,
+                              double tol, int check_every, const float *x0_dev, float *x_out_dev,
+                              double *trace_dev, sl1m_solve_info *info_host, void *stream) {
+    if (!(tol >= 0.0) || check_every < 1) return fail(SL1M_ERR_PARAM, "sl1m_solve_tol: tol < 0 or check_every < 1");
+    if (!info_host) return fail(SL1M_ERR_NULL, "sl1m_solve_tol: info_host is required (it carries n_iter_done)");
+    return solve_impl(p, vis_dev, lambda, L, n_pow, max_iter, tol, check_every, x0_dev, x_out_dev, trace_dev,
+                      info_host, stream);
+}
+
+extern "C" int sl1m_dirty_image(sl1m_plan *p, const float *vis_dev, float scale, float *img_dev, void *stream) {
+    if (!p || !vis_dev || !img_dev) return fail(SL1M_ERR_NULL, "sl1m_dirty_image: NULL argument");
+    if (!std::isfinite(scale)) return fail(SL1M_ERR_PARAM, "sl1m_dirty_image: non-finite scale");
+    int st = sl1m_adjoint(p, vis_dev, img_dev, stream);
+    if (st) return st;
+    scale_clip_kernel<<<egrid((size_t)p->n_pix), ET, 0, (cudaStream_t)stream>>>(img_dev, scale, (int)p->n_pix);
+    p->launches++;
+    return check_launch("sl1m_dirty_image");
 }
 
 extern "C" int sl1m_solve_host(sl1m_plan *p, const float *vis_host, float lambda, float L, int n_pow, int n_iter,

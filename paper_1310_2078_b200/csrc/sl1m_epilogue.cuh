@@ -216,4 +216,10 @@ __global__ void __launch_bounds__(ET) l1_nnz_kernel(const float *I_sorted, int n
     }
 }
 
+// Dirty image as a starting point (reading R22): img = max(0, scale * img).
+__global__ void __launch_bounds__(ET) scale_clip_kernel(float *img, float scale, int n) {
+    const int k = blockIdx.x * ET + threadIdx.x;
+    if (k < n) img[k] = fmaxf(0.f, scale * img[k]);
+}
+
 }  // namespace sl1m

@@ -283,3 +283,63 @@ def test_config5_solver_reduced(sl):
     err = rel_l2(x.cpu().numpy(), ref["x"])
     assert err <= TOL_IMAGE, err
     plan.close()
+
+
+# ----------------------------------------------------------------------------- NEXT-1: stopping rule, dirty image
+def test_tolerance_stop_matches_oracle(sl):
+    """sl1m_solve_tol against oracle.fista_tol on config 1 (reading R21).
+    The decision |E_k - E_{k-1}| <= tol |E_k| is taken in fp64 on both sides from fp32-computed
+    (GPU) or fp64-computed (oracle) E, so near the threshold the stop may move by a look or two:
+    the image is compared at the GPU's own stopping index, the index within 3 looks."""
+    import torch
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = fista_lambda(wl)
+    plan = sl.Plan.from_workload(wl)
+    Vd = _dev(V, torch.complex64)
+    for tol, every in ((1e-3, 1), (1e-5, 5), (1e-7, 10)):
+        ref = o.fista_tol(V, lam, L, max_iter=600, tol=tol, check_every=every)
+        x, info = plan.solve_tol(Vd, lam, L, max_iter=600, tol=tol, check_every=every)
+        k = info.n_iter_done
+        assert 2 <= k <= 600 and (k % every == 0 or k == 600)
+        assert abs(k - ref["n_iter_done"]) <= 3 * every, (tol, every, k, ref["n_iter_done"])
+        same_k = o.fista(V, lam, L, k)
+        assert rel_l2(x.cpu().numpy(), same_k["x"]) <= TOL_IMAGE
+        assert abs(info.l2_term - same_k["l2_term"]) <= 2e-3 * same_k["l2_term"]
+    # the cap: tol = 0 can only be met by an exactly stationary E; a caller-supplied trace is filled
+    trace = torch.zeros(3 * 7, dtype=torch.float64, device="cuda")
+    x, info = plan.solve_tol(Vd, lam, L, max_iter=7, tol=0.0, check_every=1, trace=trace)
+    assert info.n_iter_done == 7
+    ref7 = o.fista(V, lam, L, 7, want_trace=True)
+    tr = trace.cpu().numpy().reshape(-1, 3)
+    assert np.max(np.abs(tr[:, 0] - ref7["trace"][:, 0]) / ref7["trace"][:, 0]) < 2e-3
+    # error paths
+    with pytest.raises(sl.Sl1mError):
+        plan.solve_tol(Vd, lam, L, max_iter=5, tol=-1.0)
+    with pytest.raises(sl.Sl1mError):
+        plan.solve_tol(Vd, lam, L, max_iter=5, tol=1e-3, check_every=0)
+    plan.close()
+
+
+def test_dirty_image_start_matches_oracle(sl):
+    """sl1m_dirty_image (reading R22) and a solve started from it."""
+    import torch
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = fista_lambda(wl)
+    plan = sl.Plan.from_workload(wl)
+    Vd = _dev(V, torch.complex64)
+    d = plan.dirty_image(Vd)
+    d_ref = o.dirty_image(V, 1.0 / wl.n_vis)
+    assert rel_l2(d.cpu().numpy(), d_ref) <= TOL_APPLY
+    assert float(d.min()) >= 0.0 and np.count_nonzero(d_ref) > 10
+    d2 = plan.dirty_image(Vd, scale=2.5 / wl.n_vis)
+    assert rel_l2(d2.cpu().numpy(), 2.5 * d_ref) <= TOL_APPLY
+    x, _ = plan.solve(Vd, lam, L=L, n_iter=50, x0=d)
+    ref = o.fista(V, lam, L, 50, x0=d_ref)
+    assert rel_l2(x.cpu().numpy(), ref["x"]) <= TOL_IMAGE
+    plan.close()
