@@ -154,6 +154,26 @@ def run_reference(args, rank: int):
     print(json.dumps(line), flush=True)
 
 
+def reduce_over_ranks(total_ms: float, e2e_ms: float, launches: int, world: int, device):
+    """Replicas only: every rank ran the same workload on its own GPU, with no
+    data-path collective.  The job's time is the MAX over ranks (device-timed), its launch count the
+    SUM.  `device` is the rank's CUDA device under NCCL, or "cpu" under gloo (the CPU tests)."""
+    if world <= 1:
+        return total_ms, e2e_ms, launches
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([total_ms, e2e_ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ln = torch.tensor([launches], device=device, dtype=torch.int64)
+    dist.all_reduce(ln, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), int(ln[0])
+
+
+def aggregate_value(world: int, terms_per_step: float, steps: int, t_max_ms: float) -> float:
+    """Whole-job throughput: the terms ALL ranks processed / the max-over-ranks time."""
+    return world * terms_per_step * steps / (t_max_ms * 1e-3)
+
+
 def run_ours(args, rank: int, world: int, local_rank: int):
     import torch
     import torch.distributed as dist
@@ -260,22 +280,15 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     d2h = 4 * wl.n_pix
 
     # ---------------- reduce over ranks (replicas) ----------------
-    t_max = total_ms
     e2e_mean = sum(e2e_ms) / len(e2e_ms)
-    if world > 1:
-        t = torch.tensor([total_ms, e2e_mean], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_max, e2e_mean = float(t[0]), float(t[1])
-        ln = torch.tensor([launches], device=dev, dtype=torch.int64)
-        dist.all_reduce(ln)
-        launches = int(ln[0])
+    t_max, e2e_mean, launches = reduce_over_ranks(total_ms, e2e_mean, launches, world, dev)
     if rank != 0:
         plan.close()
         return
 
     terms_per_step = 2.0 * n_terms                 # one A and one A^H
-    value = world * terms_per_step * args.steps / (t_max * 1e-3)
-    e2e_value = world * terms_per_step / (e2e_mean * 1e-3)
+    value = aggregate_value(world, terms_per_step, args.steps, t_max)
+    e2e_value = aggregate_value(world, terms_per_step, 1, e2e_mean)
     f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     desc = plan.describe()
     fwd_ms, adj_ms = statistics.median(t_fwd), statistics.median(t_adj)
