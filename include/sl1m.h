@@ -153,6 +153,56 @@ int sl1m_solve_tol(sl1m_plan *plan, const float *vis_dev, float lambda, float L,
  */
 int sl1m_dirty_image(sl1m_plan *plan, const float *vis_dev, float scale, float *img_dev, void *stream);
 
+/*
+ * Coarse-to-fine / adaptive quadtree acceleration (section 4.5, Fig. 10: "the
+ * system is solved at a low resolution, and pixels where emission is detected are then
+ * subdivided ... refinement of all pixels greater than 1 per cent of the maximum"; a 13x speed-up
+ * in the paper).  What the paper leaves open is fixed by DESIGN.md reading R23:
+ *  - a pixel is a square of side s_k centred on (l_k, m_k); it splits iff I_k > frac * max_j I_j
+ *    and s_k/2 >= min_side, and is replaced IN PLACE by four children of side s_k/2 centred on
+ *    l_k -/+ s_k/4, m_k -/+ s_k/4 (l fastest); every other pixel stays (mixed sizes in one
+ *    solve).  frac < 0 splits every pixel: the plain coarse-to-fine strategy.
+ *  - "upscale the previously calculated solution": a child starts from I_k/4.
+ *
+ * sl1m_quadtree_refine -- ONE split step, pure host code (needs no GPU).  All pointers HOST.
+ *   in:  n pixels (l, m, side fp64; I fp32, e.g. the image a solve returned)
+ *   out: l_out, m_out, side_out, I0_out [capacity >= n + 3 * (number split)], parent_out
+ *        (nullable: index of the input pixel each output pixel came from), *n_out, *n_refined.
+ *   SL1M_ERR_SIZE if capacity is too small (nothing written).
+ */
+int sl1m_quadtree_refine(int64_t n, const double *l, const double *m, const double *side,
+                         const float *I, double frac, double min_side, int64_t capacity,
+                         double *l_out, double *m_out, double *side_out, float *I0_out,
+                         int64_t *parent_out, int64_t *n_out, int64_t *n_refined);
+
+typedef struct {
+    int64_t n_pix;       /* pixels solved at this level                          */
+    float L;             /* step constant used (power iteration x L_safety)      */
+    int32_t n_iter_done; /* FISTA iterations until the stopping rule / the cap   */
+    double l2_term, l1_term;
+    int64_t nnz;
+    double seconds;      /* wall time of the level: plan + L + solve + read-back */
+} sl1m_qt_level;
+
+/*
+ * sl1m_quadtree_solve -- the driver: at most n_levels times { plan the current pixel list,
+ * L = L_safety * sl1m_max_eig(n_pow), sl1m_solve_tol(lambda, max_iter, tol, check_every) warm-
+ * started from the upscaled previous level, split }.  Stops early when no pixel splits.
+ * Pixels that can still split are Gaussian pixels of sigma_k = sigma_factor * s_k (eq 16/17 by
+ * gauss_model), pixels at the resolution limit (s_k/2 < min_side) and all pixels when
+ * sigma_factor == 0 are delta pixels (eq 9).  Unit gains.
+ *   uvw HOST [n_vis][3] fp64; vis_host HOST [n_vis][2] fp32; l0, m0, side0 HOST [n0] fp64.
+ *   outputs HOST [capacity]: final leaves (l, m, side) and their fluxes x; *n_out leaves.
+ *   levels_out HOST [n_levels] or NULL; *n_levels_done.  Synchronises `stream` at every level.
+ */
+int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float *vis_host, int64_t n0,
+                        const double *l0, const double *m0, const double *side0, int n_levels,
+                        double frac, double min_side, double sigma_factor, int gauss_model,
+                        float lambda, float L_safety, int n_pow, int max_iter, double tol,
+                        int check_every, int64_t capacity, double *l_out, double *m_out,
+                        double *side_out, float *x_out, int64_t *n_out, sl1m_qt_level *levels_out,
+                        int *n_levels_done, void *stream);
+
 /* sl1m_solve with HOST vis / x0 / x_out (trace not available); always synchronises. */
 int sl1m_solve_host(sl1m_plan *plan, const float *vis_host, float lambda, float L, int n_pow,
                     int n_iter, const float *x0_host, float *x_out_host,

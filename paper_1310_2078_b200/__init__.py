@@ -8,5 +8,5 @@ raises.
 """
 from .binding import (  # noqa: F401
     GAUSS_PARAXIAL, GAUSS_WIDEFIELD, Plan, Sl1mError, SolveInfo, build_library, library_path,
-    load_library, exported_symbols,
+    load_library, exported_symbols, quadtree_refine, quadtree_solve,
 )

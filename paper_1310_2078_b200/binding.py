@@ -32,6 +32,12 @@ class _PlanInfo(ctypes.Structure):
         "adj_packed_pairs")] + [("reserved", ctypes.c_int32 * 3)]
 
 
+class _QtLevel(ctypes.Structure):
+    _fields_ = [("n_pix", ctypes.c_int64), ("L", ctypes.c_float), ("n_iter_done", ctypes.c_int32),
+                ("l2_term", ctypes.c_double), ("l1_term", ctypes.c_double), ("nnz", ctypes.c_int64),
+                ("seconds", ctypes.c_double)]
+
+
 class _SolveInfo(ctypes.Structure):
     _fields_ = [("n_iter_done", ctypes.c_int32), ("L_used", ctypes.c_float),
                 ("l2_term", ctypes.c_double), ("l1_term", ctypes.c_double), ("nnz", ctypes.c_int64)]
@@ -82,6 +88,13 @@ def load_library():
     lib.sl1m_solve_tol.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int,
                                    vp, vp, vp, ctypes.POINTER(_SolveInfo), vp]
     lib.sl1m_dirty_image.argtypes = [vp, vp, f32, vp, vp]
+    f64 = ctypes.c_double
+    lib.sl1m_quadtree_refine.argtypes = [i64, vp, vp, vp, vp, f64, f64, i64, vp, vp, vp, vp, vp,
+                                         ctypes.POINTER(i64), ctypes.POINTER(i64)]
+    lib.sl1m_quadtree_solve.argtypes = [i64, vp, vp, i64, vp, vp, vp, ctypes.c_int, f64, f64, f64, ctypes.c_int,
+                                        f32, f32, ctypes.c_int, ctypes.c_int, f64, ctypes.c_int, i64, vp, vp, vp,
+                                        vp, ctypes.POINTER(i64), ctypes.POINTER(_QtLevel),
+                                        ctypes.POINTER(ctypes.c_int), vp]
     lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
     lib.sl1m_launch_count.argtypes = [vp]
     lib.sl1m_launch_count.restype = i64
@@ -123,6 +136,47 @@ def _dev_ptr(t, dtype, numel: int, name: str):
             and t.numel() == numel):
         raise ValueError(f"{name}: need a contiguous CUDA tensor of {dtype} with {numel} elements")
     return ctypes.c_void_p(t.data_ptr())
+
+
+def quadtree_refine(l, m, side, I, frac: float, min_side: float):
+    """sl1m_quadtree_refine (pure host code).  Returns (l, m, side, I0, parent, n_refined)."""
+    l, m, side = (np.ascontiguousarray(a, dtype=np.float64) for a in (l, m, side))
+    I = np.ascontiguousarray(I, dtype=np.float32)
+    n = int(l.shape[0])
+    cap = 4 * n
+    lo, mo, so = np.empty(cap), np.empty(cap), np.empty(cap)
+    xo, po = np.empty(cap, np.float32), np.empty(cap, np.int64)
+    n_out, n_ref = ctypes.c_int64(0), ctypes.c_int64(0)
+    _check(load_library().sl1m_quadtree_refine(n, _np_ptr(l), _np_ptr(m), _np_ptr(side), _np_ptr(I), float(frac),
+                                               float(min_side), cap, _np_ptr(lo), _np_ptr(mo), _np_ptr(so),
+                                               _np_ptr(xo), _np_ptr(po), ctypes.byref(n_out), ctypes.byref(n_ref)))
+    k = n_out.value
+    return lo[:k].copy(), mo[:k].copy(), so[:k].copy(), xo[:k].copy(), po[:k].copy(), int(n_ref.value)
+
+
+def quadtree_solve(uvw, vis, l0, m0, side0, n_levels: int, frac: float, min_side: float, lam: float,
+                   n_pow: int = 30, L_safety: float = 1.05, max_iter: int = 1000, tol: float = 1e-6,
+                   check_every: int = 10, sigma_factor: float = 1.0, gauss_model: int = 1, capacity: int = None,
+                   stream=None):
+    """sl1m_quadtree_solve: coarse-to-fine / adaptive quadtree driver.
+    Host arrays in, host arrays out: dict(l, m, side, x, levels=[...])."""
+    uvw = np.ascontiguousarray(uvw, dtype=np.float64)
+    vis = np.ascontiguousarray(vis, dtype=np.complex64)
+    l0, m0, side0 = (np.ascontiguousarray(a, dtype=np.float64) for a in (l0, m0, side0))
+    n0 = int(l0.shape[0])
+    cap = int(capacity) if capacity is not None else n0 * 4 ** max(int(n_levels) - 1, 0)
+    lo, mo, so, xo = np.empty(cap), np.empty(cap), np.empty(cap), np.empty(cap, np.float32)
+    levels = (_QtLevel * max(int(n_levels), 1))()
+    n_out, n_done = ctypes.c_int64(0), ctypes.c_int(0)
+    _check(load_library().sl1m_quadtree_solve(
+        int(uvw.shape[0]), _np_ptr(uvw), _np_ptr(vis), n0, _np_ptr(l0), _np_ptr(m0), _np_ptr(side0), int(n_levels),
+        float(frac), float(min_side), float(sigma_factor), int(gauss_model), float(lam), float(L_safety), int(n_pow),
+        int(max_iter), float(tol), int(check_every), cap, _np_ptr(lo), _np_ptr(mo), _np_ptr(so), _np_ptr(xo),
+        ctypes.byref(n_out), levels, ctypes.byref(n_done), _stream_ptr(stream)))
+    k = n_out.value
+    lv = [dict(n_pix=int(q.n_pix), L=float(q.L), n_iter_done=int(q.n_iter_done), l2_term=float(q.l2_term),
+               l1_term=float(q.l1_term), nnz=int(q.nnz), seconds=float(q.seconds)) for q in levels[:n_done.value]]
+    return dict(l=lo[:k].copy(), m=mo[:k].copy(), side=so[:k].copy(), x=xo[:k].copy(), levels=lv)
 
 
 class Plan:

@@ -6,7 +6,8 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "sl1m.cu")
-DEPS = [SRC, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"),
+SRC_QT = os.path.join(_HERE, "csrc", "sl1m_quadtree.cu")
+DEPS = [SRC, SRC_QT, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"),
         os.path.join(os.path.dirname(_HERE), "include", "sl1m.h")]
 LIB = os.path.join(_HERE, "libsl1m.so")
 
@@ -25,7 +26,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     stale = not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(d) for d in DEPS)
     if force or stale:
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [_nvcc(), *NVCC_FLAGS, "-o", tmp, SRC]
+        cmd = [_nvcc(), *NVCC_FLAGS, "-o", tmp, SRC, SRC_QT]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)

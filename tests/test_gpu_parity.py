@@ -343,3 +343,70 @@ def test_dirty_image_start_matches_oracle(sl):
     ref = o.fista(V, lam, L, 50, x0=d_ref)
     assert rel_l2(x.cpu().numpy(), ref["x"]) <= TOL_IMAGE
     plan.close()
+
+
+# ----------------------------------------------------------------------------- NEXT-3: quadtree driver
+def _toy_quadtree_problem():
+    rng = np.random.default_rng(77)
+    Nf, field = 64, 0.05
+    df = field / Nf
+
+    def grid(N, d):
+        k = np.arange(N * N)
+        return (k % N - N / 2 + 0.5) * d, (k // N - N / 2 + 0.5) * d
+    ant = rng.uniform(-1, 1, (200, 2))
+    ant = ant[(ant ** 2).sum(1) <= 1][:16] * 500.0 / 1.99862
+    p, q = np.triu_indices(16, 1)
+    base = ant[p] - ant[q]
+    uv = np.concatenate([base @ np.array([[np.cos(t), -np.sin(t)], [np.sin(t), np.cos(t)]]).T
+                         for t in np.linspace(0, np.pi, 6, endpoint=False)])
+    uvw = np.concatenate([uv, 40.0 * rng.uniform(-1, 1, (uv.shape[0], 1))], 1)
+    lf, mf = grid(Nf, df)
+    src = rng.choice(np.flatnonzero((np.abs(lf) < 0.4 * field) & (np.abs(mf) < 0.4 * field)), 6, replace=False)
+    x_true = np.zeros(Nf * Nf)
+    x_true[src] = rng.uniform(1.0, 3.0, 6)
+    V = oracle.Oracle(uvw, lf, mf).forward(x_true).astype(np.complex64)
+    l0, m0 = grid(8, field / 8)
+    return uvw, V, l0, m0, np.full(64, field / 8), df, lf, mf, src, x_true
+
+
+def test_quadtree_driver_matches_oracle(sl):
+    """sl1m_quadtree_solve against oracle.quadtree_solve (reading R23) with a fixed
+    iteration count per level (tol = 0), so both sides walk the same path.  The split decision
+    I_k > frac max I is taken on the fp32 image on the GPU side and on the fp64 image in the oracle: a
+    leaf within rounding of the threshold may differ, so the leaf sets are compared up to 2 %, and every
+    leaf that matters (flux above 5 % of the maximum) must be common; fluxes are compared on common leaves."""
+    uvw, V, l0, m0, side0, df, lf, mf, src, x_true = _toy_quadtree_problem()
+    lam = 0.02 * float(np.abs(oracle.Oracle(uvw, l0, m0).adjoint(V)).max())
+    kw = dict(n_levels=4, frac=0.01, min_side=df * 0.999, lam=lam, n_pow=30, L_safety=1.05, max_iter=150, tol=0.0,
+              check_every=50, sigma_factor=1.0)
+    ref = oracle.quadtree_solve(uvw, V, l0, m0, side0, **kw)
+    got = sl.quadtree_solve(uvw, V, l0, m0, side0, **kw)
+    assert len(got["levels"]) == len(ref["levels"]) == 4
+    for a, b in zip(got["levels"], ref["levels"]):
+        assert abs(a["n_pix"] - b["n_pix"]) <= 0.02 * b["n_pix"] + 3
+        assert a["n_iter_done"] == b["n_iter_done"] == 150
+        assert abs(a["L"] - b["L"]) <= 1e-3 * b["L"]
+
+    def keyed(r):
+        q = df / 4
+        return {(int(round(a / q)), int(round(b / q)), int(round(c / q))): float(x)
+                for a, b, c, x in zip(r["l"], r["m"], r["side"], r["x"])}
+    kg, kr = keyed(got), keyed(ref)
+    common = sorted(set(kg) & set(kr))
+    assert len(set(kg) ^ set(kr)) <= 0.02 * len(kr) + 3
+    top = max(kr.values())
+    assert all(k in kg for k, v in kr.items() if v > 0.05 * top)
+    xg, xr = np.array([kg[k] for k in common]), np.array([kr[k] for k in common])
+    assert rel_l2(xg, xr) <= 5 * TOL_IMAGE, rel_l2(xg, xr)
+    # and it found the sky: every true source sits in a finest-level leaf with its flux
+    for s in src:
+        k = (int(round(lf[s] / (df / 4))), int(round(mf[s] / (df / 4))), 4)
+        assert k in kg and abs(kg[k] - x_true[s]) < 0.05 * x_true[s]
+    assert got["l"].shape[0] < 0.25 * 64 * 64
+    # frac < 0: plain coarse-to-fine, every level is the full regular grid
+    c2f = sl.quadtree_solve(uvw, V, l0, m0, side0, n_levels=3, frac=-1.0, min_side=0.0, lam=lam, max_iter=30, tol=0.0,
+                            check_every=10, sigma_factor=0.0)
+    assert [lv["n_pix"] for lv in c2f["levels"]] == [64, 256, 1024]
+    with pytest.raises(sl.Sl1mError):
+        sl.quadtree_solve(uvw, V, l0, m0, side0, n_levels=3, frac=-1.0, min_side=0.0, lam=lam, capacity=100)

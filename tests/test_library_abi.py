@@ -87,3 +87,37 @@ def test_sass_has_tma_bulk_copy_and_mufu():
     sass = subprocess.run([cuobjdump, "-sass", sl.library_path()], capture_output=True, text=True).stdout
     assert "UBLKCP" in sass and "MUFU.SIN" in sass and "MUFU.COS" in sass and "MUFU.EX2" in sass
     assert "sm_100a" in sass
+
+
+def test_quadtree_refine_host_logic_is_bit_exact_against_the_oracle():
+    """sl1m_quadtree_refine is pure host code (no GPU needed): on the same fp32 image it must take
+    exactly the oracle's decisions (reading R23) -- same leaves, same order, same start values."""
+    import numpy as np
+    import oracle
+    rng = np.random.default_rng(3)
+    N, d = 12, 0.004
+    k = np.arange(N * N)
+    l, m, side = (k % N - N / 2 + 0.5) * d, (k // N - N / 2 + 0.5) * d, np.full(N * N, d)
+    I = np.where(rng.uniform(size=N * N) < 0.3, rng.pareto(1.5, N * N), 0.0).astype(np.float32)
+    for frac, min_side in ((0.01, 0.0), (0.2, d / 4), (-1.0, 0.0), (0.05, d)):
+        for _ in range(3):
+            got = sl.quadtree_refine(l, m, side, I, frac, min_side)
+            want = oracle.quadtree_refine(l, m, side, I.astype(np.float64), frac, min_side)
+            assert got[5] == want[5]
+            for a, b in zip(got[:3], want[:3]):
+                assert np.array_equal(a, b)
+            assert np.array_equal(got[3].astype(np.float64), want[3]) and np.array_equal(got[4], want[4])
+            l, m, side = got[0], got[1], got[2]
+            I = (got[3] * rng.uniform(0.2, 1.5, got[3].shape[0])).astype(np.float32)
+        l, m, side = (k % N - N / 2 + 0.5) * d, (k // N - N / 2 + 0.5) * d, np.full(N * N, d)
+        I = np.where(rng.uniform(size=N * N) < 0.3, rng.pareto(1.5, N * N), 0.0).astype(np.float32)
+    # capacity too small: refused, nothing else
+    lib = sl.load_library()
+    import ctypes
+    out = np.empty(4), np.empty(4), np.empty(4), np.empty(4, np.float32)
+    n_out, n_ref = ctypes.c_int64(), ctypes.c_int64()
+    four = np.array([-1.0, 1.0, -1.0, 1.0]), np.array([-1.0, -1.0, 1.0, 1.0]), np.full(4, 2.0), np.ones(4, np.float32)
+    st = lib.sl1m_quadtree_refine(4, *(a.ctypes.data_as(ctypes.c_void_p) for a in four), 0.5, 0.0, 4,
+                                  *(a.ctypes.data_as(ctypes.c_void_p) for a in out), None, ctypes.byref(n_out),
+                                  ctypes.byref(n_ref))
+    assert st == 2  # SL1M_ERR_SIZE
