@@ -203,6 +203,33 @@ int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float *vis_host,
                         double *side_out, float *x_out, int64_t *n_out, sl1m_qt_level *levels_out,
                         int *n_levels_done, void *stream);
 
+/*
+ * Batched channels (NEXT-4 of the scope table).  The paper's data sets are 61-127 spectral channels
+ * (and two polarisations) of ONE observing geometry, each deconvolved independently
+ * (PAPER.md:68, 279, 307); the baselines in wavelengths scale with frequency (PAPER.md:61,
+ * "b = lambda (u, v, w)").  sl1m_plan_set_channels turns a plan into a batch of n_chan
+ * independent problems that share the pixel list, the gain table and the baseline geometry:
+ * channel c uses uvw * scale[c] (scale[c] = nu_c / nu_0, HOST [n_chan], > 0).  Afterwards
+ *   sl1m_forward   takes x  DEV [n_chan][n_pix]     and writes vis DEV [n_chan][n_vis][2],
+ *   sl1m_adjoint   takes r  DEV [n_chan][n_vis][2]  and writes img DEV [n_chan][n_pix],
+ * in ONE launch per step (grid z = channel), which is what fills the GPU when one channel's
+ * problem is small; sl1m_max_eig_batch / sl1m_solve_batch are the per-channel versions of
+ * sl1m_max_eig / sl1m_solve:
+ *   L_out_host, lambda_host, L_host, info_host   HOST [n_chan]   (L_host[c] <= 0 => power iteration)
+ *   vis_dev DEV [n_chan][n_vis][2]; x0_dev (nullable), x_out_dev DEV [n_chan][n_pix];
+ *   trace_dev DEV [n_chan][max(n_iter,1)][3] or NULL.
+ * Channels never interact: every result equals the single-channel call on uvw * scale[c].
+ * The single-problem calls (sl1m_max_eig, sl1m_solve, sl1m_solve_tol, sl1m_dirty_image, *_host)
+ * return SL1M_ERR_PARAM on a plan with more than one channel.  Re-allocates the plan's
+ * workspaces; synchronises the device.
+ */
+int sl1m_plan_set_channels(sl1m_plan *plan, int32_t n_chan, const double *scale_host);
+int32_t sl1m_plan_n_chan(const sl1m_plan *plan);
+int sl1m_max_eig_batch(sl1m_plan *plan, int n_pow, float *L_out_host, void *stream);
+int sl1m_solve_batch(sl1m_plan *plan, const float *vis_dev, const float *lambda_host,
+                     const float *L_host, int n_pow, int n_iter, const float *x0_dev,
+                     float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host, void *stream);
+
 /* sl1m_solve with HOST vis / x0 / x_out (trace not available); always synchronises. */
 int sl1m_solve_host(sl1m_plan *plan, const float *vis_host, float lambda, float L, int n_pow,
                     int n_iter, const float *x0_host, float *x_out_host,

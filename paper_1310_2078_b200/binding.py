@@ -88,6 +88,11 @@ def load_library():
     lib.sl1m_solve_tol.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int,
                                    vp, vp, vp, ctypes.POINTER(_SolveInfo), vp]
     lib.sl1m_dirty_image.argtypes = [vp, vp, f32, vp, vp]
+    lib.sl1m_plan_set_channels.argtypes = [vp, ctypes.c_int32, vp]
+    lib.sl1m_plan_n_chan.argtypes = [vp]
+    lib.sl1m_plan_n_chan.restype = ctypes.c_int32
+    lib.sl1m_max_eig_batch.argtypes = [vp, ctypes.c_int, vp, vp]
+    lib.sl1m_solve_batch.argtypes = [vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp]
     f64 = ctypes.c_double
     lib.sl1m_quadtree_refine.argtypes = [i64, vp, vp, vp, vp, f64, f64, i64, vp, vp, vp, vp, vp,
                                          ctypes.POINTER(i64), ctypes.POINTER(i64)]
@@ -222,6 +227,18 @@ class Plan:
                                     int(gauss_model), flags))
         self._h = h
         self.n_vis, self.n_pix = int(uvw.shape[0]), int(l.shape[0])
+        self.n_chan = 1
+
+    def set_channels(self, scale):
+        """sl1m_plan_set_channels: a batch of len(scale) channels, channel c on uvw * scale[c].
+        forward/adjoint then take and return [n_chan][.] tensors; use max_eig_batch / solve_batch."""
+        sc = np.ascontiguousarray(scale, dtype=np.float64).ravel()
+        _check(load_library().sl1m_plan_set_channels(self._h, int(sc.shape[0]), _np_ptr(sc)))
+        self.n_chan = int(load_library().sl1m_plan_n_chan(self._h))
+        return self
+
+    def _shape(self, n):
+        return (n,) if self.n_chan == 1 else (self.n_chan, n)
 
     @classmethod
     def from_workload(cls, wl, gains_device=None):
@@ -244,9 +261,9 @@ class Plan:
         """sl1m_forward: x float32 [n_pix] -> complex64 [n_vis]."""
         import torch
         if out is None:
-            out = torch.empty(self.n_vis, dtype=torch.complex64, device=x.device)
-        _check(load_library().sl1m_forward(self._h, _dev_ptr(x, torch.float32, self.n_pix, "x"),
-                                           _dev_ptr(out, torch.complex64, self.n_vis, "out"),
+            out = torch.empty(self._shape(self.n_vis), dtype=torch.complex64, device=x.device)
+        _check(load_library().sl1m_forward(self._h, _dev_ptr(x, torch.float32, self.n_chan * self.n_pix, "x"),
+                                           _dev_ptr(out, torch.complex64, self.n_chan * self.n_vis, "out"),
                                            _stream_ptr(stream)))
         return out
 
@@ -254,9 +271,9 @@ class Plan:
         """sl1m_adjoint: r complex64 [n_vis] -> float32 [n_pix]."""
         import torch
         if out is None:
-            out = torch.empty(self.n_pix, dtype=torch.float32, device=r.device)
-        _check(load_library().sl1m_adjoint(self._h, _dev_ptr(r, torch.complex64, self.n_vis, "r"),
-                                           _dev_ptr(out, torch.float32, self.n_pix, "out"),
+            out = torch.empty(self._shape(self.n_pix), dtype=torch.float32, device=r.device)
+        _check(load_library().sl1m_adjoint(self._h, _dev_ptr(r, torch.complex64, self.n_chan * self.n_vis, "r"),
+                                           _dev_ptr(out, torch.float32, self.n_chan * self.n_pix, "out"),
                                            _stream_ptr(stream)))
         return out
 
@@ -264,6 +281,32 @@ class Plan:
         L = ctypes.c_float(0.0)
         _check(load_library().sl1m_max_eig(self._h, int(n_pow), ctypes.byref(L), _stream_ptr(stream)))
         return float(L.value)
+
+    def max_eig_batch(self, n_pow: int = 30, stream=None) -> np.ndarray:
+        """sl1m_max_eig_batch: one L per channel."""
+        L = np.zeros(self.n_chan, np.float32)
+        _check(load_library().sl1m_max_eig_batch(self._h, int(n_pow), _np_ptr(L), _stream_ptr(stream)))
+        return L
+
+    def solve_batch(self, vis, lam, L, n_iter: int, n_pow: int = 30, x0=None, out=None, trace=None,
+                    want_info: bool = True, stream=None):
+        """sl1m_solve_batch: vis [n_chan][n_vis] complex64, lam / L per channel (scalars are broadcast).
+        Returns (x [n_chan][n_pix], [SolveInfo per channel] or None)."""
+        import torch
+        C = self.n_chan
+        lam_a = np.ascontiguousarray(np.broadcast_to(np.asarray(lam, np.float32), (C,)))
+        L_a = np.ascontiguousarray(np.broadcast_to(np.asarray(L, np.float32), (C,)))
+        if out is None:
+            out = torch.empty((C, self.n_pix), dtype=torch.float32, device=vis.device)
+        infos = (_SolveInfo * C)()
+        _check(load_library().sl1m_solve_batch(
+            self._h, _dev_ptr(vis, torch.complex64, C * self.n_vis, "vis"), _np_ptr(lam_a), _np_ptr(L_a), int(n_pow),
+            int(n_iter), _dev_ptr(x0, torch.float32, C * self.n_pix, "x0"),
+            _dev_ptr(out, torch.float32, C * self.n_pix, "out"),
+            _dev_ptr(trace, torch.float64, C * 3 * max(int(n_iter), 1), "trace") if trace is not None else None,
+            ctypes.cast(infos, ctypes.c_void_p) if want_info else None, _stream_ptr(stream)))
+        res = [SolveInfo(i.n_iter_done, i.L_used, i.l2_term, i.l1_term, i.nnz) for i in infos] if want_info else None
+        return out, res
 
     def solve(self, vis, lam: float, L: float = 0.0, n_pow: int = 30, n_iter: int = 100, x0=None,
               out=None, trace=None, want_info: bool = True, stream=None):

@@ -67,6 +67,9 @@ struct sl1m_plan {
     double *scalars = nullptr;   // [4] device scalars (norm2, l2, l1, nnz)
     // host-buffer variants
     float *h_x = nullptr, *h_vis = nullptr, *h_img = nullptr;   // device staging for *_host calls
+    int n_chan = 1;               // batched channels (NEXT-4): every per-image / per-visibility buffer is [n_chan][.]
+    double *chan_scale = nullptr; // DEV [n_chan] nu_c / nu_0, NULL while n_chan == 1
+    float2 *step_c = nullptr;     // DEV [n_chan] (1/L_c, lambda_c/L_c) for the batched solver
     double *trace_buf = nullptr;  // plan-owned trace for sl1m_solve_tol when the caller passes none
     int trace_cap = 0;
     int64_t launches = 0;
@@ -75,12 +78,18 @@ struct sl1m_plan {
 
 namespace {
 
+int single_channel_only(const sl1m_plan *p, const char *what) {
+    if (p && p->n_chan != 1)
+        return fail(SL1M_ERR_PARAM, std::string(what) + ": the plan has several channels; use the *_batch call");
+    return SL1M_OK;
+}
+
 void free_plan(sl1m_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
-                    p->trace_buf};
+                    p->trace_buf, p->chan_scale, p->step_c};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -121,7 +130,68 @@ ApplyParams make_params(const sl1m_plan *p) {
     P.gA = p->gA;
     P.ws_v = p->ws_v;
     P.ws_p = p->ws_p;
+    P.chan_scale = p->chan_scale;
+    P.ws_v_stride = (size_t)p->fwd_split * (size_t)p->n_vis_int;
+    P.ws_p_stride = (size_t)p->adj_split * (size_t)p->n_pix_pad;
     return P;
+}
+
+// Launch configuration (enough CTAs for 148 SMs x 4 resident CTAs x several waves, shared between the
+// channels of a batch) and the workspaces, all [n_chan][.].  Called at plan creation and again by
+// sl1m_plan_set_channels.
+int configure_and_allocate(sl1m_plan *p) {
+    // ---- launch configuration: enough CTAs for 148 SMs x 4 resident CTAs x several waves ----
+    const int target = std::max(SM_COUNT_B200 * 2, SM_COUNT_B200 * 4 * 8 / p->n_chan);   // CTAs per channel
+    {
+        const int64_t nvi = p->n_vis_int;
+        int rv = 8;
+        while (rv > 1 && p->gk != 2 && (int64_t)((nvi + NT * rv - 1) / (NT * rv)) * p->n_tiles * p->n_chan < 2 * SM_COUNT_B200)
+            rv >>= 1;
+#ifdef SL1M_FORCE_R
+        rv = SL1M_FORCE_R;
+#endif
+        p->fwd_rv = rv;
+        p->fwd_vtiles = (int)((nvi + NT * rv - 1) / (NT * rv));
+        int split = std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
+        p->fwd_per_split = (p->n_tiles + split - 1) / split;
+        p->fwd_split = (p->n_tiles + p->fwd_per_split - 1) / p->fwd_per_split;
+    }
+    {
+        const int n_chunks = (p->n_vis_int + VC - 1) / VC;
+        int rp = 8;
+        while (rp > 1 && (int64_t)(p->n_pix_pad / (NT * rp)) * n_chunks * p->n_chan < 2 * SM_COUNT_B200) rp >>= 1;
+#ifdef SL1M_FORCE_R
+        rp = SL1M_FORCE_R;
+#endif
+        p->adj_rp = rp;
+        p->adj_pgroups = p->n_pix_pad / (NT * rp);
+        int split = std::min(n_chunks, std::max(1, (target + p->adj_pgroups - 1) / p->adj_pgroups));
+        p->adj_per_split = (n_chunks + split - 1) / split;
+        p->adj_split = (n_chunks + p->adj_per_split - 1) / p->adj_per_split;
+    }
+
+    // ---- workspaces ----
+    const size_t npad = (size_t)p->n_pix_pad, C = (size_t)p->n_chan;
+    for (void **q : {(void **)&p->ws_v, (void **)&p->ws_p, (void **)&p->resid, (void **)&p->I_sorted, (void **)&p->y_sorted,
+                     (void **)&p->g_sorted, (void **)&p->part_a, (void **)&p->part_b, (void **)&p->part_c, (void **)&p->scalars}) {
+        if (*q) cudaFree(*q);
+        *q = nullptr;
+    }
+    CUDA_TRY(cudaMalloc((void **)&p->ws_v, C * (size_t)p->fwd_split * (size_t)p->n_vis_int * sizeof(float2)));
+    CUDA_TRY(cudaMalloc((void **)&p->ws_p, C * (size_t)p->adj_split * npad * sizeof(float)));
+    CUDA_TRY(cudaMalloc((void **)&p->resid, C * (size_t)p->n_vis_int * sizeof(float2)));
+    CUDA_TRY(cudaMalloc((void **)&p->I_sorted, C * npad * sizeof(float)));
+    CUDA_TRY(cudaMalloc((void **)&p->y_sorted, C * npad * sizeof(float)));
+    CUDA_TRY(cudaMalloc((void **)&p->g_sorted, C * npad * sizeof(float)));
+    p->n_part = (int)std::max<size_t>((npad + ET - 1) / ET, ((size_t)p->n_vis_int + ET - 1) / ET);
+    CUDA_TRY(cudaMalloc((void **)&p->part_a, C * (size_t)p->n_part * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&p->part_b, C * (size_t)p->n_part * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&p->part_c, C * (size_t)p->n_part * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&p->scalars, C * 4 * sizeof(double)));
+    CUDA_TRY(cudaMemset(p->scalars, 0, C * 4 * sizeof(double)));
+    CUDA_TRY(cudaDeviceSynchronize());
+
+    return SL1M_OK;
 }
 
 }  // namespace
@@ -335,51 +405,10 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
             return fail(e2 == cudaErrorMemoryAllocation ? SL1M_ERR_ALLOC : SL1M_ERR_CUDA, cudaGetErrorString(e2));
     }
 
-    // ---- launch configuration: enough CTAs for 148 SMs x 4 resident CTAs x several waves ----
-    const int target = SM_COUNT_B200 * 4 * 8;
     {
-        const int64_t nvi = p->n_vis_int;
-        int rv = 8;
-        while (rv > 1 && p->gk != 2 && (int64_t)((nvi + NT * rv - 1) / (NT * rv)) * p->n_tiles < 2 * SM_COUNT_B200)
-            rv >>= 1;
-#ifdef SL1M_FORCE_R
-        rv = SL1M_FORCE_R;
-#endif
-        p->fwd_rv = rv;
-        p->fwd_vtiles = (int)((nvi + NT * rv - 1) / (NT * rv));
-        int split = std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
-        p->fwd_per_split = (p->n_tiles + split - 1) / split;
-        p->fwd_split = (p->n_tiles + p->fwd_per_split - 1) / p->fwd_per_split;
+        int st2 = configure_and_allocate(p);
+        if (st2) return st2;
     }
-    {
-        const int n_chunks = (p->n_vis_int + VC - 1) / VC;
-        int rp = 8;
-        while (rp > 1 && (int64_t)(p->n_pix_pad / (NT * rp)) * n_chunks < 2 * SM_COUNT_B200) rp >>= 1;
-#ifdef SL1M_FORCE_R
-        rp = SL1M_FORCE_R;
-#endif
-        p->adj_rp = rp;
-        p->adj_pgroups = p->n_pix_pad / (NT * rp);
-        int split = std::min(n_chunks, std::max(1, (target + p->adj_pgroups - 1) / p->adj_pgroups));
-        p->adj_per_split = (n_chunks + split - 1) / split;
-        p->adj_split = (n_chunks + p->adj_per_split - 1) / p->adj_per_split;
-    }
-
-    // ---- workspaces ----
-    const size_t npad = (size_t)p->n_pix_pad;
-    CUDA_TRY(cudaMalloc((void **)&p->ws_v, (size_t)p->fwd_split * (size_t)p->n_vis_int * sizeof(float2)));
-    CUDA_TRY(cudaMalloc((void **)&p->ws_p, (size_t)p->adj_split * npad * sizeof(float)));
-    CUDA_TRY(cudaMalloc((void **)&p->resid, (size_t)p->n_vis_int * sizeof(float2)));
-    CUDA_TRY(cudaMalloc((void **)&p->I_sorted, npad * sizeof(float)));
-    CUDA_TRY(cudaMalloc((void **)&p->y_sorted, npad * sizeof(float)));
-    CUDA_TRY(cudaMalloc((void **)&p->g_sorted, npad * sizeof(float)));
-    p->n_part = (int)std::max<size_t>((npad + ET - 1) / ET, ((size_t)p->n_vis_int + ET - 1) / ET);
-    CUDA_TRY(cudaMalloc((void **)&p->part_a, (size_t)p->n_part * sizeof(double)));
-    CUDA_TRY(cudaMalloc((void **)&p->part_b, (size_t)p->n_part * sizeof(double)));
-    CUDA_TRY(cudaMalloc((void **)&p->part_c, (size_t)p->n_part * sizeof(double)));
-    CUDA_TRY(cudaMalloc((void **)&p->scalars, 4 * sizeof(double)));
-    CUDA_TRY(cudaMemset(p->scalars, 0, 4 * sizeof(double)));
-    CUDA_TRY(cudaDeviceSynchronize());
 
     guard.p = nullptr;
     *out = p;
@@ -392,6 +421,7 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
 namespace {
 
 inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
+inline dim3 cgrid(const sl1m_plan *p, size_t n) { return dim3((unsigned)egrid(n), (unsigned)p->n_chan); }  // x: elements, y: channel
 
 template <int PK, int GK>
 void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
@@ -427,7 +457,7 @@ void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
 void launch_fwd(sl1m_plan *p, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->fwd_per_split;
-    dim3 grid(p->fwd_vtiles, p->fwd_split);
+    dim3 grid(p->fwd_vtiles, p->fwd_split, p->n_chan);
     const int key = (p->gauss ? 3 : 0) + p->gk;
     switch (key) {
         case 0: launch_fwd_rv<0, 0>(p, P, grid, s); break;
@@ -445,7 +475,7 @@ void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->adj_per_split;
     P.r = r;
-    dim3 grid(p->adj_pgroups, p->adj_split);
+    dim3 grid(p->adj_pgroups, p->adj_split, p->n_chan);
     const int key = (p->gauss ? 3 : 0) + p->gk;
     switch (key) {
         case 0: launch_adj_rp<0, 0>(p, P, grid, s); break;
@@ -469,10 +499,10 @@ int check_launch(const char *what) {
 extern "C" int sl1m_forward(sl1m_plan *p, const float *x_dev, float *vis_dev, void *stream) {
     if (!p || !x_dev || !vis_dev) return fail(SL1M_ERR_NULL, "sl1m_forward: NULL argument");
     cudaStream_t s = (cudaStream_t)stream;
-    pack_caller_kernel<<<egrid(p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->perm, x_dev, p->n_pix_pad);
+    pack_caller_kernel<<<cgrid(p, p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->perm, x_dev, p->n_pix_pad, (int)p->n_pix);
     launch_fwd(p, s);
-    fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
-                                                         (float2 *)vis_dev, 0, nullptr);
+    fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
+                                                            (float2 *)vis_dev, 0, nullptr, (int)p->n_vis, p->n_part);
     p->launches += 2;
     return check_launch("sl1m_forward");
 }
@@ -482,13 +512,14 @@ extern "C" int sl1m_adjoint(sl1m_plan *p, const float *r_dev, float *img_dev, vo
     cudaStream_t s = (cudaStream_t)stream;
     const float2 *r_int = (const float2 *)r_dev;
     if (p->vperm) {
-        vis_gather_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>((const float2 *)r_dev, p->vperm, p->resid, p->n_vis_int);
+        vis_gather_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>((const float2 *)r_dev, p->vperm, p->resid, p->n_vis_int,
+                                                                (int)p->n_vis);
         p->launches++;
         r_int = p->resid;
     }
     launch_adj(p, r_int, s);
-    adj_reduce_kernel<<<egrid(p->n_pix_pad), ET, 0, s>>>(p->ws_p, p->adj_split, p->n_pix_pad, p->amp, p->perm,
-                                                         img_dev, nullptr, nullptr);
+    adj_reduce_kernel<<<cgrid(p, p->n_pix_pad), ET, 0, s>>>(p->ws_p, p->adj_split, p->n_pix_pad, p->amp, p->perm,
+                                                            img_dev, nullptr, nullptr, (int)p->n_pix, p->n_part);
     p->launches += 1;
     return check_launch("sl1m_adjoint");
 }
@@ -504,6 +535,7 @@ int ensure_host_staging(sl1m_plan *p) {
 
 extern "C" int sl1m_forward_host(sl1m_plan *p, const float *x_host, float *vis_host, void *stream) {
     if (!p || !x_host || !vis_host) return fail(SL1M_ERR_NULL, "sl1m_forward_host: NULL argument");
+    if (int stc = single_channel_only(p, "sl1m_forward_host")) return stc;
     cudaStream_t s = (cudaStream_t)stream;
     int st = ensure_host_staging(p);
     if (st) return st;
@@ -516,6 +548,7 @@ extern "C" int sl1m_forward_host(sl1m_plan *p, const float *x_host, float *vis_h
 
 extern "C" int sl1m_adjoint_host(sl1m_plan *p, const float *r_host, float *img_host, void *stream) {
     if (!p || !r_host || !img_host) return fail(SL1M_ERR_NULL, "sl1m_adjoint_host: NULL argument");
+    if (int stc = single_channel_only(p, "sl1m_adjoint_host")) return stc;
     cudaStream_t s = (cudaStream_t)stream;
     int st = ensure_host_staging(p);
     if (st) return st;
@@ -529,34 +562,46 @@ extern "C" int sl1m_adjoint_host(sl1m_plan *p, const float *r_host, float *img_h
 // ------------------------------------------------------------------------------------------
 // a7: power iteration, entirely on the device; one synchronise at the end
 // ------------------------------------------------------------------------------------------
-extern "C" int sl1m_max_eig(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
+namespace {
+// L_out_host: HOST [n_chan]
+int max_eig_impl(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
     if (!p || !L_out_host) return fail(SL1M_ERR_NULL, "sl1m_max_eig: NULL argument");
     if (n_pow < 1) return fail(SL1M_ERR_PARAM, "n_pow must be >= 1");
     cudaStream_t s = (cudaStream_t)stream;
     const int npad = p->n_pix_pad;
     // x0 = 1/sqrt(n_pix) on real pixels
-    fill_kernel<<<egrid(npad), ET, 0, s>>>(p->g_sorted, (float)(1.0 / std::sqrt((double)p->n_pix)), p->perm, npad);
-    pack_sorted_kernel<<<egrid(npad), ET, 0, s>>>(p->pix4, p->amp, p->g_sorted, npad);
+    fill_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->g_sorted, (float)(1.0 / std::sqrt((double)p->n_pix)), p->perm, npad);
+    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->g_sorted, npad);
     p->launches += 2;
     for (int it = 0; it < n_pow; ++it) {
         launch_fwd(p, s);
-        fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
-                                                             p->resid, 1, nullptr);
+        fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
+                                                                p->resid, 1, nullptr, (int)p->n_vis, p->n_part);
         launch_adj(p, p->resid, s);
-        adj_reduce_kernel<<<egrid(npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->perm, nullptr,
-                                                     p->g_sorted, p->part_a);
-        sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, nullptr, nullptr, egrid(npad), 0, 0, p->scalars, nullptr,
-                                             nullptr);
-        normalize_pack_kernel<<<egrid(npad), ET, 0, s>>>(p->g_sorted, p->scalars, p->amp, p->pix4, npad);
+        adj_reduce_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->perm, nullptr,
+                                                        p->g_sorted, p->part_a, (int)p->n_pix, p->n_part);
+        sum_partials_kernel<<<p->n_chan, ET, 0, s>>>(p->part_a, nullptr, nullptr, egrid(npad), 0, 0, p->scalars, nullptr,
+                                                     nullptr, p->n_part, 4);
+        normalize_pack_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->g_sorted, p->scalars, p->amp, p->pix4, npad);
         p->launches += 4;
     }
     int st = check_launch("sl1m_max_eig");
     if (st) return st;
-    double norm2 = 0.0;
-    CUDA_TRY(cudaMemcpyAsync(&norm2, p->scalars, sizeof(double), cudaMemcpyDeviceToHost, s));
+    std::vector<double> h(4 * (size_t)p->n_chan);
+    CUDA_TRY(cudaMemcpyAsync(h.data(), p->scalars, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
     CUDA_TRY(cudaStreamSynchronize(s));
-    *L_out_host = (float)std::sqrt(norm2);
+    for (int c = 0; c < p->n_chan; ++c) L_out_host[c] = (float)std::sqrt(h[4 * (size_t)c]);
     return SL1M_OK;
+}
+}  // namespace
+
+extern "C" int sl1m_max_eig(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
+    if (int st = single_channel_only(p, "sl1m_max_eig")) return st;
+    return max_eig_impl(p, n_pow, L_out_host, stream);
+}
+
+extern "C" int sl1m_max_eig_batch(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
+    return max_eig_impl(p, n_pow, L_out_host, stream);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -564,12 +609,21 @@ extern "C" int sl1m_max_eig(sl1m_plan *p, int n_pow, float *L_out_host, void *st
 // ------------------------------------------------------------------------------------------
 namespace {
 // Shared body of sl1m_solve (tol < 0: fixed iteration count) and sl1m_solve_tol.
-int solve_impl(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int n_iter, double tol,
-               int check_every, const float *x0_dev, float *x_out_dev, double *trace_dev,
+int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const float *L_c_in, int n_pow,
+               int n_iter, double tol, int check_every, const float *x0_dev, float *x_out_dev, double *trace_dev,
                sl1m_solve_info *info_host, void *stream) {
-    if (!p || !vis_dev || !x_out_dev) return fail(SL1M_ERR_NULL, "sl1m_solve: NULL argument");
-    if (!(lambda >= 0.f) || n_iter < 0) return fail(SL1M_ERR_PARAM, "lambda < 0 or n_iter < 0");
-    if (!(L > 0.f) && n_pow < 1) return fail(SL1M_ERR_PARAM, "L <= 0 needs n_pow >= 1");
+    // lambda_c, L_c_in: HOST [n_chan]; vis/x0/x_out: DEV [n_chan][.]; trace: DEV [n_chan][n_iter][3];
+    // info_host: HOST [n_chan].  tol >= 0 (single channel only) enables the stopping rule.
+    if (!p || !vis_dev || !x_out_dev || !lambda_c || !L_c_in) return fail(SL1M_ERR_NULL, "sl1m_solve: NULL argument");
+    if (n_iter < 0) return fail(SL1M_ERR_PARAM, "n_iter < 0");
+    const int C = p->n_chan;
+    std::vector<float> L_c(L_c_in, L_c_in + C);
+    bool need_L = false;
+    for (int c = 0; c < C; ++c) {
+        if (!(lambda_c[c] >= 0.f)) return fail(SL1M_ERR_PARAM, "lambda < 0");
+        need_L |= !(L_c[c] > 0.f);
+    }
+    if (need_L && n_pow < 1) return fail(SL1M_ERR_PARAM, "L <= 0 needs n_pow >= 1");
     cudaStream_t s = (cudaStream_t)stream;
     const int npad = p->n_pix_pad;
     int st;
@@ -583,22 +637,36 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_
         }
         trace_dev = p->trace_buf;
     }
-    if (!(L > 0.f)) {
-        if ((st = sl1m_max_eig(p, n_pow, &L, stream))) return st;
-        if (!(L > 0.f)) return fail(SL1M_ERR_PARAM, "power iteration returned L <= 0 (zero operator)");
+    if (need_L) {
+        std::vector<float> L_pow((size_t)C);
+        if ((st = max_eig_impl(p, n_pow, L_pow.data(), stream))) return st;
+        for (int c = 0; c < C; ++c) {
+            if (!(L_c[c] > 0.f)) L_c[c] = L_pow[c];
+            if (!(L_c[c] > 0.f)) return fail(SL1M_ERR_PARAM, "power iteration returned L <= 0 (zero operator)");
+        }
     }
-    const float inv_L = (float)(1.0 / (double)L);
-    const float thr = (float)((double)lambda / (double)L);
+    const float inv_L = (float)(1.0 / (double)L_c[0]);
+    const float thr = (float)((double)lambda_c[0] / (double)L_c[0]);
+    const float2 *step_c = nullptr;
+    if (C > 1) {                      // per-channel (1/L_c, lambda_c/L_c) on the device
+        std::vector<float2> h((size_t)C);
+        for (int c = 0; c < C; ++c)
+            h[c] = make_float2((float)(1.0 / (double)L_c[c]), (float)((double)lambda_c[c] / (double)L_c[c]));
+        CUDA_TRY(cudaMemcpyAsync(p->step_c, h.data(), (size_t)C * sizeof(float2), cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaStreamSynchronize(s));   // h is a stack-lifetime staging buffer
+        step_c = p->step_c;
+    }
+    const size_t trace_stride = 3 * (size_t)std::max(n_iter, 1);   // doubles per channel in trace_dev
 
     // y_1 = I_0 = x0 (or 0), in sorted order; a*y_1 packed into the pixel tiles
     if (x0_dev) {
-        gather_kernel<<<egrid(npad), ET, 0, s>>>(x0_dev, p->perm, p->I_sorted, npad);
+        gather_kernel<<<cgrid(p, npad), ET, 0, s>>>(x0_dev, p->perm, p->I_sorted, npad, (int)p->n_pix);
         p->launches++;
     } else {
-        CUDA_TRY(cudaMemsetAsync(p->I_sorted, 0, (size_t)npad * sizeof(float), s));
+        CUDA_TRY(cudaMemsetAsync(p->I_sorted, 0, (size_t)C * npad * sizeof(float), s));
     }
-    CUDA_TRY(cudaMemcpyAsync(p->y_sorted, p->I_sorted, (size_t)npad * sizeof(float), cudaMemcpyDeviceToDevice, s));
-    pack_sorted_kernel<<<egrid(npad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, npad);
+    CUDA_TRY(cudaMemcpyAsync(p->y_sorted, p->I_sorted, (size_t)C * npad * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, npad);
     p->launches++;
 
     double t = 1.0;
@@ -608,19 +676,19 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_
         const float beta = (float)((t - 1.0) / t_next);
         t = t_next;
         launch_fwd(p, s);
-        fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
-                                                             (const float2 *)vis_dev, p->resid, 1,
-                                                             trace_dev ? p->part_a : nullptr);
+        fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
+                                                                (const float2 *)vis_dev, p->resid, 1,
+                                                                trace_dev ? p->part_a : nullptr, (int)p->n_vis, p->n_part);
         launch_adj(p, p->resid, s);
-        fista_update_kernel<<<egrid(npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->pix4, p->I_sorted,
-                                                       p->y_sorted, inv_L, thr, beta,
-                                                       trace_dev ? p->part_b : nullptr,
-                                                       trace_dev ? p->part_c : nullptr);
+        fista_update_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->pix4, p->I_sorted,
+                                                          p->y_sorted, inv_L, thr, beta,
+                                                          trace_dev ? p->part_b : nullptr,
+                                                          trace_dev ? p->part_c : nullptr, step_c, p->n_part);
         p->launches += 2;
         if (trace_dev) {
-            sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
+            sum_partials_kernel<<<C, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
                                                  egrid(npad), trace_dev + 3 * (size_t)k, trace_dev + 3 * (size_t)k + 1,
-                                                 trace_dev + 3 * (size_t)k + 2);
+                                                 trace_dev + 3 * (size_t)k + 2, p->n_part, trace_stride);
             p->launches++;
         }
         n_done = k + 1;
@@ -630,34 +698,37 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_
             double h[6];
             CUDA_TRY(cudaMemcpyAsync(h, trace_dev + 3 * (size_t)(n_done - 2), sizeof(h), cudaMemcpyDeviceToHost, s));
             CUDA_TRY(cudaStreamSynchronize(s));
-            const double E_before = h[0] + 2.0 * (double)lambda * h[1];
-            const double E_now = h[3] + 2.0 * (double)lambda * h[4];
+            const double E_before = h[0] + 2.0 * (double)lambda_c[0] * h[1];
+            const double E_now = h[3] + 2.0 * (double)lambda_c[0] * h[4];
             if (std::fabs(E_now - E_before) <= tol * std::fabs(E_now)) break;
         }
     }
-    scatter_kernel<<<egrid(npad), ET, 0, s>>>(p->I_sorted, p->perm, x_out_dev, npad);
+    scatter_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->I_sorted, p->perm, x_out_dev, npad, (int)p->n_pix);
     p->launches++;
     if ((st = check_launch("sl1m_solve"))) return st;
 
     if (info_host) {
         // one extra forward for ||M I_K - V||^2 (Table 1's L2 term)
-        pack_sorted_kernel<<<egrid(npad), ET, 0, s>>>(p->pix4, p->amp, p->I_sorted, npad);
+        pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->I_sorted, npad);
         launch_fwd(p, s);
-        fwd_reduce_kernel<<<egrid(p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
-                                                             (const float2 *)vis_dev, p->resid, 1, p->part_a);
-        l1_nnz_kernel<<<egrid(npad), ET, 0, s>>>(p->I_sorted, npad, p->part_b, p->part_c);
-        sum_partials_kernel<<<1, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
-                                             egrid(npad), p->scalars + 1, p->scalars + 2, p->scalars + 3);
+        fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
+                                                                (const float2 *)vis_dev, p->resid, 1, p->part_a,
+                                                                (int)p->n_vis, p->n_part);
+        l1_nnz_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->I_sorted, npad, p->part_b, p->part_c, p->n_part);
+        sum_partials_kernel<<<C, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
+                                             egrid(npad), p->scalars + 1, p->scalars + 2, p->scalars + 3, p->n_part, 4);
         p->launches += 4;
         if ((st = check_launch("sl1m_solve(info)"))) return st;
-        double h[4];
-        CUDA_TRY(cudaMemcpyAsync(h, p->scalars, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
+        std::vector<double> h(4 * (size_t)C);
+        CUDA_TRY(cudaMemcpyAsync(h.data(), p->scalars, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
         CUDA_TRY(cudaStreamSynchronize(s));
-        info_host->n_iter_done = n_done;
-        info_host->L_used = L;
-        info_host->l2_term = h[1];
-        info_host->l1_term = h[2];
-        info_host->nnz = (int64_t)(h[3] + 0.5);
+        for (int c = 0; c < C; ++c) {
+            info_host[c].n_iter_done = n_done;
+            info_host[c].L_used = L_c[c];
+            info_host[c].l2_term = h[4 * c + 1];
+            info_host[c].l1_term = h[4 * c + 2];
+            info_host[c].nnz = (int64_t)(h[4 * c + 3] + 0.5);
+        }
     }
     return SL1M_OK;
 }
@@ -666,20 +737,68 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_
 extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int n_iter,
                           const float *x0_dev, float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host,
                           void *stream) {
-    return solve_impl(p, vis_dev, lambda, L, n_pow, n_iter, -1.0, 1, x0_dev, x_out_dev, trace_dev, info_host, stream);
+    if (int st = single_channel_only(p, "sl1m_solve")) return st;
+    return solve_impl(p, vis_dev, &lambda, &L, n_pow, n_iter, -1.0, 1, x0_dev, x_out_dev, trace_dev, info_host, stream);
 }
 
 extern "C" int sl1m_solve_tol(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int max_iter,
                               double tol, int check_every, const float *x0_dev, float *x_out_dev,
                               double *trace_dev, sl1m_solve_info *info_host, void *stream) {
+    if (int st = single_channel_only(p, "sl1m_solve_tol")) return st;
     if (!(tol >= 0.0) || check_every < 1) return fail(SL1M_ERR_PARAM, "sl1m_solve_tol: tol < 0 or check_every < 1");
     if (!info_host) return fail(SL1M_ERR_NULL, "sl1m_solve_tol: info_host is required (it carries n_iter_done)");
-    return solve_impl(p, vis_dev, lambda, L, n_pow, max_iter, tol, check_every, x0_dev, x_out_dev, trace_dev,
+    return solve_impl(p, vis_dev, &lambda, &L, n_pow, max_iter, tol, check_every, x0_dev, x_out_dev, trace_dev,
                       info_host, stream);
 }
 
+extern "C" int sl1m_solve_batch(sl1m_plan *p, const float *vis_dev, const float *lambda_host, const float *L_host,
+                                int n_pow, int n_iter, const float *x0_dev, float *x_out_dev, double *trace_dev,
+                                sl1m_solve_info *info_host, void *stream) {
+    return solve_impl(p, vis_dev, lambda_host, L_host, n_pow, n_iter, -1.0, 1, x0_dev, x_out_dev, trace_dev,
+                      info_host, stream);
+}
+
+// NEXT-4: turn the plan into a batch of n_chan channels that share pixels, gains and baseline
+// geometry; channel c sees uvw * scale[c].
+extern "C" int sl1m_plan_set_channels(sl1m_plan *p, int32_t n_chan, const double *scale_host) {
+    if (!p || !scale_host) return fail(SL1M_ERR_NULL, "sl1m_plan_set_channels: NULL argument");
+    if (n_chan < 1 || n_chan > 65535) return fail(SL1M_ERR_SIZE, "n_chan must be in [1, 65535]");
+    for (int c = 0; c < n_chan; ++c)
+        if (!std::isfinite(scale_host[c]) || !(scale_host[c] > 0.0))
+            return fail(SL1M_ERR_DOMAIN, "channel scale must be finite and > 0");
+    const size_t npad = (size_t)p->n_pix_pad;
+    // replicate the pixel tiles: channel c keeps its own a*x in pix4[c][.].w
+    float4 *pix_new = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&pix_new, (size_t)n_chan * npad * sizeof(float4)));
+    for (int c = 0; c < n_chan; ++c) {
+        cudaError_t e = cudaMemcpy(pix_new + (size_t)c * npad, p->pix4, npad * sizeof(float4), cudaMemcpyDeviceToDevice);
+        if (e != cudaSuccess) { cudaFree(pix_new); return fail(SL1M_ERR_CUDA, cudaGetErrorString(e)); }
+    }
+    cudaFree(p->pix4);
+    p->pix4 = pix_new;
+    if (p->chan_scale) cudaFree(p->chan_scale);
+    if (p->step_c) cudaFree(p->step_c);
+    p->chan_scale = nullptr;
+    p->step_c = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&p->chan_scale, (size_t)n_chan * sizeof(double)));
+    CUDA_TRY(cudaMemcpy(p->chan_scale, scale_host, (size_t)n_chan * sizeof(double), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMalloc((void **)&p->step_c, (size_t)n_chan * sizeof(float2)));
+    p->n_chan = n_chan;
+    for (void **q : {(void **)&p->h_x, (void **)&p->h_vis, (void **)&p->h_img}) {   // single-channel staging
+        if (*q) cudaFree(*q);
+        *q = nullptr;
+    }
+    int st = configure_and_allocate(p);
+    if (st) return st;
+    CUDA_TRY(cudaDeviceSynchronize());
+    return SL1M_OK;
+}
+
+extern "C" int32_t sl1m_plan_n_chan(const sl1m_plan *p) { return p ? p->n_chan : 0; }
+
 extern "C" int sl1m_dirty_image(sl1m_plan *p, const float *vis_dev, float scale, float *img_dev, void *stream) {
     if (!p || !vis_dev || !img_dev) return fail(SL1M_ERR_NULL, "sl1m_dirty_image: NULL argument");
+    if (int stc = single_channel_only(p, "sl1m_dirty_image")) return stc;
     if (!std::isfinite(scale)) return fail(SL1M_ERR_PARAM, "sl1m_dirty_image: non-finite scale");
     int st = sl1m_adjoint(p, vis_dev, img_dev, stream);
     if (st) return st;
@@ -692,6 +811,7 @@ extern "C" int sl1m_solve_host(sl1m_plan *p, const float *vis_host, float lambda
                                const float *x0_host, float *x_out_host, sl1m_solve_info *info_host,
                                void *stream) {
     if (!p || !vis_host || !x_out_host) return fail(SL1M_ERR_NULL, "sl1m_solve_host: NULL argument");
+    if (int stc = single_channel_only(p, "sl1m_solve_host")) return stc;
     cudaStream_t s = (cudaStream_t)stream;
     int st = ensure_host_staging(p);
     if (st) return st;

@@ -28,27 +28,33 @@ __device__ __forceinline__ double block_sum(double v) {
 
 // pix4[k].w = a_k * x[perm[k]]   (caller order -> sorted, padded pixels get 0)
 __global__ void __launch_bounds__(ET) pack_caller_kernel(float4 *pix4, const float *amp, const int *perm,
-                                                         const float *x, int n_pix_pad) {
+                                                         const float *x, int n_pix_pad, int n_pix) {
     const int k = blockIdx.x * ET + threadIdx.x;
     if (k >= n_pix_pad) return;
+    pix4 += (size_t)blockIdx.y * n_pix_pad;   // blockIdx.y = channel (NEXT-4); caller arrays are [n_chan][n_pix]
+    x += (size_t)blockIdx.y * n_pix;
     const int src = perm[k];
     pix4[k].w = (src >= 0) ? amp[k] * x[src] : 0.f;
 }
 
 // sorted[k] = caller[perm[k]] (0 on padding)
 __global__ void __launch_bounds__(ET) gather_kernel(const float *caller, const int *perm, float *sorted,
-                                                    int n_pix_pad) {
+                                                    int n_pix_pad, int n_pix) {
     const int k = blockIdx.x * ET + threadIdx.x;
     if (k >= n_pix_pad) return;
+    caller += (size_t)blockIdx.y * n_pix;
+    sorted += (size_t)blockIdx.y * n_pix_pad;
     const int src = perm[k];
     sorted[k] = (src >= 0) ? caller[src] : 0.f;
 }
 
 // caller[perm[k]] = sorted[k]
 __global__ void __launch_bounds__(ET) scatter_kernel(const float *sorted, const int *perm, float *caller,
-                                                     int n_pix_pad) {
+                                                     int n_pix_pad, int n_pix) {
     const int k = blockIdx.x * ET + threadIdx.x;
     if (k >= n_pix_pad) return;
+    caller += (size_t)blockIdx.y * n_pix;
+    sorted += (size_t)blockIdx.y * n_pix_pad;
     const int dst = perm[k];
     if (dst >= 0) caller[dst] = sorted[k];
 }
@@ -57,11 +63,14 @@ __global__ void __launch_bounds__(ET) scatter_kernel(const float *sorted, const 
 __global__ void __launch_bounds__(ET) pack_sorted_kernel(float4 *pix4, const float *amp, const float *xs,
                                                          int n_pix_pad) {
     const int k = blockIdx.x * ET + threadIdx.x;
+    pix4 += (size_t)blockIdx.y * n_pix_pad;
+    xs += (size_t)blockIdx.y * n_pix_pad;
     if (k < n_pix_pad) pix4[k].w = amp[k] * xs[k];
 }
 
 __global__ void __launch_bounds__(ET) fill_kernel(float *p, float v, const int *perm, int n_pix_pad) {
     const int k = blockIdx.x * ET + threadIdx.x;
+    p += (size_t)blockIdx.y * n_pix_pad;
     if (k < n_pix_pad) p[k] = (perm[k] >= 0) ? v : 0.f;
 }
 
@@ -71,9 +80,13 @@ __global__ void __launch_bounds__(ET) fill_kernel(float *p, float v, const int *
 // part[block] = sum |value|^2 (fp64).
 __global__ void __launch_bounds__(ET) fwd_reduce_kernel(const float2 *ws, int n_split, int n_int,
                                                         const int *vperm, const float2 *V, float2 *out,
-                                                        int out_internal, double *part) {
+                                                        int out_internal, double *part, int n_vis, int n_part) {
     const int js = blockIdx.x * ET + threadIdx.x;
     double sq = 0.0;
+    ws += (size_t)blockIdx.y * n_split * n_int;          // blockIdx.y = channel
+    if (V) V += (size_t)blockIdx.y * n_vis;
+    out += (size_t)blockIdx.y * (out_internal ? n_int : n_vis);
+    if (part) part += (size_t)blockIdx.y * n_part;
     if (js < n_int) {
         const int jc = vperm ? vperm[js] : js;
         float re = 0.f, im = 0.f;
@@ -101,9 +114,11 @@ __global__ void __launch_bounds__(ET) fwd_reduce_kernel(const float2 *ws, int n_
 
 // internal[js] = caller[vperm[js]] (0 on padding): brings an API residual into the internal order.
 __global__ void __launch_bounds__(ET) vis_gather_kernel(const float2 *caller, const int *vperm, float2 *internal,
-                                                        int n_int) {
+                                                        int n_int, int n_vis) {
     const int js = blockIdx.x * ET + threadIdx.x;
     if (js >= n_int) return;
+    caller += (size_t)blockIdx.y * n_vis;
+    internal += (size_t)blockIdx.y * n_int;
     const int jc = vperm[js];
     internal[js] = (jc >= 0) ? caller[jc] : make_float2(0.f, 0.f);
 }
@@ -111,9 +126,13 @@ __global__ void __launch_bounds__(ET) vis_gather_kernel(const float2 *caller, co
 // Adjoint epilogue: g_k = a_k sum_s ws[s][k]; scattered to the caller's order and/or kept sorted.
 __global__ void __launch_bounds__(ET) adj_reduce_kernel(const float *ws, int n_split, int n_pix_pad,
                                                         const float *amp, const int *perm, float *img_caller,
-                                                        float *g_sorted, double *part) {
+                                                        float *g_sorted, double *part, int n_pix, int n_part) {
     const int k = blockIdx.x * ET + threadIdx.x;
     double sq = 0.0;
+    ws += (size_t)blockIdx.y * n_split * n_pix_pad;      // blockIdx.y = channel
+    if (img_caller) img_caller += (size_t)blockIdx.y * n_pix;
+    if (g_sorted) g_sorted += (size_t)blockIdx.y * n_pix_pad;
+    if (part) part += (size_t)blockIdx.y * n_part;
     if (k < n_pix_pad) {
         float g = 0.f;
         for (int s = 0; s < n_split; ++s) g += ws[(size_t)s * n_pix_pad + k];
@@ -135,9 +154,23 @@ __global__ void __launch_bounds__(ET) adj_reduce_kernel(const float *ws, int n_s
 __global__ void __launch_bounds__(ET) fista_update_kernel(const float *ws, int n_split, int n_pix_pad,
                                                           const float *amp, float4 *pix4, float *I_sorted,
                                                           float *y_sorted, float inv_L, float thr, float beta,
-                                                          double *part_l1, double *part_nnz) {
+                                                          double *part_l1, double *part_nnz,
+                                                          const float2 *step_c, int n_part) {
     const int k = blockIdx.x * ET + threadIdx.x;
     double l1 = 0.0, nz = 0.0;
+    const int c = blockIdx.y;                            // channel; step_c[c] = (1/L_c, lambda_c/L_c) when batched
+    ws += (size_t)c * n_split * n_pix_pad;
+    pix4 += (size_t)c * n_pix_pad;
+    I_sorted += (size_t)c * n_pix_pad;
+    y_sorted += (size_t)c * n_pix_pad;
+    if (step_c) {
+        inv_L = step_c[c].x;
+        thr = step_c[c].y;
+    }
+    if (part_l1) {
+        part_l1 += (size_t)c * n_part;
+        part_nnz += (size_t)c * n_part;
+    }
     if (k < n_pix_pad) {
         float g = 0.f;
         for (int s = 0; s < n_split; ++s) g += ws[(size_t)s * n_pix_pad + k];
@@ -167,16 +200,17 @@ __global__ void __launch_bounds__(ET) fista_update_kernel(const float *ws, int n
 // out[i] = sum of n partials of array i, i < n_arrays (single CTA, fixed order).
 __global__ void __launch_bounds__(ET) sum_partials_kernel(const double *p0, const double *p1, const double *p2,
                                                           int n0, int n1, int n2, double *out0, double *out1,
-                                                          double *out2) {
+                                                          double *out2, int n_part, size_t out_stride) {
     const double *ps[3] = {p0, p1, p2};
     const int ns[3] = {n0, n1, n2};
     double *outs[3] = {out0, out1, out2};
+    const size_t c = blockIdx.x;                         // one CTA per channel
     for (int a = 0; a < 3; ++a) {
         if (!ps[a] || !outs[a]) continue;
         double v = 0.0;
-        for (int i = threadIdx.x; i < ns[a]; i += ET) v += ps[a][i];
+        for (int i = threadIdx.x; i < ns[a]; i += ET) v += ps[a][c * n_part + i];
         const double t = block_sum(v);
-        if (threadIdx.x == 0) *outs[a] = t;
+        if (threadIdx.x == 0) outs[a][c * out_stride] = t;
     }
 }
 
@@ -185,6 +219,9 @@ __global__ void __launch_bounds__(ET) normalize_pack_kernel(const float *g_sorte
                                                             const float *amp, float4 *pix4, int n_pix_pad) {
     const int k = blockIdx.x * ET + threadIdx.x;
     if (k >= n_pix_pad) return;
+    g_sorted += (size_t)blockIdx.y * n_pix_pad;
+    pix4 += (size_t)blockIdx.y * n_pix_pad;
+    norm2 += (size_t)blockIdx.y * 4;                     // scalars are [n_chan][4]
     const double nrm = sqrt(*norm2);
     const float x = (nrm > 0.0) ? (float)((double)g_sorted[k] / nrm) : 0.f;
     pix4[k].w = amp[k] * x;
@@ -205,8 +242,11 @@ __global__ void __launch_bounds__(ET) gains_layout_kernel(const float2 *raw, int
 
 // Block partials of sum I and nnz I over a sorted image (for the final info struct).
 __global__ void __launch_bounds__(ET) l1_nnz_kernel(const float *I_sorted, int n_pix_pad, double *part_l1,
-                                                    double *part_nnz) {
+                                                    double *part_nnz, int n_part) {
     const int k = blockIdx.x * ET + threadIdx.x;
+    I_sorted += (size_t)blockIdx.y * n_pix_pad;
+    part_l1 += (size_t)blockIdx.y * n_part;
+    part_nnz += (size_t)blockIdx.y * n_part;
     const float v = (k < n_pix_pad) ? I_sorted[k] : 0.f;
     const double t1 = block_sum((double)v);
     const double t2 = block_sum(v != 0.f ? 1.0 : 0.0);

@@ -57,7 +57,16 @@ struct ApplyParams {
     const float2 *r;                // adjoint input [n_vis] (re, im)
     float2 *ws_v;                   // forward partials [n_split][n_vis]
     float *ws_p;                    // adjoint partials [n_split][n_pix_pad]
+    // batched channels (NEXT-4): blockIdx.z = channel c.  Channel c sees the baselines u, v, w
+    // scaled by chan_scale[c] (= nu_c / nu_0, "b = lambda (u, v, w)"), its own a*x in
+    // pix4[c][.].w, its own residual r[c][.] and its own partials.  chan_scale == NULL: one channel.
+    const double *chan_scale;       // [n_chan] or NULL
+    size_t ws_v_stride, ws_p_stride;   // elements per channel of ws_v / ws_p
 };
+
+__device__ __forceinline__ double chan_scale_of(const ApplyParams &P) {
+    return P.chan_scale ? P.chan_scale[blockIdx.z] : 1.0;    // x * 1.0 is exact: one channel is unchanged
+}
 
 // ------------------------------------------------------------------------------------------
 // PTX helpers: mbarrier + 1-D TMA bulk copy (cp.async.bulk -> SASS UBLKCP)
@@ -283,12 +292,14 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     float uf[RV], vf[RV], wf[RV], wl[RV], re[RV], im[RV];
     int ap[RV], aq[RV];
     const int jlast = P.n_vis - 1;
+    const double sc = chan_scale_of(P);
+    const float4 *pix4 = P.pix4 + (size_t)blockIdx.z * P.n_pix_pad;
 #pragma unroll
     for (int r = 0; r < RV; ++r) {
         const int j = min(jbase + r * NT + tid, jlast);
-        const double wd = __ldg(P.w64 + j);
-        uf[r] = static_cast<float>(TWO_PI * __ldg(P.u64 + j));
-        vf[r] = static_cast<float>(TWO_PI * __ldg(P.v64 + j));
+        const double wd = sc * __ldg(P.w64 + j);
+        uf[r] = static_cast<float>(TWO_PI * (sc * __ldg(P.u64 + j)));
+        vf[r] = static_cast<float>(TWO_PI * (sc * __ldg(P.v64 + j)));
         wf[r] = static_cast<float>(TWO_PI * wd);
         wl[r] = static_cast<float>(wd);
         re[r] = 0.f;
@@ -311,7 +322,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     __syncthreads();
     auto issue = [&](int t, int st) {
         mbar_expect_tx(&s_bar[st], kBytes);
-        tma_bulk_g2s(&s_pix[st][0], P.pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
         if (PK) tma_bulk_g2s(&s_pixg[st][0], P.pixg + (size_t)t * TP, TP * sizeof(float2), &s_bar[st]);
     };
     if (tid == 0) {
@@ -327,7 +338,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
             const int j = min(jbase + r * NT + tid, jlast);
-            const double ud = __ldg(P.u64 + j), vd = __ldg(P.v64 + j), wd = __ldg(P.w64 + j);
+            const double ud = sc * __ldg(P.u64 + j), vd = sc * __ldg(P.v64 + j), wd = sc * __ldg(P.w64 + j);
             x0[r] = centre_phase(ud, vd, wd, c);
             if (PK) {
                 uc[r] = static_cast<float>(ud - wd * c.x);
@@ -399,7 +410,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
         if (tid == 0 && t + 2 < t1) issue(t + 2, st);
     }
 
-    float2 *out = P.ws_v + (size_t)blockIdx.y * P.n_vis;
+    float2 *out = P.ws_v + (size_t)blockIdx.z * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
 #pragma unroll
     for (int r = 0; r < RV; ++r) {
         const int j = jbase + r * NT + tid;
@@ -426,14 +437,16 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
     const int t1 = min(t0 + P.per_split, P.n_tiles);
     const int jbase = blockIdx.x * (NT * RV);
     const int jlast = P.n_vis - 1;
+    const double sc = chan_scale_of(P);
+    const float4 *pix4 = P.pix4 + (size_t)blockIdx.z * P.n_pix_pad;
 
     f32x2 U[NPAIR], V[NPAIR], W[NPAIR], RE[NPAIR], IM[NPAIR];
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
         const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
-        U[i] = pk2(static_cast<float>(TWO_PI * __ldg(P.u64 + ja)), static_cast<float>(TWO_PI * __ldg(P.u64 + jb)));
-        V[i] = pk2(static_cast<float>(TWO_PI * __ldg(P.v64 + ja)), static_cast<float>(TWO_PI * __ldg(P.v64 + jb)));
-        W[i] = pk2(static_cast<float>(TWO_PI * __ldg(P.w64 + ja)), static_cast<float>(TWO_PI * __ldg(P.w64 + jb)));
+        U[i] = pk2(static_cast<float>(TWO_PI * (sc * __ldg(P.u64 + ja))), static_cast<float>(TWO_PI * (sc * __ldg(P.u64 + jb))));
+        V[i] = pk2(static_cast<float>(TWO_PI * (sc * __ldg(P.v64 + ja))), static_cast<float>(TWO_PI * (sc * __ldg(P.v64 + jb))));
+        W[i] = pk2(static_cast<float>(TWO_PI * (sc * __ldg(P.w64 + ja))), static_cast<float>(TWO_PI * (sc * __ldg(P.w64 + jb))));
         RE[i] = pk2(0.f, 0.f);
         IM[i] = pk2(0.f, 0.f);
     }
@@ -447,7 +460,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
     __syncthreads();
     auto issue = [&](int t, int st) {
         mbar_expect_tx(&s_bar[st], kBytes);
-        tma_bulk_g2s(&s_pix[st][0], P.pix4 + (size_t)t * TP, kBytes, &s_bar[st]);
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, kBytes, &s_bar[st]);
     };
     if (tid == 0) {
         if (t0 < t1) issue(t0, 0);
@@ -488,8 +501,8 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
 #pragma unroll
         for (int i = 0; i < NPAIR; ++i) {
             const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
-            X0[i] = pk2(centre_phase(__ldg(P.u64 + ja), __ldg(P.v64 + ja), __ldg(P.w64 + ja), c),
-                        centre_phase(__ldg(P.u64 + jb), __ldg(P.v64 + jb), __ldg(P.w64 + jb), c));
+            X0[i] = pk2(centre_phase(sc * __ldg(P.u64 + ja), sc * __ldg(P.v64 + ja), sc * __ldg(P.w64 + ja), c),
+                        centre_phase(sc * __ldg(P.u64 + jb), sc * __ldg(P.v64 + jb), sc * __ldg(P.w64 + jb), c));
         }
         mbar_wait(&s_bar[st], parity);
 #pragma unroll 1
@@ -503,7 +516,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         if (tid == 0 && t + 2 < t1) issue(t + 2, st);
     }
 
-    float2 *out = P.ws_v + (size_t)blockIdx.y * P.n_vis;
+    float2 *out = P.ws_v + (size_t)blockIdx.z * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
         float ra, rb, ia, ib;
@@ -553,6 +566,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     }
 
     const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const double sc = chan_scale_of(P);
     const int c0 = blockIdx.y * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
 
@@ -571,10 +585,10 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
         float2 rr = make_float2(0.f, 0.f);
         int2 a = make_int2(0, 0);
         if (j < P.n_vis) {
-            u = P.u64[j];
-            v = P.v64[j];
-            w = P.w64[j];
-            rr = P.r[j];
+            u = sc * P.u64[j];
+            v = sc * P.v64[j];
+            w = sc * P.w64[j];
+            rr = P.r[(size_t)blockIdx.z * P.n_vis + j];
             if (GK) a = make_int2(P.ant_p[j], P.ant_q[j]);
         }
         s_vis[buf][slot] = make_float4(static_cast<float>(TWO_PI * u), static_cast<float>(TWO_PI * v),
@@ -682,7 +696,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
         __syncthreads();
     }
 
-    float *out = P.ws_p + (size_t)blockIdx.y * P.n_pix_pad;
+    float *out = P.ws_p + (size_t)blockIdx.z * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
 }
@@ -717,6 +731,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
     }
 
     const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const double sc = chan_scale_of(P);
     const int c0 = blockIdx.y * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
 
@@ -725,10 +740,10 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
         double u = 0.0, v = 0.0, w = 0.0;
         float2 rr = make_float2(0.f, 0.f);
         if (j < P.n_vis) {
-            u = P.u64[j];
-            v = P.v64[j];
-            w = P.w64[j];
-            rr = P.r[j];
+            u = sc * P.u64[j];
+            v = sc * P.v64[j];
+            w = sc * P.w64[j];
+            rr = P.r[(size_t)blockIdx.z * P.n_vis + j];
         }
         const float uf = static_cast<float>(TWO_PI * u), vf = static_cast<float>(TWO_PI * v),
                     wf = static_cast<float>(TWO_PI * w);
@@ -777,7 +792,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
         __syncthreads();
     }
 
-    float *out = P.ws_p + (size_t)blockIdx.y * P.n_pix_pad;
+    float *out = P.ws_p + (size_t)blockIdx.z * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
         float a, b;

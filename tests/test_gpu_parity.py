@@ -410,3 +410,59 @@ def test_quadtree_driver_matches_oracle(sl):
     assert [lv["n_pix"] for lv in c2f["levels"]] == [64, 256, 1024]
     with pytest.raises(sl.Sl1mError):
         sl.quadtree_solve(uvw, V, l0, m0, side0, n_levels=3, frac=-1.0, min_side=0.0, lam=lam, capacity=100)
+
+
+# ----------------------------------------------------------------------------- NEXT-4: batched channels
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_batched_channels_match_per_channel_oracle(sl, cfg):
+    """sl1m_plan_set_channels + batched forward / adjoint / max_eig / solve: channel c must equal the
+    oracle on uvw * scale[c] (baselines in wavelengths scale with frequency; PAPER.md:68, 279:
+    channels are deconvolved independently).  Config 1 (delta) and a shrunk config 3 (Gaussian pixels)."""
+    import torch
+    wl = make_workload(cfg) if cfg == 1 else make_workload(3, n_side=32, n_src=20, n_ant=12, n_steps=4)
+    scale = np.array([1.0, 0.93, 1.07, 1.21])
+    C = scale.shape[0]
+    rng = np.random.default_rng(50 + cfg)
+    plan = sl.Plan.from_workload(wl).set_channels(scale)
+    assert plan.n_chan == C
+    X = rng.uniform(0, 1, (C, wl.n_pix))
+    X[:, rng.uniform(size=wl.n_pix) < 0.5] = 0.0
+    R = (rng.standard_normal((C, wl.n_vis)) + 1j * rng.standard_normal((C, wl.n_vis))).astype(np.complex64)
+    Vg = plan.forward(_dev(X, torch.float32)).cpu().numpy()
+    Gg = plan.adjoint(_dev(R, torch.complex64)).cpu().numpy()
+    Lg = plan.max_eig_batch(8)
+    assert Vg.shape == (C, wl.n_vis) and Gg.shape == (C, wl.n_pix)
+    oracles = [oracle.Oracle(wl.uvw * s, wl.l, wl.m, wl.sigma, gauss_model=wl.gauss_model) for s in scale]
+    Vs = []
+    for c, o in enumerate(oracles):
+        assert rel_l2(Vg[c], o.forward(X[c])) <= TOL_APPLY
+        assert rel_l2(Gg[c], o.adjoint(R[c])) <= TOL_APPLY
+        assert abs(Lg[c] - o.max_eig(8)) <= 1e-4 * o.max_eig(8)
+        Vs.append((o.forward(wl.x_true * (1.0 + 0.1 * c)) + wl.noise).astype(np.complex64))
+    # batched solve: per-channel lambda and L, traces, infos
+    K = 40
+    lam = fista_lambda(wl) * np.array([1.0, 0.5, 2.0, 1.0])
+    L = np.array([o.max_eig(30) * 1.05 for o in oracles])
+    trace = torch.zeros(C * 3 * K, dtype=torch.float64, device="cuda")
+    x, infos = plan.solve_batch(_dev(np.stack(Vs), torch.complex64), lam, L, n_iter=K, trace=trace)
+    x = x.cpu().numpy()
+    tr = trace.cpu().numpy().reshape(C, K, 3)
+    for c, o in enumerate(oracles):
+        ref = o.fista(Vs[c], lam[c], L[c], K, want_trace=True)
+        assert rel_l2(x[c], ref["x"]) <= TOL_IMAGE, (c, rel_l2(x[c], ref["x"]))
+        assert abs(infos[c].l2_term - ref["l2_term"]) <= 2e-3 * ref["l2_term"]
+        assert abs(infos[c].l1_term - ref["l1_term"]) <= 2e-3 * ref["l1_term"] + 1e-6
+        assert np.max(np.abs(tr[c, :, 0] - ref["trace"][:, 0]) / ref["trace"][:, 0]) < 2e-3
+        assert infos[c].n_iter_done == K and abs(infos[c].L_used - L[c]) <= 1e-6 * L[c]
+    # a batch of one channel with scale 1 is bit-identical to the plain plan
+    p1 = sl.Plan.from_workload(wl)
+    pb = sl.Plan.from_workload(wl).set_channels([1.0])
+    x0 = _dev(X[0], torch.float32)
+    assert torch.equal(p1.forward(x0), pb.forward(x0))
+    # single-problem calls refuse a multi-channel plan
+    with pytest.raises(sl.Sl1mError):
+        plan.max_eig(3)
+    with pytest.raises(sl.Sl1mError):
+        plan.solve(_dev(Vs[0], torch.complex64), 1.0, L=1.0, n_iter=1)
+    for q in (plan, p1, pb):
+        q.close()
