@@ -423,34 +423,46 @@ namespace {
 inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
 inline dim3 cgrid(const sl1m_plan *p, size_t n) { return dim3((unsigned)egrid(n), (unsigned)p->n_chan); }  // x: elements, y: channel
 
-template <int PK, int GK>
+template <int PK, int GK, bool B>
 void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
     if constexpr (GK == 2) {
-        fwd_kernel<8, PK, 2><<<grid, NT, 0, s>>>(P);
+        fwd_kernel<8, PK, 2, B><<<grid, NT, 0, s>>>(P);
     } else {
         switch (p->fwd_rv) {
             case 8:
-                if constexpr (PK == 0 && GK == 0) fwd_kernel_x2<SL1M_FWD_NPQ><<<grid, NT, 0, s>>>(P);
-                else fwd_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P);
+                if constexpr (PK == 0 && GK == 0) fwd_kernel_x2<SL1M_FWD_NPQ, B><<<grid, NT, 0, s>>>(P);
+                else fwd_kernel<8, PK, GK, B><<<grid, NT, 0, s>>>(P);
                 break;
-            case 4: fwd_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
-            case 2: fwd_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
-            default: fwd_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
+            case 4: fwd_kernel<4, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
+            case 2: fwd_kernel<2, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
+            default: fwd_kernel<1, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
         }
     }
 }
 
-template <int PK, int GK>
+template <int PK, int GK, bool B>
 void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
     switch (p->adj_rp) {
         case 8:
-            if constexpr (PK == 0 && GK == 0) adj_kernel_x2<SL1M_ADJ_NPQ><<<grid, NT, 0, s>>>(P);
-            else adj_kernel<8, PK, GK><<<grid, NT, 0, s>>>(P);
+            if constexpr (PK == 0 && GK == 0) adj_kernel_x2<SL1M_ADJ_NPQ, B><<<grid, NT, 0, s>>>(P);
+            else adj_kernel<8, PK, GK, B><<<grid, NT, 0, s>>>(P);
             break;
-        case 4: adj_kernel<4, PK, GK><<<grid, NT, 0, s>>>(P); break;
-        case 2: adj_kernel<2, PK, GK><<<grid, NT, 0, s>>>(P); break;
-        default: adj_kernel<1, PK, GK><<<grid, NT, 0, s>>>(P); break;
+        case 4: adj_kernel<4, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
+        case 2: adj_kernel<2, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
+        default: adj_kernel<1, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
     }
+}
+
+// BATCH instantiations (blockIdx.z = channel, per-channel uvw scale) only when the plan has channels.
+template <int PK, int GK>
+void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
+    if (p->chan_scale) launch_fwd_rv<PK, GK, true>(p, P, grid, s);
+    else launch_fwd_rv<PK, GK, false>(p, P, grid, s);
+}
+template <int PK, int GK>
+void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
+    if (p->chan_scale) launch_adj_rp<PK, GK, true>(p, P, grid, s);
+    else launch_adj_rp<PK, GK, false>(p, P, grid, s);
 }
 
 // forward main kernel: pix4.w must already hold a*x in sorted order; fills ws_v.

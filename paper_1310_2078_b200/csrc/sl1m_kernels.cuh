@@ -64,8 +64,15 @@ struct ApplyParams {
     size_t ws_v_stride, ws_p_stride;   // elements per channel of ws_v / ws_p
 };
 
+// BATCH is a compile-time switch: the single-channel instantiations carry no channel arithmetic at
+// all (measured: even a live fp64 scale register costs the packed forward kernel 7 %).
+template <bool BATCH>
 __device__ __forceinline__ double chan_scale_of(const ApplyParams &P) {
-    return P.chan_scale ? P.chan_scale[blockIdx.z] : 1.0;    // x * 1.0 is exact: one channel is unchanged
+    return BATCH ? P.chan_scale[blockIdx.z] : 1.0;
+}
+template <bool BATCH>
+__device__ __forceinline__ size_t chan_index() {
+    return BATCH ? (size_t)blockIdx.z : (size_t)0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -276,7 +283,7 @@ struct PolySplit {
 // forward:  ws_v[split][j] = sum_{k in split} M_jk x_k        (a1)
 // grid = (vis tiles of NT*RV, pixel splits); block = NT
 // ------------------------------------------------------------------------------------------
-template <int RV, int PK, int GK>
+template <int RV, int PK, int GK, bool BATCH = false>
 __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : (GK == 2 ? 4 : 1)) fwd_kernel(const ApplyParams P) {
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(128) float2 s_pixg[PK ? 2 : 1][PK ? TP : 1];
@@ -292,8 +299,8 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     float uf[RV], vf[RV], wf[RV], wl[RV], re[RV], im[RV];
     int ap[RV], aq[RV];
     const int jlast = P.n_vis - 1;
-    const double sc = chan_scale_of(P);
-    const float4 *pix4 = P.pix4 + (size_t)blockIdx.z * P.n_pix_pad;
+    const double sc = chan_scale_of<BATCH>(P);
+    const float4 *pix4 = P.pix4 + chan_index<BATCH>() * P.n_pix_pad;
 #pragma unroll
     for (int r = 0; r < RV; ++r) {
         const int j = min(jbase + r * NT + tid, jlast);
@@ -410,7 +417,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
         if (tid == 0 && t + 2 < t1) issue(t + 2, st);
     }
 
-    float2 *out = P.ws_v + (size_t)blockIdx.z * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
+    float2 *out = P.ws_v + chan_index<BATCH>() * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
 #pragma unroll
     for (int r = 0; r < RV; ++r) {
         const int j = jbase + r * NT + tid;
@@ -425,7 +432,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
 // every 16 terms (2 consecutive pixels x 8 visibilities) take the polynomial path; NP16 is even
 // (whole pairs).  im is accumulated with the opposite sign and negated in the epilogue.
 // ------------------------------------------------------------------------------------------
-template <int NPQ>
+template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const ApplyParams P) {
     constexpr int RV = 8, NPAIR = 4;
     // NPQ of the 16 pairs of 4 consecutive pixels take the polynomial path: pixel q gets (NPQ + 3 - q) / 4
@@ -437,8 +444,8 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
     const int t1 = min(t0 + P.per_split, P.n_tiles);
     const int jbase = blockIdx.x * (NT * RV);
     const int jlast = P.n_vis - 1;
-    const double sc = chan_scale_of(P);
-    const float4 *pix4 = P.pix4 + (size_t)blockIdx.z * P.n_pix_pad;
+    const double sc = chan_scale_of<BATCH>(P);
+    const float4 *pix4 = P.pix4 + chan_index<BATCH>() * P.n_pix_pad;
 
     f32x2 U[NPAIR], V[NPAIR], W[NPAIR], RE[NPAIR], IM[NPAIR];
 #pragma unroll
@@ -516,7 +523,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         if (tid == 0 && t + 2 < t1) issue(t + 2, st);
     }
 
-    float2 *out = P.ws_v + (size_t)blockIdx.z * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
+    float2 *out = P.ws_v + chan_index<BATCH>() * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
         float ra, rb, ia, ib;
@@ -534,7 +541,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
 // Warp w owns the 32*RP consecutive sorted pixels starting at base + w*32*RP; with RP = 8 that
 // is exactly one tile (one centre per warp), with RP <= 2 the whole CTA sits inside one tile.
 // ------------------------------------------------------------------------------------------
-template <int RP, int PK, int GK>
+template <int RP, int PK, int GK, bool BATCH = false>
 __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS : (GK == 2 ? 4 : 1)) adj_kernel(const ApplyParams P) {
     constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
     __shared__ __align__(16) float4 s_vis[2][VC];        // (u', v', w', w)
@@ -566,7 +573,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     }
 
     const int n_chunks = (P.n_vis + VC - 1) / VC;
-    const double sc = chan_scale_of(P);
+    const double sc = chan_scale_of<BATCH>(P);
     const int c0 = blockIdx.y * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
 
@@ -588,7 +595,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
             u = sc * P.u64[j];
             v = sc * P.v64[j];
             w = sc * P.w64[j];
-            rr = P.r[(size_t)blockIdx.z * P.n_vis + j];
+            rr = P.r[chan_index<BATCH>() * P.n_vis + j];
             if (GK) a = make_int2(P.ant_p[j], P.ant_q[j]);
         }
         s_vis[buf][slot] = make_float4(static_cast<float>(TWO_PI * u), static_cast<float>(TWO_PI * v),
@@ -696,7 +703,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
         __syncthreads();
     }
 
-    float *out = P.ws_p + (size_t)blockIdx.z * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
+    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
 }
@@ -708,7 +715,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
 // LDS.128 + one LDS.64 feed 8 terms.  NPQ of every 16 pairs (4 consecutive visibilities x 4
 // pairs) take the polynomial path.
 // ------------------------------------------------------------------------------------------
-template <int NPQ>
+template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const ApplyParams P) {
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
     __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre)
@@ -731,7 +738,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
     }
 
     const int n_chunks = (P.n_vis + VC - 1) / VC;
-    const double sc = chan_scale_of(P);
+    const double sc = chan_scale_of<BATCH>(P);
     const int c0 = blockIdx.y * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
 
@@ -743,7 +750,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
             u = sc * P.u64[j];
             v = sc * P.v64[j];
             w = sc * P.w64[j];
-            rr = P.r[(size_t)blockIdx.z * P.n_vis + j];
+            rr = P.r[chan_index<BATCH>() * P.n_vis + j];
         }
         const float uf = static_cast<float>(TWO_PI * u), vf = static_cast<float>(TWO_PI * v),
                     wf = static_cast<float>(TWO_PI * w);
@@ -792,7 +799,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
         __syncthreads();
     }
 
-    float *out = P.ws_p + (size_t)blockIdx.z * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
+    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
         float a, b;
