@@ -99,6 +99,7 @@ def test_config1_solver_200_iterations(sl):
     x, info = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=wl.n_iter, trace=trace)
     x = x.cpu().numpy()
     err = rel_l2(x, ref["x"])
+    print("solver image rel-L2", wl.name, err)
     assert err <= TOL_IMAGE, err
     assert np.all(x >= 0)
     assert info.n_iter_done == wl.n_iter and abs(info.L_used - L) <= 1e-6 * L
@@ -143,6 +144,7 @@ def test_config2_solver_reduced(sl):
     plan = sl.Plan.from_workload(wl)
     x, info = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=50)
     err = rel_l2(x.cpu().numpy(), ref["x"])
+    print("solver image rel-L2", wl.name, err)
     assert err <= TOL_IMAGE, err
     plan.close()
 
@@ -177,6 +179,7 @@ def test_config3_solver_reduced(sl):
     plan = sl.Plan.from_workload(wl)
     x, _ = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=25)
     err = rel_l2(x.cpu().numpy(), ref["x"])
+    print("solver image rel-L2", wl.name, err)
     assert err <= TOL_IMAGE, err
     plan.close()
 
@@ -222,6 +225,7 @@ def test_config4_solver_reduced(sl):
     plan = sl.Plan.from_workload(wl)
     x, _ = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=25)
     err = rel_l2(x.cpu().numpy(), ref["x"])
+    print("solver image rel-L2", wl.name, err)
     assert err <= TOL_IMAGE, err
     plan.close()
 
@@ -281,6 +285,7 @@ def test_config5_solver_reduced(sl):
     plan = sl.Plan.from_workload(wl)
     x, _ = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=10)
     err = rel_l2(x.cpu().numpy(), ref["x"])
+    print("solver image rel-L2", wl.name, err)
     assert err <= TOL_IMAGE, err
     plan.close()
 
