@@ -26,7 +26,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     stale = not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(d) for d in DEPS)
     if force or stale:
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [_nvcc(), *NVCC_FLAGS, "-o", tmp, SRC, SRC_QT]
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("SL1M_NVCC_EXTRA", "").split(), "-o", tmp, SRC, SRC_QT]   # SL1M_NVCC_EXTRA: tuning -D flags
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)

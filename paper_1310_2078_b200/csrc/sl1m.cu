@@ -45,6 +45,7 @@ struct sl1m_plan {
     int *vperm = nullptr;        // internal position -> caller index (-1 = padding); NULL = identity
     int n_pix_pad = 0, n_tiles = 0, n_ant = 0;
     bool gauss = false, gains = false;
+    int pk = 0;                  // pixel kind of the kernels: 0 delta, 1 Gaussian (per-pixel sigma), 2 Gaussian with one sigma per tile
     // device arrays
     double *u64 = nullptr, *v64 = nullptr, *w64 = nullptr;
     int *ant_p = nullptr, *ant_q = nullptr;
@@ -247,8 +248,6 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     p->n_ant = gains ? n_ant : 0;
     p->gauss = any_gauss;
     p->gains = gains != nullptr;
-    p->n_pix_pad = (int)(((n_pix + PIX_PAD - 1) / PIX_PAD) * PIX_PAD);
-    p->n_tiles = p->n_pix_pad / TP;
 
     try {
         // ---- Morton sort of the pixel list: consecutive runs are spatially compact ----
@@ -264,10 +263,39 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
             const uint32_t iy = (uint32_t)std::min(65535.0, (m[k] - mmin) / ext * 65535.0);
             keys[(size_t)k] = {spread16(ix) | (spread16(iy) << 1), (int)k};
         }
+        // Gaussian plans with few distinct sigma values (multi-scale layers) are sorted by
+        // sigma class first, each class padded to whole tiles: every tile then has ONE sigma, which
+        // makes q = w sigma^2, 1/(1+q^2) and the exponent scale per-(visibility, tile) constants
+        // instead of per-term work (kernels with PK == 2).  Otherwise plain Morton order (PK == 1).
+        std::vector<double> classes;
+        if (any_gauss) {
+            for (int64_t k = 0; k < n_pix && classes.size() <= 16; ++k)
+                if (std::find(classes.begin(), classes.end(), sigma[k]) == classes.end()) classes.push_back(sigma[k]);
+            if (classes.size() > 16) classes.clear();
+            std::sort(classes.begin(), classes.end());
+        }
+        const bool by_class = !classes.empty() && !gains;
+        auto class_of = [&](int k) -> int {
+            return by_class ? (int)(std::find(classes.begin(), classes.end(), sigma[k]) - classes.begin()) : 0;
+        };
         std::stable_sort(keys.begin(), keys.end(),
-                         [](const std::pair<uint32_t, int> &a, const std::pair<uint32_t, int> &b) {
-                             return a.first < b.first;
+                         [&](const std::pair<uint32_t, int> &a, const std::pair<uint32_t, int> &b) {
+                             const int ca = class_of(a.second), cb = class_of(b.second);
+                             return ca != cb ? ca < cb : a.first < b.first;
                          });
+        // slots: sorted position -> caller pixel, -1 on padding (class boundaries and the tail)
+        std::vector<int> slots;
+        slots.reserve((size_t)n_pix + (classes.size() + 1) * TP + PIX_PAD);
+        for (size_t i = 0; i < keys.size(); ++i) {
+            if (by_class && i > 0 && class_of(keys[i].second) != class_of(keys[i - 1].second))
+                while (slots.size() % TP) slots.push_back(-1);
+            slots.push_back(keys[i].second);
+        }
+        while (slots.size() % PIX_PAD) slots.push_back(-1);
+        if (slots.size() > ((size_t)1 << 30)) return fail(SL1M_ERR_SIZE, "padded pixel count beyond 2^30");
+        p->n_pix_pad = (int)slots.size();
+        p->n_tiles = p->n_pix_pad / TP;
+        p->pk = any_gauss ? (by_class ? 2 : 1) : 0;
 
         // ---- per-tile fp64 centres, per-pixel fp32 offsets (step a0) ----
         const size_t npad = (size_t)p->n_pix_pad;
@@ -278,30 +306,33 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         std::vector<int> perm(npad, -1);
         const double PI = 3.14159265358979323846, LOG2E = 1.4426950408889634074;
         for (int t = 0; t < p->n_tiles; ++t) {
-            const int64_t k0 = (int64_t)t * TP, k1 = std::min<int64_t>(k0 + TP, n_pix);
-            if (k0 >= n_pix) break;
-            double a0 = 1e300, a1 = -1e300, b0 = 1e300, b1 = -1e300;
-            for (int64_t s = k0; s < k1; ++s) {
-                const int k = keys[(size_t)s].second;
+            const size_t k0 = (size_t)t * TP, k1 = k0 + TP;
+            double a0 = 1e300, a1 = -1e300, b0 = 1e300, b1 = -1e300, sig_tile = 0.0;
+            for (size_t s = k0; s < k1; ++s) {
+                const int k = slots[s];
+                if (k < 0) continue;
                 a0 = std::min(a0, l[k]); a1 = std::max(a1, l[k]);
                 b0 = std::min(b0, m[k]); b1 = std::max(b1, m[k]);
+                if (sigma) sig_tile = sigma[k];
             }
+            if (a0 > a1) continue;   // a tile of padding only
             const double lc = 0.5 * (a0 + a1), mc = 0.5 * (b0 + b1);
             const double rc2 = lc * lc + mc * mc;
             const double nc = -rc2 / (1.0 + std::sqrt(1.0 - rc2));   // n - 1 at the centre
-            cen[(size_t)t] = make_double4(lc, mc, nc, 0.0);
-            for (int64_t s = k0; s < k1; ++s) {
-                const int k = keys[(size_t)s].second;
+            cen[(size_t)t] = make_double4(lc, mc, nc, sig_tile * sig_tile);   // .w = sigma^2 of the tile (PK == 2)
+            for (size_t s = k0; s < k1; ++s) {
+                const int k = slots[s];
+                if (k < 0) continue;
                 const double r2 = l[k] * l[k] + m[k] * m[k];
                 const double n = std::sqrt(1.0 - r2);
                 const double sg = sigma ? sigma[k] : 0.0;
                 // eq (9)/(17): n' = n - 1 (cancellation-free); eq (16): n' = -r^2/2; sigma == 0 => eq (9)
                 const double npr = (sg > 0.0 && gauss_model == SL1M_GAUSS_PARAXIAL) ? -0.5 * r2
                                                                                      : -r2 / (1.0 + n);
-                pix4[(size_t)s] = make_float4((float)(l[k] - lc), (float)(m[k] - mc), (float)(npr - nc), 0.f);
-                amp[(size_t)s] = (float)(1.0 / n);
-                perm[(size_t)s] = k;
-                if (any_gauss) pixg[(size_t)s] = make_float2((float)(sg * sg), (float)(-PI * LOG2E * sg * sg));
+                pix4[s] = make_float4((float)(l[k] - lc), (float)(m[k] - mc), (float)(npr - nc), 0.f);
+                amp[s] = (float)(1.0 / n);
+                perm[s] = k;
+                if (any_gauss) pixg[s] = make_float2((float)(sg * sg), (float)(-PI * LOG2E * sg * sg));
             }
         }
 
@@ -470,8 +501,9 @@ void launch_fwd(sl1m_plan *p, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->fwd_per_split;
     dim3 grid(p->fwd_vtiles, p->fwd_split, p->n_chan);
-    const int key = (p->gauss ? 3 : 0) + p->gk;
+    const int key = p->pk * 3 + p->gk;   // pk == 2 (one sigma per tile) only exists with unit gains
     switch (key) {
+        case 6: launch_fwd_rv<2, 0>(p, P, grid, s); break;
         case 0: launch_fwd_rv<0, 0>(p, P, grid, s); break;
         case 1: launch_fwd_rv<0, 1>(p, P, grid, s); break;
         case 2: launch_fwd_rv<0, 2>(p, P, grid, s); break;
@@ -488,8 +520,9 @@ void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
     P.per_split = p->adj_per_split;
     P.r = r;
     dim3 grid(p->adj_pgroups, p->adj_split, p->n_chan);
-    const int key = (p->gauss ? 3 : 0) + p->gk;
+    const int key = p->pk * 3 + p->gk;
     switch (key) {
+        case 6: launch_adj_rp<2, 0>(p, P, grid, s); break;
         case 0: launch_adj_rp<0, 0>(p, P, grid, s); break;
         case 1: launch_adj_rp<0, 1>(p, P, grid, s); break;
         case 2: launch_adj_rp<0, 2>(p, P, grid, s); break;
@@ -857,7 +890,8 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     const bool plain = !pk && p->gk == 0;          // delta pixels, unit gains
     o->fwd_poly_per16 = !plain ? 0 : (p->fwd_rv == 8 ? SL1M_FWD_NPQ : (p->fwd_rv == 4 ? (SL1M_FWD_NPOLY8 / 2) * 4 : 0));
     o->adj_poly_per16 = !plain ? 0 : (p->adj_rp == 8 ? SL1M_ADJ_NPQ : (p->adj_rp == 4 ? (SL1M_ADJ_NPOLY8 / 2) * 4 : 0));
-    o->mufu_per_term_mufu_path = pk ? 4 : 2;
+    o->mufu_per_term_mufu_path = p->pk == 2 ? 3 : (pk ? 4 : 2);
+    o->gaussian = p->pk;
     o->fwd_packed_pairs = plain && p->fwd_rv == 8;
     o->adj_packed_pairs = plain && p->adj_rp == 8;
     return SL1M_OK;

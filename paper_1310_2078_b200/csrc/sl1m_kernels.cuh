@@ -246,6 +246,38 @@ __device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, 
     }
 }
 
+// Gaussian pixels with ONE sigma per tile (PK == 2): everything that depends only on (visibility, tile)
+// is hoisted out of the term.  With q = w s^2, den = 1 + q^2:
+//   E' = s2 * cE + lr,  cE = -pi log2(e) s^2 / den,  lr = log2(1/den)   =>  2^E' = e^A / den
+//   X' = X - q A = (X + q ln2 lr) - q ln2 E'                              (the lr part is folded into x0)
+//   entry = 2^E' (1 + i q)(cos X' - i sin X')
+// per term: 15 FP32 + 3 MUFU (ex2, sin, cos) instead of 20 + 4.
+__device__ __forceinline__ void gauss_tile_constants(double w, double sig2, float &q, float &cE, float &lr,
+                                                     float &x0) {
+    const double qd = w * sig2;
+    const double rden = 1.0 / (1.0 + qd * qd);
+    q = static_cast<float>(qd);
+    cE = static_cast<float>(-3.14159265358979323846 * 1.4426950408889634074 * sig2 * rden);
+    const double lrd = log2(rden);
+    lr = static_cast<float>(lrd);
+    // fold q ln2 lr into the centre phase, reduced again to [-pi, pi]
+    double t = (static_cast<double>(x0) + 0.69314718055994530942 * qd * lrd) * (1.0 / TWO_PI);
+    t -= rint(t);
+    x0 = static_cast<float>(t * TWO_PI);
+}
+// entry = amp (cr + i ci); the caller folds amp into its own multiplier (a x, or nothing)
+__device__ __forceinline__ void gen_entry_tile(float X, float du, float dv, float q, float cE, float lr,
+                                               float &amp, float &cr, float &ci) {
+    const float s2 = fmaf(dv, dv, du * du);
+    const float Ep = fmaf(s2, cE, lr);
+    const float Xp = fmaf(-0.69314718056f * q, Ep, X);   // -ln2 q is loop-invariant: hoisted by the compiler
+    amp = ex2_approx(Ep);
+    float s, c;
+    __sincosf(Xp, &s, &c);
+    cr = fmaf(q, s, c);                                   // Re (1 + i q)(c - i s)
+    ci = fmaf(q, c, -s);                                  // Im
+}
+
 // Tuning constants of the delta-pixel / unit-gain kernels (measured on B200):
 //   *_NPOLY8   how many of a thread's 8 register-tile entries take the polynomial sincos path
 //   *_MIN_CTAS resident CTAs per SM the kernel is compiled for (register budget 65536/(128*n))
@@ -261,6 +293,13 @@ __device__ __forceinline__ void gen_entry(float X, float du, float dv, float w, 
 #endif
 #ifndef SL1M_ADJ_NPQ
 #define SL1M_ADJ_NPQ 4
+#endif
+//   *_GT_MIN_CTAS  the one-sigma-per-tile Gaussian kernels (PK == 2)
+#ifndef SL1M_FWD_GT_MIN_CTAS
+#define SL1M_FWD_GT_MIN_CTAS 4
+#endif
+#ifndef SL1M_ADJ_GT_MIN_CTAS
+#define SL1M_ADJ_GT_MIN_CTAS 5
 #endif
 #ifndef SL1M_FWD_X2_MIN_CTAS
 #define SL1M_FWD_X2_MIN_CTAS 4
@@ -284,9 +323,9 @@ struct PolySplit {
 // grid = (vis tiles of NT*RV, pixel splits); block = NT
 // ------------------------------------------------------------------------------------------
 template <int RV, int PK, int GK, bool BATCH = false>
-__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : (GK == 2 ? 4 : 1)) fwd_kernel(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : (GK == 2 ? 4 : (PK == 2 ? SL1M_FWD_GT_MIN_CTAS : 1))) fwd_kernel(const ApplyParams P) {
     __shared__ __align__(128) float4 s_pix[2][TP];
-    __shared__ __align__(128) float2 s_pixg[PK ? 2 : 1][PK ? TP : 1];
+    __shared__ __align__(128) float2 s_pixg[PK == 1 ? 2 : 1][PK == 1 ? TP : 1];
     __shared__ __align__(8) uint64_t s_bar[2];
 
     const int tid = threadIdx.x;
@@ -320,7 +359,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     // entries are samples of ONE baseline (p, q): the gain product G is loaded once per pixel.
     static_assert(GK != 2 || RV == 8, "grouped gains need RV == 8");
 
-    constexpr uint32_t kBytes = TP * sizeof(float4) + (PK ? TP * sizeof(float2) : 0);
+    constexpr uint32_t kBytes = TP * sizeof(float4) + (PK == 1 ? TP * sizeof(float2) : 0);
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
@@ -330,7 +369,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     auto issue = [&](int t, int st) {
         mbar_expect_tx(&s_bar[st], kBytes);
         tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
-        if (PK) tma_bulk_g2s(&s_pixg[st][0], P.pixg + (size_t)t * TP, TP * sizeof(float2), &s_bar[st]);
+        if (PK == 1) tma_bulk_g2s(&s_pixg[st][0], P.pixg + (size_t)t * TP, TP * sizeof(float2), &s_bar[st]);
     };
     if (tid == 0) {
         if (t0 < t1) issue(t0, 0);
@@ -342,6 +381,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
         const uint32_t parity = ((t - t0) >> 1) & 1;
         const double4 c = P.cen[t];
         float x0[RV], uc[RV], vc[RV];
+        float tq[PK == 2 ? RV : 1], tcE[PK == 2 ? RV : 1], tlr[PK == 2 ? RV : 1];   // per-(visibility, tile) constants
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
             const int j = min(jbase + r * NT + tid, jlast);
@@ -351,6 +391,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 uc[r] = static_cast<float>(ud - wd * c.x);
                 vc[r] = static_cast<float>(vd - wd * c.y);
             }
+            if (PK == 2) gauss_tile_constants(wd, c.w, tq[r], tcE[r], tlr[r], x0[r]);
         }
         mbar_wait(&s_bar[st], parity);
         const float2 *gbase = GK ? P.gF + (size_t)t * TP * P.n_ant : nullptr;
@@ -377,7 +418,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 Gwi = px.w * fmaf(gp.y, gq.x, -gp.x * gq.y);
             }
             float sig2 = 0.f, nsp = 0.f;
-            if (PK) {
+            if (PK == 1) {
                 const float2 pg = s_pixg[st][p];
                 sig2 = pg.x;
                 nsp = pg.y;
@@ -392,6 +433,14 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 }
                 float ere, eim;
                 uint32_t sgn;
+                if (PK == 2) {
+                    float amp;
+                    gen_entry_tile(X, du, dv, tq[r], tcE[r], tlr[r], amp, ere, eim);
+                    const float t = px.w * amp;
+                    re[r] = fmaf(t, ere, re[r]);
+                    im[r] = fmaf(t, eim, im[r]);
+                    continue;
+                }
                 if (r < PolySplit<RV, PK, GK, SL1M_FWD_NPOLY8>::N) gen_entry<PK, true>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
                 else gen_entry<PK, false>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
                 const float wt = (r < PolySplit<RV, PK, GK, SL1M_FWD_NPOLY8>::N) ? fxor(px.w, sgn) : px.w;
@@ -542,12 +591,13 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
 // is exactly one tile (one centre per warp), with RP <= 2 the whole CTA sits inside one tile.
 // ------------------------------------------------------------------------------------------
 template <int RP, int PK, int GK, bool BATCH = false>
-__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS : (GK == 2 ? 4 : 1)) adj_kernel(const ApplyParams P) {
+__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS : (GK == 2 ? 4 : (PK == 2 ? SL1M_ADJ_GT_MIN_CTAS : 1))) adj_kernel(const ApplyParams P) {
     constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
     __shared__ __align__(16) float4 s_vis[2][VC];        // (u', v', w', w)
     __shared__ __align__(8) float2 s_r[2][VC];           // residual (re, im)
     __shared__ float s_x0[2][VC][NCEN];
     __shared__ __align__(8) float2 s_uc[PK ? 2 : 1][PK ? VC : 1][PK ? NCEN : 1];
+    __shared__ __align__(16) float4 s_tc[PK == 2 ? 2 : 1][PK == 2 ? VC : 1][PK == 2 ? NCEN : 1];   // (q, cE, lr, x0')
     __shared__ __align__(8) int2 s_ant[GK ? 2 : 1][GK ? VC : 1];   // GK == 2 uses the first VC/8 only
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -565,7 +615,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
         dm[i] = px.y;
         dn[i] = px.z;
         acc[i] = 0.f;
-        if (PK) {
+        if (PK == 1) {
             const float2 pg = P.pixg[k];
             sig2[i] = pg.x;
             nsp[i] = pg.y;
@@ -606,10 +656,16 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
 #pragma unroll
         for (int c = 0; c < NCEN; ++c) {
             const double4 cen = P.cen[tile0 + c];   // L1-resident; not worth 24 registers
-            s_x0[buf][slot][c] = centre_phase(u, v, w, cen);
+            float x0c = centre_phase(u, v, w, cen);
             if (PK)
                 s_uc[buf][slot][c] = make_float2(static_cast<float>(u - w * cen.x),
                                                  static_cast<float>(v - w * cen.y));
+            if (PK == 2) {
+                float q, cE, lr;
+                gauss_tile_constants(w, cen.w, q, cE, lr, x0c);
+                s_tc[buf][slot][c] = make_float4(q, cE, lr, x0c);
+            }
+            s_x0[buf][slot][c] = x0c;
         }
     };
 
@@ -649,6 +705,8 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
             const float4 vv = s_vis[buf][t];
             const float2 rr = s_r[buf][t];
             const float x0 = s_x0[buf][t][mycen];
+            float4 tc = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (PK == 2) tc = s_tc[buf][t][mycen];
             float ucx = 0.f, ucy = 0.f;
             if (PK) {
                 const float2 uc = s_uc[buf][t][mycen];
@@ -671,6 +729,12 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 }
                 float ere, eim;
                 uint32_t sgn;
+                if (PK == 2) {   // one sigma per tile: Re conj(M / a) r = amp (cr r_re + ci r_im)
+                    float amp;
+                    gen_entry_tile(X, du, dv, tc.x, tc.y, tc.z, amp, ere, eim);
+                    acc[i] = fmaf(amp, fmaf(eim, rr.y, ere * rr.x), acc[i]);
+                    continue;
+                }
                 if (i < PolySplit<RP, PK, GK, SL1M_ADJ_NPOLY8>::N) {
                     gen_entry<PK, true>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim, sgn);
                     ere = fxor(ere, sgn);

@@ -198,3 +198,34 @@ def test_error_paths(sl):
     assert lib.sl1m_forward(None, None, None, None) == 1           # SL1M_ERR_NULL
     lib.sl1m_destroy(None)                                          # NULL-safe
     plan.close()
+
+
+@pytest.mark.parametrize("model", [1, 0])
+def test_sigma_classes_one_sigma_per_tile_path(sl, model):
+    """Plans with at most 16 distinct sigma values (multi-scale layers) are sorted by sigma
+    class and use the one-sigma-per-tile kernels (describe()['gaussian'] == 2): ragged class sizes (padding
+    inside the sorted list), a sigma = 0 class (eq 9, reading R15), large defocus q = w sigma^2 ~ 1, the
+    solver on top, and the same list with 40 distinct sigmas falling back to the per-pixel kernels (== 1)."""
+    import torch
+    rng = np.random.default_rng(79 + model)
+    n_vis, n_pix = 1300, 3001
+    uvw = rng.uniform(-1, 1, (n_vis, 3)) * np.array([300.0, 300.0, 9000.0])
+    l = rng.uniform(-0.03, 0.03, n_pix)
+    m = rng.uniform(-0.03, 0.03, n_pix)
+    values = np.array([0.0, 4e-4, 1.7e-3, 6e-3, 1.1e-2])
+    sigma = values[rng.choice(5, n_pix, p=[0.05, 0.5, 0.3, 0.1, 0.05])]
+    x = rng.uniform(0, 1, n_pix).astype(np.float32)
+    r = (rng.standard_normal(n_vis) + 1j * rng.standard_normal(n_vis)).astype(np.complex64)
+    for sg, want_pk in ((sigma, 2), (sigma * rng.choice(np.linspace(0.9, 1.1, 40), n_pix), 1)):
+        o = oracle.Oracle(uvw, l, m, sg, gauss_model=model)
+        plan = sl.Plan(uvw, l, m, sg, gauss_model=model)
+        assert plan.describe()["gaussian"] == want_pk
+        assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x)) <= 2e-4
+        assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r)) <= 2e-4
+        if want_pk == 2:
+            V = (o.forward(x) + 0.05 * r).astype(np.complex64)
+            L = o.max_eig(20) * 1.05
+            assert abs(plan.max_eig(20) * 1.05 - L) <= 1e-4 * L
+            xs, _ = plan.solve(_dev(V, torch.complex64), 0.3, L=L, n_iter=30)
+            assert rel_l2(xs.cpu().numpy(), o.fista(V, 0.3, L, 30)["x"]) <= 1e-3
+        plan.close()
