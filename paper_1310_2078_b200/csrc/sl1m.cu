@@ -457,7 +457,8 @@ inline dim3 cgrid(const sl1m_plan *p, size_t n) { return dim3((unsigned)egrid(n)
 template <int PK, int GK, bool B>
 void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
     if constexpr (GK == 2) {
-        fwd_kernel<8, PK, 2, B><<<grid, NT, 0, s>>>(P);
+        if constexpr (PK == 0) fwd_kernel_x2<SL1M_FWD_G2_NPQ, B, true><<<grid, NT, 0, s>>>(P);
+        else fwd_kernel<8, PK, 2, B><<<grid, NT, 0, s>>>(P);
     } else {
         switch (p->fwd_rv) {
             case 8:
@@ -476,6 +477,7 @@ void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
     switch (p->adj_rp) {
         case 8:
             if constexpr (PK == 0 && GK == 0) adj_kernel_x2<SL1M_ADJ_NPQ, B><<<grid, NT, 0, s>>>(P);
+            else if constexpr (PK == 0 && GK == 2) adj_kernel_g2x2<SL1M_ADJ_G2_NPQ, B><<<grid, NT, 0, s>>>(P);
             else adj_kernel<8, PK, GK, B><<<grid, NT, 0, s>>>(P);
             break;
         case 4: adj_kernel<4, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
@@ -888,12 +890,15 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->adj_chunks_per_split = p->adj_per_split;
     const int pk = p->gauss ? 1 : 0;
     const bool plain = !pk && p->gk == 0;          // delta pixels, unit gains
-    o->fwd_poly_per16 = !plain ? 0 : (p->fwd_rv == 8 ? SL1M_FWD_NPQ : (p->fwd_rv == 4 ? (SL1M_FWD_NPOLY8 / 2) * 4 : 0));
-    o->adj_poly_per16 = !plain ? 0 : (p->adj_rp == 8 ? SL1M_ADJ_NPQ : (p->adj_rp == 4 ? (SL1M_ADJ_NPOLY8 / 2) * 4 : 0));
+    const bool grouped = !pk && p->gk == 2;        // delta pixels, baseline-grouped gains
+    o->fwd_poly_per16 = plain ? (p->fwd_rv == 8 ? SL1M_FWD_NPQ : (p->fwd_rv == 4 ? (SL1M_FWD_NPOLY8 / 2) * 4 : 0))
+                              : (grouped ? SL1M_FWD_G2_NPQ : 0);
+    o->adj_poly_per16 = plain ? (p->adj_rp == 8 ? SL1M_ADJ_NPQ : (p->adj_rp == 4 ? (SL1M_ADJ_NPOLY8 / 2) * 4 : 0))
+                              : (grouped && p->adj_rp == 8 ? SL1M_ADJ_G2_NPQ : 0);
     o->mufu_per_term_mufu_path = p->pk == 2 ? 3 : (pk ? 4 : 2);
     o->gaussian = p->pk;
-    o->fwd_packed_pairs = plain && p->fwd_rv == 8;
-    o->adj_packed_pairs = plain && p->adj_rp == 8;
+    o->fwd_packed_pairs = (plain && p->fwd_rv == 8) || grouped;
+    o->adj_packed_pairs = (plain || grouped) && p->adj_rp == 8;
     return SL1M_OK;
 }
 

@@ -301,6 +301,13 @@ __device__ __forceinline__ void gen_entry_tile(float X, float du, float dv, floa
 #ifndef SL1M_ADJ_GT_MIN_CTAS
 #define SL1M_ADJ_GT_MIN_CTAS 5
 #endif
+//   *_G2_NPQ   the same fraction for the packed kernels with baseline-grouped gains
+#ifndef SL1M_FWD_G2_NPQ
+#define SL1M_FWD_G2_NPQ 4
+#endif
+#ifndef SL1M_ADJ_G2_NPQ
+#define SL1M_ADJ_G2_NPQ 4
+#endif
 #ifndef SL1M_FWD_X2_MIN_CTAS
 #define SL1M_FWD_X2_MIN_CTAS 4
 #endif
@@ -481,7 +488,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
 // every 16 terms (2 consecutive pixels x 8 visibilities) take the polynomial path; NP16 is even
 // (whole pairs).  im is accumulated with the opposite sign and negated in the epilogue.
 // ------------------------------------------------------------------------------------------
-template <int NPQ, bool BATCH = false>
+template <int NPQ, bool BATCH = false, bool GAINS = false>
 __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const ApplyParams P) {
     constexpr int RV = 8, NPAIR = 4;
     // NPQ of the 16 pairs of 4 consecutive pixels take the polynomial path: pixel q gets (NPQ + 3 - q) / 4
@@ -506,6 +513,14 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         RE[i] = pk2(0.f, 0.f);
         IM[i] = pk2(0.f, 0.f);
     }
+    // GAINS ("baseline-grouped" plan, gk == 2): the thread's 8 visibilities are samples of ONE baseline
+    // (p, q), so G = g_p conj(g_q) is formed once per pixel and shared by the 4 pairs.
+    int ap = 0, aq = 0;
+    if (GAINS) {
+        const int j0 = min(jbase + tid, jlast);
+        ap = P.ant_p[j0];
+        aq = P.ant_q[j0];
+    }
 
     constexpr uint32_t kBytes = TP * sizeof(float4);
     if (tid == 0) {
@@ -524,12 +539,35 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
     }
 
     // one pixel against the 4 pairs; the first NPOLY pairs use the FMA-pipe polynomial
-    auto pixel = [&](const float4 px, const f32x2 (&X0)[NPAIR], auto npoly_tag) {
+    auto pixel = [&](const float4 px, const f32x2 (&X0)[NPAIR], auto npoly_tag, float Gwr, float Gwi) {
         constexpr int NPOLY = decltype(npoly_tag)::value;
         const f32x2 pxx = bc2(px.x), pxy = bc2(px.y), pxz = bc2(px.z);
 #pragma unroll
         for (int i = 0; i < NPAIR; ++i) {
             const f32x2 X = fma2(U[i], pxx, fma2(V[i], pxy, fma2(W[i], pxz, X0[i])));
+            if (GAINS) {
+                // (a x G)(c - i s):  RE += Gwr c + Gwi s,   IM (negated, as below) += Gwr s - Gwi c
+                f32x2 s, c;
+                if (i < NPOLY) {
+                    uint32_t ka, kb;
+                    sincos_poly2(X, s, c, ka, kb);
+                    float sa, sb, ca, cb;
+                    up2(s, sa, sb);
+                    up2(c, ca, cb);
+                    s = pk2(flip_if_odd(sa, ka), flip_if_odd(sb, kb));
+                    c = pk2(flip_if_odd(ca, ka), flip_if_odd(cb, kb));
+                } else {
+                    float xa, xb, sa, ca, sb, cb;
+                    up2(X, xa, xb);
+                    __sincosf(xa, &sa, &ca);
+                    __sincosf(xb, &sb, &cb);
+                    s = pk2(sa, sb);
+                    c = pk2(ca, cb);
+                }
+                RE[i] = fma2(bc2(Gwr), c, fma2(bc2(Gwi), s, RE[i]));
+                IM[i] = fma2(bc2(Gwr), s, fma2(bc2(-Gwi), c, IM[i]));
+                continue;
+            }
             if (i < NPOLY) {
                 f32x2 s, c;
                 uint32_t ka, kb;
@@ -561,12 +599,40 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
                         centre_phase(sc * __ldg(P.u64 + jb), sc * __ldg(P.v64 + jb), sc * __ldg(P.w64 + jb), c));
         }
         mbar_wait(&s_bar[st], parity);
+        if (GAINS) {
+            // gain rows of the tile, gF[k][a]: register prefetch 4 pixels ahead (cold in L1 on first touch)
+            const float2 *gbase = P.gF + (size_t)t * TP * P.n_ant;
+            float2 gp[4], gq[4];
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                gp[d] = __ldg(gbase + (size_t)d * P.n_ant + ap);
+                gq[d] = __ldg(gbase + (size_t)d * P.n_ant + aq);
+            }
 #pragma unroll 1
-        for (int p = 0; p < TP; p += 4) {
-            pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{});
-            pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{});
-            pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{});
-            pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{});
+            for (int p = 0; p < TP; p += 4) {
+                float Gwr[4], Gwi[4];
+#pragma unroll
+                for (int d = 0; d < 4; ++d) {
+                    const float w = s_pix[st][p + d].w;
+                    Gwr[d] = w * fmaf(gp[d].y, gq[d].y, gp[d].x * gq[d].x);    // a x Re(g_p conj g_q)
+                    Gwi[d] = w * fmaf(gp[d].y, gq[d].x, -gp[d].x * gq[d].y);
+                    const int pn = min(p + 4 + d, TP - 1);
+                    gp[d] = __ldg(gbase + (size_t)pn * P.n_ant + ap);
+                    gq[d] = __ldg(gbase + (size_t)pn * P.n_ant + aq);
+                }
+                pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, Gwr[0], Gwi[0]);
+                pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, Gwr[1], Gwi[1]);
+                pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, Gwr[2], Gwi[2]);
+                pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{}, Gwr[3], Gwi[3]);
+            }
+        } else {
+#pragma unroll 1
+            for (int p = 0; p < TP; p += 4) {
+                pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, 0.f, 0.f);
+                pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, 0.f, 0.f);
+                pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, 0.f, 0.f);
+                pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{}, 0.f, 0.f);
+            }
         }
         __syncthreads();  // every thread is done with stage st
         if (tid == 0 && t + 2 < t1) issue(t + 2, st);
@@ -859,6 +925,150 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
             visibility(s_vc[buf][mycen][t + 1], s_r[buf][t + 1], std::integral_constant<int, (NPQ + 2) / 4>{});
             visibility(s_vc[buf][mycen][t + 2], s_r[buf][t + 2], std::integral_constant<int, (NPQ + 1) / 4>{});
             visibility(s_vc[buf][mycen][t + 3], s_r[buf][t + 3], std::integral_constant<int, NPQ / 4>{});
+        }
+        __syncthreads();
+    }
+
+    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        float a, b;
+        up2(ACC[i], a, b);
+        out[kfirst + (2 * i) * 32 + lane] = a;
+        out[kfirst + (2 * i + 1) * 32 + lane] = b;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// adjoint, delta pixels, baseline-grouped gains (gk == 2), packed-pair variant (RP = 8).
+// A chunk is 16 baseline groups x 8 samples, staged group-major.  Per group the thread forms
+// G_i = g_p(i) conj(g_q(i)) for its 8 pixels once (next group's gain rows prefetched), accumulates
+// Z_i = sum_samples conj(e) r over the 8 samples, then acc_i += Re(conj(G_i) Z_i).
+// ------------------------------------------------------------------------------------------
+#ifndef SL1M_ADJ_G2X2_MIN_CTAS
+#define SL1M_ADJ_G2X2_MIN_CTAS 4
+#endif
+template <int NPQ, bool BATCH = false>
+__global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(const ApplyParams P) {
+    constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP, NG = VC / 8;
+    __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre), slot = group * 8 + sample
+    __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, r_im)
+    __shared__ __align__(8) int2 s_ant[2][NG];           // the group's (p, q)
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int base = blockIdx.x * (NT * RP);
+    const int kfirst = base + warp * (32 * RP);
+    const int tile0 = base / TP;
+    const int mycen = (kfirst / TP) - tile0;
+
+    f32x2 DL[NPAIR], DM[NPAIR], DN[NPAIR], ACC[NPAIR];
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        const float4 pa = P.pix4[kfirst + (2 * i) * 32 + lane], pb = P.pix4[kfirst + (2 * i + 1) * 32 + lane];
+        DL[i] = pk2(pa.x, pb.x);
+        DM[i] = pk2(pa.y, pb.y);
+        DN[i] = pk2(pa.z, pb.z);
+        ACC[i] = pk2(0.f, 0.f);
+    }
+
+    const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const double sc = chan_scale_of<BATCH>(P);
+    const int c0 = blockIdx.y * P.per_split;
+    const int c1 = min(c0 + P.per_split, n_chunks);
+
+    // the plan stores sample r of group g at (g / 128) * 1024 + r * 128 + g % 128 (the forward's thread layout)
+    auto stage = [&](int chunk, int buf) {
+        const int g = chunk * NG + (tid & 15), r = tid >> 4;
+        const int j = (g >> 7) * (NT * 8) + r * NT + (g & 127);
+        const int slot = (tid & 15) * 8 + r;
+        double u = 0.0, v = 0.0, w = 0.0;
+        float2 rr = make_float2(0.f, 0.f);
+        int2 a = make_int2(0, 0);
+        if (j < P.n_vis) {
+            u = sc * P.u64[j];
+            v = sc * P.v64[j];
+            w = sc * P.w64[j];
+            rr = P.r[chan_index<BATCH>() * P.n_vis + j];
+            a = make_int2(P.ant_p[j], P.ant_q[j]);
+        }
+        const float uf = static_cast<float>(TWO_PI * u), vf = static_cast<float>(TWO_PI * v),
+                    wf = static_cast<float>(TWO_PI * w);
+        s_r[buf][slot] = rr;
+        if (tid < NG) s_ant[buf][tid] = a;   // sample 0 carries the group's (p, q)
+#pragma unroll
+        for (int c = 0; c < NCEN; ++c)
+            s_vc[buf][c][slot] = make_float4(uf, vf, wf, centre_phase(u, v, w, P.cen[tile0 + c]));
+    };
+
+    auto load_gains = [&](int2 a, float2 (&gp)[RP], float2 (&gq)[RP]) {
+#pragma unroll
+        for (int i = 0; i < RP; ++i) {
+            gp[i] = __ldg(P.gA + (size_t)a.x * P.n_pix_pad + kfirst + lane + i * 32);
+            gq[i] = __ldg(P.gA + (size_t)a.y * P.n_pix_pad + kfirst + lane + i * 32);
+        }
+    };
+
+    f32x2 ZR[NPAIR], ZI[NPAIR];
+    auto visibility = [&](const float4 vv, const float2 rr, auto npoly_tag) {
+        constexpr int NPOLY = decltype(npoly_tag)::value;
+        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z), x0 = bc2(vv.w);
+        const f32x2 rre = bc2(rr.x), rim = bc2(rr.y), nrim = bc2(-rr.y);
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i) {
+            const f32x2 X = fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, x0)));
+            f32x2 s, c;
+            if (i < NPOLY) {
+                uint32_t ka, kb;
+                sincos_poly2(X, s, c, ka, kb);
+                float sa, sb, ca, cb;
+                up2(s, sa, sb);
+                up2(c, ca, cb);
+                s = pk2(flip_if_odd(sa, ka), flip_if_odd(sb, kb));
+                c = pk2(flip_if_odd(ca, ka), flip_if_odd(cb, kb));
+            } else {
+                float xa, xb, sa, ca, sb, cb;
+                up2(X, xa, xb);
+                __sincosf(xa, &sa, &ca);
+                __sincosf(xb, &sb, &cb);
+                s = pk2(sa, sb);
+                c = pk2(ca, cb);
+            }
+            // z = conj(e) r = (c + i s)(r_re + i r_im)
+            ZR[i] = fma2(c, rre, fma2(s, nrim, ZR[i]));
+            ZI[i] = fma2(c, rim, fma2(s, rre, ZI[i]));
+        }
+    };
+
+    if (c0 < c1) stage(c0, 0);
+    __syncthreads();
+    for (int ch = c0; ch < c1; ++ch) {
+        const int buf = (ch - c0) & 1;
+        if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
+        float2 gp[RP], gq[RP];
+        load_gains(s_ant[buf][0], gp, gq);
+#pragma unroll 1
+        for (int g = 0; g < NG; ++g) {
+            f32x2 GR[NPAIR], GI[NPAIR];
+#pragma unroll
+            for (int i = 0; i < NPAIR; ++i) {
+                const float2 pa = gp[2 * i], qa = gq[2 * i], pb = gp[2 * i + 1], qb = gq[2 * i + 1];
+                GR[i] = pk2(fmaf(pa.y, qa.y, pa.x * qa.x), fmaf(pb.y, qb.y, pb.x * qb.x));      // Re g_p conj g_q
+                GI[i] = pk2(fmaf(pa.y, qa.x, -pa.x * qa.y), fmaf(pb.y, qb.x, -pb.x * qb.y));    // Im
+                ZR[i] = pk2(0.f, 0.f);
+                ZI[i] = pk2(0.f, 0.f);
+            }
+            load_gains(s_ant[buf][min(g + 1, NG - 1)], gp, gq);   // next group's rows
+            const int t = g * 8;
+            visibility(s_vc[buf][mycen][t], s_r[buf][t], std::integral_constant<int, (NPQ + 3) / 4>{});
+            visibility(s_vc[buf][mycen][t + 1], s_r[buf][t + 1], std::integral_constant<int, (NPQ + 2) / 4>{});
+            visibility(s_vc[buf][mycen][t + 2], s_r[buf][t + 2], std::integral_constant<int, (NPQ + 1) / 4>{});
+            visibility(s_vc[buf][mycen][t + 3], s_r[buf][t + 3], std::integral_constant<int, NPQ / 4>{});
+            visibility(s_vc[buf][mycen][t + 4], s_r[buf][t + 4], std::integral_constant<int, (NPQ + 3) / 4>{});
+            visibility(s_vc[buf][mycen][t + 5], s_r[buf][t + 5], std::integral_constant<int, (NPQ + 2) / 4>{});
+            visibility(s_vc[buf][mycen][t + 6], s_r[buf][t + 6], std::integral_constant<int, (NPQ + 1) / 4>{});
+            visibility(s_vc[buf][mycen][t + 7], s_r[buf][t + 7], std::integral_constant<int, NPQ / 4>{});
+#pragma unroll
+            for (int i = 0; i < NPAIR; ++i) ACC[i] = fma2(GR[i], ZR[i], fma2(GI[i], ZI[i], ACC[i]));   // Re(conj(G) Z)
         }
         __syncthreads();
     }
