@@ -418,13 +418,18 @@ def test_quadtree_driver_matches_oracle(sl):
 
 
 # ----------------------------------------------------------------------------- NEXT-4: batched channels
-@pytest.mark.parametrize("cfg", [1, 3])
+@pytest.mark.parametrize("cfg", [1, 3, 4])
 def test_batched_channels_match_per_channel_oracle(sl, cfg):
     """sl1m_plan_set_channels + batched forward / adjoint / max_eig / solve: channel c must equal the
     oracle on uvw * scale[c] (baselines in wavelengths scale with frequency; PAPER.md:68, 279:
     channels are deconvolved independently).  Config 1 (delta) and a shrunk config 3 (Gaussian pixels)."""
     import torch
-    wl = make_workload(cfg) if cfg == 1 else make_workload(3, n_side=32, n_src=20, n_ant=12, n_steps=4)
+    if cfg == 1:
+        wl = make_workload(1)
+    elif cfg == 3:
+        wl = make_workload(3, n_side=32, n_src=20, n_ant=12, n_steps=4)
+    else:   # shared gain table, baseline-grouped kernels (8 hour-angle steps -> groups of 8 samples)
+        wl = make_workload(4, n_side=48, n_src=30, n_ant=12, n_steps=8)
     scale = np.array([1.0, 0.93, 1.07, 1.21])
     C = scale.shape[0]
     rng = np.random.default_rng(50 + cfg)
@@ -437,7 +442,10 @@ def test_batched_channels_match_per_channel_oracle(sl, cfg):
     Gg = plan.adjoint(_dev(R, torch.complex64)).cpu().numpy()
     Lg = plan.max_eig_batch(8)
     assert Vg.shape == (C, wl.n_vis) and Gg.shape == (C, wl.n_pix)
-    oracles = [oracle.Oracle(wl.uvw * s, wl.l, wl.m, wl.sigma, gauss_model=wl.gauss_model) for s in scale]
+    oracles = [oracle.Oracle(wl.uvw * s, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, wl.gains, gauss_model=wl.gauss_model)
+               for s in scale]
+    if cfg == 4:
+        assert plan.describe()["gains"] == 2
     Vs = []
     for c, o in enumerate(oracles):
         assert rel_l2(Vg[c], o.forward(X[c])) <= TOL_APPLY
