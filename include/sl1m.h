@@ -60,6 +60,10 @@ typedef enum {
 
 /* flags for sl1m_plan_create */
 #define SL1M_GAINS_ON_DEVICE 1u /* `gains` is a DEV pointer (default: HOST) */
+#define SL1M_PHASE_FP64 2u      /* accumulate the whole phase in fp64 (delta pixels, unit gains, one channel).
+                                 * Chosen automatically when the fp32 phase remainder inside a pixel tile could
+                                 * exceed 256 rad (a tile spanning > 40 fringes of the longest baseline: a badly
+                                 * undersampled image); the default kernels are exact enough otherwise. */
 
 /*
  * sl1m_plan_create -- build the operator for one set of visibilities and pixels.
@@ -249,7 +253,9 @@ typedef struct {
     int32_t mufu_per_term_mufu_path;     /* 2 (delta) or 4 (Gaussian)                              */
     int32_t fwd_packed_pairs;            /* 1 = the packed fp32x2 (FFMA2) forward kernel is in use  */
     int32_t adj_packed_pairs;
-    int32_t reserved[3];
+    int32_t phase_fp64;                  /* 1 = the fp64-phase kernels are in use                    */
+    float phase_span_rad;                /* plan-time bound on the fp32 phase remainder in a tile    */
+    int32_t reserved[1];
 } sl1m_plan_info;
 int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
 

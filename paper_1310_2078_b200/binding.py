@@ -14,6 +14,7 @@ from .build import LIB, build_library
 GAUSS_PARAXIAL = 0   # eq (16)
 GAUSS_WIDEFIELD = 1  # eq (17)
 GAINS_ON_DEVICE = 1
+PHASE_FP64 = 2
 
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "sl1m.h")
 
@@ -29,7 +30,7 @@ class _PlanInfo(ctypes.Structure):
         "n_pix_padded", "n_tiles", "gaussian", "gains", "fwd_rv", "fwd_vis_tiles", "fwd_pixel_splits",
         "fwd_tiles_per_split", "fwd_poly_per16", "adj_rp", "adj_pixel_groups", "adj_vis_splits",
         "adj_chunks_per_split", "adj_poly_per16", "mufu_per_term_mufu_path", "fwd_packed_pairs",
-        "adj_packed_pairs")] + [("reserved", ctypes.c_int32 * 3)]
+        "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("reserved", ctypes.c_int32 * 1)]
 
 
 class _QtLevel(ctypes.Structure):
@@ -188,7 +189,7 @@ class Plan:
     """sl1m_plan_create / sl1m_destroy.  Inputs are host arrays (numpy); see include/sl1m.h."""
 
     def __init__(self, uvw, l, m, sigma=None, ant_p=None, ant_q=None, gains=None,
-                 gauss_model: int = GAUSS_WIDEFIELD):
+                 gauss_model: int = GAUSS_WIDEFIELD, phase_fp64: bool = False):
         import torch
         self._h = None
         lib = load_library()
@@ -200,7 +201,7 @@ class Plan:
         sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64).ravel()
         if sg is not None and sg.shape != l.shape:
             raise ValueError("sigma and l differ in length")
-        n_ant, g, flags = 0, None, 0
+        n_ant, g, flags = 0, None, (PHASE_FP64 if phase_fp64 else 0)
         ap = aq = None
         gptr = None
         if gains is not None:
@@ -391,7 +392,8 @@ class Plan:
         """sl1m_plan_describe: launch configuration and instruction mix."""
         info = _PlanInfo()
         _check(load_library().sl1m_plan_describe(self._h, ctypes.byref(info)))
-        return {n: int(getattr(info, n)) for n, _ in _PlanInfo._fields_ if n != "reserved"}
+        return {n: (float(getattr(info, n)) if n == "phase_span_rad" else int(getattr(info, n)))
+                for n, _ in _PlanInfo._fields_ if n != "reserved"}
 
     @property
     def launch_count(self) -> int:

@@ -68,6 +68,9 @@ struct sl1m_plan {
     double *scalars = nullptr;   // [4] device scalars (norm2, l2, l1, nnz)
     // host-buffer variants
     float *h_x = nullptr, *h_vis = nullptr, *h_img = nullptr;   // device staging for *_host calls
+    bool phase64 = false;         // fp64-phase kernels (delta pixels, unit gains) -- flag or automatic
+    double4 *pixd = nullptr;      // DEV [n_pix_pad] (dl, dm, dn', 0) as doubles, only with phase64
+    double phase_span = 0.0;      // plan-time bound on the fp32 phase remainder, radians
     int n_chan = 1;               // batched channels (NEXT-4): every per-image / per-visibility buffer is [n_chan][.]
     double *chan_scale = nullptr; // DEV [n_chan] nu_c / nu_0, NULL while n_chan == 1
     float2 *step_c = nullptr;     // DEV [n_chan] (1/L_c, lambda_c/L_c) for the batched solver
@@ -90,7 +93,7 @@ void free_plan(sl1m_plan *p) {
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
-                    p->trace_buf, p->chan_scale, p->step_c};
+                    p->trace_buf, p->chan_scale, p->step_c, p->pixd};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -155,6 +158,7 @@ int configure_and_allocate(sl1m_plan *p) {
 #ifdef SL1M_FORCE_R
         rv = SL1M_FORCE_R;
 #endif
+        if (p->phase64) rv = std::min(rv, 4);   // fp64 uvw live in registers
         p->fwd_rv = rv;
         p->fwd_vtiles = (int)((nvi + NT * rv - 1) / (NT * rv));
         int split = std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
@@ -168,6 +172,7 @@ int configure_and_allocate(sl1m_plan *p) {
 #ifdef SL1M_FORCE_R
         rp = SL1M_FORCE_R;
 #endif
+        if (p->phase64) rp = std::min(rp, 4);
         p->adj_rp = rp;
         p->adj_pgroups = p->n_pix_pad / (NT * rp);
         int split = std::min(n_chunks, std::max(1, (target + p->adj_pgroups - 1) / p->adj_pgroups));
@@ -217,7 +222,7 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     if (gains && n_ant < 1) return fail(SL1M_ERR_SIZE, "n_ant must be >= 1 with gains");
     if (gauss_model != SL1M_GAUSS_PARAXIAL && gauss_model != SL1M_GAUSS_WIDEFIELD)
         return fail(SL1M_ERR_PARAM, "unknown gauss_model");
-    if (flags & ~SL1M_GAINS_ON_DEVICE) return fail(SL1M_ERR_PARAM, "unknown flag");
+    if (flags & ~(SL1M_GAINS_ON_DEVICE | SL1M_PHASE_FP64)) return fail(SL1M_ERR_PARAM, "unknown flag");
     for (int64_t j = 0; j < 3 * n_vis; ++j)
         if (!std::isfinite(uvw[j])) return fail(SL1M_ERR_DOMAIN, "non-finite uvw");
     bool any_gauss = false;
@@ -308,6 +313,13 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         std::vector<double4> cen((size_t)p->n_tiles, make_double4(0.0, 0.0, 0.0, 0.0));
         std::vector<float> amp(npad, 0.f);
         std::vector<int> perm(npad, -1);
+        std::vector<double4> pixd(npad, make_double4(0.0, 0.0, 0.0, 0.0));
+        double umax = 0.0, vmax = 0.0, wmax = 0.0, span = 0.0;
+        for (int64_t j = 0; j < n_vis; ++j) {
+            umax = std::max(umax, std::fabs(uvw[3 * j]));
+            vmax = std::max(vmax, std::fabs(uvw[3 * j + 1]));
+            wmax = std::max(wmax, std::fabs(uvw[3 * j + 2]));
+        }
         const double PI = 3.14159265358979323846, LOG2E = 1.4426950408889634074;
         for (int t = 0; t < p->n_tiles; ++t) {
             const size_t k0 = (size_t)t * TP, k1 = k0 + TP;
@@ -334,6 +346,9 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
                 const double npr = (sg > 0.0 && gauss_model == SL1M_GAUSS_PARAXIAL) ? -0.5 * r2
                                                                                      : -r2 / (1.0 + n);
                 pix4[s] = make_float4((float)(l[k] - lc), (float)(m[k] - mc), (float)(npr - nc), 0.f);
+                pixd[s] = make_double4(l[k] - lc, m[k] - mc, npr - nc, 0.0);
+                span = std::max(span, 2.0 * PI * (umax * std::fabs(l[k] - lc) + vmax * std::fabs(m[k] - mc) +
+                                                  wmax * std::fabs(npr - nc)));
                 amp[s] = (float)(1.0 / n);
                 perm[s] = k;
                 if (any_gauss) pixg[s] = make_float2((float)(sg * sg), (float)(-PI * LOG2E * sg * sg));
@@ -406,6 +421,11 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         if ((st = upload(&p->cen, cen.data(), cen.size()))) return st;
         if ((st = upload(&p->amp, amp.data(), npad))) return st;
         if ((st = upload(&p->perm, perm.data(), npad))) return st;
+        // fp64-phase kernels: on request, or when the fp32 remainder could exceed ~256 rad (sin.approx
+        // loses 4e-5 there, profiles/r1_microbench.md); delta pixels with unit gains only.
+        p->phase_span = span;
+        p->phase64 = !any_gauss && !gains && ((flags & SL1M_PHASE_FP64) || span > 256.0);
+        if (p->phase64 && (st = upload(&p->pixd, pixd.data(), npad))) return st;
         if (gains) {
             if ((st = upload(&p->ant_p, vperm.empty() ? ant_p : ip.data(), nvi))) return st;
             if ((st = upload(&p->ant_q, vperm.empty() ? ant_q : iq.data(), nvi))) return st;
@@ -507,6 +527,15 @@ void launch_fwd(sl1m_plan *p, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->fwd_per_split;
     dim3 grid(p->fwd_vtiles, p->fwd_split, p->n_chan);
+    if (p->phase64 && p->n_chan == 1) {
+        switch (p->fwd_rv) {
+            case 4: fwd_kernel_p64<4><<<grid, NT, 0, s>>>(P, p->pixd); break;
+            case 2: fwd_kernel_p64<2><<<grid, NT, 0, s>>>(P, p->pixd); break;
+            default: fwd_kernel_p64<1><<<grid, NT, 0, s>>>(P, p->pixd); break;
+        }
+        p->launches++;
+        return;
+    }
     const int key = p->pk * 3 + p->gk;   // pk == 2 (one sigma per tile) only exists with unit gains
     switch (key) {
         case 6: launch_fwd_rv<2, 0>(p, P, grid, s); break;
@@ -526,6 +555,15 @@ void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
     P.per_split = p->adj_per_split;
     P.r = r;
     dim3 grid(p->adj_pgroups, p->adj_split, p->n_chan);
+    if (p->phase64 && p->n_chan == 1) {
+        switch (p->adj_rp) {
+            case 4: adj_kernel_p64<4><<<grid, NT, 0, s>>>(P, p->pixd); break;
+            case 2: adj_kernel_p64<2><<<grid, NT, 0, s>>>(P, p->pixd); break;
+            default: adj_kernel_p64<1><<<grid, NT, 0, s>>>(P, p->pixd); break;
+        }
+        p->launches++;
+        return;
+    }
     const int key = p->pk * 3 + p->gk;
     switch (key) {
         case 6: launch_adj_rp<2, 0>(p, P, grid, s); break;
@@ -901,6 +939,9 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
                               : (grouped && p->adj_rp == 8 ? SL1M_ADJ_G2_NPQ : 0);
     o->mufu_per_term_mufu_path = p->pk == 2 ? 3 : (pk ? 4 : 2);
     o->gaussian = p->pk;
+    o->phase_fp64 = p->phase64 && p->n_chan == 1;
+    o->phase_span_rad = (float)p->phase_span;
+    if (o->phase_fp64) o->fwd_poly_per16 = o->adj_poly_per16 = 0;
     o->fwd_packed_pairs = (plain && p->fwd_rv == 8) || grouped;
     o->adj_packed_pairs = (plain || grouped) && p->adj_rp == 8;
     return SL1M_OK;

@@ -1083,4 +1083,162 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// fp64-phase variants (NEXT-2 of the scope table: "higher-precision phase path selectable per
+// plan"), delta pixels, unit gains.  The fp32 remainder u' dl + v' dm + w' dn' of the default
+// kernels is accurate while it stays within a few hundred radians, i.e. while a 16 x 16-pixel tile
+// spans at most a few tens of fringes of the longest baseline -- always true for a sensibly sampled
+// image, not for a badly undersampled one.  Here the whole phase is accumulated in fp64 TURNS
+// (3 DFMA on the otherwise idle FP64 pipe), its fraction is taken exactly with the magic-number add
+// (1.5 * 2^20: the low word of the sum is frac * 2^32), and 23 bits of it are handed to
+// sin.approx / cos.approx: phase error <= 4e-7 rad for any baseline length.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float phase64_to_radians(double turns) {
+    const double m = turns + 1572864.0;                        // 1.5 * 2^20: ulp = 2^-32
+    const int frac32 = __double2loint(m);                      // round(turns * 2^32) mod 2^32, signed
+    const int s23 = frac32 >> 9;                               // [-2^22, 2^22)
+    const float f = __int_as_float(0x4B400000 + s23) - 12582912.0f;   // exactly s23
+    return f * 7.490140565847157e-07f;                         // 2 pi / 2^23
+}
+
+template <int RV>
+__global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, const double4 *pixd) {
+    __shared__ __align__(128) float4 s_pix[2][TP];
+    __shared__ __align__(128) double4 s_pixd[2][TP];   // (dl, dm, dn', 0) as doubles
+    __shared__ __align__(8) uint64_t s_bar[2];
+    const int tid = threadIdx.x;
+    const int t0 = blockIdx.y * P.per_split;
+    const int t1 = min(t0 + P.per_split, P.n_tiles);
+    const int jbase = blockIdx.x * (NT * RV);
+    const int jlast = P.n_vis - 1;
+    double ud[RV], vd[RV], wd[RV];
+    float re[RV], im[RV];
+#pragma unroll
+    for (int r = 0; r < RV; ++r) {
+        const int j = min(jbase + r * NT + tid, jlast);
+        ud[r] = __ldg(P.u64 + j);
+        vd[r] = __ldg(P.v64 + j);
+        wd[r] = __ldg(P.w64 + j);
+        re[r] = 0.f;
+        im[r] = 0.f;
+    }
+    constexpr uint32_t kBytes = TP * (sizeof(float4) + sizeof(double4));
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int t, int st) {
+        mbar_expect_tx(&s_bar[st], kBytes);
+        tma_bulk_g2s(&s_pix[st][0], P.pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
+        tma_bulk_g2s(&s_pixd[st][0], pixd + (size_t)t * TP, TP * sizeof(double4), &s_bar[st]);
+    };
+    if (tid == 0) {
+        if (t0 < t1) issue(t0, 0);
+        if (t0 + 1 < t1) issue(t0 + 1, 1);
+    }
+    for (int t = t0; t < t1; ++t) {
+        const int st = (t - t0) & 1;
+        const uint32_t parity = ((t - t0) >> 1) & 1;
+        const double4 c = P.cen[t];
+        double x0[RV];
+#pragma unroll
+        for (int r = 0; r < RV; ++r) {
+            double tt = fma(ud[r], c.x, fma(vd[r], c.y, wd[r] * c.z));
+            x0[r] = tt - rint(tt);
+        }
+        mbar_wait(&s_bar[st], parity);
+#pragma unroll 2
+        for (int p = 0; p < TP; ++p) {
+            const double4 pd = s_pixd[st][p];
+            const float wt = s_pix[st][p].w;
+#pragma unroll
+            for (int r = 0; r < RV; ++r) {
+                const float X = phase64_to_radians(fma(ud[r], pd.x, fma(vd[r], pd.y, fma(wd[r], pd.z, x0[r]))));
+                float s, c2;
+                __sincosf(X, &s, &c2);
+                re[r] = fmaf(wt, c2, re[r]);
+                im[r] = fmaf(-wt, s, im[r]);
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && t + 2 < t1) issue(t + 2, st);
+    }
+    float2 *out = P.ws_v + (size_t)blockIdx.y * P.n_vis;
+#pragma unroll
+    for (int r = 0; r < RV; ++r) {
+        const int j = jbase + r * NT + tid;
+        if (j < P.n_vis) out[j] = make_float2(re[r], im[r]);
+    }
+}
+
+template <int RP>
+__global__ void __launch_bounds__(NT, 3) adj_kernel_p64(const ApplyParams P, const double4 *pixd) {
+    constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
+    __shared__ __align__(32) double4 s_vis[2][VC];       // (u, v, w, 0) in wavelengths
+    __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, r_im)
+    __shared__ double s_x0[2][VC][NCEN];                 // frac(u l_c + v m_c + w n'_c), turns
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int base = blockIdx.x * (NT * RP);
+    const int kfirst = base + warp * (32 * RP);
+    const int tile0 = base / TP;
+    const int mycen = (kfirst / TP) - tile0;
+    double dl[RP], dm[RP], dn[RP];
+    float acc[RP];
+#pragma unroll
+    for (int i = 0; i < RP; ++i) {
+        const double4 pd = pixd[kfirst + i * 32 + lane];
+        dl[i] = pd.x;
+        dm[i] = pd.y;
+        dn[i] = pd.z;
+        acc[i] = 0.f;
+    }
+    const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const int c0 = blockIdx.y * P.per_split;
+    const int c1 = min(c0 + P.per_split, n_chunks);
+    auto stage = [&](int chunk, int buf) {
+        const int j = chunk * VC + tid;
+        double u = 0.0, v = 0.0, w = 0.0;
+        float2 rr = make_float2(0.f, 0.f);
+        if (j < P.n_vis) {
+            u = P.u64[j];
+            v = P.v64[j];
+            w = P.w64[j];
+            rr = P.r[j];
+        }
+        s_vis[buf][tid] = make_double4(u, v, w, 0.0);
+        s_r[buf][tid] = rr;
+#pragma unroll
+        for (int c = 0; c < NCEN; ++c) {
+            const double4 cen = P.cen[tile0 + c];
+            const double tt = fma(u, cen.x, fma(v, cen.y, w * cen.z));
+            s_x0[buf][tid][c] = tt - rint(tt);
+        }
+    };
+    if (c0 < c1) stage(c0, 0);
+    __syncthreads();
+    for (int ch = c0; ch < c1; ++ch) {
+        const int buf = (ch - c0) & 1;
+        if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
+#pragma unroll 2
+        for (int t = 0; t < VC; ++t) {
+            const double4 vv = s_vis[buf][t];
+            const float2 rr = s_r[buf][t];
+            const double x0 = s_x0[buf][t][mycen];
+#pragma unroll
+            for (int i = 0; i < RP; ++i) {
+                const float X = phase64_to_radians(fma(vv.x, dl[i], fma(vv.y, dm[i], fma(vv.z, dn[i], x0))));
+                float s, c;
+                __sincosf(X, &s, &c);
+                acc[i] = fmaf(c, rr.x, fmaf(-s, rr.y, acc[i]));   // Re (c + i s)(r_re + i r_im)
+            }
+        }
+        __syncthreads();
+    }
+    float *out = P.ws_p + (size_t)blockIdx.y * P.n_pix_pad;
+#pragma unroll
+    for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
+}
+
 }  // namespace sl1m

@@ -229,3 +229,40 @@ def test_sigma_classes_one_sigma_per_tile_path(sl, model):
             xs, _ = plan.solve(_dev(V, torch.complex64), 0.3, L=L, n_iter=30)
             assert rel_l2(xs.cpu().numpy(), o.fista(V, 0.3, L, 30)["x"]) <= 1e-3
         plan.close()
+
+
+def test_fp64_phase_path(sl):
+    """NEXT-2 ("higher-precision phase path selectable per plan"): (i) forced with the flag on config 1 it
+    matches the oracle like the default kernels; (ii) a badly undersampled image -- config 1's pixels under
+    30 km baselines, where a 16 x 16-pixel tile spans ~700 fringes and the fp32 remainder would reach
+    thousands of radians -- selects it automatically and still meets 2e-4 (applies) and 1e-3 (solver)."""
+    import torch
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    rng = np.random.default_rng(5)
+    x = rng.uniform(0, 1, wl.n_pix).astype(np.float32)
+    r = (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis)).astype(np.complex64)
+    plan = sl.Plan.from_workload(wl)
+    assert plan.describe()["phase_fp64"] == 0 and plan.describe()["phase_span_rad"] < 256.0
+    plan.close()
+    plan = sl.Plan(wl.uvw, wl.l, wl.m, phase_fp64=True)
+    assert plan.describe()["phase_fp64"] == 1
+    assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x)) <= 2e-5
+    assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r)) <= 2e-5
+    plan.close()
+    for n_pix_side in (32, 64):      # 64: several pixel groups (R = 4 kernels)
+        wl = make_workload(1, n_side=n_pix_side)
+        uvw = wl.uvw * 30.0
+        uvw[:, 2] = 200.0 * rng.uniform(-1, 1, wl.n_vis)
+        o = oracle.Oracle(uvw, wl.l, wl.m)
+        plan = sl.Plan(uvw, wl.l, wl.m)
+        d = plan.describe()
+        assert d["phase_fp64"] == 1 and d["phase_span_rad"] > 1000.0
+        x = rng.uniform(0, 1, wl.n_pix).astype(np.float32)
+        assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x)) <= 2e-4
+        assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r)) <= 2e-4
+        V = (o.forward(wl.x_true) + wl.noise).astype(np.complex64)
+        L = o.max_eig(20) * 1.05
+        xs, _ = plan.solve(_dev(V, torch.complex64), 0.5, L=L, n_iter=40)
+        assert rel_l2(xs.cpu().numpy(), o.fista(V, 0.5, L, 40)["x"]) <= 1e-3
+        plan.close()
