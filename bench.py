@@ -304,12 +304,12 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         f = per16 / 16.0
         gauss, gains = int(desc["gaussian"]), bool(desc["gains"])   # gaussian: 0 delta, 1 per-pixel sigma, 2 per-tile sigma
         mufu = desc["mufu_per_term_mufu_path"] * (1.0 - f)
-        lane_mufu_path = {0: 6.0, 1: 20.0, 2: 16.0}[gauss]   # delta: 3 phase + FMUL.RZ + 2 accumulate
+        lane_mufu_path = {0: 6.0, 1: 20.0, 2: 13.0 if packed else 16.0}[gauss]   # delta: 3 phase + FMUL.RZ + 2 accumulate
         lane_poly_path = 18.0                        # 3 phase + 3 reduce + 1 + 5 sin + 4 cos + 2 accumulate
         grouped = int(desc["gains"]) == 2            # one gain product per pixel per 8 samples: +2 lane-ops per term
         lanes = lane_mufu_path * (1.0 - f) + lane_poly_path * f + (2.5 if grouped else (10.0 if gains else 0.0))
         if packed:   # FFMA2 halves the issue slots of everything but FMUL.RZ and MUFU
-            slots = 5.5 * (1.0 - f) + 11.0 * f + 0.25 + (1.5 if grouped else 0.0)
+            slots = (10.0 if gauss == 2 else 5.5) * (1.0 - f) + 11.0 * f + 0.25 + (1.5 if grouped else 0.0)
         else:
             slots = {0: 8.0, 1: 24.0, 2: 19.0}[gauss] * (1.0 - f) + 20.0 * f + 0.125 + (10.0 if gains else 0.0)
         b_mufu = SM_COUNT * MUFU_PER_SM_PER_CLK * clock_hz / mufu

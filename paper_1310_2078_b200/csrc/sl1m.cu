@@ -487,6 +487,7 @@ void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
         switch (p->fwd_rv) {
             case 8:
                 if constexpr (PK == 0 && GK == 0) fwd_kernel_x2<SL1M_FWD_NPQ, B><<<grid, NT, 0, s>>>(P);
+                else if constexpr (PK == 2 && GK == 0) fwd_kernel_gtx2<B><<<grid, NT, 0, s>>>(P);
                 else fwd_kernel<8, PK, GK, B><<<grid, NT, 0, s>>>(P);
                 break;
             case 4: fwd_kernel<4, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
@@ -502,6 +503,7 @@ void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
         case 8:
             if constexpr (PK == 0 && GK == 0) adj_kernel_x2<SL1M_ADJ_NPQ, B><<<grid, NT, 0, s>>>(P);
             else if constexpr (PK == 0 && GK == 2) adj_kernel_g2x2<SL1M_ADJ_G2_NPQ, B><<<grid, NT, 0, s>>>(P);
+            else if constexpr (PK == 2 && GK == 0) adj_kernel_gtx2<B><<<grid, NT, 0, s>>>(P);
             else adj_kernel<8, PK, GK, B><<<grid, NT, 0, s>>>(P);
             break;
         case 4: adj_kernel<4, PK, GK, B><<<grid, NT, 0, s>>>(P); break;
@@ -942,8 +944,9 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->phase_fp64 = p->phase64 && p->n_chan == 1;
     o->phase_span_rad = (float)p->phase_span;
     if (o->phase_fp64) o->fwd_poly_per16 = o->adj_poly_per16 = 0;
-    o->fwd_packed_pairs = (plain && p->fwd_rv == 8) || grouped;
-    o->adj_packed_pairs = (plain || grouped) && p->adj_rp == 8;
+    const bool tile_gauss = p->pk == 2 && p->gk == 0;
+    o->fwd_packed_pairs = ((plain || tile_gauss) && p->fwd_rv == 8) || grouped;
+    o->adj_packed_pairs = (plain || grouped || tile_gauss) && p->adj_rp == 8;
     return SL1M_OK;
 }
 

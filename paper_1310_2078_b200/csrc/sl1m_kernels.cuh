@@ -33,7 +33,8 @@ namespace sl1m {
 constexpr int TP = 256;        // pixels per tile (one fp64 centre per tile)
 constexpr int NT = 128;        // threads per CTA in the apply kernels
 constexpr int VC = 128;        // visibilities per staged chunk in the adjoint
-constexpr int PIX_PAD = 1024;  // pixel arrays are padded to a multiple of this
+constexpr int PIX_PAD = 1024;
+constexpr int NPAIR_X2 = 4;    // register pairs per thread in the packed kernels  // pixel arrays are padded to a multiple of this
 constexpr double TWO_PI = 6.283185307179586476925286766559;
 
 struct ApplyParams {
@@ -1073,6 +1074,228 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
         __syncthreads();
     }
 
+    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        float a, b;
+        up2(ACC[i], a, b);
+        out[kfirst + (2 * i) * 32 + lane] = a;
+        out[kfirst + (2 * i + 1) * 32 + lane] = b;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Gaussian pixels with one sigma per tile (PK == 2), unit gains, packed-pair variants (R = 8).
+// Same arithmetic as gen_entry_tile, two terms per FFMA2: 14 (forward) / 12 (adjoint) packed ops +
+// 2 FMUL.RZ + 6 MUFU per pair.  Next to a scalar FFMA stream every MUFU costs ~2 extra FMA-side
+// cycles, next to FFMA2 well under 1 (profiles/r1_microbench.md): packing is what lets the 3-MUFU
+// loop run near the MUFU bound.
+// ------------------------------------------------------------------------------------------
+#ifndef SL1M_FWD_GTX2_MIN_CTAS
+#define SL1M_FWD_GTX2_MIN_CTAS 4
+#endif
+#ifndef SL1M_ADJ_GTX2_MIN_CTAS
+#define SL1M_ADJ_GTX2_MIN_CTAS 5
+#endif
+__device__ __forceinline__ void sincos2(f32x2 X, f32x2 &s, f32x2 &c) {
+    float xa, xb, sa, ca, sb, cb;
+    up2(X, xa, xb);
+    __sincosf(xa, &sa, &ca);
+    __sincosf(xb, &sb, &cb);
+    s = pk2(sa, sb);
+    c = pk2(ca, cb);
+}
+__device__ __forceinline__ f32x2 ex2_2(f32x2 E) {
+    float a, b;
+    up2(E, a, b);
+    return pk2(ex2_approx(a), ex2_approx(b));
+}
+
+template <bool BATCH = false>
+__global__ void __launch_bounds__(NT, SL1M_FWD_GTX2_MIN_CTAS) fwd_kernel_gtx2(const ApplyParams P) {
+    constexpr int RV = 8, NPAIR = 4;
+    __shared__ __align__(128) float4 s_pix[2][TP];
+    __shared__ __align__(8) uint64_t s_bar[2];
+    // (1 + i q) is the same for every pixel of a tile (q = w sigma_tile^2), so the pixel loop only sums
+    // T = sum a x 2^E' (cos X' - i sin X') in registers; at the end of the tile the running totals, kept in
+    // shared memory ([pair][thread], own slots only), take (1 + i q) T.  Saves 2 FFMA2 per pair and 24 registers.
+    __shared__ __align__(8) f32x2 s_acc[2 * NPAIR_X2][NT];
+    const int tid = threadIdx.x;
+    const int t0 = blockIdx.y * P.per_split;
+    const int t1 = min(t0 + P.per_split, P.n_tiles);
+    const int jbase = blockIdx.x * (NT * RV);
+    const int jlast = P.n_vis - 1;
+    const double sc = chan_scale_of<BATCH>(P);
+    const float4 *pix4 = P.pix4 + chan_index<BATCH>() * P.n_pix_pad;
+
+    f32x2 U[NPAIR], V[NPAIR], W[NPAIR], NWL[NPAIR];
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
+        const double wa = sc * __ldg(P.w64 + ja), wb = sc * __ldg(P.w64 + jb);
+        U[i] = pk2(static_cast<float>(TWO_PI * (sc * __ldg(P.u64 + ja))), static_cast<float>(TWO_PI * (sc * __ldg(P.u64 + jb))));
+        V[i] = pk2(static_cast<float>(TWO_PI * (sc * __ldg(P.v64 + ja))), static_cast<float>(TWO_PI * (sc * __ldg(P.v64 + jb))));
+        W[i] = pk2(static_cast<float>(TWO_PI * wa), static_cast<float>(TWO_PI * wb));
+        NWL[i] = pk2(static_cast<float>(-wa), static_cast<float>(-wb));
+        s_acc[i][tid] = pk2(0.f, 0.f);
+        s_acc[NPAIR + i][tid] = pk2(0.f, 0.f);
+    }
+    constexpr uint32_t kBytes = TP * sizeof(float4);
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int t, int st) {
+        mbar_expect_tx(&s_bar[st], kBytes);
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, kBytes, &s_bar[st]);
+    };
+    if (tid == 0) {
+        if (t0 < t1) issue(t0, 0);
+        if (t0 + 1 < t1) issue(t0 + 1, 1);
+    }
+    for (int t = t0; t < t1; ++t) {
+        const int st = (t - t0) & 1;
+        const uint32_t parity = ((t - t0) >> 1) & 1;
+        const double4 c = P.cen[t];
+        f32x2 X0[NPAIR], UC[NPAIR], VC2[NPAIR], CE[NPAIR], LR[NPAIR], CX[NPAIR], TC[NPAIR], TS[NPAIR];
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i) {
+            float x0[2], uc[2], vc[2], q[2], cE[2], lr[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int j = min(jbase + (2 * i + h) * NT + tid, jlast);
+                const double ud = sc * __ldg(P.u64 + j), vd = sc * __ldg(P.v64 + j), wd = sc * __ldg(P.w64 + j);
+                x0[h] = centre_phase(ud, vd, wd, c);
+                uc[h] = static_cast<float>(ud - wd * c.x);
+                vc[h] = static_cast<float>(vd - wd * c.y);
+                gauss_tile_constants(wd, c.w, q[h], cE[h], lr[h], x0[h]);
+            }
+            X0[i] = pk2(x0[0], x0[1]);
+            UC[i] = pk2(uc[0], uc[1]);
+            VC2[i] = pk2(vc[0], vc[1]);
+            TC[i] = pk2(0.f, 0.f);
+            TS[i] = pk2(0.f, 0.f);
+            CE[i] = pk2(cE[0], cE[1]);
+            LR[i] = pk2(lr[0], lr[1]);
+            CX[i] = pk2(-0.69314718056f * q[0], -0.69314718056f * q[1]);
+        }
+        mbar_wait(&s_bar[st], parity);
+#pragma unroll 1
+        for (int p = 0; p < TP; ++p) {
+            const float4 px = s_pix[st][p];
+            const f32x2 bx = bc2(px.x), by = bc2(px.y), bz = bc2(px.z), bw = bc2(px.w);
+#pragma unroll
+            for (int i = 0; i < NPAIR; ++i) {
+                const f32x2 X = fma2(U[i], bx, fma2(V[i], by, fma2(W[i], bz, X0[i])));
+                const f32x2 du = fma2(NWL[i], bx, UC[i]), dv = fma2(NWL[i], by, VC2[i]);
+                const f32x2 s2 = fma2(dv, dv, mul2(du, du));
+                const f32x2 Ep = fma2(s2, CE[i], LR[i]);
+                const f32x2 Xp = fma2(CX[i], Ep, X);
+                const f32x2 tw = mul2(bw, ex2_2(Ep));            // a x 2^E'
+                f32x2 s, cc;
+                sincos2(Xp, s, cc);
+                TC[i] = fma2(tw, cc, TC[i]);
+                TS[i] = fma2(tw, s, TS[i]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i) {   // totals += (1 + i q)(TC - i TS):  re += TC + q TS,  -im += TS - q TC
+            const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
+            const f32x2 Q = pk2(static_cast<float>(sc * __ldg(P.w64 + ja) * c.w), static_cast<float>(sc * __ldg(P.w64 + jb) * c.w));
+            float qa, qb;
+            up2(Q, qa, qb);
+            s_acc[i][tid] = add2(s_acc[i][tid], fma2(Q, TS[i], TC[i]));
+            s_acc[NPAIR + i][tid] = add2(s_acc[NPAIR + i][tid], fma2(pk2(-qa, -qb), TC[i], TS[i]));
+        }
+        __syncthreads();
+        if (tid == 0 && t + 2 < t1) issue(t + 2, st);
+    }
+    float2 *out = P.ws_v + chan_index<BATCH>() * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        float ra, rb, ia, ib;
+        up2(s_acc[i][tid], ra, rb);
+        up2(s_acc[NPAIR + i][tid], ia, ib);
+        const int ja = jbase + (2 * i) * NT + tid, jb = jbase + (2 * i + 1) * NT + tid;
+        if (ja < P.n_vis) out[ja] = make_float2(ra, -ia);
+        if (jb < P.n_vis) out[jb] = make_float2(rb, -ib);
+    }
+}
+
+template <bool BATCH = false>
+__global__ void __launch_bounds__(NT, SL1M_ADJ_GTX2_MIN_CTAS) adj_kernel_gtx2(const ApplyParams P) {
+    constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
+    __shared__ __align__(16) float4 s_vis[2][VC];            // (u', v', w', -w)
+    __shared__ __align__(16) float4 s_ca[2][NCEN][VC];       // per centre: (x0', uc, vc, cX = -ln2 q)
+    __shared__ __align__(16) float4 s_cb[2][NCEN][VC];       // per centre: (cE, lr, A = r_re + q r_im, B = q r_re - r_im)
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int base = blockIdx.x * (NT * RP);
+    const int kfirst = base + warp * (32 * RP);
+    const int tile0 = base / TP;
+    const int mycen = (kfirst / TP) - tile0;
+    f32x2 DL[NPAIR], DM[NPAIR], DN[NPAIR], ACC[NPAIR];
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        const float4 pa = P.pix4[kfirst + (2 * i) * 32 + lane], pb = P.pix4[kfirst + (2 * i + 1) * 32 + lane];
+        DL[i] = pk2(pa.x, pb.x);
+        DM[i] = pk2(pa.y, pb.y);
+        DN[i] = pk2(pa.z, pb.z);
+        ACC[i] = pk2(0.f, 0.f);
+    }
+    const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const double sc = chan_scale_of<BATCH>(P);
+    const int c0 = blockIdx.y * P.per_split;
+    const int c1 = min(c0 + P.per_split, n_chunks);
+    auto stage = [&](int chunk, int buf) {
+        const int j = chunk * VC + tid;
+        double u = 0.0, v = 0.0, w = 0.0;
+        float2 rr = make_float2(0.f, 0.f);
+        if (j < P.n_vis) {
+            u = sc * P.u64[j];
+            v = sc * P.v64[j];
+            w = sc * P.w64[j];
+            rr = P.r[chan_index<BATCH>() * P.n_vis + j];
+        }
+        s_vis[buf][tid] = make_float4(static_cast<float>(TWO_PI * u), static_cast<float>(TWO_PI * v),
+                                      static_cast<float>(TWO_PI * w), static_cast<float>(-w));
+#pragma unroll
+        for (int c = 0; c < NCEN; ++c) {
+            const double4 cen = P.cen[tile0 + c];
+            float x0 = centre_phase(u, v, w, cen), q, cE, lr;
+            gauss_tile_constants(w, cen.w, q, cE, lr, x0);
+            s_ca[buf][c][tid] = make_float4(x0, static_cast<float>(u - w * cen.x), static_cast<float>(v - w * cen.y),
+                                            -0.69314718056f * q);
+            // Re conj(M/a) r = amp ((c + q s) r_re + (q c - s) r_im) = amp (c A + s B)
+            s_cb[buf][c][tid] = make_float4(cE, lr, fmaf(q, rr.y, rr.x), fmaf(q, rr.x, -rr.y));
+        }
+    };
+    if (c0 < c1) stage(c0, 0);
+    __syncthreads();
+    for (int ch = c0; ch < c1; ++ch) {
+        const int buf = (ch - c0) & 1;
+        if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
+#pragma unroll 2
+        for (int t = 0; t < VC; ++t) {
+            const float4 vv = s_vis[buf][t], ca = s_ca[buf][mycen][t], cb = s_cb[buf][mycen][t];
+            const f32x2 bu = bc2(vv.x), bv = bc2(vv.y), bw = bc2(vv.z), bnw = bc2(vv.w);
+            const f32x2 bx0 = bc2(ca.x), buc = bc2(ca.y), bvc = bc2(ca.z), bcx = bc2(ca.w);
+            const f32x2 bce = bc2(cb.x), blr = bc2(cb.y), bA = bc2(cb.z), bB = bc2(cb.w);
+#pragma unroll
+            for (int i = 0; i < NPAIR; ++i) {
+                const f32x2 X = fma2(DL[i], bu, fma2(DM[i], bv, fma2(DN[i], bw, bx0)));
+                const f32x2 du = fma2(DL[i], bnw, buc), dv = fma2(DM[i], bnw, bvc);
+                const f32x2 s2 = fma2(dv, dv, mul2(du, du));
+                const f32x2 Ep = fma2(s2, bce, blr);
+                const f32x2 Xp = fma2(bcx, Ep, X);
+                f32x2 s, c;
+                sincos2(Xp, s, c);
+                ACC[i] = fma2(ex2_2(Ep), fma2(c, bA, mul2(s, bB)), ACC[i]);
+            }
+        }
+        __syncthreads();
+    }
     float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
