@@ -113,12 +113,21 @@ def _oracle_sample(wl, seconds: float):
     rate = min(nr0, wl.n_vis) * wl.n_pix / max(time.perf_counter() - t, 1e-9)
     n_rows = int(min(wl.n_vis, max(cores, rate * seconds / 2 / wl.n_pix)))
     n_cols = int(min(wl.n_pix, max(cores, rate * seconds / 2 / wl.n_vis)))
-    rows = rng.choice(wl.n_vis, n_rows, replace=False)
-    cols = rng.choice(wl.n_pix, n_cols, replace=False)
-    t = time.perf_counter()
-    o.forward(x, rows=rows)
-    o.adjoint(r, cols=cols)
-    dt = time.perf_counter() - t
+    for attempt in range(2):
+        rows = rng.choice(wl.n_vis, n_rows, replace=False)
+        cols = rng.choice(wl.n_pix, n_cols, replace=False)
+        t = time.perf_counter()
+        o.forward(x, rows=rows)
+        o.adjoint(r, cols=cols)
+        dt = time.perf_counter() - t
+        # the small probe under-estimates the rate (thread start-up): if the sample came out much shorter
+        # than asked for, size it again from its own rate, once
+        grow = seconds / max(dt, 1e-9)
+        if attempt == 0 and grow > 1.5 and (n_rows < wl.n_vis or n_cols < wl.n_pix):
+            n_rows = int(min(wl.n_vis, n_rows * grow))
+            n_cols = int(min(wl.n_pix, n_cols * grow))
+            continue
+        break
     terms = n_rows * wl.n_pix + n_cols * wl.n_vis
     return {"value": terms / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"forward of {n_rows} sampled visibility rows x all {wl.n_pix} pixels (dense image) + "
