@@ -64,6 +64,8 @@ typedef enum {
                                  * Chosen automatically when the fp32 phase remainder inside a pixel tile could
                                  * exceed 256 rad (a tile spanning > 40 fringes of the longest baseline: a badly
                                  * undersampled image); the default kernels are exact enough otherwise. */
+#define SL1M_DENSE_FORWARD 4u   /* switch the zero-skipping forward off (see sl1m_forward_active_pixels): every
+                                 * pixel is streamed even where x_k == 0.  For A/B measurements and tests. */
 
 /*
  * sl1m_plan_create -- build the operator for one set of visibilities and pixels.
@@ -255,9 +257,22 @@ typedef struct {
     int32_t adj_packed_pairs;
     int32_t phase_fp64;                  /* 1 = the fp64-phase kernels are in use                    */
     float phase_span_rad;                /* plan-time bound on the fp32 phase remainder in a tile    */
-    int32_t reserved[1];
+    int32_t zero_skip;                   /* 1 = the forward streams only pixels with x_k != 0       */
 } sl1m_plan_info;
 int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
+
+/*
+ * Zero-skipping forward.  The image of an L1 solve is sparse and non-negative (eq (18), PAPER.md:194-197:
+ * T^d zeroes every x_i <= d), so most terms M_jk x_k of the forward are exactly zero.  Whenever a*x is packed
+ * into the pixel tiles (sl1m_forward, every FISTA iteration, the power iteration) the pixels with x_k != 0 are
+ * moved to the front of a compact copy of their tile, in their original order, and the forward kernel streams
+ * only those; the result is the same sum with the zero terms left out.  Plans with a gain table, with per-pixel
+ * sigma (more than 16 distinct values) or with fp64 phase keep the dense forward (sl1m_plan_info.zero_skip == 0),
+ * as does SL1M_DENSE_FORWARD.  The adjoint always evaluates every term.
+ * n_active_host: HOST [n_chan]; pixels the most recently packed forward input streams per channel (padded to
+ * 4 per tile; n_pix_padded when the plan does not skip).  Synchronises `stream`.
+ */
+int sl1m_forward_active_pixels(sl1m_plan *plan, int64_t *n_active_host, void *stream);
 
 /* Number of kernels this plan has launched since creation (for bench.py's gpu_launches). */
 int64_t sl1m_launch_count(const sl1m_plan *plan);

@@ -15,6 +15,7 @@ GAUSS_PARAXIAL = 0   # eq (16)
 GAUSS_WIDEFIELD = 1  # eq (17)
 GAINS_ON_DEVICE = 1
 PHASE_FP64 = 2
+DENSE_FORWARD = 4
 
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "sl1m.h")
 
@@ -30,7 +31,7 @@ class _PlanInfo(ctypes.Structure):
         "n_pix_padded", "n_tiles", "gaussian", "gains", "fwd_rv", "fwd_vis_tiles", "fwd_pixel_splits",
         "fwd_tiles_per_split", "fwd_poly_per16", "adj_rp", "adj_pixel_groups", "adj_vis_splits",
         "adj_chunks_per_split", "adj_poly_per16", "mufu_per_term_mufu_path", "fwd_packed_pairs",
-        "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("reserved", ctypes.c_int32 * 1)]
+        "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("zero_skip", ctypes.c_int32)]
 
 
 class _QtLevel(ctypes.Structure):
@@ -102,6 +103,7 @@ def load_library():
                                         vp, ctypes.POINTER(i64), ctypes.POINTER(_QtLevel),
                                         ctypes.POINTER(ctypes.c_int), vp]
     lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
+    lib.sl1m_forward_active_pixels.argtypes = [vp, vp, vp]
     lib.sl1m_launch_count.argtypes = [vp]
     lib.sl1m_launch_count.restype = i64
     lib.sl1m_plan_n_vis.argtypes = [vp]
@@ -189,7 +191,7 @@ class Plan:
     """sl1m_plan_create / sl1m_destroy.  Inputs are host arrays (numpy); see include/sl1m.h."""
 
     def __init__(self, uvw, l, m, sigma=None, ant_p=None, ant_q=None, gains=None,
-                 gauss_model: int = GAUSS_WIDEFIELD, phase_fp64: bool = False):
+                 gauss_model: int = GAUSS_WIDEFIELD, phase_fp64: bool = False, dense_forward: bool = False):
         import torch
         self._h = None
         lib = load_library()
@@ -201,7 +203,7 @@ class Plan:
         sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64).ravel()
         if sg is not None and sg.shape != l.shape:
             raise ValueError("sigma and l differ in length")
-        n_ant, g, flags = 0, None, (PHASE_FP64 if phase_fp64 else 0)
+        n_ant, g, flags = 0, None, (PHASE_FP64 if phase_fp64 else 0) | (DENSE_FORWARD if dense_forward else 0)
         ap = aq = None
         gptr = None
         if gains is not None:
@@ -242,9 +244,9 @@ class Plan:
         return (n,) if self.n_chan == 1 else (self.n_chan, n)
 
     @classmethod
-    def from_workload(cls, wl, gains_device=None):
+    def from_workload(cls, wl, gains_device=None, dense_forward: bool = False):
         g = wl.gains if gains_device is None else gains_device
-        return cls(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model)
+        return cls(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model, dense_forward=dense_forward)
 
     def close(self):
         if self._h is not None:
@@ -393,7 +395,13 @@ class Plan:
         info = _PlanInfo()
         _check(load_library().sl1m_plan_describe(self._h, ctypes.byref(info)))
         return {n: (float(getattr(info, n)) if n == "phase_span_rad" else int(getattr(info, n)))
-                for n, _ in _PlanInfo._fields_ if n != "reserved"}
+                for n, _ in _PlanInfo._fields_}
+
+    def forward_active_pixels(self, stream=None):
+        """sl1m_forward_active_pixels: pixels the most recently packed forward input streams (per channel)."""
+        out = np.zeros(self.n_chan, dtype=np.int64)
+        _check(load_library().sl1m_forward_active_pixels(self._h, _np_ptr(out), _stream_ptr(stream)))
+        return int(out[0]) if self.n_chan == 1 else out
 
     @property
     def launch_count(self) -> int:

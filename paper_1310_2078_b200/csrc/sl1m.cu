@@ -50,6 +50,9 @@ struct sl1m_plan {
     double *u64 = nullptr, *v64 = nullptr, *w64 = nullptr;
     int *ant_p = nullptr, *ant_q = nullptr;
     float4 *pix4 = nullptr;
+    float4 *pixc = nullptr;       // [n_chan][n_pix_pad] compact tiles of the zero-skipping forward (NULL = dense forward)
+    int *tile_cnt = nullptr;      // [n_chan][n_tiles] pixels per compact tile
+    bool dense_forward = false;   // SL1M_DENSE_FORWARD: never skip
     float2 *pixg = nullptr;
     double4 *cen = nullptr;
     float *amp = nullptr;
@@ -93,7 +96,7 @@ void free_plan(sl1m_plan *p) {
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
-                    p->trace_buf, p->chan_scale, p->step_c, p->pixd};
+                    p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -183,7 +186,8 @@ int configure_and_allocate(sl1m_plan *p) {
     // ---- workspaces ----
     const size_t npad = (size_t)p->n_pix_pad, C = (size_t)p->n_chan;
     for (void **q : {(void **)&p->ws_v, (void **)&p->ws_p, (void **)&p->resid, (void **)&p->I_sorted, (void **)&p->y_sorted,
-                     (void **)&p->g_sorted, (void **)&p->part_a, (void **)&p->part_b, (void **)&p->part_c, (void **)&p->scalars}) {
+                     (void **)&p->g_sorted, (void **)&p->part_a, (void **)&p->part_b, (void **)&p->part_c, (void **)&p->scalars,
+                     (void **)&p->pixc, (void **)&p->tile_cnt}) {
         if (*q) cudaFree(*q);
         *q = nullptr;
     }
@@ -199,6 +203,13 @@ int configure_and_allocate(sl1m_plan *p) {
     CUDA_TRY(cudaMalloc((void **)&p->part_c, C * (size_t)p->n_part * sizeof(double)));
     CUDA_TRY(cudaMalloc((void **)&p->scalars, C * 4 * sizeof(double)));
     CUDA_TRY(cudaMemset(p->scalars, 0, C * 4 * sizeof(double)));
+    // zero-skipping forward: kernels without a per-pixel side array (gains, per-pixel sigma, fp64 offsets)
+    if (!p->dense_forward && p->gk == 0 && p->pk != 1 && !(p->phase64 && p->n_chan == 1)) {
+        CUDA_TRY(cudaMalloc((void **)&p->pixc, C * npad * sizeof(float4)));
+        CUDA_TRY(cudaMalloc((void **)&p->tile_cnt, C * (size_t)p->n_tiles * sizeof(int)));
+        CUDA_TRY(cudaMemset(p->pixc, 0, C * npad * sizeof(float4)));
+        CUDA_TRY(cudaMemset(p->tile_cnt, 0, C * (size_t)p->n_tiles * sizeof(int)));
+    }
     CUDA_TRY(cudaDeviceSynchronize());
 
     return SL1M_OK;
@@ -222,7 +233,7 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     if (gains && n_ant < 1) return fail(SL1M_ERR_SIZE, "n_ant must be >= 1 with gains");
     if (gauss_model != SL1M_GAUSS_PARAXIAL && gauss_model != SL1M_GAUSS_WIDEFIELD)
         return fail(SL1M_ERR_PARAM, "unknown gauss_model");
-    if (flags & ~(SL1M_GAINS_ON_DEVICE | SL1M_PHASE_FP64)) return fail(SL1M_ERR_PARAM, "unknown flag");
+    if (flags & ~(SL1M_GAINS_ON_DEVICE | SL1M_PHASE_FP64 | SL1M_DENSE_FORWARD)) return fail(SL1M_ERR_PARAM, "unknown flag");
     for (int64_t j = 0; j < 3 * n_vis; ++j)
         if (!std::isfinite(uvw[j])) return fail(SL1M_ERR_DOMAIN, "non-finite uvw");
     bool any_gauss = false;
@@ -252,6 +263,7 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         ~Guard() { if (p) free_plan(p); }
     } guard{p};
     CUDA_TRY(cudaGetDevice(&p->device));
+    p->dense_forward = (flags & SL1M_DENSE_FORWARD) != 0;
     p->n_vis = n_vis;
     p->n_pix = n_pix;
     p->n_ant = gains ? n_ant : 0;
@@ -477,6 +489,7 @@ namespace {
 
 inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
 inline dim3 cgrid(const sl1m_plan *p, size_t n) { return dim3((unsigned)egrid(n), (unsigned)p->n_chan); }  // x: elements, y: channel
+inline ZeroSkip zs_of(const sl1m_plan *p) { return ZeroSkip{p->pixc, p->tile_cnt}; }
 
 template <int PK, int GK, bool B>
 void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
@@ -538,6 +551,10 @@ void launch_fwd(sl1m_plan *p, cudaStream_t s) {
         p->launches++;
         return;
     }
+    if (p->pixc) {   // zero-skipping: stream the compact tiles the packing kernel left behind
+        P.pix4 = p->pixc;
+        P.tile_cnt = p->tile_cnt;
+    }
     const int key = p->pk * 3 + p->gk;   // pk == 2 (one sigma per tile) only exists with unit gains
     switch (key) {
         case 6: launch_fwd_rv<2, 0>(p, P, grid, s); break;
@@ -590,7 +607,7 @@ int check_launch(const char *what) {
 extern "C" int sl1m_forward(sl1m_plan *p, const float *x_dev, float *vis_dev, void *stream) {
     if (!p || !x_dev || !vis_dev) return fail(SL1M_ERR_NULL, "sl1m_forward: NULL argument");
     cudaStream_t s = (cudaStream_t)stream;
-    pack_caller_kernel<<<cgrid(p, p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->perm, x_dev, p->n_pix_pad, (int)p->n_pix);
+    pack_caller_kernel<<<cgrid(p, p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->perm, x_dev, p->n_pix_pad, (int)p->n_pix, zs_of(p));
     launch_fwd(p, s);
     fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
                                                             (float2 *)vis_dev, 0, nullptr, (int)p->n_vis, p->n_part);
@@ -662,7 +679,7 @@ int max_eig_impl(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
     const int npad = p->n_pix_pad;
     // x0 = 1/sqrt(n_pix) on real pixels
     fill_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->g_sorted, (float)(1.0 / std::sqrt((double)p->n_pix)), p->perm, npad);
-    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->g_sorted, npad);
+    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->g_sorted, npad, zs_of(p));
     p->launches += 2;
     for (int it = 0; it < n_pow; ++it) {
         launch_fwd(p, s);
@@ -673,7 +690,7 @@ int max_eig_impl(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
                                                         p->g_sorted, p->part_a, (int)p->n_pix, p->n_part);
         sum_partials_kernel<<<p->n_chan, ET, 0, s>>>(p->part_a, nullptr, nullptr, egrid(npad), 0, 0, p->scalars, nullptr,
                                                      nullptr, p->n_part, 4);
-        normalize_pack_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->g_sorted, p->scalars, p->amp, p->pix4, npad);
+        normalize_pack_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->g_sorted, p->scalars, p->amp, p->pix4, npad, zs_of(p));
         p->launches += 4;
     }
     int st = check_launch("sl1m_max_eig");
@@ -757,7 +774,7 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
         CUDA_TRY(cudaMemsetAsync(p->I_sorted, 0, (size_t)C * npad * sizeof(float), s));
     }
     CUDA_TRY(cudaMemcpyAsync(p->y_sorted, p->I_sorted, (size_t)C * npad * sizeof(float), cudaMemcpyDeviceToDevice, s));
-    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, npad);
+    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, npad, zs_of(p));
     p->launches++;
 
     double t = 1.0;
@@ -774,7 +791,7 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
         fista_update_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->pix4, p->I_sorted,
                                                           p->y_sorted, inv_L, thr, beta,
                                                           trace_dev ? p->part_b : nullptr,
-                                                          trace_dev ? p->part_c : nullptr, step_c, p->n_part);
+                                                          trace_dev ? p->part_c : nullptr, step_c, p->n_part, zs_of(p));
         p->launches += 2;
         if (trace_dev) {
             sum_partials_kernel<<<C, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
@@ -800,7 +817,7 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
 
     if (info_host) {
         // one extra forward for ||M I_K - V||^2 (Table 1's L2 term)
-        pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->I_sorted, npad);
+        pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->I_sorted, npad, zs_of(p));
         launch_fwd(p, s);
         fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
                                                                 (const float2 *)vis_dev, p->resid, 1, p->part_a,
@@ -943,10 +960,30 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->gaussian = p->pk;
     o->phase_fp64 = p->phase64 && p->n_chan == 1;
     o->phase_span_rad = (float)p->phase_span;
+    o->zero_skip = p->pixc != nullptr;
     if (o->phase_fp64) o->fwd_poly_per16 = o->adj_poly_per16 = 0;
     const bool tile_gauss = p->pk == 2 && p->gk == 0;
     o->fwd_packed_pairs = ((plain || tile_gauss) && p->fwd_rv == 8) || grouped;
     o->adj_packed_pairs = (plain || grouped || tile_gauss) && p->adj_rp == 8;
+    return SL1M_OK;
+}
+
+extern "C" int sl1m_forward_active_pixels(sl1m_plan *p, int64_t *n_active_host, void *stream) {
+    if (!p || !n_active_host) return fail(SL1M_ERR_NULL, "sl1m_forward_active_pixels: NULL argument");
+    const size_t C = (size_t)p->n_chan, T = (size_t)p->n_tiles;
+    if (!p->tile_cnt) {   // dense forward: every (padded) pixel is streamed
+        for (size_t c = 0; c < C; ++c) n_active_host[c] = (int64_t)p->n_pix_pad;
+        return SL1M_OK;
+    }
+    std::vector<int> h(C * T);
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(cudaMemcpyAsync(h.data(), p->tile_cnt, h.size() * sizeof(int), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    for (size_t c = 0; c < C; ++c) {
+        int64_t n = 0;
+        for (size_t t = 0; t < T; ++t) n += h[c * T + t];
+        n_active_host[c] = n;
+    }
     return SL1M_OK;
 }
 

@@ -26,15 +26,48 @@ __device__ __forceinline__ double block_sum(double v) {
     return t;  // valid in thread 0
 }
 
+// Zero-skipping forward.  A CTA of the packing kernels (ET == TP threads) holds exactly
+// tile blockIdx.x.  The entries with a*x != 0 move to the front of the COMPACT copy of the tile in their
+// original order, padded with a*x = 0 entries to a multiple of 4; zs.cnt[c][tile] = the padded count.  The
+// forward kernels stream only that many pixels of the tile: the skipped terms are exactly zero.
+struct ZeroSkip {
+    float4 *pixc;   // DEV [n_chan][n_pix_pad] compact tiles, NULL = off (gains, per-pixel sigma, fp64 phase)
+    int *cnt;       // DEV [n_chan][n_tiles]
+};
+static_assert(ET == TP, "one packing CTA per pixel tile");
+__device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int n_pix_pad, float4 v) {
+    if (!zs.pixc) return;                                // uniform over the grid
+    __shared__ int s_wcnt[ET / 32];
+    const bool nz = (v.w != 0.f);                        // NaN counts as non-zero: it propagates as in the dense path
+    const unsigned b = __ballot_sync(0xffffffffu, nz);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) s_wcnt[warp] = __popc(b);
+    __syncthreads();
+    int base = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < ET / 32; ++w) {
+        const int c = s_wcnt[w];
+        base += (w < warp) ? c : 0;
+        total += c;
+    }
+    float4 *tile = zs.pixc + chan * n_pix_pad + (size_t)blockIdx.x * TP;
+    if (nz) tile[base + __popc(b & ((1u << lane) - 1u))] = v;
+    const int cnt4 = (total + 3) & ~3;
+    if ((int)threadIdx.x < cnt4 - total) tile[total + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (threadIdx.x == 0) zs.cnt[chan * (size_t)(n_pix_pad / TP) + blockIdx.x] = cnt4;
+}
+
 // pix4[k].w = a_k * x[perm[k]]   (caller order -> sorted, padded pixels get 0)
 __global__ void __launch_bounds__(ET) pack_caller_kernel(float4 *pix4, const float *amp, const int *perm,
-                                                         const float *x, int n_pix_pad, int n_pix) {
-    const int k = blockIdx.x * ET + threadIdx.x;
-    if (k >= n_pix_pad) return;
+                                                         const float *x, int n_pix_pad, int n_pix, ZeroSkip zs) {
+    const int k = blockIdx.x * ET + threadIdx.x;         // n_pix_pad is a multiple of ET: no ragged CTA
     pix4 += (size_t)blockIdx.y * n_pix_pad;   // blockIdx.y = channel (NEXT-4); caller arrays are [n_chan][n_pix]
     x += (size_t)blockIdx.y * n_pix;
     const int src = perm[k];
-    pix4[k].w = (src >= 0) ? amp[k] * x[src] : 0.f;
+    float4 v = pix4[k];
+    v.w = (src >= 0) ? amp[k] * x[src] : 0.f;
+    pix4[k].w = v.w;
+    compact_tile(zs, blockIdx.y, n_pix_pad, v);
 }
 
 // sorted[k] = caller[perm[k]] (0 on padding)
@@ -61,11 +94,14 @@ __global__ void __launch_bounds__(ET) scatter_kernel(const float *sorted, const 
 
 // pix4[k].w = a_k * xs[k]  (sorted order in)
 __global__ void __launch_bounds__(ET) pack_sorted_kernel(float4 *pix4, const float *amp, const float *xs,
-                                                         int n_pix_pad) {
+                                                         int n_pix_pad, ZeroSkip zs) {
     const int k = blockIdx.x * ET + threadIdx.x;
     pix4 += (size_t)blockIdx.y * n_pix_pad;
     xs += (size_t)blockIdx.y * n_pix_pad;
-    if (k < n_pix_pad) pix4[k].w = amp[k] * xs[k];
+    float4 v = pix4[k];
+    v.w = amp[k] * xs[k];
+    pix4[k].w = v.w;
+    compact_tile(zs, blockIdx.y, n_pix_pad, v);
 }
 
 __global__ void __launch_bounds__(ET) fill_kernel(float *p, float v, const int *perm, int n_pix_pad) {
@@ -155,9 +191,10 @@ __global__ void __launch_bounds__(ET) fista_update_kernel(const float *ws, int n
                                                           const float *amp, float4 *pix4, float *I_sorted,
                                                           float *y_sorted, float inv_L, float thr, float beta,
                                                           double *part_l1, double *part_nnz,
-                                                          const float2 *step_c, int n_part) {
+                                                          const float2 *step_c, int n_part, ZeroSkip zs) {
     const int k = blockIdx.x * ET + threadIdx.x;
     double l1 = 0.0, nz = 0.0;
+    float4 pv = make_float4(0.f, 0.f, 0.f, 0.f);
     const int c = blockIdx.y;                            // channel; step_c[c] = (1/L_c, lambda_c/L_c) when batched
     ws += (size_t)c * n_split * n_pix_pad;
     pix4 += (size_t)c * n_pix_pad;
@@ -183,10 +220,13 @@ __global__ void __launch_bounds__(ET) fista_update_kernel(const float *ws, int n
         const float y_new = fmaf(beta, I_new - I_old, I_new);
         I_sorted[k] = I_new;
         y_sorted[k] = y_new;
-        pix4[k].w = a * y_new;
+        pv = pix4[k];
+        pv.w = a * y_new;
+        pix4[k].w = pv.w;
         l1 = I_new;
         nz = (I_new != 0.f) ? 1.0 : 0.0;
     }
+    compact_tile(zs, c, n_pix_pad, pv);
     if (part_l1) {
         const double t1 = block_sum(l1);
         const double t2 = block_sum(nz);
@@ -216,15 +256,18 @@ __global__ void __launch_bounds__(ET) sum_partials_kernel(const double *p0, cons
 
 // Power iteration (a7): x = g / ||g||, packed straight into the pixel tiles; norm2 on device.
 __global__ void __launch_bounds__(ET) normalize_pack_kernel(const float *g_sorted, const double *norm2,
-                                                            const float *amp, float4 *pix4, int n_pix_pad) {
+                                                            const float *amp, float4 *pix4, int n_pix_pad,
+                                                            ZeroSkip zs) {
     const int k = blockIdx.x * ET + threadIdx.x;
-    if (k >= n_pix_pad) return;
     g_sorted += (size_t)blockIdx.y * n_pix_pad;
     pix4 += (size_t)blockIdx.y * n_pix_pad;
     norm2 += (size_t)blockIdx.y * 4;                     // scalars are [n_chan][4]
     const double nrm = sqrt(*norm2);
     const float x = (nrm > 0.0) ? (float)((double)g_sorted[k] / nrm) : 0.f;
-    pix4[k].w = amp[k] * x;
+    float4 v = pix4[k];
+    v.w = amp[k] * x;
+    pix4[k].w = v.w;
+    compact_tile(zs, blockIdx.y, n_pix_pad, v);
 }
 
 // Gain table re-layout: raw [n_ant][n_pix] (caller order) -> gF [n_pix_pad][n_ant], gA [n_ant][n_pix_pad].

@@ -48,6 +48,11 @@ struct ApplyParams {
     const float4 *pix4;             // [n_pix_pad] (dl, dm, dn', a*x)   .w rewritten per forward
     const float2 *pixg;             // [n_pix_pad] (sigma^2, -pi log2(e) sigma^2)  (Gaussian only)
     const double4 *cen;             // [n_tiles]   (l_c, m_c, n'_c, 0)
+    // zero-skipping forward: when tile_cnt != NULL, pix4 is the COMPACT copy of the
+    // tiles -- the pixels of tile t with a*x != 0 moved to its front in their original order -- and
+    // tile_cnt[c][t] is how many of them the forward has to stream (rounded up to a multiple of 4, the
+    // padding entries carry a*x = 0).  Exact: a skipped term is a*x*M_jk = 0.  Unit-gain kernels only.
+    const int *tile_cnt;            // [n_chan][n_tiles] or NULL (dense: every tile has TP pixels)
     // gains
     int n_ant;
     const float2 *gF;               // [n_pix_pad][n_ant]  forward layout
@@ -74,6 +79,11 @@ __device__ __forceinline__ double chan_scale_of(const ApplyParams &P) {
 template <bool BATCH>
 __device__ __forceinline__ size_t chan_index() {
     return BATCH ? (size_t)blockIdx.z : (size_t)0;
+}
+// pixels of tile t the forward streams (a multiple of 4; TP without the zero-skipping compaction)
+template <bool BATCH>
+__device__ __forceinline__ int tile_pixels(const ApplyParams &P, int t) {
+    return P.tile_cnt ? __ldg(P.tile_cnt + chan_index<BATCH>() * P.n_tiles + t) : TP;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -367,7 +377,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     // entries are samples of ONE baseline (p, q): the gain product G is loaded once per pixel.
     static_assert(GK != 2 || RV == 8, "grouped gains need RV == 8");
 
-    constexpr uint32_t kBytes = TP * sizeof(float4) + (PK == 1 ? TP * sizeof(float2) : 0);
+    constexpr bool ZSKIP = (PK != 1 && GK == 0);   // zero-skipping needs no per-pixel side array (sigma, gains)
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
@@ -375,8 +385,9 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     }
     __syncthreads();
     auto issue = [&](int t, int st) {
-        mbar_expect_tx(&s_bar[st], kBytes);
-        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
+        const uint32_t b4 = (uint32_t)(ZSKIP ? max(tile_pixels<BATCH>(P, t), 4) : TP) * (uint32_t)sizeof(float4);
+        mbar_expect_tx(&s_bar[st], b4 + (PK == 1 ? TP * (uint32_t)sizeof(float2) : 0u));
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, b4, &s_bar[st]);
         if (PK == 1) tma_bulk_g2s(&s_pixg[st][0], P.pixg + (size_t)t * TP, TP * sizeof(float2), &s_bar[st]);
     };
     if (tid == 0) {
@@ -388,10 +399,12 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
         const int st = (t - t0) & 1;
         const uint32_t parity = ((t - t0) >> 1) & 1;
         const double4 c = P.cen[t];
+        const int npx = ZSKIP ? tile_pixels<BATCH>(P, t) : TP;
         float x0[RV], uc[RV], vc[RV];
         float tq[PK == 2 ? RV : 1], tcE[PK == 2 ? RV : 1], tlr[PK == 2 ? RV : 1];   // per-(visibility, tile) constants
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
+            if (ZSKIP && npx == 0) continue;     // empty tile (uniform over the CTA): nothing to prepare
             const int j = min(jbase + r * NT + tid, jlast);
             const double ud = sc * __ldg(P.u64 + j), vd = sc * __ldg(P.v64 + j), wd = sc * __ldg(P.w64 + j);
             x0[r] = centre_phase(ud, vd, wd, c);
@@ -412,7 +425,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
             gq1 = __ldg(gbase + P.n_ant + aq[0]);
         }
 #pragma unroll 2
-        for (int p = 0; p < TP; ++p) {
+        for (int p = 0; p < npx; ++p) {
             const float4 px = s_pix[st][p];
             float Gwr = 0.f, Gwi = 0.f;
             if (GK == 2) {
@@ -523,16 +536,16 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         aq = P.ant_q[j0];
     }
 
-    constexpr uint32_t kBytes = TP * sizeof(float4);
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
-    auto issue = [&](int t, int st) {
-        mbar_expect_tx(&s_bar[st], kBytes);
-        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, kBytes, &s_bar[st]);
+    auto issue = [&](int t, int st) {   // only the pixels the tile has to stream (an empty tile still moves 64 B: barrier phases stay in step)
+        const uint32_t bytes = (uint32_t)max(tile_pixels<BATCH>(P, t), 4) * (uint32_t)sizeof(float4);
+        mbar_expect_tx(&s_bar[st], bytes);
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, bytes, &s_bar[st]);
     };
     if (tid == 0) {
         if (t0 < t1) issue(t0, 0);
@@ -591,13 +604,16 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
     for (int t = t0; t < t1; ++t) {
         const int st = (t - t0) & 1;
         const uint32_t parity = ((t - t0) >> 1) & 1;
-        const double4 c = P.cen[t];
+        const int npx = tile_pixels<BATCH>(P, t);   // zero-skipping: pixels with a*x != 0 (all TP when dense)
         f32x2 X0[NPAIR];
+        if (npx > 0) {
+            const double4 c = P.cen[t];
 #pragma unroll
-        for (int i = 0; i < NPAIR; ++i) {
-            const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
-            X0[i] = pk2(centre_phase(sc * __ldg(P.u64 + ja), sc * __ldg(P.v64 + ja), sc * __ldg(P.w64 + ja), c),
-                        centre_phase(sc * __ldg(P.u64 + jb), sc * __ldg(P.v64 + jb), sc * __ldg(P.w64 + jb), c));
+            for (int i = 0; i < NPAIR; ++i) {
+                const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
+                X0[i] = pk2(centre_phase(sc * __ldg(P.u64 + ja), sc * __ldg(P.v64 + ja), sc * __ldg(P.w64 + ja), c),
+                            centre_phase(sc * __ldg(P.u64 + jb), sc * __ldg(P.v64 + jb), sc * __ldg(P.w64 + jb), c));
+            }
         }
         mbar_wait(&s_bar[st], parity);
         if (GAINS) {
@@ -610,7 +626,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
                 gq[d] = __ldg(gbase + (size_t)d * P.n_ant + aq);
             }
 #pragma unroll 1
-            for (int p = 0; p < TP; p += 4) {
+            for (int p = 0; p < npx; p += 4) {
                 float Gwr[4], Gwi[4];
 #pragma unroll
                 for (int d = 0; d < 4; ++d) {
@@ -628,7 +644,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
             }
         } else {
 #pragma unroll 1
-            for (int p = 0; p < TP; p += 4) {
+            for (int p = 0; p < npx; p += 4) {
                 pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, 0.f, 0.f);
                 pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, 0.f, 0.f);
                 pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, 0.f, 0.f);
@@ -1140,16 +1156,16 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_GTX2_MIN_CTAS) fwd_kernel_gtx2(co
         s_acc[i][tid] = pk2(0.f, 0.f);
         s_acc[NPAIR + i][tid] = pk2(0.f, 0.f);
     }
-    constexpr uint32_t kBytes = TP * sizeof(float4);
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
-    auto issue = [&](int t, int st) {
-        mbar_expect_tx(&s_bar[st], kBytes);
-        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, kBytes, &s_bar[st]);
+    auto issue = [&](int t, int st) {   // only the pixels the tile has to stream (zero-skipping; >= 64 B)
+        const uint32_t bytes = (uint32_t)max(tile_pixels<BATCH>(P, t), 4) * (uint32_t)sizeof(float4);
+        mbar_expect_tx(&s_bar[st], bytes);
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, bytes, &s_bar[st]);
     };
     if (tid == 0) {
         if (t0 < t1) issue(t0, 0);
@@ -1159,6 +1175,13 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_GTX2_MIN_CTAS) fwd_kernel_gtx2(co
         const int st = (t - t0) & 1;
         const uint32_t parity = ((t - t0) >> 1) & 1;
         const double4 c = P.cen[t];
+        const int npx = tile_pixels<BATCH>(P, t);
+        if (npx == 0) {                          // empty tile (uniform over the CTA): consume the stage and move on
+            mbar_wait(&s_bar[st], parity);
+            __syncthreads();
+            if (tid == 0 && t + 2 < t1) issue(t + 2, st);
+            continue;
+        }
         f32x2 X0[NPAIR], UC[NPAIR], VC2[NPAIR], CE[NPAIR], LR[NPAIR], CX[NPAIR], TC[NPAIR], TS[NPAIR];
 #pragma unroll
         for (int i = 0; i < NPAIR; ++i) {
@@ -1183,7 +1206,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_GTX2_MIN_CTAS) fwd_kernel_gtx2(co
         }
         mbar_wait(&s_bar[st], parity);
 #pragma unroll 1
-        for (int p = 0; p < TP; ++p) {
+        for (int p = 0; p < npx; ++p) {
             const float4 px = s_pix[st][p];
             const f32x2 bx = bc2(px.x), by = bc2(px.y), bz = bc2(px.z), bw = bc2(px.w);
 #pragma unroll

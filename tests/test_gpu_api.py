@@ -266,3 +266,62 @@ def test_fp64_phase_path(sl):
         xs, _ = plan.solve(_dev(V, torch.complex64), 0.5, L=L, n_iter=40)
         assert rel_l2(xs.cpu().numpy(), o.fista(V, 0.5, L, 40)["x"]) <= 1e-3
         plan.close()
+
+
+@pytest.mark.parametrize("kind", ["delta", "gauss_tiles", "delta_small"])
+def test_zero_skipping_forward(sl, kind):
+    """The forward streams only pixels with x_k != 0 (sl1m_forward_active_pixels; eq (18), PAPER.md:194-197,
+    makes the iterates sparse).  Against the oracle and against a SL1M_DENSE_FORWARD plan: an all-zero image,
+    one source, tiles holding 1..5 non-zeros (ragged padding to 4), 1 % and 60 % random density, a dense image;
+    the packed R = 8 kernels, the one-sigma-per-tile Gaussian kernels and the scalar small-problem kernels."""
+    import torch
+    rng = np.random.default_rng(11)
+    if kind == "delta_small":
+        wl = make_workload(1)                       # RV = 1 scalar kernels
+    elif kind == "delta":
+        wl = make_workload(2, n_side=128, n_steps=3, n_src=30)
+    else:
+        wl = make_workload(3, n_side=64, n_steps=4, n_src=30)
+    o = oracle.Oracle.from_workload(wl)
+    plan = sl.Plan.from_workload(wl)
+    dense = sl.Plan.from_workload(wl, dense_forward=True)
+    assert plan.describe()["zero_skip"] == 1 and dense.describe()["zero_skip"] == 0
+    n = wl.n_pix
+    cases = {}
+    cases["zero"] = np.zeros(n, np.float32)
+    one = np.zeros(n, np.float32); one[n // 3] = 2.5
+    cases["one"] = one
+    few = np.zeros(n, np.float32); few[rng.choice(n, 37, replace=False)] = rng.uniform(0.1, 3, 37)
+    cases["few"] = few
+    for dens in (0.01, 0.6):
+        x = np.where(rng.uniform(size=n) < dens, rng.uniform(0.1, 1, n), 0).astype(np.float32)
+        cases["d%g" % dens] = x
+    cases["dense"] = rng.uniform(0.1, 1, n).astype(np.float32)
+    for name, x in cases.items():
+        xd = _dev(x, torch.float32)
+        v = plan.forward(xd).cpu().numpy()
+        act = plan.forward_active_pixels()
+        nnz = int(np.count_nonzero(x))
+        assert nnz <= act <= min(nnz + 3 * plan.describe()["n_tiles"], plan.describe()["n_pix_padded"]), (name, nnz, act)
+        vd = dense.forward(xd).cpu().numpy()
+        assert dense.forward_active_pixels() == dense.describe()["n_pix_padded"]
+        want = o.forward(x)
+        if nnz == 0:
+            assert not v.any() and not vd.any()
+            continue
+        assert rel_l2(v, want) <= 2e-4, (name, rel_l2(v, want))
+        assert rel_l2(v, vd) <= 2e-5, (name, rel_l2(v, vd))
+        assert np.array_equal(v, plan.forward(xd).cpu().numpy())            # bit-stable
+    # the solver takes the same iterates with and without skipping (differences: which terms take the
+    # polynomial sincos, i.e. rounding only)
+    V = _dev((o.forward(cases["few"]) + 0.01 * (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis))
+              ).astype(np.complex64), torch.complex64)
+    L = dense.max_eig(8) * 1.05
+    assert abs(plan.max_eig(8) * 1.05 / L - 1) < 1e-5
+    lam = 0.02 * float(np.abs(dense.adjoint(V).cpu().numpy()).max())
+    a, ia = plan.solve(V, lam, L=L, n_iter=30)
+    b, ib = dense.solve(V, lam, L=L, n_iter=30)
+    assert rel_l2(a.cpu().numpy(), b.cpu().numpy()) <= 1e-4
+    assert 0 < ia.nnz < n and abs(ia.nnz - ib.nnz) <= max(2, ib.nnz // 100)
+    assert plan.forward_active_pixels() < plan.describe()["n_pix_padded"]   # the last forward really skipped
+    plan.close(); dense.close()
