@@ -236,8 +236,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     t_wall0 = time.time()
     torch.cuda.synchronize()
     for _ in range(args.steps):
-        flush.zero_()
         nnz_steps.append(torch.count_nonzero(x))      # outside the timed events; read back after the loop
+        flush.zero_()
         a, b = ev(), ev()
         a.record(stream)
         plan.solve(V, lam, L=L, n_iter=1, x0=x, out=x_next, want_info=False)

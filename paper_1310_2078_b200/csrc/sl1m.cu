@@ -52,6 +52,7 @@ struct sl1m_plan {
     float4 *pix4 = nullptr;
     float4 *pixc = nullptr;       // [n_chan][n_pix_pad] compact tiles of the zero-skipping forward (NULL = dense forward)
     int *tile_cnt = nullptr;      // [n_chan][n_tiles] pixels per compact tile
+    float2 *gFc = nullptr;        // [n_chan][n_pix_pad][n_ant] gain rows of the compact entries (gain plans only)
     bool dense_forward = false;   // SL1M_DENSE_FORWARD: never skip
     float2 *pixg = nullptr;
     double4 *cen = nullptr;
@@ -96,7 +97,7 @@ void free_plan(sl1m_plan *p) {
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
-                    p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt};
+                    p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -187,7 +188,7 @@ int configure_and_allocate(sl1m_plan *p) {
     const size_t npad = (size_t)p->n_pix_pad, C = (size_t)p->n_chan;
     for (void **q : {(void **)&p->ws_v, (void **)&p->ws_p, (void **)&p->resid, (void **)&p->I_sorted, (void **)&p->y_sorted,
                      (void **)&p->g_sorted, (void **)&p->part_a, (void **)&p->part_b, (void **)&p->part_c, (void **)&p->scalars,
-                     (void **)&p->pixc, (void **)&p->tile_cnt}) {
+                     (void **)&p->pixc, (void **)&p->tile_cnt, (void **)&p->gFc}) {
         if (*q) cudaFree(*q);
         *q = nullptr;
     }
@@ -203,12 +204,19 @@ int configure_and_allocate(sl1m_plan *p) {
     CUDA_TRY(cudaMalloc((void **)&p->part_c, C * (size_t)p->n_part * sizeof(double)));
     CUDA_TRY(cudaMalloc((void **)&p->scalars, C * 4 * sizeof(double)));
     CUDA_TRY(cudaMemset(p->scalars, 0, C * 4 * sizeof(double)));
-    // zero-skipping forward: kernels without a per-pixel side array (gains, per-pixel sigma, fp64 offsets)
-    if (!p->dense_forward && p->gk == 0 && p->pk != 1 && !(p->phase64 && p->n_chan == 1)) {
+    // zero-skipping forward: every kernel but those with a per-pixel side array in shared memory (per-pixel
+    // sigma, fp64 offsets).  Gain plans keep a compact copy of the gain rows next to the compact tiles
+    // (n_chan x the table; not beyond 8 GiB -- such a plan keeps the dense forward).
+    const size_t gfc_bytes = p->gk != 0 ? C * npad * (size_t)p->n_ant * sizeof(float2) : 0;
+    if (!p->dense_forward && p->pk != 1 && !(p->phase64 && p->n_chan == 1) && gfc_bytes <= ((size_t)8 << 30)) {
         CUDA_TRY(cudaMalloc((void **)&p->pixc, C * npad * sizeof(float4)));
         CUDA_TRY(cudaMalloc((void **)&p->tile_cnt, C * (size_t)p->n_tiles * sizeof(int)));
         CUDA_TRY(cudaMemset(p->pixc, 0, C * npad * sizeof(float4)));
         CUDA_TRY(cudaMemset(p->tile_cnt, 0, C * (size_t)p->n_tiles * sizeof(int)));
+        if (gfc_bytes) {
+            CUDA_TRY(cudaMalloc((void **)&p->gFc, gfc_bytes));
+            CUDA_TRY(cudaMemset(p->gFc, 0, gfc_bytes));
+        }
     }
     CUDA_TRY(cudaDeviceSynchronize());
 
@@ -489,7 +497,7 @@ namespace {
 
 inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
 inline dim3 cgrid(const sl1m_plan *p, size_t n) { return dim3((unsigned)egrid(n), (unsigned)p->n_chan); }  // x: elements, y: channel
-inline ZeroSkip zs_of(const sl1m_plan *p) { return ZeroSkip{p->pixc, p->tile_cnt}; }
+inline ZeroSkip zs_of(const sl1m_plan *p) { return ZeroSkip{p->pixc, p->tile_cnt, p->gF, p->gFc, p->n_ant}; }
 
 template <int PK, int GK, bool B>
 void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
@@ -554,6 +562,7 @@ void launch_fwd(sl1m_plan *p, cudaStream_t s) {
     if (p->pixc) {   // zero-skipping: stream the compact tiles the packing kernel left behind
         P.pix4 = p->pixc;
         P.tile_cnt = p->tile_cnt;
+        P.gFc = p->gFc;
     }
     const int key = p->pk * 3 + p->gk;   // pk == 2 (one sigma per tile) only exists with unit gains
     switch (key) {

@@ -30,14 +30,21 @@ __device__ __forceinline__ double block_sum(double v) {
 // tile blockIdx.x.  The entries with a*x != 0 move to the front of the COMPACT copy of the tile in their
 // original order, padded with a*x = 0 entries to a multiple of 4; zs.cnt[c][tile] = the padded count.  The
 // forward kernels stream only that many pixels of the tile: the skipped terms are exactly zero.
+// Plans with a gain table: the forward-layout gain rows gF[k][.] of the compact entries are copied next to them
+// (gFc, same tile layout), so the kernels keep walking consecutive rows; a full tile is not copied (the kernels
+// read gF for it).  A dense image therefore costs nothing extra, a sparse one n_ant * 8 B per non-zero pixel.
 struct ZeroSkip {
-    float4 *pixc;   // DEV [n_chan][n_pix_pad] compact tiles, NULL = off (gains, per-pixel sigma, fp64 phase)
-    int *cnt;       // DEV [n_chan][n_tiles]
+    float4 *pixc;        // DEV [n_chan][n_pix_pad] compact tiles, NULL = off (per-pixel sigma, fp64 phase)
+    int *cnt;            // DEV [n_chan][n_tiles]
+    const float2 *gF;    // DEV [n_pix_pad][n_ant] or NULL (unit gains)
+    float2 *gFc;         // DEV [n_chan][n_pix_pad][n_ant]
+    int n_ant;
 };
 static_assert(ET == TP, "one packing CTA per pixel tile");
 __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int n_pix_pad, float4 v) {
     if (!zs.pixc) return;                                // uniform over the grid
     __shared__ int s_wcnt[ET / 32];
+    __shared__ uint8_t s_src[ET];                        // original in-tile index of compact entry p (gain rows)
     const bool nz = (v.w != 0.f);                        // NaN counts as non-zero: it propagates as in the dense path
     const unsigned b = __ballot_sync(0xffffffffu, nz);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -51,10 +58,25 @@ __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int
         total += c;
     }
     float4 *tile = zs.pixc + chan * n_pix_pad + (size_t)blockIdx.x * TP;
-    if (nz) tile[base + __popc(b & ((1u << lane) - 1u))] = v;
+    if (nz) {
+        const int pos = base + __popc(b & ((1u << lane) - 1u));
+        tile[pos] = v;
+        s_src[pos] = (uint8_t)threadIdx.x;
+    }
     const int cnt4 = (total + 3) & ~3;
     if ((int)threadIdx.x < cnt4 - total) tile[total + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (threadIdx.x == 0) zs.cnt[chan * (size_t)(n_pix_pad / TP) + blockIdx.x] = cnt4;
+    if (zs.gF && total < TP && total > 0) {              // gain rows of the compact entries (padding: a*x = 0, any row)
+        __syncthreads();
+        const size_t row0 = (size_t)blockIdx.x * TP;
+        const float2 *src = zs.gF + row0 * zs.n_ant;
+        float2 *dst = zs.gFc + (chan * n_pix_pad + row0) * zs.n_ant;
+        const int n = cnt4 * zs.n_ant;
+        for (int i = threadIdx.x; i < n; i += ET) {
+            const int row = i / zs.n_ant, a = i - row * zs.n_ant;
+            dst[i] = src[(size_t)s_src[min(row, total - 1)] * zs.n_ant + a];
+        }
+    }
 }
 
 // pix4[k].w = a_k * x[perm[k]]   (caller order -> sorted, padded pixels get 0)

@@ -53,6 +53,8 @@ struct ApplyParams {
     // tile_cnt[c][t] is how many of them the forward has to stream (rounded up to a multiple of 4, the
     // padding entries carry a*x = 0).  Exact: a skipped term is a*x*M_jk = 0.  Unit-gain kernels only.
     const int *tile_cnt;            // [n_chan][n_tiles] or NULL (dense: every tile has TP pixels)
+    const float2 *gFc;              // [n_chan][n_pix_pad][n_ant] gain rows of the compact entries of every tile
+                                    // that is not full (a full tile is read from gF); gain plans only
     // gains
     int n_ant;
     const float2 *gF;               // [n_pix_pad][n_ant]  forward layout
@@ -84,6 +86,12 @@ __device__ __forceinline__ size_t chan_index() {
 template <bool BATCH>
 __device__ __forceinline__ int tile_pixels(const ApplyParams &P, int t) {
     return P.tile_cnt ? __ldg(P.tile_cnt + chan_index<BATCH>() * P.n_tiles + t) : TP;
+}
+// forward-layout gain rows of tile t: the compact copy when the tile was compacted (npx < TP), else the table
+template <bool BATCH>
+__device__ __forceinline__ const float2 *tile_gain_rows(const ApplyParams &P, int t, int npx) {
+    const float2 *g = (P.tile_cnt && npx < TP) ? P.gFc + chan_index<BATCH>() * (size_t)P.n_pix_pad * P.n_ant : P.gF;
+    return g + (size_t)t * TP * P.n_ant;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -377,7 +385,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     // entries are samples of ONE baseline (p, q): the gain product G is loaded once per pixel.
     static_assert(GK != 2 || RV == 8, "grouped gains need RV == 8");
 
-    constexpr bool ZSKIP = (PK != 1 && GK == 0);   // zero-skipping needs no per-pixel side array (sigma, gains)
+    constexpr bool ZSKIP = (PK != 1);   // zero-skipping: every kernel but the per-pixel-sigma ones (side array in smem)
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
@@ -415,7 +423,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
             if (PK == 2) gauss_tile_constants(wd, c.w, tq[r], tcE[r], tlr[r], x0[r]);
         }
         mbar_wait(&s_bar[st], parity);
-        const float2 *gbase = GK ? P.gF + (size_t)t * TP * P.n_ant : nullptr;
+        const float2 *gbase = GK ? tile_gain_rows<BATCH>(P, t, npx) : nullptr;
         // grouped gains: register prefetch two pixels ahead (rows are cold in L1 on first touch)
         float2 gp0, gq0, gp1, gq1;
         if (GK == 2) {
@@ -618,7 +626,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         mbar_wait(&s_bar[st], parity);
         if (GAINS) {
             // gain rows of the tile, gF[k][a]: register prefetch 4 pixels ahead (cold in L1 on first touch)
-            const float2 *gbase = P.gF + (size_t)t * TP * P.n_ant;
+            const float2 *gbase = tile_gain_rows<BATCH>(P, t, npx);
             float2 gp[4], gq[4];
 #pragma unroll
             for (int d = 0; d < 4; ++d) {
@@ -633,7 +641,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
                     const float w = s_pix[st][p + d].w;
                     Gwr[d] = w * fmaf(gp[d].y, gq[d].y, gp[d].x * gq[d].x);    // a x Re(g_p conj g_q)
                     Gwi[d] = w * fmaf(gp[d].y, gq[d].x, -gp[d].x * gq[d].y);
-                    const int pn = min(p + 4 + d, TP - 1);
+                    const int pn = min(p + 4 + d, TP - 1);   // rows past npx exist (stale or zero): harmless prefetch
                     gp[d] = __ldg(gbase + (size_t)pn * P.n_ant + ap);
                     gq[d] = __ldg(gbase + (size_t)pn * P.n_ant + aq);
                 }

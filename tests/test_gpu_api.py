@@ -268,24 +268,31 @@ def test_fp64_phase_path(sl):
         plan.close()
 
 
-@pytest.mark.parametrize("kind", ["delta", "gauss_tiles", "delta_small"])
+@pytest.mark.parametrize("kind", ["delta", "gauss_tiles", "delta_small", "gains_grouped", "gains_per_term"])
 def test_zero_skipping_forward(sl, kind):
     """The forward streams only pixels with x_k != 0 (sl1m_forward_active_pixels; eq (18), PAPER.md:194-197,
     makes the iterates sparse).  Against the oracle and against a SL1M_DENSE_FORWARD plan: an all-zero image,
     one source, tiles holding 1..5 non-zeros (ragged padding to 4), 1 % and 60 % random density, a dense image;
-    the packed R = 8 kernels, the one-sigma-per-tile Gaussian kernels and the scalar small-problem kernels."""
+    the packed R = 8 kernels, the one-sigma-per-tile Gaussian kernels, the scalar small-problem kernels, and the
+    two gain-table kernels (gain rows are looked up through the compact entries' original index)."""
     import torch
     rng = np.random.default_rng(11)
     if kind == "delta_small":
         wl = make_workload(1)                       # RV = 1 scalar kernels
     elif kind == "delta":
         wl = make_workload(2, n_side=128, n_steps=3, n_src=30)
+    elif kind == "gains_grouped":
+        wl = make_workload(4, n_side=64, n_ant=20, n_steps=8, n_src=50)      # gk == 2
+    elif kind == "gains_per_term":
+        wl = make_workload(4, n_side=64, n_ant=20, n_steps=3, n_src=50)      # gk == 1
     else:
         wl = make_workload(3, n_side=64, n_steps=4, n_src=30)
     o = oracle.Oracle.from_workload(wl)
     plan = sl.Plan.from_workload(wl)
     dense = sl.Plan.from_workload(wl, dense_forward=True)
     assert plan.describe()["zero_skip"] == 1 and dense.describe()["zero_skip"] == 0
+    if kind.startswith("gains"):
+        assert plan.describe()["gains"] == (2 if kind == "gains_grouped" else 1)
     n = wl.n_pix
     cases = {}
     cases["zero"] = np.zeros(n, np.float32)
