@@ -37,7 +37,7 @@ MUFU_PER_SM_PER_CLK = 16      # 4 SFU lanes per SM sub-partition x 4 (measured 1
 SM_COUNT = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (config, kernel) -> bytes
-NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 29.33e6, (5, "adj"): 30.30e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 58.47e6, (5, "adj"): 35.78e6, (4, "fwd"): 341.1e6, (4, "adj"): 11578.2e6}
 
 
 def _peaks():
@@ -232,11 +232,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     time.sleep(0.3)
     launches0 = plan.launch_count
     pairs = []
-    nnz_steps = []          # non-zero pixels of each step's forward input (zero-skipping forward), device scalars
+    nnz_steps = []          # non-zero pixels of each step's forward input (zero-skipping forward)
     t_wall0 = time.time()
     torch.cuda.synchronize()
     for _ in range(args.steps):
-        nnz_steps.append(torch.count_nonzero(x))      # outside the timed events; read back after the loop
+        nnz_steps.append(torch.count_nonzero(x))      # device scalar, queued before the flush; read after the loop
         flush.zero_()
         a, b = ev(), ev()
         a.record(stream)
@@ -358,7 +358,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                       f"x 128 fp32 lanes/clk, x 128 thread-instr/clk; fwd {desc['fwd_poly_per16']}/16 and adj "
                       f"{desc['adj_poly_per16']}/16 of the terms use FMA-pipe polynomial sincos",
         "traffic_basis": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full "
-                         "(profiles/, same kernel and workload); algorithmic bytes ~30 MB per apply",
+                         "(profiles/, same kernel and workload); algorithmic bytes at config 5: ~30 MB in per apply "
+                         "+ the split partials (24 x 3.25 MB forward, 10 x 4 MB adjoint, mostly L2-resident)",
         "mufu_only_bound_Tterm_per_s": mufu_only / 1e12,
         "frac_vs_mufu_only_bound": achieved / mufu_only,
         "best_split_bound_Tterm_per_s": None if balanced is None else balanced / 1e12,
