@@ -35,6 +35,7 @@ int fail(int st, const std::string &msg) {
     } while (0)
 
 constexpr int SM_COUNT_B200 = 148;
+constexpr int GAIN_ROW_PAD = 4;   // rows of padding behind the forward-layout gain tables (prefetch distance of the kernels)
 
 }  // namespace
 
@@ -207,7 +208,7 @@ int configure_and_allocate(sl1m_plan *p) {
     // zero-skipping forward: every kernel but those with a per-pixel side array in shared memory (per-pixel
     // sigma, fp64 offsets).  Gain plans keep a compact copy of the gain rows next to the compact tiles
     // (n_chan x the table; not beyond 8 GiB -- such a plan keeps the dense forward).
-    const size_t gfc_bytes = p->gk != 0 ? C * npad * (size_t)p->n_ant * sizeof(float2) : 0;
+    const size_t gfc_bytes = p->gk != 0 ? (C * npad + GAIN_ROW_PAD) * (size_t)p->n_ant * sizeof(float2) : 0;
     if (!p->dense_forward && p->pk != 1 && !(p->phase64 && p->n_chan == 1) && gfc_bytes <= ((size_t)8 << 30)) {
         CUDA_TRY(cudaMalloc((void **)&p->pixc, C * npad * sizeof(float4)));
         CUDA_TRY(cudaMalloc((void **)&p->tile_cnt, C * (size_t)p->n_tiles * sizeof(int)));
@@ -467,7 +468,9 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
             if (e != cudaSuccess) { cudaFree(raw); return fail(SL1M_ERR_CUDA, cudaGetErrorString(e)); }
         }
         const size_t lay_n = (size_t)p->n_pix_pad * (size_t)n_ant;
-        cudaError_t e1 = cudaMalloc((void **)&p->gF, lay_n * sizeof(float2));
+        // gF carries GAIN_ROW_PAD rows of zero padding: the forward kernels prefetch one group of 4 rows ahead
+        cudaError_t e1 = cudaMalloc((void **)&p->gF, (lay_n + (size_t)GAIN_ROW_PAD * n_ant) * sizeof(float2));
+        if (e1 == cudaSuccess) e1 = cudaMemset(p->gF + lay_n, 0, (size_t)GAIN_ROW_PAD * n_ant * sizeof(float2));
         cudaError_t e2 = (e1 == cudaSuccess) ? cudaMalloc((void **)&p->gA, lay_n * sizeof(float2)) : e1;
         if (e2 == cudaSuccess) {
             dim3 grid((p->n_pix_pad + ET - 1) / ET, n_ant);

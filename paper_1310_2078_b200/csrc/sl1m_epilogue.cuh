@@ -292,7 +292,8 @@ __global__ void __launch_bounds__(ET) normalize_pack_kernel(const float *g_sorte
     compact_tile(zs, blockIdx.y, n_pix_pad, v);
 }
 
-// Gain table re-layout: raw [n_ant][n_pix] (caller order) -> gF [n_pix_pad][n_ant], gA [n_ant][n_pix_pad].
+// Gain table re-layout: raw [n_ant][n_pix] (re, im; caller order) -> gF [n_pix_pad][n_ant], gA [n_ant][n_pix_pad],
+// both in polar form.
 __global__ void __launch_bounds__(ET) gains_layout_kernel(const float2 *raw, int n_ant, int n_pix,
                                                           int n_pix_pad, const int *perm, float2 *gF,
                                                           float2 *gA) {
@@ -300,7 +301,14 @@ __global__ void __launch_bounds__(ET) gains_layout_kernel(const float2 *raw, int
     const int a = blockIdx.y;
     if (k >= n_pix_pad) return;
     const int src = perm[k];
-    const float2 g = (src >= 0) ? raw[(size_t)a * n_pix + src] : make_float2(0.f, 0.f);
+    // polar form (|g|, arg g), evaluated in fp64: the kernels multiply the entry by |g_p||g_q| and shift its
+    // phase by arg_p - arg_q (G = g_p conj(g_q)); a zero gain has amplitude 0 and phase 0
+    float2 g = make_float2(0.f, 0.f);
+    if (src >= 0) {
+        const float2 c = raw[(size_t)a * n_pix + src];
+        const double re = (double)c.x, im = (double)c.y;
+        g = make_float2((float)sqrt(re * re + im * im), (float)atan2(im, re));
+    }
     gF[(size_t)k * n_ant + a] = g;
     gA[(size_t)a * n_pix_pad + k] = g;
 }

@@ -87,6 +87,22 @@ template <bool BATCH>
 __device__ __forceinline__ int tile_pixels(const ApplyParams &P, int t) {
     return P.tile_cnt ? __ldg(P.tile_cnt + chan_index<BATCH>() * P.n_tiles + t) : TP;
 }
+// Adjoint CTA -> (pixel group, visibility split).  The grid is (pixel groups, splits) and CTAs are scheduled in
+// linear order, x fastest.  With a gain table the CTAs resident at one time should share PIXEL GROUPS (their gain
+// columns gA[a][group] then stay in L2 across the splits) instead of sharing a split: config 4 read the 256 MiB
+// table from DRAM once per split (11.5 GB per launch, profiles/r1_ncu_full_gain_kernels_config4.md).  SWAP makes
+// the split the fast index of the linear CTA number.
+template <bool SWAP>
+__device__ __forceinline__ void adj_cta(int &group, int &split) {
+    if (SWAP) {
+        const unsigned lin = blockIdx.y * gridDim.x + blockIdx.x;
+        group = (int)(lin / gridDim.y);
+        split = (int)(lin - (unsigned)group * gridDim.y);
+    } else {
+        group = (int)blockIdx.x;
+        split = (int)blockIdx.y;
+    }
+}
 // forward-layout gain rows of tile t: the compact copy when the tile was compacted (npx < TP), else the table
 template <bool BATCH>
 __device__ __forceinline__ const float2 *tile_gain_rows(const ApplyParams &P, int t, int npx) {
@@ -172,6 +188,14 @@ __device__ __forceinline__ void sincos_poly(float X, float &s, float &c, uint32_
     sign = __float_as_uint(kf) << 31;
 }
 __device__ __forceinline__ float fxor(float a, uint32_t m) { return __uint_as_float(__float_as_uint(a) ^ m); }
+// sin x, cos x by the same polynomials, signs applied (centre-phase rotations of the gain kernels: once per
+// (visibility, tile), as accurate as the polynomial terms, no MUFU, no slow-path stack frame)
+__device__ __forceinline__ void sincos_fma(float X, float &s, float &c) {
+    uint32_t sg;
+    sincos_poly(X, s, c, sg);
+    s = fxor(s, sg);
+    c = fxor(c, sg);
+}
 
 // ------------------------------------------------------------------------------------------
 // Packed fp32 pairs (sm_100a FFMA2/FMUL2/FADD2): one issue slot carries two FMAs.  The MUFU-bound
@@ -322,7 +346,7 @@ __device__ __forceinline__ void gen_entry_tile(float X, float du, float dv, floa
 #endif
 //   *_G2_NPQ   the same fraction for the packed kernels with baseline-grouped gains
 #ifndef SL1M_FWD_G2_NPQ
-#define SL1M_FWD_G2_NPQ 4
+#define SL1M_FWD_G2_NPQ 3
 #endif
 #ifndef SL1M_ADJ_G2_NPQ
 #define SL1M_ADJ_G2_NPQ 4
@@ -435,7 +459,9 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
 #pragma unroll 2
         for (int p = 0; p < npx; ++p) {
             const float4 px = s_pix[st][p];
-            float Gwr = 0.f, Gwi = 0.f;
+            // gains are stored in polar form (|g|, arg g):  G = g_p conj(g_q) = |g_p||g_q| e^{i(arg_p - arg_q)}
+            // multiplies the entry by a real factor and shifts its phase: M x = (a x |G|) e^{-i(X - gamma)}
+            float Gw = px.w, gam = 0.f;
             if (GK == 2) {
                 const float2 gp = gp0, gq = gq0;
                 gp0 = gp1;
@@ -443,8 +469,8 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 const int pn = min(p + 2, TP - 1);
                 gp1 = __ldg(gbase + (size_t)pn * P.n_ant + ap[0]);
                 gq1 = __ldg(gbase + (size_t)pn * P.n_ant + aq[0]);
-                Gwr = px.w * fmaf(gp.y, gq.y, gp.x * gq.x);    // a x G,  G = gp conj(gq)
-                Gwi = px.w * fmaf(gp.y, gq.x, -gp.x * gq.y);
+                Gw = px.w * (gp.x * gq.x);
+                gam = gp.y - gq.y;
             }
             float sig2 = 0.f, nsp = 0.f;
             if (PK == 1) {
@@ -454,7 +480,15 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
             }
 #pragma unroll
             for (int r = 0; r < RV; ++r) {
-                const float X = fmaf(uf[r], px.x, fmaf(vf[r], px.y, fmaf(wf[r], px.z, x0[r])));
+                float X = fmaf(uf[r], px.x, fmaf(vf[r], px.y, fmaf(wf[r], px.z, x0[r])));
+                float wg = Gw;
+                if (GK == 2) X -= gam;
+                if (GK == 1) {
+                    const float2 gp = __ldg(gbase + (size_t)p * P.n_ant + ap[r]);
+                    const float2 gq = __ldg(gbase + (size_t)p * P.n_ant + aq[r]);
+                    wg = px.w * (gp.x * gq.x);
+                    X -= gp.y - gq.y;
+                }
                 float du = 0.f, dv = 0.f;
                 if (PK) {
                     du = fmaf(-wl[r], px.x, uc[r]);
@@ -465,30 +499,16 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 if (PK == 2) {
                     float amp;
                     gen_entry_tile(X, du, dv, tq[r], tcE[r], tlr[r], amp, ere, eim);
-                    const float t = px.w * amp;
+                    const float t = wg * amp;
                     re[r] = fmaf(t, ere, re[r]);
                     im[r] = fmaf(t, eim, im[r]);
                     continue;
                 }
                 if (r < PolySplit<RV, PK, GK, SL1M_FWD_NPOLY8>::N) gen_entry<PK, true>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
                 else gen_entry<PK, false>(X, du, dv, wl[r], sig2, nsp, ere, eim, sgn);
-                const float wt = (r < PolySplit<RV, PK, GK, SL1M_FWD_NPOLY8>::N) ? fxor(px.w, sgn) : px.w;
-                if (GK == 2) {
-                    re[r] = fmaf(Gwr, ere, fmaf(-Gwi, eim, re[r]));
-                    im[r] = fmaf(Gwi, ere, fmaf(Gwr, eim, im[r]));
-                } else if (GK == 1) {
-                    const float2 gp = __ldg(gbase + (size_t)p * P.n_ant + ap[r]);
-                    const float2 gq = __ldg(gbase + (size_t)p * P.n_ant + aq[r]);
-                    const float Gr = fmaf(gp.y, gq.y, gp.x * gq.x);   // G = gp conj(gq)
-                    const float Gi = fmaf(gp.y, gq.x, -gp.x * gq.y);
-                    const float tr = fmaf(-Gi, eim, Gr * ere);
-                    const float ti = fmaf(Gi, ere, Gr * eim);
-                    re[r] = fmaf(wt, tr, re[r]);
-                    im[r] = fmaf(wt, ti, im[r]);
-                } else {
-                    re[r] = fmaf(wt, ere, re[r]);
-                    im[r] = fmaf(wt, eim, im[r]);
-                }
+                const float wt = (r < PolySplit<RV, PK, GK, SL1M_FWD_NPOLY8>::N) ? fxor(wg, sgn) : wg;
+                re[r] = fmaf(wt, ere, re[r]);
+                im[r] = fmaf(wt, eim, im[r]);
             }
         }
         __syncthreads();  // every thread is done with stage st
@@ -516,6 +536,9 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
     // NPQ of the 16 pairs of 4 consecutive pixels take the polynomial path: pixel q gets (NPQ + 3 - q) / 4
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(8) uint64_t s_bar[2];
+    // GAINS: RE/IM hold the sums of ONE tile without its centre phase; the running totals live here
+    // ([pair][thread], own slots only) and take e^{-i x0} (tile sum) at the end of every tile.
+    __shared__ __align__(8) f32x2 s_tot[GAINS ? 2 * NPAIR_X2 : 1][GAINS ? NT : 1];
 
     const int tid = threadIdx.x;
     const int t0 = blockIdx.y * P.per_split;
@@ -534,9 +557,17 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         W[i] = pk2(static_cast<float>(TWO_PI * (sc * __ldg(P.w64 + ja))), static_cast<float>(TWO_PI * (sc * __ldg(P.w64 + jb))));
         RE[i] = pk2(0.f, 0.f);
         IM[i] = pk2(0.f, 0.f);
+        if (GAINS) {
+            s_tot[i][tid] = pk2(0.f, 0.f);
+            s_tot[NPAIR + i][tid] = pk2(0.f, 0.f);
+        }
     }
     // GAINS ("baseline-grouped" plan, gk == 2): the thread's 8 visibilities are samples of ONE baseline
-    // (p, q), so G = g_p conj(g_q) is formed once per pixel and shared by the 4 pairs.
+    // (p, q).  Gains are stored in polar form (|g|, arg g), so G = g_p conj(g_q) = |G| e^{i gamma} with
+    // |G| = |g_p||g_q|, gamma = arg_p - arg_q, formed once per pixel and shared by the 4 pairs:
+    //     M_jk x_k = (a x |G|) e^{-i (X_rel - gamma)} e^{-i x0(j, tile)}
+    // -gamma is the innermost addend of the phase FMA chain (where the unit-gain kernel has x0) and the
+    // weight stays real: the term costs what a unit-gain term costs.  e^{-i x0} multiplies the tile's sum.
     int ap = 0, aq = 0;
     if (GAINS) {
         const int j0 = min(jbase + tid, jlast);
@@ -561,40 +592,18 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
     }
 
     // one pixel against the 4 pairs; the first NPOLY pairs use the FMA-pipe polynomial
-    auto pixel = [&](const float4 px, const f32x2 (&X0)[NPAIR], auto npoly_tag, float Gwr, float Gwi) {
+    // wgt: the real weight of the pixel (a x, times |G| with gains); ngam: -gamma (gains only)
+    auto pixel = [&](const float4 px, const f32x2 (&X0)[NPAIR], auto npoly_tag, float wgt, float ngam) {
         constexpr int NPOLY = decltype(npoly_tag)::value;
         const f32x2 pxx = bc2(px.x), pxy = bc2(px.y), pxz = bc2(px.z);
 #pragma unroll
         for (int i = 0; i < NPAIR; ++i) {
-            const f32x2 X = fma2(U[i], pxx, fma2(V[i], pxy, fma2(W[i], pxz, X0[i])));
-            if (GAINS) {
-                // (a x G)(c - i s):  RE += Gwr c + Gwi s,   IM (negated, as below) += Gwr s - Gwi c
-                f32x2 s, c;
-                if (i < NPOLY) {
-                    uint32_t ka, kb;
-                    sincos_poly2(X, s, c, ka, kb);
-                    float sa, sb, ca, cb;
-                    up2(s, sa, sb);
-                    up2(c, ca, cb);
-                    s = pk2(flip_if_odd(sa, ka), flip_if_odd(sb, kb));
-                    c = pk2(flip_if_odd(ca, ka), flip_if_odd(cb, kb));
-                } else {
-                    float xa, xb, sa, ca, sb, cb;
-                    up2(X, xa, xb);
-                    __sincosf(xa, &sa, &ca);
-                    __sincosf(xb, &sb, &cb);
-                    s = pk2(sa, sb);
-                    c = pk2(ca, cb);
-                }
-                RE[i] = fma2(bc2(Gwr), c, fma2(bc2(Gwi), s, RE[i]));
-                IM[i] = fma2(bc2(Gwr), s, fma2(bc2(-Gwi), c, IM[i]));
-                continue;
-            }
+            const f32x2 X = fma2(U[i], pxx, fma2(V[i], pxy, fma2(W[i], pxz, GAINS ? bc2(ngam) : X0[i])));
             if (i < NPOLY) {
                 f32x2 s, c;
                 uint32_t ka, kb;
                 sincos_poly2(X, s, c, ka, kb);
-                const f32x2 wt = pk2(flip_if_odd(px.w, ka), flip_if_odd(px.w, kb));
+                const f32x2 wt = pk2(flip_if_odd(wgt, ka), flip_if_odd(wgt, kb));
                 RE[i] = fma2(wt, c, RE[i]);
                 IM[i] = fma2(wt, s, IM[i]);
             } else {
@@ -602,7 +611,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
                 up2(X, xa, xb);
                 __sincosf(xa, &sa, &ca);
                 __sincosf(xb, &sb, &cb);
-                const f32x2 wt = bc2(px.w);
+                const f32x2 wt = bc2(wgt);
                 RE[i] = fma2(wt, pk2(ca, cb), RE[i]);
                 IM[i] = fma2(wt, pk2(sa, sb), IM[i]);
             }
@@ -614,7 +623,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         const uint32_t parity = ((t - t0) >> 1) & 1;
         const int npx = tile_pixels<BATCH>(P, t);   // zero-skipping: pixels with a*x != 0 (all TP when dense)
         f32x2 X0[NPAIR];
-        if (npx > 0) {
+        if (!GAINS && npx > 0) {
             const double4 c = P.cen[t];
 #pragma unroll
             for (int i = 0; i < NPAIR; ++i) {
@@ -626,37 +635,59 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         mbar_wait(&s_bar[st], parity);
         if (GAINS) {
             // gain rows of the tile, gF[k][a]: register prefetch 4 pixels ahead (cold in L1 on first touch)
+            // 32-bit element offsets from the tile's first row (one IMAD.WIDE per load instead of 64-bit index
+            // arithmetic); the tables carry 4 rows of padding, so the prefetch of the group after the last needs no clamp
             const float2 *gbase = tile_gain_rows<BATCH>(P, t, npx);
+            const unsigned na = (unsigned)P.n_ant;
+            unsigned op = (unsigned)ap, oq = (unsigned)aq;
             float2 gp[4], gq[4];
 #pragma unroll
             for (int d = 0; d < 4; ++d) {
-                gp[d] = __ldg(gbase + (size_t)d * P.n_ant + ap);
-                gq[d] = __ldg(gbase + (size_t)d * P.n_ant + aq);
+                gp[d] = __ldg(gbase + (op + d * na));
+                gq[d] = __ldg(gbase + (oq + d * na));
             }
 #pragma unroll 1
             for (int p = 0; p < npx; p += 4) {
-                float Gwr[4], Gwi[4];
+                float Gw[4], Ng[4];
 #pragma unroll
                 for (int d = 0; d < 4; ++d) {
-                    const float w = s_pix[st][p + d].w;
-                    Gwr[d] = w * fmaf(gp[d].y, gq[d].y, gp[d].x * gq[d].x);    // a x Re(g_p conj g_q)
-                    Gwi[d] = w * fmaf(gp[d].y, gq[d].x, -gp[d].x * gq[d].y);
-                    const int pn = min(p + 4 + d, TP - 1);   // rows past npx exist (stale or zero): harmless prefetch
-                    gp[d] = __ldg(gbase + (size_t)pn * P.n_ant + ap);
-                    gq[d] = __ldg(gbase + (size_t)pn * P.n_ant + aq);
+                    Gw[d] = s_pix[st][p + d].w * (gp[d].x * gq[d].x);          // a x |g_p||g_q|
+                    Ng[d] = gq[d].y - gp[d].y;                                 // -gamma
                 }
-                pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, Gwr[0], Gwi[0]);
-                pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, Gwr[1], Gwi[1]);
-                pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, Gwr[2], Gwi[2]);
-                pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{}, Gwr[3], Gwi[3]);
+                op += 4 * na;
+                oq += 4 * na;
+#pragma unroll
+                for (int d = 0; d < 4; ++d) {                // rows past npx exist (stale, zero or padding): harmless prefetch
+                    gp[d] = __ldg(gbase + (op + d * na));
+                    gq[d] = __ldg(gbase + (oq + d * na));
+                }
+                pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, Gw[0], Ng[0]);
+                pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, Gw[1], Ng[1]);
+                pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, Gw[2], Ng[2]);
+                pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{}, Gw[3], Ng[3]);
+            }
+            if (npx > 0) {   // totals += e^{-i x0} (RE - i IM):  re += RE c0 - IM s0,  -im += RE s0 + IM c0
+                const double4 c = P.cen[t];
+#pragma unroll
+                for (int i = 0; i < NPAIR; ++i) {
+                    const int ja = min(jbase + (2 * i) * NT + tid, jlast), jb = min(jbase + (2 * i + 1) * NT + tid, jlast);
+                    float sa, ca, sb, cb;
+                    sincos_fma(centre_phase(sc * __ldg(P.u64 + ja), sc * __ldg(P.v64 + ja), sc * __ldg(P.w64 + ja), c), sa, ca);
+                    sincos_fma(centre_phase(sc * __ldg(P.u64 + jb), sc * __ldg(P.v64 + jb), sc * __ldg(P.w64 + jb), c), sb, cb);
+                    const f32x2 C0 = pk2(ca, cb), S0 = pk2(sa, sb);
+                    s_tot[i][tid] = add2(s_tot[i][tid], fma2(RE[i], C0, mul2(IM[i], pk2(-sa, -sb))));
+                    s_tot[NPAIR + i][tid] = add2(s_tot[NPAIR + i][tid], fma2(RE[i], S0, mul2(IM[i], C0)));
+                    RE[i] = pk2(0.f, 0.f);
+                    IM[i] = pk2(0.f, 0.f);
+                }
             }
         } else {
 #pragma unroll 1
             for (int p = 0; p < npx; p += 4) {
-                pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, 0.f, 0.f);
-                pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, 0.f, 0.f);
-                pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, 0.f, 0.f);
-                pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{}, 0.f, 0.f);
+                pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, s_pix[st][p].w, 0.f);
+                pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, s_pix[st][p + 1].w, 0.f);
+                pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, s_pix[st][p + 2].w, 0.f);
+                pixel(s_pix[st][p + 3], X0, std::integral_constant<int, NPQ / 4>{}, s_pix[st][p + 3].w, 0.f);
             }
         }
         __syncthreads();  // every thread is done with stage st
@@ -667,8 +698,8 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
         float ra, rb, ia, ib;
-        up2(RE[i], ra, rb);
-        up2(IM[i], ia, ib);
+        up2(GAINS ? s_tot[i][tid] : RE[i], ra, rb);
+        up2(GAINS ? s_tot[NPAIR + i][tid] : IM[i], ia, ib);
         const int ja = jbase + (2 * i) * NT + tid, jb = jbase + (2 * i + 1) * NT + tid;
         if (ja < P.n_vis) out[ja] = make_float2(ra, -ia);
         if (jb < P.n_vis) out[jb] = make_float2(rb, -ib);
@@ -692,7 +723,9 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     __shared__ __align__(8) int2 s_ant[GK ? 2 : 1][GK ? VC : 1];   // GK == 2 uses the first VC/8 only
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int base = blockIdx.x * (NT * RP);
+    int cta_group, cta_split;
+    adj_cta<(GK != 0)>(cta_group, cta_split);
+    const int base = cta_group * (NT * RP);
     const int kfirst = base + warp * (32 * RP);
     const int tile0 = base / TP;
     const int mycen = (kfirst / TP) - tile0;
@@ -715,7 +748,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
 
     const int n_chunks = (P.n_vis + VC - 1) / VC;
     const double sc = chan_scale_of<BATCH>(P);
-    const int c0 = blockIdx.y * P.per_split;
+    const int c0 = cta_split * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
 
     // GK == 2: a chunk is 16 baseline groups x 8 samples.  The plan stores sample r of group g at
@@ -765,9 +798,10 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     for (int ch = c0; ch < c1; ++ch) {
         const int buf = (ch - c0) & 1;
         if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
-        // grouped gains: G_i = gp_i conj(gq_i) per pixel is loaded once per group of 8 samples; the
-        // 8 samples accumulate Z_i = sum conj(e) r first, then acc_i += Re(conj(G_i) Z_i).
-        float Gr[GK == 2 ? RP : 1], Gi[GK == 2 ? RP : 1], Zr[GK == 2 ? RP : 1], Zi[GK == 2 ? RP : 1];
+        // Gains are stored in polar form (|g|, arg g): M = a |G| e(X - gamma), |G| = |g_p||g_q|, gamma = arg_p - arg_q.
+        // Grouped gains: (|G_i|, gamma_i) per pixel is formed once per group of 8 samples; the 8 samples
+        // accumulate Z_i = sum Re(conj(e(X - gamma_i)) r) first, then acc_i += |G_i| Z_i.
+        float Ga[GK == 2 ? RP : 1], Ng[GK == 2 ? RP : 1], Zr[GK == 2 ? RP : 1];
         float2 gpn[GK == 2 ? RP : 1], gqn[GK == 2 ? RP : 1];
         if (GK == 2) {
             const int2 a = s_ant[buf][0];
@@ -783,10 +817,9 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 const int2 a = s_ant[buf][min((tb >> 3) + 1, VC / 8 - 1)];
 #pragma unroll
                 for (int i = 0; i < RP; ++i) {
-                    Gr[i] = fmaf(gpn[i].y, gqn[i].y, gpn[i].x * gqn[i].x);
-                    Gi[i] = fmaf(gpn[i].y, gqn[i].x, -gpn[i].x * gqn[i].y);
+                    Ga[i] = gpn[i].x * gqn[i].x;
+                    Ng[i] = gqn[i].y - gpn[i].y;      // -gamma
                     Zr[i] = 0.f;
-                    Zi[i] = 0.f;
                     gpn[i] = __ldg(P.gA + (size_t)a.x * P.n_pix_pad + kfirst + lane + i * 32);
                     gqn[i] = __ldg(P.gA + (size_t)a.y * P.n_pix_pad + kfirst + lane + i * 32);
                 }
@@ -812,7 +845,15 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
             }
 #pragma unroll
             for (int i = 0; i < RP; ++i) {
-                const float X = fmaf(vv.x, dl[i], fmaf(vv.y, dm[i], fmaf(vv.z, dn[i], x0)));
+                float X = fmaf(vv.x, dl[i], fmaf(vv.y, dm[i], fmaf(vv.z, dn[i], x0)));
+                float g1 = 1.f;
+                if (GK == 2) X += Ng[i];
+                if (GK == 1) {
+                    const float2 gp = __ldg(gpr + i * 32);
+                    const float2 gq = __ldg(gqr + i * 32);
+                    g1 = gp.x * gq.x;
+                    X -= gp.y - gq.y;
+                }
                 float du = 0.f, dv = 0.f;
                 if (PK) {
                     du = fmaf(-vv.w, dl[i], ucx);
@@ -833,18 +874,11 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 } else {
                     gen_entry<PK, false>(X, du, dv, vv.w, PK ? sig2[i] : 0.f, PK ? nsp[i] : 0.f, ere, eim, sgn);
                 }
-                // z = conj(e) r = (ere - i eim)(r_re + i r_im)
+                // Re(conj(e) r) = ere r_re + eim r_im, e evaluated at the gain-shifted phase
                 if (GK == 2) {
                     Zr[i] = fmaf(ere, rr.x, fmaf(eim, rr.y, Zr[i]));
-                    Zi[i] = fmaf(ere, rr.y, fmaf(-eim, rr.x, Zi[i]));
                 } else if (GK == 1) {
-                    const float zre = fmaf(eim, rr.y, ere * rr.x);
-                    const float zim = fmaf(-eim, rr.x, ere * rr.y);
-                    const float2 gp = __ldg(gpr + i * 32);
-                    const float2 gq = __ldg(gqr + i * 32);
-                    const float Gr = fmaf(gp.y, gq.y, gp.x * gq.x);
-                    const float Gi = fmaf(gp.y, gq.x, -gp.x * gq.y);
-                    acc[i] += fmaf(Gi, zim, Gr * zre);      // Re(conj(G) z)
+                    acc[i] = fmaf(g1, fmaf(eim, rr.y, ere * rr.x), acc[i]);
                 } else {
                     acc[i] = fmaf(ere, rr.x, fmaf(eim, rr.y, acc[i]));
                 }
@@ -852,13 +886,13 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
           }
             if (GK == 2) {
 #pragma unroll
-                for (int i = 0; i < RP; ++i) acc[i] = fmaf(Gr[i], Zr[i], fmaf(Gi[i], Zi[i], acc[i]));
+                for (int i = 0; i < RP; ++i) acc[i] = fmaf(Ga[i], Zr[i], acc[i]);
             }
         }
         __syncthreads();
     }
 
-    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
+    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)cta_split * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
 }
@@ -971,17 +1005,23 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
 // Z_i = sum_samples conj(e) r over the 8 samples, then acc_i += Re(conj(G_i) Z_i).
 // ------------------------------------------------------------------------------------------
 #ifndef SL1M_ADJ_G2X2_MIN_CTAS
-#define SL1M_ADJ_G2X2_MIN_CTAS 4
+#define SL1M_ADJ_G2X2_MIN_CTAS 5
 #endif
 template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(const ApplyParams P) {
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP, NG = VC / 8;
-    __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre), slot = group * 8 + sample
-    __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, r_im)
+    // Gains are stored in polar form (|g|, arg g).  With G = |G| e^{i gamma} (|G| = |g_p||g_q|, gamma = arg_p - arg_q):
+    //     Re conj(M_jk) r_j = a |G| Re( e^{i (X_rel - gamma)} (r_j e^{i x0(j, centre)}) )
+    // The residual is rotated by the centre phase ONCE per (visibility, centre) while it is staged, -gamma is the
+    // innermost addend of the phase FMA chain and the accumulation is real: a term costs what a unit-gain term costs.
+    __shared__ __align__(16) float4 s_vc[2][VC];          // (u', v', w', -), slot = group * 8 + sample
+    __shared__ __align__(8) float2 s_r[2][NCEN][VC];      // (re, -im) of r e^{i x0} for that centre
     __shared__ __align__(8) int2 s_ant[2][NG];           // the group's (p, q)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int base = blockIdx.x * (NT * RP);
+    int cta_group, cta_split;
+    adj_cta<true>(cta_group, cta_split);
+    const int base = cta_group * (NT * RP);
     const int kfirst = base + warp * (32 * RP);
     const int tile0 = base / TP;
     const int mycen = (kfirst / TP) - tile0;
@@ -998,7 +1038,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
 
     const int n_chunks = (P.n_vis + VC - 1) / VC;
     const double sc = chan_scale_of<BATCH>(P);
-    const int c0 = blockIdx.y * P.per_split;
+    const int c0 = cta_split * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
 
     // the plan stores sample r of group g at (g / 128) * 1024 + r * 128 + g % 128 (the forward's thread layout)
@@ -1018,11 +1058,14 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
         }
         const float uf = static_cast<float>(TWO_PI * u), vf = static_cast<float>(TWO_PI * v),
                     wf = static_cast<float>(TWO_PI * w);
-        s_r[buf][slot] = rr;
+        s_vc[buf][slot] = make_float4(uf, vf, wf, 0.f);
         if (tid < NG) s_ant[buf][tid] = a;   // sample 0 carries the group's (p, q)
 #pragma unroll
-        for (int c = 0; c < NCEN; ++c)
-            s_vc[buf][c][slot] = make_float4(uf, vf, wf, centre_phase(u, v, w, P.cen[tile0 + c]));
+        for (int c = 0; c < NCEN; ++c) {
+            float s0, c0;
+            sincos_fma(centre_phase(u, v, w, P.cen[tile0 + c]), s0, c0);
+            s_r[buf][c][slot] = make_float2(rr.x * c0 - rr.y * s0, -(rr.x * s0 + rr.y * c0));
+        }
     };
 
     auto load_gains = [&](int2 a, float2 (&gp)[RP], float2 (&gq)[RP]) {
@@ -1033,34 +1076,28 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
         }
     };
 
-    f32x2 ZR[NPAIR], ZI[NPAIR];
+    f32x2 Z[NPAIR], NGM[NPAIR];
+    // rr = (re, -im) of the rotated residual:  Re(e^{iX} r) = c r_re - s r_im
     auto visibility = [&](const float4 vv, const float2 rr, auto npoly_tag) {
         constexpr int NPOLY = decltype(npoly_tag)::value;
-        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z), x0 = bc2(vv.w);
-        const f32x2 rre = bc2(rr.x), rim = bc2(rr.y), nrim = bc2(-rr.y);
+        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z);
 #pragma unroll
         for (int i = 0; i < NPAIR; ++i) {
-            const f32x2 X = fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, x0)));
-            f32x2 s, c;
+            const f32x2 X = fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, NGM[i])));
             if (i < NPOLY) {
+                f32x2 s, c;
                 uint32_t ka, kb;
                 sincos_poly2(X, s, c, ka, kb);
-                float sa, sb, ca, cb;
-                up2(s, sa, sb);
-                up2(c, ca, cb);
-                s = pk2(flip_if_odd(sa, ka), flip_if_odd(sb, kb));
-                c = pk2(flip_if_odd(ca, ka), flip_if_odd(cb, kb));
+                const f32x2 fre = pk2(flip_if_odd(rr.x, ka), flip_if_odd(rr.x, kb));
+                const f32x2 fim = pk2(flip_if_odd(rr.y, ka), flip_if_odd(rr.y, kb));
+                Z[i] = fma2(c, fre, fma2(s, fim, Z[i]));
             } else {
                 float xa, xb, sa, ca, sb, cb;
                 up2(X, xa, xb);
                 __sincosf(xa, &sa, &ca);
                 __sincosf(xb, &sb, &cb);
-                s = pk2(sa, sb);
-                c = pk2(ca, cb);
+                Z[i] = fma2(pk2(ca, cb), bc2(rr.x), fma2(pk2(sa, sb), bc2(rr.y), Z[i]));
             }
-            // z = conj(e) r = (c + i s)(r_re + i r_im)
-            ZR[i] = fma2(c, rre, fma2(s, nrim, ZR[i]));
-            ZI[i] = fma2(c, rim, fma2(s, rre, ZI[i]));
         }
     };
 
@@ -1073,32 +1110,31 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
         load_gains(s_ant[buf][0], gp, gq);
 #pragma unroll 1
         for (int g = 0; g < NG; ++g) {
-            f32x2 GR[NPAIR], GI[NPAIR];
+            f32x2 GA[NPAIR];
 #pragma unroll
             for (int i = 0; i < NPAIR; ++i) {
                 const float2 pa = gp[2 * i], qa = gq[2 * i], pb = gp[2 * i + 1], qb = gq[2 * i + 1];
-                GR[i] = pk2(fmaf(pa.y, qa.y, pa.x * qa.x), fmaf(pb.y, qb.y, pb.x * qb.x));      // Re g_p conj g_q
-                GI[i] = pk2(fmaf(pa.y, qa.x, -pa.x * qa.y), fmaf(pb.y, qb.x, -pb.x * qb.y));    // Im
-                ZR[i] = pk2(0.f, 0.f);
-                ZI[i] = pk2(0.f, 0.f);
+                GA[i] = pk2(pa.x * qa.x, pb.x * qb.x);        // |g_p||g_q|
+                NGM[i] = pk2(qa.y - pa.y, qb.y - pb.y);       // -gamma
+                Z[i] = pk2(0.f, 0.f);
             }
             load_gains(s_ant[buf][min(g + 1, NG - 1)], gp, gq);   // next group's rows
             const int t = g * 8;
-            visibility(s_vc[buf][mycen][t], s_r[buf][t], std::integral_constant<int, (NPQ + 3) / 4>{});
-            visibility(s_vc[buf][mycen][t + 1], s_r[buf][t + 1], std::integral_constant<int, (NPQ + 2) / 4>{});
-            visibility(s_vc[buf][mycen][t + 2], s_r[buf][t + 2], std::integral_constant<int, (NPQ + 1) / 4>{});
-            visibility(s_vc[buf][mycen][t + 3], s_r[buf][t + 3], std::integral_constant<int, NPQ / 4>{});
-            visibility(s_vc[buf][mycen][t + 4], s_r[buf][t + 4], std::integral_constant<int, (NPQ + 3) / 4>{});
-            visibility(s_vc[buf][mycen][t + 5], s_r[buf][t + 5], std::integral_constant<int, (NPQ + 2) / 4>{});
-            visibility(s_vc[buf][mycen][t + 6], s_r[buf][t + 6], std::integral_constant<int, (NPQ + 1) / 4>{});
-            visibility(s_vc[buf][mycen][t + 7], s_r[buf][t + 7], std::integral_constant<int, NPQ / 4>{});
+            visibility(s_vc[buf][t], s_r[buf][mycen][t], std::integral_constant<int, (NPQ + 3) / 4>{});
+            visibility(s_vc[buf][t + 1], s_r[buf][mycen][t + 1], std::integral_constant<int, (NPQ + 2) / 4>{});
+            visibility(s_vc[buf][t + 2], s_r[buf][mycen][t + 2], std::integral_constant<int, (NPQ + 1) / 4>{});
+            visibility(s_vc[buf][t + 3], s_r[buf][mycen][t + 3], std::integral_constant<int, NPQ / 4>{});
+            visibility(s_vc[buf][t + 4], s_r[buf][mycen][t + 4], std::integral_constant<int, (NPQ + 3) / 4>{});
+            visibility(s_vc[buf][t + 5], s_r[buf][mycen][t + 5], std::integral_constant<int, (NPQ + 2) / 4>{});
+            visibility(s_vc[buf][t + 6], s_r[buf][mycen][t + 6], std::integral_constant<int, (NPQ + 1) / 4>{});
+            visibility(s_vc[buf][t + 7], s_r[buf][mycen][t + 7], std::integral_constant<int, NPQ / 4>{});
 #pragma unroll
-            for (int i = 0; i < NPAIR; ++i) ACC[i] = fma2(GR[i], ZR[i], fma2(GI[i], ZI[i], ACC[i]));   // Re(conj(G) Z)
+            for (int i = 0; i < NPAIR; ++i) ACC[i] = fma2(GA[i], Z[i], ACC[i]);
         }
         __syncthreads();
     }
 
-    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
+    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)cta_split * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < NPAIR; ++i) {
         float a, b;
