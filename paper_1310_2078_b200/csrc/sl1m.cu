@@ -67,6 +67,7 @@ struct sl1m_plan {
     float2 *ws_v = nullptr;      // [fwd_split][n_vis]
     float *ws_p = nullptr;       // [adj_split][n_pix_pad]
     float2 *resid = nullptr;     // [n_vis]   residual / forward result
+    float2 *rpol = nullptr;      // [n_vis]   residual in polar form (|r|, arg r) for the one-cosine adjoint kernels
     float *I_sorted = nullptr, *y_sorted = nullptr, *g_sorted = nullptr;   // [n_pix_pad]
     double *part_a = nullptr, *part_b = nullptr, *part_c = nullptr;        // block partials
     int n_part = 0;
@@ -98,7 +99,7 @@ void free_plan(sl1m_plan *p) {
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
-                    p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc};
+                    p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc, p->rpol};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -189,13 +190,14 @@ int configure_and_allocate(sl1m_plan *p) {
     const size_t npad = (size_t)p->n_pix_pad, C = (size_t)p->n_chan;
     for (void **q : {(void **)&p->ws_v, (void **)&p->ws_p, (void **)&p->resid, (void **)&p->I_sorted, (void **)&p->y_sorted,
                      (void **)&p->g_sorted, (void **)&p->part_a, (void **)&p->part_b, (void **)&p->part_c, (void **)&p->scalars,
-                     (void **)&p->pixc, (void **)&p->tile_cnt, (void **)&p->gFc}) {
+                     (void **)&p->pixc, (void **)&p->tile_cnt, (void **)&p->gFc, (void **)&p->rpol}) {
         if (*q) cudaFree(*q);
         *q = nullptr;
     }
     CUDA_TRY(cudaMalloc((void **)&p->ws_v, C * (size_t)p->fwd_split * (size_t)p->n_vis_int * sizeof(float2)));
     CUDA_TRY(cudaMalloc((void **)&p->ws_p, C * (size_t)p->adj_split * npad * sizeof(float)));
     CUDA_TRY(cudaMalloc((void **)&p->resid, C * (size_t)p->n_vis_int * sizeof(float2)));
+    CUDA_TRY(cudaMalloc((void **)&p->rpol, C * (size_t)p->n_vis_int * sizeof(float2)));
     CUDA_TRY(cudaMalloc((void **)&p->I_sorted, C * npad * sizeof(float)));
     CUDA_TRY(cudaMalloc((void **)&p->y_sorted, C * npad * sizeof(float)));
     CUDA_TRY(cudaMalloc((void **)&p->g_sorted, C * npad * sizeof(float)));
@@ -525,7 +527,16 @@ template <int PK, int GK, bool B>
 void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
     switch (p->adj_rp) {
         case 8:
-            if constexpr (PK == 0 && GK == 0) adj_kernel_x2<SL1M_ADJ_NPQ, B><<<grid, NT, 0, s>>>(P);
+            if constexpr (PK == 0 && GK == 0) {
+#ifdef SL1M_ADJ_TWO_MUFU
+                adj_kernel_x2<SL1M_ADJ_NPQ, B><<<grid, NT, 0, s>>>(P);
+#else
+                ApplyParams Q = P;      // one cosine per term: the kernel reads the residual in polar form
+                vis_polar_kernel<<<dim3((unsigned)egrid((size_t)p->n_vis_int), (unsigned)p->n_chan), ET, 0, s>>>(P.r, p->rpol, p->n_vis_int);
+                Q.r = p->rpol;
+                adj_kernel_c1<SL1M_ADJ_C1_NPQ, B><<<grid, NT, 0, s>>>(Q);
+#endif
+            }
             else if constexpr (PK == 0 && GK == 2) adj_kernel_g2x2<SL1M_ADJ_G2_NPQ, B><<<grid, NT, 0, s>>>(P);
             else if constexpr (PK == 2 && GK == 0) adj_kernel_gtx2<B><<<grid, NT, 0, s>>>(P);
             else adj_kernel<8, PK, GK, B><<<grid, NT, 0, s>>>(P);
@@ -606,6 +617,9 @@ void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
         default: launch_adj_rp<1, 2>(p, P, grid, s); break;
     }
     p->launches++;
+#ifndef SL1M_ADJ_TWO_MUFU
+    if (key == 0 && p->adj_rp == 8) p->launches++;   // vis_polar_kernel in front of the one-cosine kernel
+#endif
 }
 
 int check_launch(const char *what) {

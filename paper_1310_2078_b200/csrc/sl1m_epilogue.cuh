@@ -181,6 +181,18 @@ __global__ void __launch_bounds__(ET) vis_gather_kernel(const float2 *caller, co
     internal[js] = (jc >= 0) ? caller[jc] : make_float2(0.f, 0.f);
 }
 
+// Residual in polar form for the one-cosine adjoint kernels: rp[j] = (|r_j|, arg r_j), evaluated in fp64.
+// Re(e^{iX} r) = |r| cos(X + arg r) (the image is real, reading C3).
+__global__ void __launch_bounds__(ET) vis_polar_kernel(const float2 *r, float2 *rp, int n_int) {
+    const int js = blockIdx.x * ET + threadIdx.x;
+    if (js >= n_int) return;
+    r += (size_t)blockIdx.y * n_int;                     // blockIdx.y = channel
+    rp += (size_t)blockIdx.y * n_int;
+    const float2 v = r[js];
+    const double re = (double)v.x, im = (double)v.y;
+    rp[js] = make_float2((float)sqrt(re * re + im * im), (float)atan2(im, re));
+}
+
 // Adjoint epilogue: g_k = a_k sum_s ws[s][k]; scattered to the caller's order and/or kept sorted.
 __global__ void __launch_bounds__(ET) adj_reduce_kernel(const float *ws, int n_split, int n_pix_pad,
                                                         const float *amp, const int *perm, float *img_caller,

@@ -999,6 +999,124 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
 }
 
 // ------------------------------------------------------------------------------------------
+// adjoint, delta pixels / unit gains, ONE COSINE per term (RP = 8, packed pairs).
+// The image is real (reading C3), so the adjoint only needs
+//     Re( conj(M_jk) r_j ) / a_k = Re( e^{+i X_jk} r_j ) = |r_j| cos(X_jk + arg r_j):
+// with the residual in polar form (P.r = (|r|, arg r), written by vis_polar_kernel) arg r_j joins the
+// per-(visibility, centre) phase x0 as the innermost addend of the phase chain, and a term is 3 FFMA
+// (phase) + FMUL.RZ + ONE MUFU.COS + 1 FFMA (accumulate) instead of 2 MUFU + 2 FFMA.  NPQ of every 16
+// pairs take an FMA-pipe cosine polynomial instead (same reduction and coefficients as sincos_poly2).
+// ------------------------------------------------------------------------------------------
+#ifndef SL1M_ADJ_C1_NPQ
+#define SL1M_ADJ_C1_NPQ 1
+#endif
+#ifndef SL1M_ADJ_C1_MIN_CTAS
+#define SL1M_ADJ_C1_MIN_CTAS 5
+#endif
+__device__ __forceinline__ void cos_poly2(f32x2 X, f32x2 &c, uint32_t &k_lo, uint32_t &k_hi) {
+    const f32x2 kf = fma2(X, bc2(0.318309886183790672f), bc2(12582912.0f));
+    const f32x2 kr = add2(kf, bc2(-12582912.0f));
+    const f32x2 r = fma2(kr, bc2(-3.14159265358979324f), X);
+    const f32x2 z = mul2(r, r);
+    f32x2 pc = fma2(z, bc2(2.3423957827617414e-05f), bc2(-0.0013866969384253025f));
+    pc = fma2(z, pc, bc2(0.04166554659605026f));
+    pc = fma2(z, pc, bc2(-0.49999991059303284f));
+    c = fma2(z, pc, bc2(1.0f));
+    float a, b;
+    up2(kf, a, b);
+    k_lo = __float_as_uint(a);
+    k_hi = __float_as_uint(b);
+}
+template <int NPQ, bool BATCH = false>
+__global__ void __launch_bounds__(NT, SL1M_ADJ_C1_MIN_CTAS) adj_kernel_c1(const ApplyParams P) {
+    constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
+    __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre + arg r)
+    __shared__ float s_R[2][VC];                          // |r|
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int base = blockIdx.x * (NT * RP);
+    const int kfirst = base + warp * (32 * RP);
+    const int tile0 = base / TP;
+    const int mycen = (kfirst / TP) - tile0;
+
+    f32x2 DL[NPAIR], DM[NPAIR], DN[NPAIR], ACC[NPAIR];
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        const float4 pa = P.pix4[kfirst + (2 * i) * 32 + lane], pb = P.pix4[kfirst + (2 * i + 1) * 32 + lane];
+        DL[i] = pk2(pa.x, pb.x);
+        DM[i] = pk2(pa.y, pb.y);
+        DN[i] = pk2(pa.z, pb.z);
+        ACC[i] = pk2(0.f, 0.f);
+    }
+
+    const int n_chunks = (P.n_vis + VC - 1) / VC;
+    const double sc = chan_scale_of<BATCH>(P);
+    const int c0 = blockIdx.y * P.per_split;
+    const int c1 = min(c0 + P.per_split, n_chunks);
+
+    auto stage = [&](int chunk, int buf) {
+        const int j = chunk * VC + tid;   // NT == VC
+        double u = 0.0, v = 0.0, w = 0.0;
+        float2 rp = make_float2(0.f, 0.f);   // (|r|, arg r)
+        if (j < P.n_vis) {
+            u = sc * P.u64[j];
+            v = sc * P.v64[j];
+            w = sc * P.w64[j];
+            rp = P.r[chan_index<BATCH>() * P.n_vis + j];
+        }
+        const float uf = static_cast<float>(TWO_PI * u), vf = static_cast<float>(TWO_PI * v),
+                    wf = static_cast<float>(TWO_PI * w);
+        s_R[buf][tid] = rp.x;
+#pragma unroll
+        for (int c = 0; c < NCEN; ++c)   // both addends lie in [-pi, pi]
+            s_vc[buf][c][tid] = make_float4(uf, vf, wf, centre_phase(u, v, w, P.cen[tile0 + c]) + rp.y);
+    };
+
+    auto visibility = [&](const float4 vv, const float R, auto npoly_tag) {
+        constexpr int NPOLY = decltype(npoly_tag)::value;
+        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z), x0 = bc2(vv.w);
+#pragma unroll
+        for (int i = 0; i < NPAIR; ++i) {
+            const f32x2 X = fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, x0)));
+            if (i < NPOLY) {
+                f32x2 c;
+                uint32_t ka, kb;
+                cos_poly2(X, c, ka, kb);
+                ACC[i] = fma2(c, pk2(flip_if_odd(R, ka), flip_if_odd(R, kb)), ACC[i]);
+            } else {
+                float xa, xb;
+                up2(X, xa, xb);
+                ACC[i] = fma2(pk2(__cosf(xa), __cosf(xb)), bc2(R), ACC[i]);
+            }
+        }
+    };
+
+    if (c0 < c1) stage(c0, 0);
+    __syncthreads();
+    for (int ch = c0; ch < c1; ++ch) {
+        const int buf = (ch - c0) & 1;
+        if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
+#pragma unroll 1
+        for (int t = 0; t < VC; t += 4) {
+            visibility(s_vc[buf][mycen][t], s_R[buf][t], std::integral_constant<int, (NPQ + 3) / 4>{});
+            visibility(s_vc[buf][mycen][t + 1], s_R[buf][t + 1], std::integral_constant<int, (NPQ + 2) / 4>{});
+            visibility(s_vc[buf][mycen][t + 2], s_R[buf][t + 2], std::integral_constant<int, (NPQ + 1) / 4>{});
+            visibility(s_vc[buf][mycen][t + 3], s_R[buf][t + 3], std::integral_constant<int, NPQ / 4>{});
+        }
+        __syncthreads();
+    }
+
+    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
+#pragma unroll
+    for (int i = 0; i < NPAIR; ++i) {
+        float a, b;
+        up2(ACC[i], a, b);
+        out[kfirst + (2 * i) * 32 + lane] = a;
+        out[kfirst + (2 * i + 1) * 32 + lane] = b;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // adjoint, delta pixels, baseline-grouped gains (gk == 2), packed-pair variant (RP = 8).
 // A chunk is 16 baseline groups x 8 samples, staged group-major.  Per group the thread forms
 // G_i = g_p(i) conj(g_q(i)) for its 8 pixels once (next group's gain rows prefetched), accumulates
