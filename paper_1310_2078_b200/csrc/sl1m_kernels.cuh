@@ -1011,7 +1011,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
 #define SL1M_ADJ_C1_NPQ 1
 #endif
 #ifndef SL1M_ADJ_C1_MIN_CTAS
-#define SL1M_ADJ_C1_MIN_CTAS 5
+#define SL1M_ADJ_C1_MIN_CTAS 6
 #endif
 __device__ __forceinline__ void cos_poly2(f32x2 X, f32x2 &c, uint32_t &k_lo, uint32_t &k_hi) {
     const f32x2 kf = fma2(X, bc2(0.318309886183790672f), bc2(12582912.0f));
@@ -1129,11 +1129,11 @@ template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(const ApplyParams P) {
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP, NG = VC / 8;
     // Gains are stored in polar form (|g|, arg g).  With G = |G| e^{i gamma} (|G| = |g_p||g_q|, gamma = arg_p - arg_q):
-    //     Re conj(M_jk) r_j = a |G| Re( e^{i (X_rel - gamma)} (r_j e^{i x0(j, centre)}) )
-    // The residual is rotated by the centre phase ONCE per (visibility, centre) while it is staged, -gamma is the
-    // innermost addend of the phase FMA chain and the accumulation is real: a term costs what a unit-gain term costs.
+    //     Re conj(M_jk) r_j = a |G| Re( e^{i (X_rel - gamma)} r_j e^{i x0(j, centre)} ) = a |G| |r_j| cos(X_rel - gamma + phi'),
+    // phi' = arg r_j + x0(j, centre), formed ONCE per (visibility, centre) while the chunk is staged.  -gamma is the
+    // innermost addend of the phase FMA chain, phi' one more add; ONE cosine per term, real accumulation.
     __shared__ __align__(16) float4 s_vc[2][VC];          // (u', v', w', -), slot = group * 8 + sample
-    __shared__ __align__(8) float2 s_r[2][NCEN][VC];      // (re, -im) of r e^{i x0} for that centre
+    __shared__ __align__(8) float2 s_r[2][NCEN][VC];      // (|r|, arg r + x0 of that centre)
     __shared__ __align__(8) int2 s_ant[2][NG];           // the group's (p, q)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -1178,12 +1178,10 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
                     wf = static_cast<float>(TWO_PI * w);
         s_vc[buf][slot] = make_float4(uf, vf, wf, 0.f);
         if (tid < NG) s_ant[buf][tid] = a;   // sample 0 carries the group's (p, q)
+        const float R = sqrtf(fmaf(rr.x, rr.x, rr.y * rr.y)), phi = atan2f(rr.y, rr.x);
 #pragma unroll
-        for (int c = 0; c < NCEN; ++c) {
-            float s0, c0;
-            sincos_fma(centre_phase(u, v, w, P.cen[tile0 + c]), s0, c0);
-            s_r[buf][c][slot] = make_float2(rr.x * c0 - rr.y * s0, -(rr.x * s0 + rr.y * c0));
-        }
+        for (int c = 0; c < NCEN; ++c)
+            s_r[buf][c][slot] = make_float2(R, phi + centre_phase(u, v, w, P.cen[tile0 + c]));   // both in [-pi, pi]
     };
 
     auto load_gains = [&](int2 a, float2 (&gp)[RP], float2 (&gq)[RP]) {
@@ -1195,26 +1193,22 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
     };
 
     f32x2 Z[NPAIR], NGM[NPAIR];
-    // rr = (re, -im) of the rotated residual:  Re(e^{iX} r) = c r_re - s r_im
+    // rr = (|r|, phi')
     auto visibility = [&](const float4 vv, const float2 rr, auto npoly_tag) {
         constexpr int NPOLY = decltype(npoly_tag)::value;
-        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z);
+        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z), ph = bc2(rr.y);
 #pragma unroll
         for (int i = 0; i < NPAIR; ++i) {
-            const f32x2 X = fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, NGM[i])));
+            const f32x2 X = add2(fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, NGM[i]))), ph);
             if (i < NPOLY) {
-                f32x2 s, c;
+                f32x2 c;
                 uint32_t ka, kb;
-                sincos_poly2(X, s, c, ka, kb);
-                const f32x2 fre = pk2(flip_if_odd(rr.x, ka), flip_if_odd(rr.x, kb));
-                const f32x2 fim = pk2(flip_if_odd(rr.y, ka), flip_if_odd(rr.y, kb));
-                Z[i] = fma2(c, fre, fma2(s, fim, Z[i]));
+                cos_poly2(X, c, ka, kb);
+                Z[i] = fma2(c, pk2(flip_if_odd(rr.x, ka), flip_if_odd(rr.x, kb)), Z[i]);
             } else {
-                float xa, xb, sa, ca, sb, cb;
+                float xa, xb;
                 up2(X, xa, xb);
-                __sincosf(xa, &sa, &ca);
-                __sincosf(xb, &sb, &cb);
-                Z[i] = fma2(pk2(ca, cb), bc2(rr.x), fma2(pk2(sa, sb), bc2(rr.y), Z[i]));
+                Z[i] = fma2(pk2(__cosf(xa), __cosf(xb)), bc2(rr.x), Z[i]);
             }
         }
     };
@@ -1414,7 +1408,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_GTX2_MIN_CTAS) adj_kernel_gtx2(co
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
     __shared__ __align__(16) float4 s_vis[2][VC];            // (u', v', w', -w)
     __shared__ __align__(16) float4 s_ca[2][NCEN][VC];       // per centre: (x0', uc, vc, cX = -ln2 q)
-    __shared__ __align__(16) float4 s_cb[2][NCEN][VC];       // per centre: (cE, lr, A = r_re + q r_im, B = q r_re - r_im)
+    __shared__ __align__(16) float4 s_cb[2][NCEN][VC];       // per centre: (cE, lr, R = |(A, B)|, -) with A = r_re + q r_im, B = q r_re - r_im
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int base = blockIdx.x * (NT * RP);
     const int kfirst = base + warp * (32 * RP);
@@ -1450,10 +1444,12 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_GTX2_MIN_CTAS) adj_kernel_gtx2(co
             const double4 cen = P.cen[tile0 + c];
             float x0 = centre_phase(u, v, w, cen), q, cE, lr;
             gauss_tile_constants(w, cen.w, q, cE, lr, x0);
-            s_ca[buf][c][tid] = make_float4(x0, static_cast<float>(u - w * cen.x), static_cast<float>(v - w * cen.y),
-                                            -0.69314718056f * q);
-            // Re conj(M/a) r = amp ((c + q s) r_re + (q c - s) r_im) = amp (c A + s B)
-            s_cb[buf][c][tid] = make_float4(cE, lr, fmaf(q, rr.y, rr.x), fmaf(q, rr.x, -rr.y));
+            // Re conj(M/a) r = amp ((c + q s) r_re + (q c - s) r_im) = amp (c A + s B) = amp R cos(X' - psi),
+            // (R, psi) the polar form of (A, B): ONE cosine per term, psi folded into the centre phase
+            const float A = fmaf(q, rr.y, rr.x), B = fmaf(q, rr.x, -rr.y);
+            s_ca[buf][c][tid] = make_float4(x0 - atan2f(B, A), static_cast<float>(u - w * cen.x),
+                                            static_cast<float>(v - w * cen.y), -0.69314718056f * q);
+            s_cb[buf][c][tid] = make_float4(cE, lr, sqrtf(fmaf(A, A, B * B)), 0.f);
         }
     };
     if (c0 < c1) stage(c0, 0);
@@ -1466,7 +1462,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_GTX2_MIN_CTAS) adj_kernel_gtx2(co
             const float4 vv = s_vis[buf][t], ca = s_ca[buf][mycen][t], cb = s_cb[buf][mycen][t];
             const f32x2 bu = bc2(vv.x), bv = bc2(vv.y), bw = bc2(vv.z), bnw = bc2(vv.w);
             const f32x2 bx0 = bc2(ca.x), buc = bc2(ca.y), bvc = bc2(ca.z), bcx = bc2(ca.w);
-            const f32x2 bce = bc2(cb.x), blr = bc2(cb.y), bA = bc2(cb.z), bB = bc2(cb.w);
+            const f32x2 bce = bc2(cb.x), blr = bc2(cb.y), bR = bc2(cb.z);
 #pragma unroll
             for (int i = 0; i < NPAIR; ++i) {
                 const f32x2 X = fma2(DL[i], bu, fma2(DM[i], bv, fma2(DN[i], bw, bx0)));
@@ -1474,9 +1470,9 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_GTX2_MIN_CTAS) adj_kernel_gtx2(co
                 const f32x2 s2 = fma2(dv, dv, mul2(du, du));
                 const f32x2 Ep = fma2(s2, bce, blr);
                 const f32x2 Xp = fma2(bcx, Ep, X);
-                f32x2 s, c;
-                sincos2(Xp, s, c);
-                ACC[i] = fma2(ex2_2(Ep), fma2(c, bA, mul2(s, bB)), ACC[i]);
+                float xa, xb;
+                up2(Xp, xa, xb);
+                ACC[i] = fma2(mul2(ex2_2(Ep), pk2(__cosf(xa), __cosf(xb))), bR, ACC[i]);
             }
         }
         __syncthreads();
