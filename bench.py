@@ -312,23 +312,35 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     fwd_ms, adj_ms = statistics.median(t_fwd), statistics.median(t_adj)
 
-    def bound(per16, packed, clock_hz):
-        """Issue-rate bound (terms/s) of one apply kernel for ITS OWN instruction mix (SASS-counted,
-        DESIGN.md section 6).  A fraction f = per16/16 of the terms takes the FMA-pipe polynomial
-        sincos (0 MUFU), the rest the MUFU path.  Three per-SM limits, each in terms/clk:
+    def bound(kind, per16, packed, clock_hz):
+        """Issue-rate bound (terms/s) of one apply kernel (`kind` = "fwd" or "adj") for ITS OWN instruction mix
+        (SASS-counted).  A fraction f = per16/16 of the terms takes an FMA-pipe polynomial
+        (0 MUFU), the rest the MUFU path.  Three per-SM limits, each in terms/clk:
           MUFU pipe   16 results/clk            / (mufu_per_term * (1 - f))
           FMA pipe    128 fp32 lanes/clk        / lane-ops per term (an FFMA2 is 2 lane-ops)
           issue       4 warp-instr = 128 thread-instr/clk / issue slots per term
-        peak = the smallest of the three."""
+        peak = the smallest of the three.  The adjoint of a REAL image needs one cosine per term,
+        Re(e^{iX} r) = |r| cos(X + arg r): 1 MUFU + 5 lane-ops (3 phase + FMUL.RZ + 1 accumulate)."""
         f = per16 / 16.0
         gauss, gains = int(desc["gaussian"]), bool(desc["gains"])   # gaussian: 0 delta, 1 per-pixel sigma, 2 per-tile sigma
-        mufu = desc["mufu_per_term_mufu_path"] * (1.0 - f)
-        lane_mufu_path = {0: 6.0, 1: 20.0, 2: 13.0 if packed else 16.0}[gauss]   # delta: 3 phase + FMUL.RZ + 2 accumulate
-        lane_poly_path = 18.0                        # 3 phase + 3 reduce + 1 + 5 sin + 4 cos + 2 accumulate
-        grouped = int(desc["gains"]) == 2            # one gain product per pixel per 8 samples: +2 lane-ops per term
-        lanes = lane_mufu_path * (1.0 - f) + lane_poly_path * f + (2.5 if grouped else (10.0 if gains else 0.0))
+        grouped = int(desc["gains"]) == 2            # one polar gain product per pixel per 8 samples
+        m_term = desc["adj_mufu_per_term"] if kind == "adj" else desc["mufu_per_term_mufu_path"]
+        one_cos = kind == "adj" and m_term == 1
+        mufu = m_term * (1.0 - f)
+        if one_cos:
+            lane_mufu_path, lane_poly_path = 5.0, 12.0          # poly: 3 phase + 3 reduce + 1 + 4 cos + 1 accumulate
+            extra = 1.5 if grouped else 0.0                      # + phase add per term, gain product per 8 terms
+        else:
+            lane_mufu_path = {0: 6.0, 1: 20.0, 2: (12.0 if kind == "adj" else 13.0) if packed else 16.0}[gauss]
+            lane_poly_path = 18.0                    # 3 phase + 3 reduce + 1 + 5 sin + 4 cos + 2 accumulate
+            extra = 0.5 if grouped else (10.0 if gains else 0.0)
+        lanes = lane_mufu_path * (1.0 - f) + lane_poly_path * f + extra
         if packed:   # FFMA2 halves the issue slots of everything but FMUL.RZ and MUFU
-            slots = (10.0 if gauss == 2 else 5.5) * (1.0 - f) + 11.0 * f + 0.25 + (1.5 if grouped else 0.0)
+            if one_cos:
+                slots = 4.0 * (1.0 - f) + 7.5 * f + 0.25 + (1.0 if grouped else 0.0)
+            else:
+                slots = ((7.5 if kind == "adj" else 10.0) if gauss == 2 else 5.5) * (1.0 - f) + 11.0 * f + 0.25 \
+                    + (2.2 if grouped else 0.0)      # gains: address arithmetic of 8 gain loads per 4 pixels
         else:
             slots = {0: 8.0, 1: 24.0, 2: 19.0}[gauss] * (1.0 - f) + 20.0 * f + 0.125 + (10.0 if gains else 0.0)
         b_mufu = SM_COUNT * MUFU_PER_SM_PER_CLK * clock_hz / mufu
@@ -336,17 +348,24 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         b_issue = SM_COUNT * 128.0 * clock_hz / slots
         return min(b_mufu, b_fma, b_issue), b_mufu, b_fma, b_issue
 
-    pk_f, pk_f_mufu, pk_f_fma, pk_f_issue = bound(desc["fwd_poly_per16"], desc["fwd_packed_pairs"], f_max)
-    pk_a, pk_a_mufu, pk_a_fma, pk_a_issue = bound(desc["adj_poly_per16"], desc["adj_packed_pairs"], f_max)
-    mufu_only = SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / desc["mufu_per_term_mufu_path"]
-    # best any MUFU/FMA split of this instruction set could do (delta pixels): 16(1-f) = 6(1-f) + 18 f
-    f_bal = 10.0 / 28.0
-    balanced = (SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / (2.0 * (1.0 - f_bal))
-                if not (desc["gaussian"] or desc["gains"]) else None)
+    pk_f, pk_f_mufu, pk_f_fma, pk_f_issue = bound("fwd", desc["fwd_poly_per16"], desc["fwd_packed_pairs"], f_max)
+    pk_a, pk_a_mufu, pk_a_fma, pk_a_issue = bound("adj", desc["adj_poly_per16"], desc["adj_packed_pairs"], f_max)
     ach_f, ach_a = n_terms / (fwd_ms * 1e-3), n_terms / (adj_ms * 1e-3)
-    dom_is_adj = adj_ms >= fwd_ms
+    # the dominant kernel of the TIMED STEP: the adjoint evaluates every term, the forward only the non-zero pixels
+    step_ms_mean = t_max / args.steps
+    dom_is_adj = adj_ms >= step_ms_mean - adj_ms
+    m_dom = desc["adj_mufu_per_term"] if dom_is_adj else desc["mufu_per_term_mufu_path"]
+    mufu_only = SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / m_dom      # every term on the MUFU path
+    # best any MUFU/FMA split of the dominant kernel's instruction set could do (delta pixels, unit gains):
+    # MUFU time = FMA time, m (1-f)/16 = (a (1-f) + b f)/128 with (m, a, b) = (2, 6, 18) forward, (1, 5, 12) adjoint
+    m_, a_, b_ = (1.0, 5.0, 12.0) if (dom_is_adj and m_dom == 1) else (2.0, 6.0, 18.0)
+    f_bal = (8.0 * m_ - a_) / (8.0 * m_ - a_ + b_)
+    balanced = (SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / (m_ * (1.0 - f_bal))
+                if not (desc["gaussian"] or desc["gains"]) else None)
     dom = "sl1m::adj_kernel" if dom_is_adj else "sl1m::fwd_kernel"
-    if (desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"]):
+    if dom_is_adj and desc["adj_packed_pairs"] and desc["adj_mufu_per_term"] == 1 and not desc["gains"]:
+        dom += "_c1"
+    elif (desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"]):
         dom += "_x2"
     achieved, peak = (ach_a, pk_a) if dom_is_adj else (ach_f, pk_f)
     traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "adj" if dom_is_adj else "fwd"))
@@ -356,9 +375,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "peak_basis": f"min(MUFU pipe, FMA pipe, issue slots) for the kernel's own SASS instruction mix at "
                       f"{f_max/1e6:.0f} MHz (sm_max_mhz, {peaks_src}): {SM_COUNT} SMs x {MUFU_PER_SM_PER_CLK} MUFU/clk, "
                       f"x 128 fp32 lanes/clk, x 128 thread-instr/clk; fwd {desc['fwd_poly_per16']}/16 and adj "
-                      f"{desc['adj_poly_per16']}/16 of the terms use FMA-pipe polynomial sincos",
+                      f"{desc['adj_poly_per16']}/16 of the terms use FMA-pipe polynomials; MUFU per MUFU-path term: fwd "
+                      f"{desc['mufu_per_term_mufu_path']}, adj {desc['adj_mufu_per_term']} (real image: one cosine per adjoint term)",
         "traffic_basis": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full "
-                         "(profiles/, same kernel and workload); algorithmic bytes at config 5: ~30 MB in per apply "
+                         "(profiles/, same kernel and workload; null = not captured); algorithmic bytes at config 5: ~30 MB in per apply "
                          "+ the split partials (24 x 3.25 MB forward, 10 x 4 MB adjoint, mostly L2-resident)",
         "mufu_only_bound_Tterm_per_s": mufu_only / 1e12,
         "frac_vs_mufu_only_bound": achieved / mufu_only,
@@ -373,7 +393,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                 "not an HBM-bound path: the matrix is generated, never read",
     }
     if clocks.get("sm_mhz"):
-        pk_c = bound(desc["adj_poly_per16"] if dom_is_adj else desc["fwd_poly_per16"],
+        pk_c = bound("adj" if dom_is_adj else "fwd", desc["adj_poly_per16"] if dom_is_adj else desc["fwd_poly_per16"],
                      desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"], clocks["sm_mhz"] * 1e6)[0]
         roof["frac_at_sampled_clock"] = achieved / pk_c
 

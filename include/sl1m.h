@@ -252,12 +252,15 @@ typedef struct {
     int32_t adj_rp;                      /* pixels per thread in the adjoint kernel                */
     int32_t adj_pixel_groups, adj_vis_splits, adj_chunks_per_split;
     int32_t adj_poly_per16;
-    int32_t mufu_per_term_mufu_path;     /* 2 (delta) or 4 (Gaussian)                              */
+    int32_t mufu_per_term_mufu_path;     /* forward: 2 (delta), 3 (Gaussian, one sigma per tile) or 4 (Gaussian) */
     int32_t fwd_packed_pairs;            /* 1 = the packed fp32x2 (FFMA2) forward kernel is in use  */
     int32_t adj_packed_pairs;
     int32_t phase_fp64;                  /* 1 = the fp64-phase kernels are in use                    */
     float phase_span_rad;                /* plan-time bound on the fp32 phase remainder in a tile    */
     int32_t zero_skip;                   /* 1 = the forward streams only pixels with x_k != 0       */
+    int32_t adj_mufu_per_term;           /* MUFU per MUFU-path term of the ADJOINT: 1 with the one-cosine kernels
+                                          * (Re(e^{iX} r) = |r| cos(X + arg r)), 2 with per-tile-sigma Gaussian
+                                          * pixels (ex2 + cos), else as the forward                  */
 } sl1m_plan_info;
 int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
 

@@ -31,7 +31,7 @@ class _PlanInfo(ctypes.Structure):
         "n_pix_padded", "n_tiles", "gaussian", "gains", "fwd_rv", "fwd_vis_tiles", "fwd_pixel_splits",
         "fwd_tiles_per_split", "fwd_poly_per16", "adj_rp", "adj_pixel_groups", "adj_vis_splits",
         "adj_chunks_per_split", "adj_poly_per16", "mufu_per_term_mufu_path", "fwd_packed_pairs",
-        "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("zero_skip", ctypes.c_int32)]
+        "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("zero_skip", ctypes.c_int32), ("adj_mufu_per_term", ctypes.c_int32)]
 
 
 class _QtLevel(ctypes.Structure):

@@ -980,13 +980,26 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     const bool grouped = !pk && p->gk == 2;        // delta pixels, baseline-grouped gains
     o->fwd_poly_per16 = plain ? (p->fwd_rv == 8 ? SL1M_FWD_NPQ : (p->fwd_rv == 4 ? (SL1M_FWD_NPOLY8 / 2) * 4 : 0))
                               : (grouped ? SL1M_FWD_G2_NPQ : 0);
-    o->adj_poly_per16 = plain ? (p->adj_rp == 8 ? SL1M_ADJ_NPQ : (p->adj_rp == 4 ? (SL1M_ADJ_NPOLY8 / 2) * 4 : 0))
+#ifdef SL1M_ADJ_TWO_MUFU
+    constexpr int adj_npq8 = SL1M_ADJ_NPQ;
+#else
+    constexpr int adj_npq8 = SL1M_ADJ_C1_NPQ;
+#endif
+    o->adj_poly_per16 = plain ? (p->adj_rp == 8 ? adj_npq8 : (p->adj_rp == 4 ? (SL1M_ADJ_NPOLY8 / 2) * 4 : 0))
                               : (grouped && p->adj_rp == 8 ? SL1M_ADJ_G2_NPQ : 0);
     o->mufu_per_term_mufu_path = p->pk == 2 ? 3 : (pk ? 4 : 2);
     o->gaussian = p->pk;
     o->phase_fp64 = p->phase64 && p->n_chan == 1;
     o->phase_span_rad = (float)p->phase_span;
     o->zero_skip = p->pixc != nullptr;
+    o->adj_mufu_per_term = o->mufu_per_term_mufu_path;
+    if (p->adj_rp == 8 && !(p->phase64 && p->n_chan == 1)) {
+#ifndef SL1M_ADJ_TWO_MUFU
+        if (p->pk == 0 && p->gk == 0) o->adj_mufu_per_term = 1;    // adj_kernel_c1
+#endif
+        if (p->pk == 0 && p->gk == 2) o->adj_mufu_per_term = 1;    // adj_kernel_g2x2
+        if (p->pk == 2 && p->gk == 0) o->adj_mufu_per_term = 2;    // adj_kernel_gtx2
+    }
     if (o->phase_fp64) o->fwd_poly_per16 = o->adj_poly_per16 = 0;
     const bool tile_gauss = p->pk == 2 && p->gk == 0;
     o->fwd_packed_pairs = ((plain || tile_gauss) && p->fwd_rv == 8) || grouped;
