@@ -349,7 +349,7 @@ __device__ __forceinline__ void gen_entry_tile(float X, float du, float dv, floa
 #define SL1M_FWD_G2_NPQ 3
 #endif
 #ifndef SL1M_ADJ_G2_NPQ
-#define SL1M_ADJ_G2_NPQ 4
+#define SL1M_ADJ_G2_NPQ 1
 #endif
 #ifndef SL1M_FWD_X2_MIN_CTAS
 #define SL1M_FWD_X2_MIN_CTAS 4
