@@ -37,7 +37,7 @@ MUFU_PER_SM_PER_CLK = 16      # 4 SFU lanes per SM sub-partition x 4 (measured 1
 SM_COUNT = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (config, kernel) -> bytes
-NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 58.47e6, (5, "adj"): 35.78e6, (4, "fwd"): 341.1e6, (4, "adj"): 315.7e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 58.53e6, (5, "adj"): 35.12e6, (4, "fwd"): 340.6e6, (4, "adj"): 318.1e6}
 
 
 def _peaks():
