@@ -332,3 +332,32 @@ def test_zero_skipping_forward(sl, kind):
     assert 0 < ia.nnz < n and abs(ia.nnz - ib.nnz) <= max(2, ib.nnz // 100)
     assert plan.forward_active_pixels() < plan.describe()["n_pix_padded"]   # the last forward really skipped
     plan.close(); dense.close()
+
+
+@pytest.mark.parametrize("n_steps", [8, 3])
+def test_polar_gain_corner_cases(sl, n_steps):
+    """The gain tables are kept in polar form (|g|, arg g).  Exact zeros, negative real and purely imaginary gains
+    (arg = pi, +-pi/2: gamma_p - gamma_q reaches +-2 pi), gains of very different magnitude, and a residual with exact
+    zeros (|r| = 0, arg r = 0 in the one-cosine adjoint); grouped (8 samples) and per-term (3 samples) kernels."""
+    import torch
+    wl = make_workload(4, n_side=64, n_ant=12, n_steps=n_steps, n_src=40)
+    rng = np.random.default_rng(23)
+    g = np.array(wl.gains, dtype=np.complex64, copy=True)
+    n_ant, n_pix = g.shape
+    g[0, ::7] = 0.0
+    g[1, :] = -np.abs(g[1, :])
+    g[2, :] = 1j * np.abs(g[2, :])
+    g[3, :] = -1j * np.abs(g[3, :])
+    g[4, :] *= 1e3
+    g[5, :] *= 1e-3
+    o = oracle.Oracle(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model)
+    plan = sl.Plan(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model)
+    assert plan.describe()["gains"] == (2 if n_steps == 8 else 1)
+    x = np.where(rng.uniform(size=n_pix) < 0.3, rng.uniform(0.1, 1, n_pix), 0).astype(np.float32)
+    r = (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis)).astype(np.complex64)
+    r[::5] = 0
+    r[1::5] = np.abs(r[1::5])              # arg r = 0
+    r[2::5] = -np.abs(r[2::5])             # arg r = pi
+    assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x)) <= 2e-4
+    assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r)) <= 2e-4
+    plan.close()

@@ -218,3 +218,53 @@ def test_gains_factorisation_cases():
     o2 = oracle.Oracle(uvw, l, m, ant_p=p, ant_q=q, gains=np.repeat(b[None, :], n_ant, 0).astype(np.complex64))
     want2 = unit.forward(b.astype(np.float64) ** 2 * x)
     assert np.max(np.abs(o2.forward(x) - want2)) < 1e-12
+
+
+def test_polar_identities_used_by_the_cuda_kernels():
+    """DESIGN.md section 6, pinned against the oracle's literal complex arithmetic (delta and Gaussian entries, both models):
+    (i)  polar gains: with G = g_p conj(g_q) = |G| e^{i gamma}, the entry with gains is |G| times the unit-gain entry
+         evaluated with its phase shifted by -gamma, i.e. M_gain = |G| e^{i gamma} M_unit (a real weight and a phase shift);
+    (ii) one-cosine adjoint: Re(conj(M) r) = |M| |r| cos(arg r - arg M); for a delta pixel arg M = gamma - X, so the term
+         is (|G|/n) |r| cos(X - gamma + arg r);
+    (iii) Gaussian: A cos X' + B sin X' = R cos(X' - psi) with A = r_re + q r_im, B = q r_re - r_im, (R, psi) = polar(A, B)."""
+    rng = np.random.default_rng(17)
+    n_ant, n_pix = 4, 6
+    p, q = np.triu_indices(n_ant, 1)
+    uvw = rng.uniform(-800, 800, size=(len(p), 3))
+    l = rng.uniform(-0.1, 0.1, n_pix)
+    m = rng.uniform(-0.1, 0.1, n_pix)
+    sig = np.where(rng.uniform(size=n_pix) < 0.5, 0.0, 10 ** rng.uniform(-4, -2, n_pix))
+    g = (rng.standard_normal((n_ant, n_pix)) + 1j * rng.standard_normal((n_ant, n_pix))).astype(np.complex64)
+    g[0, 0] = 0.0                       # a zero gain: amplitude 0, phase 0
+    g[1, 1] = -2.0                      # phase pi
+    g[2, 2] = 3.0j                      # phase pi/2
+    for model in (0, 1):
+        unit = oracle.Oracle(uvw, l, m, sigma=sig, gauss_model=model)
+        og = oracle.Oracle(uvw, l, m, sigma=sig, ant_p=p, ant_q=q, gains=g, gauss_model=model)
+        g64 = g.astype(np.complex128)
+        amp, ph = np.abs(g64), np.angle(g64)
+        for j in range(len(p)):
+            r = complex(rng.standard_normal(), rng.standard_normal())
+            for k in range(n_pix):
+                Mu, Mg = unit.entry(j, k), og.entry(j, k)
+                G_amp = amp[p[j], k] * amp[q[j], k]
+                gamma = ph[p[j], k] - ph[q[j], k]
+                assert abs(Mg - G_amp * np.exp(1j * gamma) * Mu) <= 1e-13 * max(abs(Mu) * max(G_amp, 1), 1e-30)      # (i)
+                want = (np.conj(Mg) * r).real
+                got = abs(Mg) * abs(r) * math.cos(np.angle(r) - np.angle(Mg)) if abs(Mg) > 0 else 0.0
+                assert abs(got - want) <= 1e-12 * max(abs(Mg) * abs(r), 1e-30)                                         # (ii)
+                if sig[k] == 0.0:      # delta pixel: the phase the kernel forms explicitly
+                    n0 = math.sqrt(1 - l[k] ** 2 - m[k] ** 2)
+                    X = 2 * math.pi * (uvw[j, 0] * l[k] + uvw[j, 1] * m[k] + uvw[j, 2] * (n0 - 1))
+                    got2 = G_amp / n0 * abs(r) * math.cos(X - gamma + np.angle(r))
+                    assert abs(got2 - want) <= 1e-9 * max(abs(Mg) * abs(r), 1e-30)
+    for _ in range(200):                                                                                              # (iii)
+        qq, Xp = rng.uniform(-3, 3), rng.uniform(-50, 50)
+        r = complex(rng.standard_normal(), rng.standard_normal())
+        A, B = r.real + qq * r.imag, qq * r.real - r.imag
+        R, psi = math.hypot(A, B), math.atan2(B, A)
+        lhs = A * math.cos(Xp) + B * math.sin(Xp)
+        assert abs(lhs - R * math.cos(Xp - psi)) <= 1e-12 * max(R, 1e-30)
+        # and A cos X' + B sin X' is Re((1 + iq) conj(c - i s) ... ) of the kernels' entry form: Re conj((1+iq)(c - is)) r
+        c, s = math.cos(Xp), math.sin(Xp)
+        assert abs(lhs - (np.conj((1 + 1j * qq) * (c - 1j * s)) * r).real) <= 1e-12 * max(R, 1e-30)
