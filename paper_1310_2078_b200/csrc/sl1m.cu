@@ -146,6 +146,26 @@ ApplyParams make_params(const sl1m_plan *p) {
     return P;
 }
 
+// Split count of an apply: `units` CTAs per split (visibility tiles / pixel groups) x n_chan channels, `n_items` work
+// items (pixel tiles / visibility chunks) to divide among the splits, `slots` CTAs resident on the GPU at one time.
+// Every CTA of an apply costs the same, so the launch takes ceil(CTAs / slots) CTA-durations: around the wanted
+// number of waves, take the split count that wastes the least of the last wave (config 5: 24 forward splits = 16.09
+// waves run as 17; 25 = 16.77).  A CTA with few items pays its fixed start-up cost more often: mild penalty.
+int pick_split(int units, int n_items, int slots, int waves, int n_chan) {
+    const double want = (double)slots * waves / std::max(1, n_chan);          // CTAs per channel
+    const int s_lo = std::max(1, (int)(0.75 * want / units)), s_hi = std::max(s_lo, (int)(1.6 * want / units) + 1);
+    int best = std::min(n_items, std::max(1, (int)((want + units - 1) / units)));
+    double best_score = -1.0;
+    for (int s0 = s_lo; s0 <= std::min(s_hi, n_items); ++s0) {
+        const int per = (n_items + s0 - 1) / s0, s_eff = (n_items + per - 1) / per;
+        const double w = (double)units * s_eff * n_chan / slots;
+        const double eff = w / std::ceil(w - 1e-9);
+        const double score = eff * per / (per + 0.25);
+        if (score > best_score + 1e-12) { best_score = score; best = s_eff; }
+    }
+    return best;
+}
+
 // Launch configuration (enough CTAs for 148 SMs x 4 resident CTAs x several waves, shared between the
 // channels of a batch) and the workspaces, all [n_chan][.].  Called at plan creation and again by
 // sl1m_plan_set_channels.
@@ -167,7 +187,11 @@ int configure_and_allocate(sl1m_plan *p) {
         if (p->phase64) rv = std::min(rv, 4);   // fp64 uvw live in registers
         p->fwd_rv = rv;
         p->fwd_vtiles = (int)((nvi + NT * rv - 1) / (NT * rv));
-        int split = std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
+        // resident CTAs per SM of the forward kernel this plan launches (its __launch_bounds__)
+        const int fwd_ctas = (rv == 8 || p->gk == 2) ? 4 : (p->pk == 0 && p->gk == 0 ? SL1M_FWD_MIN_CTAS : 4);
+        int split = (nvi * (int64_t)p->n_tiles >= (int64_t)64 * SM_COUNT_B200)
+                        ? pick_split(p->fwd_vtiles, p->n_tiles, SM_COUNT_B200 * fwd_ctas, waves, p->n_chan)
+                        : std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
         p->fwd_per_split = (p->n_tiles + split - 1) / split;
         p->fwd_split = (p->n_tiles + p->fwd_per_split - 1) / p->fwd_per_split;
     }
@@ -181,7 +205,11 @@ int configure_and_allocate(sl1m_plan *p) {
         if (p->phase64) rp = std::min(rp, 4);
         p->adj_rp = rp;
         p->adj_pgroups = p->n_pix_pad / (NT * rp);
-        int split = std::min(n_chunks, std::max(1, (target + p->adj_pgroups - 1) / p->adj_pgroups));
+        const bool one_cos = rp == 8 && p->pk == 0 && p->gk == 0 && !p->phase64;
+        const int adj_ctas = one_cos ? SL1M_ADJ_C1_MIN_CTAS : (rp == 8 ? 5 : (p->pk == 0 && p->gk == 0 ? SL1M_ADJ_MIN_CTAS : 4));
+        int split = ((int64_t)p->adj_pgroups * n_chunks >= (int64_t)64 * SM_COUNT_B200)
+                        ? pick_split(p->adj_pgroups, n_chunks, SM_COUNT_B200 * adj_ctas, waves, p->n_chan)
+                        : std::min(n_chunks, std::max(1, (target + p->adj_pgroups - 1) / p->adj_pgroups));
         p->adj_per_split = (n_chunks + split - 1) / split;
         p->adj_split = (n_chunks + p->adj_per_split - 1) / p->adj_per_split;
     }
