@@ -58,15 +58,20 @@ __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int
         total += c;
     }
     float4 *tile = zs.pixc + chan * n_pix_pad + (size_t)blockIdx.x * TP;
+    const int cnt4 = (total + 3) & ~3;
+    if (cnt4 == TP) {                                    // (nearly) full: keep the ORIGINAL order -- the gain kernels read
+        tile[threadIdx.x] = v;                           // the rows of a tile with TP entries from the table itself
+        if (threadIdx.x == 0) zs.cnt[chan * (size_t)(n_pix_pad / TP) + blockIdx.x] = TP;
+        return;                                          // uniform over the CTA
+    }
     if (nz) {
         const int pos = base + __popc(b & ((1u << lane) - 1u));
         tile[pos] = v;
         s_src[pos] = (uint8_t)threadIdx.x;
     }
-    const int cnt4 = (total + 3) & ~3;
     if ((int)threadIdx.x < cnt4 - total) tile[total + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (threadIdx.x == 0) zs.cnt[chan * (size_t)(n_pix_pad / TP) + blockIdx.x] = cnt4;
-    if (zs.gF && total < TP && total > 0) {              // gain rows of the compact entries (padding: a*x = 0, any row)
+    if (zs.gF && total > 0) {                            // gain rows of the compact entries (padding: a*x = 0, any row)
         __syncthreads();
         const size_t row0 = (size_t)blockIdx.x * TP;
         const float2 *src = zs.gF + row0 * zs.n_ant;

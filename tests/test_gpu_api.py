@@ -300,6 +300,10 @@ def test_zero_skipping_forward(sl, kind):
     cases["one"] = one
     few = np.zeros(n, np.float32); few[rng.choice(n, 37, replace=False)] = rng.uniform(0.1, 3, 37)
     cases["few"] = few
+    almost = rng.uniform(0.1, 1, n).astype(np.float32)       # tiles with 253-255 of 256 entries: "nearly full" tiles keep
+    almost[::97] = 0                                          # their original order (gain rows come from the table)
+    almost[5::131] = 0
+    cases["almost_full"] = almost
     for dens in (0.01, 0.6):
         x = np.where(rng.uniform(size=n) < dens, rng.uniform(0.1, 1, n), 0).astype(np.float32)
         cases["d%g" % dens] = x
