@@ -90,7 +90,9 @@ int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uvw, const in
 /* v = M x.  x DEV [n_pix] fp32 (real), vis DEV [n_vis][2] fp32.  Asynchronous on stream. */
 int sl1m_forward(sl1m_plan *plan, const float *x_dev, float *vis_dev, void *stream);
 
-/* g = Re M^H r.  r DEV [n_vis][2] fp32, img DEV [n_pix] fp32.  Asynchronous on stream. */
+/* g = Re M^H r.  r DEV [n_vis][2] fp32, img DEV [n_pix] fp32.  Asynchronous on stream.
+ * The image is real (PAPER.md:192-197 thresholds x_i > d), so only the real part is formed; the kernels evaluate
+ * it as sum_j |M_jk| |r_j| cos(arg r_j - arg M_jk): one cosine per term. */
 int sl1m_adjoint(sl1m_plan *plan, const float *r_dev, float *img_dev, void *stream);
 
 /* Same applies with HOST buffers: H2D copy, apply, D2H copy, stream synchronise. */
