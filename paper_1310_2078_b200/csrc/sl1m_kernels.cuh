@@ -1269,6 +1269,14 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(co
 #ifndef SL1M_ADJ_GTX2_MIN_CTAS
 #define SL1M_ADJ_GTX2_MIN_CTAS 5
 #endif
+//   *_GTX2_NP4  of a thread's 4 register pairs, how many take the FMA-pipe polynomial for sin/cos (forward) or
+//               cos (adjoint); ex2 stays on the MUFU pipe
+#ifndef SL1M_FWD_GTX2_NP4
+#define SL1M_FWD_GTX2_NP4 0
+#endif
+#ifndef SL1M_ADJ_GTX2_NP4
+#define SL1M_ADJ_GTX2_NP4 1
+#endif
 __device__ __forceinline__ void sincos2(f32x2 X, f32x2 &s, f32x2 &c) {
     float xa, xb, sa, ca, sb, cb;
     up2(X, xa, xb);
@@ -1372,9 +1380,17 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_GTX2_MIN_CTAS) fwd_kernel_gtx2(co
                 const f32x2 s2 = fma2(dv, dv, mul2(du, du));
                 const f32x2 Ep = fma2(s2, CE[i], LR[i]);
                 const f32x2 Xp = fma2(CX[i], Ep, X);
-                const f32x2 tw = mul2(bw, ex2_2(Ep));            // a x 2^E'
+                f32x2 tw = mul2(bw, ex2_2(Ep));                  // a x 2^E'
                 f32x2 s, cc;
-                sincos2(Xp, s, cc);
+                if (i < SL1M_FWD_GTX2_NP4) {                     // pipe balance: this pair's sin/cos on the FMA pipe
+                    uint32_t ka, kb;
+                    sincos_poly2(Xp, s, cc, ka, kb);
+                    float ta, tb;
+                    up2(tw, ta, tb);
+                    tw = pk2(flip_if_odd(ta, ka), flip_if_odd(tb, kb));
+                } else {
+                    sincos2(Xp, s, cc);
+                }
                 TC[i] = fma2(tw, cc, TC[i]);
                 TS[i] = fma2(tw, s, TS[i]);
             }
@@ -1470,9 +1486,18 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_GTX2_MIN_CTAS) adj_kernel_gtx2(co
                 const f32x2 s2 = fma2(dv, dv, mul2(du, du));
                 const f32x2 Ep = fma2(s2, bce, blr);
                 const f32x2 Xp = fma2(bcx, Ep, X);
-                float xa, xb;
-                up2(Xp, xa, xb);
-                ACC[i] = fma2(mul2(ex2_2(Ep), pk2(__cosf(xa), __cosf(xb))), bR, ACC[i]);
+                if (i < SL1M_ADJ_GTX2_NP4) {                     // pipe balance: this pair's cosine on the FMA pipe
+                    f32x2 c;
+                    uint32_t ka, kb;
+                    cos_poly2(Xp, c, ka, kb);
+                    float ea, eb;
+                    up2(ex2_2(Ep), ea, eb);
+                    ACC[i] = fma2(mul2(pk2(flip_if_odd(ea, ka), flip_if_odd(eb, kb)), c), bR, ACC[i]);
+                } else {
+                    float xa, xb;
+                    up2(Xp, xa, xb);
+                    ACC[i] = fma2(mul2(ex2_2(Ep), pk2(__cosf(xa), __cosf(xb))), bR, ACC[i]);
+                }
             }
         }
         __syncthreads();
