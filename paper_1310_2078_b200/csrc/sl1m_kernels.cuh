@@ -1011,7 +1011,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const 
 #define SL1M_ADJ_C1_NPQ 1
 #endif
 #ifndef SL1M_ADJ_C1_MIN_CTAS
-#define SL1M_ADJ_C1_MIN_CTAS 6
+#define SL1M_ADJ_C1_MIN_CTAS 8
 #endif
 __device__ __forceinline__ void cos_poly2(f32x2 X, f32x2 &c, uint32_t &k_lo, uint32_t &k_hi) {
     const f32x2 kf = fma2(X, bc2(0.318309886183790672f), bc2(12582912.0f));
