@@ -197,7 +197,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 
     wl = make_workload(args.config)
     t_plan = time.perf_counter()
-    plan = sl.Plan.from_workload(wl)
+    plan = sl.Plan.from_workload(wl, dense_forward=args.dense_forward)
     torch.cuda.synchronize()
     t_plan = time.perf_counter() - t_plan
     n_terms = float(wl.n_pix) * float(wl.n_vis)
@@ -438,6 +438,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=16.0, dest="cpu_seconds")
     ap.add_argument("--ref-seconds", type=float, default=8.0, dest="ref_seconds")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dense-forward", action="store_true", dest="dense_forward",
+                    help="SL1M_DENSE_FORWARD: the forward evaluates every term, also where the image is zero (A/B of the zero-skipping forward)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     rank = int(os.environ.get("RANK", "0"))
