@@ -410,7 +410,10 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         // With gains, visibilities are grouped by baseline (p, q) into groups of 8 samples (padded):
         // the gain product g_p conj(g_q) of a group is then loaded once per pixel instead of once
         // per term.  Sample r of group g sits at (g / 128) * 1024 + r * 128 + g % 128, which is the
-        // forward kernel's thread layout.  Used when padding costs < 25 %; else per-term gains.
+        // forward kernel's thread layout.  Used when the groups are at least 34 % full on average: measured at
+        // config 4, a grouped apply costs the same whatever its fill (8.2 + 5.0 ms per forward + adjoint for 8 slots)
+        // and the per-term kernels run at 0.52 / 1.4e12 terms/s, so 3 samples per baseline are still 1.3x faster
+        // grouped (13.2 against 17.2 ms) and 5 samples 2.1x; below that, per-term gains.
         std::vector<int> vperm;
         std::vector<int> ip, iq;
         p->n_vis_int = (int)n_vis;
@@ -430,7 +433,7 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
                 s0 = s1;
             }
             const int64_t n_groups_pad = ((n_groups + NT - 1) / NT) * NT;
-            if ((double)n_vis >= 0.75 * (double)(n_groups * 8) && n_groups_pad * 8 < ((int64_t)1 << 30)) {
+            if ((double)n_vis >= 0.34 * (double)(n_groups * 8) && n_groups_pad * 8 < ((int64_t)1 << 30)) {
                 p->gk = 2;
                 p->n_vis_int = (int)(n_groups_pad * 8);
                 vperm.assign((size_t)p->n_vis_int, -1);

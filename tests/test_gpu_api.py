@@ -284,7 +284,7 @@ def test_zero_skipping_forward(sl, kind):
     elif kind == "gains_grouped":
         wl = make_workload(4, n_side=64, n_ant=20, n_steps=8, n_src=50)      # gk == 2
     elif kind == "gains_per_term":
-        wl = make_workload(4, n_side=64, n_ant=20, n_steps=3, n_src=50)      # gk == 1
+        wl = make_workload(4, n_side=64, n_ant=20, n_steps=2, n_src=50)      # gk == 1
     else:
         wl = make_workload(3, n_side=64, n_steps=4, n_src=30)
     o = oracle.Oracle.from_workload(wl)
@@ -338,11 +338,11 @@ def test_zero_skipping_forward(sl, kind):
     plan.close(); dense.close()
 
 
-@pytest.mark.parametrize("n_steps", [8, 3])
+@pytest.mark.parametrize("n_steps", [8, 2])
 def test_polar_gain_corner_cases(sl, n_steps):
     """The gain tables are kept in polar form (|g|, arg g).  Exact zeros, negative real and purely imaginary gains
     (arg = pi, +-pi/2: gamma_p - gamma_q reaches +-2 pi), gains of very different magnitude, and a residual with exact
-    zeros (|r| = 0, arg r = 0 in the one-cosine adjoint); grouped (8 samples) and per-term (3 samples) kernels."""
+    zeros (|r| = 0, arg r = 0 in the one-cosine adjoint); grouped (8 samples) and per-term (2 samples) kernels."""
     import torch
     wl = make_workload(4, n_side=64, n_ant=12, n_steps=n_steps, n_src=40)
     rng = np.random.default_rng(23)

@@ -191,11 +191,11 @@ def test_config4_gains_applies_reduced_full_output(sl):
     print("config4-reduced", res)
 
 
-@pytest.mark.parametrize("n_steps,expect_gk", [(8, 2), (7, 2), (16, 2), (3, 1)])
+@pytest.mark.parametrize("n_steps,expect_gk", [(8, 2), (7, 2), (16, 2), (3, 2), (2, 1)])
 def test_config4_gains_grouped_and_generic_paths(sl, n_steps, expect_gk):
     """Baseline-grouped gain kernels (8 samples of one baseline share one gain product; 7 -> one
-    padded slot per group, 16 -> two groups per baseline) and the per-term fallback (3 samples
-    would waste 5/8 of each group)."""
+    padded slot per group, 16 -> two groups per baseline, 3 -> five padded slots, still faster than
+    per-term gains) and the per-term fallback (2 samples per baseline: groups only a quarter full)."""
     wl = make_workload(4, n_side=64, n_ant=20, n_steps=n_steps, n_src=50)
     plan = sl.Plan.from_workload(wl)
     assert plan.describe()["gains"] == expect_gk
