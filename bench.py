@@ -37,7 +37,7 @@ MUFU_PER_SM_PER_CLK = 16      # 4 SFU lanes per SM sub-partition x 4 (measured 1
 SM_COUNT = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (config, kernel) -> bytes
-NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 99.89e6, (5, "adj"): 43.28e6, (4, "fwd"): 341.8e6, (4, "adj"): 325.9e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 100.70e6, (5, "adj"): 52.56e6, (4, "fwd"): 341.8e6, (4, "adj"): 328.0e6}
 
 
 def _peaks():
@@ -379,7 +379,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                       f"{desc['mufu_per_term_mufu_path']}, adj {desc['adj_mufu_per_term']} (real image: one cosine per adjoint term)",
         "traffic_basis": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full "
                          "(profiles/, same kernel and workload; null = not captured); algorithmic bytes at config 5: ~30 MB in per apply "
-                         "+ the split partials (37 x 3.25 MB forward, 13 x 4 MB adjoint, mostly L2-resident)",
+                         "+ the split partials (37 x 3.25 MB forward, 15 x 4 MB adjoint, partly L2-resident)",
         "mufu_only_bound_Tterm_per_s": mufu_only / 1e12,
         "frac_vs_mufu_only_bound": achieved / mufu_only,
         "best_split_bound_Tterm_per_s": None if balanced is None else balanced / 1e12,
