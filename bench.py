@@ -363,10 +363,15 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     balanced = (SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / (m_ * (1.0 - f_bal))
                 if not (desc["gaussian"] or desc["gains"]) else None)
     dom = "sl1m::adj_kernel" if dom_is_adj else "sl1m::fwd_kernel"
-    if dom_is_adj and desc["adj_packed_pairs"] and desc["adj_mufu_per_term"] == 1 and not desc["gains"]:
-        dom += "_c1"
-    elif (desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"]):
-        dom += "_x2"
+    if (desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"]):      # the packed R = 8 kernels
+        if int(desc["gaussian"]) == 2:
+            dom += "_gtx2"
+        elif dom_is_adj and int(desc["gains"]) == 2:
+            dom += "_g2x2"
+        elif dom_is_adj and desc["adj_mufu_per_term"] == 1:
+            dom += "_c1"
+        else:
+            dom += "_x2"
     achieved, peak = (ach_a, pk_a) if dom_is_adj else (ach_f, pk_f)
     traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "adj" if dom_is_adj else "fwd"))
     roof = {
