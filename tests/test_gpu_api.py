@@ -323,6 +323,11 @@ def test_zero_skipping_forward(sl, kind):
         assert rel_l2(v, want) <= 2e-4, (name, rel_l2(v, want))
         assert rel_l2(v, vd) <= 2e-5, (name, rel_l2(v, vd))
         assert np.array_equal(v, plan.forward(xd).cpu().numpy())            # bit-stable
+    # a NaN pixel counts as non-zero: it reaches every visibility, as in the dense forward
+    xn = cases["few"].copy()
+    xn[n // 2] = np.nan
+    assert np.isnan(plan.forward(_dev(xn, torch.float32)).cpu().numpy()).all()
+    assert np.isnan(dense.forward(_dev(xn, torch.float32)).cpu().numpy()).all()
     # the solver takes the same iterates with and without skipping (differences: which terms take the
     # polynomial sincos, i.e. rounding only)
     V = _dev((o.forward(cases["few"]) + 0.01 * (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis))
