@@ -1024,12 +1024,12 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->phase_span_rad = (float)p->phase_span;
     o->zero_skip = p->pixc != nullptr;
     o->adj_mufu_per_term = o->mufu_per_term_mufu_path;
-    if (p->adj_rp == 8 && !(p->phase64 && p->n_chan == 1)) {
-#ifndef SL1M_ADJ_TWO_MUFU
-        if (p->pk == 0 && p->gk == 0) o->adj_mufu_per_term = 1;    // adj_kernel_c1
+    if (!(p->phase64 && p->n_chan == 1)) {
+        if (p->pk == 0) o->adj_mufu_per_term = 1;    // delta pixels: one cosine per term in every adjoint kernel
+#ifdef SL1M_ADJ_TWO_MUFU
+        if (p->pk == 0 && p->gk == 0 && p->adj_rp == 8) o->adj_mufu_per_term = 2;   // adj_kernel_x2 (A/B build)
 #endif
-        if (p->pk == 0 && p->gk == 2) o->adj_mufu_per_term = 1;    // adj_kernel_g2x2
-        if (p->pk == 2 && p->gk == 0) o->adj_mufu_per_term = 2;    // adj_kernel_gtx2
+        if (p->pk == 2 && p->gk == 0 && p->adj_rp == 8) o->adj_mufu_per_term = 2;    // adj_kernel_gtx2: ex2 + cos
     }
     if (o->phase_fp64) o->fwd_poly_per16 = o->adj_poly_per16 = 0;
     const bool tile_gauss = p->pk == 2 && p->gk == 0;

@@ -774,6 +774,12 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
         }
         s_vis[buf][slot] = make_float4(static_cast<float>(TWO_PI * u), static_cast<float>(TWO_PI * v),
                                        static_cast<float>(TWO_PI * w), static_cast<float>(w));
+        // delta pixels: one cosine per term, Re(e^{iX} r) = |r| cos(X + arg r); arg r joins the centre phases below
+        float rphi = 0.f;
+        if (PK == 0) {
+            rphi = atan2f(rr.y, rr.x);
+            rr = make_float2(sqrtf(fmaf(rr.x, rr.x, rr.y * rr.y)), 0.f);
+        }
         s_r[buf][slot] = rr;
         if (GK == 1) s_ant[buf][slot] = a;
         if (GK == 2 && tid < 16) s_ant[buf][tid] = a;   // sample 0 carries the group's (p, q)
@@ -789,7 +795,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 gauss_tile_constants(w, cen.w, q, cE, lr, x0c);
                 s_tc[buf][slot][c] = make_float4(q, cE, lr, x0c);
             }
-            s_x0[buf][slot][c] = x0c;
+            s_x0[buf][slot][c] = x0c + rphi;
         }
     };
 
@@ -861,6 +867,19 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
                 }
                 float ere, eim;
                 uint32_t sgn;
+                if (PK == 0) {   // delta pixel: |r| cos(X + arg r), rr.x = |r| (arg r is inside x0)
+                    float cv;
+                    if (i < PolySplit<RP, PK, GK, SL1M_ADJ_NPOLY8>::N) {
+                        float sv;
+                        sincos_poly(X, sv, cv, sgn);         // the unused sine polynomial is dead code
+                        cv = fxor(cv, sgn);
+                    } else {
+                        cv = __cosf(X);
+                    }
+                    if (GK == 2) Zr[i] = fmaf(cv, rr.x, Zr[i]);
+                    else acc[i] = fmaf(GK == 1 ? g1 * rr.x : rr.x, cv, acc[i]);
+                    continue;
+                }
                 if (PK == 2) {   // one sigma per tile: Re conj(M / a) r = amp (cr r_re + ci r_im)
                     float amp;
                     gen_entry_tile(X, du, dv, tc.x, tc.y, tc.z, amp, ere, eim);
