@@ -280,6 +280,28 @@ int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
  */
 int sl1m_forward_active_pixels(sl1m_plan *plan, int64_t *n_active_host, void *stream);
 
+/*
+ * sl1m_measure_peaks -- issue-rate micro-benchmark for the roofline the operator is held against.
+ * The operator is a GENERATED matrix-vector product (the matrix is never stored), bound by the XU
+ * (MUFU.SIN/COS/EX2) and FMA pipes, not by HBM; the denominators are therefore measured with those instructions in
+ * the kernels' own launch shape (128-thread CTAs, 8 per SM on every SM, chains of independent instructions).
+ * Runs ~10 short kernels on `stream` (about 50 ms in all), synchronises, needs no plan.  All rates are for the
+ * whole GPU at the clock the probes ran at (sm_clock_mhz, from clock64 over the event-timed duration).
+ */
+typedef struct {
+    int32_t n_sm;
+    double sm_clock_mhz;                 /* SM clock during the MUFU probe                                         */
+    double mufu_per_s, mufu_per_clk_sm;  /* MUFU.EX2 alone: results/s, results per clock per SM (nominal 16)        */
+    double mufu_cos_per_clk_sm;          /* MUFU.COS alone (same pipe)                                              */
+    double ffma_per_s, ffma_per_clk_sm;  /* scalar FFMA alone (nominal 128 per clock per SM)                        */
+    double ffma2_lanes_per_s, ffma2_lanes_per_clk_sm;   /* packed FFMA2, counted in fp32 lanes (2 per instruction)  */
+    double coissue_mufu_per_clk_sm;      /* 4 MUFU + 12 FFMA2 + 4 FMUL.RZ per body: MUFU results per clock per SM   */
+    double coissue_ffma2_lanes_per_clk_sm;   /* ... and the FFMA2 lanes per clock per SM achieved beside them       */
+    double coissue_cycles_per_iter;      /* sub-partition cycles per warp per body (profiles/r1_microbench.md: 35.3) */
+    double coissue_adj_mufu_per_clk_sm;  /* 4 MUFU.COS + 8 FFMA2 + 4 FMUL.RZ per body (the one-cosine adjoint's mix) */
+} sl1m_peaks;
+int sl1m_measure_peaks(sl1m_peaks *out_host, void *stream);
+
 /* Number of kernels this plan has launched since creation (for bench.py's gpu_launches). */
 int64_t sl1m_launch_count(const sl1m_plan *plan);
 

@@ -58,7 +58,7 @@ def _load():
         lib.oracle_threshold.argtypes = [f64, f64]
         lib.oracle_threshold.restype = f64
         lib.oracle_fista.argtypes = [P, vp, f64, f64, i32, vp, vp, vp, vp]
-        lib.oracle_fista_tol.argtypes = [P, vp, f64, f64, i32, f64, i32, vp, vp, vp, vp]
+        lib.oracle_fista_tol.argtypes = [P, vp, f64, f64, i32, f64, f64, i32, vp, vp, vp, vp, vp]
         lib.oracle_fista_tol.restype = i32
         _lib = lib
     return _lib
@@ -153,32 +153,39 @@ class Oracle:
         return float(_load().oracle_max_eig(ctypes.byref(self._c), int(n_pow)))
 
     # O5
-    def fista(self, V, lam: float, L: float, n_iter: int, x0=None, want_trace: bool = False):
+    def fista(self, V, lam: float, L: float, n_iter: int, x0=None, want_trace: bool = False,
+              want_info: bool = True):
+        """want_info=False passes info3 = NULL: the C routine then skips its closing forward for
+        ||M I_K - V||^2 (one whole apply at config 5)."""
         V = np.ascontiguousarray(np.asarray(V, dtype=np.complex128)).view(np.float64)
         assert V.shape[0] == 2 * self.n_vis
         x0a = None if x0 is None else np.ascontiguousarray(x0, dtype=np.float64)
         x = np.zeros(self.n_pix)
         trace = np.zeros((max(n_iter, 1), 3)) if want_trace else None
-        info = np.zeros(3)
+        info = np.zeros(3) if want_info else None
         _load().oracle_fista(ctypes.byref(self._c), _ptr(V), float(lam), float(L), int(n_iter),
                              _ptr(x0a), _ptr(x), _ptr(trace), _ptr(info))
-        out = dict(x=x, l2_term=float(info[0]), l1_term=float(info[1]), nnz=int(info[2]))
+        out = dict(x=x)
+        if want_info:
+            out.update(l2_term=float(info[0]), l1_term=float(info[1]), nnz=int(info[2]))
         if want_trace:
             out["trace"] = trace[:n_iter]
         return out
 
-    # O5 + the termination rule of PAPER.md:194 / :239 (reading R21)
-    def fista_tol(self, V, lam: float, L: float, max_iter: int, tol: float, check_every: int = 1, x0=None):
+    # O5 + the termination rules of PAPER.md:194 / :239 (readings R21: total error; R24: number of non-zeros)
+    def fista_tol(self, V, lam: float, L: float, max_iter: int, tol: float, check_every: int = 1, x0=None,
+                  nnz_tol: float = -1.0):
         V = np.ascontiguousarray(np.asarray(V, dtype=np.complex128)).view(np.float64)
         assert V.shape[0] == 2 * self.n_vis
         x0a = None if x0 is None else np.ascontiguousarray(x0, dtype=np.float64)
         x = np.zeros(self.n_pix)
         trace = np.zeros((max(max_iter, 1), 3))
         info = np.zeros(3)
+        E = np.zeros(max(max_iter, 1))
         n_done = _load().oracle_fista_tol(ctypes.byref(self._c), _ptr(V), float(lam), float(L), int(max_iter),
-                                          float(tol), int(check_every), _ptr(x0a), _ptr(x), _ptr(trace),
-                                          _ptr(info))
-        return dict(x=x, n_iter_done=int(n_done), trace=trace[:n_done], l2_term=float(info[0]),
+                                          float(tol), float(nnz_tol), int(check_every), _ptr(x0a), _ptr(x), _ptr(trace),
+                                          _ptr(info), _ptr(E))
+        return dict(x=x, n_iter_done=int(n_done), trace=trace[:n_done], E=E[:n_done], l2_term=float(info[0]),
                     l1_term=float(info[1]), nnz=int(info[2]))
 
     # PAPER.md:327 "use the dirty image as the initial condition": the back-projected data,

@@ -173,12 +173,18 @@ double oracle_threshold(double x, double d) { return (x > d) ? x - d : 0.0; }
  * already has -- E_k = ||M y_k - V||^2 + 2 lambda sum I_k, i.e. eq (10) with lambda_paper =
  * 2 lambda (reading R9) and the residual of y_k (MFISTA's extra evaluation of M is what the
  * paper avoids).  The rule is looked at only when k is a multiple of check_every
- * (k >= 2): stop after iteration k iff |E_k - E_{k-1}| <= tol * |E_k|.  tol < 0 never stops.
+ * (k >= 2): stop after iteration k iff |E_k - E_{k-1}| <= tol * |E_k|.  tol < 0 switches this rule off.
+ * The same sentence of PAPER.md:194 offers a second criterion, "or when there is a sufficiently small
+ * change in the number of non-zero entries in I_k".  Reading R24: with N_k = nnz(I_k), at the
+ * same looked-at iterations k >= 2, stop iff |N_k - N_{k-1}| <= nnz_tol * N_k (nnz_tol = 0: the support
+ * size did not change at all); nnz_tol < 0 switches this rule off.  The paper joins the two with "or":
+ * the run stops as soon as either enabled rule holds.
  * Returns the number of iterations done. */
 int32_t oracle_fista_tol(const oracle_problem *P, const double *V /* [n_vis][2] */, double lambda, double L,
-                         int32_t n_iter /* cap */, double tol, int32_t check_every,
+                         int32_t n_iter /* cap */, double tol, double nnz_tol, int32_t check_every,
                          const double *x0 /* nullable */, double *x_out /* [n_pix] */,
-                         double *trace /* [n_iter][3] or NULL */, double *info3 /* nullable */) {
+                         double *trace /* [n_iter][3] or NULL */, double *info3 /* nullable */,
+                         double *E_out /* [n_iter] or NULL: the E_k the rule looked at */) {
     const int64_t np = P->n_pix, nv = P->n_vis;
     double *Ik = (double *)calloc(np, sizeof(double));
     double *Iprev = (double *)calloc(np, sizeof(double));
@@ -188,7 +194,7 @@ int32_t oracle_fista_tol(const oracle_problem *P, const double *V /* [n_vis][2] 
     if (x0) { memcpy(Ik, x0, sizeof(double) * np); memcpy(y, x0, sizeof(double) * np); }
     double t = 1.0;
     const double d = lambda / L;
-    double E_prev = 0.0;
+    double E_prev = 0.0, N_prev = 0.0;
     int32_t n_done = 0;
     for (int32_t it = 0; it < n_iter; ++it) {
         oracle_forward(P, y, nv, NULL, r);
@@ -209,9 +215,12 @@ int32_t oracle_fista_tol(const oracle_problem *P, const double *V /* [n_vis][2] 
         if (trace) { trace[3 * it] = l2; trace[3 * it + 1] = l1; trace[3 * it + 2] = nnz; }
         n_done = it + 1;
         const double E = l2 + 2.0 * lambda * l1;                       /* eq (10), reading R21 */
-        const int look = tol >= 0.0 && n_done >= 2 && check_every >= 1 && (n_done % check_every) == 0;
-        if (look && fabs(E - E_prev) <= tol * fabs(E)) break;
+        if (E_out) E_out[it] = E;
+        const int look = n_done >= 2 && check_every >= 1 && (n_done % check_every) == 0;
+        if (look && tol >= 0.0 && fabs(E - E_prev) <= tol * fabs(E)) break;
+        if (look && nnz_tol >= 0.0 && fabs(nnz - N_prev) <= nnz_tol * nnz) break;   /* reading R24 */
         E_prev = E;
+        N_prev = nnz;
     }
     memcpy(x_out, Ik, sizeof(double) * np);
     if (info3) {
@@ -229,5 +238,5 @@ int32_t oracle_fista_tol(const oracle_problem *P, const double *V /* [n_vis][2] 
 void oracle_fista(const oracle_problem *P, const double *V /* [n_vis][2] */, double lambda, double L,
                   int32_t n_iter, const double *x0 /* nullable */, double *x_out /* [n_pix] */,
                   double *trace /* [n_iter][3] or NULL */, double *info3 /* nullable */) {
-    (void)oracle_fista_tol(P, V, lambda, L, n_iter, -1.0, 1, x0, x_out, trace, info3);
+    (void)oracle_fista_tol(P, V, lambda, L, n_iter, -1.0, -1.0, 1, x0, x_out, trace, info3, NULL);
 }

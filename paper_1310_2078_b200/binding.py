@@ -34,6 +34,13 @@ class _PlanInfo(ctypes.Structure):
         "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("zero_skip", ctypes.c_int32), ("adj_mufu_per_term", ctypes.c_int32)]
 
 
+class _Peaks(ctypes.Structure):
+    _fields_ = [("n_sm", ctypes.c_int32)] + [(n, ctypes.c_double) for n in (
+        "sm_clock_mhz", "mufu_per_s", "mufu_per_clk_sm", "mufu_cos_per_clk_sm", "ffma_per_s", "ffma_per_clk_sm",
+        "ffma2_lanes_per_s", "ffma2_lanes_per_clk_sm", "coissue_mufu_per_clk_sm", "coissue_ffma2_lanes_per_clk_sm",
+        "coissue_cycles_per_iter", "coissue_adj_mufu_per_clk_sm")]
+
+
 class _QtLevel(ctypes.Structure):
     _fields_ = [("n_pix", ctypes.c_int64), ("L", ctypes.c_float), ("n_iter_done", ctypes.c_int32),
                 ("l2_term", ctypes.c_double), ("l1_term", ctypes.c_double), ("nnz", ctypes.c_int64),
@@ -69,11 +76,13 @@ _lib = None
 
 
 def load_library():
-    """Load libsl1m.so (building it if the sources are newer).  Raises if it cannot be had."""
+    """Load libsl1m.so, rebuilding it first when it is missing or older than any of its sources
+    (build_library's mtime check; a no-op when up to date).  SL1M_LIBRARY names a prebuilt library
+    to load as is.  Raises if the library cannot be had."""
     global _lib
     if _lib is not None:
         return _lib
-    path = os.environ.get("SL1M_LIBRARY") or (build_library() if not os.path.exists(LIB) or os.environ.get("SL1M_REBUILD") else LIB)
+    path = os.environ.get("SL1M_LIBRARY") or build_library(force=bool(os.environ.get("SL1M_REBUILD")))
     lib = ctypes.CDLL(path)
     vp, i64, i32, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
     lib.sl1m_plan_create.argtypes = [ctypes.POINTER(vp), i64, vp, vp, vp, i64, vp, vp, vp, i32, vp,
@@ -104,6 +113,7 @@ def load_library():
                                         ctypes.POINTER(ctypes.c_int), vp]
     lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
     lib.sl1m_forward_active_pixels.argtypes = [vp, vp, vp]
+    lib.sl1m_measure_peaks.argtypes = [ctypes.POINTER(_Peaks), vp]
     lib.sl1m_launch_count.argtypes = [vp]
     lib.sl1m_launch_count.restype = i64
     lib.sl1m_plan_n_vis.argtypes = [vp]
@@ -144,6 +154,13 @@ def _dev_ptr(t, dtype, numel: int, name: str):
             and t.numel() == numel):
         raise ValueError(f"{name}: need a contiguous CUDA tensor of {dtype} with {numel} elements")
     return ctypes.c_void_p(t.data_ptr())
+
+
+def measure_peaks(stream=None) -> dict:
+    """sl1m_measure_peaks: MUFU / FFMA / FFMA2 issue rates of this GPU (roofline denominators)."""
+    pk = _Peaks()
+    _check(load_library().sl1m_measure_peaks(ctypes.byref(pk), _stream_ptr(stream)))
+    return {n: (int(getattr(pk, n)) if n == "n_sm" else float(getattr(pk, n))) for n, _ in _Peaks._fields_}
 
 
 def quadtree_refine(l, m, side, I, frac: float, min_side: float):

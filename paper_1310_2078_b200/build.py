@@ -7,7 +7,8 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "sl1m.cu")
 SRC_QT = os.path.join(_HERE, "csrc", "sl1m_quadtree.cu")
-DEPS = [SRC, SRC_QT, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"),
+SRC_PK = os.path.join(_HERE, "csrc", "sl1m_peaks.cu")
+DEPS = [SRC, SRC_QT, SRC_PK, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"),
         os.path.join(os.path.dirname(_HERE), "include", "sl1m.h")]
 LIB = os.path.join(_HERE, "libsl1m.so")
 
@@ -26,7 +27,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     stale = not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(d) for d in DEPS)
     if force or stale:
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("SL1M_NVCC_EXTRA", "").split(), "-o", tmp, SRC, SRC_QT]   # SL1M_NVCC_EXTRA: tuning -D flags
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("SL1M_NVCC_EXTRA", "").split(), "-o", tmp, SRC, SRC_QT, SRC_PK]   # SL1M_NVCC_EXTRA: tuning -D flags
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)

@@ -247,6 +247,75 @@ def test_tolerance_stop_rule():
     assert o.fista_tol(V, lam=lam, L=L, max_iter=37, tol=-1.0)["n_iter_done"] == 37
 
 
+def test_total_error_weight_is_eq10_at_the_independent_minimiser():
+    """Reading R21: the E the stopping rule looks at is eq (10) written for the
+    listing's lambda, E = ||M y - V||^2 + 2 lambda sum I.  Pin without restating it: at convergence
+    y_k = I_k = I*, so E_K must equal TWICE the minimum of F(I) = 1/2 ||V - M I||^2 + lambda sum I
+    over I >= 0, and that minimum comes from scipy.optimize.nnls (an independent library solve,
+    not from the oracle).  A `lambda` for `2 lambda` slip gives 2 F* - lambda sum I*, off by 10 %."""
+    rng = np.random.default_rng(31)
+    o = _tiny(rng, n_vis=80, n_pix=30)
+    x_true = np.zeros(o.n_pix)
+    x_true[[3, 11, 17, 25]] = [1.0, 0.4, 2.5, 0.7]
+    V = o.forward(x_true) + 0.01 * (rng.standard_normal(o.n_vis) + 1j * rng.standard_normal(o.n_vis))
+    M = o.dense()
+    H = (M.conj().T @ M).real
+    L = np.linalg.eigvalsh(H)[-1] * 1.0001
+    lam = 0.5
+    b = (M.conj().T @ V).real - lam
+    Rch = np.linalg.cholesky(H).T
+    x_nnls, _ = scipy.optimize.nnls(Rch, np.linalg.solve(Rch.T, b), maxiter=2000)
+    Fstar = 0.5 * np.sum(np.abs(M @ x_nnls - V) ** 2) + lam * np.sum(x_nnls)
+    r = o.fista_tol(V, lam=lam, L=L, max_iter=4000, tol=-1.0)
+    assert r["n_iter_done"] == 4000 and r["E"].shape == (4000,)
+    assert abs(r["E"][-1] - 2.0 * Fstar) < 1e-9 * Fstar
+    assert lam * np.sum(x_nnls) > 0.05 * Fstar          # the L1 part is a visible share of E: the weight matters
+    # and E_1 is the residual of y_1 = 0 plus the L1 part of I_1
+    I1 = o.fista(V, lam=lam, L=L, n_iter=1)["x"]
+    assert abs(r["E"][0] - (np.sum(np.abs(V) ** 2) + 2.0 * lam * I1.sum())) < 1e-9
+
+
+def test_nnz_change_stop_rule():
+    """Reading R24 ("... or when there is a sufficiently small change in the number of
+    non-zero entries in I_k"): at the looked-at iterations k >= 2 stop iff |N_k - N_{k-1}| <= nnz_tol N_k.
+    (i)  DFT lattice: the iterates are constant from I_1 on, so N_2 = N_1 and the rule fires at the
+         first looked-at k >= 2 (the E rule needs k >= 3 there: y_2 != y_1).
+    (ii) the stop index equals the one recomputed here from np.count_nonzero of the fixed-K iterates
+         (the images themselves, not the oracle's own nnz column).
+    (iii) "or": with both rules on, the run stops at the earlier of the two indices; only truncation."""
+    o = _dft_lattice()
+    rng = np.random.default_rng(8)
+    V = rng.standard_normal(64) + 1j * rng.standard_normal(64)
+    for every, want in ((1, 2), (2, 2), (3, 3), (5, 5)):
+        r = o.fista_tol(V, lam=3.0, L=64.0, max_iter=50, tol=-1.0, nnz_tol=0.0, check_every=every)
+        assert r["n_iter_done"] == want
+    rng = np.random.default_rng(36)
+    o = _tiny(rng, n_vis=60, n_pix=120)                      # more pixels than data: the support keeps moving
+    x_true = np.zeros(o.n_pix)
+    x_true[rng.choice(o.n_pix, 12, replace=False)] = rng.uniform(0.5, 3.0, 12)
+    V = o.forward(x_true) + 0.05 * (rng.standard_normal(o.n_vis) + 1j * rng.standard_normal(o.n_vis))
+    L = o.max_eig(200) * 1.05
+    lam, K = 0.3, 300
+    N = np.array([np.count_nonzero(o.fista(V, lam=lam, L=L, n_iter=k)["x"]) for k in range(1, K + 1)])
+    assert len(set(N[:40].tolist())) > 3                     # the support size really changes early on
+    seen = set()
+    for nnz_tol in (0.2, 0.05, 0.0):
+        for every in (1, 4):
+            ks = [k for k in range(2, K + 1) if k % every == 0 and abs(int(N[k - 1]) - int(N[k - 2])) <= nnz_tol * N[k - 1]]
+            want = ks[0] if ks else K
+            r = o.fista_tol(V, lam=lam, L=L, max_iter=K, tol=-1.0, nnz_tol=nnz_tol, check_every=every)
+            assert r["n_iter_done"] == want, (nnz_tol, every, r["n_iter_done"], want)
+            assert np.array_equal(r["x"], o.fista(V, lam=lam, L=L, n_iter=want)["x"])
+            seen.add(want)
+    assert len(seen) >= 2 and min(seen) >= 2
+    # (iii) either rule
+    k_E = o.fista_tol(V, lam=lam, L=L, max_iter=K, tol=1e-5)["n_iter_done"]
+    k_N = o.fista_tol(V, lam=lam, L=L, max_iter=K, tol=-1.0, nnz_tol=0.0)["n_iter_done"]
+    k_any = o.fista_tol(V, lam=lam, L=L, max_iter=K, tol=1e-5, nnz_tol=0.0)["n_iter_done"]
+    assert k_any == min(k_E, k_N) and k_E != k_N
+    assert o.fista_tol(V, lam=lam, L=L, max_iter=23, tol=-1.0, nnz_tol=-1.0)["n_iter_done"] == 23
+
+
 def test_dirty_image_start():
     """Reading R22: the dirty image max(0, s Re A^H V) as I_0.  On the DFT lattice
     Re A^H V / N^2 is numpy's inverse FFT; and FISTA's first iterate from zero is
