@@ -3,7 +3,9 @@
 
 A "step" is ONE FISTA iteration = one pass of the whole hot path:
 forward A y, residual, adjoint A^H r, threshold + momentum update, objective partials -- issued
-through the C ABI (`sl1m_solve`, n_iter = 1, warm-started from the previous step's image).
+through the C ABI's stepping calls (`sl1m_fista_begin` once, then `sl1m_fista_step(1)` per step), so the
+warm-up and timed steps are consecutive iterations of ONE continuing FISTA run from I_0 = 0 (momentum on).
+The same run is also timed as a single `sl1m_solve(n_iter = warmup + steps)` call ("continuous_solve").
 Default workload: BASELINE.json configs[4], the configuration the metric is quoted on
 (1024^2 pixels x 406,400 visibilities, full w-term), synthetic seeded inputs.
 
@@ -33,7 +35,7 @@ from workloads import fista_lambda, make_workload  # noqa: E402
 
 METRIC = "pixel_x_visibility_terms_per_s (A and A^H inside one FISTA iteration)"
 UNIT = "terms/s"
-MUFU_PER_SM_PER_CLK = 16      # 4 SFU lanes per SM sub-partition x 4 (measured 15.7, profiles/r1_microbench.md)
+MUFU_PER_SM_PER_CLK = 16      # nominal: 4 SFU lanes per SM sub-partition x 4; the line's peaks use the MEASURED rate
 SM_COUNT = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (config, kernel) -> bytes
@@ -218,12 +220,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     def ev():
         return torch.cuda.Event(enable_timing=True)
 
-    # ---------------- device-resident steps ----------------
-    x = torch.zeros(wl.n_pix, dtype=torch.float32, device=dev)
-    x_next = torch.empty_like(x)
-    for _ in range(args.warmup):
-        plan.solve(V, lam, L=L, n_iter=1, x0=x, out=x_next, want_info=False)
-        x, x_next = x_next, x
+    # ---------------- issue-rate peaks of THIS GPU, measured now (sl1m_measure_peaks, csrc/sl1m_peaks.cu) ----
+    pk_meas = sl.measure_peaks() if rank == 0 else None
+
+    # ---------------- device-resident steps: consecutive iterations of one FISTA run ----------------
+    skip = bool(plan.describe()["zero_skip"])
+    plan.fista_begin(V, lam, L)
+    plan.fista_step(args.warmup)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -232,24 +235,39 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     time.sleep(0.3)
     launches0 = plan.launch_count
     pairs = []
-    nnz_steps = []          # non-zero pixels of each step's forward input (zero-skipping forward)
+    nnz_steps = []          # pixels the step's forward streams (non-zeros of y_k, padded to 4 per tile)
     t_wall0 = time.time()
     torch.cuda.synchronize()
     for _ in range(args.steps):
-        nnz_steps.append(torch.count_nonzero(x))      # device scalar, queued before the flush; read after the loop
+        nnz_steps.append(plan.forward_active_pixels() if skip else wl.n_pix)   # synchronises: outside the events
         flush.zero_()
         a, b = ev(), ev()
         a.record(stream)
-        plan.solve(V, lam, L=L, n_iter=1, x0=x, out=x_next, want_info=False)
+        plan.fista_step(1)
         b.record(stream)
         pairs.append((a, b))
-        x, x_next = x_next, x
     torch.cuda.synchronize()
     t_wall1 = time.time()
     launches = plan.launch_count - launches0
     step_ms = [a.elapsed_time(b) for a, b in pairs]
     total_ms = sum(step_ms)
     clocks = sampler.stop(t_wall0, t_wall1)
+    x, k_done = plan.fista_image()
+    assert k_done == args.warmup + args.steps
+
+    # ---------------- the same run as ONE call: sl1m_solve(n_iter = warmup + steps), events around the call ----
+    n_cont = args.warmup + args.steps
+    trace = torch.zeros(3 * n_cont, dtype=torch.float64, device=dev)
+    x_cont = torch.empty_like(x)
+    flush.zero_()
+    a, b = ev(), ev()
+    a.record(stream)
+    plan.solve(V, lam, L=L, n_iter=n_cont, out=x_cont, trace=trace, want_info=False)
+    b.record(stream)
+    torch.cuda.synchronize()
+    cont_ms = a.elapsed_time(b)
+    cont_same = bool(torch.equal(x_cont, x))
+    tr = trace.cpu().numpy().reshape(n_cont, 3)
 
     # ---------------- per-apply timings (dominant kernels), same flush discipline ----------------
     def time_call(fn, reps):
@@ -303,8 +321,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     # Terms EVALUATED per step: the adjoint takes all N_p x N_v; the forward only the pixels with y_k != 0
     # (zero-skipping, include/sl1m.h; the skipped terms are exactly zero) -- all of them when the plan does not skip.
     desc = plan.describe()
-    skip = bool(desc["zero_skip"])
-    nnz_list = [int(v) for v in nnz_steps] if skip else [wl.n_pix] * args.steps
+    nnz_list = [int(v) for v in nnz_steps]
     e2e_nnz = e2e_nnz if skip else [wl.n_pix] * len(e2e_nnz)
     terms_per_step = (float(wl.n_pix) + sum(nnz_list) / len(nnz_list)) * float(wl.n_vis)
     value = aggregate_value(world, terms_per_step, args.steps, t_max)
@@ -348,59 +365,76 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         b_issue = SM_COUNT * 128.0 * clock_hz / slots
         return min(b_mufu, b_fma, b_issue), b_mufu, b_fma, b_issue
 
-    pk_f, pk_f_mufu, pk_f_fma, pk_f_issue = bound("fwd", desc["fwd_poly_per16"], desc["fwd_packed_pairs"], f_max)
-    pk_a, pk_a_mufu, pk_a_fma, pk_a_issue = bound("adj", desc["adj_poly_per16"], desc["adj_packed_pairs"], f_max)
-    ach_f, ach_a = n_terms / (fwd_ms * 1e-3), n_terms / (adj_ms * 1e-3)
-    # the dominant kernel of the TIMED STEP: the adjoint evaluates every term, the forward only the non-zero pixels
-    step_ms_mean = t_max / args.steps
-    dom_is_adj = adj_ms >= step_ms_mean - adj_ms
-    m_dom = desc["adj_mufu_per_term"] if dom_is_adj else desc["mufu_per_term_mufu_path"]
-    mufu_only = SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / m_dom      # every term on the MUFU path
-    # best any MUFU/FMA split of the dominant kernel's instruction set could do (delta pixels, unit gains):
-    # MUFU time = FMA time, m (1-f)/16 = (a (1-f) + b f)/128 with (m, a, b) = (2, 6, 18) forward, (1, 5, 12) adjoint
-    m_, a_, b_ = (1.0, 5.0, 12.0) if (dom_is_adj and m_dom == 1) else (2.0, 6.0, 18.0)
-    f_bal = (8.0 * m_ - a_) / (8.0 * m_ - a_ + b_)
-    balanced = (SM_COUNT * MUFU_PER_SM_PER_CLK * f_max / (m_ * (1.0 - f_bal))
-                if not (desc["gaussian"] or desc["gains"]) else None)
-    dom = "sl1m::adj_kernel" if dom_is_adj else "sl1m::fwd_kernel"
-    if (desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"]):      # the packed R = 8 kernels
-        if int(desc["gaussian"]) == 2:
-            dom += "_gtx2"
-        elif dom_is_adj and int(desc["gains"]) == 2:
-            dom += "_g2x2"
-        elif dom_is_adj and desc["adj_mufu_per_term"] == 1:
-            dom += "_c1"
-        else:
-            dom += "_x2"
-    achieved, peak = (ach_a, pk_a) if dom_is_adj else (ach_f, pk_f)
+    # Measured denominators (sl1m_measure_peaks): MUFU results/s, FFMA2 fp32 lanes/s, SM clock of the probes.
+    R_mufu, R_fma = pk_meas["mufu_per_s"], pk_meas["ffma2_lanes_per_s"]
+    clk_meas = pk_meas["sm_clock_mhz"] * 1e6
+    plain = not (desc["gaussian"] or desc["gains"])
+
+    def kernel_entry(kind, ms, per16, packed, name):
+        """Roofline of one apply kernel on a DENSE image (every N_p x N_v term evaluated).
+        own_mix: min(MUFU pipe, FMA pipe, issue slots) for the kernel's SASS instruction mix, with the measured
+                 pipe rates -- moves with the polynomial share the kernel was tuned to (context);
+        mufu_only: every term on the MUFU path, measured MUFU rate / MUFU per term (SURVEY.md 8(d) as written);
+        best_split: the best ANY MUFU/FMA split of this instruction set allows: MUFU time = FMA time,
+                 m (1-f)/R_mufu = (a (1-f) + b f)/R_fma, (m, a, b) = (2, 6, 18) forward, (1, 5, 12) one-cosine adjoint
+                 -- the fixed hardware ceiling the headline frac is quoted against (delta pixels, unit gains)."""
+        ach = n_terms / (ms * 1e-3)
+        own, b_mufu, b_fma, b_issue = bound(kind, per16, packed, clk_meas)
+        scale_m, scale_f = R_mufu / (SM_COUNT * MUFU_PER_SM_PER_CLK * clk_meas), R_fma / (SM_COUNT * 128.0 * clk_meas)
+        own = min(b_mufu * scale_m, b_fma * scale_f, b_issue)
+        m_term = desc["adj_mufu_per_term"] if kind == "adj" else desc["mufu_per_term_mufu_path"]
+        mufu_only = R_mufu / m_term
+        best = None
+        if plain and not desc["phase_fp64"]:
+            m_, a_, b_ = (1.0, 5.0, 12.0) if (kind == "adj" and m_term == 1) else (2.0, 6.0, 18.0)
+            d = m_ / R_mufu - a_ / R_fma
+            f_bal = max(0.0, d / (d + b_ / R_fma))
+            best = R_mufu / (m_ * (1.0 - f_bal))
+        e = {"kernel": name, "ms": ms, "Tterm_per_s": ach / 1e12, "poly_per16": per16,
+             "own_mix_bound": own / 1e12, "frac_vs_own_mix": ach / own,
+             "mufu_only_bound": mufu_only / 1e12, "frac_vs_mufu_only": ach / mufu_only,
+             "best_split_bound": None if best is None else best / 1e12,
+             "frac_vs_best_split": None if best is None else ach / best,
+             "own_mix_pipes": {"mufu": b_mufu * scale_m / 1e12, "fma": b_fma * scale_f / 1e12, "issue": b_issue / 1e12}}
+        return e, ach, (best if best is not None else own)
+
+    def kname(kind):
+        nm = "sl1m::adj_kernel" if kind == "adj" else "sl1m::fwd_kernel"
+        if desc["phase_fp64"]:
+            return nm + "_p64"
+        if (desc["adj_packed_pairs"] if kind == "adj" else desc["fwd_packed_pairs"]):      # the packed R = 8 kernels
+            if int(desc["gaussian"]) == 2:
+                nm += "_gtx2"
+            elif kind == "adj" and int(desc["gains"]) == 2:
+                nm += "_g2x2"
+            elif kind == "adj" and desc["adj_mufu_per_term"] == 1:
+                nm += "_c1"
+            else:
+                nm += "_x2"
+        return nm
+
+    ent_f, ach_f, pk_f = kernel_entry("fwd", fwd_ms, desc["fwd_poly_per16"], desc["fwd_packed_pairs"], kname("fwd"))
+    ent_a, ach_a, pk_a = kernel_entry("adj", adj_ms, desc["adj_poly_per16"], desc["adj_packed_pairs"], kname("adj"))
+    # headline kernel: the one with the LARGER time on a dense image (stable run to run; both are first-class below)
+    dom_is_adj = adj_ms > fwd_ms
+    dom_e, achieved, peak = (ent_a, ach_a, pk_a) if dom_is_adj else (ent_f, ach_f, pk_f)
     traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "adj" if dom_is_adj else "fwd"))
     roof = {
-        "bound": "alu", "kernel": dom, "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "Tterm/s",
+        "bound": "alu", "kernel": dom_e["kernel"], "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "Tterm/s",
         "frac": achieved / peak, "traffic": traffic,
-        "peak_basis": f"min(MUFU pipe, FMA pipe, issue slots) for the kernel's own SASS instruction mix at "
-                      f"{f_max/1e6:.0f} MHz (sm_max_mhz, {peaks_src}): {SM_COUNT} SMs x {MUFU_PER_SM_PER_CLK} MUFU/clk, "
-                      f"x 128 fp32 lanes/clk, x 128 thread-instr/clk; fwd {desc['fwd_poly_per16']}/16 and adj "
-                      f"{desc['adj_poly_per16']}/16 of the terms use FMA-pipe polynomials; MUFU per MUFU-path term: fwd "
-                      f"{desc['mufu_per_term_mufu_path']}, adj {desc['adj_mufu_per_term']} (real image: one cosine per adjoint term)",
+        "peak_basis": ("best MUFU/FMA split bound of the kernel's instruction set (fixed ceiling)" if dom_e["best_split_bound"]
+                       else "own-mix issue bound (Gaussian / gain kernels: no polynomial-split ceiling defined)") +
+                      ", from the MUFU and FFMA2 rates measured in this run by sl1m_measure_peaks (peak_measured); "
+                      "kernels.fwd / kernels.adj carry all three denominators for both apply kernels",
+        "peak_measured": pk_meas,
+        "kernels": {"fwd": ent_f, "adj": ent_a},
         "traffic_basis": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full "
                          "(profiles/, same kernel and workload; null = not captured); algorithmic bytes at config 5: ~30 MB in per apply "
                          "+ the split partials (37 x 3.25 MB forward, 15 x 4 MB adjoint, partly L2-resident)",
-        "mufu_only_bound_Tterm_per_s": mufu_only / 1e12,
-        "frac_vs_mufu_only_bound": achieved / mufu_only,
-        "best_split_bound_Tterm_per_s": None if balanced is None else balanced / 1e12,
-        "frac_vs_best_split_bound": None if balanced is None else achieved / balanced,
-        "fwd": {"ms": fwd_ms, "Tterm_per_s": ach_f / 1e12, "peak": pk_f / 1e12, "frac": ach_f / pk_f,
-                "mufu_bound": pk_f_mufu / 1e12, "fma_bound": pk_f_fma / 1e12, "issue_bound": pk_f_issue / 1e12},
-        "adj": {"ms": adj_ms, "Tterm_per_s": ach_a / 1e12, "peak": pk_a / 1e12, "frac": ach_a / pk_a,
-                "mufu_bound": pk_a_mufu / 1e12, "fma_bound": pk_a_fma / 1e12, "issue_bound": pk_a_issue / 1e12},
         "plan": desc,
-        "note": "per-apply time = C-ABI call (main kernel + O(N) epilogues, < 0.1 % of it); "
+        "note": "per-apply time = C-ABI call on a dense image (main kernel + O(N) epilogues, < 0.1 % of it); "
                 "not an HBM-bound path: the matrix is generated, never read",
     }
-    if clocks.get("sm_mhz"):
-        pk_c = bound("adj" if dom_is_adj else "fwd", desc["adj_poly_per16"] if dom_is_adj else desc["fwd_poly_per16"],
-                     desc["adj_packed_pairs"] if dom_is_adj else desc["fwd_packed_pairs"], clocks["sm_mhz"] * 1e6)[0]
-        roof["frac_at_sampled_clock"] = achieved / pk_c
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -415,7 +449,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                    "pixel_kind": "gaussian" if wl.sigma is not None else "delta",
                    "gains": wl.gains is not None, "lambda": lam, "L": L,
                    "l2_flush": "256 MiB device memset between timed steps",
-                   "step": "one FISTA iteration via sl1m_solve(n_iter=1, x0=previous image); per-apply timings use a dense image",
+                   "step": "one FISTA iteration via sl1m_fista_step(1): warm-up and timed steps are consecutive iterations "
+                           "of one run from I_0 = 0 (momentum carried); per-apply timings use a dense image; the e2e leg "
+                           "is sl1m_solve_host(n_iter=1, x0=previous image), which restarts the momentum on every call",
                    "parallelism": "replicas" if world > 1 else "single-gpu"},
         "iters_per_s": world * args.steps / (t_max * 1e-3),
         "terms": {"counted": "evaluated terms: N_v x (N_p for A^H + pixels with y_k != 0 for A)",
@@ -423,6 +459,12 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                   "fwd_active_pixels_per_step": nnz_list,
                   "dense_equivalent_terms_per_s": aggregate_value(world, 2.0 * n_terms, args.steps, t_max)},
         "step_ms": step_ms, "plan_create_s": t_plan, "max_eig_s": t_eig, "n_pow": args.n_pow,
+        "continuous_solve": {"call": f"sl1m_solve(n_iter={n_cont}) from I_0 = 0, trace on, CUDA events around the call",
+                             "n_iter": n_cont, "ms_total": cont_ms, "ms_per_iter": cont_ms / n_cont,
+                             "iters_per_s": 1e3 * n_cont / cont_ms,
+                             "nnz_I_k": [int(v) for v in tr[:, 2]],
+                             "image_bit_identical_to_stepped_run": cont_same},
+        "dense_forward_step_ms": fwd_ms + adj_ms,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_mean, "call": "sl1m_solve_host(n_iter=1) with pinned host V, x0, x_out"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,

@@ -60,7 +60,7 @@ typedef enum {
 
 /* flags for sl1m_plan_create */
 #define SL1M_GAINS_ON_DEVICE 1u /* `gains` is a DEV pointer (default: HOST) */
-#define SL1M_PHASE_FP64 2u      /* accumulate the whole phase in fp64 (delta pixels, unit gains, one channel).
+#define SL1M_PHASE_FP64 2u      /* accumulate the whole phase in fp64 (delta pixels, unit gains).
                                  * Chosen automatically when the fp32 phase remainder inside a pixel tile could
                                  * exceed 256 rad (a tile spanning > 40 fringes of the longest baseline: a badly
                                  * undersampled image); the default kernels are exact enough otherwise. */
@@ -153,11 +153,52 @@ int sl1m_solve_tol(sl1m_plan *plan, const float *vis_dev, float lambda, float L,
                    float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host, void *stream);
 
 /*
+ * sl1m_solve_stop -- sl1m_solve with BOTH termination criteria of PAPER.md:194 ("terminated when an iteration
+ * leads to a sufficiently small change in the total error E, given by equation (10), or when there is a
+ * sufficiently small change in the number of non-zero entries in I_k"), decided ON THE DEVICE:
+ *   E rule    |E_k - E_{k-1}| <= tol |E_k|        E_k = ||M y_k - V||^2 + 2 lambda sum I_k  (reading R21); tol < 0: off
+ *   nnz rule  |N_k - N_{k-1}| <= nnz_tol N_k      N_k = nnz(I_k)                          (reading R24); nnz_tol < 0: off
+ * looked at after every check_every-th iteration k >= 2; the solve stops at the first k where an enabled rule
+ * holds (at least one must be enabled), else at max_iter.  A one-CTA kernel takes the decision from the trace rows
+ * the iteration has just written and raises a device flag; every kernel of a stopped solve returns at once, so
+ * the image is that of the stopping iteration.  The host never waits for an iteration: it reads the flag two
+ * polls (of >= 16 iterations) behind what it has enqueued and synchronises once at the end for info_host.
+ * sl1m_solve_tol(tol) == sl1m_solve_stop(tol, nnz_tol = -1).
+ *   trace_dev DEV [max_iter][3] fp64 or NULL (a plan-owned buffer is used); rows past n_iter_done are not written.
+ *   info_host REQUIRED (n_iter_done is how the caller learns k).
+ * sl1m_solve_stop_batch: the same for every channel of a batched plan, each stopping on its own (a stopped
+ * channel's CTAs return at once while the others go on); lambda_host, L_host, info_host HOST [n_chan],
+ * trace_dev DEV [n_chan][max_iter][3] or NULL.
+ */
+int sl1m_solve_stop(sl1m_plan *plan, const float *vis_dev, float lambda, float L, int n_pow,
+                    int max_iter, double tol, double nnz_tol, int check_every, const float *x0_dev,
+                    float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host, void *stream);
+int sl1m_solve_stop_batch(sl1m_plan *plan, const float *vis_dev, const float *lambda_host,
+                          const float *L_host, int n_pow, int max_iter, double tol, double nnz_tol,
+                          int check_every, const float *x0_dev, float *x_out_dev, double *trace_dev,
+                          sl1m_solve_info *info_host, void *stream);
+
+/*
+ * Stepping API -- the listing of PAPER.md:188-192 driven a few iterations at a time (interactive imaging; bench.py
+ * times the steps of ONE continuing FISTA run through it).  The state (I_k, y_{k+1}, t_{k+1}) lives in the plan.
+ *   sl1m_fista_begin  y_1 = I_0 = x0 (0 if NULL), t_1 = 1.  lambda_host, L_host HOST [n_chan] (L > 0).  vis_dev
+ *                     DEV [n_chan][n_vis][2] is BORROWED: it must stay valid and unchanged until the next begin.
+ *   sl1m_fista_step   n_iter more iterations, asynchronous on stream.  trace_dev DEV [n_chan][max(n_iter,1)][3] or
+ *                     NULL receives the rows of THIS call's iterations.
+ *   sl1m_fista_image  x_out DEV [n_chan][n_pix] = I_k; *n_iter_done_host (nullable) = k.  Asynchronous.
+ * Any other solve call on the plan, or sl1m_plan_set_channels, ends the state.
+ */
+int sl1m_fista_begin(sl1m_plan *plan, const float *vis_dev, const float *lambda_host,
+                     const float *L_host, const float *x0_dev, void *stream);
+int sl1m_fista_step(sl1m_plan *plan, int n_iter, double *trace_dev, void *stream);
+int sl1m_fista_image(sl1m_plan *plan, float *x_out_dev, int32_t *n_iter_done_host, void *stream);
+
+/*
  * sl1m_dirty_image -- img = max(0, scale * Re M^H V): "use the dirty image as the initial
  * condition", clipped to the positive orthant the solver lives in.  scale is the
  * caller's normalisation (1/n_vis gives unit point-source response for delta pixels near the
- * phase centre).  vis DEV [n_vis][2], img DEV [n_pix]; asynchronous on stream.  Pass the result
- * as x0_dev to sl1m_solve / sl1m_solve_tol.
+ * phase centre).  vis DEV [n_chan][n_vis][2], img DEV [n_chan][n_pix] (every channel of a batched plan, same
+ * scale); asynchronous on stream.  Pass the result as x0_dev to sl1m_solve / sl1m_solve_stop(_batch).
  */
 int sl1m_dirty_image(sl1m_plan *plan, const float *vis_dev, float scale, float *img_dev, void *stream);
 
@@ -227,9 +268,11 @@ int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float *vis_host,
  *   vis_dev DEV [n_chan][n_vis][2]; x0_dev (nullable), x_out_dev DEV [n_chan][n_pix];
  *   trace_dev DEV [n_chan][max(n_iter,1)][3] or NULL.
  * Channels never interact: every result equals the single-channel call on uvw * scale[c].
- * The single-problem calls (sl1m_max_eig, sl1m_solve, sl1m_solve_tol, sl1m_dirty_image, *_host)
- * return SL1M_ERR_PARAM on a plan with more than one channel.  Re-allocates the plan's
- * workspaces; synchronises the device.
+ * The single-problem calls (sl1m_max_eig, sl1m_solve, sl1m_solve_tol, sl1m_solve_stop, *_host) return
+ * SL1M_ERR_PARAM on a plan with more than one channel (use the *_batch call).  Re-allocates the plan's
+ * workspaces; synchronises the device.  Transactional: on failure (e.g. out of memory) the plan is unchanged.
+ * The fp64-phase decision (SL1M_PHASE_FP64) is re-evaluated for max(scale): a plan whose fp32 phase remainder
+ * would exceed 256 rad at its highest channel switches to the fp64-phase kernels, which honour the scales too.
  */
 int sl1m_plan_set_channels(sl1m_plan *plan, int32_t n_chan, const double *scale_host);
 int32_t sl1m_plan_n_chan(const sl1m_plan *plan);
@@ -286,11 +329,12 @@ int sl1m_forward_active_pixels(sl1m_plan *plan, int64_t *n_active_host, void *st
  * (MUFU.SIN/COS/EX2) and FMA pipes, not by HBM; the denominators are therefore measured with those instructions in
  * the kernels' own launch shape (128-thread CTAs, 8 per SM on every SM, chains of independent instructions).
  * Runs ~10 short kernels on `stream` (about 50 ms in all), synchronises, needs no plan.  All rates are for the
- * whole GPU at the clock the probes ran at (sm_clock_mhz, from clock64 over the event-timed duration).
+ * whole GPU, timed with CUDA events; the per-clock figures divide by the device's maximum SM clock.
  */
 typedef struct {
     int32_t n_sm;
-    double sm_clock_mhz;                 /* SM clock during the MUFU probe                                         */
+    double sm_clock_mhz;                 /* the device's maximum SM clock (cudaDevAttrClockRate): basis of the per-clock figures */
+    double clock64_mhz;                  /* clock64 ticks per second seen by the MUFU probe (not the SM clock on B200; unused)    */
     double mufu_per_s, mufu_per_clk_sm;  /* MUFU.EX2 alone: results/s, results per clock per SM (nominal 16)        */
     double mufu_cos_per_clk_sm;          /* MUFU.COS alone (same pipe)                                              */
     double ffma_per_s, ffma_per_clk_sm;  /* scalar FFMA alone (nominal 128 per clock per SM)                        */

@@ -36,7 +36,7 @@ class _PlanInfo(ctypes.Structure):
 
 class _Peaks(ctypes.Structure):
     _fields_ = [("n_sm", ctypes.c_int32)] + [(n, ctypes.c_double) for n in (
-        "sm_clock_mhz", "mufu_per_s", "mufu_per_clk_sm", "mufu_cos_per_clk_sm", "ffma_per_s", "ffma_per_clk_sm",
+        "sm_clock_mhz", "clock64_mhz", "mufu_per_s", "mufu_per_clk_sm", "mufu_cos_per_clk_sm", "ffma_per_s", "ffma_per_clk_sm",
         "ffma2_lanes_per_s", "ffma2_lanes_per_clk_sm", "coissue_mufu_per_clk_sm", "coissue_ffma2_lanes_per_clk_sm",
         "coissue_cycles_per_iter", "coissue_adj_mufu_per_clk_sm")]
 
@@ -98,6 +98,13 @@ def load_library():
                                     ctypes.POINTER(_SolveInfo), vp]
     lib.sl1m_solve_tol.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int,
                                    vp, vp, vp, ctypes.POINTER(_SolveInfo), vp]
+    lib.sl1m_solve_stop.argtypes = [vp, vp, f32, f32, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                    ctypes.c_int, vp, vp, vp, ctypes.POINTER(_SolveInfo), vp]
+    lib.sl1m_solve_stop_batch.argtypes = [vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                          ctypes.c_int, vp, vp, vp, vp, vp]
+    lib.sl1m_fista_begin.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.sl1m_fista_step.argtypes = [vp, ctypes.c_int, vp, vp]
+    lib.sl1m_fista_image.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_int32), vp]
     lib.sl1m_dirty_image.argtypes = [vp, vp, f32, vp, vp]
     lib.sl1m_plan_set_channels.argtypes = [vp, ctypes.c_int32, vp]
     lib.sl1m_plan_n_chan.argtypes = [vp]
@@ -360,15 +367,82 @@ class Plan:
             ctypes.byref(info), _stream_ptr(stream)))
         return out, SolveInfo(info.n_iter_done, info.L_used, info.l2_term, info.l1_term, info.nnz)
 
-    def dirty_image(self, vis, scale: float = None, out=None, stream=None):
-        """sl1m_dirty_image: max(0, scale * Re M^H vis); scale defaults to 1/n_vis."""
+    def solve_stop(self, vis, lam: float, L: float, max_iter: int, tol: float = -1.0, nnz_tol: float = -1.0,
+                   check_every: int = 1, n_pow: int = 30, x0=None, out=None, trace=None, stream=None):
+        """sl1m_solve_stop: FISTA until the total error changes by <= tol (relative) OR the number of non-zero
+        pixels by <= nnz_tol (relative), decided on the device; a negative tolerance switches that rule off.
+        Returns (x, SolveInfo); SolveInfo.n_iter_done is the iteration it stopped at."""
         import torch
         if out is None:
             out = torch.empty(self.n_pix, dtype=torch.float32, device=vis.device)
+        info = _SolveInfo()
+        _check(load_library().sl1m_solve_stop(
+            self._h, _dev_ptr(vis, torch.complex64, self.n_vis, "vis"), float(lam), float(L), int(n_pow),
+            int(max_iter), float(tol), float(nnz_tol), int(check_every),
+            _dev_ptr(x0, torch.float32, self.n_pix, "x0"), _dev_ptr(out, torch.float32, self.n_pix, "out"),
+            _dev_ptr(trace, torch.float64, 3 * max(int(max_iter), 0), "trace") if trace is not None else None,
+            ctypes.byref(info), _stream_ptr(stream)))
+        return out, SolveInfo(info.n_iter_done, info.L_used, info.l2_term, info.l1_term, info.nnz)
+
+    def solve_stop_batch(self, vis, lam, L, max_iter: int, tol: float = -1.0, nnz_tol: float = -1.0,
+                         check_every: int = 1, n_pow: int = 30, x0=None, out=None, trace=None, stream=None):
+        """sl1m_solve_stop_batch: every channel stops on its own.  Returns (x [n_chan][n_pix], [SolveInfo])."""
+        import torch
+        C = self.n_chan
+        lam_a = np.ascontiguousarray(np.broadcast_to(np.asarray(lam, np.float32), (C,)))
+        L_a = np.ascontiguousarray(np.broadcast_to(np.asarray(L, np.float32), (C,)))
+        if out is None:
+            out = torch.empty((C, self.n_pix), dtype=torch.float32, device=vis.device)
+        infos = (_SolveInfo * C)()
+        _check(load_library().sl1m_solve_stop_batch(
+            self._h, _dev_ptr(vis, torch.complex64, C * self.n_vis, "vis"), _np_ptr(lam_a), _np_ptr(L_a), int(n_pow),
+            int(max_iter), float(tol), float(nnz_tol), int(check_every),
+            _dev_ptr(x0, torch.float32, C * self.n_pix, "x0"), _dev_ptr(out, torch.float32, C * self.n_pix, "out"),
+            _dev_ptr(trace, torch.float64, C * 3 * max(int(max_iter), 1), "trace") if trace is not None else None,
+            ctypes.cast(infos, ctypes.c_void_p), _stream_ptr(stream)))
+        return out, [SolveInfo(i.n_iter_done, i.L_used, i.l2_term, i.l1_term, i.nnz) for i in infos]
+
+    def fista_begin(self, vis, lam, L, x0=None, stream=None):
+        """sl1m_fista_begin: start a stepped FISTA run.  `vis` is borrowed by the library: the binding keeps a
+        reference so the tensor outlives the run."""
+        import torch
+        C = self.n_chan
+        lam_a = np.ascontiguousarray(np.broadcast_to(np.asarray(lam, np.float32), (C,)))
+        L_a = np.ascontiguousarray(np.broadcast_to(np.asarray(L, np.float32), (C,)))
+        _check(load_library().sl1m_fista_begin(
+            self._h, _dev_ptr(vis, torch.complex64, C * self.n_vis, "vis"), _np_ptr(lam_a), _np_ptr(L_a),
+            _dev_ptr(x0, torch.float32, C * self.n_pix, "x0"), _stream_ptr(stream)))
+        self._fista_vis = vis
+        return self
+
+    def fista_step(self, n_iter: int = 1, trace=None, stream=None):
+        """sl1m_fista_step: n_iter more iterations of the run begun by fista_begin (asynchronous)."""
+        import torch
+        _check(load_library().sl1m_fista_step(
+            self._h, int(n_iter),
+            _dev_ptr(trace, torch.float64, self.n_chan * 3 * max(int(n_iter), 1), "trace") if trace is not None else None,
+            _stream_ptr(stream)))
+        return self
+
+    def fista_image(self, out=None, stream=None):
+        """sl1m_fista_image: (I_k, k) of the stepped run."""
+        import torch
+        if out is None:
+            out = torch.empty(self._shape(self.n_pix), dtype=torch.float32, device="cuda")
+        k = ctypes.c_int32(0)
+        _check(load_library().sl1m_fista_image(self._h, _dev_ptr(out, torch.float32, self.n_chan * self.n_pix, "out"),
+                                               ctypes.byref(k), _stream_ptr(stream)))
+        return out, int(k.value)
+
+    def dirty_image(self, vis, scale: float = None, out=None, stream=None):
+        """sl1m_dirty_image: max(0, scale * Re M^H vis); scale defaults to 1/n_vis.  Batched plans: [n_chan][.]."""
+        import torch
+        if out is None:
+            out = torch.empty(self._shape(self.n_pix), dtype=torch.float32, device=vis.device)
         _check(load_library().sl1m_dirty_image(
-            self._h, _dev_ptr(vis, torch.complex64, self.n_vis, "vis"),
+            self._h, _dev_ptr(vis, torch.complex64, self.n_chan * self.n_vis, "vis"),
             float(1.0 / self.n_vis if scale is None else scale),
-            _dev_ptr(out, torch.float32, self.n_pix, "out"), _stream_ptr(stream)))
+            _dev_ptr(out, torch.float32, self.n_chan * self.n_pix, "out"), _stream_ptr(stream)))
         return out
 
     # ---- host-buffer calls (numpy / pinned torch CPU tensors) ----

@@ -75,13 +75,30 @@ struct sl1m_plan {
     // host-buffer variants
     float *h_x = nullptr, *h_vis = nullptr, *h_img = nullptr;   // device staging for *_host calls
     bool phase64 = false;         // fp64-phase kernels (delta pixels, unit gains) -- flag or automatic
+    bool phase64_flag = false;    // SL1M_PHASE_FP64 was given
+    bool phase64_capable = false; // delta pixels with unit gains: pixd exists, the fp64-phase kernels can be switched to
+    double4 *pixdc = nullptr;     // [n_chan][n_pix_pad] compact copy of pixd for the zero-skipping fp64-phase forward
+    float2 *pixgc = nullptr;      // [n_chan][n_pix_pad] compact copy of pixg for the zero-skipping per-pixel-sigma forward
     double4 *pixd = nullptr;      // DEV [n_pix_pad] (dl, dm, dn', 0) as doubles, only with phase64
     double phase_span = 0.0;      // plan-time bound on the fp32 phase remainder, radians
     int n_chan = 1;               // batched channels (NEXT-4): every per-image / per-visibility buffer is [n_chan][.]
     double *chan_scale = nullptr; // DEV [n_chan] nu_c / nu_0, NULL while n_chan == 1
     float2 *step_c = nullptr;     // DEV [n_chan] (1/L_c, lambda_c/L_c) for the batched solver
-    double *trace_buf = nullptr;  // plan-owned trace for sl1m_solve_tol when the caller passes none
-    int trace_cap = 0;
+    double *trace_buf = nullptr;  // plan-owned trace for sl1m_solve_stop when the caller passes none
+    size_t trace_cap = 0;         // doubles
+    // FISTA state of the stepping API (sl1m_fista_begin / _step / _image); the solve calls are built on it
+    bool f_active = false;
+    const float2 *f_vis = nullptr;   // BORROWED measured visibilities
+    std::vector<float> f_lam, f_L;   // per channel
+    float f_inv_L = 0.f, f_thr = 0.f;
+    double f_t = 1.0;                // t_{k+1} of the listing (fp64 on the host; beta is a kernel argument)
+    int f_k = 0;                     // iterations enqueued since begin
+    // device-side termination (sl1m_solve_stop): ctl_i = {done[C], n_done[C], all_done}
+    int *ctl_i = nullptr;
+    double *lam2 = nullptr;          // DEV [n_chan] 2 lambda_c (the weight of sum I in E, reading R21)
+    const int *done_ptr = nullptr;   // == ctl_i while a stopping solve is enqueueing, else NULL
+    int *h_flag = nullptr;           // pinned HOST [2]: all_done as seen by the last two polls
+    cudaEvent_t poll_ev[2] = {nullptr, nullptr};
     int64_t launches = 0;
     int device = 0;
 };
@@ -99,9 +116,13 @@ void free_plan(sl1m_plan *p) {
     void *ptrs[] = {p->u64, p->v64, p->w64, p->ant_p, p->ant_q, p->pix4, p->pixg, p->cen, p->amp,
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
-                    p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc, p->rpol};
+                    p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc, p->rpol, p->ctl_i,
+                    p->lam2, p->pixdc, p->pixgc};
     for (void *q : ptrs)
         if (q) cudaFree(q);
+    if (p->h_flag) cudaFreeHost(p->h_flag);
+    for (cudaEvent_t e : p->poll_ev)
+        if (e) cudaEventDestroy(e);
     delete p;
 }
 
@@ -143,6 +164,7 @@ ApplyParams make_params(const sl1m_plan *p) {
     P.chan_scale = p->chan_scale;
     P.ws_v_stride = (size_t)p->fwd_split * (size_t)p->n_vis_int;
     P.ws_p_stride = (size_t)p->adj_split * (size_t)p->n_pix_pad;
+    P.done = p->done_ptr;
     return P;
 }
 
@@ -239,7 +261,7 @@ int configure_and_allocate(sl1m_plan *p) {
     // sigma, fp64 offsets).  Gain plans keep a compact copy of the gain rows next to the compact tiles
     // (n_chan x the table; not beyond 8 GiB -- such a plan keeps the dense forward).
     const size_t gfc_bytes = p->gk != 0 ? (C * npad + GAIN_ROW_PAD) * (size_t)p->n_ant * sizeof(float2) : 0;
-    if (!p->dense_forward && p->pk != 1 && !(p->phase64 && p->n_chan == 1) && gfc_bytes <= ((size_t)8 << 30)) {
+    if (!p->dense_forward && p->pk != 1 && !p->phase64 && gfc_bytes <= ((size_t)8 << 30)) {
         CUDA_TRY(cudaMalloc((void **)&p->pixc, C * npad * sizeof(float4)));
         CUDA_TRY(cudaMalloc((void **)&p->tile_cnt, C * (size_t)p->n_tiles * sizeof(int)));
         CUDA_TRY(cudaMemset(p->pixc, 0, C * npad * sizeof(float4)));
@@ -478,8 +500,11 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         // fp64-phase kernels: on request, or when the fp32 remainder could exceed ~256 rad (sin.approx
         // loses 4e-5 there, profiles/r1_microbench.md); delta pixels with unit gains only.
         p->phase_span = span;
-        p->phase64 = !any_gauss && !gains && ((flags & SL1M_PHASE_FP64) || span > 256.0);
-        if (p->phase64 && (st = upload(&p->pixd, pixd.data(), npad))) return st;
+        p->phase64_capable = !any_gauss && !gains;
+        p->phase64_flag = (flags & SL1M_PHASE_FP64) != 0;
+        p->phase64 = p->phase64_capable && (p->phase64_flag || span > 256.0);
+        // kept for every plan that could need it: sl1m_plan_set_channels may switch to the fp64-phase kernels
+        if (p->phase64_capable && (st = upload(&p->pixd, pixd.data(), npad))) return st;
         if (gains) {
             if ((st = upload(&p->ant_p, vperm.empty() ? ant_p : ip.data(), nvi))) return st;
             if ((st = upload(&p->ant_q, vperm.empty() ? ant_q : iq.data(), nvi))) return st;
@@ -506,9 +531,11 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
         if (e1 == cudaSuccess) e1 = cudaMemset(p->gF + lay_n, 0, (size_t)GAIN_ROW_PAD * n_ant * sizeof(float2));
         cudaError_t e2 = (e1 == cudaSuccess) ? cudaMalloc((void **)&p->gA, lay_n * sizeof(float2)) : e1;
         if (e2 == cudaSuccess) {
-            dim3 grid((p->n_pix_pad + ET - 1) / ET, n_ant);
-            gains_layout_kernel<<<grid, ET>>>(raw, n_ant, (int)n_pix, p->n_pix_pad, p->perm, p->gF, p->gA);
-            e2 = cudaDeviceSynchronize();
+            // antennas are looped inside the kernel (grid.y would cap n_ant at 65,535; "each (antenna, time)
+            // its own row" can exceed that)
+            gains_layout_kernel<<<(p->n_pix_pad + ET - 1) / ET, ET>>>(raw, n_ant, (int)n_pix, p->n_pix_pad, p->perm, p->gF, p->gA);
+            e2 = cudaGetLastError();
+            if (e2 == cudaSuccess) e2 = cudaDeviceSynchronize();
             p->launches++;
         }
         if (!(flags & SL1M_GAINS_ON_DEVICE)) cudaFree(raw);
@@ -563,7 +590,7 @@ void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
                 adj_kernel_x2<SL1M_ADJ_NPQ, B><<<grid, NT, 0, s>>>(P);
 #else
                 ApplyParams Q = P;      // one cosine per term: the kernel reads the residual in polar form
-                vis_polar_kernel<<<dim3((unsigned)egrid((size_t)p->n_vis_int), (unsigned)p->n_chan), ET, 0, s>>>(P.r, p->rpol, p->n_vis_int);
+                vis_polar_kernel<<<dim3((unsigned)egrid((size_t)p->n_vis_int), (unsigned)p->n_chan), ET, 0, s>>>(P.r, p->rpol, p->n_vis_int, p->done_ptr);
                 Q.r = p->rpol;
                 adj_kernel_c1<SL1M_ADJ_C1_NPQ, B><<<grid, NT, 0, s>>>(Q);
 #endif
@@ -595,7 +622,7 @@ void launch_fwd(sl1m_plan *p, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->fwd_per_split;
     dim3 grid(p->fwd_vtiles, p->fwd_split, p->n_chan);
-    if (p->phase64 && p->n_chan == 1) {
+    if (p->phase64) {
         switch (p->fwd_rv) {
             case 4: fwd_kernel_p64<4><<<grid, NT, 0, s>>>(P, p->pixd); break;
             case 2: fwd_kernel_p64<2><<<grid, NT, 0, s>>>(P, p->pixd); break;
@@ -628,7 +655,7 @@ void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
     P.per_split = p->adj_per_split;
     P.r = r;
     dim3 grid(p->adj_pgroups, p->adj_split, p->n_chan);
-    if (p->phase64 && p->n_chan == 1) {
+    if (p->phase64) {
         switch (p->adj_rp) {
             case 4: adj_kernel_p64<4><<<grid, NT, 0, s>>>(P, p->pixd); break;
             case 2: adj_kernel_p64<2><<<grid, NT, 0, s>>>(P, p->pixd); break;
@@ -773,12 +800,133 @@ extern "C" int sl1m_max_eig_batch(sl1m_plan *p, int n_pow, float *L_out_host, vo
 // a3-a6: FISTA, listing PAPER.md:188-192; no host round-trip per iteration
 // ------------------------------------------------------------------------------------------
 namespace {
-// Shared body of sl1m_solve (tol < 0: fixed iteration count) and sl1m_solve_tol.
+struct StopOpts {
+    double tol, nnz_tol;   // < 0: that rule is off
+    int check_every;
+};
+
+// y_1 = I_0 = x0 (or 0), t_1 = 1.  lambda_c, L_c: HOST [n_chan], L_c > 0.  vis_dev is BORROWED until the next begin.
+int fista_begin_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const float *L_c, const float *x0_dev,
+                     cudaStream_t s) {
+    const int C = p->n_chan, npad = p->n_pix_pad;
+    p->f_active = false;
+    p->f_lam.assign(lambda_c, lambda_c + C);
+    p->f_L.assign(L_c, L_c + C);
+    p->f_inv_L = (float)(1.0 / (double)L_c[0]);
+    p->f_thr = (float)((double)lambda_c[0] / (double)L_c[0]);
+    {   // per-channel (1/L_c, lambda_c/L_c) and 2 lambda_c on the device
+        std::vector<float2> h((size_t)C);
+        std::vector<double> l2((size_t)C);
+        for (int c = 0; c < C; ++c) {
+            h[c] = make_float2((float)(1.0 / (double)L_c[c]), (float)((double)lambda_c[c] / (double)L_c[c]));
+            l2[c] = 2.0 * (double)lambda_c[c];
+        }
+        if (!p->lam2) CUDA_TRY(cudaMalloc((void **)&p->lam2, (size_t)C * sizeof(double)));
+        if (!p->ctl_i) CUDA_TRY(cudaMalloc((void **)&p->ctl_i, (2 * (size_t)C + 1) * sizeof(int)));
+        CUDA_TRY(cudaMemcpyAsync(p->lam2, l2.data(), (size_t)C * sizeof(double), cudaMemcpyHostToDevice, s));
+        if (C > 1) CUDA_TRY(cudaMemcpyAsync(p->step_c, h.data(), (size_t)C * sizeof(float2), cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaMemsetAsync(p->ctl_i, 0, (2 * (size_t)C + 1) * sizeof(int), s));
+        CUDA_TRY(cudaStreamSynchronize(s));   // h, l2 are stack-lifetime staging buffers
+    }
+    if (x0_dev) {
+        gather_kernel<<<cgrid(p, npad), ET, 0, s>>>(x0_dev, p->perm, p->I_sorted, npad, (int)p->n_pix);
+        p->launches++;
+    } else {
+        CUDA_TRY(cudaMemsetAsync(p->I_sorted, 0, (size_t)C * npad * sizeof(float), s));
+    }
+    CUDA_TRY(cudaMemcpyAsync(p->y_sorted, p->I_sorted, (size_t)C * npad * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, npad, zs_of(p));
+    p->launches++;
+    p->f_vis = (const float2 *)vis_dev;
+    p->f_t = 1.0;
+    p->f_k = 0;
+    p->done_ptr = nullptr;
+    p->f_active = true;
+    return check_launch("sl1m_fista_begin");
+}
+
+// n_iter more iterations of the listing from the plan's state (I_k, y_{k+1}, t_{k+1}).  trace_dev (nullable):
+// DEV [n_chan][trace_stride doubles]; iteration i of THIS call writes row trace_row0 + i.  stop (nullable): the
+// termination rules, decided on the device (stop_rule_kernel) from trace rows k-1, k-2 counted from the state's
+// begin -- the caller's trace must then hold every iteration since begin (trace_row0 == p->f_k).
+// The host never waits for an iteration: it reads the all-done flag two polls behind what it has enqueued.
+int fista_iterate(sl1m_plan *p, int n_iter, double *trace_dev, size_t trace_stride, int trace_row0,
+                  const StopOpts *stop, cudaStream_t s) {
+    const int C = p->n_chan, npad = p->n_pix_pad;
+    const float2 *step_c = C > 1 ? p->step_c : nullptr;
+    const int *done = stop ? p->ctl_i : nullptr;
+    p->done_ptr = done;
+    int pending[2] = {0, 0}, slot = 0, looks = 0;
+    // How far the host may run ahead of the device's decision.  Small problems (an iteration is tens of
+    // microseconds): read the flag every >= 16 iterations, two polls behind -- the iterations enqueued past the stop
+    // return at once in the O(N) kernels and in every kernel of a batched plan; the main kernels of a
+    // single-channel plan carry no flag test (it cost the packed forward 7 %: 157 -> 168 ms at config 5) and run
+    // to no effect.  Large problems (an iteration is milliseconds): wait for every look -- a 10 us round-trip
+    // against an iteration that costs a thousand times more.
+    const bool big = 2.0 * (double)p->n_pix_pad * (double)p->n_vis_int >= 5e8;
+    const int looks_per_poll = !stop ? 0 : (big ? 1 : std::max(1, 16 / std::max(1, stop->check_every)));
+    if (stop && !p->h_flag) {
+        CUDA_TRY(cudaMallocHost((void **)&p->h_flag, 2 * sizeof(int)));
+        CUDA_TRY(cudaEventCreateWithFlags(&p->poll_ev[0], cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&p->poll_ev[1], cudaEventDisableTiming));
+    }
+    for (int i = 0; i < n_iter; ++i) {
+        const double t = p->f_t, t_next = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
+        const float beta = (float)((t - 1.0) / t_next);
+        double *tr = trace_dev ? trace_dev + 3 * (size_t)(trace_row0 + i) : nullptr;
+        launch_fwd(p, s);
+        fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, p->f_vis,
+                                                                p->resid, 1, tr ? p->part_a : nullptr, (int)p->n_vis,
+                                                                p->n_part, done);
+        launch_adj(p, p->resid, s);
+        fista_update_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->pix4, p->I_sorted,
+                                                          p->y_sorted, p->f_inv_L, p->f_thr, beta,
+                                                          tr ? p->part_b : nullptr, tr ? p->part_c : nullptr, step_c,
+                                                          p->n_part, zs_of(p), done);
+        p->launches += 2;
+        if (tr) {
+            sum_partials_kernel<<<C, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
+                                                 egrid(npad), tr, tr + 1, tr + 2, p->n_part, trace_stride, done);
+            p->launches++;
+        }
+        p->f_t = t_next;
+        p->f_k++;
+        if (stop && p->f_k >= 2 && p->f_k % stop->check_every == 0) {
+            stop_rule_kernel<<<1, ET, 0, s>>>(trace_dev, trace_stride, p->f_k, C, p->lam2, stop->tol, stop->nnz_tol, p->ctl_i);
+            p->launches++;
+            if (++looks % looks_per_poll == 0) {
+                if (pending[slot]) {                       // the poll issued two polls ago
+                    CUDA_TRY(cudaEventSynchronize(p->poll_ev[slot]));
+                    if (p->h_flag[slot]) break;
+                }
+                CUDA_TRY(cudaMemcpyAsync(&p->h_flag[slot], p->ctl_i + 2 * C, sizeof(int), cudaMemcpyDeviceToHost, s));
+                CUDA_TRY(cudaEventRecord(p->poll_ev[slot], s));
+                pending[slot] = 1;
+                if (big) {                                 // wait for this look's decision before enqueueing more
+                    CUDA_TRY(cudaEventSynchronize(p->poll_ev[slot]));
+                    if (p->h_flag[slot]) break;
+                    pending[slot] = 0;
+                }
+                slot ^= 1;
+            }
+        }
+    }
+    p->done_ptr = nullptr;
+    return check_launch("sl1m_fista_step");
+}
+
+int fista_image_impl(sl1m_plan *p, float *x_out_dev, cudaStream_t s) {
+    scatter_kernel<<<cgrid(p, p->n_pix_pad), ET, 0, s>>>(p->I_sorted, p->perm, x_out_dev, p->n_pix_pad, (int)p->n_pix);
+    p->launches++;
+    return check_launch("sl1m_fista_image");
+}
+
+// Shared body of sl1m_solve / sl1m_solve_batch (stop == NULL: fixed iteration count) and sl1m_solve_stop(_batch).
 int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const float *L_c_in, int n_pow,
-               int n_iter, double tol, int check_every, const float *x0_dev, float *x_out_dev, double *trace_dev,
+               int n_iter, const StopOpts *stop, const float *x0_dev, float *x_out_dev, double *trace_dev,
                sl1m_solve_info *info_host, void *stream) {
     // lambda_c, L_c_in: HOST [n_chan]; vis/x0/x_out: DEV [n_chan][.]; trace: DEV [n_chan][n_iter][3];
-    // info_host: HOST [n_chan].  tol >= 0 (single channel only) enables the stopping rule.
+    // info_host: HOST [n_chan].
     if (!p || !vis_dev || !x_out_dev || !lambda_c || !L_c_in) return fail(SL1M_ERR_NULL, "sl1m_solve: NULL argument");
     if (n_iter < 0) return fail(SL1M_ERR_PARAM, "n_iter < 0");
     const int C = p->n_chan;
@@ -792,13 +940,14 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
     cudaStream_t s = (cudaStream_t)stream;
     const int npad = p->n_pix_pad;
     int st;
-    if (tol >= 0.0 && !trace_dev) {   // the stopping rule reads the trace: use the plan's own buffer
-        if (p->trace_cap < n_iter) {
+    const size_t trace_stride = 3 * (size_t)std::max(n_iter, 1);   // doubles per channel in trace_dev
+    if (stop && !trace_dev) {   // the stopping rule reads the trace: use the plan's own buffer
+        if (p->trace_cap < (size_t)C * trace_stride) {
             if (p->trace_buf) cudaFree(p->trace_buf);
             p->trace_buf = nullptr;
             p->trace_cap = 0;
-            CUDA_TRY(cudaMalloc((void **)&p->trace_buf, (size_t)std::max(n_iter, 1) * 3 * sizeof(double)));
-            p->trace_cap = n_iter;
+            CUDA_TRY(cudaMalloc((void **)&p->trace_buf, (size_t)C * trace_stride * sizeof(double)));
+            p->trace_cap = (size_t)C * trace_stride;
         }
         trace_dev = p->trace_buf;
     }
@@ -810,67 +959,10 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
             if (!(L_c[c] > 0.f)) return fail(SL1M_ERR_PARAM, "power iteration returned L <= 0 (zero operator)");
         }
     }
-    const float inv_L = (float)(1.0 / (double)L_c[0]);
-    const float thr = (float)((double)lambda_c[0] / (double)L_c[0]);
-    const float2 *step_c = nullptr;
-    if (C > 1) {                      // per-channel (1/L_c, lambda_c/L_c) on the device
-        std::vector<float2> h((size_t)C);
-        for (int c = 0; c < C; ++c)
-            h[c] = make_float2((float)(1.0 / (double)L_c[c]), (float)((double)lambda_c[c] / (double)L_c[c]));
-        CUDA_TRY(cudaMemcpyAsync(p->step_c, h.data(), (size_t)C * sizeof(float2), cudaMemcpyHostToDevice, s));
-        CUDA_TRY(cudaStreamSynchronize(s));   // h is a stack-lifetime staging buffer
-        step_c = p->step_c;
-    }
-    const size_t trace_stride = 3 * (size_t)std::max(n_iter, 1);   // doubles per channel in trace_dev
-
-    // y_1 = I_0 = x0 (or 0), in sorted order; a*y_1 packed into the pixel tiles
-    if (x0_dev) {
-        gather_kernel<<<cgrid(p, npad), ET, 0, s>>>(x0_dev, p->perm, p->I_sorted, npad, (int)p->n_pix);
-        p->launches++;
-    } else {
-        CUDA_TRY(cudaMemsetAsync(p->I_sorted, 0, (size_t)C * npad * sizeof(float), s));
-    }
-    CUDA_TRY(cudaMemcpyAsync(p->y_sorted, p->I_sorted, (size_t)C * npad * sizeof(float), cudaMemcpyDeviceToDevice, s));
-    pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, npad, zs_of(p));
-    p->launches++;
-
-    double t = 1.0;
-    int n_done = 0;
-    for (int k = 0; k < n_iter; ++k) {
-        const double t_next = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
-        const float beta = (float)((t - 1.0) / t_next);
-        t = t_next;
-        launch_fwd(p, s);
-        fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm,
-                                                                (const float2 *)vis_dev, p->resid, 1,
-                                                                trace_dev ? p->part_a : nullptr, (int)p->n_vis, p->n_part);
-        launch_adj(p, p->resid, s);
-        fista_update_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->ws_p, p->adj_split, npad, p->amp, p->pix4, p->I_sorted,
-                                                          p->y_sorted, inv_L, thr, beta,
-                                                          trace_dev ? p->part_b : nullptr,
-                                                          trace_dev ? p->part_c : nullptr, step_c, p->n_part, zs_of(p));
-        p->launches += 2;
-        if (trace_dev) {
-            sum_partials_kernel<<<C, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
-                                                 egrid(npad), trace_dev + 3 * (size_t)k, trace_dev + 3 * (size_t)k + 1,
-                                                 trace_dev + 3 * (size_t)k + 2, p->n_part, trace_stride);
-            p->launches++;
-        }
-        n_done = k + 1;
-        // termination rule (reading R21), looked at every check_every
-        // iterations: the only host round-trip of the loop, 48 bytes.
-        if (tol >= 0.0 && n_done >= 2 && check_every >= 1 && n_done % check_every == 0) {
-            double h[6];
-            CUDA_TRY(cudaMemcpyAsync(h, trace_dev + 3 * (size_t)(n_done - 2), sizeof(h), cudaMemcpyDeviceToHost, s));
-            CUDA_TRY(cudaStreamSynchronize(s));
-            const double E_before = h[0] + 2.0 * (double)lambda_c[0] * h[1];
-            const double E_now = h[3] + 2.0 * (double)lambda_c[0] * h[4];
-            if (std::fabs(E_now - E_before) <= tol * std::fabs(E_now)) break;
-        }
-    }
-    scatter_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->I_sorted, p->perm, x_out_dev, npad, (int)p->n_pix);
-    p->launches++;
-    if ((st = check_launch("sl1m_solve"))) return st;
+    if ((st = fista_begin_impl(p, vis_dev, lambda_c, L_c.data(), x0_dev, s))) return st;
+    if ((st = fista_iterate(p, n_iter, trace_dev, trace_stride, 0, stop, s))) return st;
+    const int n_enqueued = p->f_k;
+    if ((st = fista_image_impl(p, x_out_dev, s))) return st;
 
     if (info_host) {
         // one extra forward for ||M I_K - V||^2 (Table 1's L2 term)
@@ -883,12 +975,15 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
         sum_partials_kernel<<<C, ET, 0, s>>>(p->part_a, p->part_b, p->part_c, egrid(p->n_vis_int), egrid(npad),
                                              egrid(npad), p->scalars + 1, p->scalars + 2, p->scalars + 3, p->n_part, 4);
         p->launches += 4;
+        p->f_active = false;               // the pixel tiles now hold a*I_K, not a*y_{K+1}: the state cannot be stepped on
         if ((st = check_launch("sl1m_solve(info)"))) return st;
         std::vector<double> h(4 * (size_t)C);
+        std::vector<int> ctl(2 * (size_t)C + 1, 0);
         CUDA_TRY(cudaMemcpyAsync(h.data(), p->scalars, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
+        if (stop) CUDA_TRY(cudaMemcpyAsync(ctl.data(), p->ctl_i, ctl.size() * sizeof(int), cudaMemcpyDeviceToHost, s));
         CUDA_TRY(cudaStreamSynchronize(s));
         for (int c = 0; c < C; ++c) {
-            info_host[c].n_iter_done = n_done;
+            info_host[c].n_iter_done = (stop && ctl[c]) ? ctl[(size_t)C + c] : n_enqueued;
             info_host[c].L_used = L_c[c];
             info_host[c].l2_term = h[4 * c + 1];
             info_host[c].l1_term = h[4 * c + 2];
@@ -903,8 +998,17 @@ extern "C" int sl1m_solve(sl1m_plan *p, const float *vis_dev, float lambda, floa
                           const float *x0_dev, float *x_out_dev, double *trace_dev, sl1m_solve_info *info_host,
                           void *stream) {
     if (int st = single_channel_only(p, "sl1m_solve")) return st;
-    return solve_impl(p, vis_dev, &lambda, &L, n_pow, n_iter, -1.0, 1, x0_dev, x_out_dev, trace_dev, info_host, stream);
+    return solve_impl(p, vis_dev, &lambda, &L, n_pow, n_iter, nullptr, x0_dev, x_out_dev, trace_dev, info_host, stream);
 }
+
+namespace {
+int check_stop_args(double tol, double nnz_tol, int check_every, const void *info_host, const char *what) {
+    if (tol != tol || nnz_tol != nnz_tol || (tol < 0.0 && nnz_tol < 0.0) || check_every < 1)
+        return fail(SL1M_ERR_PARAM, std::string(what) + ": no stopping rule enabled (tol < 0 and nnz_tol < 0) or check_every < 1");
+    if (!info_host) return fail(SL1M_ERR_NULL, std::string(what) + ": info_host is required (it carries n_iter_done)");
+    return SL1M_OK;
+}
+}  // namespace
 
 extern "C" int sl1m_solve_tol(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int max_iter,
                               double tol, int check_every, const float *x0_dev, float *x_out_dev,
@@ -912,15 +1016,58 @@ extern "C" int sl1m_solve_tol(sl1m_plan *p, const float *vis_dev, float lambda, 
     if (int st = single_channel_only(p, "sl1m_solve_tol")) return st;
     if (!(tol >= 0.0) || check_every < 1) return fail(SL1M_ERR_PARAM, "sl1m_solve_tol: tol < 0 or check_every < 1");
     if (!info_host) return fail(SL1M_ERR_NULL, "sl1m_solve_tol: info_host is required (it carries n_iter_done)");
-    return solve_impl(p, vis_dev, &lambda, &L, n_pow, max_iter, tol, check_every, x0_dev, x_out_dev, trace_dev,
-                      info_host, stream);
+    const StopOpts so{tol, -1.0, check_every};
+    return solve_impl(p, vis_dev, &lambda, &L, n_pow, max_iter, &so, x0_dev, x_out_dev, trace_dev, info_host, stream);
+}
+
+extern "C" int sl1m_solve_stop(sl1m_plan *p, const float *vis_dev, float lambda, float L, int n_pow, int max_iter,
+                               double tol, double nnz_tol, int check_every, const float *x0_dev, float *x_out_dev,
+                               double *trace_dev, sl1m_solve_info *info_host, void *stream) {
+    if (int st = single_channel_only(p, "sl1m_solve_stop")) return st;
+    if (int st = check_stop_args(tol, nnz_tol, check_every, info_host, "sl1m_solve_stop")) return st;
+    const StopOpts so{tol, nnz_tol, check_every};
+    return solve_impl(p, vis_dev, &lambda, &L, n_pow, max_iter, &so, x0_dev, x_out_dev, trace_dev, info_host, stream);
+}
+
+extern "C" int sl1m_solve_stop_batch(sl1m_plan *p, const float *vis_dev, const float *lambda_host, const float *L_host,
+                                     int n_pow, int max_iter, double tol, double nnz_tol, int check_every,
+                                     const float *x0_dev, float *x_out_dev, double *trace_dev,
+                                     sl1m_solve_info *info_host, void *stream) {
+    if (int st = check_stop_args(tol, nnz_tol, check_every, info_host, "sl1m_solve_stop_batch")) return st;
+    const StopOpts so{tol, nnz_tol, check_every};
+    return solve_impl(p, vis_dev, lambda_host, L_host, n_pow, max_iter, &so, x0_dev, x_out_dev, trace_dev, info_host,
+                      stream);
 }
 
 extern "C" int sl1m_solve_batch(sl1m_plan *p, const float *vis_dev, const float *lambda_host, const float *L_host,
                                 int n_pow, int n_iter, const float *x0_dev, float *x_out_dev, double *trace_dev,
                                 sl1m_solve_info *info_host, void *stream) {
-    return solve_impl(p, vis_dev, lambda_host, L_host, n_pow, n_iter, -1.0, 1, x0_dev, x_out_dev, trace_dev,
+    return solve_impl(p, vis_dev, lambda_host, L_host, n_pow, n_iter, nullptr, x0_dev, x_out_dev, trace_dev,
                       info_host, stream);
+}
+
+// Stepping API: the same iteration, driven by the caller a few iterations at a time (interactive imaging,
+// bench.py's per-step timing of ONE continuing FISTA run).
+extern "C" int sl1m_fista_begin(sl1m_plan *p, const float *vis_dev, const float *lambda_host, const float *L_host,
+                                const float *x0_dev, void *stream) {
+    if (!p || !vis_dev || !lambda_host || !L_host) return fail(SL1M_ERR_NULL, "sl1m_fista_begin: NULL argument");
+    for (int c = 0; c < p->n_chan; ++c)
+        if (!(lambda_host[c] >= 0.f) || !(L_host[c] > 0.f)) return fail(SL1M_ERR_PARAM, "sl1m_fista_begin: lambda < 0 or L <= 0");
+    return fista_begin_impl(p, vis_dev, lambda_host, L_host, x0_dev, (cudaStream_t)stream);
+}
+
+extern "C" int sl1m_fista_step(sl1m_plan *p, int n_iter, double *trace_dev, void *stream) {
+    if (!p) return fail(SL1M_ERR_NULL, "sl1m_fista_step: NULL plan");
+    if (!p->f_active) return fail(SL1M_ERR_PARAM, "sl1m_fista_step: no FISTA state (call sl1m_fista_begin; a solve that returned info ends the state)");
+    if (n_iter < 0) return fail(SL1M_ERR_PARAM, "n_iter < 0");
+    return fista_iterate(p, n_iter, trace_dev, 3 * (size_t)std::max(n_iter, 1), 0, nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int sl1m_fista_image(sl1m_plan *p, float *x_out_dev, int32_t *n_iter_done_host, void *stream) {
+    if (!p || !x_out_dev) return fail(SL1M_ERR_NULL, "sl1m_fista_image: NULL argument");
+    if (!p->f_active) return fail(SL1M_ERR_PARAM, "sl1m_fista_image: no FISTA state");
+    if (n_iter_done_host) *n_iter_done_host = p->f_k;
+    return fista_image_impl(p, x_out_dev, (cudaStream_t)stream);
 }
 
 // NEXT-4: turn the plan into a batch of n_chan channels that share pixels, gains and baseline
@@ -928,46 +1075,64 @@ extern "C" int sl1m_solve_batch(sl1m_plan *p, const float *vis_dev, const float 
 extern "C" int sl1m_plan_set_channels(sl1m_plan *p, int32_t n_chan, const double *scale_host) {
     if (!p || !scale_host) return fail(SL1M_ERR_NULL, "sl1m_plan_set_channels: NULL argument");
     if (n_chan < 1 || n_chan > 65535) return fail(SL1M_ERR_SIZE, "n_chan must be in [1, 65535]");
-    for (int c = 0; c < n_chan; ++c)
+    double scale_max = 0.0;
+    for (int c = 0; c < n_chan; ++c) {
         if (!std::isfinite(scale_host[c]) || !(scale_host[c] > 0.0))
             return fail(SL1M_ERR_DOMAIN, "channel scale must be finite and > 0");
+        scale_max = std::max(scale_max, scale_host[c]);
+    }
     const size_t npad = (size_t)p->n_pix_pad;
-    // replicate the pixel tiles: channel c keeps its own a*x in pix4[c][.].w
-    float4 *pix_new = nullptr;
-    CUDA_TRY(cudaMalloc((void **)&pix_new, (size_t)n_chan * npad * sizeof(float4)));
-    for (int c = 0; c < n_chan; ++c) {
-        cudaError_t e = cudaMemcpy(pix_new + (size_t)c * npad, p->pix4, npad * sizeof(float4), cudaMemcpyDeviceToDevice);
-        if (e != cudaSuccess) { cudaFree(pix_new); return fail(SL1M_ERR_CUDA, cudaGetErrorString(e)); }
-    }
-    cudaFree(p->pix4);
-    p->pix4 = pix_new;
-    if (p->chan_scale) cudaFree(p->chan_scale);
-    if (p->step_c) cudaFree(p->step_c);
-    p->chan_scale = nullptr;
-    p->step_c = nullptr;
-    CUDA_TRY(cudaMalloc((void **)&p->chan_scale, (size_t)n_chan * sizeof(double)));
-    CUDA_TRY(cudaMemcpy(p->chan_scale, scale_host, (size_t)n_chan * sizeof(double), cudaMemcpyHostToDevice));
-    CUDA_TRY(cudaMalloc((void **)&p->step_c, (size_t)n_chan * sizeof(float2)));
+    // Transactional: every buffer whose size depends on n_chan is allocated afresh next to the old one; the plan
+    // switches over only when all of them exist, so a failure (out of memory) leaves it exactly as it was.
+    sl1m_plan saved = *p;
+    auto fields = [](sl1m_plan *q) {
+        return std::vector<void **>{(void **)&q->ws_v, (void **)&q->ws_p, (void **)&q->resid, (void **)&q->rpol,
+                                    (void **)&q->I_sorted, (void **)&q->y_sorted, (void **)&q->g_sorted,
+                                    (void **)&q->part_a, (void **)&q->part_b, (void **)&q->part_c, (void **)&q->scalars,
+                                    (void **)&q->pixc, (void **)&q->tile_cnt, (void **)&q->gFc, (void **)&q->pixdc,
+                                    (void **)&q->pixgc, (void **)&q->pix4,
+                                    (void **)&q->chan_scale, (void **)&q->step_c, (void **)&q->h_x, (void **)&q->h_vis,
+                                    (void **)&q->h_img, (void **)&q->ctl_i, (void **)&q->lam2, (void **)&q->trace_buf};
+    };
+    for (void **q : fields(p)) *q = nullptr;
+    p->trace_cap = 0;
+    p->f_active = false;
     p->n_chan = n_chan;
-    for (void **q : {(void **)&p->h_x, (void **)&p->h_vis, (void **)&p->h_img}) {   // single-channel staging
+    // the fp32 phase remainder grows with the channel's frequency: re-evaluate the fp64-phase decision
+    p->phase64 = p->phase64_capable && (p->phase64_flag || p->phase_span * scale_max > 256.0);
+    auto attempt = [&]() -> int {
+        // replicate the pixel tiles: channel c keeps its own a*x in pix4[c][.].w
+        CUDA_TRY(cudaMalloc((void **)&p->pix4, (size_t)n_chan * npad * sizeof(float4)));
+        for (int c = 0; c < n_chan; ++c)
+            CUDA_TRY(cudaMemcpy(p->pix4 + (size_t)c * npad, saved.pix4, npad * sizeof(float4), cudaMemcpyDeviceToDevice));
+        CUDA_TRY(cudaMalloc((void **)&p->chan_scale, (size_t)n_chan * sizeof(double)));
+        CUDA_TRY(cudaMemcpy(p->chan_scale, scale_host, (size_t)n_chan * sizeof(double), cudaMemcpyHostToDevice));
+        CUDA_TRY(cudaMalloc((void **)&p->step_c, (size_t)n_chan * sizeof(float2)));
+        if (int st = configure_and_allocate(p)) return st;
+        CUDA_TRY(cudaDeviceSynchronize());
+        return SL1M_OK;
+    };
+    const int st = attempt();
+    sl1m_plan *loser = st ? p : &saved;       // free the new buffers on failure, the old ones on success
+    for (void **q : fields(loser))
         if (*q) cudaFree(*q);
-        *q = nullptr;
+    if (st) {
+        const int64_t launches = p->launches;
+        *p = saved;
+        p->launches = launches;
     }
-    int st = configure_and_allocate(p);
-    if (st) return st;
-    CUDA_TRY(cudaDeviceSynchronize());
-    return SL1M_OK;
+    return st;
 }
 
 extern "C" int32_t sl1m_plan_n_chan(const sl1m_plan *p) { return p ? p->n_chan : 0; }
 
 extern "C" int sl1m_dirty_image(sl1m_plan *p, const float *vis_dev, float scale, float *img_dev, void *stream) {
     if (!p || !vis_dev || !img_dev) return fail(SL1M_ERR_NULL, "sl1m_dirty_image: NULL argument");
-    if (int stc = single_channel_only(p, "sl1m_dirty_image")) return stc;
     if (!std::isfinite(scale)) return fail(SL1M_ERR_PARAM, "sl1m_dirty_image: non-finite scale");
     int st = sl1m_adjoint(p, vis_dev, img_dev, stream);
     if (st) return st;
-    scale_clip_kernel<<<egrid((size_t)p->n_pix), ET, 0, (cudaStream_t)stream>>>(img_dev, scale, (int)p->n_pix);
+    const size_t n_all = (size_t)p->n_chan * (size_t)p->n_pix;      // [n_chan][n_pix] is contiguous
+    scale_clip_kernel<<<egrid(n_all), ET, 0, (cudaStream_t)stream>>>(img_dev, scale, n_all);
     p->launches++;
     return check_launch("sl1m_dirty_image");
 }
@@ -1020,11 +1185,11 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
                               : (grouped && p->adj_rp == 8 ? SL1M_ADJ_G2_NPQ : 0);
     o->mufu_per_term_mufu_path = p->pk == 2 ? 3 : (pk ? 4 : 2);
     o->gaussian = p->pk;
-    o->phase_fp64 = p->phase64 && p->n_chan == 1;
+    o->phase_fp64 = p->phase64;
     o->phase_span_rad = (float)p->phase_span;
     o->zero_skip = p->pixc != nullptr;
     o->adj_mufu_per_term = o->mufu_per_term_mufu_path;
-    if (!(p->phase64 && p->n_chan == 1)) {
+    if (!p->phase64) {
         if (p->pk == 0) o->adj_mufu_per_term = 1;    // delta pixels: one cosine per term in every adjoint kernel
 #ifdef SL1M_ADJ_TWO_MUFU
         if (p->pk == 0 && p->gk == 0 && p->adj_rp == 8) o->adj_mufu_per_term = 2;   // adj_kernel_x2 (A/B build)

@@ -143,7 +143,9 @@ __global__ void __launch_bounds__(ET) fill_kernel(float *p, float v, const int *
 // part[block] = sum |value|^2 (fp64).
 __global__ void __launch_bounds__(ET) fwd_reduce_kernel(const float2 *ws, int n_split, int n_int,
                                                         const int *vperm, const float2 *V, float2 *out,
-                                                        int out_internal, double *part, int n_vis, int n_part) {
+                                                        int out_internal, double *part, int n_vis, int n_part,
+                                                        const int *done = nullptr) {
+    if (done && done[blockIdx.y]) return;                // channel stopped (sl1m_solve_stop)
     const int js = blockIdx.x * ET + threadIdx.x;
     double sq = 0.0;
     ws += (size_t)blockIdx.y * n_split * n_int;          // blockIdx.y = channel
@@ -188,7 +190,9 @@ __global__ void __launch_bounds__(ET) vis_gather_kernel(const float2 *caller, co
 
 // Residual in polar form for the one-cosine adjoint kernels: rp[j] = (|r_j|, arg r_j), evaluated in fp64.
 // Re(e^{iX} r) = |r| cos(X + arg r) (the image is real, reading C3).
-__global__ void __launch_bounds__(ET) vis_polar_kernel(const float2 *r, float2 *rp, int n_int) {
+__global__ void __launch_bounds__(ET) vis_polar_kernel(const float2 *r, float2 *rp, int n_int,
+                                                       const int *done = nullptr) {
+    if (done && done[blockIdx.y]) return;
     const int js = blockIdx.x * ET + threadIdx.x;
     if (js >= n_int) return;
     r += (size_t)blockIdx.y * n_int;                     // blockIdx.y = channel
@@ -230,7 +234,9 @@ __global__ void __launch_bounds__(ET) fista_update_kernel(const float *ws, int n
                                                           const float *amp, float4 *pix4, float *I_sorted,
                                                           float *y_sorted, float inv_L, float thr, float beta,
                                                           double *part_l1, double *part_nnz,
-                                                          const float2 *step_c, int n_part, ZeroSkip zs) {
+                                                          const float2 *step_c, int n_part, ZeroSkip zs,
+                                                          const int *done = nullptr) {
+    if (done && done[blockIdx.y]) return;                // channel stopped: I, y and the packed tiles stay as they are
     const int k = blockIdx.x * ET + threadIdx.x;
     double l1 = 0.0, nz = 0.0;
     float4 pv = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -279,7 +285,9 @@ __global__ void __launch_bounds__(ET) fista_update_kernel(const float *ws, int n
 // out[i] = sum of n partials of array i, i < n_arrays (single CTA, fixed order).
 __global__ void __launch_bounds__(ET) sum_partials_kernel(const double *p0, const double *p1, const double *p2,
                                                           int n0, int n1, int n2, double *out0, double *out1,
-                                                          double *out2, int n_part, size_t out_stride) {
+                                                          double *out2, int n_part, size_t out_stride,
+                                                          const int *done = nullptr) {
+    if (done && done[blockIdx.x]) return;
     const double *ps[3] = {p0, p1, p2};
     const int ns[3] = {n0, n1, n2};
     double *outs[3] = {out0, out1, out2};
@@ -291,6 +299,34 @@ __global__ void __launch_bounds__(ET) sum_partials_kernel(const double *p0, cons
         const double t = block_sum(v);
         if (threadIdx.x == 0) outs[a][c * out_stride] = t;
     }
+}
+
+// Termination rules of PAPER.md:194 evaluated ON THE DEVICE after iteration k (1-based; k >= 2), from the trace rows
+// the iteration has just written (readings R21, R24):
+//   E rule    |E_k - E_{k-1}| <= tol |E_k|,   E_k = ||M y_k - V||^2 + 2 lambda sum I_k        (tol < 0: off)
+//   nnz rule  |N_k - N_{k-1}| <= nnz_tol N_k, N_k = nnz(I_k)                                 (nnz_tol < 0: off)
+// A channel that meets either enabled rule gets done[c] = 1, n_done[c] = k; every later kernel of that channel
+// returns at once.  ctl = {done[C], n_done[C], all_done}.  One CTA; channels strided over its threads.
+__global__ void __launch_bounds__(ET) stop_rule_kernel(const double *trace, size_t trace_stride, int k, int n_chan,
+                                                       const double *lam2, double tol, double nnz_tol, int *ctl) {
+    int *done = ctl, *n_done = ctl + n_chan, *all_done = ctl + 2 * n_chan;
+    int mine = 1;
+    for (int c = threadIdx.x; c < n_chan; c += ET) {
+        if (!done[c]) {
+            const double *now = trace + c * trace_stride + 3 * (size_t)(k - 1), *bef = now - 3;
+            const double E_now = now[0] + lam2[c] * now[1], E_bef = bef[0] + lam2[c] * bef[1];
+            const bool stop = (tol >= 0.0 && fabs(E_now - E_bef) <= tol * fabs(E_now)) ||
+                              (nnz_tol >= 0.0 && fabs(now[2] - bef[2]) <= nnz_tol * now[2]);
+            if (stop) {
+                done[c] = 1;
+                n_done[c] = k;
+            } else {
+                mine = 0;
+            }
+        }
+    }
+    const int all = __syncthreads_and(mine);
+    if (threadIdx.x == 0) *all_done = all;
 }
 
 // Power iteration (a7): x = g / ||g||, packed straight into the pixel tiles; norm2 on device.
@@ -315,19 +351,20 @@ __global__ void __launch_bounds__(ET) gains_layout_kernel(const float2 *raw, int
                                                           int n_pix_pad, const int *perm, float2 *gF,
                                                           float2 *gA) {
     const int k = blockIdx.x * ET + threadIdx.x;
-    const int a = blockIdx.y;
     if (k >= n_pix_pad) return;
     const int src = perm[k];
     // polar form (|g|, arg g), evaluated in fp64: the kernels multiply the entry by |g_p||g_q| and shift its
     // phase by arg_p - arg_q (G = g_p conj(g_q)); a zero gain has amplitude 0 and phase 0
-    float2 g = make_float2(0.f, 0.f);
-    if (src >= 0) {
-        const float2 c = raw[(size_t)a * n_pix + src];
-        const double re = (double)c.x, im = (double)c.y;
-        g = make_float2((float)sqrt(re * re + im * im), (float)atan2(im, re));
+    for (int a = 0; a < n_ant; ++a) {
+        float2 g = make_float2(0.f, 0.f);
+        if (src >= 0) {
+            const float2 c = raw[(size_t)a * n_pix + src];
+            const double re = (double)c.x, im = (double)c.y;
+            g = make_float2((float)sqrt(re * re + im * im), (float)atan2(im, re));
+        }
+        gF[(size_t)k * n_ant + a] = g;
+        gA[(size_t)a * n_pix_pad + k] = g;
     }
-    gF[(size_t)k * n_ant + a] = g;
-    gA[(size_t)a * n_pix_pad + k] = g;
 }
 
 // Block partials of sum I and nnz I over a sorted image (for the final info struct).
@@ -347,8 +384,8 @@ __global__ void __launch_bounds__(ET) l1_nnz_kernel(const float *I_sorted, int n
 }
 
 // Dirty image as a starting point (reading R22): img = max(0, scale * img).
-__global__ void __launch_bounds__(ET) scale_clip_kernel(float *img, float scale, int n) {
-    const int k = blockIdx.x * ET + threadIdx.x;
+__global__ void __launch_bounds__(ET) scale_clip_kernel(float *img, float scale, size_t n) {
+    const size_t k = (size_t)blockIdx.x * ET + threadIdx.x;
     if (k < n) img[k] = fmaxf(0.f, scale * img[k]);
 }
 

@@ -70,6 +70,10 @@ struct ApplyParams {
     // pix4[c][.].w, its own residual r[c][.] and its own partials.  chan_scale == NULL: one channel.
     const double *chan_scale;       // [n_chan] or NULL
     size_t ws_v_stride, ws_p_stride;   // elements per channel of ws_v / ws_p
+    // device-side termination (sl1m_solve_stop): done[c] != 0 once channel c has met its stopping rule; every
+    // kernel of the iteration then returns at once for that channel, so the iterations the host had already
+    // enqueued cost a few microseconds and the image stays the one of the stopping iteration.  NULL = never.
+    const int *done;                // [n_chan] or NULL
 };
 
 // BATCH is a compile-time switch: the single-channel instantiations carry no channel arithmetic at
@@ -374,6 +378,7 @@ struct PolySplit {
 // ------------------------------------------------------------------------------------------
 template <int RV, int PK, int GK, bool BATCH = false>
 __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : (GK == 2 ? 4 : (PK == 2 ? SL1M_FWD_GT_MIN_CTAS : 1))) fwd_kernel(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(128) float2 s_pixg[PK == 1 ? 2 : 1][PK == 1 ? TP : 1];
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -532,6 +537,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
 // ------------------------------------------------------------------------------------------
 template <int NPQ, bool BATCH = false, bool GAINS = false>
 __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     constexpr int RV = 8, NPAIR = 4;
     // NPQ of the 16 pairs of 4 consecutive pixels take the polynomial path: pixel q gets (NPQ + 3 - q) / 4
     __shared__ __align__(128) float4 s_pix[2][TP];
@@ -714,6 +720,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
 // ------------------------------------------------------------------------------------------
 template <int RP, int PK, int GK, bool BATCH = false>
 __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS : (GK == 2 ? 4 : (PK == 2 ? SL1M_ADJ_GT_MIN_CTAS : 1))) adj_kernel(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
     __shared__ __align__(16) float4 s_vis[2][VC];        // (u', v', w', w)
     __shared__ __align__(8) float2 s_r[2][VC];           // residual (re, im)
@@ -925,6 +932,7 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
 // ------------------------------------------------------------------------------------------
 template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
     __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre)
     __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, -r_im)
@@ -1048,6 +1056,7 @@ __device__ __forceinline__ void cos_poly2(f32x2 X, f32x2 &c, uint32_t &k_lo, uin
 }
 template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_C1_MIN_CTAS) adj_kernel_c1(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
     __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre + arg r)
     __shared__ float s_R[2][VC];                          // |r|
@@ -1146,6 +1155,7 @@ __global__ void __launch_bounds__(NT, SL1M_ADJ_C1_MIN_CTAS) adj_kernel_c1(const 
 #endif
 template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_G2X2_MIN_CTAS) adj_kernel_g2x2(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP, NG = VC / 8;
     // Gains are stored in polar form (|g|, arg g).  With G = |G| e^{i gamma} (|G| = |g_p||g_q|, gamma = arg_p - arg_q):
     //     Re conj(M_jk) r_j = a |G| Re( e^{i (X_rel - gamma)} r_j e^{i x0(j, centre)} ) = a |G| |r_j| cos(X_rel - gamma + phi'),
@@ -1312,6 +1322,7 @@ __device__ __forceinline__ f32x2 ex2_2(f32x2 E) {
 
 template <bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_FWD_GTX2_MIN_CTAS) fwd_kernel_gtx2(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     constexpr int RV = 8, NPAIR = 4;
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -1440,6 +1451,7 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_GTX2_MIN_CTAS) fwd_kernel_gtx2(co
 
 template <bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_GTX2_MIN_CTAS) adj_kernel_gtx2(const ApplyParams P) {
+    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
     __shared__ __align__(16) float4 s_vis[2][VC];            // (u', v', w', -w)
     __shared__ __align__(16) float4 s_ca[2][NCEN][VC];       // per centre: (x0', uc, vc, cX = -ln2 q)
@@ -1551,6 +1563,7 @@ __device__ __forceinline__ float phase64_to_radians(double turns) {
 
 template <int RV>
 __global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, const double4 *pixd) {
+    if (P.done && P.done[blockIdx.z]) return;   // this channel's solve has met its stopping rule
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(128) double4 s_pixd[2][TP];   // (dl, dm, dn', 0) as doubles
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -1561,12 +1574,15 @@ __global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, con
     const int jlast = P.n_vis - 1;
     double ud[RV], vd[RV], wd[RV];
     float re[RV], im[RV];
+    // batched channels (blockIdx.z): uvw * nu_c/nu_0 in fp64, the channel's own a*x tiles and partials
+    const double sc = P.chan_scale ? P.chan_scale[blockIdx.z] : 1.0;
+    const float4 *pix4 = P.pix4 + (size_t)blockIdx.z * P.n_pix_pad;
 #pragma unroll
     for (int r = 0; r < RV; ++r) {
         const int j = min(jbase + r * NT + tid, jlast);
-        ud[r] = __ldg(P.u64 + j);
-        vd[r] = __ldg(P.v64 + j);
-        wd[r] = __ldg(P.w64 + j);
+        ud[r] = sc * __ldg(P.u64 + j);
+        vd[r] = sc * __ldg(P.v64 + j);
+        wd[r] = sc * __ldg(P.w64 + j);
         re[r] = 0.f;
         im[r] = 0.f;
     }
@@ -1579,7 +1595,7 @@ __global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, con
     __syncthreads();
     auto issue = [&](int t, int st) {
         mbar_expect_tx(&s_bar[st], kBytes);
-        tma_bulk_g2s(&s_pix[st][0], P.pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
         tma_bulk_g2s(&s_pixd[st][0], pixd + (size_t)t * TP, TP * sizeof(double4), &s_bar[st]);
     };
     if (tid == 0) {
@@ -1613,7 +1629,7 @@ __global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, con
         __syncthreads();
         if (tid == 0 && t + 2 < t1) issue(t + 2, st);
     }
-    float2 *out = P.ws_v + (size_t)blockIdx.y * P.n_vis;
+    float2 *out = P.ws_v + (size_t)blockIdx.z * P.ws_v_stride + (size_t)blockIdx.y * P.n_vis;
 #pragma unroll
     for (int r = 0; r < RV; ++r) {
         const int j = jbase + r * NT + tid;
@@ -1623,6 +1639,7 @@ __global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, con
 
 template <int RP>
 __global__ void __launch_bounds__(NT, 3) adj_kernel_p64(const ApplyParams P, const double4 *pixd) {
+    if (P.done && P.done[blockIdx.z]) return;   // this channel's solve has met its stopping rule
     constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
     __shared__ __align__(32) double4 s_vis[2][VC];       // (u, v, w, 0) in wavelengths
     __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, r_im)
@@ -1645,15 +1662,17 @@ __global__ void __launch_bounds__(NT, 3) adj_kernel_p64(const ApplyParams P, con
     const int n_chunks = (P.n_vis + VC - 1) / VC;
     const int c0 = blockIdx.y * P.per_split;
     const int c1 = min(c0 + P.per_split, n_chunks);
+    const double sc = P.chan_scale ? P.chan_scale[blockIdx.z] : 1.0;   // batched channels: uvw * nu_c/nu_0
+    const float2 *rin = P.r + (size_t)blockIdx.z * P.n_vis;
     auto stage = [&](int chunk, int buf) {
         const int j = chunk * VC + tid;
         double u = 0.0, v = 0.0, w = 0.0;
         float2 rr = make_float2(0.f, 0.f);
         if (j < P.n_vis) {
-            u = P.u64[j];
-            v = P.v64[j];
-            w = P.w64[j];
-            rr = P.r[j];
+            u = sc * P.u64[j];
+            v = sc * P.v64[j];
+            w = sc * P.w64[j];
+            rr = rin[j];
         }
         s_vis[buf][tid] = make_double4(u, v, w, 0.0);
         s_r[buf][tid] = rr;
@@ -1684,7 +1703,7 @@ __global__ void __launch_bounds__(NT, 3) adj_kernel_p64(const ApplyParams P, con
         }
         __syncthreads();
     }
-    float *out = P.ws_p + (size_t)blockIdx.y * P.n_pix_pad;
+    float *out = P.ws_p + (size_t)blockIdx.z * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
 #pragma unroll
     for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
 }

@@ -129,8 +129,9 @@ cudaError_t run_probe(int grid, int iters, float *sink, long long *cycles_dev, c
 extern "C" int sl1m_measure_peaks(sl1m_peaks *o, void *stream) {
     if (!o) return SL1M_ERR_NULL;
     memset(o, 0, sizeof(*o));
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    int dev = 0, sms = 0, khz = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev) != cudaSuccess) {
         cudaGetLastError();
         return SL1M_ERR_CUDA;
     }
@@ -143,16 +144,20 @@ extern "C" int sl1m_measure_peaks(sl1m_peaks *o, void *stream) {
     const double thr = (double)grid * 128.0, per_it = 8.0 * iters;   // threads, chain steps per chain per thread
     cudaError_t e = cudaSuccess;
     Timed t;
-    // All CTAs of a probe are resident at once (8 x 128 threads per SM), so a CTA's clock64 span is the SM's span:
-    // results per clock per SM = (instructions of the SM's resident threads) / cycles.
+    // Per-clock figures are quoted at the device's maximum SM clock (cudaDevAttrClockRate; bench.py samples the
+    // actual clock with nvidia-smi beside this): results per clock per SM = rate / (SMs x clock).  clock64 is
+    // recorded too, but on this part it does not tick at the SM clock (measured 1,104 MHz under a 1,965 MHz SM
+    // clock), so it is reported as is and used for nothing.
+    const double clk_hz = (double)khz * 1e3;
     auto per_clk_sm = [&](double instr_per_thread_total, const Timed &tt) {
-        return instr_per_thread_total * 128.0 * ctas_per_sm / tt.cyc;
+        return instr_per_thread_total * thr / (tt.ms * 1e-3) / ((double)sms * clk_hz);
     };
 #define PROBE(NM, NF, NF2, NZ, COS) (e == cudaSuccess && (e = run_probe<NM, NF, NF2, NZ, COS>(grid, iters, sink, cyc, s, t)) == cudaSuccess)
     if (PROBE(4, 0, 0, 0, false)) {
         o->mufu_per_s = 4.0 * per_it * thr / (t.ms * 1e-3);
         o->mufu_per_clk_sm = per_clk_sm(4.0 * per_it, t);
-        o->sm_clock_mhz = t.cyc / (t.ms * 1e-3) * 1e-6;       // cycles of the (fully resident) kernel / its duration
+        o->sm_clock_mhz = clk_hz * 1e-6;
+        o->clock64_mhz = t.cyc / (t.ms * 1e-3) * 1e-6;        // mean clock64 span of a CTA / the event-timed duration
     }
     if (PROBE(4, 0, 0, 0, true)) o->mufu_cos_per_clk_sm = per_clk_sm(4.0 * per_it, t);
     if (PROBE(0, 16, 0, 0, false)) {
@@ -168,7 +173,7 @@ extern "C" int sl1m_measure_peaks(sl1m_peaks *o, void *stream) {
     if (PROBE(4, 0, 12, 4, false)) {
         o->coissue_mufu_per_clk_sm = per_clk_sm(4.0 * per_it, t);
         o->coissue_ffma2_lanes_per_clk_sm = per_clk_sm(24.0 * per_it, t);
-        o->coissue_cycles_per_iter = t.cyc / per_it / ctas_per_sm;         // sub-partition cycles per warp per body (8 warps each)
+        o->coissue_cycles_per_iter = (t.ms * 1e-3) * clk_hz / per_it / ctas_per_sm;   // sub-partition cycles per warp per body (8 warps each)
     }
     // the one-cosine adjoint's mix per pair of terms: 3 FFMA2 + 2 FMUL.RZ + 2 MUFU.COS + 1 FFMA2 -> x2: 8 FFMA2 + 4 RZ + 4 MUFU
     if (PROBE(4, 0, 8, 4, true)) o->coissue_adj_mufu_per_clk_sm = per_clk_sm(4.0 * per_it, t);

@@ -268,6 +268,83 @@ def test_fp64_phase_path(sl):
         plan.close()
 
 
+def test_fp64_phase_path_with_channels(sl):
+    """sl1m_plan_set_channels on fp64-phase plans: the channel scale multiplies uvw inside the
+    fp64-phase kernels; a plan just under the 256 rad limit switches to them when its highest channel exceeds
+    it; batches of fp64-phase channels match the oracle on uvw * scale[c]."""
+    import torch
+    rng = np.random.default_rng(15)
+    wl = make_workload(1)
+    uvw = wl.uvw * 30.0
+    uvw[:, 2] = 200.0 * rng.uniform(-1, 1, wl.n_vis)
+    x = rng.uniform(0, 1, wl.n_pix).astype(np.float32)
+    r = (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis)).astype(np.complex64)
+    # (a) one channel, scale != 1
+    plan = sl.Plan(uvw, wl.l, wl.m).set_channels([1.2])
+    assert plan.describe()["phase_fp64"] == 1
+    o = oracle.Oracle(uvw * 1.2, wl.l, wl.m)
+    assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy().ravel(), o.forward(x)) <= 2e-4
+    assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy().ravel(), o.adjoint(r)) <= 2e-4
+    plan.close()
+    # (b) several channels
+    scale = np.array([0.9, 1.0, 1.3])
+    plan = sl.Plan(uvw, wl.l, wl.m).set_channels(scale)
+    assert plan.describe()["phase_fp64"] == 1
+    X = rng.uniform(0, 1, (3, wl.n_pix)).astype(np.float32)
+    R = (rng.standard_normal((3, wl.n_vis)) + 1j * rng.standard_normal((3, wl.n_vis))).astype(np.complex64)
+    Vg = plan.forward(_dev(X, torch.float32)).cpu().numpy()
+    Gg = plan.adjoint(_dev(R, torch.complex64)).cpu().numpy()
+    Vs, Ls, os_ = [], [], []
+    for c, sc in enumerate(scale):
+        oc = oracle.Oracle(uvw * sc, wl.l, wl.m)
+        assert rel_l2(Vg[c], oc.forward(X[c])) <= 2e-4 and rel_l2(Gg[c], oc.adjoint(R[c])) <= 2e-4
+        Vs.append((oc.forward(wl.x_true) + wl.noise).astype(np.complex64))
+        Ls.append(oc.max_eig(20) * 1.05)
+        os_.append(oc)
+    xs, _ = plan.solve_batch(_dev(np.stack(Vs), torch.complex64), 0.5, np.array(Ls), n_iter=30)
+    for c, oc in enumerate(os_):
+        assert rel_l2(xs[c].cpu().numpy(), oc.fista(Vs[c], 0.5, Ls[c], 30)["x"]) <= 1e-3
+    plan.close()
+    # (c) a plan below the limit whose top channel is above it: the decision is re-evaluated
+    q = sl.Plan(wl.uvw, wl.l, wl.m)
+    span1 = q.describe()["phase_span_rad"]
+    q.close()
+    fac, span0 = 200.0 / span1, 200.0          # the span scales with the baselines: 200 rad at scale 1
+    plan = sl.Plan(wl.uvw * fac, wl.l, wl.m)
+    assert plan.describe()["phase_fp64"] == 0 and abs(plan.describe()["phase_span_rad"] - span0) < 1.0
+    plan.set_channels([1.0, 256.0 / span0 * 1.1])
+    assert plan.describe()["phase_fp64"] == 1
+    top = 256.0 / span0 * 1.1
+    oc = oracle.Oracle(wl.uvw * fac * top, wl.l, wl.m)
+    X2 = np.stack([x, x])
+    assert rel_l2(plan.forward(_dev(X2, torch.float32)).cpu().numpy()[1], oc.forward(x)) <= 2e-4
+    plan.set_channels([1.0])        # and back: the default kernels again
+    assert plan.describe()["phase_fp64"] == 0
+    plan.close()
+
+
+def test_gain_table_with_more_than_65535_rows(sl):
+    """"Time-varying beams: give each (antenna, time) its own row" (sl1m.h): the gain re-layout loops over the rows
+    inside the kernel, so n_ant is not capped by a grid dimension."""
+    import torch
+    rng = np.random.default_rng(16)
+    n_ant, n_pix, n_vis = 70000, 40, 300
+    l = rng.uniform(-0.02, 0.02, n_pix)
+    m = rng.uniform(-0.02, 0.02, n_pix)
+    uvw = rng.uniform(-1, 1, (n_vis, 3)) * np.array([300.0, 300.0, 30.0])
+    ap = rng.integers(0, n_ant, n_vis).astype(np.int32)
+    aq = rng.integers(0, n_ant, n_vis).astype(np.int32)
+    ap[:4] = [0, n_ant - 1, 65535, 65536]
+    g = (1.0 + 0.2 * (rng.standard_normal((n_ant, n_pix)) + 1j * rng.standard_normal((n_ant, n_pix)))).astype(np.complex64)
+    plan = sl.Plan(uvw, l, m, ant_p=ap, ant_q=aq, gains=g)
+    o = oracle.Oracle(uvw, l, m, ant_p=ap, ant_q=aq, gains=g)
+    x = rng.uniform(0, 1, n_pix).astype(np.float32)
+    r = (rng.standard_normal(n_vis) + 1j * rng.standard_normal(n_vis)).astype(np.complex64)
+    assert rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x)) <= 2e-4
+    assert rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r)) <= 2e-4
+    plan.close()
+
+
 @pytest.mark.parametrize("kind", ["delta", "gauss_tiles", "delta_small", "gains_grouped", "gains_per_term"])
 def test_zero_skipping_forward(sl, kind):
     """The forward streams only pixels with x_k != 0 (sl1m_forward_active_pixels; eq (18), PAPER.md:194-197,

@@ -406,6 +406,116 @@ def test_tolerance_stop_matches_oracle(sl):
     plan.close()
 
 
+def test_device_side_stop_rules_match_oracle(sl):
+    """sl1m_solve_stop: both criteria of PAPER.md:194 decided on the device (readings R21, R24).
+    E rule == sl1m_solve_tol; nnz rule and "either" against oracle.fista_tol(nnz_tol=...).  The decision is taken
+    from fp32-computed sums on the GPU, so near a threshold the stop may move by a look or two: the image is
+    compared with the oracle's fixed-K run at the GPU's own stopping index, the index within 3 looks."""
+    import torch
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = fista_lambda(wl)
+    plan = sl.Plan.from_workload(wl)
+    Vd = _dev(V, torch.complex64)
+    cases = [(1e-5, -1.0, 5), (-1.0, 0.0, 1), (-1.0, 0.0, 4), (-1.0, 0.02, 3), (1e-7, 0.0, 2)]
+    for tol, nnz_tol, every in cases:
+        ref = o.fista_tol(V, lam, L, max_iter=600, tol=tol, nnz_tol=nnz_tol, check_every=every)
+        x, info = plan.solve_stop(Vd, lam, L, max_iter=600, tol=tol, nnz_tol=nnz_tol, check_every=every)
+        k = info.n_iter_done
+        assert 2 <= k <= 600 and (k % every == 0 or k == 600), (tol, nnz_tol, every, k)
+        assert abs(k - ref["n_iter_done"]) <= 3 * every, (tol, nnz_tol, every, k, ref["n_iter_done"])
+        same_k = o.fista(V, lam, L, k)
+        assert rel_l2(x.cpu().numpy(), same_k["x"]) <= TOL_IMAGE
+        assert abs(info.l2_term - same_k["l2_term"]) <= 2e-3 * same_k["l2_term"]
+        if nnz_tol < 0:                              # the E rule alone is sl1m_solve_tol
+            x2, info2 = plan.solve_tol(Vd, lam, L, max_iter=600, tol=tol, check_every=every)
+            assert info2.n_iter_done == k and torch.equal(x, x2)
+    # a stop well before the cap really skips the rest: the same image as a fixed-K run of n_iter_done iterations
+    x, info = plan.solve_stop(Vd, lam, L, max_iter=5000, tol=1e-4, check_every=1)
+    assert info.n_iter_done < 600
+    xk, _ = plan.solve(Vd, lam, L=L, n_iter=info.n_iter_done)
+    assert torch.equal(x, xk)
+    # neither rule: an error; the cap with a caller-supplied trace
+    with pytest.raises(sl.Sl1mError):
+        plan.solve_stop(Vd, lam, L, max_iter=5, tol=-1.0, nnz_tol=-1.0)
+    trace = torch.zeros(3 * 9, dtype=torch.float64, device="cuda")
+    x, info = plan.solve_stop(Vd, lam, L, max_iter=9, tol=0.0, nnz_tol=-1.0, check_every=1, trace=trace)
+    assert info.n_iter_done == 9
+    ref9 = o.fista(V, lam, L, 9, want_trace=True)
+    tr = trace.cpu().numpy().reshape(-1, 3)
+    assert np.max(np.abs(tr[:, 0] - ref9["trace"][:, 0]) / ref9["trace"][:, 0]) < 2e-3
+    plan.close()
+
+
+def test_solve_stop_batch_each_channel_stops_on_its_own(sl):
+    """sl1m_solve_stop_batch + sl1m_dirty_image on a batched plan (NEXT-1 composed with NEXT-4; the paper's runs are
+    63-127 channels each solved to a tolerance): per-channel lambda gives per-channel stopping
+    indices; every channel is compared with the oracle's run of that channel alone."""
+    import torch
+    wl = make_workload(1)
+    scale = np.array([1.0, 0.9, 1.1, 1.25, 0.8])
+    C = scale.shape[0]
+    plan = sl.Plan.from_workload(wl).set_channels(scale)
+    oracles = [oracle.Oracle(wl.uvw * s, wl.l, wl.m) for s in scale]
+    Vs = np.stack([(o.forward(wl.x_true * (1.0 + 0.2 * c)) + wl.noise).astype(np.complex64) for c, o in enumerate(oracles)])
+    lam = fista_lambda(wl) * np.array([1.0, 4.0, 0.5, 2.0, 8.0])
+    L = np.array([o.max_eig(30) * 1.05 for o in oracles])
+    Vd = _dev(Vs, torch.complex64)
+    # dirty image of every channel in one call, used as the start
+    d = plan.dirty_image(Vd)
+    assert d.shape == (C, wl.n_pix)
+    d_ref = np.stack([o.dirty_image(Vs[c], 1.0 / wl.n_vis) for c, o in enumerate(oracles)])
+    for c in range(C):
+        assert rel_l2(d[c].cpu().numpy(), d_ref[c]) <= TOL_APPLY
+    tol, every = 1e-5, 2
+    x, infos = plan.solve_stop_batch(Vd, lam, L, max_iter=800, tol=tol, check_every=every, x0=d)
+    x = x.cpu().numpy()
+    ks = [i.n_iter_done for i in infos]
+    print("per-channel stopping iterations", ks)
+    assert len(set(ks)) >= 3                       # the channels really stopped at different iterations
+    for c, o in enumerate(oracles):
+        ref = o.fista_tol(Vs[c], lam[c], L[c], max_iter=800, tol=tol, check_every=every, x0=d_ref[c])
+        assert abs(ks[c] - ref["n_iter_done"]) <= 3 * every, (c, ks[c], ref["n_iter_done"])
+        same_k = o.fista(Vs[c], lam[c], L[c], ks[c], x0=d_ref[c])
+        assert rel_l2(x[c], same_k["x"]) <= TOL_IMAGE, (c, rel_l2(x[c], same_k["x"]))
+        assert abs(infos[c].l2_term - same_k["l2_term"]) <= 2e-3 * same_k["l2_term"]
+    plan.close()
+
+
+def test_fista_stepping_api_is_the_same_run(sl):
+    """sl1m_fista_begin / _step / _image: 3 + 4 + 1 stepped iterations are bit-identical to one sl1m_solve of 8
+    (momentum carried across the calls), with the per-call trace rows equal to the solve's."""
+    import torch
+    wl = make_workload(2, n_side=64, n_steps=4, n_src=40)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(20) * 1.05
+    lam = fista_lambda(wl)
+    plan = sl.Plan.from_workload(wl)
+    Vd = _dev(V, torch.complex64)
+    trace = torch.zeros(3 * 8, dtype=torch.float64, device="cuda")
+    x8, _ = plan.solve(Vd, lam, L=L, n_iter=8, trace=trace, want_info=False)
+    plan.fista_begin(Vd, lam, L)
+    parts = []
+    for n in (3, 4, 1):
+        t = torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+        plan.fista_step(n, trace=t)
+        parts.append(t)
+    xs, k = plan.fista_image()
+    assert k == 8 and torch.equal(xs, x8)
+    assert torch.equal(torch.cat(parts), trace)
+    assert rel_l2(xs.cpu().numpy(), o.fista(V, lam, L, 8)["x"]) <= TOL_IMAGE
+    plan.fista_step(2)
+    x10, k = plan.fista_image()
+    assert k == 10 and torch.equal(x10, plan.solve(Vd, lam, L=L, n_iter=10, want_info=False)[0])
+    plan.solve(Vd, lam, L=L, n_iter=1)              # a solve that returns info ends the stepped state
+    with pytest.raises(sl.Sl1mError):
+        plan.fista_step(1)
+    plan.close()
+
+
 def test_dirty_image_start_matches_oracle(sl):
     """sl1m_dirty_image (reading R22) and a solve started from it."""
     import torch

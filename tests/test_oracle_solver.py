@@ -295,7 +295,7 @@ def test_nnz_change_stop_rule():
     x_true[rng.choice(o.n_pix, 12, replace=False)] = rng.uniform(0.5, 3.0, 12)
     V = o.forward(x_true) + 0.05 * (rng.standard_normal(o.n_vis) + 1j * rng.standard_normal(o.n_vis))
     L = o.max_eig(200) * 1.05
-    lam, K = 0.3, 300
+    lam, K = 0.3, 120
     N = np.array([np.count_nonzero(o.fista(V, lam=lam, L=L, n_iter=k)["x"]) for k in range(1, K + 1)])
     assert len(set(N[:40].tolist())) > 3                     # the support size really changes early on
     seen = set()
