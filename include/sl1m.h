@@ -64,6 +64,11 @@ typedef enum {
                                  * Chosen automatically when the fp32 phase remainder inside a pixel tile could
                                  * exceed 256 rad (a tile spanning > 40 fringes of the longest baseline: a badly
                                  * undersampled image); the default kernels are exact enough otherwise. */
+#define SL1M_NO_PERSISTENT 8u   /* small problems (delta pixels, unit gains, one channel, < 6.7e7 terms per apply) run the
+                                 * whole FISTA loop as ONE persistent cooperative kernel -- two grid barriers per
+                                 * iteration instead of six launches (sl1m_plan_info.persistent == 1).  This flag keeps
+                                 * the multi-launch loop, for A/B measurements and tests.  Both are deterministic; they sum
+                                 * in different orders, so their images agree to rounding, not bit for bit. */
 #define SL1M_DENSE_FORWARD 4u   /* switch the zero-skipping forward off (see sl1m_forward_active_pixels): every
                                  * pixel is streamed even where x_k == 0.  For A/B measurements and tests. */
 
@@ -303,6 +308,7 @@ typedef struct {
     int32_t phase_fp64;                  /* 1 = the fp64-phase kernels are in use                    */
     float phase_span_rad;                /* plan-time bound on the fp32 phase remainder in a tile    */
     int32_t zero_skip;                   /* 1 = the forward streams only pixels with x_k != 0       */
+    int32_t persistent;                  /* 1 = the FISTA loop of this plan runs as one persistent cooperative kernel */
     int32_t adj_mufu_per_term;           /* MUFU per MUFU-path term of the ADJOINT: 1 with the one-cosine kernels
                                           * (Re(e^{iX} r) = |r| cos(X + arg r)), 2 with per-tile-sigma Gaussian
                                           * pixels (ex2 + cos), else as the forward                  */
@@ -345,6 +351,21 @@ typedef struct {
     double coissue_adj_mufu_per_clk_sm;  /* 4 MUFU.COS + 8 FFMA2 + 4 FMUL.RZ per body (the one-cosine adjoint's mix) */
 } sl1m_peaks;
 int sl1m_measure_peaks(sl1m_peaks *out_host, void *stream);
+
+/*
+ * Memory-safety net without compute-sanitizer (SURVEY.md:184; the GPU pool does not run the tool).  A library
+ * built with -DSL1M_BOUNDS (paper_1310_2078_b200.build.build_library(bounds=True) -> libsl1m_bounds.so) puts a 4 KiB
+ * canary band on both sides of every device buffer it allocates and asserts, on the device, that the two documented
+ * over-reads of the kernels (register prefetch of gain-table rows, up to 4 rows past the pixels in use) stay inside
+ * their tables.  sl1m_debug_check synchronises the device and verifies every band: SL1M_ERR_CUDA (with
+ * sl1m_last_error naming the buffer size and side) after a stray write or a failed device assertion.  In the normal
+ * build it does nothing and returns SL1M_OK.  sl1m_debug_bounds_build: 1 in the debug build, else 0.
+ */
+int sl1m_debug_check(void);
+int sl1m_debug_bounds_build(void);
+/* Debug build only (SL1M_ERR_PARAM otherwise): writes 4 bytes just past the plan's residual buffer, so that a test can
+ * see sl1m_debug_check report it. */
+int sl1m_debug_poke_past_end(sl1m_plan *plan);
 
 /* Number of kernels this plan has launched since creation (for bench.py's gpu_launches). */
 int64_t sl1m_launch_count(const sl1m_plan *plan);

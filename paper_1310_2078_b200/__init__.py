@@ -7,6 +7,6 @@ There is no CPU fallback: using the binding without the built library or without
 raises.
 """
 from .binding import (  # noqa: F401
-    GAUSS_PARAXIAL, GAUSS_WIDEFIELD, PHASE_FP64, DENSE_FORWARD, Plan, Sl1mError, SolveInfo, build_library, library_path,
+    GAUSS_PARAXIAL, GAUSS_WIDEFIELD, PHASE_FP64, DENSE_FORWARD, NO_PERSISTENT, Plan, Sl1mError, SolveInfo, build_library, library_path,
     load_library, exported_symbols, quadtree_refine, quadtree_solve, measure_peaks,
 )

@@ -16,6 +16,7 @@ GAUSS_WIDEFIELD = 1  # eq (17)
 GAINS_ON_DEVICE = 1
 PHASE_FP64 = 2
 DENSE_FORWARD = 4
+NO_PERSISTENT = 8
 
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "sl1m.h")
 
@@ -31,7 +32,7 @@ class _PlanInfo(ctypes.Structure):
         "n_pix_padded", "n_tiles", "gaussian", "gains", "fwd_rv", "fwd_vis_tiles", "fwd_pixel_splits",
         "fwd_tiles_per_split", "fwd_poly_per16", "adj_rp", "adj_pixel_groups", "adj_vis_splits",
         "adj_chunks_per_split", "adj_poly_per16", "mufu_per_term_mufu_path", "fwd_packed_pairs",
-        "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("zero_skip", ctypes.c_int32), ("adj_mufu_per_term", ctypes.c_int32)]
+        "adj_packed_pairs", "phase_fp64")] + [("phase_span_rad", ctypes.c_float), ("zero_skip", ctypes.c_int32), ("persistent", ctypes.c_int32), ("adj_mufu_per_term", ctypes.c_int32)]
 
 
 class _Peaks(ctypes.Structure):
@@ -121,6 +122,9 @@ def load_library():
     lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
     lib.sl1m_forward_active_pixels.argtypes = [vp, vp, vp]
     lib.sl1m_measure_peaks.argtypes = [ctypes.POINTER(_Peaks), vp]
+    lib.sl1m_debug_check.argtypes = []
+    lib.sl1m_debug_bounds_build.argtypes = []
+    lib.sl1m_debug_poke_past_end.argtypes = [vp]
     lib.sl1m_launch_count.argtypes = [vp]
     lib.sl1m_launch_count.restype = i64
     lib.sl1m_plan_n_vis.argtypes = [vp]
@@ -137,9 +141,14 @@ def load_library():
     return lib
 
 
+_DEBUG_CHECK = bool(os.environ.get("SL1M_DEBUG_CHECK"))   # verify the canary bands of a -DSL1M_BOUNDS build after every call
+
+
 def _check(st: int):
+    lib = load_library()
+    if st == 0 and _DEBUG_CHECK:
+        st = lib.sl1m_debug_check()
     if st != 0:
-        lib = load_library()
         raise Sl1mError(st, lib.sl1m_status_string(st).decode(), lib.sl1m_last_error().decode())
 
 
@@ -215,7 +224,8 @@ class Plan:
     """sl1m_plan_create / sl1m_destroy.  Inputs are host arrays (numpy); see include/sl1m.h."""
 
     def __init__(self, uvw, l, m, sigma=None, ant_p=None, ant_q=None, gains=None,
-                 gauss_model: int = GAUSS_WIDEFIELD, phase_fp64: bool = False, dense_forward: bool = False):
+                 gauss_model: int = GAUSS_WIDEFIELD, phase_fp64: bool = False, dense_forward: bool = False,
+                 no_persistent: bool = False):
         import torch
         self._h = None
         lib = load_library()
@@ -227,7 +237,7 @@ class Plan:
         sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64).ravel()
         if sg is not None and sg.shape != l.shape:
             raise ValueError("sigma and l differ in length")
-        n_ant, g, flags = 0, None, (PHASE_FP64 if phase_fp64 else 0) | (DENSE_FORWARD if dense_forward else 0)
+        n_ant, g, flags = 0, None, (PHASE_FP64 if phase_fp64 else 0) | (DENSE_FORWARD if dense_forward else 0) | (NO_PERSISTENT if no_persistent else 0)
         ap = aq = None
         gptr = None
         if gains is not None:
@@ -268,9 +278,10 @@ class Plan:
         return (n,) if self.n_chan == 1 else (self.n_chan, n)
 
     @classmethod
-    def from_workload(cls, wl, gains_device=None, dense_forward: bool = False):
+    def from_workload(cls, wl, gains_device=None, dense_forward: bool = False, no_persistent: bool = False):
         g = wl.gains if gains_device is None else gains_device
-        return cls(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model, dense_forward=dense_forward)
+        return cls(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model, dense_forward=dense_forward,
+                   no_persistent=no_persistent)
 
     def close(self):
         if self._h is not None:

@@ -8,9 +8,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "sl1m.cu")
 SRC_QT = os.path.join(_HERE, "csrc", "sl1m_quadtree.cu")
 SRC_PK = os.path.join(_HERE, "csrc", "sl1m_peaks.cu")
-DEPS = [SRC, SRC_QT, SRC_PK, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"),
+DEPS = [SRC, SRC_QT, SRC_PK, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"), os.path.join(_HERE, "csrc", "sl1m_persist.cuh"),
         os.path.join(os.path.dirname(_HERE), "include", "sl1m.h")]
 LIB = os.path.join(_HERE, "libsl1m.so")
+LIB_BOUNDS = os.path.join(_HERE, "libsl1m_bounds.so")      # debug build: canary bands + asserted prefetches (-DSL1M_BOUNDS)
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]
@@ -23,16 +24,18 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    stale = not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(d) for d in DEPS)
+def build_library(force: bool = False, verbose: bool = False, bounds: bool = False) -> str:
+    lib = LIB_BOUNDS if bounds else LIB
+    stale = not os.path.exists(lib) or any(os.path.getmtime(lib) < os.path.getmtime(d) for d in DEPS)
     if force or stale:
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("SL1M_NVCC_EXTRA", "").split(), "-o", tmp, SRC, SRC_QT, SRC_PK]   # SL1M_NVCC_EXTRA: tuning -D flags
+        tmp = lib + f".tmp{os.getpid()}"
+        extra = os.environ.get("SL1M_NVCC_EXTRA", "").split() + (["-DSL1M_BOUNDS"] if bounds else [])   # SL1M_NVCC_EXTRA: tuning -D flags
+        cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-o", tmp, SRC, SRC_QT, SRC_PK]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":

@@ -11,9 +11,14 @@
 #include <new>
 #include <string>
 #include <vector>
+#ifdef SL1M_BOUNDS
+#include <map>
+#include <mutex>
+#endif
 
 #include "sl1m_epilogue.cuh"
 #include "sl1m_kernels.cuh"
+#include "sl1m_persist.cuh"
 
 using namespace sl1m;
 
@@ -33,6 +38,41 @@ int fail(int st, const std::string &msg) {
             return fail(e_ == cudaErrorMemoryAllocation ? SL1M_ERR_ALLOC : SL1M_ERR_CUDA,   \
                         std::string(#expr) + ": " + cudaGetErrorString(e_));                \
     } while (0)
+
+#ifdef SL1M_BOUNDS
+// Debug build (-DSL1M_BOUNDS; SURVEY.md:184 asks for memcheck, which the GPU pool refuses to run): every device buffer
+// this file allocates gets a 4 KiB canary band of 0xA5 on both sides; sl1m_debug_check() verifies all bands.  The
+// kernels over-read by design in two documented places (register prefetch of gain rows) and those are asserted in
+// range on the device (ldg_gain); a stray WRITE by any kernel lands in a band and is caught here.
+constexpr size_t CANARY = 4096;
+struct BoundsAlloc { size_t bytes; };
+std::map<void *, BoundsAlloc> g_allocs;      // user pointer -> size
+std::mutex g_allocs_mu;
+cudaError_t bounds_malloc(void **q, size_t bytes) {
+    unsigned char *base = nullptr;
+    const size_t padded = (bytes + 255) / 256 * 256;          // keep the trailing band aligned
+    cudaError_t e = (cudaMalloc)((void **)&base, padded + 2 * CANARY);
+    if (e != cudaSuccess) return e;
+    (cudaMemset)(base, 0xA5, CANARY);
+    (cudaMemset)(base + CANARY + bytes, 0xA5, padded - bytes + CANARY);
+    *q = base + CANARY;
+    std::lock_guard<std::mutex> lk(g_allocs_mu);
+    g_allocs[*q] = BoundsAlloc{bytes};
+    return cudaSuccess;
+}
+cudaError_t bounds_free(void *q) {
+    if (!q) return cudaSuccess;
+    {
+        std::lock_guard<std::mutex> lk(g_allocs_mu);
+        auto it = g_allocs.find(q);
+        if (it == g_allocs.end()) return (cudaFree)(q);       // not ours (e.g. a caller's buffer)
+        g_allocs.erase(it);
+    }
+    return (cudaFree)((unsigned char *)q - CANARY);
+}
+#define cudaMalloc(q, n) bounds_malloc((void **)(q), (n))
+#define cudaFree(q) bounds_free((void *)(q))
+#endif
 
 constexpr int SM_COUNT_B200 = 148;
 constexpr int GAIN_ROW_PAD = 4;   // rows of padding behind the forward-layout gain tables (prefetch distance of the kernels)
@@ -99,6 +139,13 @@ struct sl1m_plan {
     const int *done_ptr = nullptr;   // == ctl_i while a stopping solve is enqueueing, else NULL
     int *h_flag = nullptr;           // pinned HOST [2]: all_done as seen by the last two polls
     cudaEvent_t poll_ev[2] = {nullptr, nullptr};
+    // persistent single-kernel FISTA of small problems (sl1m_persist.cuh)
+    bool persist = false, no_persist = false;
+    int persist_grid = 0;
+    float4 *pvis4 = nullptr;         // [n_vis] 2 pi (u, v, w)
+    float *px0 = nullptr;            // [n_tiles][n_vis] centre phases
+    double *ppart = nullptr;         // [2][3][persist_grid]
+    unsigned *pbar = nullptr;        // grid-barrier counter
     int64_t launches = 0;
     int device = 0;
 };
@@ -117,7 +164,7 @@ void free_plan(sl1m_plan *p) {
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
                     p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc, p->rpol, p->ctl_i,
-                    p->lam2, p->pixdc, p->pixgc};
+                    p->lam2, p->pixdc, p->pixgc, p->pvis4, p->px0, p->ppart, p->pbar};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (p->h_flag) cudaFreeHost(p->h_flag);
@@ -165,6 +212,10 @@ ApplyParams make_params(const sl1m_plan *p) {
     P.ws_v_stride = (size_t)p->fwd_split * (size_t)p->n_vis_int;
     P.ws_p_stride = (size_t)p->adj_split * (size_t)p->n_pix_pad;
     P.done = p->done_ptr;
+#ifdef SL1M_BOUNDS
+    P.gF_end = p->gF ? p->gF + ((size_t)p->n_pix_pad + GAIN_ROW_PAD) * (size_t)p->n_ant : nullptr;
+    P.gFc_end = p->gFc ? p->gFc + ((size_t)p->n_chan * p->n_pix_pad + GAIN_ROW_PAD) * (size_t)p->n_ant : nullptr;
+#endif
     return P;
 }
 
@@ -276,6 +327,35 @@ int configure_and_allocate(sl1m_plan *p) {
     return SL1M_OK;
 }
 
+// Small problems (delta pixels, unit gains, one channel, fp32 phase) run the FISTA loop as ONE persistent
+// cooperative kernel (sl1m_persist.cuh).  "Small": below ~6.7e7 generated terms per apply the ~19 us of launch
+// latency per multi-launch iteration outweighs what the tuned (packed, pipe-balanced) apply kernels gain per term.
+constexpr double PERSIST_MAX_TERMS = 67108864.0;
+int persist_setup(sl1m_plan *p) {
+    p->persist = false;
+    if (p->no_persist || p->pk != 0 || p->gk != 0 || p->phase64 || p->n_tiles > PERSIST_MAX_TILES ||
+        (double)p->n_pix_pad * (double)p->n_vis_int > PERSIST_MAX_TERMS)
+        return SL1M_OK;
+    int coop = 0, per_sm = 0, sms = 0;
+    CUDA_TRY(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, p->device));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fista_persistent_kernel, PT, 0));
+    if (!coop || per_sm < 1) return SL1M_OK;
+    p->persist_grid = sms;                                   // one CTA per SM
+    const size_t nv = (size_t)p->n_vis_int, nt = (size_t)p->n_tiles;
+    CUDA_TRY(cudaMalloc((void **)&p->pvis4, nv * sizeof(float4)));
+    CUDA_TRY(cudaMalloc((void **)&p->px0, nt * nv * sizeof(float)));
+    CUDA_TRY(cudaMalloc((void **)&p->ppart, 2 * 3 * (size_t)p->persist_grid * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&p->pbar, sizeof(unsigned)));
+    persist_tables_kernel<<<dim3((unsigned)((nv + 255) / 256), (unsigned)std::min<size_t>(nt, 64)), 256>>>(
+        p->u64, p->v64, p->w64, p->cen, p->n_vis_int, p->n_tiles, p->pvis4, p->px0);
+    p->launches++;
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaDeviceSynchronize());
+    p->persist = true;
+    return SL1M_OK;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------
@@ -294,7 +374,8 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     if (gains && n_ant < 1) return fail(SL1M_ERR_SIZE, "n_ant must be >= 1 with gains");
     if (gauss_model != SL1M_GAUSS_PARAXIAL && gauss_model != SL1M_GAUSS_WIDEFIELD)
         return fail(SL1M_ERR_PARAM, "unknown gauss_model");
-    if (flags & ~(SL1M_GAINS_ON_DEVICE | SL1M_PHASE_FP64 | SL1M_DENSE_FORWARD)) return fail(SL1M_ERR_PARAM, "unknown flag");
+    if (flags & ~(SL1M_GAINS_ON_DEVICE | SL1M_PHASE_FP64 | SL1M_DENSE_FORWARD | SL1M_NO_PERSISTENT))
+        return fail(SL1M_ERR_PARAM, "unknown flag");
     for (int64_t j = 0; j < 3 * n_vis; ++j)
         if (!std::isfinite(uvw[j])) return fail(SL1M_ERR_DOMAIN, "non-finite uvw");
     bool any_gauss = false;
@@ -325,6 +406,7 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     } guard{p};
     CUDA_TRY(cudaGetDevice(&p->device));
     p->dense_forward = (flags & SL1M_DENSE_FORWARD) != 0;
+    p->no_persist = (flags & SL1M_NO_PERSISTENT) != 0;
     p->n_vis = n_vis;
     p->n_pix = n_pix;
     p->n_ant = gains ? n_ant : 0;
@@ -546,6 +628,7 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
     {
         int st2 = configure_and_allocate(p);
         if (st2) return st2;
+        if ((st2 = persist_setup(p))) return st2;
     }
 
     guard.p = nullptr;
@@ -850,8 +933,53 @@ int fista_begin_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, 
 // termination rules, decided on the device (stop_rule_kernel) from trace rows k-1, k-2 counted from the state's
 // begin -- the caller's trace must then hold every iteration since begin (trace_row0 == p->f_k).
 // The host never waits for an iteration: it reads the all-done flag two polls behind what it has enqueued.
+// The same iterations as ONE launch of the persistent kernel (small single-channel problems).
+int persist_iterate(sl1m_plan *p, int n_iter, double *trace_rows, const StopOpts *stop, cudaStream_t s) {
+    if (n_iter < 1) return SL1M_OK;
+    PersistParams P;
+    memset(&P, 0, sizeof(P));
+    const int G = p->persist_grid;
+    P.n_vis = p->n_vis_int;
+    P.n_pix_pad = p->n_pix_pad;
+    P.n_tiles = p->n_tiles;
+    P.nvg = std::max(1, std::min(PG, (p->n_vis_int + G - 1) / G));
+    int npg = 1;
+    while (npg < PG && p->n_pix_pad / npg > G) npg <<= 1;    // power of two: an item never straddles a tile
+    P.npg = npg;
+    P.vis4 = p->pvis4;
+    P.x0 = p->px0;
+    P.pix4 = p->pix4;
+    P.amp = p->amp;
+    P.I_sorted = p->I_sorted;
+    P.y_sorted = p->y_sorted;
+    P.V = p->f_vis;
+    P.rpol = p->rpol;
+    P.part = p->ppart;
+    P.bar = p->pbar;
+    P.trace = trace_rows;
+    P.ctl = stop ? p->ctl_i : nullptr;
+    P.inv_L = p->f_inv_L;
+    P.thr = p->f_thr;
+    P.lam2 = 2.0 * (double)p->f_lam[0];
+    P.tol = stop ? stop->tol : -1.0;
+    P.nnz_tol = stop ? stop->nnz_tol : -1.0;
+    P.check_every = stop ? stop->check_every : 0;
+    P.k0 = p->f_k;
+    P.t0 = p->f_t;
+    P.n_iter = n_iter;
+    CUDA_TRY(cudaMemsetAsync(p->pbar, 0, sizeof(unsigned), s));
+    void *args[] = {(void *)&P};
+    CUDA_TRY(cudaLaunchCooperativeKernel((const void *)fista_persistent_kernel, dim3((unsigned)G), dim3(PT), args, 0, s));
+    p->launches++;
+    for (int i = 0; i < n_iter; ++i) p->f_t = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * p->f_t * p->f_t));
+    p->f_k += n_iter;
+    return check_launch("sl1m_fista_step(persistent)");
+}
+
 int fista_iterate(sl1m_plan *p, int n_iter, double *trace_dev, size_t trace_stride, int trace_row0,
                   const StopOpts *stop, cudaStream_t s) {
+    if (p->persist && !p->chan_scale)
+        return persist_iterate(p, n_iter, trace_dev ? trace_dev + 3 * (size_t)trace_row0 : nullptr, stop, s);
     const int C = p->n_chan, npad = p->n_pix_pad;
     const float2 *step_c = C > 1 ? p->step_c : nullptr;
     const int *done = stop ? p->ctl_i : nullptr;
@@ -1188,6 +1316,7 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->phase_fp64 = p->phase64;
     o->phase_span_rad = (float)p->phase_span;
     o->zero_skip = p->pixc != nullptr;
+    o->persistent = p->persist && !p->chan_scale;
     o->adj_mufu_per_term = o->mufu_per_term_mufu_path;
     if (!p->phase64) {
         if (p->pk == 0) o->adj_mufu_per_term = 1;    // delta pixels: one cosine per term in every adjoint kernel
@@ -1220,6 +1349,53 @@ extern "C" int sl1m_forward_active_pixels(sl1m_plan *p, int64_t *n_active_host, 
         n_active_host[c] = n;
     }
     return SL1M_OK;
+}
+
+extern "C" int sl1m_debug_check(void) {
+#ifdef SL1M_BOUNDS
+    cudaError_t e = cudaDeviceSynchronize();                  // also surfaces a device-side assert of ldg_gain
+    if (e != cudaSuccess) return fail(SL1M_ERR_CUDA, std::string("sl1m_debug_check: ") + cudaGetErrorString(e));
+    std::vector<unsigned char> h(2 * CANARY + 256);
+    std::lock_guard<std::mutex> lk(g_allocs_mu);
+    for (const auto &kv : g_allocs) {
+        const unsigned char *u = (const unsigned char *)kv.first;
+        const size_t bytes = kv.second.bytes, tail = (bytes + 255) / 256 * 256 - bytes + CANARY;
+        if ((cudaMemcpy)(h.data(), u - CANARY, CANARY, cudaMemcpyDeviceToHost) != cudaSuccess ||
+            (cudaMemcpy)(h.data() + CANARY, u + bytes, tail, cudaMemcpyDeviceToHost) != cudaSuccess)
+            return fail(SL1M_ERR_CUDA, "sl1m_debug_check: cannot read a canary band");
+        for (size_t i = 0; i < CANARY + tail; ++i)
+            if (h[i] != 0xA5) {
+                char msg[160];
+                snprintf(msg, sizeof(msg), "sl1m_debug_check: buffer of %zu bytes overwritten %s its %s (byte %zu of the band)",
+                         bytes, i < CANARY ? "before" : "past", i < CANARY ? "start" : "end", i < CANARY ? CANARY - i : i - CANARY);
+                return fail(SL1M_ERR_CUDA, msg);
+            }
+    }
+    return SL1M_OK;
+#else
+    return SL1M_OK;
+#endif
+}
+
+extern "C" int sl1m_debug_poke_past_end(sl1m_plan *p) {
+#ifdef SL1M_BOUNDS
+    if (!p) return fail(SL1M_ERR_NULL, "sl1m_debug_poke_past_end: NULL plan");
+    const float v = 1.0f;      // 4 bytes just past the residual buffer: what a one-element overrun of a kernel would do
+    CUDA_TRY((cudaMemcpy)((unsigned char *)p->resid + (size_t)p->n_chan * (size_t)p->n_vis_int * sizeof(float2), &v, sizeof(v),
+                          cudaMemcpyHostToDevice));
+    return SL1M_OK;
+#else
+    (void)p;
+    return fail(SL1M_ERR_PARAM, "sl1m_debug_poke_past_end: not a -DSL1M_BOUNDS build");
+#endif
+}
+
+extern "C" int sl1m_debug_bounds_build(void) {
+#ifdef SL1M_BOUNDS
+    return 1;
+#else
+    return 0;
+#endif
 }
 
 extern "C" int64_t sl1m_launch_count(const sl1m_plan *p) { return p ? p->launches : 0; }

@@ -27,6 +27,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <type_traits>
+#ifdef SL1M_BOUNDS
+#include <cassert>
+#endif
 
 namespace sl1m {
 
@@ -74,7 +77,22 @@ struct ApplyParams {
     // kernel of the iteration then returns at once for that channel, so the iterations the host had already
     // enqueued cost a few microseconds and the image stays the one of the stopping iteration.  NULL = never.
     const int *done;                // [n_chan] or NULL
+#ifdef SL1M_BOUNDS
+    // debug build (-DSL1M_BOUNDS): one-past-the-end of the two gain tables, padding rows included; every
+    // forward-layout gain load (the register prefetches run up to 4 rows past the pixels in use) is asserted in range
+    const float2 *gF_end, *gFc_end;
+#endif
 };
+
+// Forward-layout gain load.  The kernels prefetch rows ahead of the pixel they are on -- up to 4 rows past the last
+// pixel in use, which the tables' padding rows absorb.  The debug build asserts that every such address is inside
+// one of the two tables (compute-sanitizer is not available on the pool; tests/test_gpu_bounds.py runs this build).
+__device__ __forceinline__ float2 ldg_gain(const ApplyParams &P, const float2 *q) {
+#ifdef SL1M_BOUNDS
+    assert((q >= P.gF && q < P.gF_end) || (P.gFc && q >= P.gFc && q < P.gFc_end));
+#endif
+    return __ldg(q);
+}
 
 // BATCH is a compile-time switch: the single-channel instantiations carry no channel arithmetic at
 // all (measured: even a live fp64 scale register costs the packed forward kernel 7 %).
@@ -456,10 +474,10 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
         // grouped gains: register prefetch two pixels ahead (rows are cold in L1 on first touch)
         float2 gp0, gq0, gp1, gq1;
         if (GK == 2) {
-            gp0 = __ldg(gbase + ap[0]);
-            gq0 = __ldg(gbase + aq[0]);
-            gp1 = __ldg(gbase + P.n_ant + ap[0]);
-            gq1 = __ldg(gbase + P.n_ant + aq[0]);
+            gp0 = ldg_gain(P, gbase + ap[0]);
+            gq0 = ldg_gain(P, gbase + aq[0]);
+            gp1 = ldg_gain(P, gbase + P.n_ant + ap[0]);
+            gq1 = ldg_gain(P, gbase + P.n_ant + aq[0]);
         }
 #pragma unroll 2
         for (int p = 0; p < npx; ++p) {
@@ -472,8 +490,8 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 gp0 = gp1;
                 gq0 = gq1;
                 const int pn = min(p + 2, TP - 1);
-                gp1 = __ldg(gbase + (size_t)pn * P.n_ant + ap[0]);
-                gq1 = __ldg(gbase + (size_t)pn * P.n_ant + aq[0]);
+                gp1 = ldg_gain(P, gbase + (size_t)pn * P.n_ant + ap[0]);
+                gq1 = ldg_gain(P, gbase + (size_t)pn * P.n_ant + aq[0]);
                 Gw = px.w * (gp.x * gq.x);
                 gam = gp.y - gq.y;
             }
@@ -489,8 +507,8 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
                 float wg = Gw;
                 if (GK == 2) X -= gam;
                 if (GK == 1) {
-                    const float2 gp = __ldg(gbase + (size_t)p * P.n_ant + ap[r]);
-                    const float2 gq = __ldg(gbase + (size_t)p * P.n_ant + aq[r]);
+                    const float2 gp = ldg_gain(P, gbase + (size_t)p * P.n_ant + ap[r]);
+                    const float2 gq = ldg_gain(P, gbase + (size_t)p * P.n_ant + aq[r]);
                     wg = px.w * (gp.x * gq.x);
                     X -= gp.y - gq.y;
                 }
@@ -649,8 +667,8 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
             float2 gp[4], gq[4];
 #pragma unroll
             for (int d = 0; d < 4; ++d) {
-                gp[d] = __ldg(gbase + (op + d * na));
-                gq[d] = __ldg(gbase + (oq + d * na));
+                gp[d] = ldg_gain(P, gbase + (op + d * na));
+                gq[d] = ldg_gain(P, gbase + (oq + d * na));
             }
 #pragma unroll 1
             for (int p = 0; p < npx; p += 4) {
@@ -664,8 +682,8 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
                 oq += 4 * na;
 #pragma unroll
                 for (int d = 0; d < 4; ++d) {                // rows past npx exist (stale, zero or padding): harmless prefetch
-                    gp[d] = __ldg(gbase + (op + d * na));
-                    gq[d] = __ldg(gbase + (oq + d * na));
+                    gp[d] = ldg_gain(P, gbase + (op + d * na));
+                    gq[d] = ldg_gain(P, gbase + (oq + d * na));
                 }
                 pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, Gw[0], Ng[0]);
                 pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, Gw[1], Ng[1]);

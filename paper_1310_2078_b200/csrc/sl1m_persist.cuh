@@ -1,0 +1,322 @@
+// sl1m_persist.cuh -- the whole FISTA loop of a SMALL problem in ONE persistent cooperative kernel.
+//
+// Why: config 1 (1,024 pixels x 1,000 visibilities) is 2e6 generated terms per iteration -- under a microsecond
+// of arithmetic on 148 SMs -- but the multi-launch loop (forward, residual epilogue, polar residual, adjoint, fused
+// update, partial sums) costs 18.7 us per iteration in launch latency alone.  The paper's small real
+// data set is of this kind: 127 channels of 256^2 pixels x 11,934 visibilities, ~200 iterations each
+// (PAPER.md:279-291).  Here one CTA per SM stays resident for all iterations of the listing:
+//
+//   phase A (forward + residual, a1 + a3):  a CTA owns <= 8 visibilities; its threads split the pixel list, generate
+//       the entries (eq 9, tile-centred phase as in sl1m_kernels.cuh), reduce over the CTA in a fixed order, subtract
+//       V and leave the residual in POLAR form (|r|, arg r) in global memory.
+//   --- grid barrier ---
+//   phase B (adjoint + update, a2 + a4 + a5): a CTA owns <= 8 consecutive pixels; its threads split the
+//       visibilities, accumulate |r| cos(X + arg r) (one cosine per term: the image is real), reduce, and the pixel's
+//       owner thread applies the gradient step, T^{lambda/L} (eq 18), the momentum and re-packs a*y.
+//   --- grid barrier ---
+//   objective partials (a6), the trace row and the stopping rules (readings R21, R24) from per-CTA
+//       partials, on the device; every CTA takes the same decision from the same numbers and leaves together.
+//
+// The phase of a term is x0(j, tile) + u' dl + v' dm + w' dn' as in the tuned kernels, but x0 -- the fp64 centre
+// phase of every (visibility, tile) pair -- is iteration-invariant, so it is tabulated ONCE at plan time
+// (n_tiles x n_vis floats).  Data another CTA wrote in the previous phase is read with ld.global.cg (L1 is not
+// coherent); constants go through the read-only path.  Sums are formed in a fixed order: results are bit-stable run
+// to run, but the order differs from the multi-launch kernels', so the two paths agree to rounding, not bit for bit.
+//
+// Zero-skipping: a warp compacts its 128-pixel block to the entries with a*y != 0 (ballot + prefix popcount, order
+// kept) before generating terms, so the forward costs what the non-zero pixels cost, as in the tuned path.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "sl1m_kernels.cuh"
+
+namespace sl1m {
+
+constexpr int PT = 256;            // threads per CTA
+constexpr int PW = PT / 32;        // warps per CTA
+constexpr int PG = 8;              // visibilities (phase A) / pixels (phase B) per work item
+constexpr int PBLK = 128;          // pixels a warp compacts at a time in phase A
+constexpr int PERSIST_MAX_TILES = 512;   // 131,072 pixels: s_x0 is 16 KB of the CTA's 34 KB of static shared memory
+
+struct PersistParams {
+    int n_vis, n_pix_pad, n_tiles;
+    int nvg, npg;                  // visibilities / pixels per work item (1, 2, 4 or 8; npg divides TP)
+    const float4 *vis4;            // [n_vis] (2 pi u, 2 pi v, 2 pi w, 0)
+    const float *x0;               // [n_tiles][n_vis] centre phases, radians in [-pi, pi]
+    float4 *pix4;                  // [n_pix_pad] (dl, dm, dn', a*y); .w rewritten every iteration
+    const float *amp;              // [n_pix_pad] 1/n_k (0 on padding)
+    float *I_sorted, *y_sorted;    // [n_pix_pad] I_k, y_{k+1}
+    const float2 *V;               // [n_vis] measured visibilities
+    float2 *rpol;                  // [n_vis] residual (|r|, arg r)
+    double *part;                  // [2][3][gridDim.x] per-CTA partials (||r||^2, sum I, nnz), double-buffered by iteration parity
+    unsigned *bar;                 // grid-barrier counter, zero at launch
+    double *trace;                 // [.][3] rows of this launch's iterations, or NULL
+    int *ctl;                      // {done, n_done, all_done} (sl1m_solve_stop) or NULL
+    float inv_L, thr;
+    double lam2, tol, nnz_tol;     // stopping rules (tol, nnz_tol < 0: off)
+    int check_every;               // 0: no stopping rule
+    int k0;                        // iterations done before this launch
+    double t0;                     // t_{k0+1}
+    int n_iter;
+};
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// All CTAs of the (cooperatively launched, co-resident) grid meet here.  Monotonic counter: the n-th barrier is
+// passed when it reaches n * gridDim.x.  Release: __threadfence before the arrive; acquire: ld.acquire by the
+// polling thread, then the CTA barrier hands the visibility on to the other threads.
+__device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        __threadfence();
+        atomicAdd(bar, 1u);
+        while (ld_acquire_u32(bar) < target) {}
+    }
+    __syncthreads();
+}
+
+// Fixed-order CTA sum of N per-thread values: warp shuffles, then PW per-warp partials added in warp order.
+// Result valid in threads 0..N-1 (thread i holds sum i).
+template <int N>
+__device__ __forceinline__ float cta_sum(float (&v)[N], float (*s_red)[PG * 2 + 1]) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    }
+    __syncthreads();                      // s_red free again
+    if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) s_red[warp][i] = v[i];
+    }
+    __syncthreads();
+    float t = 0.f;
+    if (threadIdx.x < N) {
+#pragma unroll
+        for (int w = 0; w < PW; ++w) t += s_red[w][threadIdx.x];
+    }
+    return t;
+}
+
+// Sum of n doubles at p (written by other CTAs: ld.cg), by one warp in a fixed order; result in every lane.
+__device__ __forceinline__ double warp_sum_cg(const double *p, int n) {
+    double v = 0.0;
+    for (int i = threadIdx.x & 31; i < n; i += 32) v += __ldcg(p + i);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistParams P) {
+    __shared__ __align__(16) float4 s_list[PW][PBLK];       // compacted non-zero pixels of the warp's block
+    __shared__ uint16_t s_tile[PW][PBLK];                    // their tile index
+    __shared__ __align__(16) float s_x0[PERSIST_MAX_TILES][PG];   // centre phases of the CTA's phase-A item
+    __shared__ float s_red[PW][PG * 2 + 1];
+    __shared__ int s_stop;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int G = gridDim.x;
+    unsigned bar_target = 0;
+    const int items_a = (P.n_vis + P.nvg - 1) / P.nvg;
+    const int items_b = P.n_pix_pad / P.npg;
+    const bool one_item_a = items_a <= G;                    // the CTA's x0 slice never changes: stage it once
+    double t = P.t0, E_prev = 0.0, N_prev = 0.0;
+    int staged_item = -1;
+
+    for (int it = 0; it < P.n_iter; ++it) {
+        const int k = P.k0 + it + 1;                         // 1-based iteration number of the listing
+        double *part = P.part + (size_t)(k & 1) * 3 * G;
+
+        // ------------------------------------------------------------------ phase A: r = M y - V
+        double r2 = 0.0;
+        for (int item = blockIdx.x; item < items_a; item += G) {
+            const int j0 = item * P.nvg;
+            if (staged_item != item) {
+                __syncthreads();
+                for (int i = tid; i < P.n_tiles * PG; i += PT) {
+                    const int tl = i / PG, r = i - tl * PG, j = min(j0 + r, P.n_vis - 1);
+                    s_x0[tl][r] = __ldg(P.x0 + (size_t)tl * P.n_vis + j);
+                }
+                __syncthreads();
+                staged_item = one_item_a ? item : -1;
+            }
+            float uf[PG], vf[PG], wf[PG], acc[2 * PG];
+#pragma unroll
+            for (int r = 0; r < PG; ++r) {
+                const float4 v4 = __ldg(P.vis4 + min(j0 + r, P.n_vis - 1));
+                uf[r] = v4.x;
+                vf[r] = v4.y;
+                wf[r] = v4.z;
+                acc[2 * r] = 0.f;
+                acc[2 * r + 1] = 0.f;
+            }
+            // the warp's share of the pixel list, PBLK pixels at a time: compact to a*y != 0, then generate
+            for (int base = warp * PBLK; base < P.n_pix_pad; base += PW * PBLK) {
+                int cnt = 0;
+#pragma unroll
+                for (int q = 0; q < PBLK / 32; ++q) {
+                    const int kpx = base + q * 32 + lane;
+                    const float4 px = __ldcg(P.pix4 + kpx);
+                    const bool nz = px.w != 0.f;             // NaN counts as non-zero and propagates
+                    const unsigned b = __ballot_sync(0xffffffffu, nz);
+                    if (nz) {
+                        const int pos = cnt + __popc(b & ((1u << lane) - 1u));
+                        s_list[warp][pos] = px;
+                        s_tile[warp][pos] = (uint16_t)(kpx / TP);
+                    }
+                    cnt += __popc(b);
+                }
+                __syncwarp();
+                for (int i = lane; i < cnt; i += 32) {
+                    const float4 px = s_list[warp][i];
+                    const float4 *x0q = reinterpret_cast<const float4 *>(s_x0[s_tile[warp][i]]);
+                    const float4 xa = x0q[0], xb = x0q[1];
+                    const float x0r[PG] = {xa.x, xa.y, xa.z, xa.w, xb.x, xb.y, xb.z, xb.w};
+#pragma unroll
+                    for (int r = 0; r < PG; ++r) {
+                        if (r < P.nvg) {
+                            const float X = fmaf(uf[r], px.x, fmaf(vf[r], px.y, fmaf(wf[r], px.z, x0r[r])));
+                            float s, c;
+                            __sincosf(X, &s, &c);
+                            acc[2 * r] = fmaf(px.w, c, acc[2 * r]);
+                            acc[2 * r + 1] = fmaf(-px.w, s, acc[2 * r + 1]);
+                        }
+                    }
+                }
+                __syncwarp();
+            }
+            const float sum = cta_sum<2 * PG>(acc, s_red);   // thread i: re (i even) / im (i odd) of visibility i / 2
+            // pair up (re, im) in the even thread
+            const float other = __shfl_down_sync(0xffffffffu, sum, 1);
+            if (tid < 2 * P.nvg && (tid & 1) == 0) {
+                const int j = j0 + (tid >> 1);
+                if (j < P.n_vis) {
+                    const float2 v = __ldg(P.V + j);
+                    const float re = sum - v.x, im = other - v.y;
+                    P.rpol[j] = make_float2(sqrtf(fmaf(re, re, im * im)), atan2f(im, re));
+                    r2 += (double)re * re + (double)im * im;
+                }
+            }
+        }
+        if (tid < 32) {                                      // the CTA's ||r||^2 partial (even lanes of warp 0 hold terms)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+            if (tid == 0) part[blockIdx.x] = r2;
+        }
+        grid_barrier(P.bar, bar_target);
+
+        // ------------------------------------------------------------------ phase B: g = Re M^H r, update
+        // no FMA contraction: the host advances the same sequence with separate multiply and add (sl1m.cu)
+        const double t_next = 0.5 * __dadd_rn(1.0, sqrt(__dadd_rn(1.0, __dmul_rn(4.0 * t, t))));
+        const float beta = (float)((t - 1.0) / t_next);
+        t = t_next;
+        double l1 = 0.0, nz = 0.0;
+        for (int item = blockIdx.x; item < items_b; item += G) {
+            const int p0 = item * P.npg;
+            const float *x0row = P.x0 + (size_t)(p0 / TP) * P.n_vis;      // npg divides TP: one tile per item
+            float dl[PG], dm[PG], dn[PG], acc[PG];
+#pragma unroll
+            for (int i = 0; i < PG; ++i) {
+                const float4 px = __ldcg(P.pix4 + min(p0 + i, P.n_pix_pad - 1));   // .xyz are constants, .w is rewritten below
+                dl[i] = px.x;
+                dm[i] = px.y;
+                dn[i] = px.z;
+                acc[i] = 0.f;
+            }
+            for (int j = tid; j < P.n_vis; j += PT) {
+                const float4 v4 = __ldg(P.vis4 + j);
+                const float2 rp = __ldcg(P.rpol + j);
+                const float ph = __ldg(x0row + j) + rp.y;
+#pragma unroll
+                for (int i = 0; i < PG; ++i) {
+                    if (i < P.npg) {
+                        const float X = fmaf(v4.x, dl[i], fmaf(v4.y, dm[i], fmaf(v4.z, dn[i], ph)));
+                        acc[i] = fmaf(rp.x, __cosf(X), acc[i]);
+                    }
+                }
+            }
+            const float gsum = cta_sum<PG>(acc, s_red);
+            if (tid < P.npg) {
+                const int kk = p0 + tid;
+                const float a = __ldg(P.amp + kk);
+                const float g = gsum * a;
+                const float y = P.y_sorted[kk];                // own pixel: written by this thread last iteration
+                const float z = fmaf(-P.inv_L, g, y);
+                const float I_new = (z > P.thr) ? z - P.thr : 0.f;
+                const float I_old = P.I_sorted[kk];
+                const float y_new = fmaf(beta, I_new - I_old, I_new);
+                P.I_sorted[kk] = I_new;
+                P.y_sorted[kk] = y_new;
+                P.pix4[kk].w = a * y_new;
+                l1 += (double)I_new;
+                nz += (I_new != 0.f) ? 1.0 : 0.0;
+            }
+        }
+        if (tid < 32) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                l1 += __shfl_xor_sync(0xffffffffu, l1, o);
+                nz += __shfl_xor_sync(0xffffffffu, nz, o);
+            }
+            if (tid == 0) {
+                part[G + blockIdx.x] = l1;
+                part[2 * G + blockIdx.x] = nz;
+            }
+        }
+        grid_barrier(P.bar, bar_target);
+
+        // ------------------------------------------------------------------ a6: objective, trace, stopping rules
+        const bool look = P.check_every > 0 && k >= 2 && (k % P.check_every) == 0;
+        const bool before_look = P.check_every > 0 && ((k + 1) % P.check_every) == 0;
+        const bool want = look || before_look || (P.trace && blockIdx.x == 0);
+        if (want) {
+            if (warp == 0) {
+                const double l2s = warp_sum_cg(part, G), l1s = warp_sum_cg(part + G, G), nzs = warp_sum_cg(part + 2 * G, G);
+                if (lane == 0) {
+                    if (P.trace && blockIdx.x == 0) {
+                        P.trace[3 * (size_t)it] = l2s;
+                        P.trace[3 * (size_t)it + 1] = l1s;
+                        P.trace[3 * (size_t)it + 2] = nzs;
+                    }
+                    const double E = l2s + P.lam2 * l1s;
+                    int stop = 0;
+                    if (look)
+                        stop = (P.tol >= 0.0 && fabs(E - E_prev) <= P.tol * fabs(E)) ||
+                               (P.nnz_tol >= 0.0 && fabs(nzs - N_prev) <= P.nnz_tol * nzs);
+                    E_prev = E;
+                    N_prev = nzs;
+                    s_stop = stop;
+                    if (stop && blockIdx.x == 0) {
+                        P.ctl[0] = 1;
+                        P.ctl[1] = k;
+                        P.ctl[2] = 1;
+                    }
+                }
+            }
+            if (P.check_every > 0) {
+                __syncthreads();
+                if (s_stop) return;                          // same numbers, same decision in every CTA
+                __syncthreads();
+            }
+        }
+    }
+}
+
+// Plan-time tables of the persistent kernel: vis4[j] = 2 pi (u, v, w) as floats, x0[t][j] = centre phase (fp64, reduced).
+__global__ void __launch_bounds__(256) persist_tables_kernel(const double *u64, const double *v64, const double *w64,
+                                                             const double4 *cen, int n_vis, int n_tiles, float4 *vis4,
+                                                             float *x0) {
+    const int j = blockIdx.x * 256 + threadIdx.x;
+    if (j >= n_vis) return;
+    const double u = u64[j], v = v64[j], w = w64[j];
+    if (blockIdx.y == 0) vis4[j] = make_float4((float)(TWO_PI * u), (float)(TWO_PI * v), (float)(TWO_PI * w), 0.f);
+    for (int t = blockIdx.y; t < n_tiles; t += gridDim.y) x0[(size_t)t * n_vis + j] = centre_phase(u, v, w, cen[t]);
+}
+
+}  // namespace sl1m

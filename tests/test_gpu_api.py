@@ -268,6 +268,65 @@ def test_fp64_phase_path(sl):
         plan.close()
 
 
+@pytest.mark.parametrize("n_vis,n_pix", [(1, 1), (5, 3), (300, 1500), (1187, 2100), (2500, 700)])
+def test_persistent_small_problem_path(sl, n_vis, n_pix):
+    """Small problems run the whole FISTA loop as ONE persistent cooperative kernel (sl1m_persist.cuh; two grid
+    barriers per iteration).  Against the oracle (image, trace, stop index) and against the multi-launch loop of a
+    SL1M_NO_PERSISTENT plan (agree to rounding: the two sum in different orders); ragged sizes around the work-item
+    granularity (8 visibilities / 8 pixels per CTA, 148 CTAs), sparse iterates (warp-level zero skipping)."""
+    import torch
+    rng = np.random.default_rng(70 + n_vis)
+    l = rng.uniform(-0.03, 0.03, n_pix)
+    m = rng.uniform(-0.03, 0.03, n_pix)
+    uvw = rng.uniform(-1, 1, (n_vis, 3)) * np.array([300.0, 300.0, 40.0])
+    o = oracle.Oracle(uvw, l, m)
+    x_true = np.zeros(n_pix)
+    src = rng.choice(n_pix, max(1, n_pix // 40), replace=False)
+    x_true[src] = rng.uniform(0.5, 3.0, src.shape[0])
+    V = (o.forward(x_true) + 0.01 * (rng.standard_normal(n_vis) + 1j * rng.standard_normal(n_vis))).astype(np.complex64)
+    L = o.max_eig(30) * 1.05
+    lam = 0.05 * float(np.max(np.abs(o.adjoint(V)))) + 1e-3
+    K = 60
+    plan = sl.Plan(uvw, l, m)
+    ref_plan = sl.Plan(uvw, l, m, no_persistent=True)
+    assert plan.describe()["persistent"] == 1 and ref_plan.describe()["persistent"] == 0
+    Vd = _dev(V, torch.complex64)
+    trace = torch.zeros(3 * K, dtype=torch.float64, device="cuda")
+    n0 = plan.launch_count
+    x, info = plan.solve(Vd, lam, L=L, n_iter=K, trace=trace)
+    ref = o.fista(V, lam, L, K, want_trace=True)
+    xm, info_m = ref_plan.solve(Vd, lam, L=L, n_iter=K)
+    nrm = max(np.linalg.norm(ref["x"]), 1e-30)
+    assert np.linalg.norm(x.cpu().numpy() - ref["x"]) <= 1e-3 * nrm
+    assert float((x - xm).norm()) <= 1e-4 * max(float(xm.norm()), 1e-30)
+    assert np.all(x.cpu().numpy() >= 0)
+    tr = trace.cpu().numpy().reshape(K, 3)
+    assert np.max(np.abs(tr[:, 0] - ref["trace"][:, 0]) / np.maximum(ref["trace"][:, 0], 1e-30)) < 2e-3
+    assert np.max(np.abs(tr[:, 1] - ref["trace"][:, 1])) <= 2e-3 * max(ref["trace"][:, 1].max(), 1e-30)
+    assert np.max(np.abs(tr[:, 2] - ref["trace"][:, 2])) <= max(3, 0.05 * ref["trace"][:, 2].max())
+    assert abs(info.l2_term - ref["l2_term"]) <= 2e-3 * ref["l2_term"] + 1e-12
+    # bit-stable run to run, and stepped == one call
+    x2, _ = plan.solve(Vd, lam, L=L, n_iter=K, want_info=False)
+    assert torch.equal(x, x2)
+    plan.fista_begin(Vd, lam, L)
+    for n in (1, 7, K - 8):
+        plan.fista_step(n)
+    xs, k = plan.fista_image()
+    assert k == K and torch.equal(xs, x)
+    # stopping rule inside the kernel
+    if n_pix >= 700:
+        for tol, nnz_tol, every in ((1e-5, -1.0, 1), (-1.0, 0.0, 3), (1e-6, 0.0, 5)):
+            r = o.fista_tol(V, lam, L, max_iter=400, tol=tol, nnz_tol=nnz_tol, check_every=every)
+            xt, it = plan.solve_stop(Vd, lam, L, max_iter=400, tol=tol, nnz_tol=nnz_tol, check_every=every)
+            kk = it.n_iter_done
+            assert 2 <= kk <= 400 and (kk % every == 0 or kk == 400)
+            assert abs(kk - r["n_iter_done"]) <= 3 * every, (tol, nnz_tol, every, kk, r["n_iter_done"])
+            same = o.fista(V, lam, L, kk)["x"]
+            assert np.linalg.norm(xt.cpu().numpy() - same) <= 1e-3 * max(np.linalg.norm(same), 1e-30)
+    plan.close()
+    ref_plan.close()
+
+
 def test_fp64_phase_path_with_channels(sl):
     """sl1m_plan_set_channels on fp64-phase plans: the channel scale multiplies uvw inside the
     fp64-phase kernels; a plan just under the 256 rad limit switches to them when its highest channel exceeds
