@@ -215,7 +215,9 @@ int sl1m_dirty_image(sl1m_plan *plan, const float *vis_dev, float scale, float *
  *  - a pixel is a square of side s_k centred on (l_k, m_k); it splits iff I_k > frac * max_j I_j
  *    and s_k/2 >= min_side, and is replaced IN PLACE by four children of side s_k/2 centred on
  *    l_k -/+ s_k/4, m_k -/+ s_k/4 (l fastest); every other pixel stays (mixed sizes in one
- *    solve).  frac < 0 splits every pixel: the plain coarse-to-fine strategy.
+ *    solve).  frac < 0 splits every pixel of an image with any emission: the plain coarse-to-fine
+ *    strategy.  An image that is zero everywhere splits nothing, whatever frac is (no emission was detected: a
+ *    level solved with too large a lambda ends the refinement instead of quadrupling an empty grid).
  *  - "upscale the previously calculated solution": a child starts from I_k/4.
  *
  * sl1m_quadtree_refine -- ONE split step, pure host code (needs no GPU).  All pointers HOST.

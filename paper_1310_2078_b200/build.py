@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "sl1m.cu")
 SRC_QT = os.path.join(_HERE, "csrc", "sl1m_quadtree.cu")
 SRC_PK = os.path.join(_HERE, "csrc", "sl1m_peaks.cu")
-DEPS = [SRC, SRC_QT, SRC_PK, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"), os.path.join(_HERE, "csrc", "sl1m_persist.cuh"),
+DEPS = [SRC, SRC_QT, SRC_PK, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"), os.path.join(_HERE, "csrc", "sl1m_persist.cuh"), os.path.join(_HERE, "csrc", "sl1m_internal.h"),
         os.path.join(os.path.dirname(_HERE), "include", "sl1m.h")]
 LIB = os.path.join(_HERE, "libsl1m.so")
 LIB_BOUNDS = os.path.join(_HERE, "libsl1m_bounds.so")      # debug build: canary bands + asserted prefetches (-DSL1M_BOUNDS)

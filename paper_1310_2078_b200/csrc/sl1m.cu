@@ -17,6 +17,7 @@
 #endif
 
 #include "sl1m_epilogue.cuh"
+#include "sl1m_internal.h"
 #include "sl1m_kernels.cuh"
 #include "sl1m_persist.cuh"
 
@@ -30,6 +31,12 @@ int fail(int st, const std::string &msg) {
     g_last_error = msg;
     return st;
 }
+
+}  // namespace
+
+int sl1m_fail(int st, const char *msg) { return fail(st, msg ? msg : ""); }
+
+namespace {
 
 #define CUDA_TRY(expr)                                                                      \
     do {                                                                                    \

@@ -12,17 +12,20 @@
 #include <vector>
 
 #include "../../include/sl1m.h"
+#include "sl1m_internal.h"
 
 extern "C" int sl1m_quadtree_refine(int64_t n, const double *l, const double *m, const double *side, const float *I,
                                     double frac, double min_side, int64_t capacity, double *l_out, double *m_out,
                                     double *side_out, float *I0_out, int64_t *parent_out, int64_t *n_out,
                                     int64_t *n_refined) {
-    if (!l || !m || !side || !I || !l_out || !m_out || !side_out || !I0_out || !n_out || !n_refined) return SL1M_ERR_NULL;
-    if (n < 1 || capacity < n) return SL1M_ERR_SIZE;
-    if (!std::isfinite(frac) || !std::isfinite(min_side)) return SL1M_ERR_PARAM;
+    if (!l || !m || !side || !I || !l_out || !m_out || !side_out || !I0_out || !n_out || !n_refined)
+        return sl1m_fail(SL1M_ERR_NULL, "sl1m_quadtree_refine: NULL argument");
+    if (n < 1 || capacity < n) return sl1m_fail(SL1M_ERR_SIZE, "sl1m_quadtree_refine: n < 1 or capacity < n");
+    if (!std::isfinite(frac) || !std::isfinite(min_side)) return sl1m_fail(SL1M_ERR_PARAM, "sl1m_quadtree_refine: non-finite frac or min_side");
     double top = 0.0;
     for (int64_t k = 0; k < n; ++k) {
-        if (!std::isfinite(I[k]) || !(side[k] > 0.0) || !std::isfinite(side[k])) return SL1M_ERR_DOMAIN;
+        if (!std::isfinite(I[k]) || !(side[k] > 0.0) || !std::isfinite(side[k]))
+            return sl1m_fail(SL1M_ERR_DOMAIN, "sl1m_quadtree_refine: non-finite flux or side <= 0");
         if (k == 0 || (double)I[k] > top) top = (double)I[k];
     }
     const double thr = frac * top;
@@ -30,7 +33,7 @@ extern "C" int sl1m_quadtree_refine(int64_t n, const double *l, const double *m,
     int64_t n_split = 0;
     for (int64_t k = 0; k < n; ++k)
         if (top > 0.0 && (double)I[k] > thr && side[k] / 2.0 >= min_side) ++n_split;
-    if (n + 3 * n_split > capacity) return SL1M_ERR_SIZE;
+    if (n + 3 * n_split > capacity) return sl1m_fail(SL1M_ERR_SIZE, "sl1m_quadtree_refine: capacity < n + 3 * (pixels that split)");
     int64_t o = 0;
     for (int64_t k = 0; k < n; ++k) {
         const double half = side[k] / 2.0;
@@ -67,7 +70,7 @@ struct DevBuf {
     int alloc(size_t bytes) {
         if (p) cudaFree(p);
         p = nullptr;
-        return cudaMalloc(&p, bytes ? bytes : 1) == cudaSuccess ? SL1M_OK : SL1M_ERR_ALLOC;
+        return cudaMalloc(&p, bytes ? bytes : 1) == cudaSuccess ? SL1M_OK : sl1m_fail(SL1M_ERR_ALLOC, "sl1m_quadtree_solve: device allocation failed");
     }
 };
 struct PlanGuard {
@@ -83,11 +86,11 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
                                    int64_t capacity, double *l_out, double *m_out, double *side_out, float *x_out,
                                    int64_t *n_out, sl1m_qt_level *levels_out, int *n_levels_done, void *stream) {
     if (!uvw || !vis_host || !l0 || !m0 || !side0 || !l_out || !m_out || !side_out || !x_out || !n_out || !n_levels_done)
-        return SL1M_ERR_NULL;
-    if (n_vis < 1 || n0 < 1 || capacity < n0) return SL1M_ERR_SIZE;
+        return sl1m_fail(SL1M_ERR_NULL, "sl1m_quadtree_solve: NULL argument");
+    if (n_vis < 1 || n0 < 1 || capacity < n0) return sl1m_fail(SL1M_ERR_SIZE, "sl1m_quadtree_solve: n_vis < 1, n0 < 1 or capacity < n0");
     if (n_levels < 1 || !(L_safety > 0.f) || n_pow < 1 || max_iter < 0 || !(tol >= 0.0) || check_every < 1 ||
         !(sigma_factor >= 0.0) || !std::isfinite(sigma_factor))
-        return SL1M_ERR_PARAM;
+        return sl1m_fail(SL1M_ERR_PARAM, "sl1m_quadtree_solve: n_levels < 1, L_safety <= 0, n_pow < 1, max_iter < 0, tol < 0, check_every < 1 or sigma_factor < 0");
     cudaStream_t s = (cudaStream_t)stream;
     *n_out = 0;
     *n_levels_done = 0;
@@ -98,7 +101,7 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
         int st;
         if ((st = vis_dev.alloc((size_t)n_vis * 2 * sizeof(float)))) return st;
         if (cudaMemcpyAsync(vis_dev.p, vis_host, (size_t)n_vis * 2 * sizeof(float), cudaMemcpyHostToDevice, s) != cudaSuccess)
-            return SL1M_ERR_CUDA;
+            return sl1m_fail(SL1M_ERR_CUDA, "sl1m_quadtree_solve: copy of the visibilities to the device failed");
         for (int level = 0; level < n_levels; ++level) {
             const auto t_start = std::chrono::steady_clock::now();
             const int64_t n = (int64_t)l.size();
@@ -115,13 +118,13 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
             float L = 0.f;
             if ((st = sl1m_max_eig(plan.p, n_pow, &L, stream))) return st;
             L *= L_safety;
-            if (!(L > 0.f)) return SL1M_ERR_PARAM;
+            if (!(L > 0.f)) return sl1m_fail(SL1M_ERR_PARAM, "sl1m_quadtree_solve: power iteration returned L <= 0 (zero operator)");
             if ((st = x_dev.alloc((size_t)n * sizeof(float)))) return st;
             const float *x0p = nullptr;
             if (!x0.empty()) {
                 if ((st = x0_dev.alloc((size_t)n * sizeof(float)))) return st;
                 if (cudaMemcpyAsync(x0_dev.p, x0.data(), (size_t)n * sizeof(float), cudaMemcpyHostToDevice, s) != cudaSuccess)
-                    return SL1M_ERR_CUDA;
+                    return sl1m_fail(SL1M_ERR_CUDA, "sl1m_quadtree_solve: copy of the warm start to the device failed");
                 x0p = (const float *)x0_dev.p;
             }
             sl1m_solve_info info;
@@ -131,7 +134,7 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
             x.resize((size_t)n);
             if (cudaMemcpyAsync(x.data(), x_dev.p, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
                 cudaStreamSynchronize(s) != cudaSuccess)
-                return SL1M_ERR_CUDA;
+                return sl1m_fail(SL1M_ERR_CUDA, "sl1m_quadtree_solve: read-back of the level's image failed");
             if (levels_out) {
                 sl1m_qt_level &lv = levels_out[level];
                 lv.n_pix = n;
@@ -154,7 +157,7 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
             }
             if (n_split == 0) break;
             const int64_t n_new = n + 3 * n_split;
-            if (n_new > capacity) return SL1M_ERR_SIZE;
+            if (n_new > capacity) return sl1m_fail(SL1M_ERR_SIZE, "sl1m_quadtree_solve: capacity too small for the next level");
             std::vector<double> l2((size_t)n_new), m2((size_t)n_new), s2((size_t)n_new);
             std::vector<float> i2((size_t)n_new);
             int64_t got = 0, nref = 0;
@@ -175,7 +178,7 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
         }
         *n_out = n;
     } catch (const std::bad_alloc &) {
-        return SL1M_ERR_ALLOC;
+        return sl1m_fail(SL1M_ERR_ALLOC, "sl1m_quadtree_solve: host allocation failed");
     }
     return SL1M_OK;
 }

@@ -121,3 +121,10 @@ def test_quadtree_refine_host_logic_is_bit_exact_against_the_oracle():
                                   *(a.ctypes.data_as(ctypes.c_void_p) for a in out), None, ctypes.byref(n_out),
                                   ctypes.byref(n_ref))
     assert st == 2  # SL1M_ERR_SIZE
+    # ... and the failure carries its own detail text (not a stale one from an earlier call)
+    assert b"capacity" in lib.sl1m_last_error()
+    # an image that is zero everywhere splits nothing, also with frac < 0 (sl1m.h; the oracle agrees)
+    zero = np.zeros(4, np.float32)
+    got = sl.quadtree_refine(four[0], four[1], four[2], zero, -1.0, 0.0)
+    assert got[5] == 0 and got[0].shape[0] == 4
+    assert oracle.quadtree_refine(four[0], four[1], four[2], zero.astype(np.float64), -1.0, 0.0)[5] == 0
