@@ -198,8 +198,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     peaks, peaks_src = _peaks()
 
     wl = make_workload(args.config)
+    if args.jitter_sigma and wl.sigma is not None:      # a sigma of its own per pixel: the per-pixel-sigma Gaussian kernels
+        wl.sigma = wl.sigma * np.random.default_rng(777).uniform(0.7, 1.3, wl.n_pix)
     t_plan = time.perf_counter()
-    plan = sl.Plan.from_workload(wl, dense_forward=args.dense_forward)
+    plan = sl.Plan.from_workload(wl, dense_forward=args.dense_forward, no_persistent=args.no_persistent,
+                                 phase_fp64=args.phase_fp64)
     torch.cuda.synchronize()
     t_plan = time.perf_counter() - t_plan
     n_terms = float(wl.n_pix) * float(wl.n_vis)
@@ -446,7 +449,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "warmup": args.warmup, "ms_per_step": t_max / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"config{args.config}:{wl.name}", "n_pix": wl.n_pix, "n_vis": wl.n_vis,
-                   "pixel_kind": "gaussian" if wl.sigma is not None else "delta",
+                   "pixel_kind": ("gaussian-per-pixel-sigma" if args.jitter_sigma else "gaussian") if wl.sigma is not None else "delta",
+                   "flags": {"dense_forward": args.dense_forward, "no_persistent": args.no_persistent,
+                             "phase_fp64": args.phase_fp64},
                    "gains": wl.gains is not None, "lambda": lam, "L": L,
                    "l2_flush": "256 MiB device memset between timed steps",
                    "step": "one FISTA iteration via sl1m_fista_step(1): warm-up and timed steps are consecutive iterations "
@@ -487,6 +492,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dense-forward", action="store_true", dest="dense_forward",
                     help="SL1M_DENSE_FORWARD: the forward evaluates every term, also where the image is zero (A/B of the zero-skipping forward)")
+    ap.add_argument("--no-persistent", action="store_true", dest="no_persistent",
+                    help="SL1M_NO_PERSISTENT: small problems keep the multi-launch loop (A/B of the persistent kernel)")
+    ap.add_argument("--phase-fp64", action="store_true", dest="phase_fp64", help="SL1M_PHASE_FP64: the fp64-phase kernels")
+    ap.add_argument("--jitter-sigma", action="store_true", dest="jitter_sigma",
+                    help="Gaussian configs: multiply every sigma_k by a seeded U(0.7, 1.3) draw (per-pixel-sigma kernels)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     rank = int(os.environ.get("RANK", "0"))

@@ -324,8 +324,9 @@ int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
  * moved to the front of a compact copy of their tile, in their original order, and the forward kernel streams
  * only those; the result is the same sum with the zero terms left out.  With a gain table the gain rows of the
  * compact entries are copied next to them (one more table-sized buffer per channel; a full tile is not copied).
- * Plans with per-pixel sigma (more than 16 distinct values), with fp64 phase, or whose compact gain rows would
- * exceed 8 GiB keep the dense forward (sl1m_plan_info.zero_skip == 0), as does SL1M_DENSE_FORWARD.  The adjoint always evaluates every term.
+ * Kernels that stage a per-pixel side array next to the tile (per-pixel sigma; the fp64 offsets of the fp64-phase
+ * kernels) get a compact copy of that array as well.  Plans whose compact gain rows would exceed 8 GiB keep the dense
+ * forward (sl1m_plan_info.zero_skip == 0), as does SL1M_DENSE_FORWARD.  The adjoint always evaluates every term.
  * n_active_host: HOST [n_chan]; pixels the most recently packed forward input streams per channel (padded to
  * 4 per tile; n_pix_padded when the plan does not skip).  Synchronises `stream`.
  */

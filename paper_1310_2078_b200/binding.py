@@ -278,10 +278,11 @@ class Plan:
         return (n,) if self.n_chan == 1 else (self.n_chan, n)
 
     @classmethod
-    def from_workload(cls, wl, gains_device=None, dense_forward: bool = False, no_persistent: bool = False):
+    def from_workload(cls, wl, gains_device=None, dense_forward: bool = False, no_persistent: bool = False,
+                      phase_fp64: bool = False):
         g = wl.gains if gains_device is None else gains_device
         return cls(wl.uvw, wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, g, wl.gauss_model, dense_forward=dense_forward,
-                   no_persistent=no_persistent)
+                   no_persistent=no_persistent, phase_fp64=phase_fp64)
 
     def close(self):
         if self._h is not None:

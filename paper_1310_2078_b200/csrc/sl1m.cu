@@ -298,7 +298,8 @@ int configure_and_allocate(sl1m_plan *p) {
     const size_t npad = (size_t)p->n_pix_pad, C = (size_t)p->n_chan;
     for (void **q : {(void **)&p->ws_v, (void **)&p->ws_p, (void **)&p->resid, (void **)&p->I_sorted, (void **)&p->y_sorted,
                      (void **)&p->g_sorted, (void **)&p->part_a, (void **)&p->part_b, (void **)&p->part_c, (void **)&p->scalars,
-                     (void **)&p->pixc, (void **)&p->tile_cnt, (void **)&p->gFc, (void **)&p->rpol}) {
+                     (void **)&p->pixc, (void **)&p->tile_cnt, (void **)&p->gFc, (void **)&p->rpol, (void **)&p->pixdc,
+                     (void **)&p->pixgc}) {
         if (*q) cudaFree(*q);
         *q = nullptr;
     }
@@ -315,11 +316,19 @@ int configure_and_allocate(sl1m_plan *p) {
     CUDA_TRY(cudaMalloc((void **)&p->part_c, C * (size_t)p->n_part * sizeof(double)));
     CUDA_TRY(cudaMalloc((void **)&p->scalars, C * 4 * sizeof(double)));
     CUDA_TRY(cudaMemset(p->scalars, 0, C * 4 * sizeof(double)));
-    // zero-skipping forward: every kernel but those with a per-pixel side array in shared memory (per-pixel
-    // sigma, fp64 offsets).  Gain plans keep a compact copy of the gain rows next to the compact tiles
-    // (n_chan x the table; not beyond 8 GiB -- such a plan keeps the dense forward).
+    // zero-skipping forward: every forward kernel; the kernels with a per-pixel side array in shared memory
+    // (per-pixel sigma, fp64 offsets) get a compact copy of that array too.  Gain plans keep a compact copy of the
+    // gain rows next to the compact tiles (n_chan x the table; not beyond 8 GiB -- such a plan keeps the dense forward).
     const size_t gfc_bytes = p->gk != 0 ? (C * npad + GAIN_ROW_PAD) * (size_t)p->n_ant * sizeof(float2) : 0;
-    if (!p->dense_forward && p->pk != 1 && !p->phase64 && gfc_bytes <= ((size_t)8 << 30)) {
+    if (!p->dense_forward && gfc_bytes <= ((size_t)8 << 30)) {
+        if (p->phase64) {   // side arrays are compacted too
+            CUDA_TRY(cudaMalloc((void **)&p->pixdc, C * npad * sizeof(double4)));
+            CUDA_TRY(cudaMemset(p->pixdc, 0, C * npad * sizeof(double4)));
+        }
+        if (p->pk == 1) {
+            CUDA_TRY(cudaMalloc((void **)&p->pixgc, C * npad * sizeof(float2)));
+            CUDA_TRY(cudaMemset(p->pixgc, 0, C * npad * sizeof(float2)));
+        }
         CUDA_TRY(cudaMalloc((void **)&p->pixc, C * npad * sizeof(float4)));
         CUDA_TRY(cudaMalloc((void **)&p->tile_cnt, C * (size_t)p->n_tiles * sizeof(int)));
         CUDA_TRY(cudaMemset(p->pixc, 0, C * npad * sizeof(float4)));
@@ -340,7 +349,7 @@ int configure_and_allocate(sl1m_plan *p) {
 constexpr double PERSIST_MAX_TERMS = 67108864.0;
 int persist_setup(sl1m_plan *p) {
     p->persist = false;
-    if (p->no_persist || p->pk != 0 || p->gk != 0 || p->phase64 || p->n_tiles > PERSIST_MAX_TILES ||
+    if (p->no_persist || p->dense_forward || p->pk != 0 || p->gk != 0 || p->phase64 || p->n_tiles > PERSIST_MAX_TILES ||
         (double)p->n_pix_pad * (double)p->n_vis_int > PERSIST_MAX_TERMS)
         return SL1M_OK;
     int coop = 0, per_sm = 0, sms = 0;
@@ -650,7 +659,9 @@ namespace {
 
 inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
 inline dim3 cgrid(const sl1m_plan *p, size_t n) { return dim3((unsigned)egrid(n), (unsigned)p->n_chan); }  // x: elements, y: channel
-inline ZeroSkip zs_of(const sl1m_plan *p) { return ZeroSkip{p->pixc, p->tile_cnt, p->gF, p->gFc, p->n_ant}; }
+inline ZeroSkip zs_of(const sl1m_plan *p) {
+    return ZeroSkip{p->pixc, p->tile_cnt, p->gF, p->gFc, p->n_ant, p->pixd, p->pixdc, p->pixg, p->pixgc};
+}
 
 template <int PK, int GK, bool B>
 void launch_fwd_rv(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStream_t s) {
@@ -712,19 +723,21 @@ void launch_fwd(sl1m_plan *p, cudaStream_t s) {
     ApplyParams P = make_params(p);
     P.per_split = p->fwd_per_split;
     dim3 grid(p->fwd_vtiles, p->fwd_split, p->n_chan);
-    if (p->phase64) {
-        switch (p->fwd_rv) {
-            case 4: fwd_kernel_p64<4><<<grid, NT, 0, s>>>(P, p->pixd); break;
-            case 2: fwd_kernel_p64<2><<<grid, NT, 0, s>>>(P, p->pixd); break;
-            default: fwd_kernel_p64<1><<<grid, NT, 0, s>>>(P, p->pixd); break;
-        }
-        p->launches++;
-        return;
-    }
     if (p->pixc) {   // zero-skipping: stream the compact tiles the packing kernel left behind
         P.pix4 = p->pixc;
         P.tile_cnt = p->tile_cnt;
         P.gFc = p->gFc;
+        if (p->pixgc) P.pixg = p->pixgc;
+    }
+    if (p->phase64) {
+        const double4 *pd = p->pixc ? p->pixdc : p->pixd;
+        switch (p->fwd_rv) {
+            case 4: fwd_kernel_p64<4><<<grid, NT, 0, s>>>(P, pd); break;
+            case 2: fwd_kernel_p64<2><<<grid, NT, 0, s>>>(P, pd); break;
+            default: fwd_kernel_p64<1><<<grid, NT, 0, s>>>(P, pd); break;
+        }
+        p->launches++;
+        return;
     }
     const int key = p->pk * 3 + p->gk;   // pk == 2 (one sigma per tile) only exists with unit gains
     switch (key) {
@@ -746,6 +759,10 @@ void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
     P.r = r;
     dim3 grid(p->adj_pgroups, p->adj_split, p->n_chan);
     if (p->phase64) {
+        // one cosine per term here too: the kernel reads the residual in polar form
+        vis_polar_kernel<<<dim3((unsigned)egrid((size_t)p->n_vis_int), (unsigned)p->n_chan), ET, 0, s>>>(P.r, p->rpol, p->n_vis_int, p->done_ptr);
+        P.r = p->rpol;
+        p->launches++;
         switch (p->adj_rp) {
             case 4: adj_kernel_p64<4><<<grid, NT, 0, s>>>(P, p->pixd); break;
             case 2: adj_kernel_p64<2><<<grid, NT, 0, s>>>(P, p->pixd); break;
@@ -1325,6 +1342,7 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     o->zero_skip = p->pixc != nullptr;
     o->persistent = p->persist && !p->chan_scale;
     o->adj_mufu_per_term = o->mufu_per_term_mufu_path;
+    if (p->phase64) o->adj_mufu_per_term = 1;      // adj_kernel_p64: |r| cos(X + arg r)
     if (!p->phase64) {
         if (p->pk == 0) o->adj_mufu_per_term = 1;    // delta pixels: one cosine per term in every adjoint kernel
 #ifdef SL1M_ADJ_TWO_MUFU

@@ -39,6 +39,11 @@ struct ZeroSkip {
     const float2 *gF;    // DEV [n_pix_pad][n_ant] or NULL (unit gains)
     float2 *gFc;         // DEV [n_chan][n_pix_pad][n_ant]
     int n_ant;
+    // per-pixel side arrays of the kernels that stage one next to the pixel tile: compacted with it
+    const double4 *pixd; // DEV [n_pix_pad] fp64 offsets (fp64-phase plans) or NULL
+    double4 *pixdc;      // DEV [n_chan][n_pix_pad]
+    const float2 *pixg;  // DEV [n_pix_pad] (sigma^2, -pi log2(e) sigma^2) (per-pixel-sigma plans) or NULL
+    float2 *pixgc;       // DEV [n_chan][n_pix_pad]
 };
 static_assert(ET == TP, "one packing CTA per pixel tile");
 __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int n_pix_pad, float4 v) {
@@ -59,8 +64,11 @@ __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int
     }
     float4 *tile = zs.pixc + chan * n_pix_pad + (size_t)blockIdx.x * TP;
     const int cnt4 = (total + 3) & ~3;
+    const size_t k_own = (size_t)blockIdx.x * TP + threadIdx.x, side0 = chan * n_pix_pad + (size_t)blockIdx.x * TP;
     if (cnt4 == TP) {                                    // (nearly) full: keep the ORIGINAL order -- the gain kernels read
         tile[threadIdx.x] = v;                           // the rows of a tile with TP entries from the table itself
+        if (zs.pixdc) zs.pixdc[side0 + threadIdx.x] = zs.pixd[k_own];
+        if (zs.pixgc) zs.pixgc[side0 + threadIdx.x] = zs.pixg[k_own];
         if (threadIdx.x == 0) zs.cnt[chan * (size_t)(n_pix_pad / TP) + blockIdx.x] = TP;
         return;                                          // uniform over the CTA
     }
@@ -68,8 +76,14 @@ __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int
         const int pos = base + __popc(b & ((1u << lane) - 1u));
         tile[pos] = v;
         s_src[pos] = (uint8_t)threadIdx.x;
+        if (zs.pixdc) zs.pixdc[side0 + pos] = zs.pixd[k_own];
+        if (zs.pixgc) zs.pixgc[side0 + pos] = zs.pixg[k_own];
     }
-    if ((int)threadIdx.x < cnt4 - total) tile[total + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if ((int)threadIdx.x < cnt4 - total) {               // padding entries: a*x = 0 and finite side values
+        tile[total + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (zs.pixdc) zs.pixdc[side0 + total + threadIdx.x] = make_double4(0.0, 0.0, 0.0, 0.0);
+        if (zs.pixgc) zs.pixgc[side0 + total + threadIdx.x] = make_float2(0.f, 0.f);
+    }
     if (threadIdx.x == 0) zs.cnt[chan * (size_t)(n_pix_pad / TP) + blockIdx.x] = cnt4;
     if (zs.gF && total > 0) {                            // gain rows of the compact entries (padding: a*x = 0, any row)
         __syncthreads();

@@ -432,18 +432,21 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS :
     // entries are samples of ONE baseline (p, q): the gain product G is loaded once per pixel.
     static_assert(GK != 2 || RV == 8, "grouped gains need RV == 8");
 
-    constexpr bool ZSKIP = (PK != 1);   // zero-skipping: every kernel but the per-pixel-sigma ones (side array in smem)
+    constexpr bool ZSKIP = true;        // zero-skipping in every variant; PK == 1 streams the compact copy of its side array too
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
+    // P.pixg: the plan's [n_pix_pad] array, or with zero-skipping its per-channel compact copy [n_chan][n_pix_pad]
+    const float2 *pixg = (PK == 1 && P.tile_cnt) ? P.pixg + chan_index<BATCH>() * P.n_pix_pad : P.pixg;
     auto issue = [&](int t, int st) {
-        const uint32_t b4 = (uint32_t)(ZSKIP ? max(tile_pixels<BATCH>(P, t), 4) : TP) * (uint32_t)sizeof(float4);
-        mbar_expect_tx(&s_bar[st], b4 + (PK == 1 ? TP * (uint32_t)sizeof(float2) : 0u));
+        const uint32_t n4 = (uint32_t)(ZSKIP ? max(tile_pixels<BATCH>(P, t), 4) : TP);
+        const uint32_t b4 = n4 * (uint32_t)sizeof(float4);
+        mbar_expect_tx(&s_bar[st], b4 + (PK == 1 ? n4 * (uint32_t)sizeof(float2) : 0u));
         tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, b4, &s_bar[st]);
-        if (PK == 1) tma_bulk_g2s(&s_pixg[st][0], P.pixg + (size_t)t * TP, TP * sizeof(float2), &s_bar[st]);
+        if (PK == 1) tma_bulk_g2s(&s_pixg[st][0], pixg + (size_t)t * TP, n4 * (uint32_t)sizeof(float2), &s_bar[st]);
     };
     if (tid == 0) {
         if (t0 < t1) issue(t0, 0);
@@ -1604,17 +1607,20 @@ __global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, con
         re[r] = 0.f;
         im[r] = 0.f;
     }
-    constexpr uint32_t kBytes = TP * (sizeof(float4) + sizeof(double4));
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
+    // zero-skipping: pix4 / pixd are then the per-channel COMPACT copies and tile_cnt the entries to stream
+    const int *tcnt = P.tile_cnt ? P.tile_cnt + (size_t)blockIdx.z * P.n_tiles : nullptr;
+    if (tcnt) pixd += (size_t)blockIdx.z * P.n_pix_pad;
     auto issue = [&](int t, int st) {
-        mbar_expect_tx(&s_bar[st], kBytes);
-        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, TP * sizeof(float4), &s_bar[st]);
-        tma_bulk_g2s(&s_pixd[st][0], pixd + (size_t)t * TP, TP * sizeof(double4), &s_bar[st]);
+        const uint32_t n4 = (uint32_t)(tcnt ? max(__ldg(tcnt + t), 4) : TP);
+        mbar_expect_tx(&s_bar[st], n4 * (uint32_t)(sizeof(float4) + sizeof(double4)));
+        tma_bulk_g2s(&s_pix[st][0], pix4 + (size_t)t * TP, n4 * (uint32_t)sizeof(float4), &s_bar[st]);
+        tma_bulk_g2s(&s_pixd[st][0], pixd + (size_t)t * TP, n4 * (uint32_t)sizeof(double4), &s_bar[st]);
     };
     if (tid == 0) {
         if (t0 < t1) issue(t0, 0);
@@ -1631,8 +1637,9 @@ __global__ void __launch_bounds__(NT, 3) fwd_kernel_p64(const ApplyParams P, con
             x0[r] = tt - rint(tt);
         }
         mbar_wait(&s_bar[st], parity);
+        const int npx = tcnt ? __ldg(tcnt + t) : TP;
 #pragma unroll 2
-        for (int p = 0; p < TP; ++p) {
+        for (int p = 0; p < npx; ++p) {
             const double4 pd = s_pixd[st][p];
             const float wt = s_pix[st][p].w;
 #pragma unroll
@@ -1660,8 +1667,8 @@ __global__ void __launch_bounds__(NT, 3) adj_kernel_p64(const ApplyParams P, con
     if (P.done && P.done[blockIdx.z]) return;   // this channel's solve has met its stopping rule
     constexpr int NCEN = (NT * RP > TP) ? (NT * RP / TP) : 1;
     __shared__ __align__(32) double4 s_vis[2][VC];       // (u, v, w, 0) in wavelengths
-    __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, r_im)
-    __shared__ double s_x0[2][VC][NCEN];                 // frac(u l_c + v m_c + w n'_c), turns
+    __shared__ __align__(8) float2 s_r[2][VC];           // residual in polar form (|r|, arg r): one cosine per term
+    __shared__ double s_x0[2][VC][NCEN];                 // frac(u l_c + v m_c + w n'_c) + arg r / 2 pi, turns
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int base = blockIdx.x * (NT * RP);
     const int kfirst = base + warp * (32 * RP);
@@ -1698,7 +1705,7 @@ __global__ void __launch_bounds__(NT, 3) adj_kernel_p64(const ApplyParams P, con
         for (int c = 0; c < NCEN; ++c) {
             const double4 cen = P.cen[tile0 + c];
             const double tt = fma(u, cen.x, fma(v, cen.y, w * cen.z));
-            s_x0[buf][tid][c] = tt - rint(tt);
+            s_x0[buf][tid][c] = (tt - rint(tt)) + (double)rr.y * (1.0 / TWO_PI);
         }
     };
     if (c0 < c1) stage(c0, 0);
@@ -1714,9 +1721,7 @@ __global__ void __launch_bounds__(NT, 3) adj_kernel_p64(const ApplyParams P, con
 #pragma unroll
             for (int i = 0; i < RP; ++i) {
                 const float X = phase64_to_radians(fma(vv.x, dl[i], fma(vv.y, dm[i], fma(vv.z, dn[i], x0))));
-                float s, c;
-                __sincosf(X, &s, &c);
-                acc[i] = fmaf(c, rr.x, fmaf(-s, rr.y, acc[i]));   // Re (c + i s)(r_re + i r_im)
+                acc[i] = fmaf(rr.x, __cosf(X), acc[i]);           // Re e^{iX} r = |r| cos(X + arg r)
             }
         }
         __syncthreads();

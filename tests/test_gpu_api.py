@@ -404,13 +404,15 @@ def test_gain_table_with_more_than_65535_rows(sl):
     plan.close()
 
 
-@pytest.mark.parametrize("kind", ["delta", "gauss_tiles", "delta_small", "gains_grouped", "gains_per_term"])
+@pytest.mark.parametrize("kind", ["delta", "gauss_tiles", "delta_small", "gains_grouped", "gains_per_term", "gauss_pixel",
+                                  "fp64_phase"])
 def test_zero_skipping_forward(sl, kind):
     """The forward streams only pixels with x_k != 0 (sl1m_forward_active_pixels; eq (18), PAPER.md:194-197,
     makes the iterates sparse).  Against the oracle and against a SL1M_DENSE_FORWARD plan: an all-zero image,
     one source, tiles holding 1..5 non-zeros (ragged padding to 4), 1 % and 60 % random density, a dense image;
     the packed R = 8 kernels, the one-sigma-per-tile Gaussian kernels, the scalar small-problem kernels, and the
-    two gain-table kernels (gain rows are looked up through the compact entries' original index)."""
+    two gain-table kernels (gain rows are looked up through the compact entries' original index), the per-pixel-sigma
+    Gaussian kernels and the fp64-phase kernels (their per-pixel side arrays are compacted with the tile)."""
     import torch
     rng = np.random.default_rng(11)
     if kind == "delta_small":
@@ -421,6 +423,13 @@ def test_zero_skipping_forward(sl, kind):
         wl = make_workload(4, n_side=64, n_ant=20, n_steps=8, n_src=50)      # gk == 2
     elif kind == "gains_per_term":
         wl = make_workload(4, n_side=64, n_ant=20, n_steps=2, n_src=50)      # gk == 1
+    elif kind == "gauss_pixel":
+        wl = make_workload(3, n_side=64, n_steps=4, n_src=30)
+        wl.sigma = wl.sigma * rng.uniform(0.7, 1.3, wl.n_pix)                # a sigma of its own per pixel: PK == 1
+    elif kind == "fp64_phase":
+        wl = make_workload(1, n_side=64)
+        wl.uvw = wl.uvw * 30.0                                               # 30 km baselines: fp64-phase kernels
+        wl.uvw[:, 2] = 200.0 * rng.uniform(-1, 1, wl.n_vis)
     else:
         wl = make_workload(3, n_side=64, n_steps=4, n_src=30)
     o = oracle.Oracle.from_workload(wl)
@@ -429,6 +438,10 @@ def test_zero_skipping_forward(sl, kind):
     assert plan.describe()["zero_skip"] == 1 and dense.describe()["zero_skip"] == 0
     if kind.startswith("gains"):
         assert plan.describe()["gains"] == (2 if kind == "gains_grouped" else 1)
+    if kind == "gauss_pixel":
+        assert plan.describe()["gaussian"] == 1
+    if kind == "fp64_phase":
+        assert plan.describe()["phase_fp64"] == 1 and plan.describe()["adj_mufu_per_term"] == 1
     n = wl.n_pix
     cases = {}
     cases["zero"] = np.zeros(n, np.float32)
