@@ -141,7 +141,7 @@ def run_reference(args, rank: int):
     """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
     if rank != 0:
         return
-    wl = make_workload(args.config)
+    wl = make_workload(args.config, **args.overrides)
     for _ in range(args.warmup):
         _oracle_sample(wl, 0.5)
     vals, secs = [], []
@@ -197,7 +197,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     sl.load_library()
     peaks, peaks_src = _peaks()
 
-    wl = make_workload(args.config)
+    wl = make_workload(args.config, **args.overrides)
     if args.jitter_sigma and wl.sigma is not None:      # a sigma of its own per pixel: the per-pixel-sigma Gaussian kernels
         wl.sigma = wl.sigma * np.random.default_rng(777).uniform(0.7, 1.3, wl.n_pix)
     t_plan = time.perf_counter()
@@ -448,7 +448,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": t_max / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"config{args.config}:{wl.name}", "n_pix": wl.n_pix, "n_vis": wl.n_vis,
+        "config": {"workload": f"config{args.config}:{wl.name}" + (f" overrides={args.overrides}" if args.overrides else ""),
+                   "n_pix": wl.n_pix, "n_vis": wl.n_vis,
                    "pixel_kind": ("gaussian-per-pixel-sigma" if args.jitter_sigma else "gaussian") if wl.sigma is not None else "delta",
                    "flags": {"dense_forward": args.dense_forward, "no_persistent": args.no_persistent,
                              "phase_fp64": args.phase_fp64},
@@ -497,7 +498,11 @@ def main():
     ap.add_argument("--phase-fp64", action="store_true", dest="phase_fp64", help="SL1M_PHASE_FP64: the fp64-phase kernels")
     ap.add_argument("--jitter-sigma", action="store_true", dest="jitter_sigma",
                     help="Gaussian configs: multiply every sigma_k by a seeded U(0.7, 1.3) draw (per-pixel-sigma kernels)")
+    ap.add_argument("--override", action="append", default=[], metavar="KEY=VALUE",
+                    help="workloads.make_workload override for side measurements, e.g. n_steps=2 (config 4 with 2 samples per "
+                         "baseline: per-term gain kernels); the default line uses none")
     args = ap.parse_args()
+    args.overrides = {k: (float(v) if "." in v else int(v)) for k, v in (o.split("=", 1) for o in args.override)}
     args.warmup = max(args.warmup, 0)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

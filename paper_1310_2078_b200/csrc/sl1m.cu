@@ -574,6 +574,19 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
                     }
                     s0 = s1;
                 }
+            } else {
+                // Per-term gains (baselines with too few samples to group): still ORDER the visibilities by antenna
+                // pair.  A warp's 32 consecutive visibilities then share p and have consecutive q, so its two gain
+                // loads per term hit one 8-byte word (broadcast) and one contiguous 256-byte run of the pixel's gain
+                // row instead of 32 scattered words; in the adjoint consecutive staged visibilities reuse the
+                // antenna-p row from L1.
+                vperm.assign(order.begin(), order.end());
+                ip.resize((size_t)n_vis);
+                iq.resize((size_t)n_vis);
+                for (int64_t js = 0; js < n_vis; ++js) {
+                    ip[(size_t)js] = ant_p[order[(size_t)js]];
+                    iq[(size_t)js] = ant_q[order[(size_t)js]];
+                }
             }
         }
         const size_t nvi = (size_t)p->n_vis_int;
