@@ -33,10 +33,13 @@
  *   R8  FISTA momentum per Beck & Teboulle 2009a (the cited source):
  *       t_{k+1} = (1 + sqrt(1 + 4 t_k^2))/2,  y_{k+1} = I_k + ((t_k - 1)/t_{k+1})(I_k - I_{k-1}).
  *   R15 sigma_k == 0 always uses eq (9), whatever the plan's Gaussian model.
+ *   R21 termination on the total error: E_k = ||M y_k - V||^2 + 2 lambda sum I_k (eq (10) with lambda_paper = 2 lambda).
+ *   R24 termination on the support size: |nnz(I_k) - nnz(I_{k-1})| <= nnz_tol nnz(I_k); either rule stops ("or").
  *
  * Parity pins: tests/test_oracle_*.py (closed forms, limits, brute-force quadrature of eq (15)
  * and of eq (4), adjoint identity, T^d hand values, t-sequence, DFT-lattice one-step FISTA, KKT,
- * sparse recovery, L bounds).  Nothing here is "parity unpinned".
+ * sparse recovery, L bounds, E_K = 2 F* against scipy NNLS, stop indices recomputed from the fixed-K iterates).
+ * Nothing here is "parity unpinned".
  */
 #include <complex.h>
 #include <math.h>

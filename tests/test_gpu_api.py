@@ -327,6 +327,19 @@ def test_persistent_small_problem_path(sl, n_vis, n_pix):
     ref_plan.close()
 
 
+def test_measure_peaks_is_sane(sl):
+    """sl1m_measure_peaks (csrc/sl1m_peaks.cu): the roofline denominators bench.py uses.  B200: 16 MUFU results and
+    128 fp32 FMA lanes per clock per SM nominal; a sustained chain of independent instructions reaches 93-100 % of both."""
+    pk = sl.measure_peaks()
+    assert pk["n_sm"] == 148
+    assert 14.5 <= pk["mufu_per_clk_sm"] <= 16.1, pk
+    assert 14.0 <= pk["mufu_cos_per_clk_sm"] <= 16.1, pk
+    assert 112.0 <= pk["ffma_per_clk_sm"] <= 128.5, pk
+    assert 112.0 <= pk["ffma2_lanes_per_clk_sm"] <= 128.5, pk
+    assert pk["coissue_mufu_per_clk_sm"] <= pk["mufu_per_clk_sm"] * 1.01
+    assert abs(pk["mufu_per_s"] / (148 * pk["sm_clock_mhz"] * 1e6) - pk["mufu_per_clk_sm"]) < 1e-6 * pk["mufu_per_clk_sm"] + 1e-9
+
+
 def test_fp64_phase_path_with_channels(sl):
     """sl1m_plan_set_channels on fp64-phase plans: the channel scale multiplies uvw inside the
     fp64-phase kernels; a plan just under the 256 rad limit switches to them when its highest channel exceeds
