@@ -244,14 +244,18 @@ def quadtree_refine(l, m, side, I, frac: float, min_side: float):
 
 def quadtree_solve(uvw, V, l0, m0, side0, n_levels: int, frac: float, min_side: float, lam: float,
                    n_pow: int, L_safety: float, max_iter: int, tol: float, check_every: int = 1,
-                   sigma_factor: float = 0.0, gauss_model: int = 1):
-    """The driver: solve, refine, warm-start, repeat (at most n_levels solves)."""
+                   sigma_factor: float = 0.0, gauss_model: int = 1, ant_p=None, ant_q=None, gains0=None):
+    """The driver: solve, refine, warm-start, repeat (at most n_levels solves).
+    gains0 [n_ant][n0] (with ant_p, ant_q): direction-dependent gains on the starting pixel list.  The paper says
+    nothing about gains under refinement; reading R25: a child inherits the gain column of its parent
+    (the beam is taken as constant over a pixel that is being split)."""
     l, m, side = (np.asarray(a, dtype=np.float64).copy() for a in (l0, m0, side0))
+    gains = None if gains0 is None else np.asarray(gains0).astype(np.complex64)
     x0 = None
     levels = []
     for level in range(int(n_levels)):
         sigma = np.where(side / 2.0 >= min_side, sigma_factor * side, 0.0) if sigma_factor > 0 else None
-        o = Oracle(uvw, l, m, sigma, gauss_model=gauss_model)
+        o = Oracle(uvw, l, m, sigma, ant_p, ant_q, gains, gauss_model=gauss_model)
         L = o.max_eig(n_pow) * L_safety
         r = o.fista_tol(V, lam, L, max_iter, tol, check_every, x0=x0)
         I = r["x"]
@@ -259,8 +263,10 @@ def quadtree_solve(uvw, V, l0, m0, side0, n_levels: int, frac: float, min_side: 
                            l1_term=r["l1_term"], nnz=r["nnz"]))
         if level == n_levels - 1:
             break
-        l2, m2, s2, x2, _, n_ref = quadtree_refine(l, m, side, I, frac, min_side)
+        l2, m2, s2, x2, parent, n_ref = quadtree_refine(l, m, side, I, frac, min_side)
         if n_ref == 0:
             break
         l, m, side, x0 = l2, m2, s2, x2
+        if gains is not None:
+            gains = np.ascontiguousarray(gains[:, parent])            # reading R25
     return dict(l=l, m=m, side=side, x=I, levels=levels)

@@ -109,3 +109,48 @@ def test_quadtree_driver_finds_a_sparse_sky_with_few_pixels():
     bad = oracle.quadtree_solve(uvw, V, l0, m0, np.full(64, field / 8), n_levels=4, frac=0.01, min_side=df * 0.999,
                                 lam=lam, n_pow=30, L_safety=1.05, max_iter=400, tol=1e-7, check_every=10)
     assert bad["levels"][-1]["l2_term"] > 0.2 * np.sum(np.abs(V) ** 2)
+
+
+def test_quadtree_with_inherited_gains():
+    """Reading R25: under refinement a child inherits the gain column of its parent.
+    (i) gains constant over the sky, g_a(k) = c_a: then G_j = c_p conj(c_q) factors out of row j, so the driver on
+        (V, gains) must walk exactly the tree, and return exactly the fluxes, of the unit-gain driver on the rows
+        rescaled to unit gain -- here |c_a| = 1, so M_gain = D M with D unitary-diagonal and Re M^H D^H D M = Re M^H M:
+        same L, same iterates, same splits, with V' = conj(G) V.
+    (ii) a direction-dependent table: after one refine-all step the level-2 problem is the oracle's own operator
+        on the children with gains[:, parent] -- checked against an explicitly built child table."""
+    rng = np.random.default_rng(91)
+    n_ant = 7
+    ant = rng.uniform(-150, 150, (n_ant, 2))
+    p, q = np.triu_indices(n_ant, 1)
+    uv = np.concatenate([(ant[p] - ant[q]) @ np.array([[np.cos(t), -np.sin(t)], [np.sin(t), np.cos(t)]]).T
+                         for t in (0.0, 0.7, 1.9)])
+    uvw = np.concatenate([uv, rng.uniform(-5, 5, (uv.shape[0], 1))], 1)
+    ap, aq = np.tile(p, 3).astype(np.int32), np.tile(q, 3).astype(np.int32)
+    N, field = 4, 0.04
+    l0, m0 = _grid(N, field / N)
+    side0 = np.full(N * N, field / N)
+    lf, mf = _grid(4 * N, field / (4 * N))
+    x_true = np.zeros(16 * N * N)
+    x_true[rng.choice(16 * N * N, 5, replace=False)] = rng.uniform(1, 3, 5)
+    c = np.exp(1j * rng.uniform(-np.pi, np.pi, n_ant))
+    G = c[ap] * np.conj(c[aq])
+    V_unit = oracle.Oracle(uvw, lf, mf).forward(x_true)
+    V = G * V_unit
+    kw = dict(n_levels=3, frac=0.05, min_side=field / (4 * N) * 0.999, lam=0.05, n_pow=40, L_safety=1.05, max_iter=150,
+              tol=1e-9, check_every=5, sigma_factor=1.0)
+    a = oracle.quadtree_solve(uvw, V, l0, m0, side0, ant_p=ap, ant_q=aq, gains0=np.repeat(c[:, None], N * N, 1), **kw)
+    b = oracle.quadtree_solve(uvw, V_unit, l0, m0, side0, **kw)
+    assert [lv["n_pix"] for lv in a["levels"]] == [lv["n_pix"] for lv in b["levels"]] and len(a["levels"]) == 3
+    assert np.array_equal(a["l"], b["l"]) and np.array_equal(a["side"], b["side"])
+    assert np.max(np.abs(a["x"] - b["x"])) < 1e-6 * np.max(b["x"])
+    # (ii)
+    g0 = (1.0 + 0.3 * (rng.standard_normal((n_ant, N * N)) + 1j * rng.standard_normal((n_ant, N * N)))).astype(np.complex64)
+    r = oracle.quadtree_solve(uvw, V, l0, m0, side0, n_levels=2, frac=-1.0, min_side=0.0, lam=0.05, n_pow=20,
+                              L_safety=1.05, max_iter=40, tol=-1.0, ant_p=ap, ant_q=aq, gains0=g0)
+    l1, m1, s1, x1, parent, _ = oracle.quadtree_refine(l0, m0, side0, oracle.Oracle(
+        uvw, l0, m0, None, ap, aq, g0).fista_tol(V, 0.05, oracle.Oracle(uvw, l0, m0, None, ap, aq, g0).max_eig(20) * 1.05,
+                                                 40, -1.0)["x"], -1.0, 0.0)
+    child = oracle.Oracle(uvw, l1, m1, None, ap, aq, np.stack([g0[a_][parent] for a_ in range(n_ant)]))
+    want = child.fista_tol(V, 0.05, child.max_eig(20) * 1.05, 40, -1.0, x0=x1)["x"]
+    assert np.array_equal(r["l"], l1) and np.max(np.abs(r["x"] - want)) < 1e-9 * max(np.max(want), 1e-30)
