@@ -246,7 +246,7 @@ typedef struct {
  * started from the upscaled previous level, split }.  Stops early when no pixel splits.
  * Pixels that can still split are Gaussian pixels of sigma_k = sigma_factor * s_k (eq 16/17 by
  * gauss_model), pixels at the resolution limit (s_k/2 < min_side) and all pixels when
- * sigma_factor == 0 are delta pixels (eq 9).  Unit gains.
+ * sigma_factor == 0 are delta pixels (eq 9).  Unit gains (sl1m_quadtree_solve_gains takes a gain table).
  *   uvw HOST [n_vis][3] fp64; vis_host HOST [n_vis][2] fp32; l0, m0, side0 HOST [n0] fp64.
  *   outputs HOST [capacity]: final leaves (l, m, side) and their fluxes x; *n_out leaves.
  *   levels_out HOST [n_levels] or NULL; *n_levels_done.  Synchronises `stream` at every level.
@@ -258,6 +258,21 @@ int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float *vis_host,
                         int check_every, int64_t capacity, double *l_out, double *m_out,
                         double *side_out, float *x_out, int64_t *n_out, sl1m_qt_level *levels_out,
                         int *n_levels_done, void *stream);
+
+/*
+ * sl1m_quadtree_solve_gains -- the same driver with direction-dependent gains: ant_p, ant_q HOST [n_vis] int32 and
+ * gains0_host HOST [n_ant][n0][2] fp32, the gain table ON THE STARTING PIXEL LIST.  The paper does not say what the
+ * gains of a refined pixel are; reading R25: a child inherits the gain column of its parent (the beam is
+ * taken as constant over a pixel that is being split).  Everything else as sl1m_quadtree_solve.
+ */
+int sl1m_quadtree_solve_gains(int64_t n_vis, const double *uvw, const float *vis_host,
+                              const int32_t *ant_p, const int32_t *ant_q, int32_t n_ant,
+                              const float *gains0_host, int64_t n0, const double *l0, const double *m0,
+                              const double *side0, int n_levels, double frac, double min_side,
+                              double sigma_factor, int gauss_model, float lambda, float L_safety, int n_pow,
+                              int max_iter, double tol, int check_every, int64_t capacity, double *l_out,
+                              double *m_out, double *side_out, float *x_out, int64_t *n_out,
+                              sl1m_qt_level *levels_out, int *n_levels_done, void *stream);
 
 /*
  * Batched channels (NEXT-4 of the scope table).  The paper's data sets are 61-127 spectral channels

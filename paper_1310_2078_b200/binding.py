@@ -119,6 +119,10 @@ def load_library():
                                         f32, f32, ctypes.c_int, ctypes.c_int, f64, ctypes.c_int, i64, vp, vp, vp,
                                         vp, ctypes.POINTER(i64), ctypes.POINTER(_QtLevel),
                                         ctypes.POINTER(ctypes.c_int), vp]
+    lib.sl1m_quadtree_solve_gains.argtypes = [i64, vp, vp, vp, vp, i32, vp, i64, vp, vp, vp, ctypes.c_int, f64, f64, f64,
+                                              ctypes.c_int, f32, f32, ctypes.c_int, ctypes.c_int, f64, ctypes.c_int, i64,
+                                              vp, vp, vp, vp, ctypes.POINTER(i64), ctypes.POINTER(_QtLevel),
+                                              ctypes.POINTER(ctypes.c_int), vp]
     lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
     lib.sl1m_forward_active_pixels.argtypes = [vp, vp, vp]
     lib.sl1m_measure_peaks.argtypes = [ctypes.POINTER(_Peaks), vp]
@@ -198,9 +202,9 @@ def quadtree_refine(l, m, side, I, frac: float, min_side: float):
 def quadtree_solve(uvw, vis, l0, m0, side0, n_levels: int, frac: float, min_side: float, lam: float,
                    n_pow: int = 30, L_safety: float = 1.05, max_iter: int = 1000, tol: float = 1e-6,
                    check_every: int = 10, sigma_factor: float = 1.0, gauss_model: int = 1, capacity: int = None,
-                   stream=None):
-    """sl1m_quadtree_solve: coarse-to-fine / adaptive quadtree driver.
-    Host arrays in, host arrays out: dict(l, m, side, x, levels=[...])."""
+                   stream=None, ant_p=None, ant_q=None, gains0=None):
+    """sl1m_quadtree_solve (sl1m_quadtree_solve_gains when gains0 [n_ant][n0] complex64 is given): coarse-to-fine /
+    adaptive quadtree driver.  Host arrays in, host arrays out: dict(l, m, side, x, levels=[...])."""
     uvw = np.ascontiguousarray(uvw, dtype=np.float64)
     vis = np.ascontiguousarray(vis, dtype=np.complex64)
     l0, m0, side0 = (np.ascontiguousarray(a, dtype=np.float64) for a in (l0, m0, side0))
@@ -209,11 +213,24 @@ def quadtree_solve(uvw, vis, l0, m0, side0, n_levels: int, frac: float, min_side
     lo, mo, so, xo = np.empty(cap), np.empty(cap), np.empty(cap), np.empty(cap, np.float32)
     levels = (_QtLevel * max(int(n_levels), 1))()
     n_out, n_done = ctypes.c_int64(0), ctypes.c_int(0)
-    _check(load_library().sl1m_quadtree_solve(
-        int(uvw.shape[0]), _np_ptr(uvw), _np_ptr(vis), n0, _np_ptr(l0), _np_ptr(m0), _np_ptr(side0), int(n_levels),
-        float(frac), float(min_side), float(sigma_factor), int(gauss_model), float(lam), float(L_safety), int(n_pow),
-        int(max_iter), float(tol), int(check_every), cap, _np_ptr(lo), _np_ptr(mo), _np_ptr(so), _np_ptr(xo),
-        ctypes.byref(n_out), levels, ctypes.byref(n_done), _stream_ptr(stream)))
+    if gains0 is not None:
+        g = np.ascontiguousarray(gains0, dtype=np.complex64)
+        ap = np.ascontiguousarray(ant_p, dtype=np.int32)
+        aq = np.ascontiguousarray(ant_q, dtype=np.int32)
+        if g.ndim != 2 or g.shape[1] != n0 or ap.shape[0] != uvw.shape[0] or aq.shape[0] != uvw.shape[0]:
+            raise ValueError("gains0 must be [n_ant][n0]; ant_p, ant_q [n_vis]")
+        _check(load_library().sl1m_quadtree_solve_gains(
+            int(uvw.shape[0]), _np_ptr(uvw), _np_ptr(vis), _np_ptr(ap), _np_ptr(aq), int(g.shape[0]), _np_ptr(g), n0,
+            _np_ptr(l0), _np_ptr(m0), _np_ptr(side0), int(n_levels), float(frac), float(min_side), float(sigma_factor),
+            int(gauss_model), float(lam), float(L_safety), int(n_pow), int(max_iter), float(tol), int(check_every), cap,
+            _np_ptr(lo), _np_ptr(mo), _np_ptr(so), _np_ptr(xo), ctypes.byref(n_out), levels, ctypes.byref(n_done),
+            _stream_ptr(stream)))
+    else:
+        _check(load_library().sl1m_quadtree_solve(
+            int(uvw.shape[0]), _np_ptr(uvw), _np_ptr(vis), n0, _np_ptr(l0), _np_ptr(m0), _np_ptr(side0), int(n_levels),
+            float(frac), float(min_side), float(sigma_factor), int(gauss_model), float(lam), float(L_safety), int(n_pow),
+            int(max_iter), float(tol), int(check_every), cap, _np_ptr(lo), _np_ptr(mo), _np_ptr(so), _np_ptr(xo),
+            ctypes.byref(n_out), levels, ctypes.byref(n_done), _stream_ptr(stream)))
     k = n_out.value
     lv = [dict(n_pix=int(q.n_pix), L=float(q.L), n_iter_done=int(q.n_iter_done), l2_term=float(q.l2_term),
                l1_term=float(q.l1_term), nnz=int(q.nnz), seconds=float(q.seconds)) for q in levels[:n_done.value]]

@@ -79,7 +79,10 @@ struct PlanGuard {
 };
 }  // namespace
 
-extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float *vis_host, int64_t n0,
+namespace {
+// gains0: HOST [n_ant][n0][2] or NULL.  With a table, a child inherits its parent's gain column (reading R25).
+int quadtree_solve_impl(int64_t n_vis, const double *uvw, const float *vis_host, const int32_t *ant_p,
+                        const int32_t *ant_q, int32_t n_ant, const float *gains0, int64_t n0,
                                    const double *l0, const double *m0, const double *side0, int n_levels,
                                    double frac, double min_side, double sigma_factor, int gauss_model, float lambda,
                                    float L_safety, int n_pow, int max_iter, double tol, int check_every,
@@ -97,6 +100,8 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
     try {
         std::vector<double> l(l0, l0 + n0), m(m0, m0 + n0), side(side0, side0 + n0), sigma;
         std::vector<float> x0, x;                       // x0 empty on the first level: start from zero
+        std::vector<float> g, g2;                       // gain table of the current level, [n_ant][n][2]
+        if (gains0) g.assign(gains0, gains0 + (size_t)n_ant * (size_t)n0 * 2);
         DevBuf vis_dev, x0_dev, x_dev;
         int st;
         if ((st = vis_dev.alloc((size_t)n_vis * 2 * sizeof(float)))) return st;
@@ -112,8 +117,8 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
                 sig = sigma.data();
             }
             PlanGuard plan;
-            if ((st = sl1m_plan_create(&plan.p, n_vis, uvw, nullptr, nullptr, n, l.data(), m.data(), sig, 0, nullptr,
-                                       gauss_model, 0)))
+            if ((st = sl1m_plan_create(&plan.p, n_vis, uvw, gains0 ? ant_p : nullptr, gains0 ? ant_q : nullptr, n, l.data(),
+                                       m.data(), sig, gains0 ? n_ant : 0, gains0 ? g.data() : nullptr, gauss_model, 0)))
                 return st;
             float L = 0.f;
             if ((st = sl1m_max_eig(plan.p, n_pow, &L, stream))) return st;
@@ -161,9 +166,20 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
             std::vector<double> l2((size_t)n_new), m2((size_t)n_new), s2((size_t)n_new);
             std::vector<float> i2((size_t)n_new);
             int64_t got = 0, nref = 0;
+            std::vector<int64_t> parent(gains0 ? (size_t)n_new : 0);
             if ((st = sl1m_quadtree_refine(n, l.data(), m.data(), side.data(), x.data(), frac, min_side, n_new, l2.data(),
-                                           m2.data(), s2.data(), i2.data(), nullptr, &got, &nref)))
+                                           m2.data(), s2.data(), i2.data(), gains0 ? parent.data() : nullptr, &got, &nref)))
                 return st;
+            if (gains0) {                               // children inherit their parent's gain column
+                g2.resize((size_t)n_ant * (size_t)n_new * 2);
+                for (int32_t a = 0; a < n_ant; ++a)
+                    for (int64_t k = 0; k < n_new; ++k) {
+                        const size_t src = ((size_t)a * (size_t)n + (size_t)parent[(size_t)k]) * 2, dst = ((size_t)a * (size_t)n_new + (size_t)k) * 2;
+                        g2[dst] = g[src];
+                        g2[dst + 1] = g[src + 1];
+                    }
+                g.swap(g2);
+            }
             l.swap(l2);
             m.swap(m2);
             side.swap(s2);
@@ -181,4 +197,31 @@ extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float
         return sl1m_fail(SL1M_ERR_ALLOC, "sl1m_quadtree_solve: host allocation failed");
     }
     return SL1M_OK;
+}
+}  // namespace
+
+extern "C" int sl1m_quadtree_solve(int64_t n_vis, const double *uvw, const float *vis_host, int64_t n0,
+                                   const double *l0, const double *m0, const double *side0, int n_levels,
+                                   double frac, double min_side, double sigma_factor, int gauss_model, float lambda,
+                                   float L_safety, int n_pow, int max_iter, double tol, int check_every,
+                                   int64_t capacity, double *l_out, double *m_out, double *side_out, float *x_out,
+                                   int64_t *n_out, sl1m_qt_level *levels_out, int *n_levels_done, void *stream) {
+    return quadtree_solve_impl(n_vis, uvw, vis_host, nullptr, nullptr, 0, nullptr, n0, l0, m0, side0, n_levels, frac,
+                               min_side, sigma_factor, gauss_model, lambda, L_safety, n_pow, max_iter, tol, check_every,
+                               capacity, l_out, m_out, side_out, x_out, n_out, levels_out, n_levels_done, stream);
+}
+
+extern "C" int sl1m_quadtree_solve_gains(int64_t n_vis, const double *uvw, const float *vis_host,
+                                         const int32_t *ant_p, const int32_t *ant_q, int32_t n_ant,
+                                         const float *gains0_host, int64_t n0, const double *l0, const double *m0,
+                                         const double *side0, int n_levels, double frac, double min_side,
+                                         double sigma_factor, int gauss_model, float lambda, float L_safety, int n_pow,
+                                         int max_iter, double tol, int check_every, int64_t capacity, double *l_out,
+                                         double *m_out, double *side_out, float *x_out, int64_t *n_out,
+                                         sl1m_qt_level *levels_out, int *n_levels_done, void *stream) {
+    if (!ant_p || !ant_q || !gains0_host) return sl1m_fail(SL1M_ERR_NULL, "sl1m_quadtree_solve_gains: NULL gain argument");
+    if (n_ant < 1) return sl1m_fail(SL1M_ERR_SIZE, "sl1m_quadtree_solve_gains: n_ant < 1");
+    return quadtree_solve_impl(n_vis, uvw, vis_host, ant_p, ant_q, n_ant, gains0_host, n0, l0, m0, side0, n_levels, frac,
+                               min_side, sigma_factor, gauss_model, lambda, L_safety, n_pow, max_iter, tol, check_every,
+                               capacity, l_out, m_out, side_out, x_out, n_out, levels_out, n_levels_done, stream);
 }

@@ -605,6 +605,44 @@ def test_quadtree_driver_matches_oracle(sl):
         sl.quadtree_solve(uvw, V, l0, m0, side0, n_levels=3, frac=-1.0, min_side=0.0, lam=lam, capacity=100)
 
 
+def test_quadtree_driver_with_gains_matches_oracle(sl):
+    """sl1m_quadtree_solve_gains against oracle.quadtree_solve(gains0=...) (reading R25: a child inherits its parent's
+    gain column): a smooth direction-dependent gain table on the 8 x 8 starting grid, data formed with the table the
+    finest level would inherit.  Same comparison as the unit-gain driver test."""
+    uvw, V_unit, l0, m0, side0, df, lf, mf, src, x_true = _toy_quadtree_problem()
+    rng = np.random.default_rng(78)
+    n_ant = 16
+    p, q = np.triu_indices(n_ant, 1)
+    ap, aq = np.tile(p, 6).astype(np.int32), np.tile(q, 6).astype(np.int32)
+    z = (rng.standard_normal((n_ant, 3)) + 1j * rng.standard_normal((n_ant, 3))) / np.sqrt(2.0)
+    g0 = ((1.0 + 0.1 * (z[:, 0:1] + z[:, 1:2] * (l0 / 0.025)[None, :] + z[:, 2:3] * (m0 / 0.025)[None, :]))
+          * np.exp(-((l0 ** 2 + m0 ** 2) / 0.05 ** 2))[None, :]).astype(np.complex64)
+    # the fine-grid truth seen through the gains its 8 x 8 ancestor carries
+    anc = (np.floor(lf / (0.05 / 8) + 4).astype(int) + 8 * np.floor(mf / (0.05 / 8) + 4).astype(int))
+    V = oracle.Oracle(uvw, lf, mf, None, ap, aq, g0[:, anc]).forward(x_true).astype(np.complex64)
+    lam = 0.02 * float(np.abs(oracle.Oracle(uvw, l0, m0, None, ap, aq, g0).adjoint(V)).max())
+    kw = dict(n_levels=4, frac=0.01, min_side=df * 0.999, lam=lam, n_pow=30, L_safety=1.05, max_iter=150, tol=0.0,
+              check_every=50, sigma_factor=1.0, ant_p=ap, ant_q=aq, gains0=g0)
+    ref = oracle.quadtree_solve(uvw, V, l0, m0, side0, **kw)
+    got = sl.quadtree_solve(uvw, V, l0, m0, side0, **kw)
+    assert len(got["levels"]) == len(ref["levels"]) == 4
+    for a, b in zip(got["levels"], ref["levels"]):
+        assert abs(a["n_pix"] - b["n_pix"]) <= 0.02 * b["n_pix"] + 3
+        assert abs(a["L"] - b["L"]) <= 1e-3 * b["L"]
+    q4 = df / 4
+    kg = {(int(round(a / q4)), int(round(b / q4)), int(round(c / q4))): float(x) for a, b, c, x in zip(got["l"], got["m"], got["side"], got["x"])}
+    kr = {(int(round(a / q4)), int(round(b / q4)), int(round(c / q4))): float(x) for a, b, c, x in zip(ref["l"], ref["m"], ref["side"], ref["x"])}
+    common = sorted(set(kg) & set(kr))
+    assert len(set(kg) ^ set(kr)) <= 0.02 * len(kr) + 3
+    top = max(kr.values())
+    assert all(k in kg for k, v in kr.items() if v > 0.05 * top)
+    xg, xr = np.array([kg[k] for k in common]), np.array([kr[k] for k in common])
+    assert rel_l2(xg, xr) <= 5 * TOL_IMAGE, rel_l2(xg, xr)
+    for s in src:                                   # the sources are recovered through the gains
+        k = (int(round(lf[s] / q4)), int(round(mf[s] / q4)), 4)
+        assert k in kg and abs(kg[k] - x_true[s]) < 0.08 * x_true[s]
+
+
 # ----------------------------------------------------------------------------- NEXT-4: batched channels
 @pytest.mark.parametrize("cfg", [1, 3, 4])
 def test_batched_channels_match_per_channel_oracle(sl, cfg):
