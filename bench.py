@@ -259,7 +259,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     assert k_done == args.warmup + args.steps
 
     # ---------------- the same run as ONE call: sl1m_solve(n_iter = warmup + steps), events around the call ----
-    n_cont = args.warmup + args.steps
+    n_cont = args.cont_iters if args.cont_iters > 0 else args.warmup + args.steps
     trace = torch.zeros(3 * n_cont, dtype=torch.float64, device=dev)
     x_cont = torch.empty_like(x)
     flush.zero_()
@@ -468,8 +468,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "continuous_solve": {"call": f"sl1m_solve(n_iter={n_cont}) from I_0 = 0, trace on, CUDA events around the call",
                              "n_iter": n_cont, "ms_total": cont_ms, "ms_per_iter": cont_ms / n_cont,
                              "iters_per_s": 1e3 * n_cont / cont_ms,
-                             "nnz_I_k": [int(v) for v in tr[:, 2]],
-                             "image_bit_identical_to_stepped_run": cont_same},
+                             "nnz_I_k": [int(v) for v in tr[:: max(1, n_cont // 50), 2]],
+                             "image_bit_identical_to_stepped_run": cont_same if n_cont == args.warmup + args.steps else None},
         "dense_forward_step_ms": fwd_ms + adj_ms,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_mean, "call": "sl1m_solve_host(n_iter=1) with pinned host V, x0, x_out"},
@@ -498,6 +498,8 @@ def main():
     ap.add_argument("--phase-fp64", action="store_true", dest="phase_fp64", help="SL1M_PHASE_FP64: the fp64-phase kernels")
     ap.add_argument("--jitter-sigma", action="store_true", dest="jitter_sigma",
                     help="Gaussian configs: multiply every sigma_k by a seeded U(0.7, 1.3) draw (per-pixel-sigma kernels)")
+    ap.add_argument("--cont-iters", type=int, default=0, dest="cont_iters",
+                    help="iterations of the continuous_solve leg (default: warmup + steps, the stepped run's length)")
     ap.add_argument("--override", action="append", default=[], metavar="KEY=VALUE",
                     help="workloads.make_workload override for side measurements, e.g. n_steps=2 (config 4 with 2 samples per "
                          "baseline: per-term gain kernels); the default line uses none")
