@@ -153,6 +153,9 @@ struct sl1m_plan {
     float *px0 = nullptr;            // [n_tiles][n_vis] centre phases
     double *ppart = nullptr;         // [2][3][persist_grid]
     unsigned *pbar = nullptr;        // grid-barrier counter
+    float *pbeta = nullptr;          // DEV [pbeta_cap] momentum coefficients of one launch
+    int pbeta_cap = 0;
+    std::vector<float> pbeta_host;   // staging of the same (must outlive the asynchronous copy: plan-owned)
     int64_t launches = 0;
     int device = 0;
 };
@@ -171,7 +174,7 @@ void free_plan(sl1m_plan *p) {
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
                     p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc, p->rpol, p->ctl_i,
-                    p->lam2, p->pixdc, p->pixgc, p->pvis4, p->px0, p->ppart, p->pbar};
+                    p->lam2, p->pixdc, p->pixgc, p->pvis4, p->px0, p->ppart, p->pbar, p->pbeta};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (p->h_flag) cudaFreeHost(p->h_flag);
@@ -1002,13 +1005,30 @@ int persist_iterate(sl1m_plan *p, int n_iter, double *trace_rows, const StopOpts
     P.nnz_tol = stop ? stop->nnz_tol : -1.0;
     P.check_every = stop ? stop->check_every : 0;
     P.k0 = p->f_k;
-    P.t0 = p->f_t;
     P.n_iter = n_iter;
+    {   // momentum coefficients of this launch's iterations, fp64 on the host as in the multi-launch loop
+        if (p->pbeta_cap < n_iter) {
+            if (p->pbeta) cudaFree(p->pbeta);
+            p->pbeta = nullptr;
+            p->pbeta_cap = 0;
+            CUDA_TRY(cudaMalloc((void **)&p->pbeta, (size_t)n_iter * sizeof(float)));
+            p->pbeta_cap = n_iter;
+        }
+        p->pbeta_host.resize((size_t)n_iter);
+        double t = p->f_t;
+        for (int i = 0; i < n_iter; ++i) {
+            const double t_next = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
+            p->pbeta_host[(size_t)i] = (float)((t - 1.0) / t_next);
+            t = t_next;
+        }
+        CUDA_TRY(cudaMemcpyAsync(p->pbeta, p->pbeta_host.data(), (size_t)n_iter * sizeof(float), cudaMemcpyHostToDevice, s));
+        p->f_t = t;
+    }
+    P.beta = p->pbeta;
     CUDA_TRY(cudaMemsetAsync(p->pbar, 0, sizeof(unsigned), s));
     void *args[] = {(void *)&P};
     CUDA_TRY(cudaLaunchCooperativeKernel((const void *)fista_persistent_kernel, dim3((unsigned)G), dim3(PT), args, 0, s));
     p->launches++;
-    for (int i = 0; i < n_iter; ++i) p->f_t = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * p->f_t * p->f_t));
     p->f_k += n_iter;
     return check_launch("sl1m_fista_step(persistent)");
 }

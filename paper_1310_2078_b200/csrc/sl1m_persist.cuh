@@ -57,7 +57,8 @@ struct PersistParams {
     double lam2, tol, nnz_tol;     // stopping rules (tol, nnz_tol < 0: off)
     int check_every;               // 0: no stopping rule
     int k0;                        // iterations done before this launch
-    double t0;                     // t_{k0+1}
+    const float *beta;             // [n_iter] momentum coefficients (t_k - 1)/t_{k+1} of this launch's iterations, formed in
+                                   // fp64 on the host (a device fp64 sqrt + divide cost 0.3 us per iteration on the critical path)
     int n_iter;
 };
 
@@ -70,6 +71,10 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
 // passed when it reaches n * gridDim.x.  Release: __threadfence before the arrive; acquire: ld.acquire by the
 // polling thread, then the CTA barrier hands the visibility on to the other threads.
 __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target) {
+#ifdef SL1M_PP_NO_BAR
+    __syncthreads();
+    return;
+#endif
     __syncthreads();
     if (threadIdx.x == 0) {
         target += gridDim.x;
@@ -113,6 +118,23 @@ __device__ __forceinline__ double warp_sum_cg(const double *p, int n) {
     return v;
 }
 
+// The three partial arrays at once (all loads in flight together: one L2 round trip instead of three).
+__device__ __forceinline__ void warp_sum3_cg(const double *p, int n, double &a, double &b, double &c) {
+    a = b = c = 0.0;
+    for (int i = threadIdx.x & 31; i < n; i += 32) {
+        const double x = __ldcg(p + i), y = __ldcg(p + n + i), z = __ldcg(p + 2 * n + i);
+        a += x;
+        b += y;
+        c += z;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+        c += __shfl_xor_sync(0xffffffffu, c, o);
+    }
+}
+
 __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistParams P) {
     __shared__ __align__(16) float4 s_list[PW][PBLK];       // compacted non-zero pixels of the warp's block
     __shared__ uint16_t s_tile[PW][PBLK];                    // their tile index
@@ -126,8 +148,22 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
     const int items_a = (P.n_vis + P.nvg - 1) / P.nvg;
     const int items_b = P.n_pix_pad / P.npg;
     const bool one_item_a = items_a <= G;                    // the CTA's x0 slice never changes: stage it once
-    double t = P.t0, E_prev = 0.0, N_prev = 0.0;
+    double E_prev = 0.0, N_prev = 0.0;
     int staged_item = -1;
+    // the CTA that sums the partials into the trace row: the last one when it has no work item of its own
+    const int tracer = (items_a < G && items_b < G) ? G - 1 : 0;
+    // Everything that does not change from one iteration to the next stays in registers when the CTA has a single
+    // work item per phase (the small-problem case this kernel exists for): an iteration is latency-bound, and every
+    // L2 round trip taken off its critical path is 0.15 us.
+    const bool one_item_b = items_b <= G;
+    const bool res_v = one_item_b && P.n_vis <= 4 * PT;      // phase B: the thread's <= 4 visibilities live in registers
+    float uf[PG], vf[PG], wf[PG];                            // phase A: the item's visibilities
+    float2 Vj = make_float2(0.f, 0.f);
+    bool a_loaded = false, b_loaded = false;
+    float dl[PG], dm[PG], dn[PG];                            // phase B: the item's pixels
+    float a_own = 0.f, y_own = 0.f, I_own = 0.f;             // ... and the state of the pixel this thread updates
+    float4 v4r[4];
+    float x0v[4];
 
     for (int it = 0; it < P.n_iter; ++it) {
         const int k = P.k0 + it + 1;                         // 1-based iteration number of the listing
@@ -146,17 +182,22 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
                 __syncthreads();
                 staged_item = one_item_a ? item : -1;
             }
-            float uf[PG], vf[PG], wf[PG], acc[2 * PG];
+            float acc[2 * PG];
 #pragma unroll
-            for (int r = 0; r < PG; ++r) {
-                const float4 v4 = __ldg(P.vis4 + min(j0 + r, P.n_vis - 1));
-                uf[r] = v4.x;
-                vf[r] = v4.y;
-                wf[r] = v4.z;
-                acc[2 * r] = 0.f;
-                acc[2 * r + 1] = 0.f;
+            for (int r = 0; r < 2 * PG; ++r) acc[r] = 0.f;
+            if (!a_loaded) {
+#pragma unroll
+                for (int r = 0; r < PG; ++r) {
+                    const float4 v4 = __ldg(P.vis4 + min(j0 + r, P.n_vis - 1));
+                    uf[r] = v4.x;
+                    vf[r] = v4.y;
+                    wf[r] = v4.z;
+                }
+                if (tid < 2 * P.nvg && (tid & 1) == 0 && j0 + (tid >> 1) < P.n_vis) Vj = __ldg(P.V + j0 + (tid >> 1));
+                a_loaded = one_item_a;
             }
             // the warp's share of the pixel list, PBLK pixels at a time: compact to a*y != 0, then generate
+#ifndef SL1M_PP_NO_A     // timing knobs (-DSL1M_PP_NO_A / _NO_B / _NO_BAR): leave a phase or the barriers out; results are wrong
             for (int base = warp * PBLK; base < P.n_pix_pad; base += PW * PBLK) {
                 int cnt = 0;
 #pragma unroll
@@ -191,14 +232,14 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
                 }
                 __syncwarp();
             }
+#endif
             const float sum = cta_sum<2 * PG>(acc, s_red);   // thread i: re (i even) / im (i odd) of visibility i / 2
             // pair up (re, im) in the even thread
             const float other = __shfl_down_sync(0xffffffffu, sum, 1);
             if (tid < 2 * P.nvg && (tid & 1) == 0) {
                 const int j = j0 + (tid >> 1);
                 if (j < P.n_vis) {
-                    const float2 v = __ldg(P.V + j);
-                    const float re = sum - v.x, im = other - v.y;
+                    const float re = sum - Vj.x, im = other - Vj.y;
                     P.rpol[j] = make_float2(sqrtf(fmaf(re, re, im * im)), atan2f(im, re));
                     r2 += (double)re * re + (double)im * im;
                 }
@@ -212,48 +253,81 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
         grid_barrier(P.bar, bar_target);
 
         // ------------------------------------------------------------------ phase B: g = Re M^H r, update
-        // no FMA contraction: the host advances the same sequence with separate multiply and add (sl1m.cu)
-        const double t_next = 0.5 * __dadd_rn(1.0, sqrt(__dadd_rn(1.0, __dmul_rn(4.0 * t, t))));
-        const float beta = (float)((t - 1.0) / t_next);
-        t = t_next;
+        const float beta = __ldg(P.beta + it);
         double l1 = 0.0, nz = 0.0;
         for (int item = blockIdx.x; item < items_b; item += G) {
             const int p0 = item * P.npg;
             const float *x0row = P.x0 + (size_t)(p0 / TP) * P.n_vis;      // npg divides TP: one tile per item
-            float dl[PG], dm[PG], dn[PG], acc[PG];
+            float acc[PG];
 #pragma unroll
-            for (int i = 0; i < PG; ++i) {
-                const float4 px = __ldcg(P.pix4 + min(p0 + i, P.n_pix_pad - 1));   // .xyz are constants, .w is rewritten below
-                dl[i] = px.x;
-                dm[i] = px.y;
-                dn[i] = px.z;
-                acc[i] = 0.f;
-            }
-            for (int j = tid; j < P.n_vis; j += PT) {
-                const float4 v4 = __ldg(P.vis4 + j);
-                const float2 rp = __ldcg(P.rpol + j);
-                const float ph = __ldg(x0row + j) + rp.y;
+            for (int i = 0; i < PG; ++i) acc[i] = 0.f;
+            if (!b_loaded) {
 #pragma unroll
                 for (int i = 0; i < PG; ++i) {
-                    if (i < P.npg) {
-                        const float X = fmaf(v4.x, dl[i], fmaf(v4.y, dm[i], fmaf(v4.z, dn[i], ph)));
-                        acc[i] = fmaf(rp.x, __cosf(X), acc[i]);
+                    const float4 px = __ldcg(P.pix4 + min(p0 + i, P.n_pix_pad - 1));   // .xyz are constants, .w is rewritten below
+                    dl[i] = px.x;
+                    dm[i] = px.y;
+                    dn[i] = px.z;
+                }
+                if (tid < P.npg) {
+                    a_own = __ldg(P.amp + p0 + tid);
+                    y_own = P.y_sorted[p0 + tid];
+                    I_own = P.I_sorted[p0 + tid];
+                }
+                if (res_v) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int j = min(tid + q * PT, P.n_vis - 1);
+                        v4r[q] = __ldg(P.vis4 + j);
+                        x0v[q] = __ldg(x0row + j);
+                    }
+                }
+                b_loaded = one_item_b;
+            }
+#ifndef SL1M_PP_NO_B
+            if (res_v) {
+                float2 rp[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q)                        // the four residual loads are in flight together
+                    rp[q] = (tid + q * PT < P.n_vis) ? __ldcg(P.rpol + tid + q * PT) : make_float2(0.f, 0.f);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float ph = x0v[q] + rp[q].y;
+#pragma unroll
+                    for (int i = 0; i < PG; ++i) {
+                        if (i < P.npg) {
+                            const float X = fmaf(v4r[q].x, dl[i], fmaf(v4r[q].y, dm[i], fmaf(v4r[q].z, dn[i], ph)));
+                            acc[i] = fmaf(rp[q].x, __cosf(X), acc[i]);
+                        }
+                    }
+                }
+            } else {
+                for (int j = tid; j < P.n_vis; j += PT) {
+                    const float4 v4 = __ldg(P.vis4 + j);
+                    const float2 rp = __ldcg(P.rpol + j);
+                    const float ph = __ldg(x0row + j) + rp.y;
+#pragma unroll
+                    for (int i = 0; i < PG; ++i) {
+                        if (i < P.npg) {
+                            const float X = fmaf(v4.x, dl[i], fmaf(v4.y, dm[i], fmaf(v4.z, dn[i], ph)));
+                            acc[i] = fmaf(rp.x, __cosf(X), acc[i]);
+                        }
                     }
                 }
             }
+#endif
             const float gsum = cta_sum<PG>(acc, s_red);
             if (tid < P.npg) {
                 const int kk = p0 + tid;
-                const float a = __ldg(P.amp + kk);
-                const float g = gsum * a;
-                const float y = P.y_sorted[kk];                // own pixel: written by this thread last iteration
-                const float z = fmaf(-P.inv_L, g, y);
+                const float g = gsum * a_own;
+                const float z = fmaf(-P.inv_L, g, y_own);
                 const float I_new = (z > P.thr) ? z - P.thr : 0.f;
-                const float I_old = P.I_sorted[kk];
-                const float y_new = fmaf(beta, I_new - I_old, I_new);
+                const float y_new = fmaf(beta, I_new - I_own, I_new);
+                I_own = I_new;                                 // with several items per CTA these are reloaded per item
+                y_own = y_new;
                 P.I_sorted[kk] = I_new;
                 P.y_sorted[kk] = y_new;
-                P.pix4[kk].w = a * y_new;
+                P.pix4[kk].w = a_own * y_new;
                 l1 += (double)I_new;
                 nz += (I_new != 0.f) ? 1.0 : 0.0;
             }
@@ -274,12 +348,13 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
         // ------------------------------------------------------------------ a6: objective, trace, stopping rules
         const bool look = P.check_every > 0 && k >= 2 && (k % P.check_every) == 0;
         const bool before_look = P.check_every > 0 && ((k + 1) % P.check_every) == 0;
-        const bool want = look || before_look || (P.trace && blockIdx.x == 0);
+        const bool want = look || before_look || (P.trace && blockIdx.x == tracer);
         if (want) {
             if (warp == 0) {
-                const double l2s = warp_sum_cg(part, G), l1s = warp_sum_cg(part + G, G), nzs = warp_sum_cg(part + 2 * G, G);
+                double l2s, l1s, nzs;
+                warp_sum3_cg(part, G, l2s, l1s, nzs);
                 if (lane == 0) {
-                    if (P.trace && blockIdx.x == 0) {
+                    if (P.trace && blockIdx.x == tracer) {
                         P.trace[3 * (size_t)it] = l2s;
                         P.trace[3 * (size_t)it + 1] = l1s;
                         P.trace[3 * (size_t)it + 2] = nzs;
