@@ -211,6 +211,21 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     # measured data through the product path: V = A x_true + noise
     x_true = torch.from_numpy(wl.x_true.astype(np.float32)).to(dev)
     V = plan.forward(x_true) + torch.from_numpy(wl.noise.astype(np.complex64)).to(dev)
+    if args.applies_only:
+        # profiling aid (ncu -k regex:fwd_kernel -s 1 / -k regex:adj_kernel): after the sparse forward above, three
+        # forwards on a DENSE image and three adjoints, nothing else
+        yd = torch.rand(wl.n_pix, dtype=torch.float32, device=dev, generator=torch.Generator(device=dev).manual_seed(7)) + 0.5
+        ts = []
+        for fn in (lambda: plan.forward(yd), lambda: plan.adjoint(V)):
+            for _ in range(3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); fn(); b.record(stream); torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+        if rank == 0:
+            print(json.dumps({"applies_only": True, "config": args.config, "fwd_ms": ts[:3], "adj_ms": ts[3:],
+                              "plan": plan.describe()}), flush=True)
+        plan.close()
+        return
     lam = fista_lambda(wl)
     if lam == 0.0:
         lam = 0.01 * float(plan.adjoint(V).abs().max())
@@ -498,6 +513,8 @@ def main():
     ap.add_argument("--phase-fp64", action="store_true", dest="phase_fp64", help="SL1M_PHASE_FP64: the fp64-phase kernels")
     ap.add_argument("--jitter-sigma", action="store_true", dest="jitter_sigma",
                     help="Gaussian configs: multiply every sigma_k by a seeded U(0.7, 1.3) draw (per-pixel-sigma kernels)")
+    ap.add_argument("--applies-only", action="store_true", dest="applies_only",
+                    help="profiling aid: plan, one sparse forward, then 3 dense forwards and 3 adjoints; no solver, no bench line")
     ap.add_argument("--cont-iters", type=int, default=0, dest="cont_iters",
                     help="iterations of the continuous_solve leg (default: warmup + steps, the stepped run's length)")
     ap.add_argument("--override", action="append", default=[], metavar="KEY=VALUE",
