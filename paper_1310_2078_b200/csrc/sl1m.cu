@@ -101,6 +101,8 @@ struct sl1m_plan {
     float4 *pixc = nullptr;       // [n_chan][n_pix_pad] compact tiles of the zero-skipping forward (NULL = dense forward)
     int *tile_cnt = nullptr;      // [n_chan][n_tiles] pixels per compact tile
     float2 *gFc = nullptr;        // [n_chan][n_pix_pad][n_ant] gain rows of the compact entries (gain plans only)
+    float2 *gAc = nullptr;        // [n_chan][n_ant][n_pix_pad] the same in the antenna-major layout, for plans whose forward is the
+                                  // packed gain kernel (gk == 2, delta pixels): that kernel reads gA / gAc, and gF / gFc do not exist
     bool dense_forward = false;   // SL1M_DENSE_FORWARD: never skip
     float2 *pixg = nullptr;
     double4 *cen = nullptr;
@@ -174,7 +176,7 @@ void free_plan(sl1m_plan *p) {
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
                     p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc, p->rpol, p->ctl_i,
-                    p->lam2, p->pixdc, p->pixgc, p->pvis4, p->px0, p->ppart, p->pbar, p->pbeta};
+                    p->lam2, p->pixdc, p->pixgc, p->pvis4, p->px0, p->ppart, p->pbar, p->pbeta, p->gAc};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (p->h_flag) cudaFreeHost(p->h_flag);
@@ -222,7 +224,10 @@ ApplyParams make_params(const sl1m_plan *p) {
     P.ws_v_stride = (size_t)p->fwd_split * (size_t)p->n_vis_int;
     P.ws_p_stride = (size_t)p->adj_split * (size_t)p->n_pix_pad;
     P.done = p->done_ptr;
+    P.gAc = p->gAc;
 #ifdef SL1M_BOUNDS
+    P.gA_end = p->gA ? p->gA + (size_t)p->n_ant * (size_t)p->n_pix_pad + GAIN_ROW_PAD : nullptr;
+    P.gAc_end = p->gAc ? p->gAc + (size_t)p->n_chan * (size_t)p->n_ant * (size_t)p->n_pix_pad + GAIN_ROW_PAD : nullptr;
     P.gF_end = p->gF ? p->gF + ((size_t)p->n_pix_pad + GAIN_ROW_PAD) * (size_t)p->n_ant : nullptr;
     P.gFc_end = p->gFc ? p->gFc + ((size_t)p->n_chan * p->n_pix_pad + GAIN_ROW_PAD) * (size_t)p->n_ant : nullptr;
 #endif
@@ -302,7 +307,7 @@ int configure_and_allocate(sl1m_plan *p) {
     for (void **q : {(void **)&p->ws_v, (void **)&p->ws_p, (void **)&p->resid, (void **)&p->I_sorted, (void **)&p->y_sorted,
                      (void **)&p->g_sorted, (void **)&p->part_a, (void **)&p->part_b, (void **)&p->part_c, (void **)&p->scalars,
                      (void **)&p->pixc, (void **)&p->tile_cnt, (void **)&p->gFc, (void **)&p->rpol, (void **)&p->pixdc,
-                     (void **)&p->pixgc}) {
+                     (void **)&p->pixgc, (void **)&p->gAc}) {
         if (*q) cudaFree(*q);
         *q = nullptr;
     }
@@ -337,8 +342,9 @@ int configure_and_allocate(sl1m_plan *p) {
         CUDA_TRY(cudaMemset(p->pixc, 0, C * npad * sizeof(float4)));
         CUDA_TRY(cudaMemset(p->tile_cnt, 0, C * (size_t)p->n_tiles * sizeof(int)));
         if (gfc_bytes) {
-            CUDA_TRY(cudaMalloc((void **)&p->gFc, gfc_bytes));
-            CUDA_TRY(cudaMemset(p->gFc, 0, gfc_bytes));
+            float2 **dst = (p->gk == 2 && p->pk == 0) ? &p->gAc : &p->gFc;   // packed gain forward: antenna-major
+            CUDA_TRY(cudaMalloc((void **)dst, gfc_bytes));
+            CUDA_TRY(cudaMemset(*dst, 0, gfc_bytes));
         }
     }
     CUDA_TRY(cudaDeviceSynchronize());
@@ -640,10 +646,17 @@ extern "C" int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uv
             if (e != cudaSuccess) { cudaFree(raw); return fail(SL1M_ERR_CUDA, cudaGetErrorString(e)); }
         }
         const size_t lay_n = (size_t)p->n_pix_pad * (size_t)n_ant;
-        // gF carries GAIN_ROW_PAD rows of zero padding: the forward kernels prefetch one group of 4 rows ahead
-        cudaError_t e1 = cudaMalloc((void **)&p->gF, (lay_n + (size_t)GAIN_ROW_PAD * n_ant) * sizeof(float2));
-        if (e1 == cudaSuccess) e1 = cudaMemset(p->gF + lay_n, 0, (size_t)GAIN_ROW_PAD * n_ant * sizeof(float2));
-        cudaError_t e2 = (e1 == cudaSuccess) ? cudaMalloc((void **)&p->gA, lay_n * sizeof(float2)) : e1;
+        // gF (pixel-major) serves the scalar forward kernels and carries GAIN_ROW_PAD rows of zero padding (they
+        // prefetch rows ahead); the packed gain forward (gk == 2, delta pixels) reads the antenna-major gA instead,
+        // which then carries GAIN_ROW_PAD entries of padding, and gF is not built at all.
+        const bool fwd_reads_gA = p->gk == 2 && !any_gauss;
+        cudaError_t e1 = cudaSuccess;
+        if (!fwd_reads_gA) {
+            e1 = cudaMalloc((void **)&p->gF, (lay_n + (size_t)GAIN_ROW_PAD * n_ant) * sizeof(float2));
+            if (e1 == cudaSuccess) e1 = cudaMemset(p->gF + lay_n, 0, (size_t)GAIN_ROW_PAD * n_ant * sizeof(float2));
+        }
+        cudaError_t e2 = (e1 == cudaSuccess) ? cudaMalloc((void **)&p->gA, (lay_n + GAIN_ROW_PAD) * sizeof(float2)) : e1;
+        if (e2 == cudaSuccess) e2 = cudaMemset(p->gA + lay_n, 0, GAIN_ROW_PAD * sizeof(float2));
         if (e2 == cudaSuccess) {
             // antennas are looped inside the kernel (grid.y would cap n_ant at 65,535; "each (antenna, time)
             // its own row" can exceed that)
@@ -676,7 +689,7 @@ namespace {
 inline int egrid(size_t n) { return (int)((n + ET - 1) / ET); }
 inline dim3 cgrid(const sl1m_plan *p, size_t n) { return dim3((unsigned)egrid(n), (unsigned)p->n_chan); }  // x: elements, y: channel
 inline ZeroSkip zs_of(const sl1m_plan *p) {
-    return ZeroSkip{p->pixc, p->tile_cnt, p->gF, p->gFc, p->n_ant, p->pixd, p->pixdc, p->pixg, p->pixgc};
+    return ZeroSkip{p->pixc, p->tile_cnt, p->gF, p->gFc, p->n_ant, p->pixd, p->pixdc, p->pixg, p->pixgc, p->gA, p->gAc};
 }
 
 template <int PK, int GK, bool B>
@@ -1274,7 +1287,7 @@ extern "C" int sl1m_plan_set_channels(sl1m_plan *p, int32_t n_chan, const double
         return std::vector<void **>{(void **)&q->ws_v, (void **)&q->ws_p, (void **)&q->resid, (void **)&q->rpol,
                                     (void **)&q->I_sorted, (void **)&q->y_sorted, (void **)&q->g_sorted,
                                     (void **)&q->part_a, (void **)&q->part_b, (void **)&q->part_c, (void **)&q->scalars,
-                                    (void **)&q->pixc, (void **)&q->tile_cnt, (void **)&q->gFc, (void **)&q->pixdc,
+                                    (void **)&q->pixc, (void **)&q->tile_cnt, (void **)&q->gFc, (void **)&q->gAc, (void **)&q->pixdc,
                                     (void **)&q->pixgc, (void **)&q->pix4,
                                     (void **)&q->chan_scale, (void **)&q->step_c, (void **)&q->h_x, (void **)&q->h_vis,
                                     (void **)&q->h_img, (void **)&q->ctl_i, (void **)&q->lam2, (void **)&q->trace_buf};

@@ -44,6 +44,10 @@ struct ZeroSkip {
     double4 *pixdc;      // DEV [n_chan][n_pix_pad]
     const float2 *pixg;  // DEV [n_pix_pad] (sigma^2, -pi log2(e) sigma^2) (per-pixel-sigma plans) or NULL
     float2 *pixgc;       // DEV [n_chan][n_pix_pad]
+    // packed gain forward (fwd_kernel_x2<GAINS>): it reads the ANTENNA-MAJOR table, so the compact gains are kept
+    // in that layout too (gAc set => gFc unused)
+    const float2 *gA;    // DEV [n_ant][n_pix_pad]
+    float2 *gAc;         // DEV [n_chan][n_ant][n_pix_pad] or NULL
 };
 static_assert(ET == TP, "one packing CTA per pixel tile");
 __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int n_pix_pad, float4 v) {
@@ -85,7 +89,17 @@ __device__ __forceinline__ void compact_tile(const ZeroSkip zs, size_t chan, int
         if (zs.pixgc) zs.pixgc[side0 + total + threadIdx.x] = make_float2(0.f, 0.f);
     }
     if (threadIdx.x == 0) zs.cnt[chan * (size_t)(n_pix_pad / TP) + blockIdx.x] = cnt4;
-    if (zs.gF && total > 0) {                            // gain rows of the compact entries (padding: a*x = 0, any row)
+    if (zs.gAc && total > 0) {                           // antenna-major: row a of the tile, compact entries in order
+        __syncthreads();
+        const size_t t0 = (size_t)blockIdx.x * TP;
+        const float2 *src = zs.gA + t0;
+        float2 *dst = zs.gAc + chan * (size_t)zs.n_ant * n_pix_pad + t0;
+        const int n = cnt4 * zs.n_ant;
+        for (int i = threadIdx.x; i < n; i += ET) {
+            const int a = i / cnt4, pos = i - a * cnt4;
+            dst[(size_t)a * n_pix_pad + pos] = src[(size_t)a * n_pix_pad + s_src[min(pos, total - 1)]];
+        }
+    } else if (zs.gF && total > 0) {                     // gain rows of the compact entries (padding: a*x = 0, any row)
         __syncthreads();
         const size_t row0 = (size_t)blockIdx.x * TP;
         const float2 *src = zs.gF + row0 * zs.n_ant;
@@ -376,7 +390,7 @@ __global__ void __launch_bounds__(ET) gains_layout_kernel(const float2 *raw, int
             const double re = (double)c.x, im = (double)c.y;
             g = make_float2((float)sqrt(re * re + im * im), (float)atan2(im, re));
         }
-        gF[(size_t)k * n_ant + a] = g;
+        if (gF) gF[(size_t)k * n_ant + a] = g;
         gA[(size_t)a * n_pix_pad + k] = g;
     }
 }

@@ -77,10 +77,13 @@ struct ApplyParams {
     // kernel of the iteration then returns at once for that channel, so the iterations the host had already
     // enqueued cost a few microseconds and the image stays the one of the stopping iteration.  NULL = never.
     const int *done;                // [n_chan] or NULL
+    // antenna-major compact gains of the packed gain forward (fwd_kernel_x2<GAINS>): gAc[c][a][k] holds, for every
+    // tile that was compacted, the gains of its compact entries in the row layout of gA
+    const float2 *gAc;              // [n_chan][n_ant][n_pix_pad] (+ padding) or NULL
 #ifdef SL1M_BOUNDS
     // debug build (-DSL1M_BOUNDS): one-past-the-end of the two gain tables, padding rows included; every
     // forward-layout gain load (the register prefetches run up to 4 rows past the pixels in use) is asserted in range
-    const float2 *gF_end, *gFc_end;
+    const float2 *gF_end, *gFc_end, *gA_end, *gAc_end;
 #endif
 };
 
@@ -90,6 +93,15 @@ struct ApplyParams {
 __device__ __forceinline__ float2 ldg_gain(const ApplyParams &P, const float2 *q) {
 #ifdef SL1M_BOUNDS
     assert((q >= P.gF && q < P.gF_end) || (P.gFc && q >= P.gFc && q < P.gFc_end));
+#endif
+    return __ldg(q);
+}
+
+// Two consecutive pixels of one antenna's row of the antenna-major tables (gA / gAc), 16-byte aligned.
+__device__ __forceinline__ float4 ldg_gain4(const ApplyParams &P, const float4 *q) {
+#ifdef SL1M_BOUNDS
+    const float2 *q2 = reinterpret_cast<const float2 *>(q);
+    assert((q2 >= P.gA && q2 + 2 <= P.gA_end) || (P.gAc && q2 >= P.gAc && q2 + 2 <= P.gAc_end));
 #endif
     return __ldg(q);
 }
@@ -661,33 +673,34 @@ __global__ void __launch_bounds__(NT, SL1M_FWD_X2_MIN_CTAS) fwd_kernel_x2(const 
         }
         mbar_wait(&s_bar[st], parity);
         if (GAINS) {
-            // gain rows of the tile, gF[k][a]: register prefetch 4 pixels ahead (cold in L1 on first touch)
-            // 32-bit element offsets from the tile's first row (one IMAD.WIDE per load instead of 64-bit index
-            // arithmetic); the tables carry 4 rows of padding, so the prefetch of the group after the last needs no clamp
-            const float2 *gbase = tile_gain_rows<BATCH>(P, t, npx);
-            const unsigned na = (unsigned)P.n_ant;
-            unsigned op = (unsigned)ap, oq = (unsigned)aq;
-            float2 gp[4], gq[4];
-#pragma unroll
-            for (int d = 0; d < 4; ++d) {
-                gp[d] = ldg_gain(P, gbase + (op + d * na));
-                gq[d] = ldg_gain(P, gbase + (oq + d * na));
-            }
+            // Gains of the tile for the thread's two antennas, read from the ANTENNA-MAJOR table gA[a][k] (the
+            // adjoint's layout; gAc[c][a][k] holds the compact entries of a tile that was compacted): the thread
+            // walks two contiguous rows, so 4 pixels are 4 LDG.128 at pointer + immediate instead of 8 LDG.64 with
+            // a 64-bit index computation each (46 -> 6 integer instructions per 32 terms).  A lane's 128-byte line
+            // serves its next 16 pixels; a CTA keeps <= 2 x 128 such lines live, well inside L1.  Register prefetch
+            // one group of 4 pixels ahead; the rows carry 4 entries of padding behind the last tile.
+            const bool compacted = P.tile_cnt && npx < TP;
+            const float2 *grow = compacted ? P.gAc + chan_index<BATCH>() * (size_t)P.n_ant * P.n_pix_pad : P.gA;
+            const float4 *pp = reinterpret_cast<const float4 *>(grow + (size_t)ap * P.n_pix_pad + (size_t)t * TP);
+            const float4 *pq = reinterpret_cast<const float4 *>(grow + (size_t)aq * P.n_pix_pad + (size_t)t * TP);
+            float4 gp01 = ldg_gain4(P, pp), gp23 = ldg_gain4(P, pp + 1), gq01 = ldg_gain4(P, pq), gq23 = ldg_gain4(P, pq + 1);
 #pragma unroll 1
             for (int p = 0; p < npx; p += 4) {
                 float Gw[4], Ng[4];
-#pragma unroll
-                for (int d = 0; d < 4; ++d) {
-                    Gw[d] = s_pix[st][p + d].w * (gp[d].x * gq[d].x);          // a x |g_p||g_q|
-                    Ng[d] = gq[d].y - gp[d].y;                                 // -gamma
-                }
-                op += 4 * na;
-                oq += 4 * na;
-#pragma unroll
-                for (int d = 0; d < 4; ++d) {                // rows past npx exist (stale, zero or padding): harmless prefetch
-                    gp[d] = ldg_gain(P, gbase + (op + d * na));
-                    gq[d] = ldg_gain(P, gbase + (oq + d * na));
-                }
+                Gw[0] = s_pix[st][p].w * (gp01.x * gq01.x);                    // a x |g_p||g_q|
+                Ng[0] = gq01.y - gp01.y;                                       // -gamma
+                Gw[1] = s_pix[st][p + 1].w * (gp01.z * gq01.z);
+                Ng[1] = gq01.w - gp01.w;
+                Gw[2] = s_pix[st][p + 2].w * (gp23.x * gq23.x);
+                Ng[2] = gq23.y - gp23.y;
+                Gw[3] = s_pix[st][p + 3].w * (gp23.z * gq23.z);
+                Ng[3] = gq23.w - gp23.w;
+                pp += 2;
+                pq += 2;
+                gp01 = ldg_gain4(P, pp);                     // entries past npx exist (stale, next tile or padding): harmless prefetch
+                gp23 = ldg_gain4(P, pp + 1);
+                gq01 = ldg_gain4(P, pq);
+                gq23 = ldg_gain4(P, pq + 1);
                 pixel(s_pix[st][p], X0, std::integral_constant<int, (NPQ + 3) / 4>{}, Gw[0], Ng[0]);
                 pixel(s_pix[st][p + 1], X0, std::integral_constant<int, (NPQ + 2) / 4>{}, Gw[1], Ng[1]);
                 pixel(s_pix[st][p + 2], X0, std::integral_constant<int, (NPQ + 1) / 4>{}, Gw[2], Ng[2]);
