@@ -70,6 +70,15 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
 // All CTAs of the (cooperatively launched, co-resident) grid meet here.  Monotonic counter: the n-th barrier is
 // passed when it reaches n * gridDim.x.  Release: __threadfence before the arrive; acquire: ld.acquire by the
 // polling thread, then the CTA barrier hands the visibility on to the other threads.
+// SL1M_BAR_MODE bit 1: arrive with one red.release.gpu instead of __threadfence + atomicAdd; bit 0: poll with
+// ld.relaxed; bit 2: ... and no fence behind the poll.  Default 7 (measured at config 1: 5.38 us per iteration with
+// mode 0, 5.19 with 7).  Why the consumer-side fence can go: every datum another CTA produced is read with ld.global.cg
+// (L2, never L1), it reached L2 before its producer's release-arrive did, and no consumer load can issue before the
+// poll has returned the final count -- thread 0 leaves its loop on that value (control dependency, in-order issue)
+// and every other thread is held at the CTA barrier behind it.
+#ifndef SL1M_BAR_MODE
+#define SL1M_BAR_MODE 7
+#endif
 __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target) {
 #ifdef SL1M_PP_NO_BAR
     __syncthreads();
@@ -78,9 +87,23 @@ __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target) {
     __syncthreads();
     if (threadIdx.x == 0) {
         target += gridDim.x;
+#if SL1M_BAR_MODE & 2
+        asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
+#else
         __threadfence();
         atomicAdd(bar, 1u);
+#endif
+#if SL1M_BAR_MODE & 1
+        unsigned v;
+        do {
+            asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while (v < target);
+#if !(SL1M_BAR_MODE & 4)
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
+#endif
+#else
         while (ld_acquire_u32(bar) < target) {}
+#endif
     }
     __syncthreads();
 }
@@ -89,22 +112,40 @@ __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target) {
 // Result valid in threads 0..N-1 (thread i holds sum i).
 template <int N>
 __device__ __forceinline__ float cta_sum(float (&v)[N], float (*s_red)[PG * 2 + 1]) {
+    static_assert(N == 8 || N == 16, "cta_sum: 8 or 16 values per thread");
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // Warp stage: a halving butterfly -- at every step a lane keeps half of its values and sends the other half to its
+    // partner, so N values x 32 lanes take N - 1 + (5 - log2 N) shuffles instead of 5 N.  Afterwards lane l holds the
+    // warp's sum of value number (l mod N) (bit-reversed bookkeeping below); the order of additions is fixed.
+    float w[N];
 #pragma unroll
-    for (int i = 0; i < N; ++i) {
+    for (int i = 0; i < N; ++i) w[i] = v[i];
+    int idx = 0;                                             // which value this lane ends up holding
+    {
+        constexpr int STEPS = (N == 16) ? 4 : 3;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+        for (int s = 0; s < STEPS; ++s) {
+            const int half = N >> (s + 1);
+            const bool up = (lane >> s) & 1;                 // upper partner keeps the upper half
+#pragma unroll
+            for (int i = 0; i < half; ++i) {
+                const float keep = up ? w[i + half] : w[i];
+                const float give = up ? w[i] : w[i + half];
+                w[i] = keep + __shfl_xor_sync(0xffffffffu, give, 1 << s);
+            }
+            idx |= up ? half : 0;
+        }
+        // remaining lane bits: plain butterfly on the single value left
+#pragma unroll
+        for (int o = 1 << STEPS; o < 32; o <<= 1) w[0] += __shfl_xor_sync(0xffffffffu, w[0], o);
     }
     __syncthreads();                      // s_red free again
-    if (lane == 0) {
-#pragma unroll
-        for (int i = 0; i < N; ++i) s_red[warp][i] = v[i];
-    }
+    if (lane < N) s_red[warp][idx] = w[0];                   // lanes 0..N-1 cover every idx exactly once
     __syncthreads();
     float t = 0.f;
     if (threadIdx.x < N) {
 #pragma unroll
-        for (int w = 0; w < PW; ++w) t += s_red[w][threadIdx.x];
+        for (int ww = 0; ww < PW; ++ww) t += s_red[ww][threadIdx.x];
     }
     return t;
 }
@@ -118,14 +159,25 @@ __device__ __forceinline__ double warp_sum_cg(const double *p, int n) {
     return v;
 }
 
-// The three partial arrays at once (all loads in flight together: one L2 round trip instead of three).
+// The three partial arrays at once, every load in flight before the first add (one L2 round trip: this sum sits on
+// the critical path of the CTA that writes the trace row).  n <= 32 * 8 elements per array.
 __device__ __forceinline__ void warp_sum3_cg(const double *p, int n, double &a, double &b, double &c) {
+    const int lane = threadIdx.x & 31;
+    double x[8], y[8], z[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const int i = lane + 32 * q;
+        const bool in = i < n;
+        x[q] = in ? __ldcg(p + i) : 0.0;
+        y[q] = in ? __ldcg(p + n + i) : 0.0;
+        z[q] = in ? __ldcg(p + 2 * n + i) : 0.0;
+    }
     a = b = c = 0.0;
-    for (int i = threadIdx.x & 31; i < n; i += 32) {
-        const double x = __ldcg(p + i), y = __ldcg(p + n + i), z = __ldcg(p + 2 * n + i);
-        a += x;
-        b += y;
-        c += z;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        a += x[q];
+        b += y[q];
+        c += z[q];
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -200,10 +252,13 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
 #ifndef SL1M_PP_NO_A     // timing knobs (-DSL1M_PP_NO_A / _NO_B / _NO_BAR): leave a phase or the barriers out; results are wrong
             for (int base = warp * PBLK; base < P.n_pix_pad; base += PW * PBLK) {
                 int cnt = 0;
+                float4 pxq[PBLK / 32];
+#pragma unroll
+                for (int q = 0; q < PBLK / 32; ++q) pxq[q] = __ldcg(P.pix4 + base + q * 32 + lane);   // all in flight before the first ballot
 #pragma unroll
                 for (int q = 0; q < PBLK / 32; ++q) {
                     const int kpx = base + q * 32 + lane;
-                    const float4 px = __ldcg(P.pix4 + kpx);
+                    const float4 px = pxq[q];
                     const bool nz = px.w != 0.f;             // NaN counts as non-zero and propagates
                     const unsigned b = __ballot_sync(0xffffffffu, nz);
                     if (nz) {
@@ -325,8 +380,10 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
                 const float y_new = fmaf(beta, I_new - I_own, I_new);
                 I_own = I_new;                                 // with several items per CTA these are reloaded per item
                 y_own = y_new;
-                P.I_sorted[kk] = I_new;
-                P.y_sorted[kk] = y_new;
+                if (!one_item_b) {                             // one item: the state stays in registers until the kernel ends
+                    P.I_sorted[kk] = I_new;
+                    P.y_sorted[kk] = y_new;
+                }
                 P.pix4[kk].w = a_own * y_new;
                 l1 += (double)I_new;
                 nz += (I_new != 0.f) ? 1.0 : 0.0;
@@ -376,10 +433,15 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
             }
             if (P.check_every > 0) {
                 __syncthreads();
-                if (s_stop) return;                          // same numbers, same decision in every CTA
+                if (s_stop) break;                           // same numbers, same decision in every CTA
                 __syncthreads();
             }
         }
+    }
+    // the register-resident state of the CTA's pixels goes back to global memory (next launch, sl1m_fista_image)
+    if (one_item_b && blockIdx.x < items_b && tid < P.npg) {
+        P.I_sorted[blockIdx.x * P.npg + tid] = I_own;
+        P.y_sorted[blockIdx.x * P.npg + tid] = y_own;
     }
 }
 
