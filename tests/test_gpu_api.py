@@ -268,7 +268,7 @@ def test_fp64_phase_path(sl):
         plan.close()
 
 
-@pytest.mark.parametrize("n_vis,n_pix", [(1, 1), (5, 3), (300, 1500), (1187, 2100), (2500, 700)])
+@pytest.mark.parametrize("n_vis,n_pix", [(1, 1), (5, 3), (1024, 1000), (147, 1024), (300, 1500), (1187, 2100), (2500, 700)])
 def test_persistent_small_problem_path(sl, n_vis, n_pix):
     """Small problems run the whole FISTA loop as ONE persistent cooperative kernel (sl1m_persist.cuh; two grid
     barriers per iteration).  Against the oracle (image, trace, stop index) and against the multi-launch loop of a
