@@ -280,6 +280,9 @@ int configure_and_allocate(sl1m_plan *p) {
         int split = (nvi * (int64_t)p->n_tiles >= (int64_t)64 * SM_COUNT_B200)
                         ? pick_split(p->fwd_vtiles, p->n_tiles, SM_COUNT_B200 * fwd_ctas, waves, p->n_chan)
                         : std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
+#ifdef SL1M_FORCE_FWD_PER_SPLIT
+        split = (p->n_tiles + SL1M_FORCE_FWD_PER_SPLIT - 1) / SL1M_FORCE_FWD_PER_SPLIT;   // tuning knob
+#endif
         p->fwd_per_split = (p->n_tiles + split - 1) / split;
         p->fwd_split = (p->n_tiles + p->fwd_per_split - 1) / p->fwd_per_split;
     }

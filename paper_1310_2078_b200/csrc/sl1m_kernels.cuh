@@ -407,7 +407,10 @@ struct PolySplit {
 // grid = (vis tiles of NT*RV, pixel splits); block = NT
 // ------------------------------------------------------------------------------------------
 template <int RV, int PK, int GK, bool BATCH = false>
-__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : (GK == 2 ? 4 : (PK == 2 ? SL1M_FWD_GT_MIN_CTAS : 1))) fwd_kernel(const ApplyParams P) {
+#ifndef SL1M_FWD_G1_MIN_CTAS
+#define SL1M_FWD_G1_MIN_CTAS 4   // per-term gains: 255 registers (2 CTAs/SM) left the gain loads latency-bound: 9.27 -> 4.67 ms at config 4 with 2 samples per baseline
+#endif
+__global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_FWD_MIN_CTAS : (GK == 2 ? 4 : (PK == 2 ? SL1M_FWD_GT_MIN_CTAS : (PK == 0 && GK == 1 ? SL1M_FWD_G1_MIN_CTAS : 1)))) fwd_kernel(const ApplyParams P) {
     if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
     __shared__ __align__(128) float4 s_pix[2][TP];
     __shared__ __align__(128) float2 s_pixg[PK == 1 ? 2 : 1][PK == 1 ? TP : 1];
