@@ -39,7 +39,8 @@ MUFU_PER_SM_PER_CLK = 16      # nominal: 4 SFU lanes per SM sub-partition x 4; t
 SM_COUNT = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (config, kernel) -> bytes
-NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 100.70e6, (5, "adj"): 52.56e6, (4, "fwd"): 341.8e6, (4, "adj"): 328.0e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {(5, "fwd"): 100.95e6, (5, "adj"): 56.39e6, (4, "fwd"): 341.0e6, (4, "adj"): 326.0e6,
+                             (2, "fwd"): 1.56e6, (2, "adj"): 1.72e6, (3, "fwd"): 1.90e6, (3, "adj"): 2.10e6}   # profiles/r2_ncu_full_config*.md
 
 
 def _peaks():
