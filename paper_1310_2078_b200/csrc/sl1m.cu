@@ -1022,6 +1022,7 @@ int persist_iterate(sl1m_plan *p, int n_iter, double *trace_rows, const StopOpts
     P.check_every = stop ? stop->check_every : 0;
     P.k0 = p->f_k;
     P.n_iter = n_iter;
+    const double t_before = p->f_t;
     {   // momentum coefficients of this launch's iterations, fp64 on the host as in the multi-launch loop
         if (p->pbeta_cap < n_iter) {
             if (p->pbeta) cudaFree(p->pbeta);
@@ -1043,7 +1044,18 @@ int persist_iterate(sl1m_plan *p, int n_iter, double *trace_rows, const StopOpts
     P.beta = p->pbeta;
     CUDA_TRY(cudaMemsetAsync(p->pbar, 0, sizeof(unsigned), s));
     void *args[] = {(void *)&P};
-    CUDA_TRY(cudaLaunchCooperativeKernel((const void *)fista_persistent_kernel, dim3((unsigned)G), dim3(PT), args, 0, s));
+    const cudaError_t le = cudaLaunchCooperativeKernel((const void *)fista_persistent_kernel, dim3((unsigned)G), dim3(PT), args, 0, s);
+    if (le == cudaErrorCooperativeLaunchTooLarge || le == cudaErrorLaunchOutOfResources) {
+        // the grid cannot be co-resident right now (e.g. the GPU is shared): this plan goes back to the multi-launch
+        // loop for good.  Its compact tiles are rebuilt from y (the persistent kernel does not maintain them).
+        cudaGetLastError();
+        p->f_t = t_before;
+        p->persist = false;
+        pack_sorted_kernel<<<cgrid(p, p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, p->n_pix_pad, zs_of(p));
+        p->launches++;
+        return -1;                                         // caller: carry on with the multi-launch loop
+    }
+    CUDA_TRY(le);
     p->launches++;
     p->f_k += n_iter;
     return check_launch("sl1m_fista_step(persistent)");
@@ -1051,8 +1063,10 @@ int persist_iterate(sl1m_plan *p, int n_iter, double *trace_rows, const StopOpts
 
 int fista_iterate(sl1m_plan *p, int n_iter, double *trace_dev, size_t trace_stride, int trace_row0,
                   const StopOpts *stop, cudaStream_t s) {
-    if (p->persist && !p->chan_scale)
-        return persist_iterate(p, n_iter, trace_dev ? trace_dev + 3 * (size_t)trace_row0 : nullptr, stop, s);
+    if (p->persist && !p->chan_scale) {
+        const int st = persist_iterate(p, n_iter, trace_dev ? trace_dev + 3 * (size_t)trace_row0 : nullptr, stop, s);
+        if (st != -1) return st;
+    }
     const int C = p->n_chan, npad = p->n_pix_pad;
     const float2 *step_c = C > 1 ? p->step_c : nullptr;
     const int *done = stop ? p->ctl_i : nullptr;

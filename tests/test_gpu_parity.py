@@ -449,6 +449,49 @@ def test_device_side_stop_rules_match_oracle(sl):
     plan.close()
 
 
+def test_stop_rule_on_the_multi_launch_paths(sl):
+    """The device-side decision in the multi-launch loop (stop_rule_kernel + done flags): (i) config 1 on a
+    SL1M_NO_PERSISTENT plan (small problem: the host reads the flag two polls behind); (ii) the FULL config 2
+    (1.3e9 terms per apply: the host waits for every look), with the oracle's stopping index taken from the CACHED
+    full-size oracle trace (tests/golden/solver_fullsize_config2.npz) -- no oracle run at that size in the test."""
+    import os
+    import torch
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(30) * 1.05
+    lam = fista_lambda(wl)
+    plan = sl.Plan.from_workload(wl, no_persistent=True)
+    assert plan.describe()["persistent"] == 0
+    for tol, nnz_tol, every in ((1e-5, -1.0, 5), (-1.0, 0.0, 4), (1e-6, -1.0, 1)):
+        ref = o.fista_tol(V, lam, L, max_iter=600, tol=tol, nnz_tol=nnz_tol, check_every=every)
+        x, info = plan.solve_stop(_dev(V, torch.complex64), lam, L, max_iter=600, tol=tol, nnz_tol=nnz_tol, check_every=every)
+        k = info.n_iter_done
+        assert abs(k - ref["n_iter_done"]) <= 3 * every and (k % every == 0 or k == 600)
+        assert rel_l2(x.cpu().numpy(), o.fista(V, lam, L, k)["x"]) <= TOL_IMAGE
+    plan.close()
+    # (ii)
+    gc = _golden_cache_module()
+    z = np.load(gc.cache_path(2))
+    wl = make_workload(2)
+    assert gc.input_hash(wl) == str(z["input_hash"])
+    tr, lam, L = z["trace"], float(z["lam"]), float(z["L"])
+    E = tr[:, 0] + 2.0 * lam * tr[:, 1]
+    every = 5
+    rel = np.abs(np.diff(E)) / np.abs(E[1:])                 # rel[k-2] = |E_k - E_{k-1}| / |E_k|, k = 2..K
+    looks = [k for k in range(2, tr.shape[0] + 1) if k % every == 0]
+    tol = float(np.sqrt(rel[looks[3] - 2] * rel[looks[4] - 2]))   # between the 4th and 5th look's change
+    want = next((k for k in looks if rel[k - 2] <= tol), tr.shape[0])
+    assert every < want < tr.shape[0]
+    plan = sl.Plan.from_workload(wl)
+    x, info = plan.solve_stop(_dev(z["V"], torch.complex64), lam, L, max_iter=tr.shape[0], tol=tol, check_every=every)
+    print("config2 full-size stop: GPU", info.n_iter_done, "oracle trace", want)
+    assert abs(info.n_iter_done - want) <= every
+    xk, _ = plan.solve(_dev(z["V"], torch.complex64), lam, L=L, n_iter=info.n_iter_done, want_info=False)
+    assert torch.equal(x, xk)                                # stopping only truncates
+    plan.close()
+
+
 def test_solve_stop_batch_each_channel_stops_on_its_own(sl):
     """sl1m_solve_stop_batch + sl1m_dirty_image on a batched plan (NEXT-1 composed with NEXT-4; the paper's runs are
     63-127 channels each solved to a tolerance): per-channel lambda gives per-channel stopping
