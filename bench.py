@@ -212,6 +212,44 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     # measured data through the product path: V = A x_true + noise
     x_true = torch.from_numpy(wl.x_true.astype(np.float32)).to(dev)
     V = plan.forward(x_true) + torch.from_numpy(wl.noise.astype(np.complex64)).to(dev)
+    if args.batch_stop > 0:
+        # side measurement: C channels of this geometry, each solved to a tolerance in ONE call
+        # (sl1m_plan_set_channels + sl1m_dirty_image + sl1m_solve_stop_batch), against the same channels one after
+        # the other through sl1m_solve_stop on single-channel plans
+        C = args.batch_stop
+        scale = np.linspace(0.9, 1.1, C)
+        lam0 = fista_lambda(wl)
+        Vs, Ls, plans = [], [], []
+        for c in range(C):
+            pc = sl.Plan(wl.uvw * scale[c], wl.l, wl.m, wl.sigma, wl.ant_p, wl.ant_q, wl.gains, wl.gauss_model)
+            Vs.append(pc.forward(x_true * (1.0 + 0.1 * c / C)) + torch.from_numpy(wl.noise.astype(np.complex64)).to(dev))
+            Ls.append(pc.max_eig(args.n_pow) * 1.05)
+            plans.append(pc)
+        plan.set_channels(scale)
+        Vb, Lb = torch.stack(Vs).contiguous(), np.array(Ls, np.float32)
+
+        def timed(fn):
+            best = 1e30
+            for _ in range(3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); out = fn(); b.record(stream); torch.cuda.synchronize()
+                best = min(best, a.elapsed_time(b))
+            return best, out
+        kw = dict(max_iter=args.max_iter, tol=args.tol, check_every=args.check_every)
+        t_b, (xb, infos) = timed(lambda: plan.solve_stop_batch(Vb, lam0, Lb, x0=plan.dirty_image(Vb), **kw))
+        t_s, outs = timed(lambda: [plans[c].solve_stop(Vs[c], lam0, float(Lb[c]), x0=plans[c].dirty_image(Vs[c]), **kw) for c in range(C)])
+        same = max(float((xb[c] - outs[c][0]).norm() / outs[c][0].norm().clamp_min(1e-30)) for c in range(C))
+        if rank == 0:
+            print(json.dumps({"batch_stop": True, "config": args.config, "n_chan": C, "tol": args.tol, "check_every": args.check_every,
+                              "batched_ms": t_b, "one_after_the_other_ms": t_s, "speedup": t_s / t_b,
+                              "iterations_per_channel": [i.n_iter_done for i in infos],
+                              "iterations_per_channel_single_plans": [o[1].n_iter_done for o in outs],
+                              "max_rel_l2_batched_vs_single": same,
+                              "single_plans_persistent": plans[0].describe()["persistent"]}), flush=True)
+        for pc in plans:
+            pc.close()
+        plan.close()
+        return
     if args.applies_only:
         # profiling aid (ncu -k regex:fwd_kernel -s 1 / -k regex:adj_kernel): after the sparse forward above, three
         # forwards on a DENSE image and three adjoints, nothing else
@@ -514,6 +552,11 @@ def main():
     ap.add_argument("--phase-fp64", action="store_true", dest="phase_fp64", help="SL1M_PHASE_FP64: the fp64-phase kernels")
     ap.add_argument("--jitter-sigma", action="store_true", dest="jitter_sigma",
                     help="Gaussian configs: multiply every sigma_k by a seeded U(0.7, 1.3) draw (per-pixel-sigma kernels)")
+    ap.add_argument("--batch-stop", type=int, default=0, dest="batch_stop", metavar="C",
+                    help="side measurement: C channels (uvw scaled 0.9..1.1) solved to --tol in one sl1m_solve_stop_batch call")
+    ap.add_argument("--tol", type=float, default=1e-6)
+    ap.add_argument("--max-iter", type=int, default=7000, dest="max_iter")
+    ap.add_argument("--check-every", type=int, default=10, dest="check_every")
     ap.add_argument("--applies-only", action="store_true", dest="applies_only",
                     help="profiling aid: plan, one sparse forward, then 3 dense forwards and 3 adjoints; no solver, no bench line")
     ap.add_argument("--cont-iters", type=int, default=0, dest="cont_iters",
