@@ -966,6 +966,8 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
 // chunks of 128 visibilities as (u', v', w', x0[centre]) per centre plus (r_re, -r_im), so one
 // LDS.128 + one LDS.64 feed 8 terms.  NPQ of every 16 pairs (4 consecutive visibilities x 4
 // pairs) take the polynomial path.
+// A/B ONLY: this is the two-MUFU adjoint (sin and cos per term) that adj_kernel_c1 (one cosine per term)
+// replaced.  The default build never launches it; -DSL1M_ADJ_TWO_MUFU selects it for comparison runs.
 // ------------------------------------------------------------------------------------------
 template <int NPQ, bool BATCH = false>
 __global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const ApplyParams P) {
