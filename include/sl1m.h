@@ -108,7 +108,9 @@ int sl1m_adjoint_host(sl1m_plan *plan, const float *r_host, float *img_host, voi
  * sl1m_max_eig -- L = lambda_max(Re M^H M) by n_pow rounds of power iteration from the
  * deterministic start x = 1/sqrt(n_pix): g = M^H(M x), L = ||g||_2, x = g/L.  Approaches
  * lambda_max FROM BELOW; callers normally multiply by a safety factor (e.g. 1.05) before
- * passing it to sl1m_solve.  Writes *L_out_host (HOST) after one stream synchronise.
+ * passing it to sl1m_solve.  Writes *L_out_host (HOST) after one stream synchronise.  Plans that run the persistent
+ * kernel (sl1m_plan_info.persistent) do all n_pow rounds in one cooperative launch.  Overwrites the pixel tiles: ends a
+ * stepped FISTA run (sl1m_fista_begin).
  */
 int sl1m_max_eig(sl1m_plan *plan, int n_pow, float *L_out_host, void *stream);
 

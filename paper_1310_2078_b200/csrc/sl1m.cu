@@ -900,10 +900,47 @@ int max_eig_impl(sl1m_plan *p, int n_pow, float *L_out_host, void *stream) {
     if (n_pow < 1) return fail(SL1M_ERR_PARAM, "n_pow must be >= 1");
     cudaStream_t s = (cudaStream_t)stream;
     const int npad = p->n_pix_pad;
+    p->f_active = false;                 // the pixel tiles are about to hold the power iteration's vectors
     // x0 = 1/sqrt(n_pix) on real pixels
     fill_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->g_sorted, (float)(1.0 / std::sqrt((double)p->n_pix)), p->perm, npad);
     pack_sorted_kernel<<<cgrid(p, npad), ET, 0, s>>>(p->pix4, p->amp, p->g_sorted, npad, zs_of(p));
     p->launches += 2;
+    if (p->persist && !p->chan_scale) {   // small problem: all rounds in one cooperative launch (sl1m_persist.cuh)
+        PersistParams P;
+        memset(&P, 0, sizeof(P));
+        const int G = p->persist_grid;
+        P.n_vis = p->n_vis_int;
+        P.n_pix_pad = npad;
+        P.n_tiles = p->n_tiles;
+        P.nvg = std::max(1, std::min(PG, (p->n_vis_int + G - 1) / G));
+        int npg = 1;
+        while (npg < PG && npad / npg > G) npg <<= 1;
+        P.npg = npg;
+        P.vis4 = p->pvis4;
+        P.x0 = p->px0;
+        P.pix4 = p->pix4;
+        P.amp = p->amp;
+        P.rpol = p->rpol;
+        P.part = p->ppart;
+        P.bar = p->pbar;
+        P.n_iter = n_pow;
+        double *out = p->scalars;
+        CUDA_TRY(cudaMemsetAsync(p->pbar, 0, sizeof(unsigned), s));
+        void *args[] = {(void *)&P, (void *)&out};
+        const cudaError_t le = cudaLaunchCooperativeKernel((const void *)power_persistent_kernel, dim3((unsigned)G), dim3(PT), args, 0, s);
+        if (le == cudaSuccess) {
+            p->launches++;
+            int st = check_launch("sl1m_max_eig(persistent)");
+            if (st) return st;
+            double h = 0.0;
+            CUDA_TRY(cudaMemcpyAsync(&h, p->scalars, sizeof(double), cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(cudaStreamSynchronize(s));
+            L_out_host[0] = (float)std::sqrt(h);
+            return SL1M_OK;
+        }
+        if (le != cudaErrorCooperativeLaunchTooLarge && le != cudaErrorLaunchOutOfResources) CUDA_TRY(le);
+        cudaGetLastError();               // not co-resident right now: the multi-launch rounds below
+    }
     for (int it = 0; it < n_pow; ++it) {
         launch_fwd(p, s);
         fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,

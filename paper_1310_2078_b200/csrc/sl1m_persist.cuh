@@ -445,6 +445,160 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// a7 for the same small problems: n_iter rounds of the power iteration x <- g / ||g||, g = Re M^H (M x), in one
+// cooperative launch (the multi-launch version is 6 launches per round: for config 1, 30 rounds cost more than a
+// 100-iteration solve).  Same two phases and barriers as the FISTA kernel.  The normalisation needs ||g|| of the whole
+// image: phase B leaves a*g UNNORMALISED in the pixel tiles plus one fp64 partial of sum g^2 per CTA, and phase A of the
+// next round divides by the norm while it reads the tiles -- no third barrier.  out_norm2 = sum g^2 of the last round
+// (L = its square root, as sl1m_max_eig defines it).  P.pix4.w must hold a*x_0 on entry.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(PT, 1) power_persistent_kernel(const PersistParams P, double *out_norm2) {
+    __shared__ __align__(16) float4 s_list[PW][PBLK];
+    __shared__ uint16_t s_tile[PW][PBLK];
+    __shared__ __align__(16) float s_x0[PERSIST_MAX_TILES][PG];
+    __shared__ float s_red[PW][PG * 2 + 1];
+    __shared__ float s_inv;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int G = gridDim.x;
+    unsigned bar_target = 0;
+    const int items_a = (P.n_vis + P.nvg - 1) / P.nvg;
+    const int items_b = P.n_pix_pad / P.npg;
+    int staged_item = -1;
+
+    for (int it = 0; it < P.n_iter; ++it) {
+        // 1 / ||g|| of the previous round, from the per-CTA partials (every CTA forms the same number)
+        if (warp == 0) {
+            double v = 0.0;
+            if (it > 0) {
+                const double *prev = P.part + (size_t)((it - 1) & 1) * G;
+                for (int i = lane; i < G; i += 32) v += __ldcg(prev + i);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            }
+            if (lane == 0) s_inv = (it > 0) ? ((v > 0.0) ? (float)(1.0 / sqrt(v)) : 0.f) : 1.f;
+        }
+        __syncthreads();
+        const float inv = s_inv;
+        // ---- phase A: v = M x  (left in polar form for phase B)
+        for (int item = blockIdx.x; item < items_a; item += G) {
+            const int j0 = item * P.nvg;
+            if (staged_item != item) {
+                __syncthreads();
+                for (int i = tid; i < P.n_tiles * PG; i += PT) {
+                    const int tl = i / PG, r = i - tl * PG, j = min(j0 + r, P.n_vis - 1);
+                    s_x0[tl][r] = __ldg(P.x0 + (size_t)tl * P.n_vis + j);
+                }
+                __syncthreads();
+                staged_item = (items_a <= G) ? item : -1;
+            }
+            float uf[PG], vf[PG], wf[PG], acc[2 * PG];
+#pragma unroll
+            for (int r = 0; r < PG; ++r) {
+                const float4 v4 = __ldg(P.vis4 + min(j0 + r, P.n_vis - 1));
+                uf[r] = v4.x;
+                vf[r] = v4.y;
+                wf[r] = v4.z;
+                acc[2 * r] = 0.f;
+                acc[2 * r + 1] = 0.f;
+            }
+            for (int base = warp * PBLK; base < P.n_pix_pad; base += PW * PBLK) {
+                int cnt = 0;
+                float4 pxq[PBLK / 32];
+#pragma unroll
+                for (int q = 0; q < PBLK / 32; ++q) pxq[q] = __ldcg(P.pix4 + base + q * 32 + lane);
+#pragma unroll
+                for (int q = 0; q < PBLK / 32; ++q) {
+                    const int kpx = base + q * 32 + lane;
+                    float4 px = pxq[q];
+                    px.w *= inv;
+                    const bool nz = px.w != 0.f;
+                    const unsigned b = __ballot_sync(0xffffffffu, nz);
+                    if (nz) {
+                        const int pos = cnt + __popc(b & ((1u << lane) - 1u));
+                        s_list[warp][pos] = px;
+                        s_tile[warp][pos] = (uint16_t)(kpx / TP);
+                    }
+                    cnt += __popc(b);
+                }
+                __syncwarp();
+                for (int i = lane; i < cnt; i += 32) {
+                    const float4 px = s_list[warp][i];
+                    const float4 *x0q = reinterpret_cast<const float4 *>(s_x0[s_tile[warp][i]]);
+                    const float4 xa = x0q[0], xb = x0q[1];
+                    const float x0r[PG] = {xa.x, xa.y, xa.z, xa.w, xb.x, xb.y, xb.z, xb.w};
+#pragma unroll
+                    for (int r = 0; r < PG; ++r) {
+                        if (r < P.nvg) {
+                            const float X = fmaf(uf[r], px.x, fmaf(vf[r], px.y, fmaf(wf[r], px.z, x0r[r])));
+                            float sn, cs;
+                            __sincosf(X, &sn, &cs);
+                            acc[2 * r] = fmaf(px.w, cs, acc[2 * r]);
+                            acc[2 * r + 1] = fmaf(-px.w, sn, acc[2 * r + 1]);
+                        }
+                    }
+                }
+                __syncwarp();
+            }
+            const float sum = cta_sum<2 * PG>(acc, s_red);
+            const float other = __shfl_down_sync(0xffffffffu, sum, 1);
+            if (tid < 2 * P.nvg && (tid & 1) == 0 && j0 + (tid >> 1) < P.n_vis)
+                P.rpol[j0 + (tid >> 1)] = make_float2(sqrtf(fmaf(sum, sum, other * other)), atan2f(other, sum));
+        }
+        grid_barrier(P.bar, bar_target);
+        // ---- phase B: g = Re M^H v; the tiles receive a*g, the partial sum g^2
+        double g2 = 0.0;
+        for (int item = blockIdx.x; item < items_b; item += G) {
+            const int p0 = item * P.npg;
+            const float *x0row = P.x0 + (size_t)(p0 / TP) * P.n_vis;
+            float dl[PG], dm[PG], dn[PG], acc[PG];
+#pragma unroll
+            for (int i = 0; i < PG; ++i) {
+                const float4 px = __ldcg(P.pix4 + min(p0 + i, P.n_pix_pad - 1));
+                dl[i] = px.x;
+                dm[i] = px.y;
+                dn[i] = px.z;
+                acc[i] = 0.f;
+            }
+            for (int j = tid; j < P.n_vis; j += PT) {
+                const float4 v4 = __ldg(P.vis4 + j);
+                const float2 rp = __ldcg(P.rpol + j);
+                const float ph = __ldg(x0row + j) + rp.y;
+#pragma unroll
+                for (int i = 0; i < PG; ++i) {
+                    if (i < P.npg) {
+                        const float X = fmaf(v4.x, dl[i], fmaf(v4.y, dm[i], fmaf(v4.z, dn[i], ph)));
+                        acc[i] = fmaf(rp.x, __cosf(X), acc[i]);
+                    }
+                }
+            }
+            const float gsum = cta_sum<PG>(acc, s_red);
+            if (tid < P.npg) {
+                const float a = __ldg(P.amp + p0 + tid);
+                const float g = gsum * a;
+                P.pix4[p0 + tid].w = a * g;
+                if (P.y_sorted) P.y_sorted[p0 + tid] = g;          // the last round's g, for callers that want the vector
+                g2 += (double)g * g;
+            }
+        }
+        if (tid < 32) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) g2 += __shfl_xor_sync(0xffffffffu, g2, o);
+            if (tid == 0) P.part[(size_t)(it & 1) * G + blockIdx.x] = g2;
+        }
+        grid_barrier(P.bar, bar_target);
+    }
+    if (blockIdx.x == 0 && warp == 0) {
+        double v = 0.0;
+        const double *last = P.part + (size_t)((P.n_iter - 1) & 1) * G;
+        for (int i = lane; i < G; i += 32) v += __ldcg(last + i);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) *out_norm2 = v;
+    }
+}
+
 // Plan-time tables of the persistent kernel: vis4[j] = 2 pi (u, v, w) as floats, x0[t][j] = centre phase (fp64, reduced).
 __global__ void __launch_bounds__(256) persist_tables_kernel(const double *u64, const double *v64, const double *w64,
                                                              const double4 *cen, int n_vis, int n_tiles, float4 *vis4,

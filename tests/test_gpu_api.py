@@ -290,6 +290,13 @@ def test_persistent_small_problem_path(sl, n_vis, n_pix):
     plan = sl.Plan(uvw, l, m)
     ref_plan = sl.Plan(uvw, l, m, no_persistent=True)
     assert plan.describe()["persistent"] == 1 and ref_plan.describe()["persistent"] == 0
+    for n_pow in (1, 2, 9):             # the power iteration of these plans is one cooperative launch as well
+        L_ref, n0 = o.max_eig(n_pow), plan.launch_count
+        assert abs(plan.max_eig(n_pow) - L_ref) <= 1e-4 * L_ref, (n_pow, plan.max_eig(n_pow), L_ref)
+        assert abs(ref_plan.max_eig(n_pow) - L_ref) <= 1e-4 * L_ref
+    n0 = plan.launch_count
+    plan.max_eig(9)
+    assert plan.launch_count - n0 == 3  # fill, pack, one persistent launch
     Vd = _dev(V, torch.complex64)
     trace = torch.zeros(3 * K, dtype=torch.float64, device="cuda")
     n0 = plan.launch_count
