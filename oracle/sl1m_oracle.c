@@ -10,7 +10,9 @@
  * `double complex` with libm's csqrt-free primitives (sqrt, cexp); the only parallelism is an
  * OpenMP `parallel for` over independent outputs.  No blocking, fusion, reordering, range
  * reduction or real-arithmetic rewriting is done here, so it can be checked against the paper
- * by eye.  Citations are PAPER.md:<line> plus the section / equation.
+ * by eye.  The ONE deliberate shortcut: oracle_forward leaves out the terms with x_k == 0 (they add
+ * exactly 0 for finite entries), which is what makes V = M x_true affordable at 1 Mpixel.
+ * Citations are PAPER.md:<line> plus the section / equation.
  *
  *   O1 matrix entry      eq (9)  PAPER.md:117-120 (section 2.1)   delta pixels
  *                        eq (16) PAPER.md:160-163 (section 2.2)   Gaussian pixels, paraxial
