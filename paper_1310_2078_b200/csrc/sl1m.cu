@@ -155,6 +155,8 @@ struct sl1m_plan {
     float *px0 = nullptr;            // [n_tiles][n_vis] centre phases
     double *ppart = nullptr;         // [2][3][persist_grid]
     unsigned *pbar = nullptr;        // grid-barrier counter
+    bool persist_small = false;      // <= 1,024 padded pixels and visibilities: fista_persistent_small_kernel (all operands in registers)
+    float *pybuf = nullptr;          // DEV [2][n_pix_pad] its double-buffered a*y
     float *pbeta = nullptr;          // DEV [pbeta_cap] momentum coefficients of one launch
     int pbeta_cap = 0;
     std::vector<float> pbeta_host;   // staging of the same (must outlive the asynchronous copy: plan-owned)
@@ -176,7 +178,7 @@ void free_plan(sl1m_plan *p) {
                     p->perm, p->vperm, p->gF, p->gA, p->ws_v, p->ws_p, p->resid, p->I_sorted, p->y_sorted,
                     p->g_sorted, p->part_a, p->part_b, p->part_c, p->scalars, p->h_x, p->h_vis, p->h_img,
                     p->trace_buf, p->chan_scale, p->step_c, p->pixd, p->pixc, p->tile_cnt, p->gFc, p->rpol, p->ctl_i,
-                    p->lam2, p->pixdc, p->pixgc, p->pvis4, p->px0, p->ppart, p->pbar, p->pbeta, p->gAc};
+                    p->lam2, p->pixdc, p->pixgc, p->pvis4, p->px0, p->ppart, p->pbar, p->pbeta, p->gAc, p->pybuf};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (p->h_flag) cudaFreeHost(p->h_flag);
@@ -381,6 +383,12 @@ int persist_setup(sl1m_plan *p) {
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaDeviceSynchronize());
     p->persist = true;
+    // the smallest problems: every operand in registers, one work item per CTA and phase, the last CTA idle
+    if (p->n_pix_pad <= PW * PBLK && p->n_vis_int <= 4 * PT && p->persist_grid >= 130) {
+        CUDA_TRY(cudaMalloc((void **)&p->pybuf, 2 * (size_t)p->n_pix_pad * sizeof(float)));
+        CUDA_TRY(cudaMemset(p->pybuf, 0, 2 * (size_t)p->n_pix_pad * sizeof(float)));
+        p->persist_small = true;
+    }
     return SL1M_OK;
 }
 
@@ -1081,7 +1089,13 @@ int persist_iterate(sl1m_plan *p, int n_iter, double *trace_rows, const StopOpts
     P.beta = p->pbeta;
     CUDA_TRY(cudaMemsetAsync(p->pbar, 0, sizeof(unsigned), s));
     void *args[] = {(void *)&P};
-    const cudaError_t le = cudaLaunchCooperativeKernel((const void *)fista_persistent_kernel, dim3((unsigned)G), dim3(PT), args, 0, s);
+    const void *kern = (const void *)fista_persistent_kernel;
+    if (p->persist_small) {
+        P.nvg = std::max(1, (p->n_vis_int + G - 2) / (G - 1));   // the last CTA stays idle: it sums the objective partials
+        P.ybuf = p->pybuf;
+        kern = (const void *)fista_persistent_small_kernel;
+    }
+    const cudaError_t le = cudaLaunchCooperativeKernel(kern, dim3((unsigned)G), dim3(PT), args, 0, s);
     if (le == cudaErrorCooperativeLaunchTooLarge || le == cudaErrorLaunchOutOfResources) {
         // the grid cannot be co-resident right now (e.g. the GPU is shared): this plan goes back to the multi-launch
         // loop for good.  Its compact tiles are rebuilt from y (the persistent kernel does not maintain them).

@@ -60,6 +60,7 @@ struct PersistParams {
     const float *beta;             // [n_iter] momentum coefficients (t_k - 1)/t_{k+1} of this launch's iterations, formed in
                                    // fp64 on the host (a device fp64 sqrt + divide cost 0.3 us per iteration on the critical path)
     int n_iter;
+    float *ybuf;                   // [2][n_pix_pad] a*y_k, double-buffered by iteration parity (fista_persistent_small_kernel)
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
@@ -442,6 +443,239 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
     if (one_item_b && blockIdx.x < items_b && tid < P.npg) {
         P.I_sorted[blockIdx.x * P.npg + tid] = I_own;
         P.y_sorted[blockIdx.x * P.npg + tid] = y_own;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// The smallest problems (<= 1,024 padded pixels, <= 1,024 visibilities, one work item per CTA and phase: config 1).
+// The same two phases and barriers as above, specialised: every iteration-invariant operand is in registers (also the
+// (dl, dm, dn') of the pixels a thread reads in phase A), and a*y travels as 4-byte floats through a buffer that is
+// double-buffered by iteration parity instead of inside the 16-byte pixel records.  4.70 us per iteration at config 1
+// against 5.15 us for the general kernel.
+// Tried here and dropped: a ONE-barrier mode for sparse iterates, in which every pixel-owning CTA recomputes the whole
+// residual itself (nnz * n_vis sincos per CTA; 13 non-zero pixels at config 1) instead of receiving it from the
+// visibility owners -- 5.56 us: at 8 warps per SM the recomputation is a latency chain longer than the barrier it saves.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(PT, 1) fista_persistent_small_kernel(const PersistParams P) {
+    __shared__ __align__(16) float4 s_list[PW][PBLK];       // compacted non-zero pixels, per warp
+    __shared__ uint16_t s_tile[PW][PBLK];
+    __shared__ __align__(16) float s_x0[4][PG];              // centre phases of the CTA's phase-A item (<= 4 tiles)
+    __shared__ float s_red[PW][PG * 2 + 1];
+    __shared__ int s_stop;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int G = gridDim.x, cta = blockIdx.x;
+    unsigned bar_target = 0;
+    const int items_a = (P.n_vis + P.nvg - 1) / P.nvg, items_b = P.n_pix_pad / P.npg;
+    const bool has_a = cta < items_a, has_b = cta < items_b;
+    const int tracer = G - 1;                                // idle in both phases (host-side condition)
+    double E_prev = 0.0, N_prev = 0.0;
+
+    // ---- iteration-invariant operands
+    const int j0 = cta * P.nvg, p0 = cta * P.npg;
+    float uf[PG], vf[PG], wf[PG];
+    float2 Vj = make_float2(0.f, 0.f);
+    if (has_a) {
+        for (int i = tid; i < P.n_tiles * PG; i += PT) {
+            const int tl = i / PG, r = i - tl * PG;
+            s_x0[tl][r] = __ldg(P.x0 + (size_t)tl * P.n_vis + min(j0 + r, P.n_vis - 1));
+        }
+#pragma unroll
+        for (int r = 0; r < PG; ++r) {
+            const float4 v4 = __ldg(P.vis4 + min(j0 + r, P.n_vis - 1));
+            uf[r] = v4.x;
+            vf[r] = v4.y;
+            wf[r] = v4.z;
+        }
+        if (tid < 2 * P.nvg && (tid & 1) == 0 && j0 + (tid >> 1) < P.n_vis) Vj = __ldg(P.V + j0 + (tid >> 1));
+    }
+    float3 pxc[PBLK / 32];                                   // (dl, dm, dn') of the pixels this thread reads every iteration
+#pragma unroll
+    for (int q = 0; q < PBLK / 32; ++q) {
+        const int kpx = warp * PBLK + q * 32 + lane;
+        const float4 px = (kpx < P.n_pix_pad) ? __ldcg(P.pix4 + kpx) : make_float4(0.f, 0.f, 0.f, 0.f);
+        pxc[q] = make_float3(px.x, px.y, px.z);
+    }
+    float dl[PG], dm[PG], dn[PG], a_own = 0.f, y_own = 0.f, I_own = 0.f, x0v[4];
+    float4 v4r[4];
+    {
+        const float *x0row = P.x0 + (size_t)(min(p0, P.n_pix_pad - 1) / TP) * P.n_vis;
+#pragma unroll
+        for (int i = 0; i < PG; ++i) {
+            const float4 px = __ldcg(P.pix4 + min(p0 + i, P.n_pix_pad - 1));
+            dl[i] = px.x;
+            dm[i] = px.y;
+            dn[i] = px.z;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int j = min(tid + q * PT, P.n_vis - 1);
+            v4r[q] = __ldg(P.vis4 + j);
+            x0v[q] = __ldg(x0row + j);
+        }
+        if (has_b && tid < P.npg) {
+            a_own = __ldg(P.amp + p0 + tid);
+            y_own = P.y_sorted[p0 + tid];
+            I_own = P.I_sorted[p0 + tid];
+            P.ybuf[(size_t)((P.k0 + 1) & 1) * P.n_pix_pad + p0 + tid] = a_own * y_own;   // a*y of this launch's first iteration
+        }
+    }
+    grid_barrier(P.bar, bar_target);                         // the first iteration's a*y is in place
+
+    for (int it = 0; it < P.n_iter; ++it) {
+        const int k = P.k0 + it + 1;
+        double *part = P.part + (size_t)(k & 1) * 3 * G;
+        const float *ycur = P.ybuf + (size_t)(k & 1) * P.n_pix_pad;
+        float *ynext = P.ybuf + (size_t)((k + 1) & 1) * P.n_pix_pad;
+        const float beta = __ldg(P.beta + it);
+        // ---- read a*y_k, compact the non-zeros of the warp's block
+        int cnt = 0;
+        {
+            float wq[PBLK / 32];
+#pragma unroll
+            for (int q = 0; q < PBLK / 32; ++q) {
+                const int kpx = warp * PBLK + q * 32 + lane;
+                wq[q] = (kpx < P.n_pix_pad) ? __ldcg(ycur + kpx) : 0.f;
+            }
+#pragma unroll
+            for (int q = 0; q < PBLK / 32; ++q) {
+                const bool nz = wq[q] != 0.f;                // NaN counts as non-zero and propagates
+                const unsigned b = __ballot_sync(0xffffffffu, nz);
+                if (nz) {
+                    const int pos = cnt + __popc(b & ((1u << lane) - 1u));
+                    s_list[warp][pos] = make_float4(pxc[q].x, pxc[q].y, pxc[q].z, wq[q]);
+                    s_tile[warp][pos] = (uint16_t)((warp * PBLK + q * 32 + lane) / TP);
+                }
+                cnt += __popc(b);
+            }
+        }
+        __syncwarp();
+        float2 rp[4];                                        // residual of the thread's visibilities, polar
+        double r2 = 0.0;
+        {
+            // ---- phase A: the CTA's <= 8 visibilities against every non-zero pixel (each warp: its own compacted block)
+            if (has_a) {
+                float acc[2 * PG];
+#pragma unroll
+                for (int r = 0; r < 2 * PG; ++r) acc[r] = 0.f;
+                for (int i = lane; i < cnt; i += 32) {
+                    const float4 px = s_list[warp][i];
+                    const float4 *x0q = reinterpret_cast<const float4 *>(s_x0[s_tile[warp][i]]);
+                    const float4 xa = x0q[0], xb = x0q[1];
+                    const float x0r[PG] = {xa.x, xa.y, xa.z, xa.w, xb.x, xb.y, xb.z, xb.w};
+#pragma unroll
+                    for (int r = 0; r < PG; ++r) {
+                        if (r < P.nvg) {
+                            const float X = fmaf(uf[r], px.x, fmaf(vf[r], px.y, fmaf(wf[r], px.z, x0r[r])));
+                            float sn, cs;
+                            __sincosf(X, &sn, &cs);
+                            acc[2 * r] = fmaf(px.w, cs, acc[2 * r]);
+                            acc[2 * r + 1] = fmaf(-px.w, sn, acc[2 * r + 1]);
+                        }
+                    }
+                }
+                const float sum = cta_sum<2 * PG>(acc, s_red);
+                const float other = __shfl_down_sync(0xffffffffu, sum, 1);
+                if (tid < 2 * P.nvg && (tid & 1) == 0 && j0 + (tid >> 1) < P.n_vis) {
+                    const float re = sum - Vj.x, im = other - Vj.y;
+                    P.rpol[j0 + (tid >> 1)] = make_float2(sqrtf(fmaf(re, re, im * im)), atan2f(im, re));
+                    r2 = (double)re * re + (double)im * im;
+                }
+            }
+            if (tid < 32) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+                if (tid == 0) part[cta] = r2;
+            }
+            grid_barrier(P.bar, bar_target);
+            if (has_b) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    rp[q] = (tid + q * PT < P.n_vis) ? __ldcg(P.rpol + tid + q * PT) : make_float2(0.f, 0.f);
+            }
+        }
+        // ---- phase B: g = Re M^H r on the CTA's pixels, gradient step, T^{lambda/L}, momentum
+        double l1 = 0.0, nzs = 0.0;
+        if (has_b) {
+            float acc[PG];
+#pragma unroll
+            for (int i = 0; i < PG; ++i) acc[i] = 0.f;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float ph = x0v[q] + rp[q].y;
+#pragma unroll
+                for (int i = 0; i < PG; ++i) {
+                    if (i < P.npg) {
+                        const float X = fmaf(v4r[q].x, dl[i], fmaf(v4r[q].y, dm[i], fmaf(v4r[q].z, dn[i], ph)));
+                        acc[i] = fmaf(rp[q].x, __cosf(X), acc[i]);
+                    }
+                }
+            }
+            const float gsum = cta_sum<PG>(acc, s_red);
+            if (tid < P.npg) {
+                const float g = gsum * a_own;
+                const float z = fmaf(-P.inv_L, g, y_own);
+                const float I_new = (z > P.thr) ? z - P.thr : 0.f;
+                const float y_new = fmaf(beta, I_new - I_own, I_new);
+                I_own = I_new;
+                y_own = y_new;
+                ynext[p0 + tid] = a_own * y_new;
+                l1 = (double)I_new;
+                nzs = (I_new != 0.f) ? 1.0 : 0.0;
+            }
+        }
+        if (tid < 32) {
+#pragma unroll
+            for (int o = 4; o > 0; o >>= 1) {                // lanes 0..7 hold terms
+                l1 += __shfl_xor_sync(0xffffffffu, l1, o);
+                nzs += __shfl_xor_sync(0xffffffffu, nzs, o);
+            }
+            if (tid == 0) {
+                part[G + cta] = l1;
+                part[2 * G + cta] = nzs;
+            }
+        }
+        grid_barrier(P.bar, bar_target);
+        // ---- a6 on the idle CTA (trace row) and, at looked-at iterations, the stopping rules in every CTA
+        const bool look = P.check_every > 0 && k >= 2 && (k % P.check_every) == 0;
+        const bool before_look = P.check_every > 0 && ((k + 1) % P.check_every) == 0;
+        if (look || before_look || (P.trace && cta == tracer)) {
+            if (warp == 0) {
+                double l2s, l1s, nz3;
+                warp_sum3_cg(part, G, l2s, l1s, nz3);
+                if (lane == 0) {
+                    if (P.trace && cta == tracer) {
+                        P.trace[3 * (size_t)it] = l2s;
+                        P.trace[3 * (size_t)it + 1] = l1s;
+                        P.trace[3 * (size_t)it + 2] = nz3;
+                    }
+                    const double E = l2s + P.lam2 * l1s;
+                    int stop = 0;
+                    if (look)
+                        stop = (P.tol >= 0.0 && fabs(E - E_prev) <= P.tol * fabs(E)) ||
+                               (P.nnz_tol >= 0.0 && fabs(nz3 - N_prev) <= P.nnz_tol * nz3);
+                    E_prev = E;
+                    N_prev = nz3;
+                    s_stop = stop;
+                    if (stop && cta == 0) {
+                        P.ctl[0] = 1;
+                        P.ctl[1] = k;
+                        P.ctl[2] = 1;
+                    }
+                }
+            }
+            if (P.check_every > 0) {
+                __syncthreads();
+                if (s_stop) break;
+                __syncthreads();
+            }
+        }
+    }
+    // ---- the state goes back to global memory (next launch, sl1m_fista_image, the other kernels)
+    if (has_b && tid < P.npg) {
+        P.I_sorted[p0 + tid] = I_own;
+        P.y_sorted[p0 + tid] = y_own;
+        P.pix4[p0 + tid].w = a_own * y_own;
     }
 }
 
