@@ -387,6 +387,37 @@ int sl1m_debug_bounds_build(void);
  * see sl1m_debug_check report it. */
 int sl1m_debug_poke_past_end(sl1m_plan *plan);
 
+/*
+ * sl1m_forward_noalloc -- v = M x of eq (9) (delta pixels, unit gains, one channel) WITHOUT a plan
+ * and without any allocation, for callers that cannot ask the CUDA driver for memory when they need an apply:
+ * a real-time pipeline whose other streams must keep running (cudaMalloc / cudaFree hold up the whole device), a
+ * process whose device memory belongs entirely to someone else's pool (a raw cudaMalloc fails there, or takes what a
+ * neighbour was promised), a service bound to a fixed memory footprint after start-up.  Every plan-based call is
+ * closed to them because sl1m_plan_create allocates the plan's workspaces.
+ *   uvw_dev  DEV [n_vis][3] fp64, wavelengths.          l_dev, m_dev  DEV [n_pix] fp64 direction cosines.
+ *   x_dev    DEV [n_pix] fp32 image.                                  vis_dev       DEV [n_vis][2] fp32 (re, im), overwritten.
+ * All five buffers stay the caller's; they are read / written in the caller's order and not copied.
+ * Scratch: the per-split partial sums go to ONE array compiled into the library (4 MiB of device memory on every GPU
+ * that loads the library, held until the process exits).  Consequences:
+ *  - limits: n_vis <= SL1M_NOALLOC_MAX_VIS and n_pix <= SL1M_NOALLOC_MAX_PIX, else SL1M_ERR_SIZE (checked before any
+ *    device work) with sl1m_last_error() naming the limit; larger problems need a plan, or one call per block of
+ *    visibilities (rows of M are independent);
+ *  - all calls on a device share the array.  Calls issued to the SAME stream are safe back to back.  Calls that may
+ *    run at the same time on the GPU (different streams, different host threads) overwrite each other's partial sums
+ *    and give wrong visibilities without any error: serialise them yourself;
+ *  - the array keeps the previous call's contents; nothing in it has to start at zero, because every slot the final
+ *    sum reads is first written by the same call.
+ * The FIRST call on each device looks up the array's device address (once per device, the device current at the
+ * call) -- make that first call at start-up, outside any stream capture; later calls only launch two kernels.
+ * Asynchronous on `stream`; deterministic (fixed summation order).  l^2 + m^2 >= 1 is NOT checked (the inputs are
+ * on the device): such a pixel poisons the output with NaN.  Accuracy as sl1m_forward (phase in fp64, relative L2
+ * <= 2e-4 against the fp64 definition); slower than a plan's forward -- no sort, no tile centres, no zero skipping.
+ */
+#define SL1M_NOALLOC_MAX_VIS 524288   /* = 4 MiB of scratch / 8 B per complex partial */
+#define SL1M_NOALLOC_MAX_PIX 16777216
+int sl1m_forward_noalloc(int64_t n_vis, const double *uvw_dev, int64_t n_pix, const double *l_dev, const double *m_dev,
+                         const float *x_dev, float *vis_dev, void *stream);
+
 /* Number of kernels this plan has launched since creation (for bench.py's gpu_launches). */
 int64_t sl1m_launch_count(const sl1m_plan *plan);
 

@@ -8,5 +8,5 @@ raises.
 """
 from .binding import (  # noqa: F401
     GAUSS_PARAXIAL, GAUSS_WIDEFIELD, PHASE_FP64, DENSE_FORWARD, NO_PERSISTENT, Plan, Sl1mError, SolveInfo, build_library, library_path,
-    load_library, exported_symbols, quadtree_refine, quadtree_solve, measure_peaks,
+    load_library, exported_symbols, quadtree_refine, quadtree_solve, measure_peaks, forward_noalloc, NOALLOC_MAX_VIS, NOALLOC_MAX_PIX,
 )

@@ -126,6 +126,7 @@ def load_library():
     lib.sl1m_plan_describe.argtypes = [vp, ctypes.POINTER(_PlanInfo)]
     lib.sl1m_forward_active_pixels.argtypes = [vp, vp, vp]
     lib.sl1m_measure_peaks.argtypes = [ctypes.POINTER(_Peaks), vp]
+    lib.sl1m_forward_noalloc.argtypes = [i64, vp, i64, vp, vp, vp, vp, vp]
     lib.sl1m_debug_check.argtypes = []
     lib.sl1m_debug_bounds_build.argtypes = []
     lib.sl1m_debug_poke_past_end.argtypes = [vp]
@@ -181,6 +182,27 @@ def measure_peaks(stream=None) -> dict:
     pk = _Peaks()
     _check(load_library().sl1m_measure_peaks(ctypes.byref(pk), _stream_ptr(stream)))
     return {n: (int(getattr(pk, n)) if n == "n_sm" else float(getattr(pk, n))) for n, _ in _Peaks._fields_}
+
+
+NOALLOC_MAX_VIS = 524288      # SL1M_NOALLOC_MAX_VIS
+NOALLOC_MAX_PIX = 16777216    # SL1M_NOALLOC_MAX_PIX
+
+
+def forward_noalloc(uvw, l, m, x, out, stream=None):
+    """sl1m_forward_noalloc: v = M x (eq 9, delta pixels, unit gains) without a plan and without the library asking the
+    driver for memory -- for callers that cannot allocate at this point (busy real-time streams that a cudaMalloc would
+    stall, device memory owned by another pool, fixed-footprint services).  Everything is a CUDA tensor the caller made
+    beforehand: uvw [n_vis][3] float64, l / m [n_pix] float64, x [n_pix] float32, out [n_vis] complex64 (overwritten and
+    returned; this function creates no tensor).  The partial sums live in one 4 MiB array inside the library, shared by
+    every call on the device: at most NOALLOC_MAX_VIS visibilities per call, and do not let two calls overlap on the
+    GPU.  Make the first call per device at start-up (it looks up the array's address); see include/sl1m.h."""
+    import torch
+    n_vis, n_pix = int(out.numel()), int(x.numel())
+    _check(load_library().sl1m_forward_noalloc(
+        n_vis, _dev_ptr(uvw, torch.float64, 3 * n_vis, "uvw"), n_pix, _dev_ptr(l, torch.float64, n_pix, "l"),
+        _dev_ptr(m, torch.float64, n_pix, "m"), _dev_ptr(x, torch.float32, n_pix, "x"),
+        _dev_ptr(out, torch.complex64, n_vis, "out"), _stream_ptr(stream)))
+    return out
 
 
 def quadtree_refine(l, m, side, I, frac: float, min_side: float):

@@ -8,7 +8,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "sl1m.cu")
 SRC_QT = os.path.join(_HERE, "csrc", "sl1m_quadtree.cu")
 SRC_PK = os.path.join(_HERE, "csrc", "sl1m_peaks.cu")
-DEPS = [SRC, SRC_QT, SRC_PK, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"), os.path.join(_HERE, "csrc", "sl1m_persist.cuh"), os.path.join(_HERE, "csrc", "sl1m_internal.h"),
+SRC_NA = os.path.join(_HERE, "csrc", "sl1m_noalloc.cu")     # sl1m_forward_noalloc: static device scratch, no cudaMalloc
+DEPS = [SRC, SRC_QT, SRC_PK, SRC_NA, os.path.join(_HERE, "csrc", "sl1m_kernels.cuh"), os.path.join(_HERE, "csrc", "sl1m_epilogue.cuh"), os.path.join(_HERE, "csrc", "sl1m_persist.cuh"), os.path.join(_HERE, "csrc", "sl1m_internal.h"),
         os.path.join(os.path.dirname(_HERE), "include", "sl1m.h")]
 LIB = os.path.join(_HERE, "libsl1m.so")
 LIB_BOUNDS = os.path.join(_HERE, "libsl1m_bounds.so")      # debug build: canary bands + asserted prefetches (-DSL1M_BOUNDS)
@@ -30,7 +31,7 @@ def build_library(force: bool = False, verbose: bool = False, bounds: bool = Fal
     if force or stale:
         tmp = lib + f".tmp{os.getpid()}"
         extra = os.environ.get("SL1M_NVCC_EXTRA", "").split() + (["-DSL1M_BOUNDS"] if bounds else [])   # SL1M_NVCC_EXTRA: tuning -D flags
-        cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-o", tmp, SRC, SRC_QT, SRC_PK]
+        cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-o", tmp, SRC, SRC_QT, SRC_PK, SRC_NA]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)
