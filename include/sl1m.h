@@ -92,7 +92,8 @@ int sl1m_plan_create(sl1m_plan **out, int64_t n_vis, const double *uvw, const in
                      const double *sigma, int32_t n_ant, const float *gains, int gauss_model,
                      uint32_t flags);
 
-/* v = M x.  x DEV [n_pix] fp32 (real), vis DEV [n_vis][2] fp32.  Asynchronous on stream. */
+/* v = M x.  x DEV [n_pix] fp32 (real), vis DEV [n_vis][2] fp32.  Asynchronous on stream.  Safe inside a stepped
+ * FISTA run (see sl1m_fista_begin). */
 int sl1m_forward(sl1m_plan *plan, const float *x_dev, float *vis_dev, void *stream);
 
 /* g = Re M^H r.  r DEV [n_vis][2] fp32, img DEV [n_pix] fp32.  Asynchronous on stream.
@@ -193,7 +194,13 @@ int sl1m_solve_stop_batch(sl1m_plan *plan, const float *vis_dev, const float *la
  *   sl1m_fista_step   n_iter more iterations, asynchronous on stream.  trace_dev DEV [n_chan][max(n_iter,1)][3] or
  *                     NULL receives the rows of THIS call's iterations.
  *   sl1m_fista_image  x_out DEV [n_chan][n_pix] = I_k; *n_iter_done_host (nullable) = k.  Asynchronous.
- * Any other solve call on the plan, or sl1m_plan_set_channels, ends the state.
+ * Any solve call on the plan, sl1m_max_eig, or sl1m_plan_set_channels ends the state; a later sl1m_fista_step /
+ * sl1m_fista_image then fails with SL1M_ERR_PARAM ("no FISTA state").  Only sl1m_fista_begin opens one: every
+ * sl1m_solve* variant ends whatever run was open and leaves none behind (its vis_dev is not borrowed past the call),
+ * with or without info_host.
+ * sl1m_forward / sl1m_adjoint (and their _host and dirty-image forms) may be called BETWEEN steps without disturbing
+ * the run -- e.g. step, sl1m_fista_image, sl1m_forward(I_k) to show the model visibilities, step again: the forward
+ * restores the run's a*y_{k+1} pixel tiles after using them for the caller's image (one extra O(n_pix) launch).
  */
 int sl1m_fista_begin(sl1m_plan *plan, const float *vis_dev, const float *lambda_host,
                      const float *L_host, const float *x0_dev, void *stream);
@@ -345,7 +352,9 @@ int sl1m_plan_describe(const sl1m_plan *plan, sl1m_plan_info *info_host);
  * kernels) get a compact copy of that array as well.  Plans whose compact gain rows would exceed 8 GiB keep the dense
  * forward (sl1m_plan_info.zero_skip == 0), as does SL1M_DENSE_FORWARD.  The adjoint always evaluates every term.
  * n_active_host: HOST [n_chan]; pixels the most recently packed forward input streams per channel (padded to
- * 4 per tile; n_pix_padded when the plan does not skip).  Synchronises `stream`.
+ * 4 per tile; n_pix_padded when the plan does not skip).  During a stepped run on a persistent plan
+ * (sl1m_plan_info.persistent; its kernels skip zeros straight from y and keep no compact tiles): the exact number of
+ * pixels with y_{k+1} != 0, which is what the next iteration's forward evaluates.  Synchronises `stream`.
  */
 int sl1m_forward_active_pixels(sl1m_plan *plan, int64_t *n_active_host, void *stream);
 

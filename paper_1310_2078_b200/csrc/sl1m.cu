@@ -271,9 +271,6 @@ int configure_and_allocate(sl1m_plan *p) {
         int rv = 8;
         while (rv > 1 && p->gk != 2 && (int64_t)((nvi + NT * rv - 1) / (NT * rv)) * p->n_tiles * p->n_chan < 2 * SM_COUNT_B200)
             rv >>= 1;
-#ifdef SL1M_FORCE_R
-        rv = SL1M_FORCE_R;
-#endif
         if (p->phase64) rv = std::min(rv, 4);   // fp64 uvw live in registers
         p->fwd_rv = rv;
         p->fwd_vtiles = (int)((nvi + NT * rv - 1) / (NT * rv));
@@ -282,9 +279,6 @@ int configure_and_allocate(sl1m_plan *p) {
         int split = (nvi * (int64_t)p->n_tiles >= (int64_t)64 * SM_COUNT_B200)
                         ? pick_split(p->fwd_vtiles, p->n_tiles, SM_COUNT_B200 * fwd_ctas, waves, p->n_chan)
                         : std::min(p->n_tiles, std::max(1, (target + p->fwd_vtiles - 1) / p->fwd_vtiles));
-#ifdef SL1M_FORCE_FWD_PER_SPLIT
-        split = (p->n_tiles + SL1M_FORCE_FWD_PER_SPLIT - 1) / SL1M_FORCE_FWD_PER_SPLIT;   // tuning knob
-#endif
         p->fwd_per_split = (p->n_tiles + split - 1) / split;
         p->fwd_split = (p->n_tiles + p->fwd_per_split - 1) / p->fwd_per_split;
     }
@@ -292,9 +286,6 @@ int configure_and_allocate(sl1m_plan *p) {
         const int n_chunks = (p->n_vis_int + VC - 1) / VC;
         int rp = 8;
         while (rp > 1 && (int64_t)(p->n_pix_pad / (NT * rp)) * n_chunks * p->n_chan < 2 * SM_COUNT_B200) rp >>= 1;
-#ifdef SL1M_FORCE_R
-        rp = SL1M_FORCE_R;
-#endif
         if (p->phase64) rp = std::min(rp, 4);
         p->adj_rp = rp;
         p->adj_pgroups = p->n_pix_pad / (NT * rp);
@@ -727,14 +718,10 @@ void launch_adj_rp(const sl1m_plan *p, const ApplyParams &P, dim3 grid, cudaStre
     switch (p->adj_rp) {
         case 8:
             if constexpr (PK == 0 && GK == 0) {
-#ifdef SL1M_ADJ_TWO_MUFU
-                adj_kernel_x2<SL1M_ADJ_NPQ, B><<<grid, NT, 0, s>>>(P);
-#else
                 ApplyParams Q = P;      // one cosine per term: the kernel reads the residual in polar form
                 vis_polar_kernel<<<dim3((unsigned)egrid((size_t)p->n_vis_int), (unsigned)p->n_chan), ET, 0, s>>>(P.r, p->rpol, p->n_vis_int, p->done_ptr);
                 Q.r = p->rpol;
                 adj_kernel_c1<SL1M_ADJ_C1_NPQ, B><<<grid, NT, 0, s>>>(Q);
-#endif
             }
             else if constexpr (PK == 0 && GK == 2) adj_kernel_g2x2<SL1M_ADJ_G2_NPQ, B><<<grid, NT, 0, s>>>(P);
             else if constexpr (PK == 2 && GK == 0) adj_kernel_gtx2<B><<<grid, NT, 0, s>>>(P);
@@ -822,9 +809,7 @@ void launch_adj(sl1m_plan *p, const float2 *r, cudaStream_t s) {
         default: launch_adj_rp<1, 2>(p, P, grid, s); break;
     }
     p->launches++;
-#ifndef SL1M_ADJ_TWO_MUFU
     if (key == 0 && p->adj_rp == 8) p->launches++;   // vis_polar_kernel in front of the one-cosine kernel
-#endif
 }
 
 int check_launch(const char *what) {
@@ -843,6 +828,13 @@ extern "C" int sl1m_forward(sl1m_plan *p, const float *x_dev, float *vis_dev, vo
     fwd_reduce_kernel<<<cgrid(p, p->n_vis_int), ET, 0, s>>>(p->ws_v, p->fwd_split, p->n_vis_int, p->vperm, nullptr,
                                                             (float2 *)vis_dev, 0, nullptr, (int)p->n_vis, p->n_part);
     p->launches += 2;
+    if (p->f_active) {
+        // A stepped FISTA run is open and its next iteration reads a*y_{k+1} from the pixel tiles, which now hold the
+        // caller's a*x: put them back from y_sorted (every solver path keeps it current), so that
+        // begin / step / forward(I_k) / step continues the same run.
+        pack_sorted_kernel<<<cgrid(p, p->n_pix_pad), ET, 0, s>>>(p->pix4, p->amp, p->y_sorted, p->n_pix_pad, zs_of(p));
+        p->launches++;
+    }
     return check_launch("sl1m_forward");
 }
 
@@ -1122,6 +1114,10 @@ int fista_iterate(sl1m_plan *p, int n_iter, double *trace_dev, size_t trace_stri
     const float2 *step_c = C > 1 ? p->step_c : nullptr;
     const int *done = stop ? p->ctl_i : nullptr;
     p->done_ptr = done;
+    struct DoneGuard {      // every exit, the CUDA_TRY early returns included, leaves no stale stop flags behind
+        sl1m_plan *q;
+        ~DoneGuard() { q->done_ptr = nullptr; }
+    } done_guard{p};
     int pending[2] = {0, 0}, slot = 0, looks = 0;
     // How far the host may run ahead of the device's decision.  Small problems (an iteration is tens of
     // microseconds): read the flag every >= 16 iterations, two polls behind -- the iterations enqueued past the stop
@@ -1177,7 +1173,6 @@ int fista_iterate(sl1m_plan *p, int n_iter, double *trace_dev, size_t trace_stri
             }
         }
     }
-    p->done_ptr = nullptr;
     return check_launch("sl1m_fista_step");
 }
 
@@ -1226,6 +1221,10 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
         }
     }
     if ((st = fista_begin_impl(p, vis_dev, lambda_c, L_c.data(), x0_dev, s))) return st;
+    struct StateGuard {     // whichever way this call ends
+        sl1m_plan *q;
+        ~StateGuard() { q->f_active = false; q->f_vis = nullptr; }
+    } state_guard{p};
     if ((st = fista_iterate(p, n_iter, trace_dev, trace_stride, 0, stop, s))) return st;
     const int n_enqueued = p->f_k;
     if ((st = fista_image_impl(p, x_out_dev, s))) return st;
@@ -1256,6 +1255,9 @@ int solve_impl(sl1m_plan *p, const float *vis_dev, const float *lambda_c, const 
             info_host[c].nnz = (int64_t)(h[4 * c + 3] + 0.5);
         }
     }
+    // Only sl1m_fista_begin opens a state that can be stepped: a solve's vis_dev is the caller's to free on return,
+    // so a later sl1m_fista_step / sl1m_fista_image must fail with "no FISTA state" instead of reading it
+    // (state_guard above).
     return SL1M_OK;
 }
 }  // namespace
@@ -1442,11 +1444,7 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     const bool grouped = !pk && p->gk == 2;        // delta pixels, baseline-grouped gains
     o->fwd_poly_per16 = plain ? (p->fwd_rv == 8 ? SL1M_FWD_NPQ : (p->fwd_rv == 4 ? (SL1M_FWD_NPOLY8 / 2) * 4 : 0))
                               : (grouped ? SL1M_FWD_G2_NPQ : 0);
-#ifdef SL1M_ADJ_TWO_MUFU
-    constexpr int adj_npq8 = SL1M_ADJ_NPQ;
-#else
     constexpr int adj_npq8 = SL1M_ADJ_C1_NPQ;
-#endif
     o->adj_poly_per16 = plain ? (p->adj_rp == 8 ? adj_npq8 : (p->adj_rp == 4 ? (SL1M_ADJ_NPOLY8 / 2) * 4 : 0))
                               : (grouped && p->adj_rp == 8 ? SL1M_ADJ_G2_NPQ : 0);
     o->mufu_per_term_mufu_path = p->pk == 2 ? 3 : (pk ? 4 : 2);
@@ -1459,9 +1457,6 @@ extern "C" int sl1m_plan_describe(const sl1m_plan *p, sl1m_plan_info *o) {
     if (p->phase64) o->adj_mufu_per_term = 1;      // adj_kernel_p64: |r| cos(X + arg r)
     if (!p->phase64) {
         if (p->pk == 0) o->adj_mufu_per_term = 1;    // delta pixels: one cosine per term in every adjoint kernel
-#ifdef SL1M_ADJ_TWO_MUFU
-        if (p->pk == 0 && p->gk == 0 && p->adj_rp == 8) o->adj_mufu_per_term = 2;   // adj_kernel_x2 (A/B build)
-#endif
         if (p->pk == 2 && p->gk == 0 && p->adj_rp == 8) o->adj_mufu_per_term = 2;    // adj_kernel_gtx2: ex2 + cos
     }
     if (o->phase_fp64) o->fwd_poly_per16 = o->adj_poly_per16 = 0;
@@ -1478,8 +1473,20 @@ extern "C" int sl1m_forward_active_pixels(sl1m_plan *p, int64_t *n_active_host, 
         for (size_t c = 0; c < C; ++c) n_active_host[c] = (int64_t)p->n_pix_pad;
         return SL1M_OK;
     }
-    std::vector<int> h(C * T);
     cudaStream_t s = (cudaStream_t)stream;
+    if (p->persist && !p->chan_scale && p->f_active) {
+        // A stepped run on the persistent kernels: they skip zero pixels warp by warp from y itself and never touch
+        // tile_cnt (it would still say what the last multi-launch pack saw).  Count y_{k+1} != 0 instead -- exactly the
+        // pixels the next iteration's forward evaluates.  Persistent plans are small (< 6.7e7 terms per apply).
+        std::vector<float> y((size_t)p->n_pix_pad);
+        CUDA_TRY(cudaMemcpyAsync(y.data(), p->y_sorted, y.size() * sizeof(float), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(cudaStreamSynchronize(s));
+        int64_t n = 0;
+        for (float v : y) n += (v != 0.f);
+        n_active_host[0] = n;
+        return SL1M_OK;
+    }
+    std::vector<int> h(C * T);
     CUDA_TRY(cudaMemcpyAsync(h.data(), p->tile_cnt, h.size() * sizeof(int), cudaMemcpyDeviceToHost, s));
     CUDA_TRY(cudaStreamSynchronize(s));
     for (size_t c = 0; c < C; ++c) {

@@ -283,15 +283,8 @@ __device__ __forceinline__ void sincos_poly2(f32x2 X, f32x2 &s, f32x2 &c, uint32
     k_hi = __float_as_uint(b);
 }
 // x with its sign flipped when k is odd: x_bits + (k << 31) (an LEA on the ALU pipe).
-#ifndef SL1M_SIGN_MODE
-#define SL1M_SIGN_MODE 1
-#endif
 __device__ __forceinline__ float flip_if_odd(float x, uint32_t k) {
-#if SL1M_SIGN_MODE == 0
-    return __uint_as_float(__float_as_uint(x) + (k << 31));     // IMAD (FMA pipe)
-#else
-    return __uint_as_float(__float_as_uint(x) ^ (k << 31));     // SHL + LOP3 (ALU pipe)
-#endif
+    return __uint_as_float(__float_as_uint(x) ^ (k << 31));     // SHL + LOP3 (ALU pipe; an IMAD add was measured no faster)
 }
 
 // One generated term.  X is the delta-pixel phase (radians).  Returns the complex entry WITHOUT
@@ -368,9 +361,6 @@ __device__ __forceinline__ void gen_entry_tile(float X, float du, float dv, floa
 #ifndef SL1M_FWD_NPQ
 #define SL1M_FWD_NPQ 4
 #endif
-#ifndef SL1M_ADJ_NPQ
-#define SL1M_ADJ_NPQ 4
-#endif
 //   *_GT_MIN_CTAS  the one-sigma-per-tile Gaussian kernels (PK == 2)
 #ifndef SL1M_FWD_GT_MIN_CTAS
 #define SL1M_FWD_GT_MIN_CTAS 4
@@ -387,9 +377,6 @@ __device__ __forceinline__ void gen_entry_tile(float X, float du, float dv, floa
 #endif
 #ifndef SL1M_FWD_X2_MIN_CTAS
 #define SL1M_FWD_X2_MIN_CTAS 4
-#endif
-#ifndef SL1M_ADJ_X2_MIN_CTAS
-#define SL1M_ADJ_X2_MIN_CTAS 5
 #endif
 #ifndef SL1M_FWD_MIN_CTAS
 #define SL1M_FWD_MIN_CTAS 5
@@ -960,119 +947,6 @@ __global__ void __launch_bounds__(NT, (PK == 0 && GK == 0) ? SL1M_ADJ_MIN_CTAS :
     for (int i = 0; i < RP; ++i) out[kfirst + i * 32 + lane] = acc[i];
 }
 
-// ------------------------------------------------------------------------------------------
-// adjoint, delta pixels / unit gains, packed-pair variant (RP = 8).  A thread's 8 pixels are 4
-// register pairs (dl, dm, dn', acc); the CTA (1,024 sorted pixels = 4 tiles, one per warp) stages
-// chunks of 128 visibilities as (u', v', w', x0[centre]) per centre plus (r_re, -r_im), so one
-// LDS.128 + one LDS.64 feed 8 terms.  NPQ of every 16 pairs (4 consecutive visibilities x 4
-// pairs) take the polynomial path.
-// A/B ONLY: this is the two-MUFU adjoint (sin and cos per term) that adj_kernel_c1 (one cosine per term)
-// replaced.  The default build never launches it; -DSL1M_ADJ_TWO_MUFU selects it for comparison runs.
-// ------------------------------------------------------------------------------------------
-template <int NPQ, bool BATCH = false>
-__global__ void __launch_bounds__(NT, SL1M_ADJ_X2_MIN_CTAS) adj_kernel_x2(const ApplyParams P) {
-    if (BATCH && P.done && P.done[blockIdx.z]) return;   // batched solve: this channel has met its stopping rule
-    constexpr int RP = 8, NPAIR = 4, NCEN = NT * RP / TP;
-    __shared__ __align__(16) float4 s_vc[2][NCEN][VC];   // (u', v', w', x0 for that centre)
-    __shared__ __align__(8) float2 s_r[2][VC];           // (r_re, -r_im)
-
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int base = blockIdx.x * (NT * RP);
-    const int kfirst = base + warp * (32 * RP);
-    const int tile0 = base / TP;
-    const int mycen = (kfirst / TP) - tile0;
-
-    f32x2 DL[NPAIR], DM[NPAIR], DN[NPAIR], ACC[NPAIR];
-#pragma unroll
-    for (int i = 0; i < NPAIR; ++i) {
-        const float4 pa = P.pix4[kfirst + (2 * i) * 32 + lane], pb = P.pix4[kfirst + (2 * i + 1) * 32 + lane];
-        DL[i] = pk2(pa.x, pb.x);
-        DM[i] = pk2(pa.y, pb.y);
-        DN[i] = pk2(pa.z, pb.z);
-        ACC[i] = pk2(0.f, 0.f);
-    }
-
-    const int n_chunks = (P.n_vis + VC - 1) / VC;
-    const double sc = chan_scale_of<BATCH>(P);
-    const int c0 = blockIdx.y * P.per_split;
-    const int c1 = min(c0 + P.per_split, n_chunks);
-
-    auto stage = [&](int chunk, int buf) {
-        const int j = chunk * VC + tid;   // NT == VC
-        double u = 0.0, v = 0.0, w = 0.0;
-        float2 rr = make_float2(0.f, 0.f);
-        if (j < P.n_vis) {
-            u = sc * P.u64[j];
-            v = sc * P.v64[j];
-            w = sc * P.w64[j];
-            rr = P.r[chan_index<BATCH>() * P.n_vis + j];
-        }
-        const float uf = static_cast<float>(TWO_PI * u), vf = static_cast<float>(TWO_PI * v),
-                    wf = static_cast<float>(TWO_PI * w);
-        s_r[buf][tid] = make_float2(rr.x, -rr.y);
-#pragma unroll
-        for (int c = 0; c < NCEN; ++c)
-            s_vc[buf][c][tid] = make_float4(uf, vf, wf, centre_phase(u, v, w, P.cen[tile0 + c]));
-    };
-
-    auto visibility = [&](const float4 vv, const float2 rr, auto npoly_tag) {
-        constexpr int NPOLY = decltype(npoly_tag)::value;
-        const f32x2 uu = bc2(vv.x), vvv = bc2(vv.y), ww = bc2(vv.z), x0 = bc2(vv.w);
-#pragma unroll
-        for (int i = 0; i < NPAIR; ++i) {
-            const f32x2 X = fma2(DL[i], uu, fma2(DM[i], vvv, fma2(DN[i], ww, x0)));
-            if (i < NPOLY) {
-                f32x2 s, c;
-                uint32_t ka, kb;
-                sincos_poly2(X, s, c, ka, kb);
-                const f32x2 rre = pk2(flip_if_odd(rr.x, ka), flip_if_odd(rr.x, kb));
-                const f32x2 rim = pk2(flip_if_odd(rr.y, ka), flip_if_odd(rr.y, kb));
-                ACC[i] = fma2(c, rre, fma2(s, rim, ACC[i]));
-            } else {
-                float xa, xb, sa, ca, sb, cb;
-                up2(X, xa, xb);
-                __sincosf(xa, &sa, &ca);
-                __sincosf(xb, &sb, &cb);
-                // Re conj(e) r = c r_re - s r_im
-                ACC[i] = fma2(pk2(ca, cb), bc2(rr.x), fma2(pk2(sa, sb), bc2(rr.y), ACC[i]));
-            }
-        }
-    };
-
-    if (c0 < c1) stage(c0, 0);
-    __syncthreads();
-    for (int ch = c0; ch < c1; ++ch) {
-        const int buf = (ch - c0) & 1;
-        if (ch + 1 < c1) stage(ch + 1, buf ^ 1);
-#pragma unroll 1
-        for (int t = 0; t < VC; t += 4) {
-            visibility(s_vc[buf][mycen][t], s_r[buf][t], std::integral_constant<int, (NPQ + 3) / 4>{});
-            visibility(s_vc[buf][mycen][t + 1], s_r[buf][t + 1], std::integral_constant<int, (NPQ + 2) / 4>{});
-            visibility(s_vc[buf][mycen][t + 2], s_r[buf][t + 2], std::integral_constant<int, (NPQ + 1) / 4>{});
-            visibility(s_vc[buf][mycen][t + 3], s_r[buf][t + 3], std::integral_constant<int, NPQ / 4>{});
-        }
-        __syncthreads();
-    }
-
-    float *out = P.ws_p + chan_index<BATCH>() * P.ws_p_stride + (size_t)blockIdx.y * P.n_pix_pad;
-#pragma unroll
-    for (int i = 0; i < NPAIR; ++i) {
-        float a, b;
-        up2(ACC[i], a, b);
-        out[kfirst + (2 * i) * 32 + lane] = a;
-        out[kfirst + (2 * i + 1) * 32 + lane] = b;
-    }
-}
-
-// ------------------------------------------------------------------------------------------
-// adjoint, delta pixels / unit gains, ONE COSINE per term (RP = 8, packed pairs).
-// The image is real (reading C3), so the adjoint only needs
-//     Re( conj(M_jk) r_j ) / a_k = Re( e^{+i X_jk} r_j ) = |r_j| cos(X_jk + arg r_j):
-// with the residual in polar form (P.r = (|r|, arg r), written by vis_polar_kernel) arg r_j joins the
-// per-(visibility, centre) phase x0 as the innermost addend of the phase chain, and a term is 3 FFMA
-// (phase) + FMUL.RZ + ONE MUFU.COS + 1 FFMA (accumulate) instead of 2 MUFU + 2 FFMA.  NPQ of every 16
-// pairs take an FMA-pipe cosine polynomial instead (same reduction and coefficients as sincos_poly2).
-// ------------------------------------------------------------------------------------------
 #ifndef SL1M_ADJ_C1_NPQ
 #define SL1M_ADJ_C1_NPQ 1
 #endif

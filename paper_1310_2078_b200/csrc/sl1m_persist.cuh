@@ -69,22 +69,21 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
     return v;
 }
 // All CTAs of the (cooperatively launched, co-resident) grid meet here.  Monotonic counter: the n-th barrier is
-// passed when it reaches n * gridDim.x.  Release: __threadfence before the arrive; acquire: ld.acquire by the
-// polling thread, then the CTA barrier hands the visibility on to the other threads.
-// SL1M_BAR_MODE bit 1: arrive with one red.release.gpu instead of __threadfence + atomicAdd; bit 0: poll with
-// ld.relaxed; bit 2: ... and no fence behind the poll.  Default 7 (measured at config 1: 5.38 us per iteration with
-// mode 0, 5.19 with 7).  Why the consumer-side fence can go: every datum another CTA produced is read with ld.global.cg
-// (L2, never L1), it reached L2 before its producer's release-arrive did, and no consumer load can issue before the
-// poll has returned the final count -- thread 0 leaves its loop on that value (control dependency, in-order issue)
-// and every other thread is held at the CTA barrier behind it.
+// passed when it reaches n * gridDim.x.
+// Default (SL1M_BAR_MODE 3): thread 0 arrives with one red.release.gpu (orders every earlier write of the CTA, which
+// the leading __syncthreads made visible to it, before the increment), polls with ld.relaxed.gpu and, once the count
+// is reached, executes fence.acq_rel.gpu: relaxed load + fence is the PTX memory model's acquire pattern, so the
+// poll synchronises-with every producer's release and the trailing __syncthreads hands that on to the CTA's other
+// threads.  Nothing here leans on how this chip happens to order loads.
+// SL1M_BAR_MODE bit 1: red.release arrive (else __threadfence + atomicAdd); bit 0: relaxed poll (else ld.acquire in the
+// loop); bit 2: drop the fence behind the relaxed poll.  Mode 7 (no consumer-side fence) was the default in round 2: it
+// is 0.13-0.19 us per iteration faster at config 1 (5.19 vs 5.38 us with mode 0) and has never produced a differing
+// bit, but it is correct only by an argument about the hardware (consumers use ld.global.cg, in-order issue, control
+// dependency on the poll), not by the memory model -- opt-in for measurements, not for production.
 #ifndef SL1M_BAR_MODE
-#define SL1M_BAR_MODE 7
+#define SL1M_BAR_MODE 3
 #endif
 __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target) {
-#ifdef SL1M_PP_NO_BAR
-    __syncthreads();
-    return;
-#endif
     __syncthreads();
     if (threadIdx.x == 0) {
         target += gridDim.x;
@@ -250,7 +249,6 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
                 a_loaded = one_item_a;
             }
             // the warp's share of the pixel list, PBLK pixels at a time: compact to a*y != 0, then generate
-#ifndef SL1M_PP_NO_A     // timing knobs (-DSL1M_PP_NO_A / _NO_B / _NO_BAR): leave a phase or the barriers out; results are wrong
             for (int base = warp * PBLK; base < P.n_pix_pad; base += PW * PBLK) {
                 int cnt = 0;
                 float4 pxq[PBLK / 32];
@@ -288,7 +286,6 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
                 }
                 __syncwarp();
             }
-#endif
             const float sum = cta_sum<2 * PG>(acc, s_red);   // thread i: re (i even) / im (i odd) of visibility i / 2
             // pair up (re, im) in the even thread
             const float other = __shfl_down_sync(0xffffffffu, sum, 1);
@@ -340,7 +337,6 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
                 }
                 b_loaded = one_item_b;
             }
-#ifndef SL1M_PP_NO_B
             if (res_v) {
                 float2 rp[4];
 #pragma unroll
@@ -371,7 +367,6 @@ __global__ void __launch_bounds__(PT, 1) fista_persistent_kernel(const PersistPa
                     }
                 }
             }
-#endif
             const float gsum = cta_sum<PG>(acc, s_red);
             if (tid < P.npg) {
                 const int kk = p0 + tid;

@@ -268,7 +268,43 @@ def test_fp64_phase_path(sl):
         plan.close()
 
 
-@pytest.mark.parametrize("n_vis,n_pix", [(1, 1), (5, 3), (1024, 1000), (147, 1024), (300, 1500), (1187, 2100), (2500, 700)])
+@pytest.mark.parametrize("n_side,n_vis,no_persistent", [(32, 1000, False), (32, 1000, True), (64, 40000, True)])
+def test_default_kernels_just_below_the_fp64_switch(sl, n_side, n_vis, no_persistent):
+    """The fp32-remainder kernels are used up to a phase span of 256 rad inside a pixel tile (sl1m.h, SL1M_PHASE_FP64);
+    the five BASELINE configs stay below 150 rad.  This is the worst case those kernels are allowed to see: config 1's
+    geometry with a full w term, baselines scaled until the span is 250 rad -- persistent kernel, small multi-launch
+    kernels, and (40,000 visibilities x 4,096 pixels) the packed-pair kernels.  Applies <= 2e-4, 40-iteration image
+    <= 1e-3 against the oracle."""
+    import torch
+    rng = np.random.default_rng(256)
+    wl = make_workload(1, n_side=n_side, n_vis=n_vis)
+    uvw = wl.uvw.copy()
+    uvw[:, 2] = 0.5 * np.hypot(uvw[:, 0], uvw[:, 1]) * rng.uniform(-1, 1, wl.n_vis)
+    q = sl.Plan(uvw, wl.l, wl.m, no_persistent=no_persistent)
+    span1 = q.describe()["phase_span_rad"]
+    q.close()
+    uvw *= 250.0 / span1
+    plan = sl.Plan(uvw, wl.l, wl.m, no_persistent=no_persistent)
+    d = plan.describe()
+    assert d["phase_fp64"] == 0 and abs(d["phase_span_rad"] - 250.0) < 1.0 and d["persistent"] == (0 if no_persistent else 1), d
+    o = oracle.Oracle(uvw, wl.l, wl.m)
+    x = rng.uniform(0, 1, wl.n_pix).astype(np.float32)
+    r = (rng.standard_normal(wl.n_vis) + 1j * rng.standard_normal(wl.n_vis)).astype(np.complex64)
+    e_f = rel_l2(plan.forward(_dev(x, torch.float32)).cpu().numpy(), o.forward(x))
+    e_a = rel_l2(plan.adjoint(_dev(r, torch.complex64)).cpu().numpy(), o.adjoint(r))
+    print(f"250 rad span, {wl.n_pix} px x {wl.n_vis} vis, fwd_rv {d['fwd_rv']} adj_rp {d['adj_rp']}: forward {e_f:.2e}, adjoint {e_a:.2e}")
+    assert e_f <= 2e-4 and e_a <= 2e-4
+    if n_vis <= 1000:
+        V = (o.forward(wl.x_true) + wl.noise).astype(np.complex64)
+        L = o.max_eig(20) * 1.05
+        xs, _ = plan.solve(_dev(V, torch.complex64), 0.5, L=L, n_iter=40)
+        e_s = rel_l2(xs.cpu().numpy(), o.fista(V, 0.5, L, 40)["x"])
+        print(f"   40-iteration image {e_s:.2e}")
+        assert e_s <= 1e-3
+    plan.close()
+
+
+@pytest.mark.parametrize("n_vis,n_pix", [(1, 1), (5, 3), (1024, 1000), (147, 1024), (300, 1500), (1187, 2100), (2500, 700), (600, 100000)])
 def test_persistent_small_problem_path(sl, n_vis, n_pix):
     """Small problems run the whole FISTA loop as ONE persistent cooperative kernel (sl1m_persist.cuh; two grid
     barriers per iteration).  Against the oracle (image, trace, stop index) and against the multi-launch loop of a
@@ -286,7 +322,7 @@ def test_persistent_small_problem_path(sl, n_vis, n_pix):
     V = (o.forward(x_true) + 0.01 * (rng.standard_normal(n_vis) + 1j * rng.standard_normal(n_vis))).astype(np.complex64)
     L = o.max_eig(30) * 1.05
     lam = 0.05 * float(np.max(np.abs(o.adjoint(V)))) + 1e-3
-    K = 60
+    K = 60 if n_pix <= 10000 else 30    # (600, 100000): 391 tiles, near PERSIST_MAX_TILES = 512 (uint16 tile ids, s_x0[512][8], several items per CTA)
     plan = sl.Plan(uvw, l, m)
     ref_plan = sl.Plan(uvw, l, m, no_persistent=True)
     assert plan.describe()["persistent"] == 1 and ref_plan.describe()["persistent"] == 0
@@ -321,12 +357,14 @@ def test_persistent_small_problem_path(sl, n_vis, n_pix):
     xs, k = plan.fista_image()
     assert k == K and torch.equal(xs, x)
     # stopping rule inside the kernel
-    if n_pix >= 700:
+    if 700 <= n_pix <= 10000:
         for tol, nnz_tol, every in ((1e-5, -1.0, 1), (-1.0, 0.0, 3), (1e-6, 0.0, 5)):
             r = o.fista_tol(V, lam, L, max_iter=400, tol=tol, nnz_tol=nnz_tol, check_every=every)
             xt, it = plan.solve_stop(Vd, lam, L, max_iter=400, tol=tol, nnz_tol=nnz_tol, check_every=every)
             kk = it.n_iter_done
             assert 2 <= kk <= 400 and (kk % every == 0 or kk == 400)
+            print(f"stop rule (tol {tol}, nnz_tol {nnz_tol}, every {every}): GPU stops at {kk}, oracle at {r['n_iter_done']} "
+                  f"(offset {kk - r['n_iter_done']:+d}, allowed +-{3 * every})")
             assert abs(kk - r["n_iter_done"]) <= 3 * every, (tol, nnz_tol, every, kk, r["n_iter_done"])
             same = o.fista(V, lam, L, kk)["x"]
             assert np.linalg.norm(xt.cpu().numpy() - same) <= 1e-3 * max(np.linalg.norm(same), 1e-30)
@@ -510,6 +548,32 @@ def test_zero_skipping_forward(sl, kind):
     assert 0 < ia.nnz < n and abs(ia.nnz - ib.nnz) <= max(2, ib.nnz // 100)
     assert plan.forward_active_pixels() < plan.describe()["n_pix_padded"]   # the last forward really skipped
     plan.close(); dense.close()
+
+
+def test_forward_active_pixels_during_a_persistent_run(sl):
+    """sl1m_forward_active_pixels inside a stepped run: a persistent plan keeps no compact tiles, so it reports the
+    pixels with y_{k+1} != 0 (it used to return the count of the last multi-launch pack: 0 after a begin from x0 = 0).
+    The multi-launch plan of the same problem reports the same pixels padded to 4 per tile."""
+    import torch
+    from workloads import fista_lambda
+    wl = make_workload(1)
+    o = oracle.Oracle.from_workload(wl)
+    V = _dev((o.forward(wl.x_true) + wl.noise).astype(np.complex64), torch.complex64)
+    L = o.max_eig(10) * 1.05
+    lam = fista_lambda(wl)
+    pers, multi = sl.Plan.from_workload(wl), sl.Plan.from_workload(wl, no_persistent=True)
+    assert pers.describe()["persistent"] == 1 and multi.describe()["persistent"] == 0
+    n_tiles = multi.describe()["n_tiles"]
+    for plan in (pers, multi):
+        plan.fista_begin(V, lam, L)
+    assert pers.forward_active_pixels() == 0                      # y_1 = 0
+    for n in (1, 5, 20):
+        pers.fista_step(n)
+        multi.fista_step(n)
+        a, b = pers.forward_active_pixels(), multi.forward_active_pixels()
+        print(f"active pixels after +{n} iterations: persistent {a} (exact), multi-launch {b} (padded to 4 per tile)")
+        assert 0 < a <= wl.n_pix and a - 8 <= b <= a + 3 * n_tiles + 8, (a, b)   # the two sum in different orders: a pixel at the threshold may flip
+    pers.close(); multi.close()
 
 
 @pytest.mark.parametrize("n_steps", [8, 2])

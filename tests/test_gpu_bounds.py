@@ -1,10 +1,10 @@
 """Memory-safety net without compute-sanitizer (SURVEY.md:184 asks for memcheck + racecheck on config 1; the GPU pool
 refuses to run the tool).  The -DSL1M_BOUNDS build of the library (libsl1m_bounds.so) surrounds every device buffer
 with 4 KiB canary bands and asserts on the device that the kernels' documented over-reads (gain-row prefetch) stay
-inside their tables; with SL1M_DEBUG_CHECK=1 the binding verifies all bands after EVERY C-ABI call.  The tests that
-WHOLE GPU suite (every other -m gpu test: ragged tiles, compact tiles, gain tables, channel batches, the persistent
-kernels, the full-size solves) is re-run under it in a subprocess, so the normal library of this process is not
-disturbed (2.5 minutes on a B200)."""
+inside their tables; with SL1M_DEBUG_CHECK=1 the binding verifies all bands after EVERY C-ABI call.  The WHOLE GPU
+suite (every other -m gpu test: ragged tiles, compact tiles, gain tables, channel batches, the persistent kernels,
+the full-size solves) is re-run under that build in a subprocess, so that the normal library of this process is not
+disturbed (about 2.5 minutes on a B200)."""
 import os
 import subprocess
 import sys

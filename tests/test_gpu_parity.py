@@ -14,8 +14,14 @@ pytestmark = pytest.mark.gpu
 TOL_APPLY = 2e-4
 TOL_IMAGE = 1e-3
 # Per-element bound next to the whole-vector relative L2: no single output may be off by more than
-# 50 x TOL of the largest expected magnitude (a wrong element of small true value hides in an L2 norm).
-ELEM_FACTOR = 50.0
+# 5 x TOL of the largest expected magnitude (a wrong element of small true value hides in an L2 norm).  Largest
+# observed: 1.5e-5 of the maximum (profiles/r2_parity_numbers.txt), against the 1e-3 (apply) / 5e-3 (image) this allows.
+ELEM_FACTOR = 5.0
+
+
+# Quadtree driver: four solves in a row, each started from the level before (reading R23); set after printing what a
+# B200 run measures (profiles/r3_parity_numbers.txt).
+QT_TOL_IMAGE = 5 * TOL_IMAGE
 
 
 def max_elem_err(got, want):
@@ -98,7 +104,10 @@ def test_config1_applies_full(sl):
     print("config1", res)
 
 
-def test_config1_solver_200_iterations(sl):
+@pytest.mark.parametrize("path", ["default", "no_persistent", "phase_fp64"])
+def test_config1_solver_200_iterations(sl, path):
+    """BASELINE config 1: 200 iterations against the fp64 oracle, on each of the three solver paths a plan of this
+    size can take -- the persistent kernel (default), the multi-launch loop, and the fp64-phase kernels."""
     import torch
     wl = make_workload(1)
     o = oracle.Oracle.from_workload(wl)
@@ -106,12 +115,14 @@ def test_config1_solver_200_iterations(sl):
     L = o.max_eig(30) * 1.05
     lam = fista_lambda(wl)
     ref = o.fista(V, lam, L, wl.n_iter, want_trace=True)
-    plan = sl.Plan.from_workload(wl)
+    plan = sl.Plan.from_workload(wl, no_persistent=(path == "no_persistent"), phase_fp64=(path == "phase_fp64"))
+    d = plan.describe()
+    assert d["persistent"] == (1 if path == "default" else 0) and d["phase_fp64"] == (1 if path == "phase_fp64" else 0), d
     trace = torch.zeros(wl.n_iter * 3, dtype=torch.float64, device="cuda")
     x, info = plan.solve(_dev(V, torch.complex64), lam, L=L, n_iter=wl.n_iter, trace=trace)
     x = x.cpu().numpy()
     err = rel_l2(x, ref["x"])
-    print("solver image rel-L2", wl.name, err)
+    print("solver image rel-L2", wl.name, path, err)
     assert err <= TOL_IMAGE, err
     assert np.all(x >= 0)
     assert info.n_iter_done == wl.n_iter and abs(info.L_used - L) <= 1e-6 * L
@@ -387,6 +398,7 @@ def test_tolerance_stop_matches_oracle(sl):
         x, info = plan.solve_tol(Vd, lam, L, max_iter=600, tol=tol, check_every=every)
         k = info.n_iter_done
         assert 2 <= k <= 600 and (k % every == 0 or k == 600)
+        print(f"stop index: GPU {k}, oracle {ref['n_iter_done']} (offset {k - ref['n_iter_done']:+d}, allowed +-{3 * every})")
         assert abs(k - ref["n_iter_done"]) <= 3 * every, (tol, every, k, ref["n_iter_done"])
         same_k = o.fista(V, lam, L, k)
         assert rel_l2(x.cpu().numpy(), same_k["x"]) <= TOL_IMAGE
@@ -425,6 +437,7 @@ def test_device_side_stop_rules_match_oracle(sl):
         x, info = plan.solve_stop(Vd, lam, L, max_iter=600, tol=tol, nnz_tol=nnz_tol, check_every=every)
         k = info.n_iter_done
         assert 2 <= k <= 600 and (k % every == 0 or k == 600), (tol, nnz_tol, every, k)
+        print(f"stop index: GPU {k}, oracle {ref['n_iter_done']} (offset {k - ref['n_iter_done']:+d}, allowed +-{3 * every})")
         assert abs(k - ref["n_iter_done"]) <= 3 * every, (tol, nnz_tol, every, k, ref["n_iter_done"])
         same_k = o.fista(V, lam, L, k)
         assert rel_l2(x.cpu().numpy(), same_k["x"]) <= TOL_IMAGE
@@ -467,6 +480,7 @@ def test_stop_rule_on_the_multi_launch_paths(sl):
         ref = o.fista_tol(V, lam, L, max_iter=600, tol=tol, nnz_tol=nnz_tol, check_every=every)
         x, info = plan.solve_stop(_dev(V, torch.complex64), lam, L, max_iter=600, tol=tol, nnz_tol=nnz_tol, check_every=every)
         k = info.n_iter_done
+        print(f"stop index: GPU {k}, oracle {ref['n_iter_done']} (offset {k - ref['n_iter_done']:+d}, allowed +-{3 * every})")
         assert abs(k - ref["n_iter_done"]) <= 3 * every and (k % every == 0 or k == 600)
         assert rel_l2(x.cpu().numpy(), o.fista(V, lam, L, k)["x"]) <= TOL_IMAGE
     plan.close()
@@ -520,6 +534,7 @@ def test_solve_stop_batch_each_channel_stops_on_its_own(sl):
     assert len(set(ks)) >= 3                       # the channels really stopped at different iterations
     for c, o in enumerate(oracles):
         ref = o.fista_tol(Vs[c], lam[c], L[c], max_iter=800, tol=tol, check_every=every, x0=d_ref[c])
+        print(f"stop index: GPU {ks[c]}, oracle {ref['n_iter_done']} (offset {ks[c] - ref['n_iter_done']:+d}, allowed +-{3 * every})")
         assert abs(ks[c] - ref["n_iter_done"]) <= 3 * every, (c, ks[c], ref["n_iter_done"])
         same_k = o.fista(Vs[c], lam[c], L[c], ks[c], x0=d_ref[c])
         assert rel_l2(x[c], same_k["x"]) <= TOL_IMAGE, (c, rel_l2(x[c], same_k["x"]))
@@ -556,6 +571,47 @@ def test_fista_stepping_api_is_the_same_run(sl):
     plan.solve(Vd, lam, L=L, n_iter=1)              # a solve that returns info ends the stepped state
     with pytest.raises(sl.Sl1mError):
         plan.fista_step(1)
+    plan.close()
+
+
+@pytest.mark.parametrize("path", ["persistent_small", "persistent_general", "multi_launch"])
+def test_forward_between_fista_steps_does_not_disturb_the_run(sl, path):
+    """begin / step / forward(I_k) / adjoint / step is the same run as begin / step / step (sl1m.h, stepping API): the
+    forward borrows the pixel tiles for the caller's image and must hand back a*y_{k+1}.  On every solver path."""
+    import torch
+    if path == "persistent_small":
+        wl = make_workload(1)
+    else:
+        wl = make_workload(2, n_side=64, n_steps=4, n_src=40)
+    o = oracle.Oracle.from_workload(wl)
+    V = _measured(o, wl)
+    L = o.max_eig(20) * 1.05
+    lam = fista_lambda(wl)
+    plan = sl.Plan.from_workload(wl, no_persistent=(path == "multi_launch"))
+    assert plan.describe()["persistent"] == (0 if path == "multi_launch" else 1)
+    Vd = _dev(V, torch.complex64)
+    plan.fista_begin(Vd, lam, L)
+    plan.fista_step(12)
+    x12 = plan.fista_image()[0].clone()
+    plan.fista_begin(Vd, lam, L)
+    plan.fista_step(5)
+    x5 = plan.fista_image()[0].clone()
+    v5 = plan.forward(x5)                                  # model visibilities of I_5, as an interactive caller would
+    assert rel_l2(v5.cpu().numpy(), o.forward(x5.cpu().numpy().astype(np.float64))) <= TOL_APPLY
+    plan.adjoint(v5 - Vd)
+    plan.forward(torch.rand_like(x5))                      # and of something unrelated to the run
+    plan.fista_step(7)
+    xs, k = plan.fista_image()
+    assert k == 12 and torch.equal(xs, x12), rel_l2(xs.cpu().numpy(), x12.cpu().numpy())
+    e = rel_l2(xs.cpu().numpy(), o.fista(V, lam, L, 12)["x"])
+    print(f"forward between steps [{path}]: image after 5 + 7 iterations vs the oracle's 12: {e:.2e}")
+    assert e <= TOL_IMAGE
+    # no solve variant leaves a steppable state behind, with or without info (its vis is not borrowed past the call)
+    plan.solve(Vd, lam, L=L, n_iter=2, want_info=False)
+    with pytest.raises(sl.Sl1mError, match="no FISTA state"):
+        plan.fista_step(1)
+    with pytest.raises(sl.Sl1mError, match="no FISTA state"):
+        plan.fista_image()
     plan.close()
 
 
@@ -634,7 +690,11 @@ def test_quadtree_driver_matches_oracle(sl):
     top = max(kr.values())
     assert all(k in kg for k, v in kr.items() if v > 0.05 * top)
     xg, xr = np.array([kg[k] for k in common]), np.array([kr[k] for k in common])
-    assert rel_l2(xg, xr) <= 5 * TOL_IMAGE, rel_l2(xg, xr)
+    print("quadtree (unit gains): image rel-L2 on common leaves %.2e, leaf sets differ in %d of %d, per-level |dL|/L %s, "
+          "per-level n_pix GPU %s oracle %s" % (rel_l2(xg, xr), len(set(kg) ^ set(kr)), len(kr),
+          ["%.1e" % (abs(a["L"] - b["L"]) / b["L"]) for a, b in zip(got["levels"], ref["levels"])],
+          [a["n_pix"] for a in got["levels"]], [b["n_pix"] for b in ref["levels"]]))
+    assert rel_l2(xg, xr) <= QT_TOL_IMAGE, rel_l2(xg, xr)
     # and it found the sky: every true source sits in a finest-level leaf with its flux
     for s in src:
         k = (int(round(lf[s] / (df / 4))), int(round(mf[s] / (df / 4))), 4)
@@ -680,7 +740,11 @@ def test_quadtree_driver_with_gains_matches_oracle(sl):
     top = max(kr.values())
     assert all(k in kg for k, v in kr.items() if v > 0.05 * top)
     xg, xr = np.array([kg[k] for k in common]), np.array([kr[k] for k in common])
-    assert rel_l2(xg, xr) <= 5 * TOL_IMAGE, rel_l2(xg, xr)
+    print("quadtree (gains): image rel-L2 on common leaves %.2e, leaf sets differ in %d of %d, per-level |dL|/L %s, "
+          "per-level n_pix GPU %s oracle %s" % (rel_l2(xg, xr), len(set(kg) ^ set(kr)), len(kr),
+          ["%.1e" % (abs(a["L"] - b["L"]) / b["L"]) for a, b in zip(got["levels"], ref["levels"])],
+          [a["n_pix"] for a in got["levels"]], [b["n_pix"] for b in ref["levels"]]))
+    assert rel_l2(xg, xr) <= QT_TOL_IMAGE, rel_l2(xg, xr)
     for s in src:                                   # the sources are recovered through the gains
         k = (int(round(lf[s] / q4)), int(round(mf[s] / q4)), 4)
         assert k in kg and abs(kg[k] - x_true[s]) < 0.08 * x_true[s]
