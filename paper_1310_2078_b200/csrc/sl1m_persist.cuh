@@ -70,18 +70,19 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
 }
 // All CTAs of the (cooperatively launched, co-resident) grid meet here.  Monotonic counter: the n-th barrier is
 // passed when it reaches n * gridDim.x.
-// Default (SL1M_BAR_MODE 3): thread 0 arrives with one red.release.gpu (orders every earlier write of the CTA, which
-// the leading __syncthreads made visible to it, before the increment), polls with ld.relaxed.gpu and, once the count
-// is reached, executes fence.acq_rel.gpu: relaxed load + fence is the PTX memory model's acquire pattern, so the
-// poll synchronises-with every producer's release and the trailing __syncthreads hands that on to the CTA's other
-// threads.  Nothing here leans on how this chip happens to order loads.
-// SL1M_BAR_MODE bit 1: red.release arrive (else __threadfence + atomicAdd); bit 0: relaxed poll (else ld.acquire in the
-// loop); bit 2: drop the fence behind the relaxed poll.  Mode 7 (no consumer-side fence) was the default in round 2: it
-// is 0.13-0.19 us per iteration faster at config 1 (5.19 vs 5.38 us with mode 0) and has never produced a differing
-// bit, but it is correct only by an argument about the hardware (consumers use ld.global.cg, in-order issue, control
-// dependency on the poll), not by the memory model -- opt-in for measurements, not for production.
+// Default (SL1M_BAR_MODE 2): thread 0 arrives with one red.release.gpu (orders every earlier write of the CTA, which
+// the leading __syncthreads made visible to it, before the increment) and polls with ld.acquire.gpu: the poll that
+// reads the final count synchronises-with every producer's release (release/acquire pattern of the PTX memory
+// model), and the trailing __syncthreads hands that on to the CTA's other threads.  Nothing here leans on how this
+// chip happens to order loads.
+// SL1M_BAR_MODE bit 1: red.release arrive (else __threadfence + atomicAdd); bit 0: ld.relaxed poll followed by
+// fence.acq_rel.gpu (also covered by the model); bit 2: ... without that fence.  Measured at config 1, 2,000-iteration
+// solve (profiles/r3_microbench.md): mode 2 4.72 us per iteration, mode 3 5.44, mode 7 4.63.  Mode 7 (no
+// consumer-side acquire at all) was the default in round 2; it has never produced a differing bit, but it is correct
+// only by an argument about the hardware (consumers use ld.global.cg, in-order issue, control dependency on the
+// poll), not by the memory model -- it buys 0.09 us and stays an opt-in for measurements.
 #ifndef SL1M_BAR_MODE
-#define SL1M_BAR_MODE 3
+#define SL1M_BAR_MODE 2
 #endif
 __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target) {
     __syncthreads();

@@ -19,9 +19,12 @@ TOL_IMAGE = 1e-3
 ELEM_FACTOR = 5.0
 
 
-# Quadtree driver: four solves in a row, each started from the level before (reading R23); set after printing what a
-# B200 run measures (profiles/r3_parity_numbers.txt).
-QT_TOL_IMAGE = 5 * TOL_IMAGE
+# Quadtree driver: four solves in a row, each started from the level before (reading R23).  A B200 run measures image
+# rel-L2 2.9e-7 / 2.5e-7 on the leaves, identical leaf sets (0 of 271 / 268 differ) and per-level |dL|/L <= 2.7e-7
+# (profiles/r3_parity_numbers.txt): the bounds sit ~35 x above that, 100 x below north_star's 1e-3.
+QT_TOL_IMAGE = 1e-5
+QT_TOL_L = 1e-5
+QT_LEAF_DIFF = 3        # leaves allowed to differ (a pixel within fp32 rounding of the split threshold)
 
 
 def max_elem_err(got, want):
@@ -666,7 +669,7 @@ def test_quadtree_driver_matches_oracle(sl):
     """sl1m_quadtree_solve against oracle.quadtree_solve (reading R23) with a fixed
     iteration count per level (tol = 0), so both sides walk the same path.  The split decision
     I_k > frac max I is taken on the fp32 image on the GPU side and on the fp64 image in the oracle: a
-    leaf within rounding of the threshold may differ, so the leaf sets are compared up to 2 %, and every
+    leaf within rounding of the threshold may differ, so the leaf sets may differ in up to QT_LEAF_DIFF leaves, and every
     leaf that matters (flux above 5 % of the maximum) must be common; fluxes are compared on common leaves."""
     uvw, V, l0, m0, side0, df, lf, mf, src, x_true = _toy_quadtree_problem()
     lam = 0.02 * float(np.abs(oracle.Oracle(uvw, l0, m0).adjoint(V)).max())
@@ -676,9 +679,9 @@ def test_quadtree_driver_matches_oracle(sl):
     got = sl.quadtree_solve(uvw, V, l0, m0, side0, **kw)
     assert len(got["levels"]) == len(ref["levels"]) == 4
     for a, b in zip(got["levels"], ref["levels"]):
-        assert abs(a["n_pix"] - b["n_pix"]) <= 0.02 * b["n_pix"] + 3
+        assert abs(a["n_pix"] - b["n_pix"]) <= QT_LEAF_DIFF
         assert a["n_iter_done"] == b["n_iter_done"] == 150
-        assert abs(a["L"] - b["L"]) <= 1e-3 * b["L"]
+        assert abs(a["L"] - b["L"]) <= QT_TOL_L * b["L"]
 
     def keyed(r):
         q = df / 4
@@ -686,7 +689,7 @@ def test_quadtree_driver_matches_oracle(sl):
                 for a, b, c, x in zip(r["l"], r["m"], r["side"], r["x"])}
     kg, kr = keyed(got), keyed(ref)
     common = sorted(set(kg) & set(kr))
-    assert len(set(kg) ^ set(kr)) <= 0.02 * len(kr) + 3
+    assert len(set(kg) ^ set(kr)) <= QT_LEAF_DIFF
     top = max(kr.values())
     assert all(k in kg for k, v in kr.items() if v > 0.05 * top)
     xg, xr = np.array([kg[k] for k in common]), np.array([kr[k] for k in common])
@@ -730,13 +733,13 @@ def test_quadtree_driver_with_gains_matches_oracle(sl):
     got = sl.quadtree_solve(uvw, V, l0, m0, side0, **kw)
     assert len(got["levels"]) == len(ref["levels"]) == 4
     for a, b in zip(got["levels"], ref["levels"]):
-        assert abs(a["n_pix"] - b["n_pix"]) <= 0.02 * b["n_pix"] + 3
-        assert abs(a["L"] - b["L"]) <= 1e-3 * b["L"]
+        assert abs(a["n_pix"] - b["n_pix"]) <= QT_LEAF_DIFF
+        assert abs(a["L"] - b["L"]) <= QT_TOL_L * b["L"]
     q4 = df / 4
     kg = {(int(round(a / q4)), int(round(b / q4)), int(round(c / q4))): float(x) for a, b, c, x in zip(got["l"], got["m"], got["side"], got["x"])}
     kr = {(int(round(a / q4)), int(round(b / q4)), int(round(c / q4))): float(x) for a, b, c, x in zip(ref["l"], ref["m"], ref["side"], ref["x"])}
     common = sorted(set(kg) & set(kr))
-    assert len(set(kg) ^ set(kr)) <= 0.02 * len(kr) + 3
+    assert len(set(kg) ^ set(kr)) <= QT_LEAF_DIFF
     top = max(kr.values())
     assert all(k in kg for k, v in kr.items() if v > 0.05 * top)
     xg, xr = np.array([kg[k] for k in common]), np.array([kr[k] for k in common])
