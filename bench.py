@@ -342,8 +342,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     y = torch.rand(wl.n_pix, dtype=torch.float32, device=dev, generator=torch.Generator(device=dev).manual_seed(7)) + 0.5
     vis_out = torch.empty(wl.n_vis, dtype=torch.complex64, device=dev)
     img_out = torch.empty(wl.n_pix, dtype=torch.float32, device=dev)
-    reps = max(3, min(args.steps, 5))
-    plan.forward(y, out=vis_out); plan.adjoint(V, out=img_out)
+    reps = 10                                   # median of >= 10 timed applies after 3 warm-ups
+    for _ in range(3):
+        plan.forward(y, out=vis_out); plan.adjoint(V, out=img_out)
     t_fwd = time_call(lambda: plan.forward(y, out=vis_out), reps)
     t_adj = time_call(lambda: plan.adjoint(V, out=img_out), reps)
 
@@ -427,6 +428,37 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     clk_meas = pk_meas["sm_clock_mhz"] * 1e6
     plain = not (desc["gaussian"] or desc["gains"])
 
+    def fixed_ceiling(kind, m_term):
+        """The fixed ceiling of a plan TYPE (it does not move with any tuning knob): the best the instruction set of
+        the method allows when the share f of terms whose sin/cos (forward: 2 MUFU, adjoint: 1) is evaluated by the
+        FMA-pipe polynomial is free in [0, 1].  ex2 / rcp of Gaussian pixels stay on the MUFU pipe (moving them was
+        measured slower).  Lane-ops per term are the SASS counts of DESIGN.md section 6 (the same constants as
+        bound()); gains add their amortised product, the fp64-phase kernels add 4 FP64-pipe ops per term (3 DFMA + the
+        magic-number DADD) against the DFMA rate measured in this run.  Returns (terms/s, binding pipe, f)."""
+        gauss, gains_k = int(desc["gaussian"]), int(desc["gains"])
+        movable = 1.0 if kind == "adj" else 2.0                 # MUFU per term that a polynomial can replace
+        movable = min(movable, float(m_term))
+        if kind == "adj":
+            a_ = {0: 5.0, 1: 19.0, 2: 12.0}[gauss]
+            b_ = a_ + 7.0                                       # cos polynomial instead of MUFU.COS: + 3 reduce + 4 Horner
+            extra = {0: 0.0, 1: 10.0, 2: 1.5}[gains_k]
+        else:
+            a_ = {0: 6.0, 1: 20.0, 2: 13.0}[gauss]
+            b_ = a_ + 12.0                                      # sincos polynomial: + 3 reduce + 5 sin + 4 cos
+            extra = {0: 0.0, 1: 10.0, 2: 0.5}[gains_k]
+        R_f64 = pk_meas.get("dfma_per_s") or SM_COUNT * 64.0 * clk_meas
+        best, pipe, f_at = 0.0, "", 0.0
+        for i in range(0, 257):
+            f = i / 256.0
+            mufu = m_term - movable * f
+            t = {"mufu": mufu / R_mufu if mufu > 0 else 0.0, "fma": (a_ * (1.0 - f) + b_ * f + extra) / R_fma}
+            if desc["phase_fp64"]:
+                t["fp64"] = 4.0 / R_f64
+            worst = max(t, key=t.get)
+            if 1.0 / t[worst] > best:
+                best, pipe, f_at = 1.0 / t[worst], worst, f
+        return best, pipe, f_at
+
     def kernel_entry(kind, ms, per16, packed, name):
         """Roofline of one apply kernel on a DENSE image (every N_p x N_v term evaluated).
         own_mix: min(MUFU pipe, FMA pipe, issue slots) for the kernel's SASS instruction mix, with the measured
@@ -441,19 +473,21 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         own = min(b_mufu * scale_m, b_fma * scale_f, b_issue)
         m_term = desc["adj_mufu_per_term"] if kind == "adj" else desc["mufu_per_term_mufu_path"]
         mufu_only = R_mufu / m_term
-        best = None
-        if plain and not desc["phase_fp64"]:
-            m_, a_, b_ = (1.0, 5.0, 12.0) if (kind == "adj" and m_term == 1) else (2.0, 6.0, 18.0)
-            d = m_ / R_mufu - a_ / R_fma
-            f_bal = max(0.0, d / (d + b_ / R_fma))
-            best = R_mufu / (m_ * (1.0 - f_bal))
+        best, best_pipe, best_f = fixed_ceiling(kind, m_term)
         e = {"kernel": name, "ms": ms, "Tterm_per_s": ach / 1e12, "poly_per16": per16,
              "own_mix_bound": own / 1e12, "frac_vs_own_mix": ach / own,
              "mufu_only_bound": mufu_only / 1e12, "frac_vs_mufu_only": ach / mufu_only,
-             "best_split_bound": None if best is None else best / 1e12,
-             "frac_vs_best_split": None if best is None else ach / best,
+             "best_split_bound": best / 1e12, "frac_vs_best_split": ach / best,
+             "best_split_binding_pipe": best_pipe, "best_split_poly_fraction": best_f,
              "own_mix_pipes": {"mufu": b_mufu * scale_m / 1e12, "fma": b_fma * scale_f / 1e12, "issue": b_issue / 1e12}}
-        return e, ach, (best if best is not None else own)
+        if plain and not desc["phase_fp64"]:
+            # fourth denominator: what the kernel's OWN mix reaches in the co-issue micro-benchmark (MUFU beside a packed
+            # FMA stream, sl1m_peaks.cu): measured MUFU results/s under co-issue / MUFU per term at the kernel's split
+            co = pk_meas["coissue_adj_mufu_per_clk_sm" if (kind == "adj" and m_term == 1) else "coissue_mufu_per_clk_sm"]
+            co_bound = co * SM_COUNT * clk_meas / (m_term * (1.0 - per16 / 16.0))
+            e["coissue_bound"] = co_bound / 1e12
+            e["frac_vs_coissue"] = ach / co_bound
+        return e, ach, best
 
     def kname(kind):
         nm = "sl1m::adj_kernel" if kind == "adj" else "sl1m::fwd_kernel"
@@ -479,10 +513,12 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     roof = {
         "bound": "alu", "kernel": dom_e["kernel"], "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "Tterm/s",
         "frac": achieved / peak, "traffic": traffic,
-        "peak_basis": ("best MUFU/FMA split bound of the kernel's instruction set (fixed ceiling)" if dom_e["best_split_bound"]
-                       else "own-mix issue bound (Gaussian / gain kernels: no polynomial-split ceiling defined)") +
-                      ", from the MUFU and FFMA2 rates measured in this run by sl1m_measure_peaks (peak_measured); "
-                      "kernels.fwd / kernels.adj carry all three denominators for both apply kernels",
+        "peak_basis": "fixed ceiling of the plan type: the best split of sin/cos between the MUFU pipe and an FMA-pipe "
+                      "polynomial that the kernel's instruction set allows (ex2/rcp of Gaussian pixels stay on MUFU; gains add "
+                      "their amortised product; fp64-phase kernels add 4 FP64-pipe ops per term), binding pipe "
+                      f"'{dom_e['best_split_binding_pipe']}', from the MUFU, FFMA2 and DFMA rates measured in this run by "
+                      "sl1m_measure_peaks (peak_measured); kernels.fwd / kernels.adj carry every denominator (own mix, MUFU "
+                      "only, fixed ceiling, co-issue micro-benchmark) for both apply kernels",
         "peak_measured": pk_meas,
         "kernels": {"fwd": ent_f, "adj": ent_a},
         "traffic_basis": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full "

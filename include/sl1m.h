@@ -22,10 +22,13 @@
  *    void* (NULL = the legacy default stream).
  *  - The plan COPIES every plan-time input; the caller may free them on return.  Vectors passed
  *    to forward/adjoint/solve stay caller-owned; outputs are overwritten, never accumulated.
- *  - forward/adjoint are asynchronous on `stream`.  solve and max_eig enqueue all their work on
- *    `stream` without any host round-trip per iteration and synchronise once at the end, only
- *    when a host result (info / L) was asked for.  The *_host variants copy in and out of HOST
- *    buffers on `stream` and synchronise before returning.
+ *  - forward/adjoint are asynchronous on `stream`.  solve, fista_begin and max_eig copy their scalars
+ *    (lambda, L, the momentum table of a persistent plan) to the device from buffers of their own and
+ *    therefore synchronise `stream` ONCE, at the start of the call; the iterations are then enqueued
+ *    without any host round-trip per iteration (the device-side stopping rules are polled behind the
+ *    enqueue front, sl1m_solve_stop), and the call synchronises again at the end only when a host
+ *    result (info / L) was asked for.  fista_step never waits.  The *_host variants copy in and out of
+ *    HOST buffers on `stream` and synchronise before returning.
  *  - A plan owns its workspaces: do not use one plan from two streams at once.
  *  - Images are real fp32 [n_pix] in the CALLER's pixel order; visibilities are complex fp32,
  *    interleaved (re, im), [n_vis][2], in the caller's order.
@@ -378,6 +381,7 @@ typedef struct {
     double coissue_ffma2_lanes_per_clk_sm;   /* ... and the FFMA2 lanes per clock per SM achieved beside them       */
     double coissue_cycles_per_iter;      /* sub-partition cycles per warp per body (profiles/r1_microbench.md: 35.3) */
     double coissue_adj_mufu_per_clk_sm;  /* 4 MUFU.COS + 8 FFMA2 + 4 FMUL.RZ per body (the one-cosine adjoint's mix) */
+    double dfma_per_s, dfma_per_clk_sm;  /* DFMA alone on the FP64 pipe (the fp64-phase kernels: 4 FP64 ops per term)  */
 } sl1m_peaks;
 int sl1m_measure_peaks(sl1m_peaks *out_host, void *stream);
 

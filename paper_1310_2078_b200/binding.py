@@ -39,7 +39,7 @@ class _Peaks(ctypes.Structure):
     _fields_ = [("n_sm", ctypes.c_int32)] + [(n, ctypes.c_double) for n in (
         "sm_clock_mhz", "clock64_mhz", "mufu_per_s", "mufu_per_clk_sm", "mufu_cos_per_clk_sm", "ffma_per_s", "ffma_per_clk_sm",
         "ffma2_lanes_per_s", "ffma2_lanes_per_clk_sm", "coissue_mufu_per_clk_sm", "coissue_ffma2_lanes_per_clk_sm",
-        "coissue_cycles_per_iter", "coissue_adj_mufu_per_clk_sm")]
+        "coissue_cycles_per_iter", "coissue_adj_mufu_per_clk_sm", "dfma_per_s", "dfma_per_clk_sm")]
 
 
 class _QtLevel(ctypes.Structure):

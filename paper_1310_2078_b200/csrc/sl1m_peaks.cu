@@ -89,6 +89,25 @@ __global__ void __launch_bounds__(128) probe_kernel(int iters, float seed, float
     if (threadIdx.x == 0) cycles[blockIdx.x] = c1 - c0;
 }
 
+// FP64 pipe: 8 independent DFMA chains per thread, 8 deep per iteration (the fp64-phase kernels spend 3 DFMA + 1 DADD
+// per term on it).
+__global__ void __launch_bounds__(128) dfma_probe_kernel(int iters, double seed, float *sink) {
+    double d[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) d[i] = seed + 1e-6 * (double)threadIdx.x + (double)i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(d[i]) : "d"(0.999), "d"(1e-3));
+        }
+    }
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc += d[i];
+    if (acc == 123.456) sink[0] = (float)acc;                 // never true: keeps the chains alive
+}
+
 struct Timed {
     double ms;        // best of the repetitions, CUDA events on the launching stream
     double cyc;       // median-free: mean SM cycles of a CTA's loop (clock64)
@@ -178,6 +197,28 @@ extern "C" int sl1m_measure_peaks(sl1m_peaks *o, void *stream) {
     // the one-cosine adjoint's mix per pair of terms: 3 FFMA2 + 2 FMUL.RZ + 2 MUFU.COS + 1 FFMA2 -> x2: 8 FFMA2 + 4 RZ + 4 MUFU
     if (PROBE(4, 0, 8, 4, true)) o->coissue_adj_mufu_per_clk_sm = per_clk_sm(4.0 * per_it, t);
 #undef PROBE
+    if (e == cudaSuccess) {   // DFMA alone: best of 3 after a warm-up, CUDA events on the launching stream
+        cudaEvent_t e0, e1;
+        const int d_iters = 512;
+        if (cudaEventCreate(&e0) == cudaSuccess && cudaEventCreate(&e1) == cudaSuccess) {
+            double best = 1e30;
+            for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {
+                cudaEventRecord(e0, s);
+                dfma_probe_kernel<<<grid, 128, 0, s>>>(d_iters, 0.5, sink);
+                cudaEventRecord(e1, s);
+                e = cudaEventSynchronize(e1);
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, e0, e1);
+                if (rep > 0) best = std::min(best, (double)ms);
+            }
+            if (e == cudaSuccess) {
+                o->dfma_per_s = 64.0 * d_iters * thr / (best * 1e-3);
+                o->dfma_per_clk_sm = o->dfma_per_s / ((double)sms * clk_hz);
+            }
+            cudaEventDestroy(e0);
+            cudaEventDestroy(e1);
+        }
+    }
     cudaFree(sink);
     cudaFree(cyc);
     o->n_sm = sms;

@@ -382,6 +382,8 @@ def test_measure_peaks_is_sane(sl):
     assert 112.0 <= pk["ffma_per_clk_sm"] <= 128.5, pk
     assert 112.0 <= pk["ffma2_lanes_per_clk_sm"] <= 128.5, pk
     assert pk["coissue_mufu_per_clk_sm"] <= pk["mufu_per_clk_sm"] * 1.01
+    assert 48.0 <= pk["dfma_per_clk_sm"] <= 65.0, pk            # FP64 pipe: 64 DFMA per clock per SM nominal on B200
+    print("measured peaks per clock per SM:", {k: round(v, 2) for k, v in pk.items() if k.endswith("per_clk_sm")})
     assert abs(pk["mufu_per_s"] / (148 * pk["sm_clock_mhz"] * 1e6) - pk["mufu_per_clk_sm"]) < 1e-6 * pk["mufu_per_clk_sm"] + 1e-9
 
 
